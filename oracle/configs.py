@@ -1,0 +1,95 @@
+"""CPU ORACLE — test infrastructure only.
+
+The five workloads of BASELINE.json:configs evaluated primitive by primitive with the
+unfused oracle (one full loop and one materialised temporary per operation, in the
+order and parenthesisation fixed in DESIGN.md §3 / SURVEY.md §8(c)).
+"""
+from __future__ import annotations
+
+import numpy as np
+
+import oracle as orc
+
+
+def dot_product(a, b) -> float:
+    """Listing 4: a.compwise_multiply(b).sum."""
+    return orc.sum(orc.zip("mul", a, b))
+
+
+def axpy(alpha, x, y) -> np.ndarray:
+    """aX+Y: X.multiplied_by(a).plus(Y)."""
+    return orc.zip("add", orc.scalar("mul", x, alpha), y)
+
+
+def cfg0_chain(a, b, c) -> np.ndarray:
+    """z = (a+b)*2.5 - c  (BASELINE.json:configs[0])."""
+    t1 = orc.zip("add", a, b)
+    t2 = orc.scalar("mul", t1, 2.5)
+    return orc.zip("sub", t2, c)
+
+
+def cfg0(a, b, c) -> dict:
+    z = cfg0_chain(a, b, c)
+    return {
+        "z": z,
+        "sum": orc.sum(z),
+        "max": orc.max(z),
+        "min": orc.min(z),
+        "pre": orc.any(orc.cmp_scalar("gt", a, 0.99)),                   # exists(a_i > 0.99)
+        "post": orc.all(orc.cmp("eq", z, cfg0_chain(a, b, c))),          # for_all(z_i == recomputed)
+    }
+
+
+def cfg1_chain(x, y) -> np.ndarray:
+    """w = abs(x*y + 0.5) - min(x,y)*3 + x/(1+y*y), left to right  (BASELINE.json:configs[1])."""
+    t1 = orc.zip("mul", x, y)
+    t2 = orc.scalar("add", t1, 0.5)
+    t3 = orc.unary("abs", t2)
+    t4 = orc.zip("min", x, y)
+    t5 = orc.scalar("mul", t4, 3.0)
+    t6 = orc.zip("sub", t3, t5)
+    t7 = orc.zip("mul", y, y)
+    t8 = orc.scalar("add", t7, 1.0, reversed=True)
+    t9 = orc.zip("div", x, t8)
+    return orc.zip("add", t6, t9)
+
+
+def cfg1(x, y) -> dict:
+    w = cfg1_chain(x, y)
+    return {"w": w, "sum": orc.sum(w), "max": orc.max(w)}
+
+
+def cfg2(x, modulus: int = 7, residue: int = 3) -> dict:
+    """stable filter keeping x where x mod 7 == 3, count, int64 sum of kept (BASELINE.json:configs[2])."""
+    m = orc.cmp_scalar("eq", orc.scalar("mod", x, modulus), residue)
+    kept = orc.filter(x, m)
+    return {"kept": kept, "count": int(kept.size), "count_mask": orc.count(m), "sum": orc.sum(kept)}
+
+
+def cfg3(x) -> dict:
+    """pre = for_all(x_i >= 0), post = is-sorted for_all(x_i <= x_{i+1})  (BASELINE.json:configs[3])."""
+    return {"pre": orc.all(orc.cmp_scalar("ge", x, 0.0)), "post": orc.all(orc.adj("le", x))}
+
+
+def cfg4_unfused(M, k: int) -> dict:
+    """Row-update step for all j>k, primitive by primitive (BASELINE.json:configs[4])."""
+    M = np.array(M, dtype=np.float64, order="C", copy=True)
+    n_rows = M.shape[0]
+    col = orc.mat_col(M, k)                                  # column(k): copy
+    f = orc.scalar("div", col[k + 1:], M[k, k])              # f_j = M[j,k] / M[k,k]
+    t = orc.outer_mul(f, M[k, :])                            # t = f_j * M[k,c]
+    sub = orc.zip("sub", M[k + 1:, :], t)                    # M[j,c] - t
+    M[k + 1:, :] = sub
+    if n_rows - k - 1 > 0:
+        rowmax = orc.row_max(orc.unary("abs", sub))
+        colsum = orc.col_sum(sub)
+    else:
+        rowmax = np.empty(0)
+        colsum = np.zeros(M.shape[1])
+    return {"M": M, "rowmax": rowmax, "colsum": colsum}
+
+
+def cfg4(M, k: int) -> dict:
+    """Same step through the single plain-definition loop (orc_mat_step)."""
+    Mo, rowmax, colsum = orc.mat_step(M, k)
+    return {"M": Mo, "rowmax": rowmax, "colsum": colsum}
