@@ -1,0 +1,328 @@
+"""bench.py — the headline metric of BASELINE.json: fused-chain throughput (elements/s, GB/s, fraction of the HBM
+roofline) for the config-1 chain  w = abs(x*y+0.5) - min(x,y)*3 + x/(1+y*y); sum(w), max(w)  on fp32 vectors.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--log2n 28] [--impl ours|reference] [--headline-only]
+
+A step = one pass of the whole hot path through the C ABI: enqueue the ten pending operations and the two
+reductions (a1), plan build at the trigger (a2), the fused map+reduce launch (a3, a4) and the scalar hand-back (a8).
+`value` is measured with the inputs resident in HBM; `e2e` repeats the same step with HOST (pinned) inputs whose
+host->device copies are inside the timed region.  The other §8(a) rows (quantifier contracts a5, filter a6,
+matrix step a7, unfused lowering a9) are timed in the same run and reported under "per_config".
+
+N > 1 (torchrun): every rank runs the same workload on its own GPU (independent problems, no data-path
+collective: weak scaling); the time is the max over ranks.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "fused_chain_elements_per_s"
+UNIT = "elements/s"
+
+
+def peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        try:
+            return float(json.load(open(path))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region."""
+
+    def __init__(self, index: int):
+        self.index, self.samples, self.proc = index, [], None
+
+    def start(self):
+        q = "clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown," \
+            "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={q}", "--format=csv,noheader,nounits", "-lms", "100", "-i", str(self.index)],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            threading.Thread(target=self._read, daemon=True).start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.samples.append(line.strip())
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for s in self.samples:
+            f = [x.strip() for x in s.split(",")]
+            if len(f) < 6:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1]))
+            except ValueError:
+                continue
+            for name, v in zip(names, f[2:6]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None, "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+def oracle_chain_rate(x, y, seconds_target=8.0):
+    """The CPU oracle as it stands, on a bounded sample of the same workload; returns (elements/s, sample size, sum, max)."""
+    from oracle import configs as ocfg
+    m = min(x.size, 1 << 22)
+    t0 = time.perf_counter()
+    ocfg.cfg1(x[:m], y[:m])
+    dt = time.perf_counter() - t0
+    m2 = int(min(x.size, max(m, (seconds_target / max(dt, 1e-6)) * m)))
+    m2 = min(m2, 1 << 26)
+    t0 = time.perf_counter()
+    r = ocfg.cfg1(x[:m2], y[:m2])
+    dt = time.perf_counter() - t0
+    return m2 / dt, m2, r["sum"], float(r["max"])
+
+
+def run_reference(args):
+    """--impl reference: the oracle (plain single-threaded C++, unfused) timed on the host cores."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from paper_1410_6685_b200 import inputs
+    from oracle import configs as ocfg
+    m = 1 << 23                                    # bounded sample of the 2^log2n workload per step
+    x, y = inputs.normal_f32(2, 0, m), inputs.normal_f32(2, 1, m)
+    for _ in range(args.warmup):
+        ocfg.cfg1(x, y)
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        ocfg.cfg1(x, y)
+    dt = time.perf_counter() - t0
+    v = m * args.steps / dt
+    line = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+            "data": "synthetic", "config": {"workload": f"cfg1 chain fp32, oracle on a bounded sample of 2^23 elements per step (of n=2^{args.log2n})"},
+            "cpu_baseline": {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": "first 2^23 elements of the seeded x,y per step"},
+            "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line))
+
+
+def time_replay(sg, ctx, reps):
+    return sg.sg_replay_last(ctx, reps)
+
+
+def per_config(torch, sg, W, inputs, peak, quick):
+    """Device time per flush (library CUDA events, mean of replays) for the other §8(a) rows; inputs > L2 except cfg0."""
+    out = {}
+    stream = torch.cuda.current_stream().cuda_stream
+
+    def measure(name, build, alg_bytes, reps=20, flags=0, restore=None):
+        ctx = sg.sg_ctx_create(0, stream)
+        sg.sg_ctx_set_flags(ctx, flags)
+        try:
+            build(ctx)
+            sg.sg_flush(ctx)
+            st = sg.sg_plan_stats(ctx)
+            if restore is None:
+                sg.sg_replay_last(ctx, 3)
+                ms = sg.sg_replay_last(ctx, reps)
+            else:
+                times = []
+                for _ in range(min(reps, 5)):
+                    restore()
+                    times.append(sg.sg_replay_last(ctx, 1))
+                ms = float(np.mean(times))
+            b = alg_bytes if alg_bytes else st.bytes_min
+            out[name] = {"ms": ms, "algorithmic_bytes": int(b), "GB/s": b / ms / 1e6, "frac_of_peak": b / ms / 1e6 / peak, "passes": st.n_passes,
+                         "template_passes": st.n_template}
+        finally:
+            sg.sg_ctx_destroy(ctx)
+
+    # config 0 (fits in L2: a warm number, labelled)
+    n0 = 1 << 20
+    a, b, c = (torch.from_numpy(inputs.uniform_pm1_f64(1, s, n0)).cuda() for s in range(3))
+    measure("cfg0_fp64_2^20_chain_sum_max_min_contracts (L2-warm, 2 passes)", lambda ctx: W.cfg0(ctx, n0, a.data_ptr(), b.data_ptr(), c.data_ptr()), 64 << 20, 200)
+    measure("cfg0_onepass (z released, L2-warm)", lambda ctx: W.cfg0(ctx, n0, a.data_ptr(), b.data_ptr(), c.data_ptr(), keep_z=False), 24 << 20, 200)
+    del a, b, c
+    # config 1 at its own size, fused and one-kernel-per-op
+    n1 = 1 << 26
+    x = torch.from_numpy(inputs.normal_f32(2, 0, n1)).cuda()
+    y = torch.from_numpy(inputs.normal_f32(2, 1, n1)).cuda()
+    measure("cfg1_fp32_2^26_fused", lambda ctx: W.cfg1(ctx, n1, x.data_ptr(), y.data_ptr()), 8 * n1)
+    measure("cfg1_fp32_2^26_unfused_one_kernel_per_op", lambda ctx: W.cfg1(ctx, n1, x.data_ptr(), y.data_ptr()), 0, 5, sg.SG_FLAG_UNFUSED)
+    measure("cfg1_fp32_2^26_fused_bytecode", lambda ctx: W.cfg1(ctx, n1, x.data_ptr(), y.data_ptr()), 8 * n1, 5, sg.SG_FLAG_FORCE_BYTECODE)
+    del x, y
+    if quick:
+        return out
+    # config 2
+    n2 = 1 << 27
+    xi = torch.from_numpy(inputs.uniform_i31(3, 0, n2)).cuda()
+    cnt = int((xi % 7 == 3).sum().item())          # only to size the algorithmic bytes of the report
+    measure("cfg2_int32_2^27_filter_count_sum", lambda ctx: W.cfg2(ctx, n2, xi.data_ptr()), 4 * n2 + 4 * cnt)
+    del xi
+    # config 3, clean and with the seeded violation (early exit)
+    n3 = 1 << 28
+    xs_host = inputs.sorted_cumsum_f32(4, 0, n3)
+    xs = torch.from_numpy(xs_host).cuda()
+    measure("cfg3_fp32_2^28_forall_ge0_and_sorted_clean", lambda ctx: W.cfg3(ctx, n3, xs.data_ptr()), 4 * n3)
+    j = inputs.violation_index(4, n3)
+    xs[j] = 0.5 * xs[j - 1]
+    measure(f"cfg3_fp32_2^28_violation_at_{j} (early exit; time to answer)", lambda ctx: W.cfg3(ctx, n3, xs.data_ptr()), 4 * n3)
+    del xs, xs_host
+    # config 4
+    n4 = 16384
+    Mh = inputs.boosted_matrix_f64(5, 0, n4)
+    M0 = torch.from_numpy(Mh).cuda()
+    M = M0.clone()
+    del Mh
+    for k in (0, 8191):
+        rows = n4 - k - 1
+        alg = 16 * rows * n4 + 8 * n4 + 16 * rows + 8 * rows + 8 * n4
+        measure(f"cfg4_fp64_16384^2_row_update_k={k}", lambda ctx: W.cfg4(ctx, n4, M.data_ptr(), k), alg, restore=lambda: M.copy_(M0))
+    return out
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--log2n", type=int, default=28)
+    ap.add_argument("--impl", default="ours")
+    ap.add_argument("--headline-only", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3)
+    if args.impl == "reference":
+        run_reference(args)
+        return
+
+    import torch
+    from paper_1410_6685_b200 import inputs, sg
+    from paper_1410_6685_b200 import workloads as W
+
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if not torch.cuda.is_available():
+        raise RuntimeError("bench.py needs a CUDA device: the library has no CPU fallback")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    peak, peak_src = peaks()
+
+    n = 1 << args.log2n
+    xh = torch.from_numpy(inputs.normal_f32(2, 2 * rank, n)).pin_memory()
+    yh = torch.from_numpy(inputs.normal_f32(2, 2 * rank + 1, n)).pin_memory()
+    x, y = xh.cuda(), yh.cuda()
+    stream = torch.cuda.current_stream().cuda_stream
+    ctx = sg.sg_ctx_create(local, stream)
+
+    def step():
+        r = W.cfg1(ctx, n, x.data_ptr(), y.data_ptr())
+        s, m = sg.sg_scalar_get(ctx, r["sum"]), sg.sg_scalar_get(ctx, r["max"])
+        for h in r.values():
+            sg.sg_release(ctx, h)
+        return s, m
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        s0, m0 = step()
+    launches0 = sg.sg_plan_stats(ctx).launches_total
+    sampler = ClockSampler(local)
+    if rank == 0:
+        sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    kernel_ms = []
+    barrier()
+    e0.record()
+    for _ in range(args.steps):
+        step()
+        kernel_ms.append(sg.sg_last_flush_ms(ctx))     # events inside the library on the launch stream (already synchronised by the scalar read)
+    e1.record()
+    barrier()
+    total_ms = e0.elapsed_time(e1)
+    clocks = sampler.stop() if rank == 0 else None
+    launches = sg.sg_plan_stats(ctx).launches_total - launches0
+    st = sg.sg_plan_stats(ctx)
+
+    # end to end: host buffers in, scalars out, copies inside the timed region
+    barrier()
+    e2, e3 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e2e_steps = max(3, min(args.steps, 5))
+    e2.record()
+    for _ in range(e2e_steps):
+        x.copy_(xh, non_blocking=True)
+        y.copy_(yh, non_blocking=True)
+        step()
+    e3.record()
+    barrier()
+    e2e_ms = e2.elapsed_time(e3)
+
+    if dist is not None:
+        t = torch.tensor([total_ms, e2e_ms], device="cuda", dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms, e2e_ms = t.tolist()
+    if rank != 0:
+        sg.sg_ctx_destroy(ctx)
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    ms_step = total_ms / args.steps
+    k_ms = float(np.mean(kernel_ms))
+    alg_bytes = 8 * n
+    achieved = alg_bytes / k_ms / 1e6
+    cpu_rate, cpu_m, cpu_sum, cpu_max = oracle_chain_rate(xh.numpy(), yh.numpy())
+    line = {
+        "metric": METRIC, "value": world * n / (ms_step * 1e-3), "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": f"cfg1 fused 10-op chain + sum + max on fp32 x,y of 2^{args.log2n} elements (BASELINE.json metric: fused chain at 2^28)",
+                   "n": n, "seed": 2, "l2": "inputs (2 x 4n bytes) larger than L2; no flush needed", "plan_passes": st.n_passes,
+                   "template_passes": st.n_template, "step": "enqueue + plan + fused launch + scalar hand-back through the C ABI"},
+        "GB/s": world * alg_bytes / ms_step / 1e6,
+        "frac_of_8TBps": alg_bytes / ms_step / 1e6 / 8000.0,
+        "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": None,
+                     "kernel": sg.sg_template_name(st.pass_kernel[0]) if st.pass_kernel[0] else "bytecode", "kernel_ms": k_ms,
+                     "algorithmic_bytes_per_launch": alg_bytes, "peak_source": peak_src, "frac_of_8TBps": achieved / 8000.0},
+        "cpu_baseline": {"value": cpu_rate, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": f"first {cpu_m} elements of the same x,y, one timed run"},
+        "e2e": {"value": world * n / (e2e_ms / e2e_steps * 1e-3), "unit": UNIT, "h2d_bytes_per_step": 8 * n, "d2h_bytes_per_step": 16,
+                "steps": e2e_steps, "ms_per_step": e2e_ms / e2e_steps},
+        "gpu_launches": int(launches),
+        "clocks": clocks,
+        "result": {"sum": s0, "max": m0},
+    }
+    sg.sg_ctx_destroy(ctx)
+    del x, y
+    if world == 1:
+        try:
+            line["per_config"] = per_config(torch, sg, W, inputs, peak, args.headline_only)
+        except Exception as e:      # the headline stands on its own; say what failed
+            line["per_config_error"] = repr(e)
+    if dist is not None:
+        dist.destroy_process_group()
+    print(json.dumps(line))
+
+
+if __name__ == "__main__":
+    main()

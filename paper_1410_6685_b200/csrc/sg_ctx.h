@@ -1,0 +1,128 @@
+// sg_ctx.h — host runtime data structures (internal): context, handle table, pending-action list, plan.
+// PAPER.md:284 "a method call is not executed, but rather added to a list of pending actions"
+// "the optimizer constructs an execution plan from the pending operations ... a DAG, representing data and
+// kernels as two different types of nodes".  Here: Value = data node, Node = kernel node, Pass = merged kernel.
+#ifndef SG_CTX_H_
+#define SG_CTX_H_
+
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <string>
+#include <vector>
+
+#include "../../include/sg.h"
+#include "sg_kernels.h"
+#include "sg_prog.h"
+
+enum ValueKind { VK_VEC = 0, VK_MAT = 1, VK_SCALAR = 2 };
+enum NodeKind { NK_MAP = 0, NK_REDUCE = 1, NK_FILTER = 2 };
+enum OperandKind { OPD_VALUE = 0, OPD_IMM = 1, OPD_SHIFT = 2 /* value shifted by +1 element */ };
+
+struct Value {
+    int kind = VK_VEC;
+    int dtype = SG_F32;
+    int64_t rows = 1, cols = 0;     // vector: rows = 1, cols = n
+    int64_t ld = 0;                 // matrix: leading dimension in elements
+    int64_t stride = 1;             // vector: element stride (ld for a column view)
+    char* ptr = nullptr;            // element 0 when materialised
+    bool materialised = false;
+    bool owned = false;             // ptr allocated by the context
+    int node = -1;                  // producing pending node, -1 if none
+    int user_refs = 0;
+    int64_t count_slot = -1;        // filter output: scalar slot holding the kept count; cols is the capacity until resolved
+    bool count_known = true;
+    int64_t slot = -1;              // VK_SCALAR produced by a reduction: slot in the scalar slab
+    bool alive = true;
+};
+
+struct Operand {
+    int kind = OPD_VALUE;
+    int value = -1;
+    int bcast = SG_BCAST_NONE;
+    uint64_t imm = 0;               // raw bits, already converted to the node's operand dtype
+};
+
+struct Node {
+    int kind = NK_MAP;
+    uint8_t op = 0;                 // NK_MAP: OP_*; NK_REDUCE: OUT_SUM..OUT_COUNT
+    int n_opd = 0;
+    Operand opd[2];
+    int out = -1;                   // result value
+    int out2 = -1;                  // NK_FILTER: the count scalar
+    int axis = AXIS_ALL;
+    int dtype = SG_F32;             // operand dtype (V file) — SG_BOOL for pure logic nodes
+    bool is2d = false;
+    int64_t rows = 1, cols = 0;     // iteration domain
+    bool inplace = false;           // out's storage was given by the caller (dst_or_0)
+    // plan state
+    bool needed = false, post = false, done = false;
+    int pass = -1;
+};
+
+struct Contract { int value; int kind; std::string tag; };
+
+struct MemRange { const char* lo; const char* hi; const char* ptr; int64_t stride, ld, rows, cols; };
+
+struct PassInput { uint8_t kind; const char* ptr; int64_t stride; uint64_t imm; int reg; int value; bool boolvec; int64_t len; };
+
+struct Pass {
+    bool is2d = false, has_filter = false, has_store = false;
+    int dtype = -1;                 // V-file dtype, -1 = not fixed yet (only BOOL nodes so far)
+    int64_t rows = 1, cols = 0;     // domain (1-D: cols = max length)
+    std::vector<int> nodes;
+    std::vector<MemRange> reads, writes;
+    // built program
+    SgProg prog;
+    SgArgs args;
+    SgGeom geom;
+    int n_mem_in = 0, n_scalar_in = 0;
+    int64_t bytes = 0;
+};
+
+struct Launch { SgProg prog; SgArgs args; SgGeom geom; };
+
+struct sg_ctx {
+    int device = -1;
+    bool plan_only = true;
+    cudaStream_t stream = nullptr;
+    sg_alloc alloc{};
+    bool has_alloc = false;
+    uint32_t flags = 0;
+    int sm_count = 148;
+    std::string err;
+
+    std::vector<Value> values;      // handle h <-> values[h-1]
+    std::vector<Node> nodes;        // pending actions, in call order
+    std::vector<Contract> contracts;
+
+    // device resources
+    char* workspace = nullptr; size_t workspace_bytes = 0;
+    unsigned long long* tile_state = nullptr; size_t tile_state_words = 0;
+    unsigned int* ctrl = nullptr; int ctrl_words = 0;
+    uint32_t epoch = 0;
+    char* slab = nullptr;           // device scalar slots, 8 bytes each
+    char* slab_host = nullptr;      // pinned mirror
+    int64_t slab_slots = 0, slab_next = 0;
+    std::vector<int64_t> slab_free;
+    cudaEvent_t ev_done = nullptr, ev_t0 = nullptr, ev_t1 = nullptr;
+    bool mirror_pending = false;
+    uintptr_t fake_next = 0x10000000;   // plan-only contexts: distinct fake addresses
+
+    // last flush
+    std::vector<Launch> last;
+    sg_stats stats{};
+    std::vector<std::string> dumps;
+    std::vector<char*> deferred_free;
+};
+
+// sg_plan.cpp
+sg_status sg_flush_impl(sg_ctx* c);
+// helpers shared by sg_api.cpp / sg_plan.cpp
+inline int dtype_size(int dt) { return dt == SG_BOOL ? 1 : (dt == SG_F32 || dt == SG_I32) ? 4 : 8; }
+sg_status sg_fail(sg_ctx* c, sg_status code, const std::string& msg);
+void* sg_dev_alloc(sg_ctx* c, size_t bytes);
+void sg_dev_free(sg_ctx* c, void* p);
+int64_t sg_slot_alloc(sg_ctx* c);
+
+#endif  // SG_CTX_H_

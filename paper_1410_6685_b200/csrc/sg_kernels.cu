@@ -1,0 +1,214 @@
+// sg_kernels.cu — kernel instantiation, the template registry and launch geometry (sm_100a).
+#include "sg_kernels.h"
+
+#include <stdio.h>
+#include <string.h>
+
+#include <algorithm>
+
+#include "sg_filter.cuh"
+#include "sg_pass1d_tmpl.cuh"
+#include "sg_pass1d_vm.cuh"
+#include "sg_pass2d.cuh"
+
+namespace {
+
+using namespace sgk;
+
+typedef cudaError_t (*LaunchFn)(const SgArgs&, int grid, cudaStream_t);
+typedef int (*OccFn)();
+
+struct Entry {
+    const char* name;
+    const SgProg* prog;
+    LaunchFn launch;
+    OccFn occupancy;
+    int tile;       // elements per tile (1-D, filter) or strip width (2-D)
+};
+
+template <class P> constexpr int tile_of() {
+    if (P::prog.shape.flags & PF_FILTER) return BLOCK * FilterTemplateEval<P>::U * FilterTemplateEval<P>::FW;
+    return BLOCK * Meta1D<P>::E;
+}
+
+template <class P> cudaError_t launch_template(const SgArgs& a, int grid, cudaStream_t s) {
+    if constexpr ((P::prog.shape.flags & PF_2D) != 0) pass2d_template<P><<<grid, BLOCK, 0, s>>>(a);
+    else if constexpr ((P::prog.shape.flags & PF_FILTER) != 0) filter1d_template<P><<<grid, BLOCK, 0, s>>>(a);
+    else pass1d_template<P><<<grid, BLOCK, 0, s>>>(a);
+    return cudaGetLastError();
+}
+template <class P> int occupancy_template() {
+    int occ = 0;
+    cudaError_t e;
+    if constexpr ((P::prog.shape.flags & PF_2D) != 0) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, pass2d_template<P>, BLOCK, 0);
+    else if constexpr ((P::prog.shape.flags & PF_FILTER) != 0) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, filter1d_template<P>, BLOCK, 0);
+    else e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, pass1d_template<P>, BLOCK, 0);
+    return (e == cudaSuccess && occ > 0) ? occ : 1;
+}
+
+// Each SG_TEMPLATE(name, unroll, min_blocks, row_unroll, {program}) in the generated file defines a policy type
+// and registers it.  The program initialisers are written by paper_1410_6685_b200/gen_templates.py from the plan
+// builder's own canonical output, so a registered chain always matches its signature.
+#define SG_TEMPLATE(NAME, UNROLL, MINB, ROWU, ...)                                   \
+    struct T_##NAME {                                                                \
+        static constexpr SgProg prog = __VA_ARGS__;                                  \
+        static constexpr int unroll = UNROLL, min_blocks = MINB, row_unroll = ROWU;  \
+    };
+#include "sg_templates_gen.inc"
+#undef SG_TEMPLATE
+
+#define SG_TEMPLATE(NAME, UNROLL, MINB, ROWU, ...) \
+    {#NAME, &T_##NAME::prog, &launch_template<T_##NAME>, &occupancy_template<T_##NAME>, tile_of<T_##NAME>()},
+const Entry g_entries[] = {
+    {"bytecode", nullptr, nullptr, nullptr, 0},
+#include "sg_templates_gen.inc"
+};
+#undef SG_TEMPLATE
+const int g_n_entries = (int)(sizeof(g_entries) / sizeof(g_entries[0]));
+
+template <class T> cudaError_t launch_bytecode_t(const SgProg& g, const SgArgs& a, int grid, cudaStream_t s) {
+    if (g.shape.flags & PF_FILTER) filter1d_bytecode<T><<<grid, BLOCK, 0, s>>>(g, a);
+    else pass1d_bytecode<T><<<grid, BLOCK, 0, s>>>(g, a);
+    return cudaGetLastError();
+}
+template <class T> int occupancy_bytecode_t(bool filter) {
+    int occ = 0;
+    cudaError_t e = filter ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, filter1d_bytecode<T>, BLOCK, 0)
+                           : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, pass1d_bytecode<T>, BLOCK, 0);
+    return (e == cudaSuccess && occ > 0) ? occ : 1;
+}
+int occupancy_bytecode(int dtype, bool filter) {
+    switch (dtype) {
+        case DT_F32: return occupancy_bytecode_t<float>(filter);
+        case DT_F64: return occupancy_bytecode_t<double>(filter);
+        case DT_I32: return occupancy_bytecode_t<int32_t>(filter);
+        default: return occupancy_bytecode_t<long long>(filter);
+    }
+}
+
+int elem_size(int dtype) { return (dtype == DT_F32 || dtype == DT_I32) ? 4 : 8; }
+
+int fail(char* err, size_t cap, int code, const char* msg) {
+    if (err && cap) snprintf(err, cap, "%s", msg);
+    return code;
+}
+
+}  // namespace
+
+int sgk_template_count() { return g_n_entries - 1; }
+const char* sgk_template_name(int id) { return (id >= 1 && id < g_n_entries) ? g_entries[id].name : "bytecode"; }
+const SgProg* sgk_template_prog(int id) { return (id >= 1 && id < g_n_entries) ? g_entries[id].prog : nullptr; }
+int sgk_find_template(const SgProg& prog) {
+    for (int i = 1; i < g_n_entries; ++i)
+        if (memcmp(g_entries[i].prog, &prog, sizeof(SgProg)) == 0) return i;
+    return 0;
+}
+
+int sgk_plan(const SgProg& prog, SgArgs& a, int force_bytecode, int sm_count, int has_device, SgGeom* geom, char* err, size_t errcap) {
+    const int es = elem_size(prog.shape.dtype);
+    const int V = 16 / es;
+    const bool is2d = prog.shape.flags & PF_2D, isfilter = prog.shape.flags & PF_FILTER;
+    memset(geom, 0, sizeof(*geom));
+    int tid = force_bytecode ? 0 : sgk_find_template(prog);
+    if (tid == 0 && !is2d && prog.shape.n_vreg > VM_VREG)
+        return fail(err, errcap, -9, "fused chain needs more value registers than the bytecode evaluator has; flush earlier");
+
+    // alignment of every vector-accessed operand relative to the pass origin
+    long mis = -1;          // common misalignment in elements, -1 = not yet fixed
+    bool congruent = true;
+    int vec_ok = 0;
+    auto misalign = [&](const void* p) { return (long)(((uintptr_t)p % 16) / es); };
+    auto consider = [&](const void* p, int bit) {
+        if (((uintptr_t)p % es) != 0) { congruent = false; return; }
+        long m = misalign(p);
+        if (mis < 0) mis = m;
+        if (m == mis) vec_ok |= 1 << bit; else congruent = false;
+    };
+    for (int o = 0; o < prog.shape.n_out; ++o)
+        if (prog.out[o].kind == OUT_STORE) consider(a.out_ptr[o], 16 + o);
+    for (int k = 0; k < prog.shape.n_in; ++k)
+        if (prog.in[k].kind == IN_VEC || (is2d && prog.in[k].kind == IN_ROWB)) consider(a.in_ptr[k], k);
+    if (mis < 0) mis = 0;
+
+    if (is2d) {
+        if (tid == 0 && has_device) return fail(err, errcap, -10, "matrix pass has no precompiled template instance (2-D bytecode evaluator not built)");
+        bool ok = congruent && mis == 0 && (a.cols % V) == 0;
+        for (int k = 0; k < prog.shape.n_in; ++k)
+            if (prog.in[k].kind == IN_VEC && (a.in_stride[k] % V) != 0) ok = false;
+        for (int o = 0; o < prog.shape.n_out; ++o)
+            if (prog.out[o].kind == OUT_STORE && (a.out_len[o] % V) != 0) ok = false;
+        if (!ok) return fail(err, errcap, -10, "matrix pass needs 16-byte aligned rows (base, leading dimension and column count)");
+        const int occ = (has_device && tid) ? g_entries[tid].occupancy() : 2;
+        const int SW = tid ? g_entries[tid].tile : BLOCK * 2 * V;
+        a.n_strips = (int)((a.cols + SW - 1) / SW);
+        const long target = (long)sm_count * occ;
+        long max_chunks = std::max<long>(1, (a.n + RB - 1) / RB);
+        long n_chunks = std::min<long>(max_chunks, std::max<long>(1, target / std::max(1, a.n_strips)));
+        long rpc = (a.n + n_chunks - 1) / n_chunks;
+        rpc = std::max<long>(RB, (rpc + RB - 1) / RB * RB);
+        n_chunks = std::max<long>(1, (a.n + rpc - 1) / rpc);
+        a.rows_per_chunk = rpc;
+        a.n_chunks = (int)n_chunks;
+        geom->template_id = tid;
+        geom->grid = (int)(a.n_strips * n_chunks);
+        geom->tile = SW;
+        size_t off = (size_t)geom->grid * SG_MAX_OUT * sizeof(Cell);
+        for (int o = 0; o < prog.shape.n_out; ++o) {
+            a.ws_off[o] = 0;
+            if (!out_is_reduction(prog.out[o].kind)) continue;
+            if (prog.out[o].axis == AXIS_COLS) { a.ws_off[o] = (int64_t)off; off += (size_t)n_chunks * a.cols * sizeof(Cell); }
+            if (prog.out[o].axis == AXIS_ROWS) { a.ws_off[o] = (int64_t)off; off += (size_t)a.n_strips * a.n * sizeof(Cell); }
+        }
+        geom->ws_bytes = off;
+        geom->ctrl_words = a.n_strips + (int)n_chunks;
+        a.vec_ok = vec_ok;
+        a.head = 0; a.n_full_tiles = 0;
+        return 0;
+    }
+
+    if (isfilter) {
+        const int tile = tid ? g_entries[tid].tile : BLOCK * 4 * (16 / es);
+        const int occ = has_device ? (tid ? g_entries[tid].occupancy() : occupancy_bytecode(prog.shape.dtype, true)) : 4;
+        const long n_tiles = (a.n + tile - 1) / tile;
+        if (a.n >= (1ll << 40) || n_tiles > 0x7fffffffl) return fail(err, errcap, -9, "filter input too long for the tile-state word");
+        a.n_tiles = (int)n_tiles;
+        a.vec_ok = vec_ok | ((congruent && mis == 0) ? (1 << 31) : 0);
+        a.head = 0; a.n_full_tiles = 0;
+        geom->template_id = tid;
+        geom->tile = tile;
+        geom->grid = (int)std::max<long>(1, std::min<long>(n_tiles, (long)sm_count * occ));
+        geom->ws_bytes = (size_t)geom->grid * SG_MAX_OUT * sizeof(Cell);
+        geom->state_words = (size_t)n_tiles;
+        return 0;
+    }
+
+    // 1-D pass.  Template instances need every vector operand congruent (common head); otherwise the bytecode
+    // kernel runs with per-operand 128-bit eligibility.
+    if (tid && !congruent) tid = 0;
+    const int tile = tid ? g_entries[tid].tile : vm_tile(es);
+    long lmin = a.n;
+    for (int o = 0; o < prog.shape.n_out; ++o) lmin = std::min<long>(lmin, a.out_len[o]);
+    const long head = std::min<long>((V - mis) % V, a.n);
+    const long body = std::max<long>(0, lmin - head);
+    a.head = head;
+    a.n_full_tiles = body / tile;
+    a.vec_ok = vec_ok;
+    const int occ = has_device ? (tid ? g_entries[tid].occupancy() : occupancy_bytecode(prog.shape.dtype, false)) : 4;
+    long want = tid ? a.n_full_tiles : ((a.n - head + tile - 1) / tile + (head + tile - 1) / tile);
+    geom->template_id = tid;
+    geom->tile = tile;
+    geom->grid = (int)std::max<long>(1, std::min<long>(want, (long)sm_count * occ));
+    geom->ws_bytes = (size_t)geom->grid * SG_MAX_OUT * sizeof(Cell);
+    return 0;
+}
+
+cudaError_t sgk_launch(const SgProg& prog, const SgArgs& args, const SgGeom& geom, cudaStream_t stream) {
+    if (geom.template_id > 0) return g_entries[geom.template_id].launch(args, geom.grid, stream);
+    switch (prog.shape.dtype) {
+        case DT_F32: return launch_bytecode_t<float>(prog, args, geom.grid, stream);
+        case DT_F64: return launch_bytecode_t<double>(prog, args, geom.grid, stream);
+        case DT_I32: return launch_bytecode_t<int32_t>(prog, args, geom.grid, stream);
+        case DT_I64: return launch_bytecode_t<long long>(prog, args, geom.grid, stream);
+        default: return cudaErrorInvalidValue;
+    }
+}

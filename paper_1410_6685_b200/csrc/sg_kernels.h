@@ -1,0 +1,32 @@
+// sg_kernels.h — host-side interface between the plan builder (sg_runtime.cpp) and the kernels (sg_kernels.cu).
+#ifndef SG_KERNELS_H_
+#define SG_KERNELS_H_
+
+#include <cuda_runtime.h>
+#include <stddef.h>
+
+#include "sg_prog.h"
+
+struct SgGeom {
+    int template_id;        // 0 = bytecode kernel, k > 0 = template instance k
+    int grid;               // blocks
+    int tile;               // elements per tile of the chosen kernel (1-D / filter), strip width (2-D)
+    size_t ws_bytes;        // workspace bytes this launch needs (partial cells)
+    size_t state_words;     // filter: tile-state words needed
+    int ctrl_words;         // control words needed beyond the first 8 (2-D tickets)
+};
+
+// Registry of precompiled template instances (sg_templates_gen.inc).
+int sgk_template_count();
+const char* sgk_template_name(int id);              // 1-based
+const SgProg* sgk_template_prog(int id);
+int sgk_find_template(const SgProg& prog);          // 0 if none
+
+// Chooses the kernel (template instance unless force_bytecode / misaligned operands) and fills the geometry
+// fields of `args` (head, n_full_tiles, vec_ok, strips/chunks, ws_off).  sm_count/has_device: plan-only contexts
+// pass has_device = 0 and nothing touches CUDA.  Returns 0 or an sg_status error (message in err).
+int sgk_plan(const SgProg& prog, SgArgs& args, int force_bytecode, int sm_count, int has_device, SgGeom* geom, char* err, size_t errcap);
+
+cudaError_t sgk_launch(const SgProg& prog, const SgArgs& args, const SgGeom& geom, cudaStream_t stream);
+
+#endif  // SG_KERNELS_H_

@@ -1,0 +1,248 @@
+// sg_pass1d_tmpl.cuh — pass1d_template<P>: the fused 1-D pass with the program as a compile-time constant.
+// "Each method is associated with a kernel template, which the library instantiates"; here the
+// template is instantiated ahead of time over a whole merged chain instead of per method.
+#ifndef SG_PASS1D_TMPL_CUH_
+#define SG_PASS1D_TMPL_CUH_
+
+#include "sg_pass1d.cuh"
+
+namespace sgk {
+
+template <class P> struct Meta1D {
+    static constexpr SgShape S = P::prog.shape;
+    typedef typename TypeOf<S.dtype>::type T;
+    typedef typename Traits<T>::vec VEC;
+    static constexpr int V = Traits<T>::V;
+    static constexpr int U = P::unroll;                 // 128-bit loads per input per thread per tile
+    static constexpr int E = U * V;                     // elements per thread per tile
+    static constexpr int TILE = BLOCK * E;
+    static constexpr int NV = S.n_vreg > 0 ? S.n_vreg : 1;
+    static constexpr int NP = S.n_preg > 0 ? S.n_preg : 1;
+    static constexpr int NOUT = S.n_out > 0 ? S.n_out : 1;
+    static constexpr bool early_exit = (S.flags & PF_EARLY_EXIT) != 0;
+};
+
+// ---- compile-time body: one fold over the instruction list, every register index is a constant --------
+template <class P, class T, int NV, int NP, int E, int I>
+__device__ __forceinline__ void exec_instr(T (&v)[NV][E], bool (&p)[NP][E]) {
+    constexpr SgInstr ins = P::prog.code[I];
+#pragma unroll
+    for (int e = 0; e < E; ++e) {
+        if constexpr (op_is_value(ins.op)) v[ins.dst][e] = value_op<T>(ins.op, v[ins.a][e], v[ins.b][e]);
+        else if constexpr (op_is_compare(ins.op)) p[ins.dst][e] = compare_op<T>(ins.op, v[ins.a][e], v[ins.b][e]);
+        else p[ins.dst][e] = logic_op(ins.op, p[ins.a][e], p[ins.b][e]);
+    }
+}
+template <class P, class T, int NV, int NP, int E, int... I>
+__device__ __forceinline__ void exec_body(T (&v)[NV][E], bool (&p)[NP][E], std::integer_sequence<int, I...>) {
+    (exec_instr<P, T, NV, NP, E, I>(v, p), ...);
+}
+
+// ---- inputs of one full tile ---------------------------------------------------------------------------
+template <class P, int K>
+__device__ __forceinline__ void load_input_full(typename Meta1D<P>::T (&v)[Meta1D<P>::NV][Meta1D<P>::E],
+                                                bool (&p)[Meta1D<P>::NP][Meta1D<P>::E], const SgArgs& a, int64_t base) {
+    typedef Meta1D<P> M;
+    typedef typename M::T T;
+    typedef typename M::VEC VEC;
+    constexpr SgIn in = P::prog.in[K];
+    if constexpr (in.kind == IN_VEC) {
+        const VEC* src = reinterpret_cast<const VEC*>(reinterpret_cast<const T*>(a.in_ptr[K]) + base);
+#pragma unroll
+        for (int u = 0; u < M::U; ++u) {
+            VEC x = in.pad ? ld_stream_rw(src + u * BLOCK + threadIdx.x) : ld_stream(src + u * BLOCK + threadIdx.x);
+            const T* xe = reinterpret_cast<const T*>(&x);
+#pragma unroll
+            for (int e = 0; e < M::V; ++e) v[in.reg][u * M::V + e] = xe[e];
+        }
+    } else if constexpr (in.kind == IN_SHIFT) {
+        // x[i+1]: own vector shifted by one, last element from the next lane, lane 31 reads one scalar
+        constexpr int rr = P::prog.in[in.ref].reg;
+        const T* src = reinterpret_cast<const T*>(a.in_ptr[in.ref]) + base;
+#pragma unroll
+        for (int u = 0; u < M::U; ++u) {
+#pragma unroll
+            for (int e = 0; e + 1 < M::V; ++e) v[in.reg][u * M::V + e] = v[rr][u * M::V + e + 1];
+            T nxt = __shfl_down_sync(0xffffffffu, v[rr][u * M::V], 1);
+            if ((threadIdx.x & 31) == 31) nxt = __ldg(src + (size_t)(u * BLOCK + threadIdx.x + 1) * M::V);
+            v[in.reg][u * M::V + M::V - 1] = nxt;
+        }
+    } else if constexpr (in.kind == IN_STRIDED) {
+        const T* src = reinterpret_cast<const T*>(a.in_ptr[K]);
+#pragma unroll
+        for (int u = 0; u < M::U; ++u)
+#pragma unroll
+            for (int e = 0; e < M::V; ++e)
+                v[in.reg][u * M::V + e] = __ldg(src + (base + (int64_t)(u * BLOCK + threadIdx.x) * M::V + e) * a.in_stride[K]);
+    } else if constexpr (in.kind == IN_BOOLVEC) {
+        const uint8_t* src = reinterpret_cast<const uint8_t*>(a.in_ptr[K]) + base;
+#pragma unroll
+        for (int u = 0; u < M::U; ++u)
+#pragma unroll
+            for (int e = 0; e < M::V; ++e) p[in.reg][u * M::V + e] = src[(size_t)(u * BLOCK + threadIdx.x) * M::V + e] != 0;
+    }
+    // IN_SCALAR / IN_IMM are broadcast once before the tile loop
+}
+template <class P, int... K>
+__device__ __forceinline__ void load_inputs_full(typename Meta1D<P>::T (&v)[Meta1D<P>::NV][Meta1D<P>::E],
+                                                 bool (&p)[Meta1D<P>::NP][Meta1D<P>::E], const SgArgs& a, int64_t base,
+                                                 std::integer_sequence<int, K...>) {
+    (load_input_full<P, K>(v, p, a, base), ...);
+}
+
+template <class P, int E, int K>
+__device__ __forceinline__ void bcast_input(typename Meta1D<P>::T (&v)[Meta1D<P>::NV][E], const SgArgs& a) {
+    typedef typename Meta1D<P>::T T;
+    constexpr SgIn in = P::prog.in[K];
+    if constexpr (in.kind == IN_SCALAR || in.kind == IN_IMM) {
+        T s = load_elem<T>(in.kind, in.ref, K, a, 0);
+#pragma unroll
+        for (int e = 0; e < E; ++e) v[in.reg][e] = s;
+    }
+}
+template <class P, int E, int... K>
+__device__ __forceinline__ void bcast_inputs(typename Meta1D<P>::T (&v)[Meta1D<P>::NV][E], const SgArgs& a, std::integer_sequence<int, K...>) {
+    (bcast_input<P, E, K>(v, a), ...);
+}
+
+// ---- outputs of one full tile --------------------------------------------------------------------------
+template <class P, int O>
+__device__ __forceinline__ void emit_output_full(typename Meta1D<P>::T (&v)[Meta1D<P>::NV][Meta1D<P>::E],
+                                                 bool (&p)[Meta1D<P>::NP][Meta1D<P>::E], Cell (&acc)[Meta1D<P>::NOUT],
+                                                 const SgArgs& a, int64_t base) {
+    typedef Meta1D<P> M;
+    typedef typename M::T T;
+    typedef typename M::VEC VEC;
+    constexpr SgOut out = P::prog.out[O];
+    if constexpr (out.kind == OUT_STORE) {
+        VEC* dst = reinterpret_cast<VEC*>(reinterpret_cast<T*>(a.out_ptr[O]) + base);
+#pragma unroll
+        for (int u = 0; u < M::U; ++u) {
+            VEC x;
+            T* xe = reinterpret_cast<T*>(&x);
+#pragma unroll
+            for (int e = 0; e < M::V; ++e) xe[e] = v[out.src][u * M::V + e];
+            st_stream(dst + u * BLOCK + threadIdx.x, x);
+        }
+    } else if constexpr (out.kind == OUT_STORE_BOOL) {
+        uint8_t* dst = reinterpret_cast<uint8_t*>(a.out_ptr[O]) + base;
+#pragma unroll
+        for (int u = 0; u < M::U; ++u)
+#pragma unroll
+            for (int e = 0; e < M::V; ++e) dst[(size_t)(u * BLOCK + threadIdx.x) * M::V + e] = p[out.src][u * M::V + e];
+    } else if constexpr (out_is_pred_reduction(out.kind)) {
+#pragma unroll
+        for (int e = 0; e < M::E; ++e) cell_accum_pred(out.kind, acc[O], p[out.src][e]);
+    } else if constexpr (out_is_reduction(out.kind)) {
+#pragma unroll
+        for (int e = 0; e < M::E; ++e) {
+            if constexpr (out.pred == SG_NO_PRED) cell_accum_value<T>(out.kind, acc[O], v[out.src][e]);
+            else if (p[out.pred][e]) cell_accum_value<T>(out.kind, acc[O], v[out.src][e]);
+        }
+    }
+}
+template <class P, int... O>
+__device__ __forceinline__ void emit_outputs_full(typename Meta1D<P>::T (&v)[Meta1D<P>::NV][Meta1D<P>::E],
+                                                  bool (&p)[Meta1D<P>::NP][Meta1D<P>::E], Cell (&acc)[Meta1D<P>::NOUT],
+                                                  const SgArgs& a, int64_t base, std::integer_sequence<int, O...>) {
+    (emit_output_full<P, O>(v, p, acc, a, base), ...);
+}
+
+// ---- one ragged element (head / tail), E = 1 -----------------------------------------------------------
+template <class P, int K>
+__device__ __forceinline__ void load_input_one(typename Meta1D<P>::T (&v)[Meta1D<P>::NV][1], bool (&p)[Meta1D<P>::NP][1],
+                                               const SgArgs& a, int64_t i) {
+    typedef typename Meta1D<P>::T T;
+    constexpr SgIn in = P::prog.in[K];
+    if constexpr (in.kind == IN_BOOLVEC) p[in.reg][0] = (i < a.in_len[K]) && reinterpret_cast<const volatile uint8_t*>(a.in_ptr[K])[i] != 0;
+    else if constexpr (in.kind != IN_SCALAR && in.kind != IN_IMM) v[in.reg][0] = load_elem<T>(in.kind, in.ref, K, a, i);
+}
+template <class P, int O>
+__device__ __forceinline__ void emit_output_one(typename Meta1D<P>::T (&v)[Meta1D<P>::NV][1], bool (&p)[Meta1D<P>::NP][1],
+                                                Cell (&acc)[Meta1D<P>::NOUT], const SgArgs& a, int64_t i) {
+    typedef typename Meta1D<P>::T T;
+    constexpr SgOut out = P::prog.out[O];
+    if (i >= a.out_len[O]) return;
+    if constexpr (out.kind == OUT_STORE) reinterpret_cast<T*>(a.out_ptr[O])[i] = v[out.src][0];
+    else if constexpr (out.kind == OUT_STORE_BOOL) reinterpret_cast<uint8_t*>(a.out_ptr[O])[i] = p[out.src][0];
+    else if constexpr (out_is_pred_reduction(out.kind)) cell_accum_pred(out.kind, acc[O], p[out.src][0]);
+    else if constexpr (out_is_reduction(out.kind)) {
+        if constexpr (out.pred == SG_NO_PRED) cell_accum_value<T>(out.kind, acc[O], v[out.src][0]);
+        else if (p[out.pred][0]) cell_accum_value<T>(out.kind, acc[O], v[out.src][0]);
+    }
+}
+template <class P, int... K, int... I, int... O>
+__device__ __forceinline__ void ragged_range(Cell (&acc)[Meta1D<P>::NOUT], const SgArgs& a, int64_t lo, int64_t hi, int64_t start,
+                                             int64_t step, std::integer_sequence<int, K...> ks, std::integer_sequence<int, I...> is,
+                                             std::integer_sequence<int, O...>) {
+    typedef Meta1D<P> M;
+    typename M::T v[M::NV][1];
+    bool p[M::NP][1];
+    bcast_inputs<P, 1>(v, a, ks);
+    for (int64_t i = lo + start; i < hi; i += step) {
+        (load_input_one<P, K>(v, p, a, i), ...);
+        exec_body<P, typename M::T, M::NV, M::NP, 1>(v, p, is);
+        (emit_output_one<P, O>(v, p, acc, a, i), ...);
+    }
+}
+
+// ---- the kernel ----------------------------------------------------------------------------------------
+template <class P>
+__global__ void __launch_bounds__(BLOCK, P::min_blocks) pass1d_template(const __grid_constant__ SgArgs a) {
+    typedef Meta1D<P> M;
+    typedef typename M::T T;
+    constexpr auto KS = std::make_integer_sequence<int, M::S.n_in>{};
+    constexpr auto IS = std::make_integer_sequence<int, M::S.n_instr>{};
+    constexpr auto OS = std::make_integer_sequence<int, M::S.n_out>{};
+
+    constexpr SgProg g = P::prog;     // local constant copy: indexable inside unrolled loops
+    Cell acc[M::NOUT];
+    uint8_t kind[M::NOUT];
+    bool has_reduction = false;
+#pragma unroll
+    for (int o = 0; o < M::NOUT; ++o) {
+        kind[o] = (o < M::S.n_out) ? g.out[o].kind : (uint8_t)OUT_STORE;
+        acc[o] = cell_identity<T>(kind[o]);
+        has_reduction |= out_is_reduction(kind[o]);
+    }
+    unsigned int need_mask = 0, flagged = 0;
+    if constexpr (M::early_exit) {
+#pragma unroll
+        for (int o = 0; o < M::S.n_out; ++o) need_mask |= 1u << o;
+    }
+
+    {
+        T v[M::NV][M::E];
+        bool p[M::NP][M::E];
+        bcast_inputs<P, M::E>(v, a, KS);
+        for (int64_t tile = blockIdx.x; tile < a.n_full_tiles; tile += gridDim.x) {
+            if constexpr (M::early_exit) {
+                if (!a.no_early_exit && ld_volatile_u32(&a.ctrl[1]) == need_mask) break;
+            }
+            const int64_t base = a.head + tile * M::TILE;
+            load_inputs_full<P>(v, p, a, base, KS);
+            exec_body<P, T, M::NV, M::NP, M::E>(v, p, IS);
+            emit_outputs_full<P>(v, p, acc, a, base, OS);
+            if constexpr (M::early_exit) {
+#pragma unroll
+                for (int o = 0; o < M::S.n_out; ++o) {
+                    bool decided = (kind[o] == OUT_ALL) ? (acc[o].a == 0) : (acc[o].a != 0);
+                    if (!(flagged & (1u << o)) && __any_sync(0xffffffffu, decided)) {
+                        flagged |= 1u << o;
+                        if ((threadIdx.x & 31) == 0) atomicOr(&a.ctrl[1], 1u << o);
+                    }
+                }
+            }
+        }
+    }
+    // ragged head [0, head) and tail [head + full tiles, n): spread over the grid's threads
+    {
+        const int64_t gtid = (int64_t)blockIdx.x * BLOCK + threadIdx.x, gstep = (int64_t)gridDim.x * BLOCK;
+        ragged_range<P>(acc, a, 0, a.head, gtid, gstep, KS, IS, OS);
+        ragged_range<P>(acc, a, a.head + a.n_full_tiles * M::TILE, a.n, gtid, gstep, KS, IS, OS);
+    }
+    epilogue_1d<T, M::NOUT>(acc, kind, a, has_reduction);
+}
+
+}  // namespace sgk
+#endif  // SG_PASS1D_TMPL_CUH_

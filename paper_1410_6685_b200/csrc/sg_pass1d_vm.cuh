@@ -1,0 +1,220 @@
+// sg_pass1d_vm.cuh — pass1d_bytecode: the register-resident op-bytecode evaluator for chains that have no
+// precompiled template instance.  The SgProg bytes are interpreted per tile; control flow is warp-uniform (every
+// thread runs the same program), each decoded instruction is applied to a register-resident vector of E elements,
+// and the value register file is addressed by uniform switches so that it never spills to local memory.
+#ifndef SG_PASS1D_VM_CUH_
+#define SG_PASS1D_VM_CUH_
+
+#include "sg_pass1d.cuh"
+
+namespace sgk {
+
+constexpr int VM_VREG = 16;     // value registers of the bytecode evaluator (plan builder reuses dead registers)
+// elements per thread per tile: one 128-bit access per operand
+template <class T> struct VmE { static constexpr int value = 16 / (int)sizeof(T); };
+__host__ __device__ constexpr int vm_tile(int elem_size) { return BLOCK * (16 / elem_size); }
+
+#define SG_VM_CASES(X) X(0) X(1) X(2) X(3) X(4) X(5) X(6) X(7) X(8) X(9) X(10) X(11) X(12) X(13) X(14) X(15)
+
+template <class T, int E> struct VmRegs {
+    T r[VM_VREG][E];
+    __device__ __forceinline__ void get(uint8_t k, T (&o)[E]) const {
+        switch (k) {
+#define X(i) case i: _Pragma("unroll") for (int e = 0; e < E; ++e) o[e] = r[i][e]; break;
+            SG_VM_CASES(X)
+#undef X
+            default: break;
+        }
+    }
+    __device__ __forceinline__ void put(uint8_t k, const T (&o)[E]) {
+        switch (k) {
+#define X(i) case i: _Pragma("unroll") for (int e = 0; e < E; ++e) r[i][e] = o[e]; break;
+            SG_VM_CASES(X)
+#undef X
+            default: break;
+        }
+    }
+};
+
+// predicate file: SG_MAX_PREG registers x E bits packed in one 32-bit word (E <= 4)
+template <int E> __device__ __forceinline__ unsigned int pget(unsigned int pf, uint8_t k) { return (pf >> (k * E)) & ((1u << E) - 1u); }
+template <int E> __device__ __forceinline__ unsigned int pput(unsigned int pf, uint8_t k, unsigned int bits) {
+    const unsigned int m = ((1u << E) - 1u) << (k * E);
+    return (pf & ~m) | ((bits << (k * E)) & m);
+}
+
+template <class T, int E>
+__device__ __forceinline__ void vm_exec(const SgProg& g, VmRegs<T, E>& rf, unsigned int& pf) {
+    for (int i = 0; i < g.shape.n_instr; ++i) {
+        const SgInstr ins = g.code[i];
+        if (op_is_value(ins.op) || op_is_compare(ins.op)) {
+            T x[E], y[E];
+            rf.get(ins.a, x);
+            rf.get(ins.b, y);
+            if (op_is_value(ins.op)) {
+                T z[E];
+                switch (ins.op) {
+#define VOP(OPC) case OPC: _Pragma("unroll") for (int e = 0; e < E; ++e) z[e] = value_op<T>(OPC, x[e], y[e]); break;
+                    VOP(OP_ADD) VOP(OP_SUB) VOP(OP_MUL) VOP(OP_DIV) VOP(OP_MIN) VOP(OP_MAX) VOP(OP_MOD) VOP(OP_NEG) VOP(OP_ABS)
+#undef VOP
+                    default: _Pragma("unroll") for (int e = 0; e < E; ++e) z[e] = x[e]; break;
+                }
+                rf.put(ins.dst, z);
+            } else {
+                unsigned int bits = 0;
+                switch (ins.op) {
+#define COP(OPC) case OPC: _Pragma("unroll") for (int e = 0; e < E; ++e) bits |= (unsigned int)compare_op<T>(OPC, x[e], y[e]) << e; break;
+                    COP(OP_EQ) COP(OP_NE) COP(OP_LT) COP(OP_LE) COP(OP_GT)
+#undef COP
+                    default: _Pragma("unroll") for (int e = 0; e < E; ++e) bits |= (unsigned int)(x[e] >= y[e]) << e; break;
+                }
+                pf = pput<E>(pf, ins.dst, bits);
+            }
+        } else {
+            const unsigned int x = pget<E>(pf, ins.a), y = pget<E>(pf, ins.b);
+            const unsigned int z = ins.op == OP_AND ? (x & y) : ins.op == OP_OR ? (x | y) : ~x;
+            pf = pput<E>(pf, ins.dst, z);
+        }
+    }
+}
+
+// load input k for E consecutive elements starting at i (guarded: elements >= limit read as zero)
+template <class T, int E>
+__device__ __forceinline__ void vm_load(const SgProg& g, const SgArgs& a, int k, int64_t i, bool full, VmRegs<T, E>& rf, unsigned int& pf) {
+    typedef typename Traits<T>::vec VEC;
+    constexpr int V = Traits<T>::V;
+    const SgIn in = g.in[k];
+    T x[E];
+    if (in.kind == IN_VEC && full && ((a.vec_ok >> k) & 1)) {
+        const VEC* src = reinterpret_cast<const VEC*>(reinterpret_cast<const T*>(a.in_ptr[k]) + i);
+#pragma unroll
+        for (int u = 0; u < E / V; ++u) {
+            VEC w = ld_stream_rw(src + u);
+            const T* we = reinterpret_cast<const T*>(&w);
+#pragma unroll
+            for (int e = 0; e < V; ++e) x[u * V + e] = we[e];
+        }
+        rf.put(in.reg, x);
+    } else if (in.kind == IN_BOOLVEC) {
+        unsigned int bits = 0;
+#pragma unroll
+        for (int e = 0; e < E; ++e)
+            if (i + e < a.in_len[k]) bits |= (unsigned int)(reinterpret_cast<const volatile uint8_t*>(a.in_ptr[k])[i + e] != 0) << e;
+        pf = pput<E>(pf, in.reg, bits);
+    } else if (in.kind != IN_SCALAR && in.kind != IN_IMM) {
+#pragma unroll
+        for (int e = 0; e < E; ++e) x[e] = load_elem<T>(in.kind, in.ref, k, a, i + e);
+        rf.put(in.reg, x);
+    }
+}
+
+template <class T, int E>
+__device__ __forceinline__ void vm_emit(const SgProg& g, const SgArgs& a, int64_t i, int64_t hi, bool full, const VmRegs<T, E>& rf, unsigned int pf,
+                                        Cell (&acc)[SG_MAX_OUT]) {
+    typedef typename Traits<T>::vec VEC;
+    constexpr int V = Traits<T>::V;
+#pragma unroll
+    for (int o = 0; o < SG_MAX_OUT; ++o) {
+        if (o >= g.shape.n_out) break;
+        const SgOut out = g.out[o];
+        if (out.kind == OUT_FILTER) continue;      // handled by the compaction kernel
+        const int64_t len = a.out_len[o] < hi ? a.out_len[o] : hi;   // hi: end of the head range, or n
+        if (out_is_pred_reduction(out.kind) || out.kind == OUT_STORE_BOOL) {
+            const unsigned int bits = pget<E>(pf, out.src);
+#pragma unroll
+            for (int e = 0; e < E; ++e) {
+                if (i + e >= len) break;
+                if (out.kind == OUT_STORE_BOOL) reinterpret_cast<uint8_t*>(a.out_ptr[o])[i + e] = (bits >> e) & 1u;
+                else cell_accum_pred(out.kind, acc[o], (bits >> e) & 1u);
+            }
+        } else {
+            T x[E];
+            rf.get(out.src, x);
+            if (out.kind == OUT_STORE) {
+                if (full && ((a.vec_ok >> (16 + o)) & 1)) {
+                    VEC* dst = reinterpret_cast<VEC*>(reinterpret_cast<T*>(a.out_ptr[o]) + i);
+#pragma unroll
+                    for (int u = 0; u < E / V; ++u) st_stream(dst + u, *reinterpret_cast<const VEC*>(&x[u * V]));
+                } else {
+#pragma unroll
+                    for (int e = 0; e < E; ++e)
+                        if (i + e < len) reinterpret_cast<T*>(a.out_ptr[o])[i + e] = x[e];
+                }
+            } else {
+                const unsigned int mask = out.pred == SG_NO_PRED ? ((1u << E) - 1u) : pget<E>(pf, out.pred);
+#pragma unroll
+                for (int e = 0; e < E; ++e)
+                    if (i + e < len && ((mask >> e) & 1u)) {
+                        switch (out.kind) {
+                            case OUT_SUM: cell_accum_value<T>(OUT_SUM, acc[o], x[e]); break;
+                            case OUT_MAX: cell_accum_value<T>(OUT_MAX, acc[o], x[e]); break;
+                            default: cell_accum_value<T>(OUT_MIN, acc[o], x[e]); break;
+                        }
+                    }
+            }
+        }
+    }
+}
+
+template <class T>
+__global__ void __launch_bounds__(BLOCK) pass1d_bytecode(const __grid_constant__ SgProg g, const __grid_constant__ SgArgs a) {
+    constexpr int E = VmE<T>::value;
+    constexpr int VM_TILE = BLOCK * E;
+    Cell acc[SG_MAX_OUT];
+    uint8_t kind[SG_MAX_OUT];
+    bool has_reduction = false;
+    unsigned int need_mask = 0, flagged = 0;
+#pragma unroll
+    for (int o = 0; o < SG_MAX_OUT; ++o) {
+        kind[o] = (o < g.shape.n_out) ? g.out[o].kind : (uint8_t)OUT_STORE;
+        acc[o] = cell_identity<T>(kind[o]);
+        has_reduction |= out_is_reduction(kind[o]);
+        if (o < g.shape.n_out) need_mask |= 1u << o;
+    }
+    const bool early_exit = (g.shape.flags & PF_EARLY_EXIT) && !a.no_early_exit;
+
+    VmRegs<T, E> rf;
+    unsigned int pf = 0;
+    for (int k = 0; k < g.shape.n_in; ++k) {
+        const SgIn in = g.in[k];
+        if (in.kind == IN_SCALAR || in.kind == IN_IMM) {
+            T x[E];
+            const T s = load_elem<T>(in.kind, in.ref, k, a, 0);
+#pragma unroll
+            for (int e = 0; e < E; ++e) x[e] = s;
+            rf.put(in.reg, x);
+        }
+    }
+    // tiles over the aligned body [head, n) — the last tile is guarded; then the head [0, head) one vector at a time
+    const int64_t body = a.n - a.head;
+    const int64_t n_tiles = (body + VM_TILE - 1) / VM_TILE;
+    const int64_t head_tiles = (a.head + VM_TILE - 1) / VM_TILE;
+    for (int64_t tile = blockIdx.x; tile < n_tiles + head_tiles; tile += gridDim.x) {
+        if (early_exit && ld_volatile_u32(&a.ctrl[1]) == need_mask) break;
+        int64_t i, hi;
+        if (tile < n_tiles) { i = a.head + tile * VM_TILE + (int64_t)threadIdx.x * E; hi = a.n; }
+        else { i = (tile - n_tiles) * VM_TILE + (int64_t)threadIdx.x * E; hi = a.head; }
+        if (i < hi) {
+            // full: the whole vector lies inside every value's length and the body is 16-byte aligned
+            const bool full = (tile < a.n_full_tiles);
+            for (int k = 0; k < g.shape.n_in; ++k) vm_load<T, E>(g, a, k, i, full, rf, pf);
+            vm_exec<T, E>(g, rf, pf);
+            vm_emit<T, E>(g, a, i, hi, full, rf, pf, acc);
+        }
+        if (early_exit) {
+#pragma unroll
+            for (int o = 0; o < SG_MAX_OUT; ++o) {
+                if (o >= g.shape.n_out) break;
+                bool decided = (kind[o] == OUT_ALL) ? (acc[o].a == 0) : (acc[o].a != 0);
+                if (!(flagged & (1u << o)) && __any_sync(0xffffffffu, decided)) {
+                    flagged |= 1u << o;
+                    if ((threadIdx.x & 31) == 0) atomicOr(&a.ctrl[1], 1u << o);
+                }
+            }
+        }
+    }
+    epilogue_1d<T, SG_MAX_OUT>(acc, kind, a, has_reduction);
+}
+
+}  // namespace sgk
+#endif  // SG_PASS1D_VM_CUH_

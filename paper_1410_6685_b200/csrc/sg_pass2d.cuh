@@ -1,0 +1,299 @@
+// sg_pass2d.cuh — the fused matrix pass: elementwise chain over a rows x cols row-major
+// domain with ROW-/COL-broadcast vector operands, in-place store, and per-row / per-column /
+// whole-matrix reductions in the same pass.  The Gaussian-elimination row update of Listing 5 (PAPER.md:315-322,
+// 337-356) for ALL rows j > k is one launch of this kernel — the paper's per-row launches are what made that
+// benchmark slow.
+//
+// Tiling: block (strip s, chunk ch) owns columns [s*SW, (s+1)*SW) and rows [ch*rpc, (ch+1)*rpc).  A thread owns
+// E = U*V fixed columns (128-bit accesses) for every row of the chunk, so ROW-broadcast operands and per-column
+// accumulators live in registers for the whole chunk.  Loads of RU rows are issued before the first is used.
+// Per-column partials are combined over chunks by the last block of the strip, per-row partials over strips by
+// the last block of the chunk, both in fixed order (deterministic; no floating-point atomics).
+#ifndef SG_PASS2D_CUH_
+#define SG_PASS2D_CUH_
+
+#include "sg_pass1d_tmpl.cuh"
+
+namespace sgk {
+
+constexpr int RB = 32;      // rows per batch between the two barriers of the per-row combine
+
+template <class T> __device__ __forceinline__ void store_final(uint8_t kind, void* base, int64_t idx, const Cell& c) {
+    const unsigned long long r = cell_final<T>(kind, c);
+    if ((kind == OUT_MAX || kind == OUT_MIN) && sizeof(T) == 4) reinterpret_cast<uint32_t*>(base)[idx] = (uint32_t)r;
+    else reinterpret_cast<unsigned long long*>(base)[idx] = r;
+}
+__device__ __forceinline__ Cell ldcg_cell(const Cell* p) {
+    Cell c;
+    const unsigned long long* s = reinterpret_cast<const unsigned long long*>(p);
+    c.a = __ldcg(s); c.b = __ldcg(s + 1);
+    return c;
+}
+
+struct Slots2D { int vec[SG_MAX_IN]; int row[SG_MAX_OUT]; };
+
+template <class P> struct Meta2D : Meta1D<P> {
+    typedef Meta1D<P> B;
+    static constexpr int RU = P::row_unroll;
+    static constexpr int SW = BLOCK * B::E;     // strip width in columns
+    static constexpr int count_kind(uint8_t kind) {
+        int n = 0;
+        for (int k = 0; k < B::S.n_in; ++k) n += (P::prog.in[k].kind == kind);
+        return n;
+    }
+    static constexpr int NVECIN = count_kind(IN_VEC) > 0 ? count_kind(IN_VEC) : 1;
+    static constexpr int vec_slot(int K) {
+        int n = 0;
+        for (int k = 0; k < K; ++k) n += (P::prog.in[k].kind == IN_VEC);
+        return n;
+    }
+    static constexpr int count_axis(uint8_t axis) {
+        int n = 0;
+        for (int o = 0; o < B::S.n_out; ++o) n += (out_is_reduction(P::prog.out[o].kind) && P::prog.out[o].axis == axis);
+        return n;
+    }
+    static constexpr int NROWS = count_axis(AXIS_ROWS) > 0 ? count_axis(AXIS_ROWS) : 1;
+    static constexpr int row_slot(int O) {
+        int n = 0;
+        for (int o = 0; o < O; ++o) n += (out_is_reduction(P::prog.out[o].kind) && P::prog.out[o].axis == AXIS_ROWS);
+        return n;
+    }
+    static constexpr bool has_axis(uint8_t axis) { return count_axis(axis) > 0; }
+    static constexpr Slots2D slots() {
+        Slots2D s{};
+        for (int k = 0; k < SG_MAX_IN; ++k) s.vec[k] = k < B::S.n_in ? vec_slot(k) : 0;
+        for (int o = 0; o < SG_MAX_OUT; ++o) s.row[o] = o < B::S.n_out ? row_slot(o) : 0;
+        return s;
+    }
+    static constexpr Slots2D SLOTS = slots();
+    static constexpr bool HAS_ROWS = has_axis(AXIS_ROWS), HAS_COLS = has_axis(AXIS_COLS);
+};
+
+template <class P>
+__global__ void __launch_bounds__(BLOCK, P::min_blocks) pass2d_template(const __grid_constant__ SgArgs a) {
+    typedef Meta2D<P> M;
+    typedef typename M::T T;
+    typedef typename M::VEC VEC;
+    constexpr int U = M::U, V = M::V, E = M::E, RU = M::RU, NOUT = M::NOUT;
+    constexpr auto IS = std::make_integer_sequence<int, M::S.n_instr>{};
+    constexpr SgProg g = P::prog;                 // local constant copy: indexable inside unrolled loops
+    constexpr Slots2D slots = M::SLOTS;
+
+    __shared__ Cell s_row[M::NROWS][WARPS][RB];
+
+    const int strip = blockIdx.x % a.n_strips, chunk = blockIdx.x / a.n_strips;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int64_t r_begin = (int64_t)chunk * a.rows_per_chunk;
+    const int64_t r_end = (r_begin + a.rows_per_chunk < a.n) ? (r_begin + a.rows_per_chunk) : a.n;
+    int64_t col[U];
+    bool cvalid[U];
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+        col[u] = (int64_t)strip * M::SW + (int64_t)(u * BLOCK + threadIdx.x) * V;
+        cvalid[u] = col[u] + V <= a.cols;
+    }
+
+    T v[M::NV][E];
+    bool p[M::NP][E];
+    Cell acc[NOUT];             // AXIS_ALL
+    Cell acc_col[NOUT][E];      // AXIS_COLS (unused entries are dead code)
+    uint8_t kind[NOUT];
+    bool has_all = false;
+#pragma unroll
+    for (int o = 0; o < NOUT; ++o) {
+        kind[o] = (o < M::S.n_out && g.out[o].axis == AXIS_ALL) ? g.out[o].kind : (uint8_t)OUT_STORE;
+        acc[o] = cell_identity<T>(kind[o]);
+        has_all |= out_is_reduction(kind[o]);
+#pragma unroll
+        for (int e = 0; e < E; ++e) acc_col[o][e] = cell_identity<T>(o < M::S.n_out ? g.out[o].kind : (uint8_t)OUT_STORE);
+    }
+
+    // operands that do not depend on the row: immediates, device scalars, ROW-broadcast vectors
+#pragma unroll
+    for (int k = 0; k < M::S.n_in; ++k) {
+        const SgIn in = g.in[k];
+        if (in.kind == IN_SCALAR || in.kind == IN_IMM) {
+            const T s = load_elem<T>(in.kind, in.ref, k, a, 0);
+#pragma unroll
+            for (int e = 0; e < E; ++e) v[in.reg][e] = s;
+        } else if (in.kind == IN_ROWB) {
+#pragma unroll
+            for (int u = 0; u < U; ++u) {
+                VEC x = VEC();
+                if (cvalid[u]) x = *reinterpret_cast<const VEC*>(reinterpret_cast<const T*>(a.in_ptr[k]) + col[u]);
+                const T* xe = reinterpret_cast<const T*>(&x);
+#pragma unroll
+                for (int e = 0; e < V; ++e) v[in.reg][u * V + e] = xe[e];
+            }
+        }
+    }
+
+    for (int64_t rb = r_begin; rb < r_end; rb += RB) {
+        const int64_t rb_end = (rb + RB < r_end) ? rb + RB : r_end;
+        for (int64_t r0 = rb; r0 < rb_end; r0 += RU) {
+            VEC ld[M::NVECIN][RU][U];
+#pragma unroll
+            for (int k = 0; k < M::S.n_in; ++k) {
+                const SgIn in = g.in[k];
+                if (in.kind != IN_VEC) continue;
+                const int slot = slots.vec[k];
+#pragma unroll
+                for (int j = 0; j < RU; ++j) {
+                    if (r0 + j < rb_end) {
+                        const T* rowp = reinterpret_cast<const T*>(a.in_ptr[k]) + (r0 + j) * a.in_stride[k];
+#pragma unroll
+                        for (int u = 0; u < U; ++u)
+                            if (cvalid[u]) ld[slot][j][u] = in.pad ? ld_stream_rw(reinterpret_cast<const VEC*>(rowp + col[u]))
+                                                                   : ld_stream(reinterpret_cast<const VEC*>(rowp + col[u]));
+                    }
+                }
+            }
+#pragma unroll
+            for (int j = 0; j < RU; ++j) {
+                const int64_t r = r0 + j;
+                if (r >= rb_end) break;
+#pragma unroll
+                for (int k = 0; k < M::S.n_in; ++k) {
+                    const SgIn in = g.in[k];
+                    if (in.kind == IN_VEC) {
+                        const int slot = slots.vec[k];
+#pragma unroll
+                        for (int u = 0; u < U; ++u) {
+                            const T* xe = reinterpret_cast<const T*>(&ld[slot][j][u]);
+#pragma unroll
+                            for (int e = 0; e < V; ++e) v[in.reg][u * V + e] = xe[e];
+                        }
+                    } else if (in.kind == IN_COLB) {
+                        const T s = __ldg(reinterpret_cast<const T*>(a.in_ptr[k]) + r);
+#pragma unroll
+                        for (int e = 0; e < E; ++e) v[in.reg][e] = s;
+                    }
+                }
+                exec_body<P, T, M::NV, M::NP, E>(v, p, IS);
+#pragma unroll
+                for (int o = 0; o < M::S.n_out; ++o) {
+                    const SgOut out = g.out[o];
+                    if (out.kind == OUT_STORE) {
+                        T* rowp = reinterpret_cast<T*>(a.out_ptr[o]) + r * a.out_len[o];
+#pragma unroll
+                        for (int u = 0; u < U; ++u) {
+                            if (!cvalid[u]) continue;
+                            VEC x;
+                            T* xe = reinterpret_cast<T*>(&x);
+#pragma unroll
+                            for (int e = 0; e < V; ++e) xe[e] = v[out.src][u * V + e];
+                            st_stream(reinterpret_cast<VEC*>(rowp + col[u]), x);
+                        }
+                    } else if (out_is_reduction(out.kind)) {
+                        Cell rowc = cell_identity<T>(out.kind);
+#pragma unroll
+                        for (int u = 0; u < U; ++u) {
+                            if (!cvalid[u]) continue;
+#pragma unroll
+                            for (int e = 0; e < V; ++e) {
+                                const int ee = u * V + e;
+                                Cell& dstc = (out.axis == AXIS_ALL) ? acc[o] : (out.axis == AXIS_COLS) ? acc_col[o][ee] : rowc;
+                                if (out_is_pred_reduction(out.kind)) cell_accum_pred(out.kind, dstc, p[out.src][ee]);
+                                else if (out.pred == SG_NO_PRED || p[out.pred == SG_NO_PRED ? 0 : out.pred][ee]) cell_accum_value<T>(out.kind, dstc, v[out.src][ee]);
+                            }
+                        }
+                        if (out.axis == AXIS_ROWS) {
+#pragma unroll
+                            for (int d = 16; d >= 1; d >>= 1) {
+                                Cell other = cell_shfl_xor(rowc, d);
+                                cell_combine<T>(out.kind, rowc, other);
+                            }
+                            if (lane == 0) s_row[slots.row[o]][warp][(int)(r - rb)] = rowc;
+                        }
+                    }
+                }
+            }
+        }
+        if (M::HAS_ROWS) {
+            __syncthreads();
+            if ((int64_t)threadIdx.x < rb_end - rb) {
+#pragma unroll
+                for (int o = 0; o < M::S.n_out; ++o) {
+                    const SgOut out = g.out[o];
+                    if (!(out_is_reduction(out.kind) && out.axis == AXIS_ROWS)) continue;
+                    Cell c = s_row[slots.row[o]][0][threadIdx.x];
+#pragma unroll
+                    for (int w = 1; w < WARPS; ++w) cell_combine<T>(out.kind, c, s_row[slots.row[o]][w][threadIdx.x]);
+                    Cell* ws = reinterpret_cast<Cell*>(reinterpret_cast<char*>(a.workspace) + a.ws_off[o]);
+                    ws[(size_t)strip * a.n + rb + threadIdx.x] = c;
+                }
+            }
+            __syncthreads();
+        }
+    }
+
+    // per-column partials of this chunk
+    if (M::HAS_COLS) {
+#pragma unroll
+        for (int o = 0; o < M::S.n_out; ++o) {
+            const SgOut out = g.out[o];
+            if (!(out_is_reduction(out.kind) && out.axis == AXIS_COLS)) continue;
+            Cell* ws = reinterpret_cast<Cell*>(reinterpret_cast<char*>(a.workspace) + a.ws_off[o]);
+#pragma unroll
+            for (int u = 0; u < U; ++u) {
+                if (!cvalid[u]) continue;
+#pragma unroll
+                for (int e = 0; e < V; ++e) ws[(size_t)chunk * a.cols + col[u] + e] = acc_col[o][u * V + e];
+            }
+        }
+    }
+
+    // tickets: last block of the strip combines the chunks, last block of the chunk combines the strips
+    if (M::HAS_COLS || M::HAS_ROWS) {
+        __shared__ unsigned int s_flags;
+        unsigned int* ctrl2 = a.ctrl + 8;
+        __threadfence();
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            unsigned int f = 0;
+            if (M::HAS_COLS && atomicAdd(&ctrl2[strip], 1u) == (unsigned int)a.n_chunks - 1) f |= 1u;
+            if (M::HAS_ROWS && atomicAdd(&ctrl2[a.n_strips + chunk], 1u) == (unsigned int)a.n_strips - 1) f |= 2u;
+            s_flags = f;
+        }
+        __syncthreads();
+        const unsigned int f = s_flags;
+        if (f) __threadfence();
+        if (f & 1u) {
+#pragma unroll
+            for (int o = 0; o < M::S.n_out; ++o) {
+                const SgOut out = g.out[o];
+                if (!(out_is_reduction(out.kind) && out.axis == AXIS_COLS)) continue;
+                const Cell* ws = reinterpret_cast<const Cell*>(reinterpret_cast<char*>(a.workspace) + a.ws_off[o]);
+#pragma unroll
+                for (int u = 0; u < U; ++u) {
+                    if (!cvalid[u]) continue;
+#pragma unroll
+                    for (int e = 0; e < V; ++e) {
+                        Cell c = cell_identity<T>(out.kind);
+                        for (int ch = 0; ch < a.n_chunks; ++ch) cell_combine<T>(out.kind, c, ldcg_cell(&ws[(size_t)ch * a.cols + col[u] + e]));
+                        store_final<T>(out.kind, a.out_ptr[o], col[u] + e, c);
+                    }
+                }
+            }
+            if (threadIdx.x == 0) ctrl2[strip] = 0;
+        }
+        if (f & 2u) {
+#pragma unroll
+            for (int o = 0; o < M::S.n_out; ++o) {
+                const SgOut out = g.out[o];
+                if (!(out_is_reduction(out.kind) && out.axis == AXIS_ROWS)) continue;
+                const Cell* ws = reinterpret_cast<const Cell*>(reinterpret_cast<char*>(a.workspace) + a.ws_off[o]);
+                for (int64_t r = r_begin + threadIdx.x; r < r_end; r += BLOCK) {
+                    Cell c = cell_identity<T>(out.kind);
+                    for (int s = 0; s < a.n_strips; ++s) cell_combine<T>(out.kind, c, ldcg_cell(&ws[(size_t)s * a.n + r]));
+                    store_final<T>(out.kind, a.out_ptr[o], r, c);
+                }
+            }
+            if (threadIdx.x == 0) ctrl2[a.n_strips + chunk] = 0;
+        }
+    }
+    epilogue_1d<T, NOUT>(acc, kind, a, has_all);
+}
+
+}  // namespace sgk
+#endif  // SG_PASS2D_CUH_

@@ -1,0 +1,362 @@
+// sg_plan.cpp — the plan builder and flush.
+//
+// "Before generating kernels, the optimizer constructs an execution plan from the pending operations.  The plan
+// takes the form of a DAG ... The optimizer then traverses the DAG, merging kernel vertices and collapsing
+// intermediate dependencies where possible".  Here: liveness decides which data nodes are
+// materialised (a live user handle) and which collapse into registers (anonymous intermediates);
+// kernel nodes are merged greedily into PASSES — one fused launch each — under three kinds of edge:
+//   register edges  (producer and consumer may share a pass),
+//   scalar edges    (a reduction result consumed elementwise: consumer pass > producer pass),
+//   memory edges    (RAW / WAR / WAW on overlapping storage of in-place operations and views).
+// SG_FLAG_UNFUSED turns every pending operation into its own pass with a materialised result: the naive
+// "one kernel per method call" plan of PAPER.md:282, kept as the measurement baseline.
+#include <stdio.h>
+#include <string.h>
+
+#include <algorithm>
+#include <map>
+
+#include "sg_ctx.h"
+
+sg_status sg_build_pass(sg_ctx* c, Pass& P, std::vector<char*>& temps, std::string& dump);   // sg_build.cpp
+
+namespace {
+
+int es_of(const Value& v) { return dtype_size(v.dtype); }
+
+MemRange range_of(const Value& v) {
+    MemRange r;
+    const int64_t es = es_of(v);
+    r.ptr = v.ptr; r.stride = v.stride; r.ld = v.ld; r.rows = v.rows; r.cols = v.cols;
+    r.lo = v.ptr;
+    if (v.kind == VK_MAT) r.hi = v.ptr + ((v.rows > 0 ? (v.rows - 1) * v.ld : 0) + v.cols) * es;
+    else if (v.kind == VK_SCALAR) r.hi = v.ptr + es;
+    else r.hi = v.ptr + ((v.cols > 0 ? (v.cols - 1) * v.stride : 0) + 1) * es;
+    return r;
+}
+bool overlaps(const MemRange& a, const MemRange& b) { return a.lo < b.hi && b.lo < a.hi; }
+bool same_view(const MemRange& a, const MemRange& b) {
+    return a.ptr == b.ptr && a.stride == b.stride && a.ld == b.ld && a.rows == b.rows && a.cols == b.cols;
+}
+
+bool pending(const sg_ctx* c, const Value& v) { return v.node >= 0 && !c->nodes[v.node].done; }
+
+}  // namespace
+
+sg_status sg_flush_impl(sg_ctx* c) {
+    const bool unfused = c->flags & SG_FLAG_UNFUSED;
+    std::vector<Node>& N = c->nodes;
+    std::vector<Value>& V = c->values;
+    int64_t launches_total = c->stats.launches_total;
+    if (N.empty()) return SG_OK;
+    memset(&c->stats, 0, sizeof(c->stats));
+    c->stats.launches_total = launches_total;
+    c->dumps.clear();
+
+    // ---- 1. liveness: which pending operations are needed at all ----------------------------------------
+    std::vector<int> work;
+    auto need = [&](int i) { if (i >= 0 && !N[i].done && !N[i].needed) { N[i].needed = true; work.push_back(i); } };
+    for (size_t i = 0; i < N.size(); ++i) {
+        if (N[i].done) continue;
+        const bool live = (N[i].out >= 0 && V[N[i].out].user_refs > 0) || (N[i].out2 >= 0 && V[N[i].out2].user_refs > 0) || N[i].inplace;
+        if (live) need((int)i);
+    }
+    for (const Contract& k : c->contracts) need(V[k.value].node);
+    while (!work.empty()) {
+        const int i = work.back(); work.pop_back();
+        for (int j = 0; j < N[i].n_opd; ++j)
+            if (N[i].opd[j].kind != OPD_IMM) need(V[N[i].opd[j].value].node);
+    }
+    // values that will exist in memory after this flush (live handle or caller-provided storage)
+    auto materialises = [&](const Node& n) {
+        if (n.kind != NK_MAP) return false;
+        return unfused || n.inplace || V[n.out].user_refs > 0;
+    };
+    // ---- 2. POST contracts read stored results (R17): mark their predicate cone ----------------
+    std::vector<int> post_group(N.size(), -1);
+    std::vector<std::vector<int>> post_leaves(c->contracts.size());
+    for (size_t ki = 0; ki < c->contracts.size(); ++ki) {
+        const Contract& k = c->contracts[ki];
+        if (k.kind != SG_CONTRACT_POST) continue;
+        std::vector<int> st{V[k.value].node};
+        while (!st.empty()) {
+            const int i = st.back(); st.pop_back();
+            if (i < 0 || N[i].done || N[i].post) continue;
+            N[i].post = true;
+            post_group[i] = (int)ki;
+            for (int j = 0; j < N[i].n_opd; ++j) {
+                if (N[i].opd[j].kind == OPD_IMM) continue;
+                const Value& v = V[N[i].opd[j].value];
+                if (!pending(c, v)) continue;
+                if (materialises(N[v.node])) { post_leaves[ki].push_back(v.node); continue; }   // leaf: read back from memory
+                st.push_back(v.node);
+            }
+        }
+    }
+
+    // ---- 3. pass assignment ------------------------------------------------------------------------------
+    std::vector<Pass> passes;
+    std::vector<char> spill(V.size(), 0);       // value must be stored because a later pass consumes it
+    for (size_t i = 0; i < N.size(); ++i) {
+        Node& X = N[i];
+        if (X.done || !X.needed) continue;
+        int lb = 0, forced = -1;
+        std::vector<MemRange> reads, writes;
+        std::vector<int> reg_producers;
+        for (int j = 0; j < X.n_opd; ++j) {
+            if (X.opd[j].kind == OPD_IMM) continue;
+            const Value& v = V[X.opd[j].value];
+            if (pending(c, v) && N[v.node].needed) {
+                const Node& Y = N[v.node];
+                if (Y.kind == NK_MAP) {
+                    const bool via_memory = unfused || (X.post && materialises(Y)) || X.opd[j].kind == OPD_SHIFT;
+                    lb = std::max(lb, Y.pass + (via_memory ? 1 : 0));
+                    if (!via_memory) reg_producers.push_back(v.node);
+                    if (X.opd[j].kind == OPD_SHIFT) spill[X.opd[j].value] = 1;
+                } else if (Y.kind == NK_REDUCE) {
+                    lb = std::max(lb, Y.pass + 1);
+                } else {    // NK_FILTER: only a reduction over the kept values may follow, in the same pass
+                    if (X.kind != NK_REDUCE) return sg_fail(c, SG_ERR_UNSUPPORTED, "operation on a pending filter output");
+                    forced = Y.pass;
+                }
+            } else {
+                if (!v.materialised && v.slot < 0) return sg_fail(c, SG_ERR_ARG, "operand has neither storage nor a pending producer");
+                if (v.slot >= 0) continue;                      // scalar slot written by an earlier flush
+                reads.push_back(range_of(v));
+            }
+        }
+        if (X.post && post_group[i] >= 0)       // the whole predicate of a POST contract runs after the results it reads are stored
+            for (int y : post_leaves[post_group[i]])
+                if (N[y].pass >= 0) lb = std::max(lb, N[y].pass + 1);
+        if (X.kind == NK_MAP && X.inplace) writes.push_back(range_of(V[X.out]));
+        if (X.kind == NK_FILTER && X.inplace) writes.push_back(range_of(V[X.out]));
+        for (size_t q = 0; q < passes.size(); ++q) {
+            for (const MemRange& r : reads)
+                for (const MemRange& w : passes[q].writes)
+                    if (overlaps(r, w)) lb = std::max(lb, (int)q + 1);                          // RAW through memory
+            for (const MemRange& w : writes) {
+                for (const MemRange& w2 : passes[q].writes)
+                    if (overlaps(w, w2)) lb = std::max(lb, (int)q + 1);                         // WAW
+                for (const MemRange& r : passes[q].reads)
+                    if (overlaps(w, r)) lb = std::max(lb, (int)q + (same_view(w, r) ? 0 : 1));  // WAR: same pass only index-for-index
+            }
+        }
+        // within this very operation: an in-place result may alias an operand only index-for-index
+        for (const MemRange& w : writes)
+            for (const MemRange& r : reads)
+                if (overlaps(w, r) && !same_view(w, r)) return sg_fail(c, SG_ERR_ALIAS, "in-place operation reads a shifted or overlapping view of its destination");
+
+        const bool stores = materialises(X);
+        const int xdt = (X.dtype == SG_BOOL) ? -1 : X.dtype;
+        auto compatible = [&](const Pass& P) {
+            if (unfused) return false;
+            if (P.is2d != X.is2d) return false;
+            if (X.is2d) { if (P.rows != X.rows || P.cols != X.cols) return false; }
+            else if (std::llabs((long long)(P.cols - X.cols)) > 1024) return false;
+            if (xdt >= 0 && P.dtype >= 0 && P.dtype != xdt) return false;
+            if (X.kind == NK_FILTER && (P.has_filter || P.has_store || X.is2d)) return false;
+            if (stores && P.has_filter) return false;
+            if ((int)P.nodes.size() + 1 > SG_MAX_INSTR) return false;
+            int outs = 0;
+            for (int k : P.nodes) outs += (N[k].kind != NK_MAP) || materialises(N[k]) || spill[N[k].out];
+            if (outs + 1 > SG_MAX_OUT) return false;
+            return true;
+        };
+        int p = -1;
+        if (forced >= 0) {
+            if (lb > forced) return sg_fail(c, SG_ERR_UNSUPPORTED, "reduction over a filter output cannot share the filter's pass");
+            p = forced;
+        } else {
+            for (size_t q = (size_t)lb; q < passes.size(); ++q)
+                if (compatible(passes[q])) { p = (int)q; break; }
+            if (p < 0) {
+                passes.emplace_back();
+                p = (int)passes.size() - 1;
+                passes[p].is2d = X.is2d; passes[p].rows = X.rows; passes[p].cols = X.cols;
+            }
+        }
+        Pass& P = passes[p];
+        X.pass = p;
+        P.nodes.push_back((int)i);
+        if (!X.is2d) P.cols = std::max(P.cols, X.cols);
+        if (xdt >= 0 && P.dtype < 0) P.dtype = xdt;
+        P.has_filter |= (X.kind == NK_FILTER);
+        P.has_store |= stores;
+        for (const MemRange& r : reads) P.reads.push_back(r);
+        for (const MemRange& w : writes) P.writes.push_back(w);
+        for (int y : reg_producers)
+            if (N[y].pass < p) {                                // register edge became a cross-pass edge: spill the value
+                spill[N[y].out] = 1;
+                if (passes[N[y].pass].has_filter) return sg_fail(c, SG_ERR_UNSUPPORTED, "a filter pass cannot materialise an intermediate");
+                passes[N[y].pass].has_store = true;
+            }
+    }
+    if (passes.size() > 16) return sg_fail(c, SG_ERR_CAPACITY, "more than 16 passes in one flush");
+
+    // ---- 4. programs, outputs, geometry ------------------------------------------------------------------
+    // spilled intermediates become context-owned temporaries, released after the launches are queued
+    std::vector<char*> temps;
+    c->stats.n_passes = (int32_t)passes.size();
+    for (const Node& n : N) c->stats.n_nodes += (!n.done && n.needed);
+    std::vector<char> spill_copy = spill;
+    for (size_t pi = 0; pi < passes.size(); ++pi) {
+        Pass& P = passes[pi];
+        // mark spilled values by giving them a (hidden) reference for the duration of the build
+        for (int k : P.nodes)
+            if (N[k].kind == NK_MAP && spill_copy[N[k].out] && V[N[k].out].user_refs == 0) V[N[k].out].user_refs = -1;
+        std::string dump;
+        sg_status s = sg_build_pass(c, P, temps, dump);
+        if (s != SG_OK) return s;
+        c->dumps.push_back(dump);
+        char err[256] = {0};
+        int rc = sgk_plan(P.prog, P.args, (c->flags & SG_FLAG_FORCE_BYTECODE) ? 1 : 0, c->sm_count, c->plan_only ? 0 : 1, &P.geom, err, sizeof(err));
+        if (rc != 0) return sg_fail(c, (sg_status)rc, err);
+        P.args.no_early_exit = (c->flags & SG_FLAG_NO_EARLY_EXIT) ? 1 : 0;
+        if (pi < 16) {
+            c->stats.pass_n_in[pi] = P.n_mem_in;
+            c->stats.pass_n_instr[pi] = P.prog.shape.n_instr;
+            c->stats.pass_n_out[pi] = P.prog.shape.n_out;
+            c->stats.pass_n_args[pi] = P.n_mem_in + P.n_scalar_in + P.prog.shape.n_out;
+            c->stats.pass_kernel[pi] = P.geom.template_id;
+        }
+        c->stats.bytes_min += P.bytes;
+        if (P.geom.template_id > 0) c->stats.n_template++; else c->stats.n_bytecode++;
+    }
+
+    // ---- 5. resources and launches -----------------------------------------------------------------------
+    c->last.clear();
+    if (!c->plan_only) {
+        size_t ws = 0, st = 0; int cw = 0;
+        for (const Pass& P : passes) { ws = std::max(ws, P.geom.ws_bytes); st = std::max(st, P.geom.state_words); cw = std::max(cw, P.geom.ctrl_words); }
+        if (cw + 8 > c->ctrl_words) return sg_fail(c, SG_ERR_CAPACITY, "matrix pass needs more ticket words than the control block holds");
+        if (ws > c->workspace_bytes) {
+            cudaStreamSynchronize(c->stream);
+            if (c->workspace) cudaFree(c->workspace);
+            c->workspace_bytes = ws + ws / 4;
+            if (cudaMalloc((void**)&c->workspace, c->workspace_bytes) != cudaSuccess) { c->workspace = nullptr; c->workspace_bytes = 0; cudaGetLastError(); return sg_fail(c, SG_ERR_OOM, "workspace allocation failed"); }
+        }
+        if (st > c->tile_state_words) {
+            cudaStreamSynchronize(c->stream);
+            if (c->tile_state) cudaFree(c->tile_state);
+            c->tile_state_words = st + st / 4;
+            if (cudaMalloc((void**)&c->tile_state, 8 * c->tile_state_words) != cudaSuccess || cudaMemset(c->tile_state, 0, 8 * c->tile_state_words) != cudaSuccess) {
+                c->tile_state = nullptr; c->tile_state_words = 0; cudaGetLastError();
+                return sg_fail(c, SG_ERR_OOM, "tile-state allocation failed");
+            }
+        }
+        cudaEventRecord(c->ev_t0, c->stream);
+        for (Pass& P : passes) {
+            P.args.workspace = c->workspace;
+            P.args.tile_state = c->tile_state;
+            P.args.ctrl = c->ctrl;
+            if (P.prog.shape.flags & PF_FILTER) {
+                if (++c->epoch > 0x3ffff0u) {       // epoch tag about to wrap: clear the states once
+                    cudaMemsetAsync(c->tile_state, 0, 8 * c->tile_state_words, c->stream);
+                    c->epoch = 1;
+                }
+                P.args.epoch = c->epoch;
+            }
+            cudaError_t e = sgk_launch(P.prog, P.args, P.geom, c->stream);
+            if (e != cudaSuccess) return sg_fail(c, SG_ERR_CUDA, std::string("kernel launch failed: ") + cudaGetErrorString(e));
+            c->last.push_back({P.prog, P.args, P.geom});
+            launches_total++;
+        }
+        cudaEventRecord(c->ev_t1, c->stream);
+        // a8: hand the flush's scalars back in one copy
+        int64_t lo = c->slab_slots, hi = -1;
+        for (const Node& n : N) {
+            if (n.done || !n.needed) continue;
+            for (int o : {n.out, n.out2})
+                if (o >= 0 && V[o].kind == VK_SCALAR && V[o].slot >= 0) { lo = std::min(lo, V[o].slot); hi = std::max(hi, V[o].slot); }
+        }
+        if (hi >= lo) {
+            if (cudaMemcpyAsync(c->slab_host + 8 * lo, c->slab + 8 * lo, 8 * (size_t)(hi - lo + 1), cudaMemcpyDeviceToHost, c->stream) != cudaSuccess)
+                return sg_fail(c, SG_ERR_CUDA, "scalar hand-back failed");
+        }
+        cudaEventRecord(c->ev_done, c->stream);
+        // storage released since the previous flush goes back now; this flush's temporaries stay until the next
+        // flush so that sg_replay_last can re-run the same launches
+        for (char* t : c->deferred_free) sg_dev_free(c, t);
+        c->deferred_free = temps;
+    } else {
+        for (Pass& P : passes) c->last.push_back({P.prog, P.args, P.geom});
+    }
+    c->stats.launches_total = launches_total;
+
+    // ---- 6. commit: results now have storage; the pending list is consumed -------------------------------
+    for (Node& n : N) {
+        if (n.done) continue;
+        n.done = true;
+        for (int o : {n.out, n.out2}) {
+            if (o < 0) continue;
+            Value& v = V[o];
+            if (v.user_refs < 0) v.user_refs = 0;
+            if (v.node >= 0 && &N[v.node] == &n) v.node = -1;
+        }
+    }
+    for (Value& v : V) if (v.node >= 0 && N[v.node].done) v.node = -1;
+    N.clear();
+    for (Value& v : V) {            // unreferenced results die with the flush
+        if (!v.alive || v.user_refs > 0) continue;
+        if (v.owned && v.ptr) { c->deferred_free.push_back(v.ptr); v.ptr = nullptr; v.owned = false; }
+        if (v.kind == VK_SCALAR && v.slot >= 0) {
+            bool contract = false;
+            for (const Contract& k : c->contracts) contract |= (&V[k.value] == &v);
+            if (!contract) { c->slab_free.push_back(v.slot); v.slot = -1; v.alive = false; }
+        } else v.alive = false;
+    }
+
+    // ---- 7. contracts: evaluated on the device with the data; read with the scalars ----
+    sg_status result = SG_OK;
+    if (!c->contracts.empty()) {
+        if (!c->plan_only && cudaEventSynchronize(c->ev_done) != cudaSuccess) return sg_fail(c, SG_ERR_CUDA, "event sync failed");
+        for (const Contract& k : c->contracts) {
+            const Value& v = V[k.value];
+            bool ok = true;
+            if (!c->plan_only && v.slot >= 0) ok = c->slab_host[8 * v.slot] != 0;
+            if (!ok && result == SG_OK) {
+                result = SG_ERR_CONTRACT;
+                c->err = std::string(k.kind == SG_CONTRACT_PRE ? "precondition" : "postcondition") + " violated: " + k.tag;
+            }
+        }
+        c->contracts.clear();
+    }
+    if (!c->plan_only) {
+        cudaError_t e = cudaGetLastError();
+        if (e != cudaSuccess) return sg_fail(c, SG_ERR_CUDA, cudaGetErrorString(e));
+    }
+    return result;
+}
+
+extern "C" sg_status sg_last_flush_ms(sg_ctx* c, float* ms) {
+    if (!c || !ms) return SG_ERR_ARG;
+    if (c->plan_only) { *ms = 0.f; return SG_OK; }
+    if (cudaEventSynchronize(c->ev_t1) != cudaSuccess || cudaEventElapsedTime(ms, c->ev_t0, c->ev_t1) != cudaSuccess) {
+        cudaGetLastError();
+        return sg_fail(c, SG_ERR_CUDA, "no timed flush");
+    }
+    return SG_OK;
+}
+
+extern "C" sg_status sg_replay_last(sg_ctx* c, int32_t reps, float* ms_per_rep) {
+    if (!c || !ms_per_rep || reps <= 0) return SG_ERR_ARG;
+    if (c->plan_only) { *ms_per_rep = 0.f; return SG_OK; }
+    if (c->last.empty()) return sg_fail(c, SG_ERR_ARG, "nothing to replay");
+    cudaEventRecord(c->ev_t0, c->stream);
+    for (int r = 0; r < reps; ++r)
+        for (Launch& l : c->last) {
+            if (l.prog.shape.flags & PF_FILTER) {
+                if (++c->epoch > 0x3ffff0u) { cudaMemsetAsync(c->tile_state, 0, 8 * c->tile_state_words, c->stream); c->epoch = 1; }
+                l.args.epoch = c->epoch;
+            }
+            cudaError_t e = sgk_launch(l.prog, l.args, l.geom, c->stream);
+            if (e != cudaSuccess) return sg_fail(c, SG_ERR_CUDA, cudaGetErrorString(e));
+            c->stats.launches_total++;
+        }
+    cudaEventRecord(c->ev_t1, c->stream);
+    float ms = 0.f;
+    if (cudaEventSynchronize(c->ev_t1) != cudaSuccess || cudaEventElapsedTime(&ms, c->ev_t0, c->ev_t1) != cudaSuccess)
+        return sg_fail(c, SG_ERR_CUDA, cudaGetErrorString(cudaGetLastError()));
+    *ms_per_rep = ms / reps;
+    return SG_OK;
+}

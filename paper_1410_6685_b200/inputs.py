@@ -17,6 +17,9 @@ stand in for them.
 """
 from __future__ import annotations
 
+import concurrent.futures
+import os
+
 import numpy as np
 
 _GAMMA = np.uint64(0x9E3779B97F4A7C15)
@@ -64,31 +67,43 @@ def _chunks(n: int):
         yield s, min(_CHUNK, n - s)
 
 
+def _fill(out: np.ndarray, fn) -> np.ndarray:
+    """out[s:s+c] = fn(s, c) for every chunk; chunks are independent (counter-based), so threads may fill them."""
+    n = out.size
+    chunks = list(_chunks(n))
+    workers = min(len(chunks), os.cpu_count() or 1, 16)
+
+    def job(sc):
+        out[sc[0]:sc[0] + sc[1]] = fn(*sc)
+
+    if workers <= 1:
+        for sc in chunks:
+            job(sc)
+    else:
+        with concurrent.futures.ThreadPoolExecutor(max_workers=workers) as ex:
+            list(ex.map(job, chunks))
+    return out
+
+
 def uniform_pm1_f64(seed: int, stream: int, n: int) -> np.ndarray:
     """float64[n], 2*u01 - 1 in [-1, 1)  (configs 0 and 4)."""
-    out = np.empty(n, dtype=np.float64)
-    for s, c in _chunks(n):
-        out[s:s + c] = 2.0 * u01(seed, stream, s, c) - 1.0
-    return out
+    return _fill(np.empty(n, dtype=np.float64), lambda s, c: 2.0 * u01(seed, stream, s, c) - 1.0)
 
 
 def normal_f32(seed: int, stream: int, n: int) -> np.ndarray:
     """float32[n] ~ N(0,1): Box-Muller in float64 on counters (2i, 2i+1), one output per pair (config 1)."""
-    out = np.empty(n, dtype=np.float32)
-    for s, c in _chunks(n):
+    def chunk(s, c):
         u = u01(seed, stream, 2 * s, 2 * c)
         u1 = 1.0 - u[0::2]          # (0, 1]
         u2 = u[1::2]
-        out[s:s + c] = (np.sqrt(-2.0 * np.log(u1)) * np.cos(2.0 * np.pi * u2)).astype(np.float32)
-    return out
+        return (np.sqrt(-2.0 * np.log(u1)) * np.cos(2.0 * np.pi * u2)).astype(np.float32)
+
+    return _fill(np.empty(n, dtype=np.float32), chunk)
 
 
 def uniform_i31(seed: int, stream: int, n: int) -> np.ndarray:
     """int32[n] uniform on [0, 2^31): bits >> 33 (config 2)."""
-    out = np.empty(n, dtype=np.int32)
-    for s, c in _chunks(n):
-        out[s:s + c] = (bits(seed, stream, s, c) >> np.uint64(33)).astype(np.int32)
-    return out
+    return _fill(np.empty(n, dtype=np.int32), lambda s, c: (bits(seed, stream, s, c) >> np.uint64(33)).astype(np.int32))
 
 
 def sorted_cumsum_f32(seed: int, stream: int, n: int) -> np.ndarray:

@@ -1,0 +1,168 @@
+"""The paper's example programs and the five BASELINE.json workloads written against the C ABI (sg.py).
+
+These are USER programs in the sense of the paper's listings: they only call collection primitives; every
+arithmetic step runs inside libsafegpu.so.  Device pointers are plain ints (``tensor.data_ptr()``); with a
+plan-only context (device -1) they may be None.  Each function returns a dict of handles; nothing executes
+until a scalar is read or sg_flush is called.
+"""
+from __future__ import annotations
+
+from . import sg
+from .sg import F, H, I
+
+
+def dot_product(ctx, dtype, n, pa, pb):
+    """Listing 4: a.compwise_multiply(b).sum — the product is an anonymous intermediate."""
+    a = sg.sg_vec_create(ctx, dtype, n, pa)
+    b = sg.sg_vec_create(ctx, dtype, n, pb)
+    prod = sg.sg_enqueue(ctx, sg.SG_MUL, [a, b])
+    s = sg.sg_reduce(ctx, prod, sg.SG_SUM)
+    sg.sg_release(ctx, prod)
+    return {"a": a, "b": b, "sum": s}
+
+
+def axpy(ctx, dtype, n, alpha, px, py, pout=None):
+    """aX+Y: X.multiplied_by(a).plus(Y) — one elementwise kernel with one extra scalar argument."""
+    x = sg.sg_vec_create(ctx, dtype, n, px)
+    y = sg.sg_vec_create(ctx, dtype, n, py)
+    ax = sg.sg_enqueue(ctx, sg.SG_MUL, [x, F(alpha)])
+    if pout is not None:
+        out = sg.sg_vec_create(ctx, dtype, n, pout)
+        r = sg.sg_enqueue(ctx, sg.SG_ADD, [ax, y], dst_or_0=out)
+    else:
+        r = sg.sg_enqueue(ctx, sg.SG_ADD, [ax, y])
+    sg.sg_release(ctx, ax)
+    return {"x": x, "y": y, "out": r}
+
+
+def ge_row_op(ctx, n, prow_i, prow_step, pivot):
+    """row(i).divided_by(pivot); row(i).in_place_minus(row(step)) -> (A[i]/pivot) - A[step]."""
+    ri = sg.sg_vec_create(ctx, sg.SG_F64, n, prow_i)
+    rs = sg.sg_vec_create(ctx, sg.SG_F64, n, prow_step)
+    sg.sg_enqueue(ctx, sg.SG_DIV, [ri, F(pivot)], dst_or_0=ri)
+    sg.sg_enqueue(ctx, sg.SG_SUB, [ri, rs], dst_or_0=ri)
+    return {"row_i": ri, "row_step": rs}
+
+
+def _cfg0_chain(ctx, a, b, c, dst=0):
+    t1 = sg.sg_enqueue(ctx, sg.SG_ADD, [a, b])
+    t2 = sg.sg_enqueue(ctx, sg.SG_MUL, [t1, F(2.5)])
+    z = sg.sg_enqueue(ctx, sg.SG_SUB, [t2, c], dst_or_0=dst)
+    sg.sg_release(ctx, t1)
+    sg.sg_release(ctx, t2)
+    return z
+
+
+def cfg0(ctx, n, pa, pb, pc, pz=None, keep_z=True, contracts=True):
+    """BASELINE.json:configs[0]: z = (a+b)*2.5 - c; sum/max/min(z); pre exists(a>0.99); post for_all(z == recomputed).
+
+    keep_z=True  (plan P2): z is a named result -> stored by pass A; the postcondition re-reads it in pass B.
+    keep_z=False (plan P1): z is released -> everything is one pass over a, b, c.
+    """
+    a = sg.sg_vec_create(ctx, sg.SG_F64, n, pa)
+    b = sg.sg_vec_create(ctx, sg.SG_F64, n, pb)
+    c = sg.sg_vec_create(ctx, sg.SG_F64, n, pc)
+    res = {"a": a, "b": b, "c": c}
+    if contracts:
+        m = sg.sg_enqueue(ctx, sg.SG_GT, [a, F(0.99)])
+        res["pre"] = sg.sg_exists(ctx, m)
+        sg.sg_release(ctx, m)
+        sg.sg_contract(ctx, res["pre"], sg.SG_CONTRACT_PRE, "exists(a_i > 0.99)")
+    dst = sg.sg_vec_create(ctx, sg.SG_F64, n, pz) if (keep_z and pz is not None) else 0
+    z = _cfg0_chain(ctx, a, b, c, dst)
+    res["z"] = z
+    res["sum"] = sg.sg_reduce(ctx, z, sg.SG_SUM)
+    res["max"] = sg.sg_reduce(ctx, z, sg.SG_RMAX)
+    res["min"] = sg.sg_reduce(ctx, z, sg.SG_RMIN)
+    if contracts:
+        z2 = _cfg0_chain(ctx, a, b, c)
+        eq = sg.sg_enqueue(ctx, sg.SG_EQ, [z, z2])
+        res["post"] = sg.sg_forall(ctx, eq)
+        sg.sg_release(ctx, z2)
+        sg.sg_release(ctx, eq)
+        sg.sg_contract(ctx, res["post"], sg.SG_CONTRACT_POST, "for_all(z_i == (a_i+b_i)*2.5-c_i)")
+    if not keep_z:
+        sg.sg_release(ctx, z)
+        res.pop("z")
+    return res
+
+
+def cfg1_chain(ctx, x, y):
+    """w = abs(x*y + 0.5) - min(x,y)*3 + x/(1+y*y), ten primitives, left to right (BASELINE.json:configs[1])."""
+    t1 = sg.sg_enqueue(ctx, sg.SG_MUL, [x, y])
+    t2 = sg.sg_enqueue(ctx, sg.SG_ADD, [t1, F(0.5)])
+    t3 = sg.sg_enqueue(ctx, sg.SG_ABS, [t2])
+    t4 = sg.sg_enqueue(ctx, sg.SG_MIN, [x, y])
+    t5 = sg.sg_enqueue(ctx, sg.SG_MUL, [t4, F(3.0)])
+    t6 = sg.sg_enqueue(ctx, sg.SG_SUB, [t3, t5])
+    t7 = sg.sg_enqueue(ctx, sg.SG_MUL, [y, y])
+    t8 = sg.sg_enqueue(ctx, sg.SG_ADD, [F(1.0), t7])
+    t9 = sg.sg_enqueue(ctx, sg.SG_DIV, [x, t8])
+    w = sg.sg_enqueue(ctx, sg.SG_ADD, [t6, t9])
+    for t in (t1, t2, t3, t4, t5, t6, t7, t8, t9):
+        sg.sg_release(ctx, t)
+    return w
+
+
+def cfg1(ctx, n, px, py, keep_w=False):
+    x = sg.sg_vec_create(ctx, sg.SG_F32, n, px)
+    y = sg.sg_vec_create(ctx, sg.SG_F32, n, py)
+    w = cfg1_chain(ctx, x, y)
+    res = {"x": x, "y": y, "sum": sg.sg_reduce(ctx, w, sg.SG_SUM), "max": sg.sg_reduce(ctx, w, sg.SG_RMAX)}
+    if keep_w:
+        res["w"] = w
+    else:
+        sg.sg_release(ctx, w)
+    return res
+
+
+def cfg2(ctx, n, px, pout=None, capacity=0, modulus=7, residue=3):
+    """BASELINE.json:configs[2]: stable filter keeping x where x mod 7 == 3, count, int64 sum of the kept values."""
+    x = sg.sg_vec_create(ctx, sg.SG_I32, n, px)
+    r = sg.sg_enqueue(ctx, sg.SG_MOD, [x, I(modulus)])
+    m = sg.sg_enqueue(ctx, sg.SG_EQ, [r, I(residue)])
+    kept, count = sg.sg_filter(ctx, x, m, pout, capacity)
+    s = sg.sg_reduce(ctx, kept, sg.SG_SUM)
+    sg.sg_release(ctx, r)
+    sg.sg_release(ctx, m)
+    return {"x": x, "kept": kept, "count": count, "sum": s}
+
+
+def cfg3(ctx, n, px, contracts=False):
+    """BASELINE.json:configs[3]: pre for_all(x_i >= 0), post is-sorted for_all(x_i <= x_{i+1})."""
+    x = sg.sg_vec_create(ctx, sg.SG_F32, n, px)
+    ge = sg.sg_enqueue(ctx, sg.SG_GE, [x, F(0.0)])
+    pre = sg.sg_forall(ctx, ge)
+    sg.sg_release(ctx, ge)
+    post = sg.sg_forall_adjacent(ctx, x, sg.SG_LE)
+    if contracts:
+        sg.sg_contract(ctx, pre, sg.SG_CONTRACT_PRE, "for_all(x_i >= 0)")
+        sg.sg_contract(ctx, post, sg.SG_CONTRACT_PRE, "is_sorted")
+    return {"x": x, "pre": pre, "post": post}
+
+
+def cfg4(ctx, n, pM, k, ld=None):
+    """BASELINE.json:configs[4]: M[j,:] -= (M[j,k]/M[k,k]) * M[k,:] for all j>k, fused with row-wise max|.| and column sums.
+
+    Pass 1 (vector): f = column(k)[k+1:] / M[k,k]  — read BEFORE the rows are modified.
+    Pass 2 (matrix): t = f (COL-broadcast) * row(k) (ROW-broadcast); rows(k+1..) -= t in place; rowmax, colsum.
+    """
+    ld = n if ld is None else ld
+    M = sg.sg_mat_create(ctx, sg.SG_F64, n, n, ld, pM)
+    res = {"M": M}
+    if k + 1 >= n:
+        return res
+    piv = sg.sg_mat_elem(ctx, M, k, k)
+    col = sg.sg_mat_col(ctx, M, k, k + 1, n)
+    f = sg.sg_enqueue(ctx, sg.SG_DIV, [col, piv])
+    rowk = sg.sg_mat_row(ctx, M, k)
+    sub = sg.sg_mat_rows(ctx, M, k + 1, n)
+    t = sg.sg_enqueue(ctx, sg.SG_MUL, [H(f, sg.SG_BCAST_COL), H(rowk, sg.SG_BCAST_ROW)])
+    sg.sg_enqueue(ctx, sg.SG_SUB, [sub, t], dst_or_0=sub)
+    ab = sg.sg_enqueue(ctx, sg.SG_ABS, [sub])
+    res["rowmax"] = sg.sg_reduce(ctx, ab, sg.SG_RMAX, sg.SG_AXIS_ROWS)
+    res["colsum"] = sg.sg_reduce(ctx, sub, sg.SG_SUM, sg.SG_AXIS_COLS)
+    for h in (col, t, ab, piv, f):
+        sg.sg_release(ctx, h)
+    res["sub"] = sub
+    return res
