@@ -126,7 +126,7 @@ def time_replay(sg, ctx, reps):
     return sg.sg_replay_last(ctx, reps)
 
 
-def per_config(torch, sg, W, inputs, peak, quick):
+def per_config(torch, sg, W, inputs, peak, which):
     """Device time per flush (library CUDA events, mean of replays) for the other §8(a) rows; inputs > L2 except cfg0."""
     out = {}
     stream = torch.cuda.current_stream().cuda_stream
@@ -136,7 +136,11 @@ def per_config(torch, sg, W, inputs, peak, quick):
         sg.sg_ctx_set_flags(ctx, flags)
         try:
             build(ctx)
-            sg.sg_flush(ctx)
+            try:
+                sg.sg_flush(ctx)
+            except sg.SgError as e:         # a violated contract is the expected outcome of the injected-violation run
+                if e.status != sg.SG_ERR_CONTRACT:
+                    raise
             st = sg.sg_plan_stats(ctx)
             if restore is None:
                 sg.sg_replay_last(ctx, 3)
@@ -153,12 +157,28 @@ def per_config(torch, sg, W, inputs, peak, quick):
         finally:
             sg.sg_ctx_destroy(ctx)
 
+    if "cfg0" in which:
+        cfg0_section(torch, sg, W, inputs, measure)
+    if "cfg1" in which:
+        cfg1_section(torch, sg, W, inputs, measure)
+    if "cfg2" in which:
+        cfg2_section(torch, sg, W, inputs, measure)
+    if "cfg3" in which:
+        cfg3_section(torch, sg, W, inputs, measure)
+    if "cfg4" in which:
+        cfg4_section(torch, sg, W, inputs, measure)
+    return out
+
+
+def cfg0_section(torch, sg, W, inputs, measure):
     # config 0 (fits in L2: a warm number, labelled)
     n0 = 1 << 20
     a, b, c = (torch.from_numpy(inputs.uniform_pm1_f64(1, s, n0)).cuda() for s in range(3))
     measure("cfg0_fp64_2^20_chain_sum_max_min_contracts (L2-warm, 2 passes)", lambda ctx: W.cfg0(ctx, n0, a.data_ptr(), b.data_ptr(), c.data_ptr()), 64 << 20, 200)
     measure("cfg0_onepass (z released, L2-warm)", lambda ctx: W.cfg0(ctx, n0, a.data_ptr(), b.data_ptr(), c.data_ptr(), keep_z=False), 24 << 20, 200)
-    del a, b, c
+
+
+def cfg1_section(torch, sg, W, inputs, measure):
     # config 1 at its own size, fused and one-kernel-per-op
     n1 = 1 << 26
     x = torch.from_numpy(inputs.normal_f32(2, 0, n1)).cuda()
@@ -166,15 +186,16 @@ def per_config(torch, sg, W, inputs, peak, quick):
     measure("cfg1_fp32_2^26_fused", lambda ctx: W.cfg1(ctx, n1, x.data_ptr(), y.data_ptr()), 8 * n1)
     measure("cfg1_fp32_2^26_unfused_one_kernel_per_op", lambda ctx: W.cfg1(ctx, n1, x.data_ptr(), y.data_ptr()), 0, 5, sg.SG_FLAG_UNFUSED)
     measure("cfg1_fp32_2^26_fused_bytecode", lambda ctx: W.cfg1(ctx, n1, x.data_ptr(), y.data_ptr()), 8 * n1, 5, sg.SG_FLAG_FORCE_BYTECODE)
-    del x, y
-    if quick:
-        return out
-    # config 2
+
+
+def cfg2_section(torch, sg, W, inputs, measure):
     n2 = 1 << 27
     xi = torch.from_numpy(inputs.uniform_i31(3, 0, n2)).cuda()
     cnt = int((xi % 7 == 3).sum().item())          # only to size the algorithmic bytes of the report
     measure("cfg2_int32_2^27_filter_count_sum", lambda ctx: W.cfg2(ctx, n2, xi.data_ptr()), 4 * n2 + 4 * cnt)
-    del xi
+
+
+def cfg3_section(torch, sg, W, inputs, measure):
     # config 3, clean and with the seeded violation (early exit)
     n3 = 1 << 28
     xs_host = inputs.sorted_cumsum_f32(4, 0, n3)
@@ -182,9 +203,11 @@ def per_config(torch, sg, W, inputs, peak, quick):
     measure("cfg3_fp32_2^28_forall_ge0_and_sorted_clean", lambda ctx: W.cfg3(ctx, n3, xs.data_ptr()), 4 * n3)
     j = inputs.violation_index(4, n3)
     xs[j] = 0.5 * xs[j - 1]
-    measure(f"cfg3_fp32_2^28_violation_at_{j} (early exit; time to answer)", lambda ctx: W.cfg3(ctx, n3, xs.data_ptr()), 4 * n3)
-    del xs, xs_host
-    # config 4
+    measure(f"cfg3_fp32_2^28_violation_at_{j} (both quantifiers needed: full scan)", lambda ctx: W.cfg3(ctx, n3, xs.data_ptr()), 4 * n3)
+    measure(f"cfg3_fp32_2^28_violation_at_{j} as contracts (early exit; time to answer)", lambda ctx: W.cfg3(ctx, n3, xs.data_ptr(), contracts=True), 4 * n3)
+
+
+def cfg4_section(torch, sg, W, inputs, measure):
     n4 = 16384
     Mh = inputs.boosted_matrix_f64(5, 0, n4)
     M0 = torch.from_numpy(Mh).cuda()
@@ -194,7 +217,6 @@ def per_config(torch, sg, W, inputs, peak, quick):
         rows = n4 - k - 1
         alg = 16 * rows * n4 + 8 * n4 + 16 * rows + 8 * rows + 8 * n4
         measure(f"cfg4_fp64_16384^2_row_update_k={k}", lambda ctx: W.cfg4(ctx, n4, M.data_ptr(), k), alg, restore=lambda: M.copy_(M0))
-    return out
 
 
 def main():
@@ -204,7 +226,9 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--log2n", type=int, default=28)
     ap.add_argument("--impl", default="ours")
-    ap.add_argument("--headline-only", action="store_true")
+    ap.add_argument("--headline-only", action="store_true", help="same as --configs none")
+    ap.add_argument("--configs", default="cfg0,cfg1,cfg2,cfg3,cfg4", help="per_config sections to time after the headline (or: none)")
+    ap.add_argument("--skip-headline", action="store_true", help="profiling aid: run only the --configs sections and print their JSON")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3)
     if args.impl == "reference":
@@ -226,6 +250,10 @@ def main():
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
     peak, peak_src = peaks()
+    which = [] if (args.headline_only or args.configs == "none") else args.configs.split(",")
+    if args.skip_headline:
+        print(json.dumps({"per_config": per_config(torch, sg, W, inputs, peak, which)}))
+        return
 
     n = 1 << args.log2n
     xh = torch.from_numpy(inputs.normal_f32(2, 2 * rank, n)).pin_memory()
@@ -316,7 +344,7 @@ def main():
     del x, y
     if world == 1:
         try:
-            line["per_config"] = per_config(torch, sg, W, inputs, peak, args.headline_only)
+            line["per_config"] = per_config(torch, sg, W, inputs, peak, which)
         except Exception as e:      # the headline stands on its own; say what failed
             line["per_config_error"] = repr(e)
     if dist is not None:

@@ -266,6 +266,9 @@ sg_status sg_build_pass(sg_ctx* c, Pass& P, std::vector<char*>& temps, std::stri
             }
             a.out_len[n_out] = X.cols;
             if (X.op != OUT_ALL && X.op != OUT_ANY) only_quant = false;
+            if (X.op == OUT_ALL)
+                for (const Contract& k : c->contracts)
+                    if (k.value == X.out) a.exit_any |= 1u << n_out;
             ++n_out;
         } else {    // NK_FILTER
             if (n_out >= SG_MAX_OUT) return sg_fail(c, SG_ERR_CAPACITY, "too many outputs in one pass");
@@ -298,6 +301,11 @@ sg_status sg_build_pass(sg_ctx* c, Pass& P, std::vector<char*>& temps, std::stri
         a.in_stride[k] = in.stride;
         a.in_len[k] = in.len;
         a.imm[k] = in.imm;
+        if (in.kind == IN_IMM && dtype == SG_I32) {
+            int32_t d; memcpy(&d, &in.imm, 4);
+            const uint64_t ad = d < 0 ? (uint64_t)(-(int64_t)d) : (uint64_t)d;
+            a.imm_magic[k] = ad > 1 ? (UINT64_MAX / ad + 1) : 0;
+        }
         // an input whose storage this pass also writes must not go through the read-only path
         if (in.ptr)
             for (int o = 0; o < n_out; ++o)

@@ -76,6 +76,22 @@ __device__ __forceinline__ int32_t p_abs(int32_t a) { return a < 0 ? (int32_t)(0
 __device__ __forceinline__ long long p_neg(long long a) { return (long long)(0ull - (unsigned long long)a); }
 __device__ __forceinline__ long long p_abs(long long a) { return a < 0 ? (long long)(0ull - (unsigned long long)a) : a; }
 
+// int32 division / modulo by a pass-constant divisor d (|d| > 1) with the precomputed magic M = ceil(2^64/|d|):
+// q = floor(|x| / |d|) = mulhi64(M, |x|) exactly for every 32-bit |x| (64 fractional bits >= 32 + log2 |d|).
+// C semantics: the quotient truncates toward zero, the remainder has the sign of the dividend.
+__device__ __forceinline__ int32_t fast_mod_i32(int32_t x, int32_t d, unsigned long long M) {
+    const uint32_t ad = d < 0 ? 0u - (uint32_t)d : (uint32_t)d;
+    const uint32_t ax = x < 0 ? 0u - (uint32_t)x : (uint32_t)x;
+    const uint32_t q = (uint32_t)__umul64hi(M, (unsigned long long)ax);
+    const uint32_t r = ax - q * ad;
+    return x < 0 ? (int32_t)(0u - r) : (int32_t)r;
+}
+__device__ __forceinline__ int32_t fast_div_i32(int32_t x, int32_t d, unsigned long long M) {
+    const uint32_t ax = x < 0 ? 0u - (uint32_t)x : (uint32_t)x;
+    const uint32_t q = (uint32_t)__umul64hi(M, (unsigned long long)ax);
+    return ((x < 0) != (d < 0)) ? (int32_t)(0u - q) : (int32_t)q;
+}
+
 // one value op; `op` is a compile-time constant in template instances and a warp-uniform value in the bytecode kernel
 template <class T> __device__ __forceinline__ T value_op(uint8_t op, T a, T b) {
     switch (op) {
@@ -229,6 +245,14 @@ __device__ __forceinline__ Cell cell_shfl_xor(const Cell& c, int m) {
     Cell r;
     r.a = __shfl_xor_sync(0xffffffffu, c.a, m);
     r.b = __shfl_xor_sync(0xffffffffu, c.b, m);
+    return r;
+}
+
+// shuffle only the words the output kind uses (a double-double sum needs both, everything else only `a`)
+template <class T> __device__ __forceinline__ Cell cell_shfl_xor_kind(uint8_t kind, const Cell& c, int m) {
+    Cell r;
+    r.a = __shfl_xor_sync(0xffffffffu, c.a, m);
+    r.b = (kind == OUT_SUM && Traits<T>::is_float && sizeof(T) == 8) ? __shfl_xor_sync(0xffffffffu, c.b, m) : 0ull;
     return r;
 }
 

@@ -89,7 +89,7 @@ template <class P> struct FilterTemplateEval {
         T v[M::NV][FW];
         bool p[M::NP][FW];
         (load_k<K>(v, p, a, i, full), ...);
-        exec_body<P, T, M::NV, M::NP, FW>(v, p, is);
+        exec_body<P, T, M::NV, M::NP, FW>(v, p, a, is);
         keep = 0;
         (out_o<O>(v, p, a, i, val, keep, acc), ...);
     }
@@ -137,13 +137,17 @@ template <class TT> struct FilterBytecodeEval {
 };
 
 // ---- the kernel body -------------------------------------------------------------------------------------
+// Per tile: evaluate -> ballot ranks -> barrier -> scatter kept items into a shared-memory tile (tile-local order)
+// while warp 0 runs the look-back -> barrier -> coalesced copy of the compacted tile to its global position.
+// The id of the next tile is fetched (atomicAdd) at the start of the current one, so its latency is hidden.
 template <class EV>
 __device__ __forceinline__ void filter_body(const SgProg* g, const SgArgs& a) {
     typedef typename EV::T T;
     constexpr int U = EV::U, FW = EV::FW;
     constexpr int TILE = BLOCK * U * FW;
     constexpr int NOUT = EV::NOUT;
-    __shared__ int s_tile;
+    __shared__ T s_vals[TILE];
+    __shared__ int s_tile[2];
     __shared__ unsigned int s_warp_total[WARPS];
     __shared__ unsigned long long s_tile_excl;
 
@@ -166,12 +170,13 @@ __device__ __forceinline__ void filter_body(const SgProg* g, const SgArgs& a) {
 
     if (a.n_tiles == 0 && blockIdx.x == 0 && threadIdx.x == 0) *reinterpret_cast<long long*>(a.out_aux[fo]) = 0;
 
-    for (;;) {
-        __syncthreads();                                    // previous iteration's shared values fully consumed
-        if (threadIdx.x == 0) s_tile = (int)atomicAdd(&a.ctrl[2], 1u);
-        __syncthreads();
-        const int tile = s_tile;
+    if (threadIdx.x == 0) s_tile[0] = (int)atomicAdd(&a.ctrl[2], 1u);
+    __syncthreads();
+    for (int it = 0;; ++it) {
+        const int tile = s_tile[it & 1];
         if (tile >= a.n_tiles) break;
+        int next_tile = 0;
+        if (threadIdx.x == 0) next_tile = (int)atomicAdd(&a.ctrl[2], 1u);      // consumed just before the first barrier
         const int64_t tbase = (int64_t)tile * TILE;
         const bool full = all_vec && (tbase + TILE <= a.n);
 
@@ -192,6 +197,7 @@ __device__ __forceinline__ void filter_body(const SgProg* g, const SgArgs& a) {
             running += __popc(b0) + 2 * __popc(b1) + 4 * __popc(b2);
         }
         if (lane == 0) s_warp_total[warp] = running;
+        if (threadIdx.x == 0) s_tile[(it + 1) & 1] = next_tile;
         __syncthreads();
         unsigned int warp_excl = 0, tile_total = 0;
 #pragma unroll
@@ -200,7 +206,14 @@ __device__ __forceinline__ void filter_body(const SgProg* g, const SgArgs& a) {
             if (w < warp) warp_excl += t;
             tile_total += t;
         }
-        // decoupled look-back by warp 0
+#pragma unroll
+        for (int u = 0; u < U; ++u) {
+            unsigned int pos = warp_excl + off[u];
+#pragma unroll
+            for (int e = 0; e < FW; ++e)
+                if ((keep[u] >> e) & 1u) s_vals[pos++] = val[u][e];
+        }
+        // decoupled look-back by warp 0 (the other warps are already at the barrier below)
         if (warp == 0) {
             unsigned long long excl = 0;
             if (tile == 0) {
@@ -238,20 +251,14 @@ __device__ __forceinline__ void filter_body(const SgProg* g, const SgArgs& a) {
             }
         }
         __syncthreads();
-        const long long pos0 = (long long)s_tile_excl + warp_excl;
+        const long long tile_excl = (long long)s_tile_excl;
         bool overflow = false;
-#pragma unroll
-        for (int u = 0; u < U; ++u) {
-            long long pos = pos0 + off[u];
-#pragma unroll
-            for (int e = 0; e < FW; ++e) {
-                if ((keep[u] >> e) & 1u) {
-                    if (pos < cap) dst[pos] = val[u][e]; else overflow = true;
-                    ++pos;
-                }
-            }
+        for (unsigned int i = threadIdx.x; i < tile_total; i += BLOCK) {
+            const long long pos = tile_excl + i;
+            if (pos < cap) dst[pos] = s_vals[i]; else overflow = true;
         }
         if (overflow) a.ctrl[3] = 1u;
+        // no third barrier: the next tile's first barrier separates this copy-out from the next scatter
     }
     epilogue_1d<T, NOUT>(acc, kind, a, true);
 }

@@ -16,6 +16,9 @@ namespace {
 using namespace sgk;
 
 typedef cudaError_t (*LaunchFn)(const SgArgs&, int grid, cudaStream_t);
+template <class P> constexpr size_t smem_of() {
+    if constexpr ((P::prog.shape.flags & PF_2D) != 0) return sgk::Meta2D<P>::SMEM; else return 0;
+}
 typedef int (*OccFn)();
 
 struct Entry {
@@ -32,7 +35,11 @@ template <class P> constexpr int tile_of() {
 }
 
 template <class P> cudaError_t launch_template(const SgArgs& a, int grid, cudaStream_t s) {
-    if constexpr ((P::prog.shape.flags & PF_2D) != 0) pass2d_template<P><<<grid, BLOCK, 0, s>>>(a);
+    if constexpr ((P::prog.shape.flags & PF_2D) != 0) {
+        static bool attr_set = false;
+        if (!attr_set) { cudaFuncSetAttribute(pass2d_template<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_of<P>()); attr_set = true; }
+        pass2d_template<P><<<grid, BLOCK, smem_of<P>(), s>>>(a);
+    }
     else if constexpr ((P::prog.shape.flags & PF_FILTER) != 0) filter1d_template<P><<<grid, BLOCK, 0, s>>>(a);
     else pass1d_template<P><<<grid, BLOCK, 0, s>>>(a);
     return cudaGetLastError();
@@ -40,7 +47,10 @@ template <class P> cudaError_t launch_template(const SgArgs& a, int grid, cudaSt
 template <class P> int occupancy_template() {
     int occ = 0;
     cudaError_t e;
-    if constexpr ((P::prog.shape.flags & PF_2D) != 0) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, pass2d_template<P>, BLOCK, 0);
+    if constexpr ((P::prog.shape.flags & PF_2D) != 0) {
+        cudaFuncSetAttribute(pass2d_template<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_of<P>());
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, pass2d_template<P>, BLOCK, smem_of<P>());
+    }
     else if constexpr ((P::prog.shape.flags & PF_FILTER) != 0) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, filter1d_template<P>, BLOCK, 0);
     else e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, pass1d_template<P>, BLOCK, 0);
     return (e == cudaSuccess && occ > 0) ? occ : 1;
@@ -52,7 +62,7 @@ template <class P> int occupancy_template() {
 #define SG_TEMPLATE(NAME, UNROLL, MINB, ROWU, ...)                                   \
     struct T_##NAME {                                                                \
         static constexpr SgProg prog = __VA_ARGS__;                                  \
-        static constexpr int unroll = UNROLL, min_blocks = MINB, row_unroll = ROWU;  \
+        static constexpr int unroll = UNROLL, min_blocks = MINB, row_unroll = ROWU, stages = 3;  \
     };
 #include "sg_templates_gen.inc"
 #undef SG_TEMPLATE

@@ -23,9 +23,29 @@ template <class P> struct Meta1D {
 };
 
 // ---- compile-time body: one fold over the instruction list, every register index is a constant --------
+// index of the IN_IMM input that lives in V register `reg`, or -1 (input registers are never recycled)
+template <class P> __host__ __device__ constexpr int imm_input_of_reg(int reg) {
+    for (int k = 0; k < P::prog.shape.n_in; ++k)
+        if (P::prog.in[k].kind == IN_IMM && P::prog.in[k].reg == reg) return k;
+    return -1;
+}
+
 template <class P, class T, int NV, int NP, int E, int I>
-__device__ __forceinline__ void exec_instr(T (&v)[NV][E], bool (&p)[NP][E]) {
+__device__ __forceinline__ void exec_instr(T (&v)[NV][E], bool (&p)[NP][E], const SgArgs& a) {
     constexpr SgInstr ins = P::prog.code[I];
+    constexpr int immk = (ins.op == OP_MOD || ins.op == OP_DIV) ? imm_input_of_reg<P>(ins.b) : -1;
+    if constexpr (immk >= 0 && sizeof(T) == 4 && !Traits<T>::is_float) {
+        // x MOD d / x DIV d with an immediate divisor: multiply by the host-computed magic instead of dividing
+        const unsigned long long magic = a.imm_magic[immk];
+        int32_t d;
+        memcpy(&d, &a.imm[immk], 4);
+        if (magic != 0) {       // |d| > 1 (uniform)
+#pragma unroll
+            for (int e = 0; e < E; ++e)
+                v[ins.dst][e] = (T)(ins.op == OP_MOD ? fast_mod_i32((int32_t)v[ins.a][e], d, magic) : fast_div_i32((int32_t)v[ins.a][e], d, magic));
+            return;
+        }
+    }
 #pragma unroll
     for (int e = 0; e < E; ++e) {
         if constexpr (op_is_value(ins.op)) v[ins.dst][e] = value_op<T>(ins.op, v[ins.a][e], v[ins.b][e]);
@@ -34,8 +54,8 @@ __device__ __forceinline__ void exec_instr(T (&v)[NV][E], bool (&p)[NP][E]) {
     }
 }
 template <class P, class T, int NV, int NP, int E, int... I>
-__device__ __forceinline__ void exec_body(T (&v)[NV][E], bool (&p)[NP][E], std::integer_sequence<int, I...>) {
-    (exec_instr<P, T, NV, NP, E, I>(v, p), ...);
+__device__ __forceinline__ void exec_body(T (&v)[NV][E], bool (&p)[NP][E], const SgArgs& a, std::integer_sequence<int, I...>) {
+    (exec_instr<P, T, NV, NP, E, I>(v, p, a), ...);
 }
 
 // ---- inputs of one full tile ---------------------------------------------------------------------------
@@ -181,7 +201,7 @@ __device__ __forceinline__ void ragged_range(Cell (&acc)[Meta1D<P>::NOUT], const
     bcast_inputs<P, 1>(v, a, ks);
     for (int64_t i = lo + start; i < hi; i += step) {
         (load_input_one<P, K>(v, p, a, i), ...);
-        exec_body<P, typename M::T, M::NV, M::NP, 1>(v, p, is);
+        exec_body<P, typename M::T, M::NV, M::NP, 1>(v, p, a, is);
         (emit_output_one<P, O>(v, p, acc, a, i), ...);
     }
 }
@@ -216,12 +236,15 @@ __global__ void __launch_bounds__(BLOCK, P::min_blocks) pass1d_template(const __
         bool p[M::NP][M::E];
         bcast_inputs<P, M::E>(v, a, KS);
         for (int64_t tile = blockIdx.x; tile < a.n_full_tiles; tile += gridDim.x) {
+            // the decided word is requested together with the tile's loads and examined after the tile is processed,
+            // so the poll costs no extra round trip on the clean path
+            unsigned int decided_word = 0;
             if constexpr (M::early_exit) {
-                if (!a.no_early_exit && ld_volatile_u32(&a.ctrl[1]) == need_mask) break;
+                if (!a.no_early_exit) decided_word = ld_volatile_u32(&a.ctrl[1]);
             }
             const int64_t base = a.head + tile * M::TILE;
             load_inputs_full<P>(v, p, a, base, KS);
-            exec_body<P, T, M::NV, M::NP, M::E>(v, p, IS);
+            exec_body<P, T, M::NV, M::NP, M::E>(v, p, a, IS);
             emit_outputs_full<P>(v, p, acc, a, base, OS);
             if constexpr (M::early_exit) {
 #pragma unroll
@@ -232,6 +255,7 @@ __global__ void __launch_bounds__(BLOCK, P::min_blocks) pass1d_template(const __
                         if ((threadIdx.x & 31) == 0) atomicOr(&a.ctrl[1], 1u << o);
                     }
                 }
+                if ((decided_word & need_mask) == need_mask || (decided_word & a.exit_any) != 0) break;
             }
         }
     }

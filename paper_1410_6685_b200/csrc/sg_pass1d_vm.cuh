@@ -190,7 +190,10 @@ __global__ void __launch_bounds__(BLOCK) pass1d_bytecode(const __grid_constant__
     const int64_t n_tiles = (body + VM_TILE - 1) / VM_TILE;
     const int64_t head_tiles = (a.head + VM_TILE - 1) / VM_TILE;
     for (int64_t tile = blockIdx.x; tile < n_tiles + head_tiles; tile += gridDim.x) {
-        if (early_exit && ld_volatile_u32(&a.ctrl[1]) == need_mask) break;
+        if (early_exit) {
+            const unsigned int w = ld_volatile_u32(&a.ctrl[1]);
+            if ((w & need_mask) == need_mask || (w & a.exit_any) != 0) break;
+        }
         int64_t i, hi;
         if (tile < n_tiles) { i = a.head + tile * VM_TILE + (int64_t)threadIdx.x * E; hi = a.n; }
         else { i = (tile - n_tiles) * VM_TILE + (int64_t)threadIdx.x * E; hi = a.head; }

@@ -6,12 +6,14 @@
 //
 // Tiling: block (strip s, chunk ch) owns columns [s*SW, (s+1)*SW) and rows [ch*rpc, (ch+1)*rpc).  A thread owns
 // E = U*V fixed columns (128-bit accesses) for every row of the chunk, so ROW-broadcast operands and per-column
-// accumulators live in registers for the whole chunk.  Loads of RU rows are issued before the first is used.
+// accumulators live in registers for the whole chunk.  Rows are staged through shared memory: thread 0 issues one
+// bulk asynchronous copy (cp.async.bulk, the TMA engine) per row, NS stages of RU rows ahead of the consumers.
 // Per-column partials are combined over chunks by the last block of the strip, per-row partials over strips by
 // the last block of the chunk, both in fixed order (deterministic; no floating-point atomics).
 #ifndef SG_PASS2D_CUH_
 #define SG_PASS2D_CUH_
 
+#include "sg_bulk.cuh"
 #include "sg_pass1d_tmpl.cuh"
 
 namespace sgk {
@@ -41,7 +43,10 @@ template <class P> struct Meta2D : Meta1D<P> {
         for (int k = 0; k < B::S.n_in; ++k) n += (P::prog.in[k].kind == kind);
         return n;
     }
-    static constexpr int NVECIN = count_kind(IN_VEC) > 0 ? count_kind(IN_VEC) : 1;
+    static constexpr int NVECINREAL = count_kind(IN_VEC);
+    static constexpr int NVECIN = NVECINREAL > 0 ? NVECINREAL : 1;
+    static constexpr int NS = P::stages;            // shared-memory stages in flight
+    static constexpr size_t SMEM = (size_t)NS * NVECIN * RU * SW * sizeof(typename B::T) + NS * sizeof(uint64_t);
     static constexpr int vec_slot(int K) {
         int n = 0;
         for (int k = 0; k < K; ++k) n += (P::prog.in[k].kind == IN_VEC);
@@ -128,89 +133,107 @@ __global__ void __launch_bounds__(BLOCK, P::min_blocks) pass2d_template(const __
         }
     }
 
-    for (int64_t rb = r_begin; rb < r_end; rb += RB) {
-        const int64_t rb_end = (rb + RB < r_end) ? rb + RB : r_end;
-        for (int64_t r0 = rb; r0 < rb_end; r0 += RU) {
-            VEC ld[M::NVECIN][RU][U];
+    // ---- staged row loop: RS rows per stage, NS stages in flight (bulk copies issued by thread 0) -----------------
+    constexpr int RS = RU, NS = M::NS;
+    extern __shared__ __align__(128) unsigned char dyn_smem[];
+    T* const stage_base = reinterpret_cast<T*>(dyn_smem);
+    uint64_t* const full = reinterpret_cast<uint64_t*>(dyn_smem + (size_t)NS * M::NVECIN * RS * M::SW * sizeof(T));
+    const int64_t c0 = (int64_t)strip * M::SW;
+    const uint32_t row_bytes = (uint32_t)(((a.cols - c0) < M::SW ? (a.cols - c0) : M::SW) * sizeof(T));
+    const int64_t n_rows = r_end - r_begin;
+    const int64_t nb = (n_rows + RS - 1) / RS;
+    auto issue = [&](int64_t b) {
+        const int s = (int)(b % NS);
+        const int64_t r0 = r_begin + b * RS;
+        const int nr = (int)((r_end - r0) < RS ? (r_end - r0) : RS);
+        mbar_expect_tx(&full[s], (uint32_t)(nr * M::NVECINREAL) * row_bytes);
+#pragma unroll
+        for (int k = 0; k < M::S.n_in; ++k) {
+            if (g.in[k].kind != IN_VEC) continue;
+            T* dst = stage_base + ((size_t)s * M::NVECIN + slots.vec[k]) * RS * M::SW;
+            const T* src = reinterpret_cast<const T*>(a.in_ptr[k]) + r0 * a.in_stride[k] + c0;
+            for (int j = 0; j < nr; ++j) bulk_g2s(dst + (size_t)j * M::SW, src + (size_t)j * a.in_stride[k], row_bytes, &full[s]);
+        }
+    };
+    if (threadIdx.x == 0) {
+        for (int s = 0; s < NS; ++s) mbar_init(&full[s], 1);
+        mbar_fence_init();
+    }
+    __syncthreads();
+    if (threadIdx.x == 0)
+        for (int64_t b = 0; b < NS && b < nb; ++b) issue(b);
+
+    for (int64_t b = 0; b < nb; ++b) {
+        const int s = (int)(b % NS);
+        const int64_t r0 = r_begin + b * RS;
+        const int64_t rb = r_begin + (b * RS) / RB * RB;                // start of the current RB-row batch of the per-row combine
+        mbar_wait(&full[s], (uint32_t)((b / NS) & 1));
+#pragma unroll
+        for (int j = 0; j < RS; ++j) {
+            const int64_t r = r0 + j;
+            if (r >= r_end) break;
 #pragma unroll
             for (int k = 0; k < M::S.n_in; ++k) {
                 const SgIn in = g.in[k];
-                if (in.kind != IN_VEC) continue;
-                const int slot = slots.vec[k];
+                if (in.kind == IN_VEC) {
+                    const T* srow = stage_base + (((size_t)s * M::NVECIN + slots.vec[k]) * RS + j) * M::SW;
 #pragma unroll
-                for (int j = 0; j < RU; ++j) {
-                    if (r0 + j < rb_end) {
-                        const T* rowp = reinterpret_cast<const T*>(a.in_ptr[k]) + (r0 + j) * a.in_stride[k];
+                    for (int u = 0; u < U; ++u) {
+                        const VEC x = *reinterpret_cast<const VEC*>(srow + (u * BLOCK + threadIdx.x) * V);
+                        const T* xe = reinterpret_cast<const T*>(&x);
 #pragma unroll
-                        for (int u = 0; u < U; ++u)
-                            if (cvalid[u]) ld[slot][j][u] = in.pad ? ld_stream_rw(reinterpret_cast<const VEC*>(rowp + col[u]))
-                                                                   : ld_stream(reinterpret_cast<const VEC*>(rowp + col[u]));
+                        for (int e = 0; e < V; ++e) v[in.reg][u * V + e] = xe[e];
                     }
+                } else if (in.kind == IN_COLB) {
+                    const T sc = __ldg(reinterpret_cast<const T*>(a.in_ptr[k]) + r);
+#pragma unroll
+                    for (int e = 0; e < E; ++e) v[in.reg][e] = sc;
                 }
             }
+            exec_body<P, T, M::NV, M::NP, E>(v, p, a, IS);
 #pragma unroll
-            for (int j = 0; j < RU; ++j) {
-                const int64_t r = r0 + j;
-                if (r >= rb_end) break;
+            for (int o = 0; o < M::S.n_out; ++o) {
+                const SgOut out = g.out[o];
+                if (out.kind == OUT_STORE) {
+                    T* rowp = reinterpret_cast<T*>(a.out_ptr[o]) + r * a.out_len[o];
 #pragma unroll
-                for (int k = 0; k < M::S.n_in; ++k) {
-                    const SgIn in = g.in[k];
-                    if (in.kind == IN_VEC) {
-                        const int slot = slots.vec[k];
+                    for (int u = 0; u < U; ++u) {
+                        if (!cvalid[u]) continue;
+                        VEC x;
+                        T* xe = reinterpret_cast<T*>(&x);
 #pragma unroll
-                        for (int u = 0; u < U; ++u) {
-                            const T* xe = reinterpret_cast<const T*>(&ld[slot][j][u]);
-#pragma unroll
-                            for (int e = 0; e < V; ++e) v[in.reg][u * V + e] = xe[e];
-                        }
-                    } else if (in.kind == IN_COLB) {
-                        const T s = __ldg(reinterpret_cast<const T*>(a.in_ptr[k]) + r);
-#pragma unroll
-                        for (int e = 0; e < E; ++e) v[in.reg][e] = s;
+                        for (int e = 0; e < V; ++e) xe[e] = v[out.src][u * V + e];
+                        st_stream(reinterpret_cast<VEC*>(rowp + col[u]), x);
                     }
-                }
-                exec_body<P, T, M::NV, M::NP, E>(v, p, IS);
+                } else if (out_is_reduction(out.kind)) {
+                    Cell rowc = cell_identity<T>(out.kind);
 #pragma unroll
-                for (int o = 0; o < M::S.n_out; ++o) {
-                    const SgOut out = g.out[o];
-                    if (out.kind == OUT_STORE) {
-                        T* rowp = reinterpret_cast<T*>(a.out_ptr[o]) + r * a.out_len[o];
+                    for (int u = 0; u < U; ++u) {
+                        if (!cvalid[u]) continue;
 #pragma unroll
-                        for (int u = 0; u < U; ++u) {
-                            if (!cvalid[u]) continue;
-                            VEC x;
-                            T* xe = reinterpret_cast<T*>(&x);
-#pragma unroll
-                            for (int e = 0; e < V; ++e) xe[e] = v[out.src][u * V + e];
-                            st_stream(reinterpret_cast<VEC*>(rowp + col[u]), x);
+                        for (int e = 0; e < V; ++e) {
+                            const int ee = u * V + e;
+                            Cell& dstc = (out.axis == AXIS_ALL) ? acc[o] : (out.axis == AXIS_COLS) ? acc_col[o][ee] : rowc;
+                            if (out_is_pred_reduction(out.kind)) cell_accum_pred(out.kind, dstc, p[out.src][ee]);
+                            else if (out.pred == SG_NO_PRED || p[out.pred == SG_NO_PRED ? 0 : out.pred][ee]) cell_accum_value<T>(out.kind, dstc, v[out.src][ee]);
                         }
-                    } else if (out_is_reduction(out.kind)) {
-                        Cell rowc = cell_identity<T>(out.kind);
+                    }
+                    if (out.axis == AXIS_ROWS) {
 #pragma unroll
-                        for (int u = 0; u < U; ++u) {
-                            if (!cvalid[u]) continue;
-#pragma unroll
-                            for (int e = 0; e < V; ++e) {
-                                const int ee = u * V + e;
-                                Cell& dstc = (out.axis == AXIS_ALL) ? acc[o] : (out.axis == AXIS_COLS) ? acc_col[o][ee] : rowc;
-                                if (out_is_pred_reduction(out.kind)) cell_accum_pred(out.kind, dstc, p[out.src][ee]);
-                                else if (out.pred == SG_NO_PRED || p[out.pred == SG_NO_PRED ? 0 : out.pred][ee]) cell_accum_value<T>(out.kind, dstc, v[out.src][ee]);
-                            }
+                        for (int d = 16; d >= 1; d >>= 1) {
+                            Cell other = cell_shfl_xor_kind<T>(out.kind, rowc, d);
+                            cell_combine<T>(out.kind, rowc, other);
                         }
-                        if (out.axis == AXIS_ROWS) {
-#pragma unroll
-                            for (int d = 16; d >= 1; d >>= 1) {
-                                Cell other = cell_shfl_xor(rowc, d);
-                                cell_combine<T>(out.kind, rowc, other);
-                            }
-                            if (lane == 0) s_row[slots.row[o]][warp][(int)(r - rb)] = rowc;
-                        }
+                        if (lane == 0) s_row[slots.row[o]][warp][(int)(r - rb)] = rowc;
                     }
                 }
             }
         }
-        if (M::HAS_ROWS) {
-            __syncthreads();
+        __syncthreads();                        // every thread is done with stage s (and with this batch's s_row writes)
+        if (threadIdx.x == 0 && b + NS < nb) { fence_proxy_async(); issue(b + NS); }
+        const int64_t done_rows = (b + 1) * RS < n_rows ? (b + 1) * RS : n_rows;
+        if (M::HAS_ROWS && (done_rows % RB == 0 || done_rows == n_rows)) {
+            const int64_t rb_end = r_begin + done_rows;
             if ((int64_t)threadIdx.x < rb_end - rb) {
 #pragma unroll
                 for (int o = 0; o < M::S.n_out; ++o) {

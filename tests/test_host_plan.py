@@ -1,0 +1,217 @@
+"""Host-side tests (no GPU): the C-ABI library loads and exports every symbol include/sg.h declares, the
+scalar contracts are checked at enqueue, and the plan builder produces the plans the paper describes
+(PAPER.md:284 deferred execution, :301-309 merged kernels, :315-322 fused row operation).  Plan-only contexts
+(device -1) build plans without touching CUDA."""
+import ctypes
+import os
+import re
+import subprocess
+import sys
+
+import pytest
+
+from paper_1410_6685_b200 import sg
+from paper_1410_6685_b200 import workloads as W
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+@pytest.fixture(scope="module", autouse=True)
+def built():
+    from paper_1410_6685_b200 import build
+    build.build()
+
+
+def plan(builder, flags=0):
+    ctx = sg.sg_ctx_create(-1)
+    sg.sg_ctx_set_flags(ctx, flags)
+    try:
+        builder(ctx)
+        sg.sg_flush(ctx)
+        st = sg.sg_plan_stats(ctx)
+        dumps = [sg.sg_plan_dump(ctx, p) for p in range(st.n_passes)]
+        return st, dumps
+    finally:
+        sg.sg_ctx_destroy(ctx)
+
+
+def test_library_exports_every_declared_symbol():
+    header = open(os.path.join(ROOT, "include", "sg.h")).read()
+    header = re.sub(r"/\*.*?\*/", "", header, flags=re.S)          # prototypes only, not names mentioned in comments
+    declared = set(re.findall(r"\b(sg_[a-z0-9_]+)\s*\(", header))
+    assert len(declared) >= 30
+    lib = ctypes.CDLL(sg.lib_path())
+    for name in sorted(declared):
+        assert hasattr(lib, name), name
+    assert declared == set(sg.EXPORTS)                               # the binding has the same names
+    for name in sg.EXPORTS:
+        assert callable(getattr(sg, name)), name
+    assert "sm_100a" in sg.sg_version()
+
+
+def test_kernels_are_compiled_for_sm_100a_only():
+    out = subprocess.run(["cuobjdump", "--list-elf", sg.lib_path()], capture_output=True, text=True).stdout
+    archs = set(re.findall(r"sm_\d+a?", out))
+    assert archs == {"sm_100a"}, archs
+
+
+def test_no_device_means_failure_not_fallback():
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a GPU is present")
+    with pytest.raises(sg.SgError) as ei:
+        sg.sg_ctx_create(0)
+    assert ei.value.status == sg.SG_ERR_CUDA
+
+
+def test_template_registry_is_current():
+    assert sg.sg_template_count() >= 25
+    rc = subprocess.run([sys.executable, "-m", "paper_1410_6685_b200.gen_templates", "--check"], cwd=ROOT).returncode
+    assert rc == 0
+
+
+def test_nothing_runs_before_a_trigger():
+    # a call is added to the pending list; update / a scalar read / to_array trigger execution
+    ctx = sg.sg_ctx_create(-1)
+    r = W.dot_product(ctx, sg.SG_F64, 1000, None, None)
+    assert sg.sg_plan_stats(ctx).n_passes == 0 and sg.sg_plan_stats(ctx).launches_total == 0
+    sg.sg_scalar_get(ctx, r["sum"])                                  # trigger (1)
+    st = sg.sg_plan_stats(ctx)
+    assert st.n_passes == 1 and st.n_nodes == 2
+    sg.sg_flush(ctx)                                                 # nothing pending: no new plan
+    assert sg.sg_plan_stats(ctx).n_passes == 1
+    sg.sg_ctx_destroy(ctx)
+
+
+def test_dot_product_two_kernels_become_one():
+    # Figure 2: cmult and sum are merged; the product is never materialised
+    st, dumps = plan(lambda c: W.dot_product(c, sg.SG_F64, 1 << 20, None, None))
+    assert st.n_passes == 1 and st.pass_n_in[0] == 2 and st.pass_n_instr[0] == 1 and st.pass_n_out[0] == 1
+    assert "OUT_STORE" not in dumps[0] and "OP_MUL" in dumps[0] and "OUT_SUM" in dumps[0]
+    assert st.bytes_min == 2 * 8 * (1 << 20)
+    stu, _ = plan(lambda c: W.dot_product(c, sg.SG_F64, 1 << 20, None, None), sg.SG_FLAG_UNFUSED)
+    assert stu.n_passes == 2 and stu.bytes_min == 4 * 8 * (1 << 20)   # a*b stored, then read again
+
+
+def test_axpy_is_one_kernel_with_one_more_argument():
+    # Figure 3: X[i]+Y[i] becomes a*X[i]+Y[i]; the scalar is one extra kernel argument
+    st_add, _ = plan(lambda c: sg.sg_enqueue(c, sg.SG_ADD, [sg.sg_vec_create(c, sg.SG_F64, 100, None), sg.sg_vec_create(c, sg.SG_F64, 100, None)]))
+    st_axpy, dumps = plan(lambda c: W.axpy(c, sg.SG_F64, 100, 2.0, None, None))
+    assert st_add.n_passes == st_axpy.n_passes == 1
+    assert st_axpy.pass_n_args[0] == st_add.pass_n_args[0] + 1
+    assert st_axpy.pass_n_instr[0] == 2 and "IN_IMM" in dumps[0]
+
+
+def test_row_divide_then_subtract_is_one_expression():
+    # row(i).divided_by(pivot); row(i).in_place_minus(row(step)) -> (A[i]/pivot) - A[step]
+    st, dumps = plan(lambda c: W.ge_row_op(c, 4096, None, None, 3.0))
+    assert st.n_passes == 1 and st.pass_n_instr[0] == 2 and st.pass_n_out[0] == 1
+    assert dumps[0].count("OUT_STORE") == 1 and "OP_DIV" in dumps[0] and "OP_SUB" in dumps[0]
+    assert st.bytes_min == 3 * 8 * 4096                              # read row i, read row step, write row i
+
+
+def test_cfg0_plans():
+    n = 1 << 20
+    st, dumps = plan(lambda c: W.cfg0(c, n, None, None, None))          # P2: z stored, postcondition re-reads it
+    assert st.n_passes == 2 and st.n_template == 2
+    assert st.pass_n_in[0] == 3 and st.pass_n_out[0] == 5 and dumps[0].count("OUT_STORE") == 1
+    assert st.pass_n_in[1] == 4 and st.pass_n_out[1] == 1 and "OUT_ALL" in dumps[1]
+    assert st.bytes_min == (4 + 4) * 8 * n                           # pass A 3R+1W, pass B 4R
+    st, dumps = plan(lambda c: W.cfg0(c, n, None, None, None, keep_z=False))   # P1: everything in one pass
+    assert st.n_passes == 1 and st.bytes_min == 3 * 8 * n and "OUT_STORE" not in dumps[0]
+
+
+def test_cfg1_to_cfg4_plans():
+    st, dumps = plan(lambda c: W.cfg1(c, 1 << 26, None, None))
+    assert st.n_passes == 1 and st.pass_n_instr[0] == 10 and st.pass_n_out[0] == 2 and st.bytes_min == 8 << 26 and st.n_template == 1
+    stu, _ = plan(lambda c: W.cfg1(c, 1 << 26, None, None), sg.SG_FLAG_UNFUSED)
+    assert stu.n_passes == 12 and stu.bytes_min == 27 * (4 << 26)     # 27 vector units
+    st, dumps = plan(lambda c: W.cfg2(c, 1 << 27, None))
+    assert st.n_passes == 1 and "OUT_FILTER" in dumps[0] and st.n_template == 1
+    st, dumps = plan(lambda c: W.cfg3(c, 1 << 28, None))
+    assert st.n_passes == 1 and st.pass_n_in[0] == 1 and "IN_SHIFT" in dumps[0] and st.bytes_min == 4 << 28 and st.n_template == 1
+    st, dumps = plan(lambda c: W.cfg4(c, 16384, None, 0))
+    assert st.n_passes == 2 and "IN_STRIDED" in dumps[0] and "IN_COLB" in dumps[1] and "IN_ROWB" in dumps[1] and st.n_template == 2
+    rows = 16383
+    assert st.bytes_min == 8 * rows + 8 * rows + (2 * 8 * rows * 16384 + 8 * 16384 + 8 * rows) + 8 * rows + 8 * 16384
+
+
+def test_force_bytecode_and_unknown_chains_use_the_bytecode_kernel():
+    st, _ = plan(lambda c: W.cfg1(c, 1 << 20, None, None), sg.SG_FLAG_FORCE_BYTECODE)
+    assert st.n_bytecode == 1 and st.n_template == 0
+
+    def odd_chain(c):
+        a = sg.sg_vec_create(c, sg.SG_F32, 1000, None)
+        t = sg.sg_enqueue(c, sg.SG_MAX, [a, sg.F(0.25)])
+        u = sg.sg_enqueue(c, sg.SG_NEG, [t])
+        sg.sg_release(c, t)
+        return sg.sg_reduce(c, u, sg.SG_RMIN)
+    st, _ = plan(odd_chain)
+    assert st.n_passes == 1 and st.n_bytecode == 1
+
+
+def test_scalar_contracts_at_enqueue():
+    ctx = sg.sg_ctx_create(-1)
+    a = sg.sg_vec_create(ctx, sg.SG_F32, 10, None)
+    b = sg.sg_vec_create(ctx, sg.SG_F32, 11, None)
+    d = sg.sg_vec_create(ctx, sg.SG_F64, 10, None)
+    m = sg.sg_mat_create(ctx, sg.SG_F64, 4, 6, 6, None)
+    for ops, code in [([a, b], sg.SG_ERR_SHAPE), ([a, d], sg.SG_ERR_DTYPE), ([sg.F(1.0), sg.F(2.0)], sg.SG_ERR_ARG)]:
+        with pytest.raises(sg.SgError) as ei:
+            sg.sg_enqueue(ctx, sg.SG_ADD, ops)
+        assert ei.value.status == code
+    with pytest.raises(sg.SgError) as ei:
+        sg.sg_enqueue(ctx, sg.SG_AND, [a, a])                        # logic needs BOOL
+    assert ei.value.status == sg.SG_ERR_DTYPE
+    with pytest.raises(sg.SgError) as ei:
+        sg.sg_enqueue(ctx, sg.SG_MUL, [m, sg.H(d, sg.SG_BCAST_ROW)])  # ROW-broadcast length must equal columns (6)
+    assert ei.value.status == sg.SG_ERR_SHAPE
+    with pytest.raises(sg.SgError) as ei:
+        sg.sg_vec_subset(ctx, a, 3, 11)
+    assert ei.value.status == sg.SG_ERR_ARG
+    with pytest.raises(sg.SgError) as ei:
+        sg.sg_reduce(ctx, sg.sg_vec_create(ctx, sg.SG_F32, 0, None), sg.SG_RMAX)
+    assert ei.value.status == sg.SG_ERR_EMPTY
+    assert sg.sg_plan_stats(ctx).n_passes == 0                        # failed calls left the pending list unchanged
+    assert sg.sg_vec_count(ctx, a) == 10 and sg.sg_vec_count(ctx, m) == 24
+    sg.sg_ctx_destroy(ctx)
+
+
+def test_memory_hazards_order_the_passes():
+    # a read of column k must precede the in-place update of the rows it crosses (WAR through memory)
+    st, dumps = plan(lambda c: W.cfg4(c, 512, None, 3))
+    assert st.n_passes == 2 and "OUT_STORE" in dumps[0] and dumps[1].count("OUT_STORE") == 1
+
+    # a view read after an in-place write through another handle sees the new data: it lands in a later pass
+    def raw(c):
+        x = sg.sg_vec_create(c, sg.SG_F64, 1000, None)
+        y = sg.sg_vec_create(c, sg.SG_F64, 1000, None)
+        head = sg.sg_vec_subset(c, x, 0, 500)
+        sg.sg_enqueue(c, sg.SG_ADD, [x, y], dst_or_0=x)
+        return sg.sg_reduce(c, head, sg.SG_SUM)
+    st, _ = plan(raw)
+    assert st.n_passes == 2
+
+    # an in-place result may not alias a shifted view of its own destination
+    ctx = sg.sg_ctx_create(-1)
+    x = sg.sg_vec_create(ctx, sg.SG_F64, 1000, None)
+    lo, hi = sg.sg_vec_subset(ctx, x, 0, 999), sg.sg_vec_subset(ctx, x, 1, 1000)
+    sg.sg_enqueue(ctx, sg.SG_ADD, [lo, hi], dst_or_0=lo)
+    with pytest.raises(sg.SgError) as ei:
+        sg.sg_flush(ctx)
+    assert ei.value.status == sg.SG_ERR_ALIAS
+    sg.sg_ctx_destroy(ctx)
+
+
+def test_released_intermediates_are_never_materialised():
+    def chain(c, release):
+        a = sg.sg_vec_create(c, sg.SG_F32, 4096, None)
+        t = sg.sg_enqueue(c, sg.SG_MUL, [a, a])
+        u = sg.sg_enqueue(c, sg.SG_ADD, [t, sg.F(1.0)])
+        if release:
+            sg.sg_release(c, t)
+        return u
+    st_kept, d_kept = plan(lambda c: chain(c, False))
+    st_rel, d_rel = plan(lambda c: chain(c, True))
+    assert d_kept[0].count("OUT_STORE") == 2 and d_rel[0].count("OUT_STORE") == 1
+    assert st_kept.bytes_min - st_rel.bytes_min == 4 * 4096
