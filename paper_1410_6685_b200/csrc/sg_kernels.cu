@@ -17,7 +17,9 @@ using namespace sgk;
 
 typedef cudaError_t (*LaunchFn)(const SgArgs&, int grid, cudaStream_t);
 template <class P> constexpr size_t smem_of() {
-    if constexpr ((P::prog.shape.flags & PF_2D) != 0) return sgk::Meta2D<P>::SMEM; else return 0;
+    if constexpr ((P::prog.shape.flags & PF_2D) != 0) return sgk::Meta2D<P>::SMEM;
+    else if constexpr ((P::prog.shape.flags & PF_FILTER) != 0) return sgk::FilterTemplateEval<P>::SMEM;
+    else return 0;
 }
 typedef int (*OccFn)();
 
@@ -30,7 +32,7 @@ struct Entry {
 };
 
 template <class P> constexpr int tile_of() {
-    if (P::prog.shape.flags & PF_FILTER) return BLOCK * FilterTemplateEval<P>::U * FilterTemplateEval<P>::FW;
+    if (P::prog.shape.flags & PF_FILTER) return FilterTemplateEval<P>::TILE;
     return BLOCK * Meta1D<P>::E;
 }
 
@@ -40,20 +42,31 @@ template <class P> cudaError_t launch_template(const SgArgs& a, int grid, cudaSt
         if (!attr_set) { cudaFuncSetAttribute(pass2d_template<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_of<P>()); attr_set = true; }
         pass2d_template<P><<<grid, BLOCK, smem_of<P>(), s>>>(a);
     }
-    else if constexpr ((P::prog.shape.flags & PF_FILTER) != 0) filter1d_template<P><<<grid, BLOCK, 0, s>>>(a);
+    else if constexpr ((P::prog.shape.flags & PF_FILTER) != 0) {
+        static bool attr_set = false;
+        if (!attr_set) { cudaFuncSetAttribute(filter1d_template<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_of<P>()); attr_set = true; }
+        filter1d_template<P><<<grid, BLOCK, smem_of<P>(), s>>>(a);
+    }
     else pass1d_template<P><<<grid, BLOCK, 0, s>>>(a);
     return cudaGetLastError();
 }
 template <class P> int occupancy_template() {
+    static int cached = 0;      // one query per instance per process (the query costs tens of microseconds)
+    if (cached > 0) return cached;
     int occ = 0;
     cudaError_t e;
     if constexpr ((P::prog.shape.flags & PF_2D) != 0) {
         cudaFuncSetAttribute(pass2d_template<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_of<P>());
         e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, pass2d_template<P>, BLOCK, smem_of<P>());
     }
-    else if constexpr ((P::prog.shape.flags & PF_FILTER) != 0) e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, filter1d_template<P>, BLOCK, 0);
+    else if constexpr ((P::prog.shape.flags & PF_FILTER) != 0) {
+        cudaFuncSetAttribute(filter1d_template<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_of<P>());
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, filter1d_template<P>, BLOCK, smem_of<P>());
+    }
     else e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, pass1d_template<P>, BLOCK, 0);
-    return (e == cudaSuccess && occ > 0) ? occ : 1;
+    if (e != cudaSuccess || occ <= 0) return 1;
+    cached = occ;
+    return occ;
 }
 
 // Each SG_TEMPLATE(name, unroll, min_blocks, row_unroll, {program}) in the generated file defines a policy type
@@ -77,15 +90,24 @@ const Entry g_entries[] = {
 const int g_n_entries = (int)(sizeof(g_entries) / sizeof(g_entries[0]));
 
 template <class T> cudaError_t launch_bytecode_t(const SgProg& g, const SgArgs& a, int grid, cudaStream_t s) {
-    if (g.shape.flags & PF_FILTER) filter1d_bytecode<T><<<grid, BLOCK, 0, s>>>(g, a);
+    if (g.shape.flags & PF_FILTER) {
+        static bool attr_set = false;
+        if (!attr_set) { cudaFuncSetAttribute(filter1d_bytecode<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FilterBytecodeEval<T>::SMEM); attr_set = true; }
+        filter1d_bytecode<T><<<grid, BLOCK, FilterBytecodeEval<T>::SMEM, s>>>(g, a);
+    }
     else pass1d_bytecode<T><<<grid, BLOCK, 0, s>>>(g, a);
     return cudaGetLastError();
 }
 template <class T> int occupancy_bytecode_t(bool filter) {
+    static int cached[2] = {0, 0};
+    if (cached[filter] > 0) return cached[filter];
     int occ = 0;
-    cudaError_t e = filter ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, filter1d_bytecode<T>, BLOCK, 0)
+    if (filter) cudaFuncSetAttribute(filter1d_bytecode<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FilterBytecodeEval<T>::SMEM);
+    cudaError_t e = filter ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, filter1d_bytecode<T>, BLOCK, FilterBytecodeEval<T>::SMEM)
                            : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, pass1d_bytecode<T>, BLOCK, 0);
-    return (e == cudaSuccess && occ > 0) ? occ : 1;
+    if (e != cudaSuccess || occ <= 0) return 1;
+    cached[filter] = occ;
+    return occ;
 }
 int occupancy_bytecode(int dtype, bool filter) {
     switch (dtype) {
@@ -183,7 +205,12 @@ int sgk_plan(const SgProg& prog, SgArgs& a, int force_bytecode, int sm_count, in
         if (a.n >= (1ll << 40) || n_tiles > 0x7fffffffl) return fail(err, errcap, -9, "filter input too long for the tile-state word");
         a.n_tiles = (int)n_tiles;
         a.vec_ok = vec_ok | ((congruent && mis == 0) ? (1 << 31) : 0);
-        a.head = 0; a.n_full_tiles = 0;
+        // tiles that lie inside every vector operand's and every output's length take the unguarded (staged) path
+        long lmin = a.n;
+        for (int o = 0; o < prog.shape.n_out; ++o) lmin = std::min<long>(lmin, a.out_len[o]);
+        for (int k = 0; k < prog.shape.n_in; ++k)
+            if (prog.in[k].kind == IN_VEC) lmin = std::min<long>(lmin, a.in_len[k]);
+        a.head = 0; a.n_full_tiles = std::max<long>(0, lmin) / tile;
         geom->template_id = tid;
         geom->tile = tile;
         geom->grid = (int)std::max<long>(1, std::min<long>(n_tiles, (long)sm_count * occ));
