@@ -67,6 +67,30 @@ const char* dt_name(uint8_t d) {
     return d < 4 ? n[d] : "?";
 }
 
+// Signed magic number for truncating int32 division by d, |d| >= 2 (multiply-high scheme; the device side is
+// magic_div_i32 in sg_device.cuh).  Returns 0 for |d| <= 1.
+uint64_t i32_magic(int32_t d) {
+    const uint32_t two31 = 0x80000000u;
+    const uint32_t ad = d < 0 ? 0u - (uint32_t)d : (uint32_t)d;
+    if (ad <= 1) return 0;
+    const uint32_t t = two31 + ((uint32_t)d >> 31);
+    const uint32_t anc = t - 1 - t % ad;
+    int p = 31;
+    uint32_t q1 = two31 / anc, r1 = two31 - q1 * anc, q2 = two31 / ad, r2 = two31 - q2 * ad, delta;
+    do {
+        ++p;
+        q1 *= 2; r1 *= 2;
+        if (r1 >= anc) { ++q1; r1 -= anc; }
+        q2 *= 2; r2 *= 2;
+        if (r2 >= ad) { ++q2; r2 -= ad; }
+        delta = ad - r2;
+    } while (q1 < delta || (q1 == delta && r1 == 0));
+    uint32_t M = q2 + 1;
+    if (d < 0) M = 0u - M;
+    const int addsel = (d > 0 && (int32_t)M < 0) ? 1 : (d < 0 && (int32_t)M > 0) ? -1 : 0;
+    return (uint64_t)M | ((uint64_t)(uint32_t)(p - 32) << 32) | ((uint64_t)(uint32_t)(addsel + 1) << 40) | (1ull << 63);
+}
+
 std::string dump_prog(const SgProg& g) {
     char b[256];
     std::string s = "{";
@@ -303,8 +327,7 @@ sg_status sg_build_pass(sg_ctx* c, Pass& P, std::vector<char*>& temps, std::stri
         a.imm[k] = in.imm;
         if (in.kind == IN_IMM && dtype == SG_I32) {
             int32_t d; memcpy(&d, &in.imm, 4);
-            const uint64_t ad = d < 0 ? (uint64_t)(-(int64_t)d) : (uint64_t)d;
-            a.imm_magic[k] = ad > 1 ? (UINT64_MAX / ad + 1) : 0;
+            a.imm_magic[k] = i32_magic(d);
         }
         // an input whose storage this pass also writes must not go through the read-only path
         if (in.ptr)

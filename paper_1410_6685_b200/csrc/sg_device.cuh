@@ -76,20 +76,23 @@ __device__ __forceinline__ int32_t p_abs(int32_t a) { return a < 0 ? (int32_t)(0
 __device__ __forceinline__ long long p_neg(long long a) { return (long long)(0ull - (unsigned long long)a); }
 __device__ __forceinline__ long long p_abs(long long a) { return a < 0 ? (long long)(0ull - (unsigned long long)a) : a; }
 
-// int32 division / modulo by a pass-constant divisor d (|d| > 1) with the precomputed magic M = ceil(2^64/|d|):
-// q = floor(|x| / |d|) = mulhi64(M, |x|) exactly for every 32-bit |x| (64 fractional bits >= 32 + log2 |d|).
-// C semantics: the quotient truncates toward zero, the remainder has the sign of the dividend.
-__device__ __forceinline__ int32_t fast_mod_i32(int32_t x, int32_t d, unsigned long long M) {
-    const uint32_t ad = d < 0 ? 0u - (uint32_t)d : (uint32_t)d;
-    const uint32_t ax = x < 0 ? 0u - (uint32_t)x : (uint32_t)x;
-    const uint32_t q = (uint32_t)__umul64hi(M, (unsigned long long)ax);
-    const uint32_t r = ax - q * ad;
-    return x < 0 ? (int32_t)(0u - r) : (int32_t)r;
+// int32 division / modulo by a pass-constant divisor d (|d| >= 2) with a host-computed signed magic number
+// (the classic multiply-high scheme for truncating signed division): q = mulhi(x, M) (+x or -x when the sign of
+// M differs from that of d), arithmetic shift by s, plus one if negative.  Exact for every int32 x; the
+// remainder x - q*d has the sign of the dividend (C semantics).  Packed word: [31:0] M, [39:32] s,
+// [41:40] add selector + 1, bit 63 = valid (0 => |d| <= 1, the generic path runs).
+__device__ __forceinline__ int32_t magic_div_i32(int32_t x, unsigned long long mg) {
+    const int32_t M = (int32_t)(uint32_t)mg;
+    const int s = (int)((mg >> 32) & 0xffu);
+    const uint32_t addsel = (uint32_t)((int)((mg >> 40) & 3u) - 1);
+    int32_t q = __mulhi(x, M);
+    q = (int32_t)((uint32_t)q + (uint32_t)x * addsel);
+    q >>= s;
+    q += (int32_t)((uint32_t)q >> 31);
+    return q;
 }
-__device__ __forceinline__ int32_t fast_div_i32(int32_t x, int32_t d, unsigned long long M) {
-    const uint32_t ax = x < 0 ? 0u - (uint32_t)x : (uint32_t)x;
-    const uint32_t q = (uint32_t)__umul64hi(M, (unsigned long long)ax);
-    return ((x < 0) != (d < 0)) ? (int32_t)(0u - q) : (int32_t)q;
+__device__ __forceinline__ int32_t magic_mod_i32(int32_t x, int32_t d, unsigned long long mg) {
+    return (int32_t)((uint32_t)x - (uint32_t)magic_div_i32(x, mg) * (uint32_t)d);
 }
 
 // one value op; `op` is a compile-time constant in template instances and a warp-uniform value in the bytecode kernel

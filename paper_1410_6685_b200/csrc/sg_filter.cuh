@@ -124,7 +124,10 @@ template <class P> struct FilterTemplateEval {
                 if (in_range) cell_accum_pred(out.kind, acc[O], p[out.src][e]);
             } else if constexpr (out_is_reduction(out.kind)) {
                 if constexpr (out.pred == SG_NO_PRED) { if (in_range) cell_accum_value<T>(out.kind, acc[O], v[out.src][e]); }
-                else { if (in_range && p[out.pred][e]) cell_accum_value<T>(out.kind, acc[O], v[out.src][e]); }
+                else if constexpr (out.kind == OUT_SUM && !Traits<T>::is_float) {
+                    // masked integer sum as one widening multiply-add: acc += x * (0 or 1)
+                    acc[O].a += (unsigned long long)((long long)v[out.src][e] * (long long)(int)(in_range && p[out.pred][e]));
+                } else { if (in_range && p[out.pred][e]) cell_accum_value<T>(out.kind, acc[O], v[out.src][e]); }
             }
         }
     }
@@ -323,28 +326,30 @@ __device__ __forceinline__ void filter_body(const SgProg* g, const SgArgs& a) {
                 unsigned long long excl = 0;
                 if (prev_tile != 0) {
                     int look = prev_tile - 1;
-                    bool done = false;
                     for (;;) {
-                        bool stall = false;
+                        // ballots of all LB windows first (independent), then ONE position search and ONE warp sum
+                        int p_inc = LB * 32, p_inv = LB * 32;       // first inclusive prefix / first unpublished state, in (window, lane) order
 #pragma unroll
-                        for (int j = 0; j < LB; ++j) {
-                            if (done || stall) continue;        // uniform
+                        for (int j = LB - 1; j >= 0; --j) {
                             const unsigned long long w = lbw[j];
                             const bool valid = ((w & ST_FLAGS) != 0) && ((w & (0x3fffffull << 40)) == ep);
                             const bool inc = valid && ((w & ST_FLAGS) == ST_INC);
                             const unsigned int vmask = __ballot_sync(0xffffffffu, valid), imask = __ballot_sync(0xffffffffu, inc);
-                            const int first_invalid = (~vmask) ? (__ffs(~vmask) - 1) : 32;
-                            const int first_inc = imask ? (__ffs(imask) - 1) : 32;
-                            // contributing lanes: up to and including the first inclusive prefix, else every valid lane before the first invalid
-                            const int upto = (first_inc < first_invalid) ? first_inc + 1 : first_invalid;
-                            unsigned long long x = (lane < upto) ? (w & ST_VAL) : 0ull;
-#pragma unroll
-                            for (int d = 16; d >= 1; d >>= 1) x += __shfl_xor_sync(0xffffffffu, x, d);
-                            excl += x;
-                            if (first_inc < first_invalid) done = true;
-                            else { look -= first_invalid; stall = (first_invalid != 32); }   // a predecessor has not published yet: poll again from it
+                            if (imask) p_inc = 32 * j + __ffs(imask) - 1;
+                            if (~vmask) p_inv = 32 * j + __ffs(~vmask) - 1;
                         }
+                        // contributing states: up to and including the first inclusive prefix, else every state before the first unpublished one
+                        const bool done = p_inc < p_inv;
+                        const int upto = done ? p_inc + 1 : p_inv;
+                        unsigned long long x = 0;
+#pragma unroll
+                        for (int j = 0; j < LB; ++j)
+                            if (32 * j + lane < upto) x += lbw[j] & ST_VAL;
+#pragma unroll
+                        for (int d = 16; d >= 1; d >>= 1) x += __shfl_xor_sync(0xffffffffu, x, d);
+                        excl += x;
                         if (done) break;
+                        look -= upto;       // go deeper, or poll again from the predecessor that has not published yet
 #pragma unroll
                         for (int j = 0; j < LB; ++j) {
                             const int idx = look - lane - 32 * j;

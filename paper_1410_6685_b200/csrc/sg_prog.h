@@ -85,7 +85,7 @@ struct SgArgs {
     int64_t in_len[SG_MAX_IN];      // elements readable through the input (guards the ragged path)
     int64_t in_stride[SG_MAX_IN];   // IN_STRIDED: element stride; 2-D IN_VEC: leading dimension
     uint64_t imm[SG_MAX_IN];        // IN_IMM: raw bits of the immediate in the pass dtype
-    uint64_t imm_magic[SG_MAX_IN];  // IN_IMM, i32 passes: ceil(2^64/|d|) for division/modulo by the immediate (0 if |d| <= 1)
+    uint64_t imm_magic[SG_MAX_IN];  // IN_IMM, i32 passes: packed signed magic number for division/modulo by the immediate (0 if |d| <= 1), see magic_div_i32
     void* out_ptr[SG_MAX_OUT];      // STORE: buffer; reductions/quantifiers: 8-byte device scalar slot (AXIS_ALL) or vector
     int64_t out_len[SG_MAX_OUT];    // valid length of the output's source value (<= n); 2-D STORE: leading dimension
     int64_t out_cap[SG_MAX_OUT];    // FILTER: capacity in elements

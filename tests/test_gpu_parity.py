@@ -324,6 +324,28 @@ def test_cfg2(mode, n):
     assert bits_equal(kept, want["kept"])                            # stable: identical order
 
 
+@pytest.mark.parametrize("mode", ["template", "bytecode"])
+@pytest.mark.parametrize("modulus", [2, 3, 7, 10, 16, 641, 65536, 65537, 2**31 - 1, -2, -7, -641, -2**31, 1, -1])
+def test_filter_mod_by_any_immediate_divisor(mode, modulus):
+    """The template path divides by a pass-constant with a host-computed signed magic number: every divisor class
+    (powers of two, negative, +-1, INT_MIN) and dividends incl. negatives and INT_MIN/INT_MAX, bit-exact vs C semantics."""
+    n = 3 * 8192 + 77
+    x = (inputs.bits(11, 0, 0, n) >> np.uint64(32)).astype(np.uint32).view(np.int32).copy()     # full int32 range
+    x[:8] = [0, 1, -1, np.iinfo(np.int32).min, np.iinfo(np.int32).max, modulus if abs(modulus) < 2**31 else 0, 7, -7]
+    residue = int(x[100]) % abs(modulus) if modulus not in (1, -1) else 0
+    if x[100] < 0 and residue:
+        residue -= abs(modulus)                                      # C remainder has the sign of the dividend
+    want = ocfg.cfg2(x, modulus, residue)
+    assert want["count"] > 0
+    with Ctx(MODES[mode]) as c:
+        tx = c.torch.from_numpy(x).cuda()
+        r = W.cfg2(c.ctx, n, tx.data_ptr(), modulus=modulus, residue=residue)
+        cnt, s = c.get(r["count"]), c.get(r["sum"])
+        kept = c.read_vec(r["kept"], np.int32)
+    assert cnt == want["count"] and s == want["sum"]
+    assert bits_equal(kept, want["kept"])
+
+
 @pytest.mark.parametrize("dtype", [np.float32, np.float64, np.int64])
 def test_filter_other_dtypes_and_edge_masks(dtype):
     n = 3 * 4096 + 5
