@@ -40,11 +40,11 @@ constexpr int LB = 8;       // look-back windows (of 32 tile states) requested p
 
 __device__ __forceinline__ unsigned long long ld_state(const unsigned long long* p) {
     unsigned long long v;
-    asm volatile("ld.volatile.global.u64 %0, [%1];" : "=l"(v) : "l"(p));
+    asm volatile("ld.relaxed.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(p));
     return v;
 }
 __device__ __forceinline__ void st_state(unsigned long long* p, unsigned long long v) {
-    asm volatile("st.volatile.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
+    asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
 }
 
 // load modes of one step: guarded element loads (ragged / misaligned), 128-bit global loads, shared-memory stage
@@ -64,10 +64,13 @@ template <class P> struct FilterTemplateEval {
     static constexpr int NVEC_REAL = count_vec();
     static constexpr int U = NVEC_REAL <= 1 ? 4 * P::unroll : 4;     // steps per tile: 16 KiB per step-quadruple and input
     static constexpr int TILE = BLOCK * U * FW;
-    static constexpr int NS = P::row_unroll >= 3 ? P::row_unroll : 3;   // buffers in the ring (the pipeline needs >= 3)
-    static constexpr bool STAGED = NVEC_REAL >= 1 && (size_t)NS * NVEC_REAL * TILE * sizeof(T) <= 200 * 1024;
+    static constexpr int NS = P::row_unroll >= 2 && P::row_unroll <= 3 ? P::row_unroll : 2;   // input stages
+    static constexpr int RC = TILE;                      // elements of the compaction ring (a power of two, >= one tile)
+    static constexpr bool STAGED = NVEC_REAL >= 1 && (size_t)(NS * NVEC_REAL + 1) * TILE * sizeof(T) <= 200 * 1024;
     static constexpr int NVEC = STAGED ? NVEC_REAL : 1;
-    static constexpr size_t SMEM = (size_t)NS * NVEC * TILE * sizeof(T) + NS * sizeof(uint64_t);
+    static constexpr size_t STAGE_BYTES = STAGED ? (size_t)NS * NVEC * TILE * sizeof(T) : 0;
+    static constexpr size_t SMEM = STAGE_BYTES + (size_t)RC * sizeof(T) + NS * sizeof(uint64_t);
+    static_assert((U & (U - 1)) == 0, "filter tile must be a power of two");
     __host__ __device__ static constexpr int vec_slot(int K) {
         int n = 0;
         for (int k = 0; k < K; ++k) n += (P::prog.in[k].kind == IN_VEC);
@@ -159,9 +162,10 @@ template <class TT> struct FilterBytecodeEval {
     static constexpr int U = 4;                          // steps per tile
     static constexpr int FW = 16 / (int)sizeof(T);       // elements per thread per step (one 128-bit access)
     static constexpr int TILE = BLOCK * U * FW;
-    static constexpr int NVEC = 1, NS = 3;
+    static constexpr int NVEC = 1, NS = 2, RC = TILE;
     static constexpr bool STAGED = false;
-    static constexpr size_t SMEM = (size_t)NS * TILE * sizeof(T) + NS * sizeof(uint64_t);
+    static constexpr size_t STAGE_BYTES = 0;
+    static constexpr size_t SMEM = (size_t)RC * sizeof(T) + NS * sizeof(uint64_t);
     __device__ __forceinline__ static void issue(const SgProg*, const SgArgs&, int64_t, T*, uint64_t*) {}
     template <int MODE>
     __device__ __forceinline__ static void run(const SgProg* g, const SgArgs& a, int64_t i, const T*, int, T (&val)[FW], unsigned int& keep, Cell (&acc)[NOUT]) {
@@ -194,13 +198,14 @@ template <class TT> struct FilterBytecodeEval {
 };
 
 // ---- the kernel body -------------------------------------------------------------------------------------
-// Software pipeline over the tiles a block claims (iteration `it` uses stage it % NS):
-//   wait for the stage -> evaluate -> ballot ranks -> barrier 1 -> thread 0 refills the stage freed in the previous
-//   iteration; warp 0 PUBLISHES this tile's aggregate, RESOLVES the look-back of the PREVIOUS tile from the tile
-//   states it requested one iteration ago, and REQUESTS this tile's LB windows; every warp scatters its kept items in
-//   place (tile-local order) -> barrier 2 -> coalesced copy-out of the PREVIOUS tile at its now known global offset.
-// The look-back round trip (several microseconds under a saturated memory system) is thus overlapped with a whole
-// tile of work, and an aggregate is published without waiting for any predecessor.
+// Warp-specialised block of FILTER_THREADS = BLOCK + 32 threads:
+//   warps 0..7 (compute): wait for the stage -> evaluate -> ballot ranks -> named barrier -> thread 0 hands
+//       {tile id, tile total} to the look-back warp and refills the stage freed in the previous iteration; every
+//       warp scatters its kept items in place (tile-local order) -> wait for the PREVIOUS tile's global offset ->
+//       coalesced copy-out of the previous tile.  One barrier per tile; nothing here waits for another block.
+//   warp 8 (look-back): publishes the tile's aggregate at once, then polls LB windows (256 tile states) per round
+//       trip until it finds an inclusive prefix, publishes the tile's inclusive prefix and posts the offset.
+//       It has a whole tile time to do so before the compute warps need the offset.
 template <class EV, int MODE>
 __device__ __forceinline__ void filter_eval_tile(const SgProg* g, const SgArgs& a, int64_t tbase, const typename EV::T* stage,
                                                  typename EV::T (&val)[EV::U][EV::FW], unsigned int (&keep)[EV::U], Cell (&acc)[EV::NOUT]) {
@@ -213,16 +218,74 @@ __device__ __forceinline__ void filter_eval_tile(const SgProg* g, const SgArgs& 
     }
 }
 
+constexpr int FILTER_THREADS = BLOCK + 32;
+
+// look-back warp: exclusive prefix of `tile` (sum of the kept counts of all tiles before it).  The tile's AGGREGATE has
+// already been published by the compute warps — at once, so that no other block's look-back waits for this warp's backlog.
+__device__ __forceinline__ unsigned long long filter_lookback(unsigned long long* state, unsigned long long ep, int tile, unsigned int tile_total, int lane) {
+    if (tile == 0) return 0;        // its inclusive prefix was published with the aggregate
+    unsigned long long excl = 0;
+    int look = tile - 1;
+    for (;;) {
+        unsigned long long lbw[LB];
+#pragma unroll
+        for (int j = 0; j < LB; ++j) {
+            const int idx = look - lane - 32 * j;
+            lbw[j] = (idx >= 0) ? ld_state(&state[idx]) : (ST_INC | ep);    // virtual tile -1: inclusive prefix 0
+        }
+        // ballots of all LB windows first (independent), then ONE position search and ONE warp sum
+        int p_inc = LB * 32, p_inv = LB * 32;       // first inclusive prefix / first unpublished state, in (window, lane) order
+#pragma unroll
+        for (int j = LB - 1; j >= 0; --j) {
+            const unsigned long long w = lbw[j];
+            const bool valid = ((w & ST_FLAGS) != 0) && ((w & (0x3fffffull << 40)) == ep);
+            const bool inc = valid && ((w & ST_FLAGS) == ST_INC);
+            const unsigned int vmask = __ballot_sync(0xffffffffu, valid), imask = __ballot_sync(0xffffffffu, inc);
+            if (imask) p_inc = 32 * j + __ffs(imask) - 1;
+            if (~vmask) p_inv = 32 * j + __ffs(~vmask) - 1;
+        }
+        // contributing states: up to and including the first inclusive prefix, else every state before the first unpublished one
+        const bool done = p_inc < p_inv;
+        const int upto = done ? p_inc + 1 : p_inv;
+        unsigned long long x = 0;
+#pragma unroll
+        for (int j = 0; j < LB; ++j)
+            if (32 * j + lane < upto) x += lbw[j] & ST_VAL;
+#pragma unroll
+        for (int d = 16; d >= 1; d >>= 1) x += __shfl_xor_sync(0xffffffffu, x, d);
+        excl += x;
+        if (done) break;
+        look -= upto;       // go deeper, or poll again from the predecessor that has not published yet
+    }
+    if (lane == 0) st_state(&state[tile], ST_INC | ep | (excl + tile_total));
+    return excl;
+}
+
+
+constexpr int RUN = 4;      // consecutive tiles a block claims at once; one look-back per run
+constexpr int NR = 4;       // runs of one block whose offset may be outstanding (ring of run slots)
+constexpr int NP = 8;       // tiles of one block that may wait for their global offset (<= (NR-1)*RUN)
+
 template <class EV>
 __device__ __forceinline__ void filter_body(const SgProg* g, const SgArgs& a) {
     typedef typename EV::T T;
-    constexpr int U = EV::U, FW = EV::FW, TILE = EV::TILE, NOUT = EV::NOUT, NS = EV::NS, NVEC = EV::NVEC;
+    constexpr int U = EV::U, FW = EV::FW, TILE = EV::TILE, NOUT = EV::NOUT, NS = EV::NS, NVEC = EV::NVEC, RC = EV::RC;
+    static_assert(NP <= (NR - 1) * RUN, "a run slot must not be reused while one of its tiles is pending");
     extern __shared__ __align__(128) unsigned char dyn_smem[];
-    T* const stage_base = reinterpret_cast<T*>(dyn_smem);                                   // [NS][NVEC][TILE]
-    uint64_t* const full_bar = reinterpret_cast<uint64_t*>(dyn_smem + (size_t)NS * NVEC * TILE * sizeof(T));
-    __shared__ int s_tile[NS];
-    __shared__ unsigned int s_warp_total[WARPS];
-    __shared__ unsigned long long s_tile_excl;
+    T* const stage_base = reinterpret_cast<T*>(dyn_smem);                                   // [NS][NVEC][TILE] (staged instances)
+    T* const ring = reinterpret_cast<T*>(dyn_smem + EV::STAGE_BYTES);                       // [RC] compacted values awaiting their offset
+    uint64_t* const full_bar = reinterpret_cast<uint64_t*>(dyn_smem + EV::STAGE_BYTES + (size_t)RC * sizeof(T));
+    __shared__ int s_tile[NS + 1];                      // tile id of iteration it at [it % (NS+1)]
+    __shared__ unsigned int s_warp_total[2][WARPS];     // double-buffered: a warp may run one barrier ahead
+    __shared__ int s_ready[2];                          // thread 0 -> all: pending tiles whose offset is known (polled before the barrier)
+    __shared__ int s_q_tile[NP];                        // pending tile queue: tile id,
+    __shared__ unsigned int s_q_total[NP];              //   kept count,
+    __shared__ unsigned int s_q_lpre[NP];               //   kept count of the earlier tiles of its run,
+    __shared__ int s_q_run[NP];                         //   run number (of this block)
+    __shared__ int s_r_tile[NR];                        // compute -> look-back warp: first tile of the run (-1: no more runs)
+    __shared__ unsigned int s_r_total[NR];              //                            its kept count
+    __shared__ unsigned long long s_r_excl[NR];         // look-back warp -> compute: global offset of the run's first tile
+    __shared__ uint64_t run_posted[NR], run_resolved[NR];   // mbarriers, one arrival each
 
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const unsigned int lt_mask = (1u << lane) - 1u;
@@ -244,48 +307,97 @@ __device__ __forceinline__ void filter_body(const SgProg* g, const SgArgs& a) {
 
     if (a.n_tiles == 0 && blockIdx.x == 0 && threadIdx.x == 0) *reinterpret_cast<long long*>(a.out_aux[fo]) = 0;
 
-    // claim NS tiles; their bulk copies are in flight before the first one is touched
+    // thread 0 hands out this block's tile sequence: runs of RUN consecutive tiles claimed with one atomic each
+    int seq_base = 0, seq_j = RUN;              // thread 0 only: current run and position in it
+    auto next_tile = [&]() -> int {             // thread 0 only
+        if (seq_j == RUN) { seq_base = (int)atomicAdd(&a.ctrl[2], (unsigned int)RUN); seq_j = 0; }
+        return seq_base + seq_j++;
+    };
     if (threadIdx.x == 0) {
-        if (staged) {
-            for (int s = 0; s < NS; ++s) mbar_init(&full_bar[s], 1);
-            mbar_fence_init();
+        for (int r = 0; r < NR; ++r) {
+            mbar_init(&run_posted[r], 1);
+            mbar_init(&run_resolved[r], 1);
         }
-        for (int s = 0; s < NS; ++s) {
-            const int t = (int)atomicAdd(&a.ctrl[2], 1u);
+        if (staged)
+            for (int s = 0; s < NS; ++s) mbar_init(&full_bar[s], 1);
+        mbar_fence_init();
+        for (int s = 0; s < NS; ++s) {          // the first NS tiles: their bulk copies are in flight before the first one is touched
+            const int t = next_tile();
             s_tile[s] = t;
             if (staged && t < a.n_full_tiles) EV::issue(g, a, (int64_t)t * TILE, stage_base + (size_t)s * NVEC * TILE, &full_bar[s]);
         }
     }
     __syncthreads();
 
-    // state of the previous tile (resolved and copied out one iteration later)
-    int prev_tile = -1;
-    unsigned int prev_total = 0;
-    T* prev_cbuf = nullptr;
-    unsigned long long lbw[LB];         // warp 0: tile states requested for the previous tile's look-back
-#pragma unroll
-    for (int j = 0; j < LB; ++j) lbw[j] = 0;
+    if (warp == WARPS) {
+        // ---------------- look-back warp: one message per run, in order ----------------
+        for (int r = 0;; ++r) {
+            const int rs = r % NR;
+            mbar_wait(&run_posted[rs], (uint32_t)((r / NR) & 1));
+            const int tile = s_r_tile[rs];
+            if (tile < 0) break;
+            const unsigned int total = s_r_total[rs];
+            const unsigned long long excl = filter_lookback(state, ep, tile, total, lane);
+            if (lane == 0) {
+                s_r_excl[rs] = excl;
+                mbar_arrive(&run_resolved[rs]);
+            }
+        }
+    } else {
+        // ---------------- compute warps ----------------
+        // Pending tiles (compacted into the ring, offset not yet known) form a queue in processing order; every compute
+        // thread tracks the same queue state in registers.  A tile's offset = its run's offset + the kept counts of the
+        // run's earlier tiles (local prefix), so only the FIRST tile of a run needs a look-back; once the run's offset is
+        // known, later tiles of the run publish their INCLUSIVE prefix directly — other blocks' look-backs end there.
+        int q_head = 0, q_count = 0, n_tiles_done = 0;
+        unsigned int ring_head = 0, ring_tail = 0;
+        int run_no = -1;                        // number of the current run of this block
+        unsigned int run_lpre = 0;              // kept count of the current run's earlier tiles
+        bool overflow = false;
+        auto copy_out_oldest = [&]() {
+            const int e = q_head % NP;
+            const int r = s_q_run[e];
+            mbar_wait(&run_resolved[r % NR], (uint32_t)((r / NR) & 1));
+            const unsigned int total = s_q_total[e];
+            const long long base = (long long)(s_r_excl[r % NR] + s_q_lpre[e]);
+            for (unsigned int i = threadIdx.x; i < total; i += BLOCK) {
+                const long long pos = base + i;
+                const T v = ring[(ring_tail + i) & (RC - 1)];
+                if (pos < cap) dst[pos] = v; else overflow = true;
+            }
+            if (threadIdx.x == 0 && s_q_tile[e] == a.n_tiles - 1) *reinterpret_cast<long long*>(a.out_aux[fo]) = base + (long long)total;
+            ring_tail += total;
+            ++q_head;
+            --q_count;
+        };
+        int it = 0;
+        for (;; ++it) {
+            const int s = it % NS;
+            const int tile = s_tile[it % (NS + 1)];
+            if (tile >= a.n_tiles) break;
+            if (tile % RUN == 0) { ++run_no; run_lpre = 0; }
+            const int rs = run_no % NR;
+            // thread 0 fetches the tile of iteration it+NS now (a new run costs one atomic, whose latency hides behind the
+            // evaluation), makes the id visible before this iteration's barrier, and issues its bulk copy right after the
+            // barrier into THIS stage, which every thread has read into registers by then
+            int t_next = 0x7fffffff;
+            if (threadIdx.x == 0) t_next = next_tile();
 
-    for (int it = 0;; ++it) {
-        const int s = it % NS;
-        const int tile = s_tile[s];
-        const bool active = tile < a.n_tiles;
-        if (!active && prev_tile < 0) break;
-        T* const cbuf = stage_base + (size_t)s * NVEC * TILE;    // this tile's stage; slot 0 becomes the compaction buffer
-
-        T val[U][FW];
-        unsigned int keep[U], off[U];
-        unsigned int running = 0;
-        if (active) {
-            const int64_t tbase = (int64_t)tile * TILE;
-            const bool full = all_vec && tile < a.n_full_tiles;  // inside every operand's and output's length
-            if (staged && full) {
-                mbar_wait(&full_bar[s], (uint32_t)((it / NS) & 1));
-                filter_eval_tile<EV, FM_STAGED>(g, a, tbase, cbuf, val, keep, acc);
-            } else if (full) {
-                filter_eval_tile<EV, FM_GLOBAL>(g, a, tbase, cbuf, val, keep, acc);
-            } else {
-                filter_eval_tile<EV, FM_GUARDED>(g, a, tbase, cbuf, val, keep, acc);
+            T val[U][FW];
+            unsigned int keep[U], off[U];
+            unsigned int running = 0;
+            {
+                const int64_t tbase = (int64_t)tile * TILE;
+                const bool full = all_vec && tile < a.n_full_tiles;  // inside every operand's and output's length
+                const T* const stg = stage_base + (size_t)s * NVEC * TILE;
+                if (staged && full) {
+                    mbar_wait(&full_bar[s], (uint32_t)((it / NS) & 1));
+                    filter_eval_tile<EV, FM_STAGED>(g, a, tbase, stg, val, keep, acc);
+                } else if (full) {
+                    filter_eval_tile<EV, FM_GLOBAL>(g, a, tbase, stg, val, keep, acc);
+                } else {
+                    filter_eval_tile<EV, FM_GUARDED>(g, a, tbase, stg, val, keep, acc);
+                }
             }
 #pragma unroll
             for (int u = 0; u < U; ++u) {
@@ -295,115 +407,85 @@ __device__ __forceinline__ void filter_body(const SgProg* g, const SgArgs& a) {
                 off[u] = running + __popc(b0 & lt_mask) + 2 * __popc(b1 & lt_mask) + 4 * __popc(b2 & lt_mask);
                 running += __popc(b0) + 2 * __popc(b1) + 4 * __popc(b2);
             }
-            if (lane == 0) s_warp_total[warp] = running;
-        }
-        __syncthreads();        // 1: this tile's stage has been read into registers; warp totals visible; the previous
-                                //    iteration's copy-out (of tile it-2's ... it-1's predecessor stage) is complete
-        // the stage of tile it-2 was copied out during iteration it-1: refill it for iteration it+NS-2
-        if (threadIdx.x == 0 && it >= 2) {
-            const int sr = (it - 2) % NS;
-            const int t = (int)atomicAdd(&a.ctrl[2], 1u);
-            s_tile[sr] = t;                                     // read at the top of iteration it+NS-2, behind barrier 2
-            if (staged && t < a.n_full_tiles) {
-                fence_proxy_async();
-                EV::issue(g, a, (int64_t)t * TILE, stage_base + (size_t)sr * NVEC * TILE, &full_bar[sr]);
+            if (lane == 0) s_warp_total[it & 1][warp] = running;
+            bool run_known = false;         // thread 0: the current run's offset has been resolved already
+            if (threadIdx.x == 0) {
+                s_tile[(it + NS) % (NS + 1)] = t_next;
+                int ready = 0;      // how many of the oldest pending tiles already have their offset (non-blocking poll)
+                for (; ready < q_count; ++ready) {
+                    const int r = s_q_run[(q_head + ready) % NP];
+                    if (!mbar_test(&run_resolved[r % NR], (uint32_t)((r / NR) & 1))) break;
+                }
+                s_ready[it & 1] = ready;
+                if (tile % RUN != 0) run_known = mbar_test(&run_resolved[rs], (uint32_t)((run_no / NR) & 1));
             }
-        }
-        unsigned int warp_excl = 0, tile_total = 0;
-        if (active) {
+            named_bar_sync<1, BLOCK>();     // the stage is in registers; warp totals, next tile id and the ready count are visible
+            unsigned int warp_excl = 0, tile_total = 0;
 #pragma unroll
             for (int w = 0; w < WARPS; ++w) {
-                const unsigned int t = s_warp_total[w];
+                const unsigned int t = s_warp_total[it & 1][w];
                 if (w < warp) warp_excl += t;
                 tile_total += t;
             }
-        }
-        if (warp == 0) {
-            // (a) publish this tile's aggregate: it never waits for a predecessor
-            if (active && lane == 0) st_state(&state[tile], (tile == 0 ? ST_INC : ST_AGG) | ep | (unsigned long long)tile_total);
-            // (b) resolve the previous tile's look-back from the states requested one iteration ago
-            if (prev_tile >= 0) {
-                unsigned long long excl = 0;
-                if (prev_tile != 0) {
-                    int look = prev_tile - 1;
-                    for (;;) {
-                        // ballots of all LB windows first (independent), then ONE position search and ONE warp sum
-                        int p_inc = LB * 32, p_inv = LB * 32;       // first inclusive prefix / first unpublished state, in (window, lane) order
-#pragma unroll
-                        for (int j = LB - 1; j >= 0; --j) {
-                            const unsigned long long w = lbw[j];
-                            const bool valid = ((w & ST_FLAGS) != 0) && ((w & (0x3fffffull << 40)) == ep);
-                            const bool inc = valid && ((w & ST_FLAGS) == ST_INC);
-                            const unsigned int vmask = __ballot_sync(0xffffffffu, valid), imask = __ballot_sync(0xffffffffu, inc);
-                            if (imask) p_inc = 32 * j + __ffs(imask) - 1;
-                            if (~vmask) p_inv = 32 * j + __ffs(~vmask) - 1;
-                        }
-                        // contributing states: up to and including the first inclusive prefix, else every state before the first unpublished one
-                        const bool done = p_inc < p_inv;
-                        const int upto = done ? p_inc + 1 : p_inv;
-                        unsigned long long x = 0;
-#pragma unroll
-                        for (int j = 0; j < LB; ++j)
-                            if (32 * j + lane < upto) x += lbw[j] & ST_VAL;
-#pragma unroll
-                        for (int d = 16; d >= 1; d >>= 1) x += __shfl_xor_sync(0xffffffffu, x, d);
-                        excl += x;
-                        if (done) break;
-                        look -= upto;       // go deeper, or poll again from the predecessor that has not published yet
-#pragma unroll
-                        for (int j = 0; j < LB; ++j) {
-                            const int idx = look - lane - 32 * j;
-                            lbw[j] = (idx >= 0) ? ld_state(&state[idx]) : (ST_INC | ep);
-                        }
-                    }
-                    if (lane == 0) st_state(&state[prev_tile], ST_INC | ep | (excl + prev_total));
+            if (threadIdx.x == 0) {
+                // publish at once: the inclusive prefix if it is known (tile 0, or the run's offset is resolved), else the aggregate
+                if (tile == 0) st_state(&state[0], ST_INC | ep | (unsigned long long)tile_total);
+                else if (run_known) st_state(&state[tile], ST_INC | ep | (s_r_excl[rs] + run_lpre + tile_total));
+                else st_state(&state[tile], ST_AGG | ep | (unsigned long long)tile_total);
+                const int e = it % NP;
+                s_q_tile[e] = tile;
+                s_q_total[e] = tile_total;
+                s_q_lpre[e] = run_lpre;
+                s_q_run[e] = run_no;
+                if (tile % RUN == 0) {      // first tile of a run: hand it to the look-back warp
+                    s_r_tile[rs] = tile;
+                    s_r_total[rs] = tile_total;
+                    mbar_arrive(&run_posted[rs]);
                 }
-                if (lane == 0) {
-                    s_tile_excl = excl;
-                    if (prev_tile == a.n_tiles - 1) *reinterpret_cast<long long*>(a.out_aux[fo]) = (long long)(excl + prev_total);
+                if (staged && t_next < a.n_full_tiles) {
+                    fence_proxy_async();
+                    EV::issue(g, a, (int64_t)t_next * TILE, stage_base + (size_t)s * NVEC * TILE, &full_bar[s]);
                 }
             }
-            // (c) request this tile's LB windows of predecessor states; they are examined in the next iteration
-            if (active) {
-#pragma unroll
-                for (int j = 0; j < LB; ++j) {
-                    const int idx = tile - 1 - lane - 32 * j;
-                    lbw[j] = (idx >= 0) ? ld_state(&state[idx]) : (ST_INC | ep);    // virtual tile -1: inclusive prefix 0
-                }
+            int copied = 0;
+            if (ring_head - ring_tail + tile_total > (unsigned int)RC) {
+                // rare: the ring cannot take this tile yet — wait for the oldest offsets first
+                while (ring_head - ring_tail + tile_total > (unsigned int)RC) { copy_out_oldest(); ++copied; }
+                named_bar_sync<2, BLOCK>();
             }
-        }
-        if (active) {
 #pragma unroll
             for (int u = 0; u < U; ++u) {
-                unsigned int pos = warp_excl + off[u];
+                unsigned int pos = ring_head + warp_excl + off[u];
 #pragma unroll
                 for (int e = 0; e < FW; ++e)
-                    if ((keep[u] >> e) & 1u) cbuf[pos++] = val[u][e];
+                    if ((keep[u] >> e) & 1u) ring[(pos++) & (RC - 1)] = val[u][e];
             }
+            ring_head += tile_total;
+            run_lpre += tile_total;
+            ++q_count;
+            // copy out the tiles whose offset was known at the poll (never blocks), and as many as the queue bound demands
+            const int ready = s_ready[it & 1];
+            while (copied < ready || q_count > NP - 1) { copy_out_oldest(); ++copied; }
         }
-        __syncthreads();        // 2: the previous tile's global offset is known (and this tile is compacted)
-        if (prev_tile >= 0) {
-            const long long tile_excl = (long long)s_tile_excl;
-            bool overflow = false;
-            for (unsigned int i = threadIdx.x; i < prev_total; i += BLOCK) {
-                const long long pos = tile_excl + i;
-                if (pos < cap) dst[pos] = prev_cbuf[i]; else overflow = true;
-            }
-            if (overflow) a.ctrl[3] = 1u;
+        if (threadIdx.x == 0) {             // no run follows: release the look-back warp
+            const int rs = (run_no + 1) % NR;
+            s_r_tile[rs] = -1;
+            mbar_arrive(&run_posted[rs]);
         }
-        prev_tile = active ? tile : -1;
-        prev_total = tile_total;
-        prev_cbuf = cbuf;
+        named_bar_sync<1, BLOCK>();         // the last tile's queue entry (written by thread 0 after its barrier) is visible
+        while (q_count > 0) copy_out_oldest();
+        if (overflow) a.ctrl[3] = 1u;
+        (void)n_tiles_done;
     }
     epilogue_1d<T, NOUT>(acc, kind, a, true);
 }
 
 template <class P>
-__global__ void __launch_bounds__(BLOCK, P::min_blocks) filter1d_template(const __grid_constant__ SgArgs a) {
+__global__ void __launch_bounds__(FILTER_THREADS, P::min_blocks) filter1d_template(const __grid_constant__ SgArgs a) {
     filter_body<FilterTemplateEval<P>>(nullptr, a);
 }
 template <class T>
-__global__ void __launch_bounds__(BLOCK) filter1d_bytecode(const __grid_constant__ SgProg g, const __grid_constant__ SgArgs a) {
+__global__ void __launch_bounds__(FILTER_THREADS) filter1d_bytecode(const __grid_constant__ SgProg g, const __grid_constant__ SgArgs a) {
     filter_body<FilterBytecodeEval<T>>(&g, a);
 }
 

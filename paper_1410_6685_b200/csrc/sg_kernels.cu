@@ -45,7 +45,7 @@ template <class P> cudaError_t launch_template(const SgArgs& a, int grid, cudaSt
     else if constexpr ((P::prog.shape.flags & PF_FILTER) != 0) {
         static bool attr_set = false;
         if (!attr_set) { cudaFuncSetAttribute(filter1d_template<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_of<P>()); attr_set = true; }
-        filter1d_template<P><<<grid, BLOCK, smem_of<P>(), s>>>(a);
+        filter1d_template<P><<<grid, FILTER_THREADS, smem_of<P>(), s>>>(a);
     }
     else pass1d_template<P><<<grid, BLOCK, 0, s>>>(a);
     return cudaGetLastError();
@@ -61,7 +61,7 @@ template <class P> int occupancy_template() {
     }
     else if constexpr ((P::prog.shape.flags & PF_FILTER) != 0) {
         cudaFuncSetAttribute(filter1d_template<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_of<P>());
-        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, filter1d_template<P>, BLOCK, smem_of<P>());
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, filter1d_template<P>, FILTER_THREADS, smem_of<P>());
     }
     else e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, pass1d_template<P>, BLOCK, 0);
     if (e != cudaSuccess || occ <= 0) return 1;
@@ -93,7 +93,7 @@ template <class T> cudaError_t launch_bytecode_t(const SgProg& g, const SgArgs& 
     if (g.shape.flags & PF_FILTER) {
         static bool attr_set = false;
         if (!attr_set) { cudaFuncSetAttribute(filter1d_bytecode<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FilterBytecodeEval<T>::SMEM); attr_set = true; }
-        filter1d_bytecode<T><<<grid, BLOCK, FilterBytecodeEval<T>::SMEM, s>>>(g, a);
+        filter1d_bytecode<T><<<grid, FILTER_THREADS, FilterBytecodeEval<T>::SMEM, s>>>(g, a);
     }
     else pass1d_bytecode<T><<<grid, BLOCK, 0, s>>>(g, a);
     return cudaGetLastError();
@@ -103,7 +103,7 @@ template <class T> int occupancy_bytecode_t(bool filter) {
     if (cached[filter] > 0) return cached[filter];
     int occ = 0;
     if (filter) cudaFuncSetAttribute(filter1d_bytecode<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FilterBytecodeEval<T>::SMEM);
-    cudaError_t e = filter ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, filter1d_bytecode<T>, BLOCK, FilterBytecodeEval<T>::SMEM)
+    cudaError_t e = filter ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, filter1d_bytecode<T>, FILTER_THREADS, FilterBytecodeEval<T>::SMEM)
                            : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, pass1d_bytecode<T>, BLOCK, 0);
     if (e != cudaSuccess || occ <= 0) return 1;
     cached[filter] = occ;

@@ -36,7 +36,7 @@ __device__ __forceinline__ void block_reduce_cells(Cell (&acc)[NOUT], const uint
             Cell other = cell_shfl_down(acc[o], d);
             cell_combine<T>(kind[o], acc[o], other);
         }
-        if (lane == 0) smem[warp * NOUT + o] = acc[o];
+        if (lane == 0 && warp < WARPS) smem[warp * NOUT + o] = acc[o];     // warps beyond WARPS (a filter block's look-back warp) hold identities
     }
     __syncthreads();
     if (warp == 0) {
@@ -77,7 +77,7 @@ __device__ __forceinline__ void epilogue_1d(Cell (&acc)[NOUT], const uint8_t (&k
     for (int o = 0; o < NOUT; ++o) {
         if (!out_is_reduction(kind[o])) continue;
         Cell c = cell_identity<T>(kind[o]);
-        for (unsigned int b = threadIdx.x; b < gridDim.x; b += BLOCK) {
+        for (unsigned int b = threadIdx.x; b < gridDim.x && threadIdx.x < BLOCK; b += BLOCK) {
             Cell other;
             const unsigned long long* src = reinterpret_cast<const unsigned long long*>(&ws[(size_t)b * SG_MAX_OUT + o]);
             other.a = __ldcg(src); other.b = __ldcg(src + 1);
