@@ -32,6 +32,29 @@ __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
         "}\n" ::"r"(smem_u32(bar)), "r"(parity)
         : "memory");
 }
+// explicit shared-window accesses (32-bit shared address + byte offset): no generic-address translation per access
+template <class T> __device__ __forceinline__ void sts_elem(uint32_t base, uint32_t idx, T v) {
+    if constexpr (sizeof(T) == 4) {
+        uint32_t w; memcpy(&w, &v, 4);
+        asm volatile("st.shared.b32 [%0], %1;" ::"r"(base + idx * 4u), "r"(w) : "memory");
+    } else {
+        unsigned long long w; memcpy(&w, &v, 8);
+        asm volatile("st.shared.b64 [%0], %1;" ::"r"(base + idx * 8u), "l"(w) : "memory");
+    }
+}
+template <class T> __device__ __forceinline__ T lds_elem(uint32_t base, uint32_t idx) {
+    T v;
+    if constexpr (sizeof(T) == 4) {
+        uint32_t w;
+        asm volatile("ld.shared.b32 %0, [%1];" : "=r"(w) : "r"(base + idx * 4u) : "memory");
+        memcpy(&v, &w, 4);
+    } else {
+        unsigned long long w;
+        asm volatile("ld.shared.b64 %0, [%1];" : "=l"(w) : "r"(base + idx * 8u) : "memory");
+        memcpy(&v, &w, 8);
+    }
+    return v;
+}
 // non-blocking: has the phase with this parity completed?
 __device__ __forceinline__ bool mbar_test(uint64_t* bar, uint32_t parity) {
     uint32_t ok;

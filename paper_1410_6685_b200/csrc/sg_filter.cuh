@@ -71,6 +71,24 @@ template <class P> struct FilterTemplateEval {
     static constexpr size_t STAGE_BYTES = STAGED ? (size_t)NS * NVEC * TILE * sizeof(T) : 0;
     static constexpr size_t SMEM = STAGE_BYTES + (size_t)RC * sizeof(T) + NS * sizeof(uint64_t);
     static_assert((U & (U - 1)) == 0, "filter tile must be a power of two");
+    // index of the OUT_FILTER output; reductions over exactly the kept values (same source register, same predicate) are
+    // accumulated when the compacted values are copied out — one visit per KEPT element instead of one per element
+    __host__ __device__ static constexpr int filter_out() {
+        for (int o = 0; o < M::S.n_out; ++o)
+            if (P::prog.out[o].kind == OUT_FILTER) return o;
+        return 0;
+    }
+    __host__ __device__ static constexpr bool kept_reduction(int O) {
+        const SgOut f = P::prog.out[filter_out()], out = P::prog.out[O];
+        return (out.kind == OUT_SUM || out.kind == OUT_MAX || out.kind == OUT_MIN) && out.src == f.src && out.pred == f.pred;
+    }
+    template <int... O>
+    __device__ __forceinline__ static void accum_kept_(T x, Cell (&acc)[NOUT], std::integer_sequence<int, O...>) {
+        ((kept_reduction(O) ? cell_accum_value<T>(P::prog.out[O].kind, acc[O], x) : (void)0), ...);
+    }
+    __device__ __forceinline__ static void accum_kept(const SgProg*, T x, Cell (&acc)[NOUT]) {
+        accum_kept_(x, acc, std::make_integer_sequence<int, M::S.n_out>{});
+    }
     __host__ __device__ static constexpr int vec_slot(int K) {
         int n = 0;
         for (int k = 0; k < K; ++k) n += (P::prog.in[k].kind == IN_VEC);
@@ -125,6 +143,8 @@ template <class P> struct FilterTemplateEval {
                 keep |= (unsigned int)(in_range && p[out.pred][e]) << e;
             } else if constexpr (out_is_pred_reduction(out.kind)) {
                 if (in_range) cell_accum_pred(out.kind, acc[O], p[out.src][e]);
+            } else if constexpr (kept_reduction(O)) {
+                // accumulated at copy-out (accum_kept)
             } else if constexpr (out_is_reduction(out.kind)) {
                 if constexpr (out.pred == SG_NO_PRED) { if (in_range) cell_accum_value<T>(out.kind, acc[O], v[out.src][e]); }
                 else if constexpr (out.kind == OUT_SUM && !Traits<T>::is_float) {
@@ -167,6 +187,7 @@ template <class TT> struct FilterBytecodeEval {
     static constexpr size_t STAGE_BYTES = 0;
     static constexpr size_t SMEM = (size_t)RC * sizeof(T) + NS * sizeof(uint64_t);
     __device__ __forceinline__ static void issue(const SgProg*, const SgArgs&, int64_t, T*, uint64_t*) {}
+    __device__ __forceinline__ static void accum_kept(const SgProg*, T, Cell (&)[NOUT]) {}      // masked reductions are accumulated per element
     template <int MODE>
     __device__ __forceinline__ static void run(const SgProg* g, const SgArgs& a, int64_t i, const T*, int, T (&val)[FW], unsigned int& keep, Cell (&acc)[NOUT]) {
         const bool full = MODE != FM_GUARDED;
@@ -256,6 +277,7 @@ __device__ __forceinline__ unsigned long long filter_lookback(unsigned long long
         excl += x;
         if (done) break;
         look -= upto;       // go deeper, or poll again from the predecessor that has not published yet
+        if (p_inv < LB * 32) __nanosleep(400);      // stalled: do not hammer the state words (nor this SM's issue slots)
     }
     if (lane == 0) st_state(&state[tile], ST_INC | ep | (excl + tile_total));
     return excl;
@@ -273,7 +295,7 @@ __device__ __forceinline__ void filter_body(const SgProg* g, const SgArgs& a) {
     static_assert(NP <= (NR - 1) * RUN, "a run slot must not be reused while one of its tiles is pending");
     extern __shared__ __align__(128) unsigned char dyn_smem[];
     T* const stage_base = reinterpret_cast<T*>(dyn_smem);                                   // [NS][NVEC][TILE] (staged instances)
-    T* const ring = reinterpret_cast<T*>(dyn_smem + EV::STAGE_BYTES);                       // [RC] compacted values awaiting their offset
+    const uint32_t ring = smem_u32(dyn_smem + EV::STAGE_BYTES);                             // [RC] compacted values awaiting their offset (shared-window address)
     uint64_t* const full_bar = reinterpret_cast<uint64_t*>(dyn_smem + EV::STAGE_BYTES + (size_t)RC * sizeof(T));
     __shared__ int s_tile[NS + 1];                      // tile id of iteration it at [it % (NS+1)]
     __shared__ unsigned int s_warp_total[2][WARPS];     // double-buffered: a warp may run one barrier ahead
@@ -362,7 +384,8 @@ __device__ __forceinline__ void filter_body(const SgProg* g, const SgArgs& a) {
             const long long base = (long long)(s_r_excl[r % NR] + s_q_lpre[e]);
             for (unsigned int i = threadIdx.x; i < total; i += BLOCK) {
                 const long long pos = base + i;
-                const T v = ring[(ring_tail + i) & (RC - 1)];
+                const T v = lds_elem<T>(ring, (ring_tail + i) & (RC - 1));
+                EV::accum_kept(g, v, acc);
                 if (pos < cap) dst[pos] = v; else overflow = true;
             }
             if (threadIdx.x == 0 && s_q_tile[e] == a.n_tiles - 1) *reinterpret_cast<long long*>(a.out_aux[fo]) = base + (long long)total;
@@ -458,7 +481,7 @@ __device__ __forceinline__ void filter_body(const SgProg* g, const SgArgs& a) {
                 unsigned int pos = ring_head + warp_excl + off[u];
 #pragma unroll
                 for (int e = 0; e < FW; ++e)
-                    if ((keep[u] >> e) & 1u) ring[(pos++) & (RC - 1)] = val[u][e];
+                    if ((keep[u] >> e) & 1u) sts_elem<T>(ring, (pos++) & (RC - 1), val[u][e]);
             }
             ring_head += tile_total;
             run_lpre += tile_total;
