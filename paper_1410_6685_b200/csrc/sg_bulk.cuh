@@ -82,6 +82,13 @@ __device__ __forceinline__ void bulk_g2s(void* smem_dst, const void* gmem_src, u
                  "r"(bytes), "r"(smem_u32(bar))
                  : "memory");
 }
+// TMA tensor copy global -> shared of one box of a 2-D tensor map (128 bytes in parameter/constant/global memory,
+// 64-byte aligned): coordinates (c0 = innermost, c1); completion adds the box's bytes to `bar`
+__device__ __forceinline__ void tma_load_2d(uint32_t smem_dst, const void* tmap, int c0, int c1, uint64_t* bar) {
+    asm volatile("cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];" ::"r"(smem_dst), "l"(tmap),
+                 "r"(c0), "r"(c1), "r"(smem_u32(bar))
+                 : "memory");
+}
 // generic-proxy accesses to shared memory are ordered before later async-proxy (bulk copy) accesses
 __device__ __forceinline__ void fence_proxy_async() { asm volatile("fence.proxy.async.shared::cta;" ::: "memory"); }
 

@@ -1,29 +1,30 @@
 // sg_filter.cuh — stream-compacting filter pass (filter).
 //
-// One pass over the input: the predicate chain is evaluated in registers, kept elements are ranked by a
-// warp-ballot prefix inside the tile and by a decoupled look-back over per-tile aggregates across tiles, and
-// written in ascending index order (STABLE, R3).  Count and any reductions over the kept values
-// (masked reductions) are produced by the same pass.
+// One pass over the input: the predicate chain is evaluated in registers, kept elements are ranked inside the tile
+// by a per-thread count + warp scan and across tiles by a decoupled look-back over per-tile aggregates, and written
+// in ascending index order (STABLE, R3).  Count and reductions over the kept values are produced by the
+// same pass.
 //
-// Tile layout: warp-blocked.  A tile is BLOCK*U*FW elements (32 KiB for one input); warp w owns U*32*FW
-// consecutive elements, and in step u lane l owns the FW consecutive elements at
-//     tile + w*U*32*FW + u*32*FW + l*FW
-// so the order (warp, u, lane, e) is memory order and a ballot over lanes ranks them.
+// Tile = 256 rows of 128 bytes (32 KiB per input).  Thread t of the 256 compute threads owns ROW t: its EPT = 32
+// (4-byte types) or 16 (8-byte types) elements are CONSECUTIVE in memory, so one popc of its keep mask and one warp
+// scan rank the whole tile (no per-element ballots), and it appends its kept values in order.
 //
-// Staging: full tiles of 16-byte aligned inputs are brought into an NS-stage shared-memory ring by ONE bulk
-// asynchronous copy per input per tile (cp.async.bulk, the TMA engine; completion on an mbarrier), issued
-// NS-2 tiles ahead by thread 0 — the bytes in flight do not depend on which phase (evaluate / rank / look-back /
-// copy-out) the block is in.  The kept values are compacted IN PLACE into the stage they came from (every
-// thread holds its elements in registers by then) and copied out coalesced.
+// Staging: full tiles of 16-byte aligned inputs are brought into a 2-stage shared-memory ring by ONE TMA tensor
+// copy per input per tile (cp.async.bulk.tensor.2d, completion on an mbarrier), issued two tiles ahead by thread 0.
+// The tensor map views the input as rows of 128 bytes and applies the 128-byte swizzle: the 16-byte chunk j of row r
+// lands at chunk (j ^ (r & 7)), so thread t reads its own row with conflict-free 128-bit shared loads.  Ragged or
+// misaligned tiles are filled cooperatively (coalesced guarded loads, same swizzled layout).
 //
-// Look-back: at B200 rates a tile completes every few nanoseconds chip-wide, so a window of 32 predecessors per
-// L2 round trip never catches up with the tiles in flight, and under a saturated memory system one round trip
-// costs microseconds (measured: 17 us per tile with the textbook one-warp, one-window-at-a-time look-back).
-// Warp 0 therefore requests LB = 8 windows (256 tile states) at once and examines them ONE TILE LATER: the
-// round trip overlaps the evaluation of the block's next tile (software pipeline, see filter_body).
+// Block = 8 compute warps + 1 look-back warp (warp specialisation).  Kept values go into a shared-memory RING that
+// is decoupled from the input stages; a tile waits there until its global offset is known, while the compute warps
+// go on with the next tiles.  A block claims RUNS of consecutive tiles: only the first tile of a run needs a
+// look-back (the others add the run's local prefix), and once the run's offset is known the later tiles publish
+// their inclusive prefix directly.  The look-back warp requests LB = 8 windows (256 tile states) per round trip:
+// under a saturated memory system one round trip costs more than a microsecond (measured), and at B200 rates a
+// 32-state window never catches up with the tiles in flight.
 //
-// Tile ids are handed out by an atomic counter, NS tiles ahead per block; a block processes its claims in
-// increasing order, so the smallest unpublished tile is always held by a running block (forward progress).
+// Tile ids are handed out by an atomic counter; a block processes its claims in increasing order, so the smallest
+// unpublished tile is always held by a running block (forward progress).
 // Tile state word: [63:62] flag (1 aggregate, 2 inclusive prefix) | [61:40] launch epoch | [39:0] count.
 #ifndef SG_FILTER_CUH_
 #define SG_FILTER_CUH_
@@ -36,7 +37,13 @@ namespace sgk {
 
 constexpr unsigned long long ST_AGG = 1ull << 62, ST_INC = 2ull << 62, ST_FLAGS = 3ull << 62;
 constexpr unsigned long long ST_VAL = (1ull << 40) - 1;
-constexpr int LB = 8;       // look-back windows (of 32 tile states) requested per round trip
+constexpr int LB = 8;               // look-back windows (of 32 tile states) requested per round trip
+constexpr int FILTER_THREADS = BLOCK + 32;
+constexpr int F_CHUNKS = 8;         // 16-byte chunks per thread per tile: one 128-byte row
+constexpr int F_TILE_BYTES = BLOCK * F_CHUNKS * 16;     // 32 KiB per staged input
+constexpr int RUN = 4;              // consecutive tiles a block claims at once; one look-back per run
+constexpr int NR = 4;               // runs of one block whose offset may be outstanding (ring of run slots)
+constexpr int NP = 8;               // tiles of one block that may wait for their global offset (<= (NR-1)*RUN)
 
 __device__ __forceinline__ unsigned long long ld_state(const unsigned long long* p) {
     unsigned long long v;
@@ -46,71 +53,108 @@ __device__ __forceinline__ unsigned long long ld_state(const unsigned long long*
 __device__ __forceinline__ void st_state(unsigned long long* p, unsigned long long v) {
     asm volatile("st.relaxed.gpu.global.u64 [%0], %1;" ::"l"(p), "l"(v) : "memory");
 }
+// byte offset, inside a staged tile, of 16-byte chunk j of row r (128-byte swizzle)
+__device__ __forceinline__ uint32_t swz(uint32_t r, uint32_t j) { return r * 128u + ((j ^ (r & 7u)) << 4); }
 
-// load modes of one step: guarded element loads (ragged / misaligned), 128-bit global loads, shared-memory stage
-enum { FM_GUARDED = 0, FM_GLOBAL = 1, FM_STAGED = 2 };
-
-// ---- evaluators: produce, for the FW elements at index i, the candidate values and the keep bits ----------
+// ---- evaluators: produce, for the FW elements of one chunk starting at index i, the candidate values and keep bits ----
 template <class P> struct FilterTemplateEval {
     typedef Meta1D<P> M;
     typedef typename M::T T;
+    typedef typename M::VEC VEC;
     static constexpr int NOUT = M::NOUT;
-    static constexpr int FW = 16 / (int)sizeof(T);       // elements per thread per step (one 128-bit access)
-    static constexpr int count_vec() {
+    static constexpr int FW = 16 / (int)sizeof(T);       // elements per 16-byte chunk
+    static constexpr int EPT = F_CHUNKS * FW;            // elements per thread per tile
+    static constexpr int TILE = BLOCK * EPT;
+    static constexpr int RC = TILE;                      // elements of the compaction ring (a power of two, >= one tile)
+    static constexpr int NS = 2;                         // input stages
+    __host__ __device__ static constexpr int count_vec() {
         int n = 0;
         for (int k = 0; k < M::S.n_in; ++k) n += (P::prog.in[k].kind == IN_VEC);
         return n;
     }
-    static constexpr int NVEC_REAL = count_vec();
-    static constexpr int U = NVEC_REAL <= 1 ? 4 * P::unroll : 4;     // steps per tile: 16 KiB per step-quadruple and input
-    static constexpr int TILE = BLOCK * U * FW;
-    static constexpr int NS = P::row_unroll >= 2 && P::row_unroll <= 3 ? P::row_unroll : 2;   // input stages
-    static constexpr int RC = TILE;                      // elements of the compaction ring (a power of two, >= one tile)
-    static constexpr bool STAGED = NVEC_REAL >= 1 && (size_t)(NS * NVEC_REAL + 1) * TILE * sizeof(T) <= 200 * 1024;
-    static constexpr int NVEC = STAGED ? NVEC_REAL : 1;
-    static constexpr size_t STAGE_BYTES = STAGED ? (size_t)NS * NVEC * TILE * sizeof(T) : 0;
+    static constexpr int NSTG = count_vec() < SG_MAX_TMAP ? count_vec() : SG_MAX_TMAP;   // inputs staged through shared memory (the rest: element loads)
+    static constexpr size_t STAGE_BYTES = (size_t)NS * NSTG * F_TILE_BYTES;
     static constexpr size_t SMEM = STAGE_BYTES + (size_t)RC * sizeof(T) + NS * sizeof(uint64_t);
-    static_assert((U & (U - 1)) == 0, "filter tile must be a power of two");
-    // index of the OUT_FILTER output; reductions over exactly the kept values (same source register, same predicate) are
-    // accumulated when the compacted values are copied out — one visit per KEPT element instead of one per element
+    __host__ __device__ static constexpr int vec_slot(int K) {      // index of IN_VEC input K among the IN_VEC inputs
+        int n = 0;
+        for (int k = 0; k < K; ++k) n += (P::prog.in[k].kind == IN_VEC);
+        return n;
+    }
+    __host__ __device__ static constexpr bool staged_input(int K) { return P::prog.in[K].kind == IN_VEC && vec_slot(K) < NSTG; }
     __host__ __device__ static constexpr int filter_out() {
         for (int o = 0; o < M::S.n_out; ++o)
             if (P::prog.out[o].kind == OUT_FILTER) return o;
         return 0;
     }
+    // reductions over exactly the kept values (same source register, same predicate as the filter) are accumulated when
+    // the compacted values are copied out: one visit per KEPT element instead of one per element
     __host__ __device__ static constexpr bool kept_reduction(int O) {
         const SgOut f = P::prog.out[filter_out()], out = P::prog.out[O];
         return (out.kind == OUT_SUM || out.kind == OUT_MAX || out.kind == OUT_MIN) && out.src == f.src && out.pred == f.pred;
     }
+    template <int O>
+    __device__ __forceinline__ static void accum_kept_o(T x, Cell (&acc)[NOUT]) {
+        constexpr SgOut out = P::prog.out[O];
+        if constexpr (kept_reduction(O)) cell_accum_value<T>(out.kind, acc[O], x);
+    }
     template <int... O>
     __device__ __forceinline__ static void accum_kept_(T x, Cell (&acc)[NOUT], std::integer_sequence<int, O...>) {
-        ((kept_reduction(O) ? cell_accum_value<T>(P::prog.out[O].kind, acc[O], x) : (void)0), ...);
+        (accum_kept_o<O>(x, acc), ...);
     }
     __device__ __forceinline__ static void accum_kept(const SgProg*, T x, Cell (&acc)[NOUT]) {
         accum_kept_(x, acc, std::make_integer_sequence<int, M::S.n_out>{});
     }
-    __host__ __device__ static constexpr int vec_slot(int K) {
-        int n = 0;
-        for (int k = 0; k < K; ++k) n += (P::prog.in[k].kind == IN_VEC);
-        return n;
-    }
 
-    // thread 0: one bulk copy per IN_VEC input for tile t into stage buffer `dst` ([NVEC][TILE])
+    // thread 0: one TMA tensor copy per staged input: rows [row0, row0+256) -> stage (shared-window address)
+    template <int K>
+    __device__ __forceinline__ static void issue_k(const SgArgs& a, int row0, uint32_t stage, uint64_t* bar) {
+        if constexpr (staged_input(K)) {
+            constexpr int slot = vec_slot(K);
+            tma_load_2d(stage + (uint32_t)slot * F_TILE_BYTES, a.tmap[slot], 0, row0, bar);
+        }
+    }
     template <int... K>
-    __device__ __forceinline__ static void issue_(const SgArgs& a, int64_t tbase, T* dst, uint64_t* bar, std::integer_sequence<int, K...>) {
-        mbar_expect_tx(bar, (uint32_t)(NVEC_REAL * TILE * sizeof(T)));
-        ((P::prog.in[K].kind == IN_VEC
-              ? bulk_g2s(dst + (size_t)vec_slot(K) * TILE, reinterpret_cast<const T*>(a.in_ptr[K]) + tbase, (uint32_t)(TILE * sizeof(T)), bar)
-              : (void)0),
-         ...);
+    __device__ __forceinline__ static void issue_(const SgArgs& a, int row0, uint32_t stage, uint64_t* bar, std::integer_sequence<int, K...>) {
+        mbar_expect_tx(bar, (uint32_t)(NSTG * F_TILE_BYTES));
+        (issue_k<K>(a, row0, stage, bar), ...);
     }
-    __device__ __forceinline__ static void issue(const SgProg*, const SgArgs& a, int64_t tbase, T* dst, uint64_t* bar) {
-        issue_(a, tbase, dst, bar, std::make_integer_sequence<int, M::S.n_in>{});
+    __device__ __forceinline__ static void issue(const SgProg*, const SgArgs& a, int row0, uint32_t stage, uint64_t* bar) {
+        issue_(a, row0, stage, bar, std::make_integer_sequence<int, M::S.n_in>{});
+    }
+    // all compute threads: cooperative fill of the staged inputs of one tile (coalesced, guarded), same swizzled layout
+    template <int K>
+    __device__ __forceinline__ static void fill_k(const SgArgs& a, int64_t tbase, unsigned char* stage) {
+        if constexpr (staged_input(K)) {
+            constexpr int slot = vec_slot(K);
+            unsigned char* dstb = stage + (size_t)slot * F_TILE_BYTES;
+            const T* src = reinterpret_cast<const T*>(a.in_ptr[K]);
+            const bool vec = (a.vec_ok >> 31) & 1;                  // every vector operand 16-byte aligned
+#pragma unroll
+            for (int q = 0; q < F_CHUNKS; ++q) {
+                const int c = threadIdx.x + BLOCK * q;              // chunk of the tile, in memory order
+                const int64_t i = tbase + (int64_t)c * FW;
+                VEC w;
+                T* we = reinterpret_cast<T*>(&w);
+                if (vec && i + FW <= a.in_len[K]) w = ld_stream(reinterpret_cast<const VEC*>(src + i));
+                else {
+#pragma unroll
+                    for (int e = 0; e < FW; ++e) we[e] = load_elem<T>(IN_VEC, 0, K, a, i + e);
+                }
+                *reinterpret_cast<VEC*>(dstb + swz((uint32_t)c >> 3, (uint32_t)c & 7u)) = w;
+            }
+        }
+    }
+    template <int... K>
+    __device__ __forceinline__ static void fill_(const SgArgs& a, int64_t tbase, unsigned char* stage, std::integer_sequence<int, K...>) {
+        (fill_k<K>(a, tbase, stage), ...);
+    }
+    __device__ __forceinline__ static void fill(const SgProg*, const SgArgs& a, int64_t tbase, unsigned char* stage) {
+        fill_(a, tbase, stage, std::make_integer_sequence<int, M::S.n_in>{});
     }
 
-    template <int MODE, int K>
-    __device__ __forceinline__ static void load_k(T (&v)[M::NV][FW], bool (&p)[M::NP][FW], const SgArgs& a, int64_t i, const T* stage, int toff) {
-        typedef typename M::VEC VEC;
+    // one chunk: FW consecutive elements starting at index i; staged inputs come from the stage at byte offset choff
+    template <bool GUARDED, int K>
+    __device__ __forceinline__ static void load_k(T (&v)[M::NV][FW], bool (&p)[M::NP][FW], const SgArgs& a, int64_t i, const unsigned char* stage, uint32_t choff) {
         constexpr SgIn in = P::prog.in[K];
         if constexpr (in.kind == IN_SCALAR || in.kind == IN_IMM) {
             T s = load_elem<T>(in.kind, in.ref, K, a, 0);
@@ -119,10 +163,9 @@ template <class P> struct FilterTemplateEval {
         } else if constexpr (in.kind == IN_BOOLVEC) {
 #pragma unroll
             for (int e = 0; e < FW; ++e) p[in.reg][e] = (i + e < a.in_len[K]) && reinterpret_cast<const volatile uint8_t*>(a.in_ptr[K])[i + e] != 0;
-        } else if constexpr (in.kind == IN_VEC && MODE != FM_GUARDED) {
-            VEC w;
-            if constexpr (MODE == FM_STAGED) w = *reinterpret_cast<const VEC*>(stage + (size_t)vec_slot(K) * TILE + toff);
-            else w = ld_stream(reinterpret_cast<const VEC*>(reinterpret_cast<const T*>(a.in_ptr[K]) + i));
+        } else if constexpr (staged_input(K)) {
+            constexpr int slot = vec_slot(K);
+            const VEC w = *reinterpret_cast<const VEC*>(stage + (size_t)slot * F_TILE_BYTES + choff);
             const T* we = reinterpret_cast<const T*>(&w);
 #pragma unroll
             for (int e = 0; e < FW; ++e) v[in.reg][e] = we[e];
@@ -131,13 +174,13 @@ template <class P> struct FilterTemplateEval {
             for (int e = 0; e < FW; ++e) v[in.reg][e] = load_elem<T>(in.kind, in.ref, K, a, i + e);
         }
     }
-    template <int MODE, int O>
+    template <bool GUARDED, int O>
     __device__ __forceinline__ static void out_o(T (&v)[M::NV][FW], bool (&p)[M::NP][FW], const SgArgs& a, int64_t i, T (&val)[FW],
                                                  unsigned int& keep, Cell (&acc)[NOUT]) {
         constexpr SgOut out = P::prog.out[O];
 #pragma unroll
         for (int e = 0; e < FW; ++e) {
-            const bool in_range = (MODE != FM_GUARDED) || (i + e < a.out_len[O]);     // full tiles lie inside every output's length
+            const bool in_range = !GUARDED || (i + e < a.out_len[O]);       // full tiles lie inside every output's length
             if constexpr (out.kind == OUT_FILTER) {
                 val[e] = v[out.src][e];
                 keep |= (unsigned int)(in_range && p[out.pred][e]) << e;
@@ -147,28 +190,26 @@ template <class P> struct FilterTemplateEval {
                 // accumulated at copy-out (accum_kept)
             } else if constexpr (out_is_reduction(out.kind)) {
                 if constexpr (out.pred == SG_NO_PRED) { if (in_range) cell_accum_value<T>(out.kind, acc[O], v[out.src][e]); }
-                else if constexpr (out.kind == OUT_SUM && !Traits<T>::is_float) {
-                    // masked integer sum as one widening multiply-add: acc += x * (0 or 1)
-                    acc[O].a += (unsigned long long)((long long)v[out.src][e] * (long long)(int)(in_range && p[out.pred][e]));
-                } else { if (in_range && p[out.pred][e]) cell_accum_value<T>(out.kind, acc[O], v[out.src][e]); }
+                else { if (in_range && p[out.pred][e]) cell_accum_value<T>(out.kind, acc[O], v[out.src][e]); }
             }
         }
     }
-    template <int MODE, int... K, int... I, int... O>
-    __device__ __forceinline__ static void run_(const SgArgs& a, int64_t i, const T* stage, int toff, T (&val)[FW], unsigned int& keep, Cell (&acc)[NOUT],
-                                                std::integer_sequence<int, K...>, std::integer_sequence<int, I...> is, std::integer_sequence<int, O...>) {
+    template <bool GUARDED, int... K, int... I, int... O>
+    __device__ __forceinline__ static void run_(const SgArgs& a, int64_t i, const unsigned char* stage, uint32_t choff, T (&val)[FW], unsigned int& keep,
+                                                Cell (&acc)[NOUT], std::integer_sequence<int, K...>, std::integer_sequence<int, I...> is,
+                                                std::integer_sequence<int, O...>) {
         T v[M::NV][FW];
         bool p[M::NP][FW];
-        (load_k<MODE, K>(v, p, a, i, stage, toff), ...);
+        (load_k<GUARDED, K>(v, p, a, i, stage, choff), ...);
         exec_body<P, T, M::NV, M::NP, FW>(v, p, a, is);
         keep = 0;
-        (out_o<MODE, O>(v, p, a, i, val, keep, acc), ...);
+        (out_o<GUARDED, O>(v, p, a, i, val, keep, acc), ...);
     }
-    template <int MODE>
-    __device__ __forceinline__ static void run(const SgProg*, const SgArgs& a, int64_t i, const T* stage, int toff, T (&val)[FW], unsigned int& keep,
-                                               Cell (&acc)[NOUT]) {
-        run_<MODE>(a, i, stage, toff, val, keep, acc, std::make_integer_sequence<int, M::S.n_in>{}, std::make_integer_sequence<int, M::S.n_instr>{},
-                   std::make_integer_sequence<int, M::S.n_out>{});
+    template <bool GUARDED>
+    __device__ __forceinline__ static void run(const SgProg*, const SgArgs& a, int64_t i, const unsigned char* stage, uint32_t choff, T (&val)[FW],
+                                               unsigned int& keep, Cell (&acc)[NOUT]) {
+        run_<GUARDED>(a, i, stage, choff, val, keep, acc, std::make_integer_sequence<int, M::S.n_in>{}, std::make_integer_sequence<int, M::S.n_instr>{},
+                      std::make_integer_sequence<int, M::S.n_out>{});
     }
     __device__ __forceinline__ static uint8_t out_kind(const SgProg*, int o) {
         constexpr SgProg g = P::prog;
@@ -176,21 +217,22 @@ template <class P> struct FilterTemplateEval {
     }
 };
 
+// bytecode evaluator: nothing is staged (every operand is loaded per chunk from global memory); same tile geometry
 template <class TT> struct FilterBytecodeEval {
     typedef TT T;
     static constexpr int NOUT = SG_MAX_OUT;
-    static constexpr int U = 4;                          // steps per tile
-    static constexpr int FW = 16 / (int)sizeof(T);       // elements per thread per step (one 128-bit access)
-    static constexpr int TILE = BLOCK * U * FW;
-    static constexpr int NVEC = 1, NS = 2, RC = TILE;
-    static constexpr bool STAGED = false;
+    static constexpr int FW = 16 / (int)sizeof(T);
+    static constexpr int EPT = F_CHUNKS * FW;
+    static constexpr int TILE = BLOCK * EPT;
+    static constexpr int RC = TILE, NS = 2, NSTG = 0;
     static constexpr size_t STAGE_BYTES = 0;
     static constexpr size_t SMEM = (size_t)RC * sizeof(T) + NS * sizeof(uint64_t);
-    __device__ __forceinline__ static void issue(const SgProg*, const SgArgs&, int64_t, T*, uint64_t*) {}
+    __device__ __forceinline__ static void issue(const SgProg*, const SgArgs&, int, uint32_t, uint64_t*) {}
+    __device__ __forceinline__ static void fill(const SgProg*, const SgArgs&, int64_t, unsigned char*) {}
     __device__ __forceinline__ static void accum_kept(const SgProg*, T, Cell (&)[NOUT]) {}      // masked reductions are accumulated per element
-    template <int MODE>
-    __device__ __forceinline__ static void run(const SgProg* g, const SgArgs& a, int64_t i, const T*, int, T (&val)[FW], unsigned int& keep, Cell (&acc)[NOUT]) {
-        const bool full = MODE != FM_GUARDED;
+    template <bool GUARDED>
+    __device__ __forceinline__ static void run(const SgProg* g, const SgArgs& a, int64_t i, const unsigned char*, uint32_t, T (&val)[FW], unsigned int& keep,
+                                               Cell (&acc)[NOUT]) {
         VmRegs<T, FW> rf;
         unsigned int pf = 0;
         for (int k = 0; k < g->shape.n_in; ++k) {
@@ -201,7 +243,7 @@ template <class TT> struct FilterBytecodeEval {
 #pragma unroll
                 for (int e = 0; e < FW; ++e) x[e] = s;
                 rf.put(in.reg, x);
-            } else vm_load<T, FW>(*g, a, k, i, full, rf, pf);
+            } else vm_load<T, FW>(*g, a, k, i, !GUARDED && ((a.vec_ok >> 31) & 1), rf, pf);
         }
         vm_exec<T, FW>(*g, rf, pf);
         keep = 0;
@@ -217,29 +259,6 @@ template <class TT> struct FilterBytecodeEval {
     }
     __device__ __forceinline__ static uint8_t out_kind(const SgProg* g, int o) { return o < g->shape.n_out ? g->out[o].kind : (uint8_t)OUT_STORE; }
 };
-
-// ---- the kernel body -------------------------------------------------------------------------------------
-// Warp-specialised block of FILTER_THREADS = BLOCK + 32 threads:
-//   warps 0..7 (compute): wait for the stage -> evaluate -> ballot ranks -> named barrier -> thread 0 hands
-//       {tile id, tile total} to the look-back warp and refills the stage freed in the previous iteration; every
-//       warp scatters its kept items in place (tile-local order) -> wait for the PREVIOUS tile's global offset ->
-//       coalesced copy-out of the previous tile.  One barrier per tile; nothing here waits for another block.
-//   warp 8 (look-back): publishes the tile's aggregate at once, then polls LB windows (256 tile states) per round
-//       trip until it finds an inclusive prefix, publishes the tile's inclusive prefix and posts the offset.
-//       It has a whole tile time to do so before the compute warps need the offset.
-template <class EV, int MODE>
-__device__ __forceinline__ void filter_eval_tile(const SgProg* g, const SgArgs& a, int64_t tbase, const typename EV::T* stage,
-                                                 typename EV::T (&val)[EV::U][EV::FW], unsigned int (&keep)[EV::U], Cell (&acc)[EV::NOUT]) {
-    constexpr int U = EV::U, FW = EV::FW;
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-#pragma unroll
-    for (int u = 0; u < U; ++u) {
-        const int toff = warp * (U * 32 * FW) + u * (32 * FW) + lane * FW;
-        EV::template run<MODE>(g, a, tbase + toff, stage, toff, val[u], keep[u], acc);
-    }
-}
-
-constexpr int FILTER_THREADS = BLOCK + 32;
 
 // look-back warp: exclusive prefix of `tile` (sum of the kept counts of all tiles before it).  The tile's AGGREGATE has
 // already been published by the compute warps — at once, so that no other block's look-back waits for this warp's backlog.
@@ -284,17 +303,15 @@ __device__ __forceinline__ unsigned long long filter_lookback(unsigned long long
 }
 
 
-constexpr int RUN = 4;      // consecutive tiles a block claims at once; one look-back per run
-constexpr int NR = 4;       // runs of one block whose offset may be outstanding (ring of run slots)
-constexpr int NP = 8;       // tiles of one block that may wait for their global offset (<= (NR-1)*RUN)
 
+// ---- the kernel body -------------------------------------------------------------------------------------
 template <class EV>
 __device__ __forceinline__ void filter_body(const SgProg* g, const SgArgs& a) {
     typedef typename EV::T T;
-    constexpr int U = EV::U, FW = EV::FW, TILE = EV::TILE, NOUT = EV::NOUT, NS = EV::NS, NVEC = EV::NVEC, RC = EV::RC;
+    constexpr int FW = EV::FW, EPT = EV::EPT, TILE = EV::TILE, NOUT = EV::NOUT, NS = EV::NS, NSTG = EV::NSTG, RC = EV::RC;
     static_assert(NP <= (NR - 1) * RUN, "a run slot must not be reused while one of its tiles is pending");
-    extern __shared__ __align__(128) unsigned char dyn_smem[];
-    T* const stage_base = reinterpret_cast<T*>(dyn_smem);                                   // [NS][NVEC][TILE] (staged instances)
+    extern __shared__ __align__(1024) unsigned char dyn_smem[];
+    unsigned char* const stage_base = dyn_smem;                                             // [NS][NSTG][F_TILE_BYTES], 1024-byte aligned (swizzle)
     const uint32_t ring = smem_u32(dyn_smem + EV::STAGE_BYTES);                             // [RC] compacted values awaiting their offset (shared-window address)
     uint64_t* const full_bar = reinterpret_cast<uint64_t*>(dyn_smem + EV::STAGE_BYTES + (size_t)RC * sizeof(T));
     __shared__ int s_tile[NS + 1];                      // tile id of iteration it at [it % (NS+1)]
@@ -310,7 +327,6 @@ __device__ __forceinline__ void filter_body(const SgProg* g, const SgArgs& a) {
     __shared__ uint64_t run_posted[NR], run_resolved[NR];   // mbarriers, one arrival each
 
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const unsigned int lt_mask = (1u << lane) - 1u;
     Cell acc[NOUT];
     uint8_t kind[NOUT];
     int fo = 0;     // index of the OUT_FILTER output
@@ -324,8 +340,7 @@ __device__ __forceinline__ void filter_body(const SgProg* g, const SgArgs& a) {
     const long long cap = a.out_cap[fo];
     unsigned long long* const state = a.tile_state;
     const unsigned long long ep = ((unsigned long long)(a.epoch & 0x3fffffu)) << 40;
-    const bool all_vec = (a.vec_ok >> 31) & 1;
-    const bool staged = EV::STAGED && all_vec;
+    const bool use_tma = NSTG > 0 && ((a.vec_ok >> 30) & 1);       // tensor maps encoded: 16-byte aligned inputs, >= 1 full tile
 
     if (a.n_tiles == 0 && blockIdx.x == 0 && threadIdx.x == 0) *reinterpret_cast<long long*>(a.out_aux[fo]) = 0;
 
@@ -340,13 +355,12 @@ __device__ __forceinline__ void filter_body(const SgProg* g, const SgArgs& a) {
             mbar_init(&run_posted[r], 1);
             mbar_init(&run_resolved[r], 1);
         }
-        if (staged)
-            for (int s = 0; s < NS; ++s) mbar_init(&full_bar[s], 1);
+        for (int s = 0; s < NS; ++s) mbar_init(&full_bar[s], 1);
         mbar_fence_init();
-        for (int s = 0; s < NS; ++s) {          // the first NS tiles: their bulk copies are in flight before the first one is touched
+        for (int s = 0; s < NS; ++s) {          // the first NS tiles: their copies are in flight before the first one is touched
             const int t = next_tile();
             s_tile[s] = t;
-            if (staged && t < a.n_full_tiles) EV::issue(g, a, (int64_t)t * TILE, stage_base + (size_t)s * NVEC * TILE, &full_bar[s]);
+            if (use_tma && t < a.n_full_tiles) EV::issue(g, a, t * BLOCK, smem_u32(stage_base + (size_t)s * NSTG * F_TILE_BYTES), &full_bar[s]);
         }
     }
     __syncthreads();
@@ -371,7 +385,7 @@ __device__ __forceinline__ void filter_body(const SgProg* g, const SgArgs& a) {
         // thread tracks the same queue state in registers.  A tile's offset = its run's offset + the kept counts of the
         // run's earlier tiles (local prefix), so only the FIRST tile of a run needs a look-back; once the run's offset is
         // known, later tiles of the run publish their INCLUSIVE prefix directly — other blocks' look-backs end there.
-        int q_head = 0, q_count = 0, n_tiles_done = 0;
+        int q_head = 0, q_count = 0;
         unsigned int ring_head = 0, ring_tail = 0;
         int run_no = -1;                        // number of the current run of this block
         unsigned int run_lpre = 0;              // kept count of the current run's earlier tiles
@@ -401,36 +415,40 @@ __device__ __forceinline__ void filter_body(const SgProg* g, const SgArgs& a) {
             if (tile % RUN == 0) { ++run_no; run_lpre = 0; }
             const int rs = run_no % NR;
             // thread 0 fetches the tile of iteration it+NS now (a new run costs one atomic, whose latency hides behind the
-            // evaluation), makes the id visible before this iteration's barrier, and issues its bulk copy right after the
-            // barrier into THIS stage, which every thread has read into registers by then
+            // evaluation), makes the id visible before this iteration's barrier, and issues its copy right after the barrier
+            // into THIS stage, which every thread has read into registers by then
             int t_next = 0x7fffffff;
             if (threadIdx.x == 0) t_next = next_tile();
 
-            T val[U][FW];
-            unsigned int keep[U], off[U];
-            unsigned int running = 0;
-            {
-                const int64_t tbase = (int64_t)tile * TILE;
-                const bool full = all_vec && tile < a.n_full_tiles;  // inside every operand's and output's length
-                const T* const stg = stage_base + (size_t)s * NVEC * TILE;
-                if (staged && full) {
-                    mbar_wait(&full_bar[s], (uint32_t)((it / NS) & 1));
-                    filter_eval_tile<EV, FM_STAGED>(g, a, tbase, stg, val, keep, acc);
-                } else if (full) {
-                    filter_eval_tile<EV, FM_GLOBAL>(g, a, tbase, stg, val, keep, acc);
-                } else {
-                    filter_eval_tile<EV, FM_GUARDED>(g, a, tbase, stg, val, keep, acc);
+            const int64_t tbase = (int64_t)tile * TILE;
+            const bool full = tile < a.n_full_tiles;            // inside every operand's and output's length: no range checks
+            unsigned char* const stg = stage_base + (size_t)s * NSTG * F_TILE_BYTES;
+            if (NSTG > 0) {
+                if (use_tma && full) mbar_wait(&full_bar[s], (uint32_t)((it / NS) & 1));
+                else {
+                    EV::fill(g, a, tbase, stg);
+                    named_bar_sync<2, BLOCK>();
                 }
             }
+            T val[F_CHUNKS][FW];
+            unsigned int mask = 0;                              // keep bits of this thread's EPT consecutive elements
 #pragma unroll
-            for (int u = 0; u < U; ++u) {
-                // exclusive prefix over lanes of the per-thread keep count (0..4) from three bit-plane ballots
-                const unsigned int c = __popc(keep[u]);
-                const unsigned int b0 = __ballot_sync(0xffffffffu, c & 1u), b1 = __ballot_sync(0xffffffffu, c & 2u), b2 = __ballot_sync(0xffffffffu, c & 4u);
-                off[u] = running + __popc(b0 & lt_mask) + 2 * __popc(b1 & lt_mask) + 4 * __popc(b2 & lt_mask);
-                running += __popc(b0) + 2 * __popc(b1) + 4 * __popc(b2);
+            for (int j = 0; j < F_CHUNKS; ++j) {
+                unsigned int kj;
+                const int64_t i = tbase + (int64_t)threadIdx.x * EPT + j * FW;
+                if (full) EV::template run<false>(g, a, i, stg, swz(threadIdx.x, j), val[j], kj, acc);
+                else EV::template run<true>(g, a, i, stg, swz(threadIdx.x, j), val[j], kj, acc);
+                mask |= kj << (j * FW);
             }
-            if (lane == 0) s_warp_total[it & 1][warp] = running;
+            // rank: the thread's elements are consecutive, so one popc and one warp scan order the tile
+            const unsigned int cnt = __popc(mask);
+            unsigned int incl = cnt;
+#pragma unroll
+            for (int d = 1; d < 32; d <<= 1) {
+                const unsigned int t = __shfl_up_sync(0xffffffffu, incl, d);
+                if (lane >= d) incl += t;
+            }
+            if (lane == 31) s_warp_total[it & 1][warp] = incl;
             bool run_known = false;         // thread 0: the current run's offset has been resolved already
             if (threadIdx.x == 0) {
                 s_tile[(it + NS) % (NS + 1)] = t_next;
@@ -465,9 +483,9 @@ __device__ __forceinline__ void filter_body(const SgProg* g, const SgArgs& a) {
                     s_r_total[rs] = tile_total;
                     mbar_arrive(&run_posted[rs]);
                 }
-                if (staged && t_next < a.n_full_tiles) {
+                if (use_tma && t_next < a.n_full_tiles) {
                     fence_proxy_async();
-                    EV::issue(g, a, (int64_t)t_next * TILE, stage_base + (size_t)s * NVEC * TILE, &full_bar[s]);
+                    EV::issue(g, a, t_next * BLOCK, smem_u32(stg), &full_bar[s]);
                 }
             }
             int copied = 0;
@@ -476,12 +494,13 @@ __device__ __forceinline__ void filter_body(const SgProg* g, const SgArgs& a) {
                 while (ring_head - ring_tail + tile_total > (unsigned int)RC) { copy_out_oldest(); ++copied; }
                 named_bar_sync<2, BLOCK>();
             }
+            {
+                unsigned int pos = ring_head + warp_excl + (incl - cnt);
 #pragma unroll
-            for (int u = 0; u < U; ++u) {
-                unsigned int pos = ring_head + warp_excl + off[u];
+                for (int j = 0; j < F_CHUNKS; ++j)
 #pragma unroll
-                for (int e = 0; e < FW; ++e)
-                    if ((keep[u] >> e) & 1u) sts_elem<T>(ring, (pos++) & (RC - 1), val[u][e]);
+                    for (int e = 0; e < FW; ++e)
+                        if ((mask >> (j * FW + e)) & 1u) sts_elem<T>(ring, (pos++) & (RC - 1), val[j][e]);
             }
             ring_head += tile_total;
             run_lpre += tile_total;
@@ -498,7 +517,6 @@ __device__ __forceinline__ void filter_body(const SgProg* g, const SgArgs& a) {
         named_bar_sync<1, BLOCK>();         // the last tile's queue entry (written by thread 0 after its barrier) is visible
         while (q_count > 0) copy_out_oldest();
         if (overflow) a.ctrl[3] = 1u;
-        (void)n_tiles_done;
     }
     epilogue_1d<T, NOUT>(acc, kind, a, true);
 }

@@ -1,6 +1,8 @@
 // sg_kernels.cu — kernel instantiation, the template registry and launch geometry (sm_100a).
 #include "sg_kernels.h"
 
+#include <cuda.h>
+
 #include <stdio.h>
 #include <string.h>
 
@@ -36,6 +38,45 @@ template <class P> constexpr int tile_of() {
     return BLOCK * Meta1D<P>::E;
 }
 
+// TMA tensor map of one filter input: the vector seen as `rows` rows of 128 bytes, box = 256 rows (one tile), 128-byte
+// swizzle (sg_filter.cuh).  The driver entry point is fetched once through the runtime (no link against libcuda).
+typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*, const cuuint32_t*,
+                                  const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+bool encode_filter_tmap(void* out128, const void* base, long rows) {
+    static EncodeTiledFn fn = nullptr;
+    static bool tried = false;
+    if (!tried) {
+        tried = true;
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult q;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess && q == cudaDriverEntryPointSuccess) fn = (EncodeTiledFn)p;
+        else cudaGetLastError();
+    }
+    if (!fn || rows <= 0 || rows > 0x7fffffffl) return false;
+    static_assert(sizeof(CUtensorMap) == 128, "tensor map size");
+    const cuuint64_t dims[2] = {32, (cuuint64_t)rows};
+    const cuuint64_t strides[1] = {128};
+    const cuuint32_t box[2] = {32, (cuuint32_t)BLOCK};
+    const cuuint32_t estr[2] = {1, 1};
+    alignas(64) CUtensorMap m;
+    if (fn(&m, CU_TENSOR_MAP_DATA_TYPE_UINT32, 2, const_cast<void*>(base), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+           CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
+        return false;
+    memcpy(out128, &m, 128);
+    return true;
+}
+template <class P> bool encode_filter_tmaps(SgArgs& a) {
+    typedef FilterTemplateEval<P> EV;
+    if (EV::NSTG == 0 || !((a.vec_ok >> 31) & 1) || a.n_full_tiles <= 0) return false;
+    int slot = 0;       // index among the IN_VEC inputs
+    for (int k = 0; k < P::prog.shape.n_in; ++k) {
+        if (P::prog.in[k].kind != IN_VEC) continue;
+        if (slot < EV::NSTG && !encode_filter_tmap(a.tmap[slot], a.in_ptr[k], (long)a.n_full_tiles * BLOCK)) return false;
+        ++slot;
+    }
+    return true;
+}
+
 template <class P> cudaError_t launch_template(const SgArgs& a, int grid, cudaStream_t s) {
     if constexpr ((P::prog.shape.flags & PF_2D) != 0) {
         static bool attr_set = false;
@@ -45,7 +86,10 @@ template <class P> cudaError_t launch_template(const SgArgs& a, int grid, cudaSt
     else if constexpr ((P::prog.shape.flags & PF_FILTER) != 0) {
         static bool attr_set = false;
         if (!attr_set) { cudaFuncSetAttribute(filter1d_template<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_of<P>()); attr_set = true; }
-        filter1d_template<P><<<grid, FILTER_THREADS, smem_of<P>(), s>>>(a);
+        SgArgs a2 = a;
+        a2.vec_ok &= ~(1 << 30);
+        if (encode_filter_tmaps<P>(a2)) a2.vec_ok |= (1 << 30);
+        filter1d_template<P><<<grid, FILTER_THREADS, smem_of<P>(), s>>>(a2);
     }
     else pass1d_template<P><<<grid, BLOCK, 0, s>>>(a);
     return cudaGetLastError();
@@ -199,7 +243,7 @@ int sgk_plan(const SgProg& prog, SgArgs& a, int force_bytecode, int sm_count, in
     }
 
     if (isfilter) {
-        const int tile = tid ? g_entries[tid].tile : BLOCK * 4 * (16 / es);
+        const int tile = tid ? g_entries[tid].tile : BLOCK * F_CHUNKS * (16 / es);
         const int occ = has_device ? (tid ? g_entries[tid].occupancy() : occupancy_bytecode(prog.shape.dtype, true)) : 4;
         const long n_tiles = (a.n + tile - 1) / tile;
         if (a.n >= (1ll << 40) || n_tiles > 0x7fffffffl) return fail(err, errcap, -9, "filter input too long for the tile-state word");

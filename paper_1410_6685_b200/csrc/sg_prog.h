@@ -59,6 +59,7 @@ enum : uint8_t {
 #define SG_MAX_VREG 24
 #define SG_MAX_PREG 8
 #define SG_NO_PRED 0xFF
+#define SG_MAX_TMAP 2
 
 struct SgInstr { uint8_t op, dst, a, b; };
 struct SgIn { uint8_t kind, ref, reg, pad; };      // reg: V (or P for IN_BOOLVEC) register the input is loaded into
@@ -104,6 +105,9 @@ struct SgArgs {
     int32_t n_strips, n_chunks;
     int64_t rows_per_chunk;
     int64_t ws_off[SG_MAX_OUT];     // 2-D: byte offset in workspace of the per-chunk (AXIS_COLS) / per-strip (AXIS_ROWS) partial cells
+    // FILTER: TMA tensor maps (CUtensorMap, 128 bytes each) of the staged inputs, encoded by the launcher: the input seen as
+    // rows of 128 bytes, box = 256 rows, 128-byte swizzle (sg_filter.cuh); vec_ok bit 30 says they are valid
+    alignas(64) unsigned char tmap[SG_MAX_TMAP][128];
 };
 
 #endif  // SG_PROG_H_
