@@ -55,6 +55,24 @@ template <class T> __device__ __forceinline__ T lds_elem(uint32_t base, uint32_t
     }
     return v;
 }
+// compaction append: if bit BIT of `mask` is set, store v at shared-window byte address `addr` and advance it —
+// a predicate-producing logic op, a predicated store and a predicated add (no branch)
+template <class T, int BIT> __device__ __forceinline__ void sts_append_if(uint32_t& addr, unsigned int mask, T v) {
+    if constexpr (sizeof(T) == 4) {
+        uint32_t w; memcpy(&w, &v, 4);
+        asm volatile("{\n.reg .pred p;\n.reg .b32 t;\nand.b32 t, %2, %3;\nsetp.ne.u32 p, t, 0;\n@p st.shared.b32 [%0], %1;\n@p add.u32 %0, %0, 4;\n}\n"
+                     : "+r"(addr) : "r"(w), "r"(mask), "n"(1u << BIT) : "memory");
+    } else {
+        unsigned long long w; memcpy(&w, &v, 8);
+        asm volatile("{\n.reg .pred p;\n.reg .b32 t;\nand.b32 t, %2, %3;\nsetp.ne.u32 p, t, 0;\n@p st.shared.b64 [%0], %1;\n@p add.u32 %0, %0, 8;\n}\n"
+                     : "+r"(addr) : "l"(w), "r"(mask), "n"(1u << BIT) : "memory");
+    }
+}
+// a value the compiler must keep in a register (it will not re-derive it at every use)
+__device__ __forceinline__ uint32_t pin_reg(uint32_t x) {
+    asm volatile("mov.b32 %0, %0;" : "+r"(x));
+    return x;
+}
 // non-blocking: has the phase with this parity completed?
 __device__ __forceinline__ bool mbar_test(uint64_t* bar, uint32_t parity) {
     uint32_t ok;

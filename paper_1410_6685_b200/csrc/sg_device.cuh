@@ -91,8 +91,8 @@ __device__ __forceinline__ int32_t magic_div_i32(int32_t x, unsigned long long m
     q += (int32_t)((uint32_t)q >> 31);
     return q;
 }
-__device__ __forceinline__ int32_t magic_mod_i32(int32_t x, int32_t d, unsigned long long mg) {
-    return (int32_t)((uint32_t)magic_div_i32(x, mg) * (0u - (uint32_t)d) + (uint32_t)x);      // one multiply-add: x - q*d
+__device__ __forceinline__ int32_t magic_mod_i32(int32_t x, uint32_t neg_d, unsigned long long mg) {
+    return (int32_t)((uint32_t)magic_div_i32(x, mg) * neg_d + (uint32_t)x);      // one multiply-add: x - q*d, neg_d = -d
 }
 
 // one value op; `op` is a compile-time constant in template instances and a warp-uniform value in the bytecode kernel

@@ -296,13 +296,19 @@ __device__ __forceinline__ unsigned long long filter_lookback(unsigned long long
         excl += x;
         if (done) break;
         look -= upto;       // go deeper, or poll again from the predecessor that has not published yet
-        if (p_inv < LB * 32) __nanosleep(400);      // stalled: do not hammer the state words (nor this SM's issue slots)
+        if (p_inv < LB * 32) __nanosleep(1000);     // stalled: do not hammer the state words (nor this SM's issue slots)
     }
     if (lane == 0) st_state(&state[tile], ST_INC | ep | (excl + tile_total));
     return excl;
 }
 
 
+
+// appends the kept elements of one thread's row (keep bits in `mask`, element k = val[k / FW][k % FW]) at `addr`
+template <class T, int FW, int... K>
+__device__ __forceinline__ void scatter_row(uint32_t& addr, unsigned int mask, T (&val)[F_CHUNKS][FW], std::integer_sequence<int, K...>) {
+    (sts_append_if<T, K>(addr, mask, val[K / FW][K % FW]), ...);
+}
 
 // ---- the kernel body -------------------------------------------------------------------------------------
 template <class EV>
@@ -312,7 +318,7 @@ __device__ __forceinline__ void filter_body(const SgProg* g, const SgArgs& a) {
     static_assert(NP <= (NR - 1) * RUN, "a run slot must not be reused while one of its tiles is pending");
     extern __shared__ __align__(1024) unsigned char dyn_smem[];
     unsigned char* const stage_base = dyn_smem;                                             // [NS][NSTG][F_TILE_BYTES], 1024-byte aligned (swizzle)
-    const uint32_t ring = smem_u32(dyn_smem + EV::STAGE_BYTES);                             // [RC] compacted values awaiting their offset (shared-window address)
+    const uint32_t ring = pin_reg(smem_u32(dyn_smem + EV::STAGE_BYTES));                             // [RC] compacted values awaiting their offset (shared-window address)
     uint64_t* const full_bar = reinterpret_cast<uint64_t*>(dyn_smem + EV::STAGE_BYTES + (size_t)RC * sizeof(T));
     __shared__ int s_tile[NS + 1];                      // tile id of iteration it at [it % (NS+1)]
     __shared__ unsigned int s_warp_total[2][WARPS];     // double-buffered: a warp may run one barrier ahead
@@ -495,12 +501,19 @@ __device__ __forceinline__ void filter_body(const SgProg* g, const SgArgs& a) {
                 named_bar_sync<2, BLOCK>();
             }
             {
-                unsigned int pos = ring_head + warp_excl + (incl - cnt);
+                const unsigned int pos = ring_head + warp_excl + (incl - cnt);
+                if (((ring_head & (RC - 1)) + tile_total) <= (unsigned int)RC) {
+                    // the tile does not wrap around the ring (uniform): plain appends
+                    uint32_t addr = ring + (pos & (RC - 1)) * (uint32_t)sizeof(T);
+                    scatter_row<T, FW>(addr, mask, val, std::make_integer_sequence<int, F_CHUNKS * FW>{});
+                } else {
+                    unsigned int q = pos;
 #pragma unroll
-                for (int j = 0; j < F_CHUNKS; ++j)
+                    for (int j = 0; j < F_CHUNKS; ++j)
 #pragma unroll
-                    for (int e = 0; e < FW; ++e)
-                        if ((mask >> (j * FW + e)) & 1u) sts_elem<T>(ring, (pos++) & (RC - 1), val[j][e]);
+                        for (int e = 0; e < FW; ++e)
+                            if ((mask >> (j * FW + e)) & 1u) sts_elem<T>(ring, (q++) & (RC - 1), val[j][e]);
+                }
             }
             ring_head += tile_total;
             run_lpre += tile_total;

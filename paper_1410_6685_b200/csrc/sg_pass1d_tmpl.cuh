@@ -40,9 +40,11 @@ __device__ __forceinline__ void exec_instr(T (&v)[NV][E], bool (&p)[NP][E], cons
         int32_t d;
         memcpy(&d, &a.imm[immk], 4);
         if (magic != 0) {       // |d| > 1 (uniform)
+            uint32_t neg_d = 0u - (uint32_t)d;
+            asm volatile("" : "+r"(neg_d));     // keep -d as the (uniform) multiplier: the remainder is ONE multiply-add per element
 #pragma unroll
             for (int e = 0; e < E; ++e)
-                v[ins.dst][e] = (T)(ins.op == OP_MOD ? magic_mod_i32((int32_t)v[ins.a][e], d, magic) : magic_div_i32((int32_t)v[ins.a][e], magic));
+                v[ins.dst][e] = (T)(ins.op == OP_MOD ? magic_mod_i32((int32_t)v[ins.a][e], neg_d, magic) : magic_div_i32((int32_t)v[ins.a][e], magic));
             return;
         }
     }
