@@ -68,11 +68,12 @@ const char* dt_name(uint8_t d) {
 }
 
 // Signed magic number for truncating int32 division by d, |d| >= 2 (multiply-high scheme; the device side is
-// magic_div_i32 in sg_device.cuh).  Returns 0 for |d| <= 1.
-uint64_t i32_magic(int32_t d) {
+// magic_div_i32 in sg_device.cuh).  valid == 0 for |d| <= 1.
+SgDiv i32_magic(int32_t d) {
+    SgDiv m{};
     const uint32_t two31 = 0x80000000u;
     const uint32_t ad = d < 0 ? 0u - (uint32_t)d : (uint32_t)d;
-    if (ad <= 1) return 0;
+    if (ad <= 1) return m;
     const uint32_t t = two31 + ((uint32_t)d >> 31);
     const uint32_t anc = t - 1 - t % ad;
     int p = 31;
@@ -87,8 +88,12 @@ uint64_t i32_magic(int32_t d) {
     } while (q1 < delta || (q1 == delta && r1 == 0));
     uint32_t M = q2 + 1;
     if (d < 0) M = 0u - M;
-    const int addsel = (d > 0 && (int32_t)M < 0) ? 1 : (d < 0 && (int32_t)M > 0) ? -1 : 0;
-    return (uint64_t)M | ((uint64_t)(uint32_t)(p - 32) << 32) | ((uint64_t)(uint32_t)(addsel + 1) << 40) | (1ull << 63);
+    m.M = (int32_t)M;
+    m.addsel = (d > 0 && (int32_t)M < 0) ? 1 : (d < 0 && (int32_t)M > 0) ? -1 : 0;
+    m.s = p - 32;
+    m.neg_d = (int32_t)(0u - (uint32_t)d);
+    m.valid = 1;
+    return m;
 }
 
 std::string dump_prog(const SgProg& g) {
@@ -327,7 +332,7 @@ sg_status sg_build_pass(sg_ctx* c, Pass& P, std::vector<char*>& temps, std::stri
         a.imm[k] = in.imm;
         if (in.kind == IN_IMM && dtype == SG_I32) {
             int32_t d; memcpy(&d, &in.imm, 4);
-            a.imm_magic[k] = i32_magic(d);
+            a.imm_div[k] = i32_magic(d);
         }
         // an input whose storage this pass also writes must not go through the read-only path
         if (in.ptr)

@@ -79,20 +79,16 @@ __device__ __forceinline__ long long p_abs(long long a) { return a < 0 ? (long l
 // int32 division / modulo by a pass-constant divisor d (|d| >= 2) with a host-computed signed magic number
 // (the classic multiply-high scheme for truncating signed division): q = mulhi(x, M) (+x or -x when the sign of
 // M differs from that of d), arithmetic shift by s, plus one if negative.  Exact for every int32 x; the
-// remainder x - q*d has the sign of the dividend (C semantics).  Packed word: [31:0] M, [39:32] s,
-// [41:40] add selector + 1, bit 63 = valid (0 => |d| <= 1, the generic path runs).
-__device__ __forceinline__ int32_t magic_div_i32(int32_t x, unsigned long long mg) {
-    const int32_t M = (int32_t)(uint32_t)mg;
-    const int s = (int)((mg >> 32) & 0xffu);
-    const uint32_t addsel = (uint32_t)((int)((mg >> 40) & 3u) - 1);
-    int32_t q = __mulhi(x, M);
-    q = (int32_t)((uint32_t)q + (uint32_t)x * addsel);
-    q >>= s;
+// remainder x - q*d has the sign of the dividend (C semantics).  The fields are kernel-parameter constants.
+__device__ __forceinline__ int32_t magic_div_i32(int32_t x, const SgDiv& m) {
+    int32_t q = __mulhi(x, m.M);
+    q = (int32_t)((uint32_t)q + (uint32_t)x * (uint32_t)m.addsel);
+    q >>= m.s;
     q += (int32_t)((uint32_t)q >> 31);
     return q;
 }
-__device__ __forceinline__ int32_t magic_mod_i32(int32_t x, uint32_t neg_d, unsigned long long mg) {
-    return (int32_t)((uint32_t)magic_div_i32(x, mg) * neg_d + (uint32_t)x);      // one multiply-add: x - q*d, neg_d = -d
+__device__ __forceinline__ int32_t magic_mod_i32(int32_t x, const SgDiv& m) {
+    return (int32_t)((uint32_t)magic_div_i32(x, m) * (uint32_t)m.neg_d + (uint32_t)x);      // one multiply-add: x - q*d
 }
 
 // one value op; `op` is a compile-time constant in template instances and a warp-uniform value in the bytecode kernel

@@ -268,10 +268,21 @@ __device__ __forceinline__ unsigned long long filter_lookback(unsigned long long
     int look = tile - 1;
     for (;;) {
         unsigned long long lbw[LB];
+        // cheap poll: wait until the nearest window has no unpublished state in front of its first inclusive prefix
+        for (;;) {
+            const int idx = look - lane;
+            lbw[0] = (idx >= 0) ? ld_state(&state[idx]) : (ST_INC | ep);    // virtual tile -1: inclusive prefix 0
+            const bool valid = ((lbw[0] & ST_FLAGS) != 0) && ((lbw[0] & (0x3fffffull << 40)) == ep);
+            const bool inc = valid && ((lbw[0] & ST_FLAGS) == ST_INC);
+            const unsigned int vmask = __ballot_sync(0xffffffffu, valid), imask = __ballot_sync(0xffffffffu, inc);
+            const unsigned int before_inc = imask ? ((imask & (0u - imask)) - 1u) : 0xffffffffu;    // lanes in front of the first inclusive prefix
+            if ((~vmask & before_inc) == 0u) break;
+            __nanosleep(500);       // a near predecessor has not published yet: do not hammer the state words (nor this SM's issue slots)
+        }
 #pragma unroll
-        for (int j = 0; j < LB; ++j) {
+        for (int j = 1; j < LB; ++j) {
             const int idx = look - lane - 32 * j;
-            lbw[j] = (idx >= 0) ? ld_state(&state[idx]) : (ST_INC | ep);    // virtual tile -1: inclusive prefix 0
+            lbw[j] = (idx >= 0) ? ld_state(&state[idx]) : (ST_INC | ep);
         }
         // ballots of all LB windows first (independent), then ONE position search and ONE warp sum
         int p_inc = LB * 32, p_inv = LB * 32;       // first inclusive prefix / first unpublished state, in (window, lane) order
@@ -296,7 +307,6 @@ __device__ __forceinline__ unsigned long long filter_lookback(unsigned long long
         excl += x;
         if (done) break;
         look -= upto;       // go deeper, or poll again from the predecessor that has not published yet
-        if (p_inv < LB * 32) __nanosleep(1000);     // stalled: do not hammer the state words (nor this SM's issue slots)
     }
     if (lane == 0) st_state(&state[tile], ST_INC | ep | (excl + tile_total));
     return excl;
@@ -402,11 +412,22 @@ __device__ __forceinline__ void filter_body(const SgProg* g, const SgArgs& a) {
             mbar_wait(&run_resolved[r % NR], (uint32_t)((r / NR) & 1));
             const unsigned int total = s_q_total[e];
             const long long base = (long long)(s_r_excl[r % NR] + s_q_lpre[e]);
-            for (unsigned int i = threadIdx.x; i < total; i += BLOCK) {
-                const long long pos = base + i;
-                const T v = lds_elem<T>(ring, (ring_tail + i) & (RC - 1));
-                EV::accum_kept(g, v, acc);
-                if (pos < cap) dst[pos] = v; else overflow = true;
+            const unsigned int r0 = ring_tail & (RC - 1);
+            if (base + (long long)total <= cap && r0 + total <= (unsigned int)RC) {
+                // common case (uniform): inside the output's capacity, no wrap-around in the ring
+                T* const d0 = dst + base;
+                for (unsigned int i = threadIdx.x; i < total; i += BLOCK) {
+                    const T v = lds_elem<T>(ring, r0 + i);
+                    EV::accum_kept(g, v, acc);
+                    d0[i] = v;
+                }
+            } else {
+                for (unsigned int i = threadIdx.x; i < total; i += BLOCK) {
+                    const long long pos = base + i;
+                    const T v = lds_elem<T>(ring, (ring_tail + i) & (RC - 1));
+                    EV::accum_kept(g, v, acc);
+                    if (pos < cap) dst[pos] = v; else overflow = true;
+                }
             }
             if (threadIdx.x == 0 && s_q_tile[e] == a.n_tiles - 1) *reinterpret_cast<long long*>(a.out_aux[fo]) = base + (long long)total;
             ring_tail += total;

@@ -36,15 +36,10 @@ __device__ __forceinline__ void exec_instr(T (&v)[NV][E], bool (&p)[NP][E], cons
     constexpr int immk = (ins.op == OP_MOD || ins.op == OP_DIV) ? imm_input_of_reg<P>(ins.b) : -1;
     if constexpr (immk >= 0 && sizeof(T) == 4 && !Traits<T>::is_float) {
         // x MOD d / x DIV d with an immediate divisor: multiply-high by the host-computed magic instead of dividing
-        const unsigned long long magic = a.imm_magic[immk];
-        int32_t d;
-        memcpy(&d, &a.imm[immk], 4);
-        if (magic != 0) {       // |d| > 1 (uniform)
-            uint32_t neg_d = 0u - (uint32_t)d;
-            asm volatile("" : "+r"(neg_d));     // keep -d as the (uniform) multiplier: the remainder is ONE multiply-add per element
+        if (a.imm_div[immk].valid) {        // |d| > 1 (uniform)
 #pragma unroll
             for (int e = 0; e < E; ++e)
-                v[ins.dst][e] = (T)(ins.op == OP_MOD ? magic_mod_i32((int32_t)v[ins.a][e], neg_d, magic) : magic_div_i32((int32_t)v[ins.a][e], magic));
+                v[ins.dst][e] = (T)(ins.op == OP_MOD ? magic_mod_i32((int32_t)v[ins.a][e], a.imm_div[immk]) : magic_div_i32((int32_t)v[ins.a][e], a.imm_div[immk]));
             return;
         }
     }

@@ -78,6 +78,9 @@ struct SgProg {
     SgOut out[SG_MAX_OUT];
 };
 
+// Truncating int32 division by a pass constant d, |d| >= 2: q = (mulhi(x, M) + x*addsel) >> s, plus one if negative.
+struct SgDiv { int32_t M, addsel, s, neg_d; uint32_t valid, pad[3]; };
+
 // Runtime arguments of one pass (never part of the signature).
 struct SgArgs {
     int64_t n;                      // 1-D: domain length; 2-D: rows
@@ -86,7 +89,7 @@ struct SgArgs {
     int64_t in_len[SG_MAX_IN];      // elements readable through the input (guards the ragged path)
     int64_t in_stride[SG_MAX_IN];   // IN_STRIDED: element stride; 2-D IN_VEC: leading dimension
     uint64_t imm[SG_MAX_IN];        // IN_IMM: raw bits of the immediate in the pass dtype
-    uint64_t imm_magic[SG_MAX_IN];  // IN_IMM, i32 passes: packed signed magic number for division/modulo by the immediate (0 if |d| <= 1), see magic_div_i32
+    SgDiv imm_div[SG_MAX_IN];       // IN_IMM, i32 passes: signed magic number for division/modulo by the immediate (valid == 0 if |d| <= 1), see magic_div_i32
     void* out_ptr[SG_MAX_OUT];      // STORE: buffer; reductions/quantifiers: 8-byte device scalar slot (AXIS_ALL) or vector
     int64_t out_len[SG_MAX_OUT];    // valid length of the output's source value (<= n); 2-D STORE: leading dimension
     int64_t out_cap[SG_MAX_OUT];    // FILTER: capacity in elements
