@@ -41,9 +41,9 @@ constexpr int LB = 8;               // look-back windows (of 32 tile states) req
 constexpr int FILTER_THREADS = BLOCK + 32;
 constexpr int F_CHUNKS = 8;         // 16-byte chunks per thread per tile: one 128-byte row
 constexpr int F_TILE_BYTES = BLOCK * F_CHUNKS * 16;     // 32 KiB per staged input
-constexpr int RUN = 4;              // consecutive tiles a block claims at once; one look-back per run
-constexpr int NR = 4;               // runs of one block whose offset may be outstanding (ring of run slots)
-constexpr int NP = 8;               // tiles of one block that may wait for their global offset (<= (NR-1)*RUN)
+constexpr int RUN = 4;              // consecutive tiles a block claims at once while few values are kept (else 1); one look-back per run
+constexpr int NR = 16;              // runs of one block whose offset may be outstanding (ring of run slots)
+constexpr int NP = 8;               // tiles of one block that may wait for their global offset (each may be a run of its own: NP < NR)
 
 __device__ __forceinline__ unsigned long long ld_state(const unsigned long long* p) {
     unsigned long long v;
@@ -325,7 +325,7 @@ template <class EV>
 __device__ __forceinline__ void filter_body(const SgProg* g, const SgArgs& a) {
     typedef typename EV::T T;
     constexpr int FW = EV::FW, EPT = EV::EPT, TILE = EV::TILE, NOUT = EV::NOUT, NS = EV::NS, NSTG = EV::NSTG, RC = EV::RC;
-    static_assert(NP <= (NR - 1) * RUN, "a run slot must not be reused while one of its tiles is pending");
+    static_assert(NP < NR, "a run slot must not be reused while one of its tiles is pending");
     extern __shared__ __align__(1024) unsigned char dyn_smem[];
     unsigned char* const stage_base = dyn_smem;                                             // [NS][NSTG][F_TILE_BYTES], 1024-byte aligned (swizzle)
     const uint32_t ring = pin_reg(smem_u32(dyn_smem + EV::STAGE_BYTES));                             // [RC] compacted values awaiting their offset (shared-window address)
@@ -360,11 +360,20 @@ __device__ __forceinline__ void filter_body(const SgProg* g, const SgArgs& a) {
 
     if (a.n_tiles == 0 && blockIdx.x == 0 && threadIdx.x == 0) *reinterpret_cast<long long*>(a.out_aux[fo]) = 0;
 
-    // thread 0 hands out this block's tile sequence: runs of RUN consecutive tiles claimed with one atomic each
-    int seq_base = 0, seq_j = RUN;              // thread 0 only: current run and position in it
+    // thread 0 hands out this block's tile sequence: runs of consecutive tiles claimed with one atomic each.  A run is RUN
+    // tiles while a run's kept values fit comfortably in the ring, else ONE tile: a tile that cannot enter the ring waits
+    // for its run's offset, and with long runs that wait would chain from block to block.  Entries: (tile << 1) | first-of-run.
+    int seq_base = 0, seq_j = 0, seq_len = 0;   // thread 0 only: current run, position in it, its length
+    unsigned int last_total = (unsigned int)RC; // thread 0 only: kept count of the latest tile (pessimistic until one is known)
     auto next_tile = [&]() -> int {             // thread 0 only
-        if (seq_j == RUN) { seq_base = (int)atomicAdd(&a.ctrl[2], (unsigned int)RUN); seq_j = 0; }
-        return seq_base + seq_j++;
+        if (seq_j == seq_len) {
+            seq_len = (last_total * (unsigned int)RUN * 2u <= (unsigned int)RC) ? RUN : 1;
+            seq_base = (int)atomicAdd(&a.ctrl[2], (unsigned int)seq_len);
+            seq_j = 0;
+        }
+        const int first = (seq_j == 0);
+        const int t = seq_base + seq_j++;
+        return t >= 0x3fffffff ? 0x7ffffffe : ((t << 1) | first);
     };
     if (threadIdx.x == 0) {
         for (int r = 0; r < NR; ++r) {
@@ -374,8 +383,9 @@ __device__ __forceinline__ void filter_body(const SgProg* g, const SgArgs& a) {
         for (int s = 0; s < NS; ++s) mbar_init(&full_bar[s], 1);
         mbar_fence_init();
         for (int s = 0; s < NS; ++s) {          // the first NS tiles: their copies are in flight before the first one is touched
-            const int t = next_tile();
-            s_tile[s] = t;
+            const int tv = next_tile();
+            s_tile[s] = tv;
+            const int t = tv >> 1;
             if (use_tma && t < a.n_full_tiles) EV::issue(g, a, t * BLOCK, smem_u32(stage_base + (size_t)s * NSTG * F_TILE_BYTES), &full_bar[s]);
         }
     }
@@ -437,15 +447,17 @@ __device__ __forceinline__ void filter_body(const SgProg* g, const SgArgs& a) {
         int it = 0;
         for (;; ++it) {
             const int s = it % NS;
-            const int tile = s_tile[it % (NS + 1)];
+            const int tv = s_tile[it % (NS + 1)];
+            const int tile = tv >> 1;
+            const bool first = tv & 1;          // first tile of a run
             if (tile >= a.n_tiles) break;
-            if (tile % RUN == 0) { ++run_no; run_lpre = 0; }
+            if (first) { ++run_no; run_lpre = 0; }
             const int rs = run_no % NR;
             // thread 0 fetches the tile of iteration it+NS now (a new run costs one atomic, whose latency hides behind the
             // evaluation), makes the id visible before this iteration's barrier, and issues its copy right after the barrier
             // into THIS stage, which every thread has read into registers by then
-            int t_next = 0x7fffffff;
-            if (threadIdx.x == 0) t_next = next_tile();
+            int tv_next = 0x7ffffffe;
+            if (threadIdx.x == 0) tv_next = next_tile();
 
             const int64_t tbase = (int64_t)tile * TILE;
             const bool full = tile < a.n_full_tiles;            // inside every operand's and output's length: no range checks
@@ -478,14 +490,14 @@ __device__ __forceinline__ void filter_body(const SgProg* g, const SgArgs& a) {
             if (lane == 31) s_warp_total[it & 1][warp] = incl;
             bool run_known = false;         // thread 0: the current run's offset has been resolved already
             if (threadIdx.x == 0) {
-                s_tile[(it + NS) % (NS + 1)] = t_next;
+                s_tile[(it + NS) % (NS + 1)] = tv_next;
                 int ready = 0;      // how many of the oldest pending tiles already have their offset (non-blocking poll)
                 for (; ready < q_count; ++ready) {
                     const int r = s_q_run[(q_head + ready) % NP];
                     if (!mbar_test(&run_resolved[r % NR], (uint32_t)((r / NR) & 1))) break;
                 }
                 s_ready[it & 1] = ready;
-                if (tile % RUN != 0) run_known = mbar_test(&run_resolved[rs], (uint32_t)((run_no / NR) & 1));
+                if (!first) run_known = mbar_test(&run_resolved[rs], (uint32_t)((run_no / NR) & 1));
             }
             named_bar_sync<1, BLOCK>();     // the stage is in registers; warp totals, next tile id and the ready count are visible
             unsigned int warp_excl = 0, tile_total = 0;
@@ -505,14 +517,15 @@ __device__ __forceinline__ void filter_body(const SgProg* g, const SgArgs& a) {
                 s_q_total[e] = tile_total;
                 s_q_lpre[e] = run_lpre;
                 s_q_run[e] = run_no;
-                if (tile % RUN == 0) {      // first tile of a run: hand it to the look-back warp
+                last_total = tile_total;
+                if (first) {                // first tile of a run: hand it to the look-back warp
                     s_r_tile[rs] = tile;
                     s_r_total[rs] = tile_total;
                     mbar_arrive(&run_posted[rs]);
                 }
-                if (use_tma && t_next < a.n_full_tiles) {
+                if (use_tma && (tv_next >> 1) < a.n_full_tiles) {
                     fence_proxy_async();
-                    EV::issue(g, a, t_next * BLOCK, smem_u32(stg), &full_bar[s]);
+                    EV::issue(g, a, (tv_next >> 1) * BLOCK, smem_u32(stg), &full_bar[s]);
                 }
             }
             int copied = 0;

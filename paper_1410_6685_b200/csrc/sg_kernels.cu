@@ -246,7 +246,7 @@ int sgk_plan(const SgProg& prog, SgArgs& a, int force_bytecode, int sm_count, in
         const int tile = tid ? g_entries[tid].tile : BLOCK * F_CHUNKS * (16 / es);
         const int occ = has_device ? (tid ? g_entries[tid].occupancy() : occupancy_bytecode(prog.shape.dtype, true)) : 4;
         const long n_tiles = (a.n + tile - 1) / tile;
-        if (a.n >= (1ll << 40) || n_tiles > 0x7fffffffl) return fail(err, errcap, -9, "filter input too long for the tile-state word");
+        if (a.n >= (1ll << 40) || n_tiles >= 0x3fffffffl) return fail(err, errcap, -9, "filter input too long for the tile-state word");
         a.n_tiles = (int)n_tiles;
         a.vec_ok = vec_ok | ((congruent && mis == 0) ? (1 << 31) : 0);
         // tiles that lie inside every vector operand's and every output's length take the unguarded (staged) path

@@ -346,6 +346,22 @@ def test_filter_mod_by_any_immediate_divisor(mode, modulus):
     assert bits_equal(kept, want["kept"])
 
 
+@pytest.mark.parametrize("modulus", [1, 2, 3])
+def test_filter_high_selectivity(modulus):
+    """All / half / a third of the values kept over 128 tiles: the compaction ring fills up, tiles wait for their offsets
+    (single-tile runs), the ring wraps around; order and count stay exact."""
+    n = (1 << 20) + 11
+    x = inputs.uniform_i31(3, 7, n)
+    want = ocfg.cfg2(x, modulus, 0)
+    with Ctx() as c:
+        tx = c.torch.from_numpy(x).cuda()
+        r = W.cfg2(c.ctx, n, tx.data_ptr(), modulus=modulus, residue=0)
+        cnt, s = c.get(r["count"]), c.get(r["sum"])
+        kept = c.read_vec(r["kept"], np.int32)
+    assert cnt == want["count"] and s == want["sum"]
+    assert bits_equal(kept, want["kept"])
+
+
 @pytest.mark.parametrize("dtype", [np.float32, np.float64, np.int64])
 def test_filter_other_dtypes_and_edge_masks(dtype):
     n = 3 * 4096 + 5
