@@ -363,16 +363,19 @@ __device__ __forceinline__ void filter_body(const SgProg* g, const SgArgs& a) {
     // thread 0 hands out this block's tile sequence: runs of consecutive tiles claimed with one atomic each.  A run is RUN
     // tiles while a run's kept values fit comfortably in the ring, else ONE tile: a tile that cannot enter the ring waits
     // for its run's offset, and with long runs that wait would chain from block to block.  Entries: (tile << 1) | first-of-run.
+    // The atomic of the NEXT run is issued one call before its result is needed, so its latency never stalls warp 0.
     int seq_base = 0, seq_j = 0, seq_len = 0;   // thread 0 only: current run, position in it, its length
+    int nxt_base = 0, nxt_len = 0;              // thread 0 only: the run claimed ahead
     unsigned int last_total = (unsigned int)RC; // thread 0 only: kept count of the latest tile (pessimistic until one is known)
+    auto claim_ahead = [&]() {                  // thread 0 only
+        nxt_len = (last_total * (unsigned int)RUN * 2u <= (unsigned int)RC) ? RUN : 1;
+        nxt_base = (int)atomicAdd(&a.ctrl[2], (unsigned int)nxt_len);
+    };
     auto next_tile = [&]() -> int {             // thread 0 only
-        if (seq_j == seq_len) {
-            seq_len = (last_total * (unsigned int)RUN * 2u <= (unsigned int)RC) ? RUN : 1;
-            seq_base = (int)atomicAdd(&a.ctrl[2], (unsigned int)seq_len);
-            seq_j = 0;
-        }
+        if (seq_j == seq_len) { seq_base = nxt_base; seq_len = nxt_len; seq_j = 0; }
         const int first = (seq_j == 0);
         const int t = seq_base + seq_j++;
+        if (seq_j == seq_len) claim_ahead();
         return t >= 0x3fffffff ? 0x7ffffffe : ((t << 1) | first);
     };
     if (threadIdx.x == 0) {
@@ -382,6 +385,7 @@ __device__ __forceinline__ void filter_body(const SgProg* g, const SgArgs& a) {
         }
         for (int s = 0; s < NS; ++s) mbar_init(&full_bar[s], 1);
         mbar_fence_init();
+        claim_ahead();
         for (int s = 0; s < NS; ++s) {          // the first NS tiles: their copies are in flight before the first one is touched
             const int tv = next_tile();
             s_tile[s] = tv;
