@@ -225,15 +225,15 @@ template <class TT> struct FilterBytecodeEval {
     static constexpr int EPT = F_CHUNKS * FW;
     static constexpr int TILE = BLOCK * EPT;
     static constexpr int RC = TILE, NS = 2, NSTG = 0;
-    static constexpr size_t STAGE_BYTES = 0;
-    static constexpr size_t SMEM = (size_t)RC * sizeof(T) + NS * sizeof(uint64_t);
+    static constexpr size_t STAGE_BYTES = VM_FILE_BYTES;     // no input is staged: the stage area holds the VM's shared-memory register file
+    static constexpr size_t SMEM = STAGE_BYTES + (size_t)RC * sizeof(T) + NS * sizeof(uint64_t);
     __device__ __forceinline__ static void issue(const SgProg*, const SgArgs&, int, uint32_t, uint64_t*) {}
     __device__ __forceinline__ static void fill(const SgProg*, const SgArgs&, int64_t, unsigned char*) {}
     __device__ __forceinline__ static void accum_kept(const SgProg*, T, Cell (&)[NOUT]) {}      // masked reductions are accumulated per element
     template <bool GUARDED>
-    __device__ __forceinline__ static void run(const SgProg* g, const SgArgs& a, int64_t i, const unsigned char*, uint32_t, T (&val)[FW], unsigned int& keep,
+    __device__ __forceinline__ static void run(const SgProg* g, const SgArgs& a, int64_t i, const unsigned char* vm_file, uint32_t, T (&val)[FW], unsigned int& keep,
                                                Cell (&acc)[NOUT]) {
-        VmRegs<T, FW> rf;
+        VmRegs<T, FW> rf(smem_u32(vm_file));
         unsigned int pf = 0;
         for (int k = 0; k < g->shape.n_in; ++k) {
             const SgIn in = g->in[k];

@@ -139,7 +139,11 @@ template <class T> cudaError_t launch_bytecode_t(const SgProg& g, const SgArgs& 
         if (!attr_set) { cudaFuncSetAttribute(filter1d_bytecode<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FilterBytecodeEval<T>::SMEM); attr_set = true; }
         filter1d_bytecode<T><<<grid, FILTER_THREADS, FilterBytecodeEval<T>::SMEM, s>>>(g, a);
     }
-    else pass1d_bytecode<T><<<grid, BLOCK, 0, s>>>(g, a);
+    else {
+        static bool attr_set = false;
+        if (!attr_set) { cudaFuncSetAttribute(pass1d_bytecode<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)VM_FILE_BYTES); attr_set = true; }
+        pass1d_bytecode<T><<<grid, BLOCK, VM_FILE_BYTES, s>>>(g, a);
+    }
     return cudaGetLastError();
 }
 template <class T> int occupancy_bytecode_t(bool filter) {
@@ -147,8 +151,9 @@ template <class T> int occupancy_bytecode_t(bool filter) {
     if (cached[filter] > 0) return cached[filter];
     int occ = 0;
     if (filter) cudaFuncSetAttribute(filter1d_bytecode<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FilterBytecodeEval<T>::SMEM);
+    else cudaFuncSetAttribute(pass1d_bytecode<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)VM_FILE_BYTES);
     cudaError_t e = filter ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, filter1d_bytecode<T>, FILTER_THREADS, FilterBytecodeEval<T>::SMEM)
-                           : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, pass1d_bytecode<T>, BLOCK, 0);
+                           : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, pass1d_bytecode<T>, BLOCK, VM_FILE_BYTES);
     if (e != cudaSuccess || occ <= 0) return 1;
     cached[filter] = occ;
     return occ;

@@ -14,25 +14,27 @@ constexpr int VM_VREG = 16;     // value registers of the bytecode evaluator (pl
 template <class T> struct VmE { static constexpr int value = 16 / (int)sizeof(T); };
 __host__ __device__ constexpr int vm_tile(int elem_size) { return BLOCK * (16 / elem_size); }
 
-#define SG_VM_CASES(X) X(0) X(1) X(2) X(3) X(4) X(5) X(6) X(7) X(8) X(9) X(10) X(11) X(12) X(13) X(14) X(15)
+// The value register file lives in SHARED memory: register k of thread t is the 16-byte cell at
+//     base + k * VM_REG_STRIDE + t * 16
+// (consecutive threads -> consecutive cells: conflict-free 128-bit accesses).  A register number is then just an
+// address offset — no per-register switch, about forty hardware registers per thread instead of 160+, so three
+// blocks run per SM where one did.  VM_FILE_BYTES of dynamic shared memory per block.
+constexpr uint32_t VM_REG_STRIDE = BLOCK * 16;
+constexpr size_t VM_FILE_BYTES = (size_t)VM_VREG * VM_REG_STRIDE;
 
 template <class T, int E> struct VmRegs {
-    T r[VM_VREG][E];
+    static_assert(E * sizeof(T) == 16, "one 128-bit cell per register");
+    uint32_t base;      // shared-window address of this thread's cell of register 0
+    __device__ __forceinline__ explicit VmRegs(uint32_t file_base) : base(file_base + (threadIdx.x & (BLOCK - 1)) * 16u) {}
     __device__ __forceinline__ void get(uint8_t k, T (&o)[E]) const {
-        switch (k) {
-#define X(i) case i: _Pragma("unroll") for (int e = 0; e < E; ++e) o[e] = r[i][e]; break;
-            SG_VM_CASES(X)
-#undef X
-            default: break;
-        }
+        uint32_t w[4];
+        asm volatile("ld.shared.v4.b32 {%0,%1,%2,%3}, [%4];" : "=r"(w[0]), "=r"(w[1]), "=r"(w[2]), "=r"(w[3]) : "r"(base + k * VM_REG_STRIDE) : "memory");
+        memcpy(o, w, 16);
     }
     __device__ __forceinline__ void put(uint8_t k, const T (&o)[E]) {
-        switch (k) {
-#define X(i) case i: _Pragma("unroll") for (int e = 0; e < E; ++e) r[i][e] = o[e]; break;
-            SG_VM_CASES(X)
-#undef X
-            default: break;
-        }
+        uint32_t w[4];
+        memcpy(w, o, 16);
+        asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};" ::"r"(base + k * VM_REG_STRIDE), "r"(w[0]), "r"(w[1]), "r"(w[2]), "r"(w[3]) : "memory");
     }
 };
 
@@ -157,7 +159,8 @@ __device__ __forceinline__ void vm_emit(const SgProg& g, const SgArgs& a, int64_
 }
 
 template <class T>
-__global__ void __launch_bounds__(BLOCK) pass1d_bytecode(const __grid_constant__ SgProg g, const __grid_constant__ SgArgs a) {
+__global__ void __launch_bounds__(BLOCK, 3) pass1d_bytecode(const __grid_constant__ SgProg g, const __grid_constant__ SgArgs a) {
+    extern __shared__ __align__(16) unsigned char vm_file[];
     constexpr int E = VmE<T>::value;
     constexpr int VM_TILE = BLOCK * E;
     Cell acc[SG_MAX_OUT];
@@ -173,7 +176,7 @@ __global__ void __launch_bounds__(BLOCK) pass1d_bytecode(const __grid_constant__
     }
     const bool early_exit = (g.shape.flags & PF_EARLY_EXIT) && !a.no_early_exit;
 
-    VmRegs<T, E> rf;
+    VmRegs<T, E> rf((uint32_t)__cvta_generic_to_shared(vm_file));
     unsigned int pf = 0;
     for (int k = 0; k < g.shape.n_in; ++k) {
         const SgIn in = g.in[k];
