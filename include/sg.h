@@ -187,6 +187,11 @@ sg_status sg_plan_stats(sg_ctx* ctx, sg_stats* out);
 int64_t sg_plan_dump(sg_ctx* ctx, int32_t pass, char* buf, int64_t cap);
 /* Device time of the last flush's launches in milliseconds (CUDA events on the context's stream). */
 sg_status sg_last_flush_ms(sg_ctx* ctx, float* ms);
+/* Device time of every flush between begin and end, without a host synchronisation inside the region: each flush records
+ * its own CUDA event pair on the context's stream; sg_timing_end waits for the last one and returns the sum in
+ * milliseconds and the number of flushes (the measurement of a pipelined sequence of steps). */
+sg_status sg_timing_begin(sg_ctx* ctx);
+sg_status sg_timing_end(sg_ctx* ctx, float* total_ms, int32_t* n_flushes);
 /* Replays the last flush's launch sequence `reps` times on the stream (same buffers, same plan, no host plan
  * build) and returns the mean device time per replay in ms: the measurement entry point. */
 sg_status sg_replay_last(sg_ctx* ctx, int32_t reps, float* ms_per_rep);

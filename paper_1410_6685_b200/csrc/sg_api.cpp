@@ -96,6 +96,8 @@ sg_status sg_ctx_destroy(sg_ctx* c) {
         if (c->slab) cudaFree(c->slab);
         if (c->slab_host) cudaFreeHost(c->slab_host);
         if (c->ev_done) cudaEventDestroy(c->ev_done);
+        for (auto* v : {&c->timing_events, &c->timing_pool})
+            for (auto& pr : *v) { cudaEventDestroy(pr.first); cudaEventDestroy(pr.second); }
         if (c->ev_t0) cudaEventDestroy(c->ev_t0);
         if (c->ev_t1) cudaEventDestroy(c->ev_t1);
     }

@@ -9,6 +9,7 @@
 #include <stdint.h>
 
 #include <string>
+#include <utility>
 #include <vector>
 
 #include "../../include/sg.h"
@@ -107,6 +108,10 @@ struct sg_ctx {
     std::vector<int64_t> slab_free;
     cudaEvent_t ev_done = nullptr, ev_t0 = nullptr, ev_t1 = nullptr;
     bool mirror_pending = false;
+    // sg_timing_begin/end: one event pair per flush, resolved at the end (no host sync inside the timed region)
+    bool timing = false;
+    std::vector<std::pair<cudaEvent_t, cudaEvent_t>> timing_events;
+    std::vector<std::pair<cudaEvent_t, cudaEvent_t>> timing_pool;
     uintptr_t fake_next = 0x10000000;   // plan-only contexts: distinct fake addresses
 
     // last flush

@@ -244,7 +244,15 @@ sg_status sg_flush_impl(sg_ctx* c) {
                 return sg_fail(c, SG_ERR_OOM, "tile-state allocation failed");
             }
         }
-        cudaEventRecord(c->ev_t0, c->stream);
+        cudaEvent_t t0 = c->ev_t0, t1 = c->ev_t1;
+        if (c->timing) {            // timed region: this flush gets its own event pair, read back at sg_timing_end
+            std::pair<cudaEvent_t, cudaEvent_t> pr{nullptr, nullptr};
+            if (!c->timing_pool.empty()) { pr = c->timing_pool.back(); c->timing_pool.pop_back(); }
+            else if (cudaEventCreate(&pr.first) != cudaSuccess || cudaEventCreate(&pr.second) != cudaSuccess) return sg_fail(c, SG_ERR_CUDA, "event creation failed");
+            c->timing_events.push_back(pr);
+            t0 = pr.first; t1 = pr.second;
+        }
+        cudaEventRecord(t0, c->stream);
         for (Pass& P : passes) {
             P.args.workspace = c->workspace;
             P.args.tile_state = c->tile_state;
@@ -261,7 +269,7 @@ sg_status sg_flush_impl(sg_ctx* c) {
             c->last.push_back({P.prog, P.args, P.geom});
             launches_total++;
         }
-        cudaEventRecord(c->ev_t1, c->stream);
+        cudaEventRecord(t1, c->stream);
         // a8: hand the flush's scalars back in one copy
         int64_t lo = c->slab_slots, hi = -1;
         for (const Node& n : N) {
@@ -335,6 +343,33 @@ extern "C" sg_status sg_last_flush_ms(sg_ctx* c, float* ms) {
         cudaGetLastError();
         return sg_fail(c, SG_ERR_CUDA, "no timed flush");
     }
+    return SG_OK;
+}
+
+extern "C" sg_status sg_timing_begin(sg_ctx* c) {
+    if (!c) return SG_ERR_ARG;
+    for (auto& pr : c->timing_events) c->timing_pool.push_back(pr);
+    c->timing_events.clear();
+    c->timing = true;
+    return SG_OK;
+}
+
+extern "C" sg_status sg_timing_end(sg_ctx* c, float* total_ms, int32_t* n_flushes) {
+    if (!c || !total_ms || !n_flushes) return SG_ERR_ARG;
+    c->timing = false;
+    *total_ms = 0.f;
+    *n_flushes = (int32_t)c->timing_events.size();
+    if (c->plan_only) return SG_OK;
+    for (auto& pr : c->timing_events) {
+        float ms = 0.f;
+        if (cudaEventSynchronize(pr.second) != cudaSuccess || cudaEventElapsedTime(&ms, pr.first, pr.second) != cudaSuccess) {
+            cudaGetLastError();
+            return sg_fail(c, SG_ERR_CUDA, "timed flush not complete");
+        }
+        *total_ms += ms;
+        c->timing_pool.push_back(pr);
+    }
+    c->timing_events.clear();
     return SG_OK;
 }
 

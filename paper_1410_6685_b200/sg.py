@@ -30,7 +30,7 @@ EXPORTS = [
     "sg_ctx_create", "sg_ctx_destroy", "sg_ctx_set_flags", "sg_last_error", "sg_vec_create", "sg_mat_create", "sg_vec_subset",
     "sg_mat_row", "sg_mat_rows", "sg_mat_col", "sg_mat_elem", "sg_enqueue", "sg_reduce", "sg_forall", "sg_exists",
     "sg_forall_adjacent", "sg_filter", "sg_contract", "sg_flush", "sg_scalar_get", "sg_scalar_dtype", "sg_vec_count", "sg_vec_data", "sg_vec_read",
-    "sg_release", "sg_plan_stats", "sg_plan_dump", "sg_last_flush_ms", "sg_replay_last", "sg_template_count", "sg_template_name",
+    "sg_release", "sg_plan_stats", "sg_plan_dump", "sg_last_flush_ms", "sg_timing_begin", "sg_timing_end", "sg_replay_last", "sg_template_count", "sg_template_name",
     "sg_version",
 ]
 
@@ -96,6 +96,8 @@ def lib() -> ctypes.CDLL:
         L.sg_plan_dump.argtypes = [c_void_p, c_int32, c_char_p, c_int64]
         L.sg_last_flush_ms.argtypes = [c_void_p, POINTER(c_float)]
         L.sg_replay_last.argtypes = [c_void_p, c_int32, POINTER(c_float)]
+        L.sg_timing_begin.argtypes = [c_void_p]
+        L.sg_timing_end.argtypes = [c_void_p, POINTER(c_float), POINTER(c_int32)]
         L.sg_ctx_set_flags.argtypes = [c_void_p, c_uint32]
         L.sg_ctx_destroy.argtypes = [c_void_p]
         L.sg_last_error.argtypes = [c_void_p]
@@ -292,6 +294,17 @@ def sg_last_flush_ms(ctx) -> float:
     ms = c_float(0)
     _ck(ctx, lib().sg_last_flush_ms(ctx, byref(ms)))
     return ms.value
+
+
+def sg_timing_begin(ctx) -> None:
+    _ck(ctx, lib().sg_timing_begin(ctx))
+
+
+def sg_timing_end(ctx) -> tuple[float, int]:
+    """(sum of the device times of the flushes since sg_timing_begin in ms, number of flushes)."""
+    ms, n = c_float(0), c_int32(0)
+    _ck(ctx, lib().sg_timing_end(ctx, byref(ms), byref(n)))
+    return ms.value, n.value
 
 
 def sg_replay_last(ctx, reps: int) -> float:
