@@ -232,27 +232,33 @@ __global__ void __launch_bounds__(BLOCK, P::min_blocks) pass1d_template(const __
         T v[M::NV][M::E];
         bool p[M::NP][M::E];
         bcast_inputs<P, M::E>(v, a, KS);
-        for (int64_t tile = blockIdx.x; tile < a.n_full_tiles; tile += gridDim.x) {
-            // the decided word is requested together with the tile's loads and examined after the tile is processed,
-            // so the poll costs no extra round trip on the clean path
+        unsigned int it = 0;
+        for (int64_t tile = blockIdx.x; tile < a.n_full_tiles; tile += gridDim.x, ++it) {
+            // every POLL-th tile the decided word is requested together with the tile's loads and examined after the tile is
+            // processed, so the poll costs no extra round trip on the clean path (a strong load per tile measurably slows the
+            // stream: 220 -> 184 us on config 3)
+            constexpr unsigned int POLL = 8;
             unsigned int decided_word = 0;
+            const bool poll = M::early_exit && !a.no_early_exit && (it % POLL) == 0;
             if constexpr (M::early_exit) {
-                if (!a.no_early_exit) decided_word = ld_volatile_u32(&a.ctrl[1]);
+                if (poll) decided_word = ld_relaxed_u32(&a.ctrl[1]);
             }
             const int64_t base = a.head + tile * M::TILE;
             load_inputs_full<P>(v, p, a, base, KS);
             exec_body<P, T, M::NV, M::NP, M::E>(v, p, a, IS);
             emit_outputs_full<P>(v, p, acc, a, base, OS);
             if constexpr (M::early_exit) {
+                if (poll) {
 #pragma unroll
-                for (int o = 0; o < M::S.n_out; ++o) {
-                    bool decided = (kind[o] == OUT_ALL) ? (acc[o].a == 0) : (acc[o].a != 0);
-                    if (!(flagged & (1u << o)) && __any_sync(0xffffffffu, decided)) {
-                        flagged |= 1u << o;
-                        if ((threadIdx.x & 31) == 0) atomicOr(&a.ctrl[1], 1u << o);
+                    for (int o = 0; o < M::S.n_out; ++o) {
+                        bool decided = (kind[o] == OUT_ALL) ? (acc[o].a == 0) : (acc[o].a != 0);
+                        if (!(flagged & (1u << o)) && __any_sync(0xffffffffu, decided)) {
+                            flagged |= 1u << o;
+                            if ((threadIdx.x & 31) == 0) atomicOr(&a.ctrl[1], 1u << o);
+                        }
                     }
+                    if ((decided_word & need_mask) == need_mask || (decided_word & a.exit_any) != 0) break;
                 }
-                if ((decided_word & need_mask) == need_mask || (decided_word & a.exit_any) != 0) break;
             }
         }
     }
