@@ -83,6 +83,15 @@ class ClockSampler:
                 "samples": len(sm)}
 
 
+def ncu_traffic(kernel: str, n: int):
+    """DRAM bytes per launch of the dominant kernel from the committed ncu --set full capture (profiles/), or None."""
+    try:
+        d = json.load(open(os.path.join(ROOT, "profiles", "r01_traffic.json")))[kernel]
+        return d["traffic_bytes"] if d["n"] == n else None
+    except Exception:
+        return None
+
+
 def oracle_chain_rate(x, y, seconds_target=8.0):
     """The CPU oracle as it stands, on a bounded sample of the same workload; returns (elements/s, sample size, sum, max)."""
     from oracle import configs as ocfg
@@ -339,7 +348,8 @@ def main():
                    "template_passes": st.n_template, "step": "enqueue + plan + fused launch + scalar hand-back (async copy to the pinned mirror) through the C ABI; K steps pipelined, scalars read after the region"},
         "GB/s": world * alg_bytes / ms_step / 1e6,
         "frac_of_8TBps": alg_bytes / ms_step / 1e6 / 8000.0,
-        "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": None,
+        "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                     "traffic": ncu_traffic(sg.sg_template_name(st.pass_kernel[0]) if st.pass_kernel[0] else "bytecode", n),
                      "kernel": sg.sg_template_name(st.pass_kernel[0]) if st.pass_kernel[0] else "bytecode", "kernel_ms": k_ms,
                      "algorithmic_bytes_per_launch": alg_bytes, "peak_source": peak_src, "frac_of_8TBps": achieved / 8000.0},
         "cpu_baseline": {"value": cpu_rate, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": f"first {cpu_m} elements of the same x,y, one timed run"},
