@@ -66,7 +66,7 @@ template <class P> struct FilterTemplateEval {
     static constexpr int EPT = F_CHUNKS * FW;            // elements per thread per tile
     static constexpr int TILE = BLOCK * EPT;
     static constexpr int RC = TILE;                      // elements of the compaction ring (a power of two, >= one tile)
-    static constexpr int NS = 2;                         // input stages
+    static constexpr int NS = (P::row_unroll >= 1 && P::row_unroll <= 3) ? P::row_unroll : 2;    // input stages
     __host__ __device__ static constexpr int count_vec() {
         int n = 0;
         for (int k = 0; k < M::S.n_in; ++k) n += (P::prog.in[k].kind == IN_VEC);
@@ -420,33 +420,40 @@ __device__ __forceinline__ void filter_body(const SgProg* g, const SgArgs& a) {
         int run_no = -1;                        // number of the current run of this block
         unsigned int run_lpre = 0;              // kept count of the current run's earlier tiles
         bool overflow = false;
-        auto copy_out_oldest = [&]() {
-            const int e = q_head % NP;
-            const int r = s_q_run[e];
-            mbar_wait(&run_resolved[r % NR], (uint32_t)((r / NR) & 1));
-            const unsigned int total = s_q_total[e];
-            const long long base = (long long)(s_r_excl[r % NR] + s_q_lpre[e]);
-            const unsigned int r0 = ring_tail & (RC - 1);
-            if (base + (long long)total <= cap && r0 + total <= (unsigned int)RC) {
-                // common case (uniform): inside the output's capacity, no wrap-around in the ring
-                T* const d0 = dst + base;
-                for (unsigned int i = threadIdx.x; i < total; i += BLOCK) {
-                    const T v = lds_elem<T>(ring, r0 + i);
-                    EV::accum_kept(g, v, acc);
-                    d0[i] = v;
+        // copies out the k oldest pending tiles.  Tiles of one run are adjacent in the ring AND in the output, so each
+        // run's share goes out in ONE coalesced loop (one wait, one address computation, one set of uniform checks).
+        auto copy_out = [&](int k) {
+            while (k > 0) {
+                const int e0 = q_head % NP;
+                const int r = s_q_run[e0];
+                mbar_wait(&run_resolved[r % NR], (uint32_t)((r / NR) & 1));
+                unsigned int total = s_q_total[e0];
+                int m = 1;
+                while (m < k && s_q_run[(q_head + m) % NP] == r) { total += s_q_total[(q_head + m) % NP]; ++m; }
+                const long long base = (long long)(s_r_excl[r % NR] + s_q_lpre[e0]);
+                const unsigned int r0 = ring_tail & (RC - 1);
+                if (base + (long long)total <= cap && r0 + total <= (unsigned int)RC) {
+                    // common case (uniform): inside the output's capacity, no wrap-around in the ring
+                    T* const d0 = dst + base;
+                    for (unsigned int i = threadIdx.x; i < total; i += BLOCK) {
+                        const T v = lds_elem<T>(ring, r0 + i);
+                        EV::accum_kept(g, v, acc);
+                        d0[i] = v;
+                    }
+                } else {
+                    for (unsigned int i = threadIdx.x; i < total; i += BLOCK) {
+                        const long long pos = base + i;
+                        const T v = lds_elem<T>(ring, (ring_tail + i) & (RC - 1));
+                        EV::accum_kept(g, v, acc);
+                        if (pos < cap) dst[pos] = v; else overflow = true;
+                    }
                 }
-            } else {
-                for (unsigned int i = threadIdx.x; i < total; i += BLOCK) {
-                    const long long pos = base + i;
-                    const T v = lds_elem<T>(ring, (ring_tail + i) & (RC - 1));
-                    EV::accum_kept(g, v, acc);
-                    if (pos < cap) dst[pos] = v; else overflow = true;
-                }
+                if (threadIdx.x == 0 && s_q_tile[(q_head + m - 1) % NP] == a.n_tiles - 1) *reinterpret_cast<long long*>(a.out_aux[fo]) = base + (long long)total;
+                ring_tail += total;
+                q_head += m;
+                q_count -= m;
+                k -= m;
             }
-            if (threadIdx.x == 0 && s_q_tile[e] == a.n_tiles - 1) *reinterpret_cast<long long*>(a.out_aux[fo]) = base + (long long)total;
-            ring_tail += total;
-            ++q_head;
-            --q_count;
         };
         int it = 0;
         for (;; ++it) {
@@ -535,7 +542,7 @@ __device__ __forceinline__ void filter_body(const SgProg* g, const SgArgs& a) {
             int copied = 0;
             if (ring_head - ring_tail + tile_total > (unsigned int)RC) {
                 // rare: the ring cannot take this tile yet — wait for the oldest offsets first
-                while (ring_head - ring_tail + tile_total > (unsigned int)RC) { copy_out_oldest(); ++copied; }
+                while (ring_head - ring_tail + tile_total > (unsigned int)RC) { copy_out(1); ++copied; }
                 named_bar_sync<2, BLOCK>();
             }
             {
@@ -557,8 +564,9 @@ __device__ __forceinline__ void filter_body(const SgProg* g, const SgArgs& a) {
             run_lpre += tile_total;
             ++q_count;
             // copy out the tiles whose offset was known at the poll (never blocks), and as many as the queue bound demands
-            const int ready = s_ready[it & 1];
-            while (copied < ready || q_count > NP - 1) { copy_out_oldest(); ++copied; }
+            int k = s_ready[it & 1] - copied;
+            if (k < q_count - (NP - 1)) k = q_count - (NP - 1);
+            if (k > 0) copy_out(k);
         }
         if (threadIdx.x == 0) {             // no run follows: release the look-back warp
             const int rs = (run_no + 1) % NR;
@@ -566,7 +574,7 @@ __device__ __forceinline__ void filter_body(const SgProg* g, const SgArgs& a) {
             mbar_arrive(&run_posted[rs]);
         }
         named_bar_sync<1, BLOCK>();         // the last tile's queue entry (written by thread 0 after its barrier) is visible
-        while (q_count > 0) copy_out_oldest();
+        copy_out(q_count);
         if (overflow) a.ctrl[3] = 1u;
     }
     epilogue_1d<T, NOUT>(acc, kind, a, true);
