@@ -362,6 +362,32 @@ def test_filter_high_selectivity(modulus):
     assert bits_equal(kept, want["kept"])
 
 
+def test_filter_repeated_launches_share_tile_states():
+    """One context, many filter launches of different lengths and selectivities: the tile-state words of earlier launches
+    stay in memory and are told apart by the launch epoch only; replays (sg_replay_last) re-run the same launch."""
+    rng = np.random.default_rng(7)
+    with Ctx() as c:
+        for rep in range(24):
+            n = int(rng.integers(1, 40)) * 8192 + int(rng.integers(0, 8192))
+            modulus = int(rng.choice([1, 2, 3, 7, 50, 1000]))
+            x = inputs.uniform_i31(3, 100 + rep, n)
+            want = ocfg.cfg2(x, modulus, 0)
+            tx = c.torch.from_numpy(x).cuda()
+            r = W.cfg2(c.ctx, n, tx.data_ptr(), modulus=modulus, residue=0)
+            cnt, s = c.get(r["count"]), c.get(r["sum"])
+            kept = c.read_vec(r["kept"], np.int32)
+            assert cnt == want["count"] and s == want["sum"], (rep, n, modulus)
+            assert bits_equal(kept, want["kept"]), (rep, n, modulus)
+            if rep % 6 == 0:
+                sg.sg_replay_last(c.ctx, 3)
+                kept2 = np.empty(cnt, dtype=np.int32)
+                c.torch.cuda.synchronize()
+                sg.sg_vec_read(c.ctx, r["kept"], kept2.ctypes.data, kept2.nbytes)
+                assert bits_equal(kept2, want["kept"]) and c.get(r["count"]) == want["count"]
+            for h in r.values():
+                sg.sg_release(c.ctx, h)
+
+
 @pytest.mark.parametrize("dtype", [np.float32, np.float64, np.int64])
 def test_filter_other_dtypes_and_edge_masks(dtype):
     n = 3 * 4096 + 5
