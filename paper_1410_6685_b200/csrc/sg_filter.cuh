@@ -38,9 +38,9 @@ namespace sgk {
 constexpr unsigned long long ST_AGG = 1ull << 62, ST_INC = 2ull << 62, ST_FLAGS = 3ull << 62;
 constexpr unsigned long long ST_VAL = (1ull << 40) - 1;
 constexpr int LB = 8;               // look-back windows (of 32 tile states) requested per round trip
-constexpr int FILTER_THREADS = BLOCK + 32;
-constexpr int F_CHUNKS = 8;         // 16-byte chunks per thread per tile: one 128-byte row
-constexpr int F_TILE_BYTES = BLOCK * F_CHUNKS * 16;     // 32 KiB per staged input
+constexpr int F_ROWS = 256;         // rows of 128 bytes per tile
+constexpr int F_TILE_BYTES = F_ROWS * 128;              // 32 KiB per staged input
+constexpr int F_TILE_CHUNKS = F_TILE_BYTES / 16;        // 16-byte chunks per tile
 constexpr int RUN = 4;              // consecutive tiles a block claims at once while few values are kept (else 1); one look-back per run
 constexpr int NR = 16;              // runs of one block whose offset may be outstanding (ring of run slots)
 constexpr int NP = 8;               // tiles of one block that may wait for their global offset (each may be a run of its own: NP < NR)
@@ -63,9 +63,12 @@ template <class P> struct FilterTemplateEval {
     typedef typename M::VEC VEC;
     static constexpr int NOUT = M::NOUT;
     static constexpr int FW = 16 / (int)sizeof(T);       // elements per 16-byte chunk
-    static constexpr int EPT = F_CHUNKS * FW;            // elements per thread per tile
-    static constexpr int TILE = BLOCK * EPT;
+    static constexpr int CT = 128 * P::unroll;           // compute threads: 512 = two per row (16 compute warps), 256 = one per row
+    static constexpr int CPT = F_TILE_CHUNKS / CT;       // consecutive 16-byte chunks per thread per tile
+    static constexpr int EPT = CPT * FW;                 // consecutive elements per thread per tile
+    static constexpr int TILE = F_TILE_BYTES / (int)sizeof(T);
     static constexpr int RC = TILE;                      // elements of the compaction ring (a power of two, >= one tile)
+    static_assert(CT == 256 || CT == 512, "filter instances: unroll 2 or 4");
     static constexpr int NS = (P::row_unroll >= 1 && P::row_unroll <= 3) ? P::row_unroll : 2;    // input stages
     __host__ __device__ static constexpr int count_vec() {
         int n = 0;
@@ -130,8 +133,8 @@ template <class P> struct FilterTemplateEval {
             const T* src = reinterpret_cast<const T*>(a.in_ptr[K]);
             const bool vec = (a.vec_ok >> 31) & 1;                  // every vector operand 16-byte aligned
 #pragma unroll
-            for (int q = 0; q < F_CHUNKS; ++q) {
-                const int c = threadIdx.x + BLOCK * q;              // chunk of the tile, in memory order
+            for (int q = 0; q < CPT; ++q) {
+                const int c = threadIdx.x + CT * q;                 // chunk of the tile, in memory order
                 const int64_t i = tbase + (int64_t)c * FW;
                 VEC w;
                 T* we = reinterpret_cast<T*>(&w);
@@ -222,8 +225,9 @@ template <class TT> struct FilterBytecodeEval {
     typedef TT T;
     static constexpr int NOUT = SG_MAX_OUT;
     static constexpr int FW = 16 / (int)sizeof(T);
-    static constexpr int EPT = F_CHUNKS * FW;
-    static constexpr int TILE = BLOCK * EPT;
+    static constexpr int CT = BLOCK, CPT = F_TILE_CHUNKS / CT;
+    static constexpr int EPT = CPT * FW;
+    static constexpr int TILE = F_TILE_BYTES / (int)sizeof(T);
     static constexpr int RC = TILE, NS = 2, NSTG = 0;
     static constexpr size_t STAGE_BYTES = VM_FILE_BYTES;     // no input is staged: the stage area holds the VM's shared-memory register file
     static constexpr size_t SMEM = STAGE_BYTES + (size_t)RC * sizeof(T) + NS * sizeof(uint64_t);
@@ -315,8 +319,8 @@ __device__ __forceinline__ unsigned long long filter_lookback(unsigned long long
 
 
 // appends the kept elements of one thread's row (keep bits in `mask`, element k = val[k / FW][k % FW]) at `addr`
-template <class T, int FW, int... K>
-__device__ __forceinline__ void scatter_row(uint32_t& addr, unsigned int mask, T (&val)[F_CHUNKS][FW], std::integer_sequence<int, K...>) {
+template <class T, int FW, int CPT, int... K>
+__device__ __forceinline__ void scatter_row(uint32_t& addr, unsigned int mask, T (&val)[CPT][FW], std::integer_sequence<int, K...>) {
     (sts_append_if<T, K>(addr, mask, val[K / FW][K % FW]), ...);
 }
 
@@ -325,13 +329,14 @@ template <class EV>
 __device__ __forceinline__ void filter_body(const SgProg* g, const SgArgs& a) {
     typedef typename EV::T T;
     constexpr int FW = EV::FW, EPT = EV::EPT, TILE = EV::TILE, NOUT = EV::NOUT, NS = EV::NS, NSTG = EV::NSTG, RC = EV::RC;
+    constexpr int CT = EV::CT, CW = CT / 32, CPT = EV::CPT;       // compute threads / warps, chunks per thread
     static_assert(NP < NR, "a run slot must not be reused while one of its tiles is pending");
     extern __shared__ __align__(1024) unsigned char dyn_smem[];
     unsigned char* const stage_base = dyn_smem;                                             // [NS][NSTG][F_TILE_BYTES], 1024-byte aligned (swizzle)
     const uint32_t ring = pin_reg(smem_u32(dyn_smem + EV::STAGE_BYTES));                             // [RC] compacted values awaiting their offset (shared-window address)
     uint64_t* const full_bar = reinterpret_cast<uint64_t*>(dyn_smem + EV::STAGE_BYTES + (size_t)RC * sizeof(T));
     __shared__ int s_tile[NS + 1];                      // tile id of iteration it at [it % (NS+1)]
-    __shared__ unsigned int s_warp_total[2][WARPS];     // double-buffered: a warp may run one barrier ahead
+    __shared__ unsigned int s_warp_total[2][CW];     // double-buffered: a warp may run one barrier ahead
     __shared__ int s_ready[2];                          // thread 0 -> all: pending tiles whose offset is known (polled before the barrier)
     __shared__ int s_q_tile[NP];                        // pending tile queue: tile id,
     __shared__ unsigned int s_q_total[NP];              //   kept count,
@@ -390,12 +395,12 @@ __device__ __forceinline__ void filter_body(const SgProg* g, const SgArgs& a) {
             const int tv = next_tile();
             s_tile[s] = tv;
             const int t = tv >> 1;
-            if (use_tma && t < a.n_full_tiles) EV::issue(g, a, t * BLOCK, smem_u32(stage_base + (size_t)s * NSTG * F_TILE_BYTES), &full_bar[s]);
+            if (use_tma && t < a.n_full_tiles) EV::issue(g, a, t * F_ROWS, smem_u32(stage_base + (size_t)s * NSTG * F_TILE_BYTES), &full_bar[s]);
         }
     }
     __syncthreads();
 
-    if (warp == WARPS) {
+    if (warp == CW) {
         // ---------------- look-back warp: one message per run, in order ----------------
         for (int r = 0;; ++r) {
             const int rs = r % NR;
@@ -435,13 +440,13 @@ __device__ __forceinline__ void filter_body(const SgProg* g, const SgArgs& a) {
                 if (base + (long long)total <= cap && r0 + total <= (unsigned int)RC) {
                     // common case (uniform): inside the output's capacity, no wrap-around in the ring
                     T* const d0 = dst + base;
-                    for (unsigned int i = threadIdx.x; i < total; i += BLOCK) {
+                    for (unsigned int i = threadIdx.x; i < total; i += CT) {
                         const T v = lds_elem<T>(ring, r0 + i);
                         EV::accum_kept(g, v, acc);
                         d0[i] = v;
                     }
                 } else {
-                    for (unsigned int i = threadIdx.x; i < total; i += BLOCK) {
+                    for (unsigned int i = threadIdx.x; i < total; i += CT) {
                         const long long pos = base + i;
                         const T v = lds_elem<T>(ring, (ring_tail + i) & (RC - 1));
                         EV::accum_kept(g, v, acc);
@@ -477,17 +482,18 @@ __device__ __forceinline__ void filter_body(const SgProg* g, const SgArgs& a) {
                 if (use_tma && full) mbar_wait(&full_bar[s], (uint32_t)((it / NS) & 1));
                 else {
                     EV::fill(g, a, tbase, stg);
-                    named_bar_sync<2, BLOCK>();
+                    named_bar_sync<2, CT>();
                 }
             }
-            T val[F_CHUNKS][FW];
+            T val[CPT][FW];
             unsigned int mask = 0;                              // keep bits of this thread's EPT consecutive elements
 #pragma unroll
-            for (int j = 0; j < F_CHUNKS; ++j) {
+            for (int j = 0; j < CPT; ++j) {
                 unsigned int kj;
                 const int64_t i = tbase + (int64_t)threadIdx.x * EPT + j * FW;
-                if (full) EV::template run<false>(g, a, i, stg, swz(threadIdx.x, j), val[j], kj, acc);
-                else EV::template run<true>(g, a, i, stg, swz(threadIdx.x, j), val[j], kj, acc);
+                const uint32_t gc = threadIdx.x * CPT + j;      // chunk of the tile: row gc / 8, chunk gc % 8 of the row
+                if (full) EV::template run<false>(g, a, i, stg, swz(gc >> 3, gc & 7u), val[j], kj, acc);
+                else EV::template run<true>(g, a, i, stg, swz(gc >> 3, gc & 7u), val[j], kj, acc);
                 mask |= kj << (j * FW);
             }
             // rank: the thread's elements are consecutive, so one popc and one warp scan order the tile
@@ -510,10 +516,10 @@ __device__ __forceinline__ void filter_body(const SgProg* g, const SgArgs& a) {
                 s_ready[it & 1] = ready;
                 if (!first) run_known = mbar_test(&run_resolved[rs], (uint32_t)((run_no / NR) & 1));
             }
-            named_bar_sync<1, BLOCK>();     // the stage is in registers; warp totals, next tile id and the ready count are visible
+            named_bar_sync<1, CT>();     // the stage is in registers; warp totals, next tile id and the ready count are visible
             unsigned int warp_excl = 0, tile_total = 0;
 #pragma unroll
-            for (int w = 0; w < WARPS; ++w) {
+            for (int w = 0; w < CW; ++w) {
                 const unsigned int t = s_warp_total[it & 1][w];
                 if (w < warp) warp_excl += t;
                 tile_total += t;
@@ -536,25 +542,25 @@ __device__ __forceinline__ void filter_body(const SgProg* g, const SgArgs& a) {
                 }
                 if (use_tma && (tv_next >> 1) < a.n_full_tiles) {
                     fence_proxy_async();
-                    EV::issue(g, a, (tv_next >> 1) * BLOCK, smem_u32(stg), &full_bar[s]);
+                    EV::issue(g, a, (tv_next >> 1) * F_ROWS, smem_u32(stg), &full_bar[s]);
                 }
             }
             int copied = 0;
             if (ring_head - ring_tail + tile_total > (unsigned int)RC) {
                 // rare: the ring cannot take this tile yet — wait for the oldest offsets first
                 while (ring_head - ring_tail + tile_total > (unsigned int)RC) { copy_out(1); ++copied; }
-                named_bar_sync<2, BLOCK>();
+                named_bar_sync<2, CT>();
             }
             {
                 const unsigned int pos = ring_head + warp_excl + (incl - cnt);
                 if (((ring_head & (RC - 1)) + tile_total) <= (unsigned int)RC) {
                     // the tile does not wrap around the ring (uniform): plain appends
                     uint32_t addr = ring + (pos & (RC - 1)) * (uint32_t)sizeof(T);
-                    scatter_row<T, FW>(addr, mask, val, std::make_integer_sequence<int, F_CHUNKS * FW>{});
+                    scatter_row<T, FW, CPT>(addr, mask, val, std::make_integer_sequence<int, CPT * FW>{});
                 } else {
                     unsigned int q = pos;
 #pragma unroll
-                    for (int j = 0; j < F_CHUNKS; ++j)
+                    for (int j = 0; j < CPT; ++j)
 #pragma unroll
                         for (int e = 0; e < FW; ++e)
                             if ((mask >> (j * FW + e)) & 1u) sts_elem<T>(ring, (q++) & (RC - 1), val[j][e]);
@@ -573,7 +579,7 @@ __device__ __forceinline__ void filter_body(const SgProg* g, const SgArgs& a) {
             s_r_tile[rs] = -1;
             mbar_arrive(&run_posted[rs]);
         }
-        named_bar_sync<1, BLOCK>();         // the last tile's queue entry (written by thread 0 after its barrier) is visible
+        named_bar_sync<1, CT>();         // the last tile's queue entry (written by thread 0 after its barrier) is visible
         copy_out(q_count);
         if (overflow) a.ctrl[3] = 1u;
     }
@@ -581,11 +587,11 @@ __device__ __forceinline__ void filter_body(const SgProg* g, const SgArgs& a) {
 }
 
 template <class P>
-__global__ void __launch_bounds__(FILTER_THREADS, P::min_blocks) filter1d_template(const __grid_constant__ SgArgs a) {
+__global__ void __launch_bounds__(FilterTemplateEval<P>::CT + 32, P::min_blocks) filter1d_template(const __grid_constant__ SgArgs a) {
     filter_body<FilterTemplateEval<P>>(nullptr, a);
 }
 template <class T>
-__global__ void __launch_bounds__(FILTER_THREADS) filter1d_bytecode(const __grid_constant__ SgProg g, const __grid_constant__ SgArgs a) {
+__global__ void __launch_bounds__(BLOCK + 32) filter1d_bytecode(const __grid_constant__ SgProg g, const __grid_constant__ SgArgs a) {
     filter_body<FilterBytecodeEval<T>>(&g, a);
 }
 

@@ -56,7 +56,7 @@ bool encode_filter_tmap(void* out128, const void* base, long rows) {
     static_assert(sizeof(CUtensorMap) == 128, "tensor map size");
     const cuuint64_t dims[2] = {32, (cuuint64_t)rows};
     const cuuint64_t strides[1] = {128};
-    const cuuint32_t box[2] = {32, (cuuint32_t)BLOCK};
+    const cuuint32_t box[2] = {32, (cuuint32_t)F_ROWS};
     const cuuint32_t estr[2] = {1, 1};
     alignas(64) CUtensorMap m;
     if (fn(&m, CU_TENSOR_MAP_DATA_TYPE_UINT32, 2, const_cast<void*>(base), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
@@ -71,7 +71,7 @@ template <class P> bool encode_filter_tmaps(SgArgs& a) {
     int slot = 0;       // index among the IN_VEC inputs
     for (int k = 0; k < P::prog.shape.n_in; ++k) {
         if (P::prog.in[k].kind != IN_VEC) continue;
-        if (slot < EV::NSTG && !encode_filter_tmap(a.tmap[slot], a.in_ptr[k], (long)a.n_full_tiles * BLOCK)) return false;
+        if (slot < EV::NSTG && !encode_filter_tmap(a.tmap[slot], a.in_ptr[k], (long)a.n_full_tiles * F_ROWS)) return false;
         ++slot;
     }
     return true;
@@ -89,7 +89,7 @@ template <class P> cudaError_t launch_template(const SgArgs& a, int grid, cudaSt
         SgArgs a2 = a;
         a2.vec_ok &= ~(1 << 30);
         if (encode_filter_tmaps<P>(a2)) a2.vec_ok |= (1 << 30);
-        filter1d_template<P><<<grid, FILTER_THREADS, smem_of<P>(), s>>>(a2);
+        filter1d_template<P><<<grid, FilterTemplateEval<P>::CT + 32, smem_of<P>(), s>>>(a2);
     }
     else pass1d_template<P><<<grid, BLOCK, 0, s>>>(a);
     return cudaGetLastError();
@@ -105,7 +105,7 @@ template <class P> int occupancy_template() {
     }
     else if constexpr ((P::prog.shape.flags & PF_FILTER) != 0) {
         cudaFuncSetAttribute(filter1d_template<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_of<P>());
-        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, filter1d_template<P>, FILTER_THREADS, smem_of<P>());
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, filter1d_template<P>, FilterTemplateEval<P>::CT + 32, smem_of<P>());
     }
     else e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, pass1d_template<P>, BLOCK, 0);
     if (e != cudaSuccess || occ <= 0) return 1;
@@ -137,7 +137,7 @@ template <class T> cudaError_t launch_bytecode_t(const SgProg& g, const SgArgs& 
     if (g.shape.flags & PF_FILTER) {
         static bool attr_set = false;
         if (!attr_set) { cudaFuncSetAttribute(filter1d_bytecode<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FilterBytecodeEval<T>::SMEM); attr_set = true; }
-        filter1d_bytecode<T><<<grid, FILTER_THREADS, FilterBytecodeEval<T>::SMEM, s>>>(g, a);
+        filter1d_bytecode<T><<<grid, BLOCK + 32, FilterBytecodeEval<T>::SMEM, s>>>(g, a);
     }
     else {
         static bool attr_set = false;
@@ -152,7 +152,7 @@ template <class T> int occupancy_bytecode_t(bool filter) {
     int occ = 0;
     if (filter) cudaFuncSetAttribute(filter1d_bytecode<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FilterBytecodeEval<T>::SMEM);
     else cudaFuncSetAttribute(pass1d_bytecode<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)VM_FILE_BYTES);
-    cudaError_t e = filter ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, filter1d_bytecode<T>, FILTER_THREADS, FilterBytecodeEval<T>::SMEM)
+    cudaError_t e = filter ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, filter1d_bytecode<T>, BLOCK + 32, FilterBytecodeEval<T>::SMEM)
                            : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, pass1d_bytecode<T>, BLOCK, VM_FILE_BYTES);
     if (e != cudaSuccess || occ <= 0) return 1;
     cached[filter] = occ;
@@ -248,7 +248,7 @@ int sgk_plan(const SgProg& prog, SgArgs& a, int force_bytecode, int sm_count, in
     }
 
     if (isfilter) {
-        const int tile = tid ? g_entries[tid].tile : BLOCK * F_CHUNKS * (16 / es);
+        const int tile = tid ? g_entries[tid].tile : F_TILE_BYTES / es;
         const int occ = has_device ? (tid ? g_entries[tid].occupancy() : occupancy_bytecode(prog.shape.dtype, true)) : 4;
         const long n_tiles = (a.n + tile - 1) / tile;
         if (a.n >= (1ll << 40) || n_tiles >= 0x3fffffffl) return fail(err, errcap, -9, "filter input too long for the tile-state word");

@@ -26,8 +26,8 @@ __host__ __device__ constexpr bool out_is_pred_reduction(uint8_t k) { return k >
 // in block order (deterministic: no floating-point atomics) and writes the 8-byte results.
 // ---------------------------------------------------------------------------------------------------------
 template <class T, int NOUT>
-__device__ __forceinline__ void block_reduce_cells(Cell (&acc)[NOUT], const uint8_t (&kind)[NOUT], Cell* smem /*[WARPS*NOUT]*/) {
-    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+__device__ __forceinline__ void block_reduce_cells(Cell (&acc)[NOUT], const uint8_t (&kind)[NOUT], Cell* smem /*[32*NOUT]*/) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarps = (int)(blockDim.x >> 5);     // any block of whole warps (<= 32)
 #pragma unroll
     for (int o = 0; o < NOUT; ++o) {
         if (!out_is_reduction(kind[o])) continue;
@@ -36,16 +36,16 @@ __device__ __forceinline__ void block_reduce_cells(Cell (&acc)[NOUT], const uint
             Cell other = cell_shfl_down(acc[o], d);
             cell_combine<T>(kind[o], acc[o], other);
         }
-        if (lane == 0 && warp < WARPS) smem[warp * NOUT + o] = acc[o];     // warps beyond WARPS (a filter block's look-back warp) hold identities
+        if (lane == 0) smem[warp * NOUT + o] = acc[o];
     }
     __syncthreads();
     if (warp == 0) {
 #pragma unroll
         for (int o = 0; o < NOUT; ++o) {
             if (!out_is_reduction(kind[o])) continue;
-            Cell c = (lane < WARPS) ? smem[lane * NOUT + o] : cell_identity<T>(kind[o]);
+            Cell c = (lane < nwarps) ? smem[lane * NOUT + o] : cell_identity<T>(kind[o]);
 #pragma unroll
-            for (int d = WARPS / 2; d >= 1; d >>= 1) {
+            for (int d = 16; d >= 1; d >>= 1) {
                 Cell other = cell_shfl_down(c, d);
                 cell_combine<T>(kind[o], c, other);
             }
@@ -57,7 +57,7 @@ __device__ __forceinline__ void block_reduce_cells(Cell (&acc)[NOUT], const uint
 
 template <class T, int NOUT>
 __device__ __forceinline__ void epilogue_1d(Cell (&acc)[NOUT], const uint8_t (&kind)[NOUT], const SgArgs& a, bool need_ticket) {
-    __shared__ Cell smem[WARPS * SG_MAX_OUT];
+    __shared__ Cell smem[32 * SG_MAX_OUT];
     __shared__ unsigned int s_last;
     if (!need_ticket) return;     // passes with neither reductions nor a dynamic tile counter leave ctrl untouched
     block_reduce_cells<T, NOUT>(acc, kind, smem);
@@ -77,7 +77,7 @@ __device__ __forceinline__ void epilogue_1d(Cell (&acc)[NOUT], const uint8_t (&k
     for (int o = 0; o < NOUT; ++o) {
         if (!out_is_reduction(kind[o])) continue;
         Cell c = cell_identity<T>(kind[o]);
-        for (unsigned int b = threadIdx.x; b < gridDim.x && threadIdx.x < BLOCK; b += BLOCK) {
+        for (unsigned int b = threadIdx.x; b < gridDim.x; b += blockDim.x) {
             Cell other;
             const unsigned long long* src = reinterpret_cast<const unsigned long long*>(&ws[(size_t)b * SG_MAX_OUT + o]);
             other.a = __ldcg(src); other.b = __ldcg(src + 1);
