@@ -133,37 +133,52 @@ const Entry g_entries[] = {
 #undef SG_TEMPLATE
 const int g_n_entries = (int)(sizeof(g_entries) / sizeof(g_entries[0]));
 
-template <class T> cudaError_t launch_bytecode_t(const SgProg& g, const SgArgs& a, int grid, cudaStream_t s) {
+template <class T, int C> cudaError_t launch_pass1d_bytecode(const SgProg& g, const SgArgs& a, int grid, cudaStream_t s) {
+    static bool attr_set = false;
+    if (!attr_set) { cudaFuncSetAttribute(pass1d_bytecode<T, C>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)vm_file_bytes(VM_VREG, 1)); attr_set = true; }
+    pass1d_bytecode<T, C><<<grid, BLOCK, vm_file_bytes(g.shape.n_vreg, C), s>>>(g, a);
+    return cudaGetLastError();
+}
+template <class T> cudaError_t launch_bytecode_t(const SgProg& g, const SgArgs& a, const SgGeom& geom, cudaStream_t s) {
     if (g.shape.flags & PF_FILTER) {
         static bool attr_set = false;
         if (!attr_set) { cudaFuncSetAttribute(filter1d_bytecode<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FilterBytecodeEval<T>::SMEM); attr_set = true; }
-        filter1d_bytecode<T><<<grid, BLOCK + 32, FilterBytecodeEval<T>::SMEM, s>>>(g, a);
+        filter1d_bytecode<T><<<geom.grid, BLOCK + 32, FilterBytecodeEval<T>::SMEM, s>>>(g, a);
+        return cudaGetLastError();
     }
-    else {
-        static bool attr_set = false;
-        if (!attr_set) { cudaFuncSetAttribute(pass1d_bytecode<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)VM_FILE_BYTES); attr_set = true; }
-        pass1d_bytecode<T><<<grid, BLOCK, VM_FILE_BYTES, s>>>(g, a);
-    }
-    return cudaGetLastError();
+    return geom.vm_cells == 2 ? launch_pass1d_bytecode<T, 2>(g, a, geom.grid, s) : launch_pass1d_bytecode<T, 1>(g, a, geom.grid, s);
 }
-template <class T> int occupancy_bytecode_t(bool filter) {
-    static int cached[2] = {0, 0};
-    if (cached[filter] > 0) return cached[filter];
+// blocks per SM of the bytecode kernels (the 1-D pass depends on the size of its register file: queried once per size)
+template <class T> int occupancy_bytecode_t(bool filter, int n_vreg, int cells) {
+    static int cached_filter = 0, cached[VM_VREG + 1][VM_MAX_CELLS + 1] = {};
     int occ = 0;
-    if (filter) cudaFuncSetAttribute(filter1d_bytecode<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FilterBytecodeEval<T>::SMEM);
-    else cudaFuncSetAttribute(pass1d_bytecode<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)VM_FILE_BYTES);
-    cudaError_t e = filter ? cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, filter1d_bytecode<T>, BLOCK + 32, FilterBytecodeEval<T>::SMEM)
-                           : cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, pass1d_bytecode<T>, BLOCK, VM_FILE_BYTES);
+    cudaError_t e;
+    if (filter) {
+        if (cached_filter > 0) return cached_filter;
+        cudaFuncSetAttribute(filter1d_bytecode<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FilterBytecodeEval<T>::SMEM);
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, filter1d_bytecode<T>, BLOCK + 32, FilterBytecodeEval<T>::SMEM);
+        if (e != cudaSuccess || occ <= 0) return 1;
+        return cached_filter = occ;
+    }
+    n_vreg = std::min(std::max(n_vreg, 1), VM_VREG);
+    if (cached[n_vreg][cells] > 0) return cached[n_vreg][cells];
+    const size_t smem = vm_file_bytes(n_vreg, cells);
+    if (cells == 2) {
+        cudaFuncSetAttribute(pass1d_bytecode<T, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)vm_file_bytes(VM_VREG, 1));
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, pass1d_bytecode<T, 2>, BLOCK, smem);
+    } else {
+        cudaFuncSetAttribute(pass1d_bytecode<T, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)vm_file_bytes(VM_VREG, 1));
+        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, pass1d_bytecode<T, 1>, BLOCK, smem);
+    }
     if (e != cudaSuccess || occ <= 0) return 1;
-    cached[filter] = occ;
-    return occ;
+    return cached[n_vreg][cells] = occ;
 }
-int occupancy_bytecode(int dtype, bool filter) {
+int occupancy_bytecode(int dtype, bool filter, int n_vreg = VM_VREG, int cells = 1) {
     switch (dtype) {
-        case DT_F32: return occupancy_bytecode_t<float>(filter);
-        case DT_F64: return occupancy_bytecode_t<double>(filter);
-        case DT_I32: return occupancy_bytecode_t<int32_t>(filter);
-        default: return occupancy_bytecode_t<long long>(filter);
+        case DT_F32: return occupancy_bytecode_t<float>(filter, n_vreg, cells);
+        case DT_F64: return occupancy_bytecode_t<double>(filter, n_vreg, cells);
+        case DT_I32: return occupancy_bytecode_t<int32_t>(filter, n_vreg, cells);
+        default: return occupancy_bytecode_t<long long>(filter, n_vreg, cells);
     }
 }
 
@@ -271,7 +286,9 @@ int sgk_plan(const SgProg& prog, SgArgs& a, int force_bytecode, int sm_count, in
     // 1-D pass.  Template instances need every vector operand congruent (common head); otherwise the bytecode
     // kernel runs with per-operand 128-bit eligibility.
     if (tid && !congruent) tid = 0;
-    const int tile = tid ? g_entries[tid].tile : vm_tile(es);
+    const int cells = vm_cells(prog.shape.n_vreg);
+    const int tile = tid ? g_entries[tid].tile : vm_tile(es, cells);
+    geom->vm_cells = cells;
     long lmin = a.n;
     for (int o = 0; o < prog.shape.n_out; ++o) lmin = std::min<long>(lmin, a.out_len[o]);
     const long head = std::min<long>((V - mis) % V, a.n);
@@ -279,7 +296,7 @@ int sgk_plan(const SgProg& prog, SgArgs& a, int force_bytecode, int sm_count, in
     a.head = head;
     a.n_full_tiles = body / tile;
     a.vec_ok = vec_ok;
-    const int occ = has_device ? (tid ? g_entries[tid].occupancy() : occupancy_bytecode(prog.shape.dtype, false)) : 4;
+    const int occ = has_device ? (tid ? g_entries[tid].occupancy() : occupancy_bytecode(prog.shape.dtype, false, prog.shape.n_vreg, cells)) : 4;
     long want = tid ? a.n_full_tiles : ((a.n - head + tile - 1) / tile + (head + tile - 1) / tile);
     geom->template_id = tid;
     geom->tile = tile;
@@ -291,10 +308,10 @@ int sgk_plan(const SgProg& prog, SgArgs& a, int force_bytecode, int sm_count, in
 cudaError_t sgk_launch(const SgProg& prog, const SgArgs& args, const SgGeom& geom, cudaStream_t stream) {
     if (geom.template_id > 0) return g_entries[geom.template_id].launch(args, geom.grid, stream);
     switch (prog.shape.dtype) {
-        case DT_F32: return launch_bytecode_t<float>(prog, args, geom.grid, stream);
-        case DT_F64: return launch_bytecode_t<double>(prog, args, geom.grid, stream);
-        case DT_I32: return launch_bytecode_t<int32_t>(prog, args, geom.grid, stream);
-        case DT_I64: return launch_bytecode_t<long long>(prog, args, geom.grid, stream);
+        case DT_F32: return launch_bytecode_t<float>(prog, args, geom, stream);
+        case DT_F64: return launch_bytecode_t<double>(prog, args, geom, stream);
+        case DT_I32: return launch_bytecode_t<int32_t>(prog, args, geom, stream);
+        case DT_I64: return launch_bytecode_t<long long>(prog, args, geom, stream);
         default: return cudaErrorInvalidValue;
     }
 }

@@ -14,6 +14,7 @@ struct SgGeom {
     size_t ws_bytes;        // workspace bytes this launch needs (partial cells)
     size_t state_words;     // filter: tile-state words needed
     int ctrl_words;         // control words needed beyond the first 8 (2-D tickets)
+    int vm_cells;           // bytecode 1-D pass: cells per VM register (1 or 2)
 };
 
 // Registry of precompiled template instances (sg_templates_gen.inc).

@@ -12,29 +12,35 @@ namespace sgk {
 constexpr int VM_VREG = 16;     // value registers of the bytecode evaluator (plan builder reuses dead registers)
 // elements per thread per tile: one 128-bit access per operand
 template <class T> struct VmE { static constexpr int value = 16 / (int)sizeof(T); };
-__host__ __device__ constexpr int vm_tile(int elem_size) { return BLOCK * (16 / elem_size); }
+__host__ __device__ constexpr int vm_tile(int elem_size, int cells) { return BLOCK * (16 / elem_size) * cells; }
 
 // The value register file lives in SHARED memory: register k of thread t is the 16-byte cell at
 //     base + k * VM_REG_STRIDE + t * 16
 // (consecutive threads -> consecutive cells: conflict-free 128-bit accesses).  A register number is then just an
 // address offset — no per-register switch, about forty hardware registers per thread instead of 160+, so three
 // blocks run per SM where one did.  VM_FILE_BYTES of dynamic shared memory per block.
-constexpr uint32_t VM_REG_STRIDE = BLOCK * 16;
-constexpr size_t VM_FILE_BYTES = (size_t)VM_VREG * VM_REG_STRIDE;
+constexpr uint32_t VM_CELL_STRIDE = BLOCK * 16;      // bytes between the cells of one register (one cell per thread)
+constexpr int VM_MAX_CELLS = 2;                      // cells (independent 16-byte vectors) per register and thread
+__host__ __device__ constexpr int vm_cells(int n_vreg) { return n_vreg <= 8 ? 2 : 1; }       // keep the file <= 64 KiB
+__host__ __device__ constexpr size_t vm_file_bytes(int n_vreg, int cells) { return (size_t)(n_vreg > 0 ? n_vreg : 1) * cells * VM_CELL_STRIDE; }
+constexpr size_t VM_FILE_BYTES = (size_t)VM_VREG * VM_CELL_STRIDE;       // single-cell file of the filter evaluator
 
 template <class T, int E> struct VmRegs {
     static_assert(E * sizeof(T) == 16, "one 128-bit cell per register");
     uint32_t base;      // shared-window address of this thread's cell of register 0
-    __device__ __forceinline__ explicit VmRegs(uint32_t file_base) : base(file_base + (threadIdx.x & (BLOCK - 1)) * 16u) {}
+    uint32_t stride;    // bytes between registers = cells * VM_CELL_STRIDE
+    VmRegs() = default;
+    __device__ __forceinline__ explicit VmRegs(uint32_t file_base, int cell = 0, int cells = 1)
+        : base(file_base + (uint32_t)cell * VM_CELL_STRIDE + (threadIdx.x & (BLOCK - 1)) * 16u), stride((uint32_t)cells * VM_CELL_STRIDE) {}
     __device__ __forceinline__ void get(uint8_t k, T (&o)[E]) const {
         uint32_t w[4];
-        asm volatile("ld.shared.v4.b32 {%0,%1,%2,%3}, [%4];" : "=r"(w[0]), "=r"(w[1]), "=r"(w[2]), "=r"(w[3]) : "r"(base + k * VM_REG_STRIDE) : "memory");
+        asm volatile("ld.shared.v4.b32 {%0,%1,%2,%3}, [%4];" : "=r"(w[0]), "=r"(w[1]), "=r"(w[2]), "=r"(w[3]) : "r"(base + k * stride) : "memory");
         memcpy(o, w, 16);
     }
     __device__ __forceinline__ void put(uint8_t k, const T (&o)[E]) {
         uint32_t w[4];
         memcpy(w, o, 16);
-        asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};" ::"r"(base + k * VM_REG_STRIDE), "r"(w[0]), "r"(w[1]), "r"(w[2]), "r"(w[3]) : "memory");
+        asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};" ::"r"(base + k * stride), "r"(w[0]), "r"(w[1]), "r"(w[2]), "r"(w[3]) : "memory");
     }
 };
 
@@ -45,39 +51,66 @@ template <int E> __device__ __forceinline__ unsigned int pput(unsigned int pf, u
     return (pf & ~m) | ((bits << (k * E)) & m);
 }
 
-template <class T, int E>
-__device__ __forceinline__ void vm_exec(const SgProg& g, VmRegs<T, E>& rf, unsigned int& pf) {
+// One decode per instruction, applied to C independent cells (2 x the elements per decode, 2 x the ILP).  The result of the
+// previous value instruction stays in hardware registers: an operand that names it is not re-read from shared memory.
+template <class T, int E, int C>
+__device__ __forceinline__ void vm_exec(const SgProg& g, VmRegs<T, E> (&rf)[C], unsigned int (&pf)[C]) {
+    T last[C][E];
+    int last_dst = -1;
+#pragma unroll
+    for (int c = 0; c < C; ++c)
+#pragma unroll
+        for (int e = 0; e < E; ++e) last[c][e] = T(0);
     for (int i = 0; i < g.shape.n_instr; ++i) {
         const SgInstr ins = g.code[i];
         if (op_is_value(ins.op) || op_is_compare(ins.op)) {
-            T x[E], y[E];
-            rf.get(ins.a, x);
-            rf.get(ins.b, y);
+            T x[C][E], y[C][E];
+            const bool fa = ins.a == last_dst, fb = ins.b == last_dst;      // uniform
+#pragma unroll
+            for (int c = 0; c < C; ++c) {
+                if (fa) { _Pragma("unroll") for (int e = 0; e < E; ++e) x[c][e] = last[c][e]; } else rf[c].get(ins.a, x[c]);
+                if (fb) { _Pragma("unroll") for (int e = 0; e < E; ++e) y[c][e] = last[c][e]; } else rf[c].get(ins.b, y[c]);
+            }
             if (op_is_value(ins.op)) {
-                T z[E];
                 switch (ins.op) {
-#define VOP(OPC) case OPC: _Pragma("unroll") for (int e = 0; e < E; ++e) z[e] = value_op<T>(OPC, x[e], y[e]); break;
+#define VOP(OPC) case OPC: _Pragma("unroll") for (int c = 0; c < C; ++c) _Pragma("unroll") for (int e = 0; e < E; ++e) last[c][e] = value_op<T>(OPC, x[c][e], y[c][e]); break;
                     VOP(OP_ADD) VOP(OP_SUB) VOP(OP_MUL) VOP(OP_DIV) VOP(OP_MIN) VOP(OP_MAX) VOP(OP_MOD) VOP(OP_NEG) VOP(OP_ABS)
 #undef VOP
-                    default: _Pragma("unroll") for (int e = 0; e < E; ++e) z[e] = x[e]; break;
+                    default: _Pragma("unroll") for (int c = 0; c < C; ++c) _Pragma("unroll") for (int e = 0; e < E; ++e) last[c][e] = x[c][e]; break;
                 }
-                rf.put(ins.dst, z);
+                last_dst = ins.dst;
+#pragma unroll
+                for (int c = 0; c < C; ++c) rf[c].put(ins.dst, last[c]);
             } else {
-                unsigned int bits = 0;
-                switch (ins.op) {
-#define COP(OPC) case OPC: _Pragma("unroll") for (int e = 0; e < E; ++e) bits |= (unsigned int)compare_op<T>(OPC, x[e], y[e]) << e; break;
-                    COP(OP_EQ) COP(OP_NE) COP(OP_LT) COP(OP_LE) COP(OP_GT)
+#pragma unroll
+                for (int c = 0; c < C; ++c) {
+                    unsigned int bits = 0;
+                    switch (ins.op) {
+#define COP(OPC) case OPC: _Pragma("unroll") for (int e = 0; e < E; ++e) bits |= (unsigned int)compare_op<T>(OPC, x[c][e], y[c][e]) << e; break;
+                        COP(OP_EQ) COP(OP_NE) COP(OP_LT) COP(OP_LE) COP(OP_GT)
 #undef COP
-                    default: _Pragma("unroll") for (int e = 0; e < E; ++e) bits |= (unsigned int)(x[e] >= y[e]) << e; break;
+                        default: _Pragma("unroll") for (int e = 0; e < E; ++e) bits |= (unsigned int)(x[c][e] >= y[c][e]) << e; break;
+                    }
+                    pf[c] = pput<E>(pf[c], ins.dst, bits);
                 }
-                pf = pput<E>(pf, ins.dst, bits);
             }
         } else {
-            const unsigned int x = pget<E>(pf, ins.a), y = pget<E>(pf, ins.b);
-            const unsigned int z = ins.op == OP_AND ? (x & y) : ins.op == OP_OR ? (x | y) : ~x;
-            pf = pput<E>(pf, ins.dst, z);
+#pragma unroll
+            for (int c = 0; c < C; ++c) {
+                const unsigned int x = pget<E>(pf[c], ins.a), y = pget<E>(pf[c], ins.b);
+                const unsigned int z = ins.op == OP_AND ? (x & y) : ins.op == OP_OR ? (x | y) : ~x;
+                pf[c] = pput<E>(pf[c], ins.dst, z);
+            }
         }
     }
+}
+// single-cell form (filter evaluator)
+template <class T, int E>
+__device__ __forceinline__ void vm_exec(const SgProg& g, VmRegs<T, E>& rf, unsigned int& pf) {
+    VmRegs<T, E> r1[1] = {rf};
+    unsigned int p1[1] = {pf};
+    vm_exec<T, E, 1>(g, r1, p1);
+    pf = p1[0];
 }
 
 // load input k for E consecutive elements starting at i (guarded: elements >= limit read as zero)
@@ -158,11 +191,11 @@ __device__ __forceinline__ void vm_emit(const SgProg& g, const SgArgs& a, int64_
     }
 }
 
-template <class T>
+template <class T, int C>
 __global__ void __launch_bounds__(BLOCK, 3) pass1d_bytecode(const __grid_constant__ SgProg g, const __grid_constant__ SgArgs a) {
     extern __shared__ __align__(16) unsigned char vm_file[];
     constexpr int E = VmE<T>::value;
-    constexpr int VM_TILE = BLOCK * E;
+    constexpr int VM_TILE = BLOCK * E * C;          // C cells of BLOCK*E consecutive elements each
     Cell acc[SG_MAX_OUT];
     uint8_t kind[SG_MAX_OUT];
     bool has_reduction = false;
@@ -176,8 +209,13 @@ __global__ void __launch_bounds__(BLOCK, 3) pass1d_bytecode(const __grid_constan
     }
     const bool early_exit = (g.shape.flags & PF_EARLY_EXIT) && !a.no_early_exit;
 
-    VmRegs<T, E> rf((uint32_t)__cvta_generic_to_shared(vm_file));
-    unsigned int pf = 0;
+    const uint32_t file = (uint32_t)__cvta_generic_to_shared(vm_file);
+    VmRegs<T, E> rf[C];
+#pragma unroll
+    for (int c = 0; c < C; ++c) rf[c] = VmRegs<T, E>(file, c, C);
+    unsigned int pf[C];
+#pragma unroll
+    for (int c = 0; c < C; ++c) pf[c] = 0;
     for (int k = 0; k < g.shape.n_in; ++k) {
         const SgIn in = g.in[k];
         if (in.kind == IN_SCALAR || in.kind == IN_IMM) {
@@ -185,27 +223,36 @@ __global__ void __launch_bounds__(BLOCK, 3) pass1d_bytecode(const __grid_constan
             const T s = load_elem<T>(in.kind, in.ref, k, a, 0);
 #pragma unroll
             for (int e = 0; e < E; ++e) x[e] = s;
-            rf.put(in.reg, x);
+#pragma unroll
+            for (int c = 0; c < C; ++c) rf[c].put(in.reg, x);
         }
     }
     // tiles over the aligned body [head, n) — the last tile is guarded; then the head [0, head) one vector at a time
     const int64_t body = a.n - a.head;
     const int64_t n_tiles = (body + VM_TILE - 1) / VM_TILE;
     const int64_t head_tiles = (a.head + VM_TILE - 1) / VM_TILE;
-    for (int64_t tile = blockIdx.x; tile < n_tiles + head_tiles; tile += gridDim.x) {
-        if (early_exit) {
-            const unsigned int w = ld_volatile_u32(&a.ctrl[1]);
+    unsigned int it = 0;
+    for (int64_t tile = blockIdx.x; tile < n_tiles + head_tiles; tile += gridDim.x, ++it) {
+        if (early_exit && (it & 7u) == 0) {
+            const unsigned int w = ld_relaxed_u32(&a.ctrl[1]);
             if ((w & need_mask) == need_mask || (w & a.exit_any) != 0) break;
         }
-        int64_t i, hi;
-        if (tile < n_tiles) { i = a.head + tile * VM_TILE + (int64_t)threadIdx.x * E; hi = a.n; }
-        else { i = (tile - n_tiles) * VM_TILE + (int64_t)threadIdx.x * E; hi = a.head; }
-        if (i < hi) {
-            // full: the whole vector lies inside every value's length and the body is 16-byte aligned
+        int64_t i[C], hi;
+        const bool in_body = tile < n_tiles;
+        hi = in_body ? a.n : a.head;
+#pragma unroll
+        for (int c = 0; c < C; ++c)
+            i[c] = (in_body ? a.head + tile * VM_TILE : (tile - n_tiles) * VM_TILE) + (int64_t)c * (BLOCK * E) + (int64_t)threadIdx.x * E;
+        if (i[0] < hi) {
+            // full: the whole tile lies inside every value's length and the body is 16-byte aligned
             const bool full = (tile < a.n_full_tiles);
-            for (int k = 0; k < g.shape.n_in; ++k) vm_load<T, E>(g, a, k, i, full, rf, pf);
-            vm_exec<T, E>(g, rf, pf);
-            vm_emit<T, E>(g, a, i, hi, full, rf, pf, acc);
+#pragma unroll
+            for (int c = 0; c < C; ++c)
+                for (int k = 0; k < g.shape.n_in; ++k) vm_load<T, E>(g, a, k, i[c], full, rf[c], pf[c]);      // guarded: reads past the end give zeros
+            vm_exec<T, E, C>(g, rf, pf);
+#pragma unroll
+            for (int c = 0; c < C; ++c)
+                if (i[c] < hi) vm_emit<T, E>(g, a, i[c], hi, full, rf[c], pf[c], acc);
         }
         if (early_exit) {
 #pragma unroll
