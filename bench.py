@@ -185,6 +185,12 @@ def cfg0_section(torch, sg, W, inputs, measure):
     a, b, c = (torch.from_numpy(inputs.uniform_pm1_f64(1, s, n0)).cuda() for s in range(3))
     measure("cfg0_fp64_2^20_chain_sum_max_min_contracts (L2-warm, 2 passes)", lambda ctx: W.cfg0(ctx, n0, a.data_ptr(), b.data_ptr(), c.data_ptr()), 64 << 20, 200)
     measure("cfg0_onepass (z released, L2-warm)", lambda ctx: W.cfg0(ctx, n0, a.data_ptr(), b.data_ptr(), c.data_ptr(), keep_z=False), 24 << 20, 200)
+    # the same two plans with the L2 flushed before every repetition (a 256 MiB scratch buffer is overwritten outside the timed events)
+    scratch = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+    measure("cfg0_fp64_2^20_chain_sum_max_min_contracts (L2-cold, 2 passes)", lambda ctx: W.cfg0(ctx, n0, a.data_ptr(), b.data_ptr(), c.data_ptr()), 64 << 20, 5,
+            restore=lambda: scratch.zero_())
+    measure("cfg0_onepass (z released, L2-cold)", lambda ctx: W.cfg0(ctx, n0, a.data_ptr(), b.data_ptr(), c.data_ptr(), keep_z=False), 24 << 20, 5,
+            restore=lambda: scratch.zero_())
 
 
 def cfg1_section(torch, sg, W, inputs, measure):
