@@ -191,9 +191,266 @@ __device__ __forceinline__ void vm_emit(const SgProg& g, const SgArgs& a, int64_
     }
 }
 
+// ---------------------------------------------------------------------------------------------------------
+// Pre-decoded micro-ops.  The program is the same for every tile, so it is decoded ONCE per block into shared
+// memory: one 16-byte micro-op per instruction = {opcode, dst, a, b} where a value register is already the byte
+// offset of its cell 0 in the register file and a predicate register is already its shift in the predicate word.
+// Per instruction a tile then costs one broadcast 128-bit shared load, one indexed branch (the dense opcode switch
+// compiles to a jump table) and the operand accesses at `base + offset (+ cell * VM_CELL_STRIDE)`.
+// ---------------------------------------------------------------------------------------------------------
+// micro-op word x = opcode + forwarding variant (operand a / b is the previous value result) + VM_ST (write the result back)
+constexpr uint32_t VM_FA = OP_COUNT_, VM_FB = 2 * OP_COUNT_, VM_ST = 0x100;
+struct VmTables {
+    uint4 uop[SG_MAX_INSTR];    // {op, dst, a, b}
+    uint4 vin[SG_MAX_IN];       // 128-bit loadable vector inputs: {ptr.lo, ptr.hi, register byte offset, input index}
+    int n_vin, n_slow;          // inputs served by the list above / by the generic loader (shifted, strided, BOOL, misaligned)
+    uint8_t slow[SG_MAX_IN];
+};
+
+template <int E, int C> __device__ __forceinline__ void vm_decode(const SgProg& g, const SgArgs& a, VmTables& t) {
+    const uint32_t stride = (uint32_t)C * VM_CELL_STRIDE;
+    const int n = g.shape.n_instr;
+    // fwd[i]: which operand slot of instruction i is the result of the most recent value instruction (kept in hardware registers)
+    uint8_t fwd[SG_MAX_INSTR];
+    int last_dst = -1;
+    for (int i = 0; i < n; ++i) {
+        const SgInstr ins = g.code[i];
+        const bool reads_v = op_is_value(ins.op) || op_is_compare(ins.op);
+        const bool unary = ins.op == OP_NEG || ins.op == OP_ABS || ins.op == OP_MOV;
+        fwd[i] = 0;
+        if (reads_v && last_dst >= 0) {
+            if (ins.a == last_dst) fwd[i] = VM_FA;
+            else if (!unary && ins.b == last_dst) fwd[i] = VM_FB;
+        }
+        if (op_is_value(ins.op)) last_dst = ins.dst;
+    }
+    for (int i = 0; i < n; ++i) {
+        const SgInstr ins = g.code[i];
+        uint4 u;
+        bool store = false;
+        if (op_is_value(ins.op)) {
+            // the result must reach the shared-memory file unless every later read of it (before the register is
+            // redefined) is a forwarded operand slot and no output reads it
+            for (int o = 0; o < g.shape.n_out; ++o) {
+                const uint8_t k = g.out[o].kind;
+                if ((k == OUT_STORE || k == OUT_SUM || k == OUT_MAX || k == OUT_MIN || k == OUT_FILTER) && g.out[o].src == ins.dst) store = true;
+            }
+            for (int j = i + 1; j < n && !store; ++j) {
+                const SgInstr nx = g.code[j];
+                if (op_is_value(nx.op) || op_is_compare(nx.op)) {
+                    const bool unary = nx.op == OP_NEG || nx.op == OP_ABS || nx.op == OP_MOV;
+                    if (nx.a == ins.dst && fwd[j] != VM_FA) store = true;
+                    if (!unary && nx.b == ins.dst && fwd[j] != VM_FB) store = true;
+                }
+                if (op_is_value(nx.op) && nx.dst == ins.dst) break;
+            }
+            u.y = ins.dst * stride; u.z = ins.a * stride; u.w = ins.b * stride;
+        } else if (op_is_compare(ins.op)) { u.y = ins.dst * E; u.z = ins.a * stride; u.w = ins.b * stride; }
+        else { u.y = ins.dst * E; u.z = ins.a * E; u.w = ins.b * E; }
+        u.x = (uint32_t)ins.op + fwd[i] + (store ? VM_ST : 0u);
+        t.uop[i] = u;
+    }
+    int nv = 0, ns = 0;
+    for (int k = 0; k < g.shape.n_in; ++k) {
+        const SgIn in = g.in[k];
+        if (in.kind == IN_SCALAR || in.kind == IN_IMM) continue;      // loaded once, before the tile loop
+        if (in.kind == IN_VEC && ((a.vec_ok >> k) & 1)) {
+            const unsigned long long p = (unsigned long long)a.in_ptr[k];
+            t.vin[nv++] = make_uint4((uint32_t)p, (uint32_t)(p >> 32), in.reg * stride, (uint32_t)k);
+        } else t.slow[ns++] = (uint8_t)k;
+    }
+    t.n_vin = nv; t.n_slow = ns;
+}
+
+__device__ __forceinline__ uint4 lds128(uint32_t addr) {
+    uint4 w;
+    asm volatile("ld.shared.v4.b32 {%0,%1,%2,%3}, [%4];" : "=r"(w.x), "=r"(w.y), "=r"(w.z), "=r"(w.w) : "r"(addr) : "memory");
+    return w;
+}
+__device__ __forceinline__ void sts128(uint32_t addr, const uint4& w) {
+    asm volatile("st.shared.v4.b32 [%0], {%1,%2,%3,%4};" ::"r"(addr), "r"(w.x), "r"(w.y), "r"(w.z), "r"(w.w) : "memory");
+}
+template <class T, int E, int C> __device__ __forceinline__ void vm_get(uint32_t addr, T (&o)[C][E]) {
+#pragma unroll
+    for (int c = 0; c < C; ++c) { const uint4 w = lds128(addr + (uint32_t)c * VM_CELL_STRIDE); memcpy(o[c], &w, 16); }
+}
+template <class T, int E, int C> __device__ __forceinline__ void vm_put(uint32_t addr, const T (&o)[C][E]) {
+#pragma unroll
+    for (int c = 0; c < C; ++c) { uint4 w; memcpy(&w, o[c], 16); sts128(addr + (uint32_t)c * VM_CELL_STRIDE, w); }
+}
+
+// `base` = shared-window address of this thread's cell 0 of register 0; `uops` = address of the micro-op table.
+// `last` (the previous value result) stays in hardware registers: a forwarded operand is not re-read from shared memory and a
+// result that only forwarded operands consume is never written there (shared-memory bandwidth bounds this kernel otherwise).
+template <class T, int E, int C>
+__device__ __forceinline__ void vm_exec_uops(uint32_t uops, int n_instr, uint32_t base, unsigned int (&pf)[C]) {
+    constexpr unsigned int EM = (1u << E) - 1u;
+    T last[C][E];
+#pragma unroll
+    for (int c = 0; c < C; ++c)
+#pragma unroll
+        for (int e = 0; e < E; ++e) last[c][e] = T(0);
+    for (int i = 0; i < n_instr; ++i) {
+        const uint4 u = lds128(uops + (uint32_t)i * 16u);      // same address in every thread: a broadcast
+        switch (u.x & 0xffu) {
+#define SG_VM_EACH _Pragma("unroll") for (int c = 0; c < C; ++c) _Pragma("unroll") for (int e = 0; e < E; ++e)
+#define SG_VM_BIN(OPC)                                                                                           \
+    case OPC: {                                                                                                  \
+        T x[C][E], y[C][E];                                                                                      \
+        vm_get<T, E, C>(base + u.z, x); vm_get<T, E, C>(base + u.w, y);                                          \
+        SG_VM_EACH last[c][e] = value_op<T>(OPC, x[c][e], y[c][e]);                                              \
+    } break;                                                                                                     \
+    case OPC + VM_FA: {                                                                                          \
+        T y[C][E];                                                                                               \
+        vm_get<T, E, C>(base + u.w, y);                                                                          \
+        SG_VM_EACH last[c][e] = value_op<T>(OPC, last[c][e], y[c][e]);                                           \
+    } break;                                                                                                     \
+    case OPC + VM_FB: {                                                                                          \
+        T x[C][E];                                                                                               \
+        vm_get<T, E, C>(base + u.z, x);                                                                          \
+        SG_VM_EACH last[c][e] = value_op<T>(OPC, x[c][e], last[c][e]);                                           \
+    } break;
+#define SG_VM_UN(OPC)                                                                                            \
+    case OPC: {                                                                                                  \
+        T x[C][E];                                                                                               \
+        vm_get<T, E, C>(base + u.z, x);                                                                          \
+        SG_VM_EACH last[c][e] = value_op<T>(OPC, x[c][e], x[c][e]);                                              \
+    } break;                                                                                                     \
+    case OPC + VM_FA: {                                                                                          \
+        SG_VM_EACH last[c][e] = value_op<T>(OPC, last[c][e], last[c][e]);                                        \
+    } break;
+#define SG_VM_CMP_BODY(OPC, X, Y)                                                                                \
+        _Pragma("unroll") for (int c = 0; c < C; ++c) {                                                          \
+            unsigned int bits = 0;                                                                               \
+            _Pragma("unroll") for (int e = 0; e < E; ++e) bits |= (unsigned int)compare_op<T>(OPC, X[c][e], Y[c][e]) << e; \
+            pf[c] = (pf[c] & ~(EM << u.y)) | (bits << u.y);                                                      \
+        }
+#define SG_VM_CMP(OPC)                                                                                           \
+    case OPC: {                                                                                                  \
+        T x[C][E], y[C][E];                                                                                      \
+        vm_get<T, E, C>(base + u.z, x); vm_get<T, E, C>(base + u.w, y);                                          \
+        SG_VM_CMP_BODY(OPC, x, y)                                                                                \
+    } break;                                                                                                     \
+    case OPC + VM_FA: {                                                                                          \
+        T y[C][E];                                                                                               \
+        vm_get<T, E, C>(base + u.w, y);                                                                          \
+        SG_VM_CMP_BODY(OPC, last, y)                                                                             \
+    } break;                                                                                                     \
+    case OPC + VM_FB: {                                                                                          \
+        T x[C][E];                                                                                               \
+        vm_get<T, E, C>(base + u.z, x);                                                                          \
+        SG_VM_CMP_BODY(OPC, x, last)                                                                             \
+    } break;
+            SG_VM_BIN(OP_ADD) SG_VM_BIN(OP_SUB) SG_VM_BIN(OP_MUL) SG_VM_BIN(OP_DIV) SG_VM_BIN(OP_MIN) SG_VM_BIN(OP_MAX) SG_VM_BIN(OP_MOD)
+            SG_VM_UN(OP_NEG) SG_VM_UN(OP_ABS) SG_VM_UN(OP_MOV)
+            SG_VM_CMP(OP_EQ) SG_VM_CMP(OP_NE) SG_VM_CMP(OP_LT) SG_VM_CMP(OP_LE) SG_VM_CMP(OP_GT) SG_VM_CMP(OP_GE)
+#undef SG_VM_BIN
+#undef SG_VM_UN
+#undef SG_VM_CMP
+#undef SG_VM_CMP_BODY
+#undef SG_VM_EACH
+            case OP_AND:
+#pragma unroll
+                for (int c = 0; c < C; ++c) pf[c] = (pf[c] & ~(EM << u.y)) | ((((pf[c] >> u.z) & (pf[c] >> u.w)) & EM) << u.y);
+                break;
+            case OP_OR:
+#pragma unroll
+                for (int c = 0; c < C; ++c) pf[c] = (pf[c] & ~(EM << u.y)) | ((((pf[c] >> u.z) | (pf[c] >> u.w)) & EM) << u.y);
+                break;
+            default:    // OP_NOT
+#pragma unroll
+                for (int c = 0; c < C; ++c) pf[c] = (pf[c] & ~(EM << u.y)) | (((~(pf[c] >> u.z)) & EM) << u.y);
+                break;
+        }
+        if (u.x & VM_ST) vm_put<T, E, C>(base + u.y, last);
+    }
+}
+
+// outputs of a FULL tile (inside every value's length, vector-aligned): no per-element guards
+template <class T, int E, int C>
+__device__ __forceinline__ void vm_emit_full(const SgProg& g, const SgArgs& a, int64_t i0, uint32_t base, uint32_t stride, const unsigned int (&pf)[C],
+                                             Cell (&acc)[SG_MAX_OUT]) {
+    constexpr unsigned int EM = (1u << E) - 1u;
+#pragma unroll
+    for (int o = 0; o < SG_MAX_OUT; ++o) {
+        if (o >= g.shape.n_out) break;
+        const SgOut out = g.out[o];
+        switch (out.kind) {
+            case OUT_STORE: {
+                T x[C][E];
+                vm_get<T, E, C>(base + out.src * stride, x);
+                if ((a.vec_ok >> (16 + o)) & 1) {
+#pragma unroll
+                    for (int c = 0; c < C; ++c)
+                        st_stream(reinterpret_cast<int4*>(reinterpret_cast<T*>(a.out_ptr[o]) + i0 + (int64_t)c * (BLOCK * E)), *reinterpret_cast<const int4*>(x[c]));
+                } else {
+#pragma unroll
+                    for (int c = 0; c < C; ++c)
+#pragma unroll
+                        for (int e = 0; e < E; ++e) reinterpret_cast<T*>(a.out_ptr[o])[i0 + (int64_t)c * (BLOCK * E) + e] = x[c][e];
+                }
+            } break;
+            case OUT_STORE_BOOL:
+#pragma unroll
+                for (int c = 0; c < C; ++c)
+#pragma unroll
+                    for (int e = 0; e < E; ++e) reinterpret_cast<uint8_t*>(a.out_ptr[o])[i0 + (int64_t)c * (BLOCK * E) + e] = (pf[c] >> (out.src * E + e)) & 1u;
+                break;
+            case OUT_ALL:
+#pragma unroll
+                for (int c = 0; c < C; ++c) acc[o].a &= (unsigned long long)(((pf[c] >> (out.src * E)) & EM) == EM);
+                break;
+            case OUT_ANY:
+#pragma unroll
+                for (int c = 0; c < C; ++c) acc[o].a |= (unsigned long long)(((pf[c] >> (out.src * E)) & EM) != 0u);
+                break;
+            case OUT_COUNT:
+#pragma unroll
+                for (int c = 0; c < C; ++c) acc[o].a += (unsigned long long)__popc((pf[c] >> (out.src * E)) & EM);
+                break;
+            case OUT_SUM: case OUT_MAX: case OUT_MIN: {
+                T x[C][E];
+                vm_get<T, E, C>(base + out.src * stride, x);
+                if (out.pred == SG_NO_PRED) {
+                    if (out.kind == OUT_SUM) {
+#pragma unroll
+                        for (int c = 0; c < C; ++c)
+#pragma unroll
+                            for (int e = 0; e < E; ++e) cell_accum_value<T>(OUT_SUM, acc[o], x[c][e]);
+                    } else if (out.kind == OUT_MAX) {
+#pragma unroll
+                        for (int c = 0; c < C; ++c)
+#pragma unroll
+                            for (int e = 0; e < E; ++e) cell_accum_value<T>(OUT_MAX, acc[o], x[c][e]);
+                    } else {
+#pragma unroll
+                        for (int c = 0; c < C; ++c)
+#pragma unroll
+                            for (int e = 0; e < E; ++e) cell_accum_value<T>(OUT_MIN, acc[o], x[c][e]);
+                    }
+                } else {
+#pragma unroll
+                    for (int c = 0; c < C; ++c) {
+                        const unsigned int mask = (pf[c] >> (out.pred * E)) & EM;
+#pragma unroll
+                        for (int e = 0; e < E; ++e)
+                            if ((mask >> e) & 1u) {
+                                if (out.kind == OUT_SUM) cell_accum_value<T>(OUT_SUM, acc[o], x[c][e]);
+                                else if (out.kind == OUT_MAX) cell_accum_value<T>(OUT_MAX, acc[o], x[c][e]);
+                                else cell_accum_value<T>(OUT_MIN, acc[o], x[c][e]);
+                            }
+                    }
+                }
+            } break;
+            default: break;     // OUT_FILTER: handled by the compaction kernel
+        }
+    }
+}
+
 template <class T, int C>
 __global__ void __launch_bounds__(BLOCK, 3) pass1d_bytecode(const __grid_constant__ SgProg g, const __grid_constant__ SgArgs a) {
     extern __shared__ __align__(16) unsigned char vm_file[];
+    __shared__ __align__(16) VmTables tab;
     constexpr int E = VmE<T>::value;
     constexpr int VM_TILE = BLOCK * E * C;          // C cells of BLOCK*E consecutive elements each
     Cell acc[SG_MAX_OUT];
@@ -209,7 +466,11 @@ __global__ void __launch_bounds__(BLOCK, 3) pass1d_bytecode(const __grid_constan
     }
     const bool early_exit = (g.shape.flags & PF_EARLY_EXIT) && !a.no_early_exit;
 
+    if (threadIdx.x == 0) vm_decode<E, C>(g, a, tab);
     const uint32_t file = (uint32_t)__cvta_generic_to_shared(vm_file);
+    const uint32_t uops = (uint32_t)__cvta_generic_to_shared(tab.uop);
+    constexpr uint32_t stride = (uint32_t)C * VM_CELL_STRIDE;
+    const uint32_t base = file + threadIdx.x * 16u;
     VmRegs<T, E> rf[C];
 #pragma unroll
     for (int c = 0; c < C; ++c) rf[c] = VmRegs<T, E>(file, c, C);
@@ -227,6 +488,8 @@ __global__ void __launch_bounds__(BLOCK, 3) pass1d_bytecode(const __grid_constan
             for (int c = 0; c < C; ++c) rf[c].put(in.reg, x);
         }
     }
+    __syncthreads();
+    const int n_instr = g.shape.n_instr, n_vin = tab.n_vin, n_slow = tab.n_slow;
     // tiles over the aligned body [head, n) — the last tile is guarded; then the head [0, head) one vector at a time
     const int64_t body = a.n - a.head;
     const int64_t n_tiles = (body + VM_TILE - 1) / VM_TILE;
@@ -237,22 +500,35 @@ __global__ void __launch_bounds__(BLOCK, 3) pass1d_bytecode(const __grid_constan
             const unsigned int w = ld_relaxed_u32(&a.ctrl[1]);
             if ((w & need_mask) == need_mask || (w & a.exit_any) != 0) break;
         }
-        int64_t i[C], hi;
         const bool in_body = tile < n_tiles;
-        hi = in_body ? a.n : a.head;
+        const int64_t hi = in_body ? a.n : a.head;
+        const int64_t i0 = (in_body ? a.head + tile * VM_TILE : (tile - n_tiles) * VM_TILE) + (int64_t)threadIdx.x * E;
+        // full: the whole tile lies inside every value's length and the body is 16-byte aligned
+        const bool full = (tile < a.n_full_tiles);
+        if (full) {
+            const int64_t boff = i0 * (int64_t)sizeof(T);
+            for (int j = 0; j < n_vin; ++j) {
+                const uint4 v = tab.vin[j];
+                const char* p = reinterpret_cast<const char*>(((unsigned long long)v.y << 32) | v.x) + boff;
+                int4 w[C];
 #pragma unroll
-        for (int c = 0; c < C; ++c)
-            i[c] = (in_body ? a.head + tile * VM_TILE : (tile - n_tiles) * VM_TILE) + (int64_t)c * (BLOCK * E) + (int64_t)threadIdx.x * E;
-        if (i[0] < hi) {
-            // full: the whole tile lies inside every value's length and the body is 16-byte aligned
-            const bool full = (tile < a.n_full_tiles);
+                for (int c = 0; c < C; ++c) w[c] = ld_stream_rw(reinterpret_cast<const int4*>(p + (size_t)c * VM_CELL_STRIDE));
+#pragma unroll
+                for (int c = 0; c < C; ++c) sts128(base + v.z + (uint32_t)c * VM_CELL_STRIDE, *reinterpret_cast<const uint4*>(&w[c]));
+            }
+            for (int j = 0; j < n_slow; ++j)
+#pragma unroll
+                for (int c = 0; c < C; ++c) vm_load<T, E>(g, a, tab.slow[j], i0 + (int64_t)c * (BLOCK * E), false, rf[c], pf[c]);
+            vm_exec_uops<T, E, C>(uops, n_instr, base, pf);
+            vm_emit_full<T, E, C>(g, a, i0, base, stride, pf, acc);
+        } else if (i0 < hi) {
 #pragma unroll
             for (int c = 0; c < C; ++c)
-                for (int k = 0; k < g.shape.n_in; ++k) vm_load<T, E>(g, a, k, i[c], full, rf[c], pf[c]);      // guarded: reads past the end give zeros
-            vm_exec<T, E, C>(g, rf, pf);
+                for (int k = 0; k < g.shape.n_in; ++k) vm_load<T, E>(g, a, k, i0 + (int64_t)c * (BLOCK * E), false, rf[c], pf[c]);      // guarded: reads past the end give zeros
+            vm_exec_uops<T, E, C>(uops, n_instr, base, pf);
 #pragma unroll
             for (int c = 0; c < C; ++c)
-                if (i[c] < hi) vm_emit<T, E>(g, a, i[c], hi, full, rf[c], pf[c], acc);
+                if (i0 + (int64_t)c * (BLOCK * E) < hi) vm_emit<T, E>(g, a, i0 + (int64_t)c * (BLOCK * E), hi, false, rf[c], pf[c], acc);
         }
         if (early_exit) {
 #pragma unroll
