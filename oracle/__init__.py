@@ -212,3 +212,17 @@ def mat_step(M, kr: int, kc: int | None = None):
     colsum = np.empty(cols, dtype=np.float64)
     _chk(lib().orc_mat_step(ctypes.c_int64(rows), ctypes.c_int64(cols), ctypes.c_int64(cols), _p(M), ctypes.c_int64(kr), ctypes.c_int64(kc), _p(rowmax), _p(colsum)), "mat_step")
     return M, rowmax, colsum
+
+
+def ge_determinant(M, eps: float = 0.0):
+    """Listing 5: determinant by Gaussian elimination without pivoting, on a copy.
+
+    Returns (det, eliminated matrix, zero_step) — zero_step is the step whose |pivot| <= eps (det = 0), else -1."""
+    M = np.array(M, dtype=np.float64, order="C", copy=True)
+    if M.ndim != 2 or M.shape[0] != M.shape[1]:
+        raise ValueError("square matrix expected")
+    det = ctypes.c_double(0.0)
+    zs = ctypes.c_int64(-1)
+    _chk(lib().orc_ge_determinant(ctypes.c_int64(M.shape[0]), ctypes.c_int64(M.shape[1]), _p(M), ctypes.c_double(eps),
+                                  ctypes.byref(det), ctypes.byref(zs)), "ge_determinant")
+    return det.value, M, int(zs.value)

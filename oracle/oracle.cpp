@@ -384,4 +384,36 @@ int orc_mat_step(int64_t rows, int64_t cols, int64_t ld, double* M, int64_t kr, 
     return 0;
 }
 
+// Determinant by Gaussian elimination, Listing 5, step by step in the paper's order:
+//     Result := 1
+//     for step = 0 .. n-1:
+//         pivot := M[step][step]
+//         if pivot is approximately 0 -> Result := 0, stop         (PAPER.md:339 double_approx_equals(pivot, 0.0);
+//                                                                   the paper leaves eps open: |pivot| <= eps, R5)
+//         Result := Result * pivot
+//         for every row j > step: the row operation
+// The listing's row operation is garbled and rescales row j; the reading taken is
+// BASELINE.json:configs[4]'s textbook update, the same orc_mat_step defines: f_j = M[j][step] / pivot (read before
+// the row changes), t = f_j * M[step][c], M[j][c] = M[j][c] - t, one rounding per primitive.  M is overwritten by
+// the eliminated matrix; *zero_step = the step whose pivot was ~0, or -1.
+int orc_ge_determinant(int64_t n, int64_t ld, double* M, double eps, double* det, int64_t* zero_step) {
+    if (n < 0 || ld < n) return -3;
+    double result = 1.0;
+    *zero_step = -1;
+    for (int64_t step = 0; step < n; ++step) {
+        const double pivot = M[step * ld + step];
+        if (un(ABS, pivot) <= eps) { result = 0.0; *zero_step = step; break; }
+        result = result * pivot;
+        for (int64_t j = step + 1; j < n; ++j) {
+            const double f = M[j * ld + step] / pivot;
+            for (int64_t c = 0; c < n; ++c) {
+                double t = f * M[step * ld + c];
+                M[j * ld + c] = M[j * ld + c] - t;
+            }
+        }
+    }
+    *det = result;
+    return 0;
+}
+
 }  // extern "C"

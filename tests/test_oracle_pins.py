@@ -496,3 +496,78 @@ def test_cfg3_clean_and_injected():
     assert np.flatnonzero(orc.adj("le", x) == 0).tolist() == [j - 1]      # only the pair (j-1, j) is broken
     x[5] = -1.0
     assert ocfg.cfg3(x)["pre"] is False
+
+
+# ---------------------------------------------------------------------------------------------------------
+# Determinant by Gaussian elimination (Listing 5) — SURVEY.md §8(f)(1)
+# ---------------------------------------------------------------------------------------------------------
+def _leibniz_det(A):
+    """Brute force: sum over all permutations, exact rational arithmetic."""
+    import itertools
+    n = len(A)
+    total = Fraction(0)
+    for perm in itertools.permutations(range(n)):
+        sign = 1
+        for i in range(n):
+            for j in range(i + 1, n):
+                if perm[i] > perm[j]:
+                    sign = -sign
+        term = Fraction(sign)
+        for i in range(n):
+            term *= Fraction(float(A[i][perm[i]]))
+        total += term
+    return total
+
+
+def _exact_lu_matrix(n, rng):
+    """M = L @ U with unit-lower L and upper U of small dyadic entries and power-of-two pivots: every quotient, product
+    and difference of the elimination is exact in fp64, so it must return U bit for bit and det = prod(diag U)."""
+    L = np.tril(rng.integers(-4, 5, (n, n)) / 4.0, -1) + np.eye(n)
+    U = np.triu(rng.integers(-8, 9, (n, n)) / 2.0, 1) + np.diag(2.0 ** rng.integers(-2, 3, n) * rng.choice([-1.0, 1.0], n))
+    return L, U, L @ U
+
+
+def test_ge_determinant_exact_lu_and_brute_force():
+    rng = np.random.default_rng(11)
+    for n in (1, 2, 3, 4, 5, 6):
+        L, U, M = _exact_lu_matrix(n, rng)
+        det, E, zs = orc.ge_determinant(M)
+        assert zs == -1
+        assert np.array_equal(np.triu(E), U)                               # elimination recovers U exactly
+        assert not np.tril(E, -1).any()                                    # and exact zeros below the diagonal
+        assert Fraction(det) == math.prod(Fraction(float(u)) for u in np.diag(U))
+        assert Fraction(det) == _leibniz_det(M.tolist())                   # == the definition of the determinant
+
+
+def test_ge_determinant_hand_values_triangular_and_singular():
+    det, E, zs = orc.ge_determinant([[2.0, 3.0], [4.0, 5.0]])              # f = 2, row 1 -> [0, -1]; 2 * -1
+    assert det == -2.0 and np.array_equal(E, [[2.0, 3.0], [0.0, -1.0]]) and zs == -1
+    T = np.triu(RNG.standard_normal((7, 7))) + 3 * np.eye(7)
+    det, E, zs = orc.ge_determinant(T)                                     # upper triangular: nothing to eliminate
+    ref = 1.0
+    for d in np.diag(T):
+        ref = ref * d                                                      # PAPER.md:338, in step order
+    assert det == ref and np.array_equal(E, T)
+    det, E, zs = orc.ge_determinant([[1.0, 2.0], [2.0, 4.0]])              # second pivot 4 - 2*2 = 0 (PAPER.md:339)
+    assert det == 0.0 and zs == 1
+    det, _, zs = orc.ge_determinant([[1e-9, 1.0], [1.0, 1.0]], eps=1e-6)   # approximately-zero pivot with an explicit eps
+    assert det == 0.0 and zs == 0
+    det, _, zs = orc.ge_determinant(np.zeros((0, 0)))                      # empty product
+    assert det == 1.0 and zs == -1
+
+
+def test_ge_determinant_steps_are_matstep_and_library_det():
+    n = 48
+    M = RNG.uniform(-1, 1, (n, n)) / n + np.eye(n)
+    det, E, zs = orc.ge_determinant(M)
+    A = M.copy()                                                           # the loop is n applications of the cfg4 step
+    ref = 1.0
+    for k in range(n):
+        ref = ref * A[k, k]
+        A = orc.mat_step(A, k)[0]
+    assert det == ref and np.array_equal(E, A) and zs == -1
+    assert abs(det - np.linalg.det(M)) <= 1e-12 * abs(det)                 # LAPACK (partial pivoting): same value to rounding
+    sign, logabs = np.linalg.slogdet(M)
+    assert sign == np.sign(det) and abs(math.log(abs(det)) - logabs) <= 1e-12
+    s = 0.5                                                                # det(s*M) = s^n det(M): exact for a power of two
+    assert orc.ge_determinant(s * M)[0] == det * s ** n
