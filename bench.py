@@ -176,6 +176,8 @@ def per_config(torch, sg, W, inputs, peak, which):
         cfg3_section(torch, sg, W, inputs, measure)
     if "cfg4" in which:
         cfg4_section(torch, sg, W, inputs, measure)
+    if "ge" in which:
+        ge_section(torch, sg, W, inputs, out, peak)
     return out
 
 
@@ -222,6 +224,38 @@ def cfg3_section(torch, sg, W, inputs, measure):
     measure(f"cfg3_fp32_2^28_violation_at_{j} as contracts (early exit; time to answer)", lambda ctx: W.cfg3(ctx, n3, xs.data_ptr(), contracts=True), 4 * n3)
 
 
+def ge_section(torch, sg, W, inputs, out, peak):
+    """the whole determinant loop of Listing 5 (n steps, 3 launches each, no host synchronisation between
+    steps), device time between two events around the loop.  Algorithmic bytes: step k reads and writes the (n-k-1) x n rows
+    below the pivot row (16 B per updated element), plus the pivot row and the factor column."""
+    stream = torch.cuda.current_stream().cuda_stream
+    for n in (4096,):
+        M0 = torch.from_numpy(inputs.boosted_matrix_f64(5, 0, n) / float(n)).cuda()
+        M = M0.clone()
+        alg = sum(16 * (n - k - 1) * n + 8 * n + 24 * (n - k - 1) + 40 for k in range(n))
+        times, wall = [], []
+        det = None
+        for rep in range(3):                       # first repetition is the warm-up
+            M.copy_(M0)
+            d = torch.ones(1, dtype=torch.float64, device="cuda")
+            mp = torch.full((1,), float("inf"), dtype=torch.float64, device="cuda")
+            ctx = sg.sg_ctx_create(0, stream)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            e0.record()
+            det, ok = W.ge_determinant(ctx, n, M.data_ptr(), d.data_ptr(), mp.data_ptr())
+            e1.record()
+            torch.cuda.synchronize()
+            wall.append(1e3 * (time.perf_counter() - t0))
+            times.append(e0.elapsed_time(e1))
+            sg.sg_ctx_destroy(ctx)
+        ms = float(min(times[1:]))
+        out[f"ge_determinant_fp64_{n}^2_whole_loop ({n} steps, 3 launches each, no host sync)"] = {
+            "ms": ms, "wall_ms": float(min(wall[1:])), "algorithmic_bytes": int(alg), "GB/s": alg / ms / 1e6, "frac_of_peak": alg / ms / 1e6 / peak,
+            "passes": 3 * n - 2, "template_passes": 3 * n - 2, "det": det, "launches_per_step": 3}
+
+
 def cfg4_section(torch, sg, W, inputs, measure):
     n4 = 16384
     Mh = inputs.boosted_matrix_f64(5, 0, n4)
@@ -242,7 +276,7 @@ def main():
     ap.add_argument("--log2n", type=int, default=28)
     ap.add_argument("--impl", default="ours")
     ap.add_argument("--headline-only", action="store_true", help="same as --configs none")
-    ap.add_argument("--configs", default="cfg0,cfg1,cfg2,cfg3,cfg4", help="per_config sections to time after the headline (or: none)")
+    ap.add_argument("--configs", default="cfg0,cfg1,cfg2,cfg3,cfg4,ge", help="per_config sections to time after the headline (or: none)")
     ap.add_argument("--skip-headline", action="store_true", help="profiling aid: run only the --configs sections and print their JSON")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3)

@@ -182,6 +182,16 @@ sg_status sg_vec_read(sg_ctx* ctx, sg_handle v, void* host_out, size_t bytes);
 /* Drop the caller's reference.  An unreferenced pending intermediate is never materialised. */
 sg_status sg_release(sg_ctx* ctx, sg_handle h);
 
+/* Listing 5's loop body for steps k in [k0, k1) of the square F64 matrix m, as a library composite over the
+ * primitives above.  Step k: det <- det * M[k,k] and minpiv <- MIN(minpiv, ABS(M[k,k]))
+ * on the one-element F64 vectors det / minpiv, then for ALL rows j > k in one matrix pass M[j,:] <- M[j,:] - (M[j,k]/M[k,k]) * M[k,:]
+ * (BASELINE.json:configs[4]; the factors are read before the rows change).  The pivot stays on the device; every step is
+ * flushed asynchronously and nothing is read back, so n steps run without a host synchronisation.  The caller initialises
+ * det to 1 and minpiv to +inf and tests the zero-pivot condition of PAPER.md:339 on minpiv afterwards (sg_forall of minpiv > eps).
+ * Errors: SG_ERR_ARG (handles, range), SG_ERR_SHAPE (not square, det/minpiv not one element), SG_ERR_DTYPE, SG_ERR_UNSUPPORTED
+ * (rows not 16-byte aligned), SG_ERR_CUDA.  Operations already pending are flushed with step k0. */
+sg_status sg_mat_ge_steps(sg_ctx* ctx, sg_handle m, sg_handle det, sg_handle minpiv, int64_t k0, int64_t k1);
+
 sg_status sg_plan_stats(sg_ctx* ctx, sg_stats* out);
 /* Canonical program of pass `pass` of the last flush as text (template generator, tests). Returns bytes needed. */
 int64_t sg_plan_dump(sg_ctx* ctx, int32_t pass, char* buf, int64_t cap);

@@ -483,6 +483,49 @@ sg_status sg_contract(sg_ctx* c, sg_handle h, int32_t kind, const char* tag) {
 
 sg_status sg_flush(sg_ctx* c) { CK(c); return sg_flush_impl(c); }
 
+// Listing 5's loop body as a composite over the public primitives (no kernel of its own): the native twin of
+// workloads.ge_step + flush, so that a step costs microseconds of host time instead of a scripting language's call overhead.
+sg_status sg_mat_ge_steps(sg_ctx* c, sg_handle m, sg_handle det, sg_handle minpiv, int64_t k0, int64_t k1) {
+    CK(c);
+    Value* vm = val(c, m);
+    Value* vd = val(c, det);
+    Value* vp = val(c, minpiv);
+    if (!vm || !vd || !vp) return sg_fail(c, SG_ERR_ARG, "unknown handle");
+    if (vm->dtype != SG_F64 || vd->dtype != SG_F64 || vp->dtype != SG_F64) return sg_fail(c, SG_ERR_DTYPE, "sg_mat_ge_steps: F64 only");
+    if (vm->rows != vm->cols) return sg_fail(c, SG_ERR_SHAPE, "sg_mat_ge_steps: square matrix expected");
+    if (vd->rows * vd->cols != 1 || vp->rows * vp->cols != 1) return sg_fail(c, SG_ERR_SHAPE, "sg_mat_ge_steps: det and minpiv are one-element vectors");
+    const int64_t n = vm->rows;
+    if (k0 < 0 || k1 > n || k0 > k1) return sg_fail(c, SG_ERR_ARG, "sg_mat_ge_steps: step range");
+    auto H = [](sg_handle h, int32_t bcast) { sg_operand o; memset(&o, 0, sizeof o); o.kind = SG_OPERAND_HANDLE; o.bcast = bcast; o.h = h; return o; };
+    for (int64_t k = k0; k < k1; ++k) {
+        sg_handle tmp[8];
+        int nt = 0;
+        sg_status s = SG_OK;
+        sg_handle rowk = 0, d = 0, ad = 0, out = 0;
+#define SG_TRY(call) do { if (s == SG_OK) s = (call); } while (0)
+        SG_TRY(sg_mat_row(c, m, k, &rowk));                 if (s == SG_OK) tmp[nt++] = rowk;
+        SG_TRY(sg_vec_subset(c, rowk, k, k + 1, &d));       if (s == SG_OK) tmp[nt++] = d;
+        { sg_operand o[2] = {H(det, SG_BCAST_NONE), H(d, SG_BCAST_NONE)}; SG_TRY(sg_enqueue(c, SG_MUL, o, 2, det, &out)); }
+        { sg_operand o[1] = {H(d, SG_BCAST_NONE)}; SG_TRY(sg_enqueue(c, SG_ABS, o, 1, 0, &ad)); if (s == SG_OK) tmp[nt++] = ad; }
+        { sg_operand o[2] = {H(minpiv, SG_BCAST_NONE), H(ad, SG_BCAST_NONE)}; SG_TRY(sg_enqueue(c, SG_MIN, o, 2, minpiv, &out)); }
+        if (k + 1 < n) {
+            sg_handle piv = 0, col = 0, f = 0, sub = 0, t = 0;
+            SG_TRY(sg_mat_elem(c, m, k, k, &piv));              if (s == SG_OK) tmp[nt++] = piv;
+            SG_TRY(sg_mat_col(c, m, k, k + 1, n, &col));        if (s == SG_OK) tmp[nt++] = col;
+            { sg_operand o[2] = {H(col, SG_BCAST_NONE), H(piv, SG_BCAST_NONE)}; SG_TRY(sg_enqueue(c, SG_DIV, o, 2, 0, &f)); if (s == SG_OK) tmp[nt++] = f; }
+            SG_TRY(sg_mat_rows(c, m, k + 1, n, &sub));          if (s == SG_OK) tmp[nt++] = sub;
+            { sg_operand o[2] = {H(f, SG_BCAST_COL), H(rowk, SG_BCAST_ROW)}; SG_TRY(sg_enqueue(c, SG_MUL, o, 2, 0, &t)); if (s == SG_OK) tmp[nt++] = t; }
+            { sg_operand o[2] = {H(sub, SG_BCAST_NONE), H(t, SG_BCAST_NONE)}; SG_TRY(sg_enqueue(c, SG_SUB, o, 2, sub, &out)); }
+        }
+#undef SG_TRY
+        for (int i = nt - 1; i >= 0; --i) sg_release(c, tmp[i]);
+        if (s != SG_OK) return s;
+        s = sg_flush_impl(c);
+        if (s != SG_OK) return s;
+    }
+    return SG_OK;
+}
+
 sg_status sg_scalar_dtype(sg_ctx* c, sg_handle h, int32_t* dtype) {
     CK(c && dtype);
     Value* v = val(c, h);

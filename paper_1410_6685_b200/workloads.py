@@ -166,3 +166,53 @@ def cfg4(ctx, n, pM, k, ld=None):
         sg.sg_release(ctx, h)
     res["sub"] = sub
     return res
+
+
+def ge_step(ctx, M, n, k, det, minpiv):
+    """One step of Listing 5 enqueued without a trigger: Result := Result * pivot and the
+    smallest |pivot| so far on a one-element domain, then, for all rows j > k in ONE matrix pass, the row update of
+    BASELINE.json:configs[4] (the paper launches one kernel per row, its slow case PAPER.md:389).  The pivot stays on the
+    device (sg_mat_elem), nothing is read back."""
+    rowk = sg.sg_mat_row(ctx, M, k)
+    d = sg.sg_vec_subset(ctx, rowk, k, k + 1)                   # M[k,k] as a one-element collection
+    sg.sg_enqueue(ctx, sg.SG_MUL, [det, d], dst_or_0=det)
+    ad = sg.sg_enqueue(ctx, sg.SG_ABS, [d])
+    sg.sg_enqueue(ctx, sg.SG_MIN, [minpiv, ad], dst_or_0=minpiv)
+    tmp = [ad, d]
+    if k + 1 < n:
+        piv = sg.sg_mat_elem(ctx, M, k, k)
+        col = sg.sg_mat_col(ctx, M, k, k + 1, n)
+        f = sg.sg_enqueue(ctx, sg.SG_DIV, [col, piv])          # read BEFORE the rows change: its own small pass
+        sub = sg.sg_mat_rows(ctx, M, k + 1, n)
+        t = sg.sg_enqueue(ctx, sg.SG_MUL, [H(f, sg.SG_BCAST_COL), H(rowk, sg.SG_BCAST_ROW)])
+        sg.sg_enqueue(ctx, sg.SG_SUB, [sub, t], dst_or_0=sub)
+        tmp += [piv, col, f, t, sub]
+    return tmp + [rowk]
+
+
+def ge_determinant(ctx, n, pM, pdet, pminpiv, ld=None, eps=0.0, native=True):
+    """Listing 5: the whole determinant loop with no host synchronisation between steps.
+
+    pdet / pminpiv: device float64[1] initialised by the caller to 1.0 / +inf.  Every step is flushed asynchronously (scalar
+    + factor pass, matrix pass) — by the library composite sg_mat_ge_steps, or (native=False) by the same calls made from here.  The zero-pivot test of PAPER.md:339 is a device-evaluated contract on
+    the smallest |pivot| seen, checked once at the end: the result is 0.0 if it fails, as in the listing.
+    Returns (det, ok)."""
+    ld = n if ld is None else ld
+    M = sg.sg_mat_create(ctx, sg.SG_F64, n, n, ld, pM)
+    det = sg.sg_vec_create(ctx, sg.SG_F64, 1, pdet)
+    minpiv = sg.sg_vec_create(ctx, sg.SG_F64, 1, pminpiv)
+    if native:
+        sg.sg_mat_ge_steps(ctx, M, det, minpiv, 0, n)           # the same steps enqueued and flushed by the library itself
+    else:
+        for k in range(n):
+            for h in ge_step(ctx, M, n, k, det, minpiv):
+                sg.sg_release(ctx, h)
+            sg.sg_flush(ctx)                                    # asynchronous: plan + launches of step k, no read-back
+    gt = sg.sg_enqueue(ctx, sg.SG_GT, [minpiv, F(eps)])
+    ok = sg.sg_forall(ctx, gt)
+    value = sg.sg_reduce(ctx, det, sg.SG_SUM)                   # sum of one element: hands the scalar back (trigger (1))
+    okv = bool(sg.sg_scalar_get(ctx, ok))
+    detv = float(sg.sg_scalar_get(ctx, value))
+    for h in (gt, ok, value, det, minpiv, M):
+        sg.sg_release(ctx, h)
+    return (detv if okv else 0.0), okv

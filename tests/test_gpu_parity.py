@@ -529,3 +529,55 @@ def test_cfg4_full_size_sampled(k):
         wrow = orc.zip("sub", M[j], orc.scalar("mul", M[k], f[0]))
         assert bits_equal(grow, wrow)
         assert rowmax[j - k - 1] == orc.max(orc.unary("abs", wrow))
+
+
+# ----------------------------------------------------------------------------------------------------------
+# the whole Gaussian-elimination determinant loop (Listing 5)
+# ----------------------------------------------------------------------------------------------------------
+def ge_matrix(n, seed=5):
+    """Config 4's matrix scaled by 1/n (diagonal ~ 1, off-diagonal ~ U[-1,1)/n) so that the determinant stays finite."""
+    return inputs.boosted_matrix_f64(seed, 0, n) / float(n)
+
+
+def run_ge(c, M, ld=None, eps=0.0, native=True):
+    n = M.shape[0]
+    ld = n if ld is None else ld
+    buf = np.zeros((n, ld))
+    buf[:, :n] = M
+    t = c.torch.from_numpy(buf).cuda()
+    det = c.torch.ones(1, dtype=c.torch.float64, device="cuda")
+    minpiv = c.torch.full((1,), float("inf"), dtype=c.torch.float64, device="cuda")
+    got, ok = W.ge_determinant(c.ctx, n, t.data_ptr(), det.data_ptr(), minpiv.data_ptr(), ld=ld, eps=eps, native=native)
+    return got, ok, t.cpu().numpy()[:, :n], float(minpiv.item())
+
+
+# even n and ld: a matrix pass needs 16-byte aligned rows (SG_ERR_UNSUPPORTED otherwise, include/sg.h)
+@pytest.mark.parametrize("n,ld", [(1, 1), (2, 2), (4, 6), (18, 18), (64, 64), (130, 136), (258, 258), (514, 520)])
+def test_ge_determinant_loop(n, ld):
+    M = ge_matrix(n)
+    want_det, want_E, zs = orc.ge_determinant(M)
+    assert zs == -1
+    with Ctx() as c:
+        got, ok, E, minpiv = run_ge(c, M, ld)
+        assert ok
+        assert bits_equal(np.array([got]), np.array([want_det]))        # same products in the same order: bit-exact
+        assert bits_equal(np.ascontiguousarray(E), want_E)              # the eliminated matrix, every element
+        assert minpiv == np.min(np.abs(np.diag(want_E)))
+        if n <= 130:                                                    # the same steps driven call by call from the binding
+            got2, ok2, E2, _ = run_ge(c, M, ld, native=False)
+            assert ok2 and got2 == got and bits_equal(np.ascontiguousarray(E2), want_E)
+
+
+def test_ge_determinant_zero_pivot_contract():
+    with Ctx() as c:
+        M = np.array([[1.0, 2.0, 0.0, 0.0], [2.0, 4.0, 1.0, 0.0], [0.0, 1.0, 1.0, 0.0], [0.0, 0.0, 0.0, 1.0]])   # second pivot 4 - 2*2 = 0 (PAPER.md:339)
+        want, _, zs = orc.ge_determinant(M)
+        got, ok, _, minpiv = run_ge(c, M)
+        assert zs == 1 and want == 0.0 and got == 0.0 and not ok and minpiv == 0.0
+    with Ctx() as c:
+        M = np.array([[1e-9, 1.0], [1.0, 1.0]])                             # approximately zero with an explicit eps
+        assert orc.ge_determinant(M, eps=1e-6)[0] == 0.0
+        got, ok, _, _ = run_ge(c, M, eps=1e-6)
+        assert got == 0.0 and not ok
+        got, ok, _, _ = run_ge(c, M, eps=0.0)                               # eps = 0: the tiny pivot is accepted
+        assert ok and bits_equal(np.array([got]), np.array([orc.ge_determinant(M)[0]]))

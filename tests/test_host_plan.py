@@ -136,6 +136,38 @@ def test_cfg1_to_cfg4_plans():
     assert st.bytes_min == 8 * rows + 8 * rows + (2 * 8 * rows * 16384 + 8 * 16384 + 8 * rows) + 8 * rows + 8 * 16384
 
 
+def test_ge_step_is_two_passes_with_no_read_back():
+    """Listing 5's loop body: the paper launches one kernel per row and reads two scalars back per
+    row (its slow case); here a step is a scalar + factor pass and ONE matrix pass over all rows."""
+    def step(k, native=False):
+        def build(c):
+            M = sg.sg_mat_create(c, sg.SG_F64, 1000, 1000, 1000, None)
+            det, mp = sg.sg_vec_create(c, sg.SG_F64, 1, None), sg.sg_vec_create(c, sg.SG_F64, 1, None)
+            if native:
+                sg.sg_mat_ge_steps(c, M, det, mp, k, k + 1)          # the library composite plans the same passes
+            else:
+                for h in W.ge_step(c, M, 1000, k, det, mp):
+                    sg.sg_release(c, h)
+        return build
+    rows = 989
+    for native in (False, True):
+        st, dumps = plan(step(10, native))
+        # det, min |pivot| and the factors share one pass (values of different lengths; it has no precompiled instance and runs
+        # on the bytecode kernel); the rows change in place in the second (template instance)
+        assert st.n_passes == 2 and st.n_template == 1
+        assert "OP_MUL" in dumps[0] and "OP_MIN" in dumps[0] and "IN_STRIDED" in dumps[0] and "IN_SCALAR" in dumps[0] and dumps[0].count("OUT_STORE") == 3
+        assert "IN_COLB" in dumps[1] and "IN_ROWB" in dumps[1] and dumps[1].count("OUT_STORE") == 1
+        assert abs(st.bytes_min - ((3 * 8 + 2 * 8) + (8 * rows + 8 + 8 * rows) + (2 * 8 * rows * 1000 + 8 * 1000 + 8 * rows))) <= 8
+    st, dumps = plan(step(999))                                       # last step: only the scalar pass
+    assert st.n_passes == 1 and "IN_COLB" not in dumps[0]
+    def far(c):                                                       # factor column much longer than one element: three passes, all instances
+        M = sg.sg_mat_create(c, sg.SG_F64, 4096, 4096, 4096, None)
+        det, mp = sg.sg_vec_create(c, sg.SG_F64, 1, None), sg.sg_vec_create(c, sg.SG_F64, 1, None)
+        sg.sg_mat_ge_steps(c, M, det, mp, 6, 7)
+    st, dumps = plan(far)
+    assert st.n_passes == 3 and st.n_template == 3
+
+
 def test_force_bytecode_and_unknown_chains_use_the_bytecode_kernel():
     st, _ = plan(lambda c: W.cfg1(c, 1 << 20, None, None), sg.SG_FLAG_FORCE_BYTECODE)
     assert st.n_bytecode == 1 and st.n_template == 0
