@@ -229,7 +229,7 @@ def ge_section(torch, sg, W, inputs, out, peak):
     steps), device time between two events around the loop.  Algorithmic bytes: step k reads and writes the (n-k-1) x n rows
     below the pivot row (16 B per updated element), plus the pivot row and the factor column."""
     stream = torch.cuda.current_stream().cuda_stream
-    for n in (4096,):
+    for n in (4096, 8192):
         M0 = torch.from_numpy(inputs.boosted_matrix_f64(5, 0, n) / float(n)).cuda()
         M = M0.clone()
         alg = sum(16 * (n - k - 1) * n + 8 * n + 24 * (n - k - 1) + 40 for k in range(n))

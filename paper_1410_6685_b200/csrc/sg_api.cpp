@@ -19,6 +19,7 @@ static Value* val(sg_ctx* c, sg_handle h) {
 }
 static sg_handle new_value(sg_ctx* c, const Value& v) {
     c->values.push_back(v);
+    c->live.push_back((int)c->values.size() - 1);
     return (sg_handle)c->values.size();
 }
 
@@ -619,7 +620,7 @@ sg_status sg_plan_stats(sg_ctx* c, sg_stats* out) { CK(c && out); *out = c->stat
 
 int64_t sg_plan_dump(sg_ctx* c, int32_t pass, char* buf, int64_t cap) {
     if (!c || pass < 0 || (size_t)pass >= c->dumps.size()) return -1;
-    const std::string& s = c->dumps[pass];
+    const std::string s = sg_dump_prog(c->dumps[pass]);
     if (buf && cap > 0) { int64_t n = (int64_t)s.size() < cap - 1 ? (int64_t)s.size() : cap - 1; memcpy(buf, s.data(), n); buf[n] = 0; }
     return (int64_t)s.size() + 1;
 }

@@ -122,6 +122,8 @@ std::string dump_prog(const SgProg& g) {
 
 }  // namespace
 
+std::string sg_dump_prog(const SgProg& g) { return dump_prog(g); }
+
 sg_status sg_build_pass(sg_ctx* c, Pass& P, std::vector<char*>& temps, std::string& dump) {
     std::vector<Node>& N = c->nodes;
     std::vector<Value>& V = c->values;
@@ -345,6 +347,6 @@ sg_status sg_build_pass(sg_ctx* c, Pass& P, std::vector<char*>& temps, std::stri
     g.shape.n_vreg = (uint8_t)B.n_vreg;
     g.shape.n_preg = (uint8_t)B.n_preg;
     if (only_quant && n_out > 0 && !P.is2d) g.shape.flags |= PF_EARLY_EXIT;
-    dump = dump_prog(g);
+    (void)dump;      // the text form is produced on demand (sg_dump_prog): it costs more than the plan itself
     return SG_OK;
 }

@@ -94,6 +94,7 @@ struct sg_ctx {
     std::string err;
 
     std::vector<Value> values;      // handle h <-> values[h-1]
+    std::vector<int> live;          // indices of values that may still be alive (compacted at every flush: a flush costs O(live), not O(history))
     std::vector<Node> nodes;        // pending actions, in call order
     std::vector<Contract> contracts;
 
@@ -117,12 +118,13 @@ struct sg_ctx {
     // last flush
     std::vector<Launch> last;
     sg_stats stats{};
-    std::vector<std::string> dumps;
+    std::vector<SgProg> dumps;      // canonical programs of the last flush; sg_plan_dump renders them as text on demand
     std::vector<char*> deferred_free;
 };
 
 // sg_plan.cpp
 sg_status sg_flush_impl(sg_ctx* c);
+std::string sg_dump_prog(const SgProg& g);   // sg_build.cpp
 // helpers shared by sg_api.cpp / sg_plan.cpp
 inline int dtype_size(int dt) { return dt == SG_BOOL ? 1 : (dt == SG_F32 || dt == SG_I32) ? 4 : 8; }
 sg_status sg_fail(sg_ctx* c, sg_status code, const std::string& msg);

@@ -96,7 +96,7 @@ sg_status sg_flush_impl(sg_ctx* c) {
 
     // ---- 3. pass assignment ------------------------------------------------------------------------------
     std::vector<Pass> passes;
-    std::vector<char> spill(V.size(), 0);       // value must be stored because a later pass consumes it
+    std::vector<char> spill(V.size(), 0);       // value must be stored because a later pass consumes it (1 byte per handle ever made)
     for (size_t i = 0; i < N.size(); ++i) {
         Node& X = N[i];
         if (X.done || !X.needed) continue;
@@ -207,7 +207,7 @@ sg_status sg_flush_impl(sg_ctx* c) {
         std::string dump;
         sg_status s = sg_build_pass(c, P, temps, dump);
         if (s != SG_OK) return s;
-        c->dumps.push_back(dump);
+        c->dumps.push_back(P.prog);
         char err[256] = {0};
         int rc = sgk_plan(P.prog, P.args, (c->flags & SG_FLAG_FORCE_BYTECODE) ? 1 : 0, c->sm_count, c->plan_only ? 0 : 1, &P.geom, err, sizeof(err));
         if (rc != 0) return sg_fail(c, (sg_status)rc, err);
@@ -302,17 +302,22 @@ sg_status sg_flush_impl(sg_ctx* c) {
             if (v.node >= 0 && &N[v.node] == &n) v.node = -1;
         }
     }
-    for (Value& v : V) if (v.node >= 0 && N[v.node].done) v.node = -1;
+    for (int i : c->live) { Value& v = V[i]; if (v.node >= 0 && N[v.node].done) v.node = -1; }
     N.clear();
-    for (Value& v : V) {            // unreferenced results die with the flush
-        if (!v.alive || v.user_refs > 0) continue;
-        if (v.owned && v.ptr) { c->deferred_free.push_back(v.ptr); v.ptr = nullptr; v.owned = false; }
-        if (v.kind == VK_SCALAR && v.slot >= 0) {
-            bool contract = false;
-            for (const Contract& k : c->contracts) contract |= (&V[k.value] == &v);
-            if (!contract) { c->slab_free.push_back(v.slot); v.slot = -1; v.alive = false; }
-        } else v.alive = false;
+    size_t keep = 0;
+    for (int i : c->live) {         // unreferenced results die with the flush
+        Value& v = V[i];
+        if (v.alive && v.user_refs <= 0) {
+            if (v.owned && v.ptr) { c->deferred_free.push_back(v.ptr); v.ptr = nullptr; v.owned = false; }
+            if (v.kind == VK_SCALAR && v.slot >= 0) {
+                bool contract = false;
+                for (const Contract& k : c->contracts) contract |= (&V[k.value] == &v);
+                if (!contract) { c->slab_free.push_back(v.slot); v.slot = -1; v.alive = false; }
+            } else v.alive = false;
+        }
+        if (v.alive) c->live[keep++] = i;
     }
+    c->live.resize(keep);
 
     // ---- 7. contracts: evaluated on the device with the data; read with the scalars ----
     sg_status result = SG_OK;
