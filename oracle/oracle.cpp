@@ -20,6 +20,7 @@
 // dtype codes: 0 = f32, 1 = f64, 2 = i32, 3 = i64.   Booleans are 1 byte, 0/1.
 // All functions return 0 on success, a negative code on a bad argument.
 
+#include <cmath>
 #include <cstdint>
 #include <cstring>
 #include <limits>
@@ -28,7 +29,7 @@ namespace {
 
 enum { F32 = 0, F64 = 1, I32 = 2, I64 = 3 };
 enum { ADD = 0, SUB = 1, MUL = 2, DIV = 3, MIN = 4, MAX = 5, MOD = 6 };      // binary arithmetic
-enum { NEG = 0, ABS = 1 };                                                    // unary
+enum { NEG = 0, ABS = 1, SQRT = 2 };                                          // unary
 enum { EQ = 0, NE = 1, LT = 2, LE = 3, GT = 4, GE = 5 };                      // comparisons
 enum { AND = 0, OR = 1, NOT = 2 };                                            // logical
 
@@ -101,12 +102,16 @@ template <class T> int scalar_t(int op, int64_t n, const T* a, T s, int reversed
 }
 
 // unary NEG / ABS: sign-bit operations for floats (abs(-0) = +0), wrap for ints.
+// SQRT (the agent of Listing `project`: `a.project(agent sqrt)`): the IEEE-754 correctly rounded
+// square root in the collection's own dtype (sqrt(-0) = -0, sqrt(x<0) = NaN); floats only (R20).
 inline float un(int op, float a) {
+    if (op == SQRT) return std::sqrt(a);
     uint32_t u; std::memcpy(&u, &a, 4);
     u = (op == NEG) ? (u ^ 0x80000000u) : (u & 0x7fffffffu);
     std::memcpy(&a, &u, 4); return a;
 }
 inline double un(int op, double a) {
+    if (op == SQRT) return std::sqrt(a);
     uint64_t u; std::memcpy(&u, &a, 8);
     u = (op == NEG) ? (u ^ 0x8000000000000000ull) : (u & 0x7fffffffffffffffull);
     std::memcpy(&a, &u, 8); return a;
@@ -122,7 +127,8 @@ inline int64_t un(int op, int64_t a) {
     return (int64_t)u;
 }
 template <class T> int unary_t(int op, int64_t n, const T* a, T* out) {
-    if (op != NEG && op != ABS) return -2;
+    if (op == SQRT && std::numeric_limits<T>::is_integer) return -3;
+    if (op != NEG && op != ABS && op != SQRT) return -2;
     for (int64_t i = 0; i < n; ++i) out[i] = un(op, a[i]);
     return 0;
 }
