@@ -20,7 +20,7 @@ from . import build as _build
 
 _DT = {np.dtype(np.float32): 0, np.dtype(np.float64): 1, np.dtype(np.int32): 2, np.dtype(np.int64): 3}
 _BIN = {"add": 0, "sub": 1, "mul": 2, "div": 3, "min": 4, "max": 5, "mod": 6}
-_UN = {"neg": 0, "abs": 1}
+_UN = {"neg": 0, "abs": 1, "sqrt": 2}
 _CMP = {"eq": 0, "ne": 1, "lt": 2, "le": 3, "gt": 4, "ge": 5}
 _LOG = {"and": 0, "or": 1, "not": 2}
 
@@ -75,7 +75,10 @@ def scalar(op: str, a, s, reversed: bool = False) -> np.ndarray:
 
 
 def unary(op: str, a) -> np.ndarray:
+    """neg / abs (sign-bit operations) and sqrt (correctly rounded, floats only: the `project(agent sqrt)` of PAPER.md:171-175)."""
     a = _c(a)
+    if op == "sqrt" and a.dtype.kind != "f":
+        raise TypeError("sqrt needs a float collection")
     out = np.empty_like(a)
     _chk(lib().orc_unary(_UN[op], _DT[a.dtype], _n(a), _p(a), _p(out)), "unary")
     return out
@@ -123,6 +126,17 @@ def sum(a):
         out = np.zeros(1, dtype=np.int64)
     _chk(lib().orc_sum(_DT[a.dtype], _n(a), _p(a), _p(out)), "sum")
     return out[0].item()
+
+
+def avg(a) -> float:
+    """avg = sum(a) / count, one fp64 division of the once-rounded fp64 sum (int collections: the wrapping int64
+    sum converted to fp64 first).  Empty collection: ValueError (R4)."""
+    a = _c(a)
+    if a.size == 0:
+        raise ValueError("avg: empty collection")
+    num = np.array([sum(a)], dtype=np.float64)
+    den = np.array([a.size], dtype=np.float64)
+    return zip("div", num, den)[0].item()
 
 
 def _extremum(is_max: int, a):

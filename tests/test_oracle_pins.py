@@ -571,3 +571,87 @@ def test_ge_determinant_steps_are_matstep_and_library_det():
     assert sign == np.sign(det) and abs(math.log(abs(det)) - logabs) <= 1e-12
     s = 0.5                                                                # det(s*M) = s^n det(M): exact for a power of two
     assert orc.ge_determinant(s * M)[0] == det * s ** n
+
+
+# ----------------------------------------------------------------------------------------------------------
+# rest of the vector API — sqrt projection, avg,
+# compwise_divide with its built-in non-zero contract (Listing 2), approximate equality
+#
+# ----------------------------------------------------------------------------------------------------------
+def _is_correctly_rounded_sqrt(x: float, r: float, dtype) -> bool:
+    """r == RN(sqrt(x)) decided in exact integer/rational arithmetic: the two neighbours' midpoints bracket sqrt(x),
+    i.e. ((r_prev + r)/2)^2 <= x <= ((r + r_next)/2)^2 (a tie cannot occur for sqrt of a binary float)."""
+    lo = np.nextafter(dtype(r), dtype(-np.inf))
+    hi = np.nextafter(dtype(r), dtype(np.inf))
+    X, R, LO, HI = Fraction(float(x)), Fraction(float(r)), Fraction(float(lo)), Fraction(float(hi))
+    return ((LO + R) / 2) ** 2 < X < ((R + HI) / 2) ** 2 or R * R == X
+
+
+@pytest.mark.parametrize("dtype", [np.float32, np.float64])
+def test_sqrt_is_correctly_rounded(dtype):
+    a = np.concatenate([RNG.uniform(0, 4, 300), RNG.uniform(0, 1e-30, 50), RNG.uniform(1e30, 1e38, 50),
+                        [2.0, 3.0, 0.5, 1e-40 if dtype is np.float32 else 5e-324]]).astype(dtype)
+    r = orc.unary("sqrt", a)
+    assert r.dtype == a.dtype
+    for x, y in zip(a, r):
+        assert _is_correctly_rounded_sqrt(x, y, dtype), (x, y)
+
+
+@pytest.mark.parametrize("dtype", [np.float32, np.float64])
+def test_sqrt_perfect_squares_and_special_values(dtype):
+    k = np.arange(0, 4096, dtype=np.int64)
+    assert np.array_equal(orc.unary("sqrt", (k * k).astype(dtype)), k.astype(dtype))          # exact (k^2 < 2^24)
+    p = np.array([4.0 ** e for e in range(-20, 21)], dtype=dtype)
+    assert np.array_equal(orc.unary("sqrt", p), np.array([2.0 ** e for e in range(-20, 21)], dtype=dtype))
+    s = orc.unary("sqrt", np.array([0.0, -0.0, np.inf, -1.0, np.nan], dtype=dtype))
+    assert s[0] == 0 and not np.signbit(s[0]) and s[1] == 0 and np.signbit(s[1]) and s[2] == np.inf
+    assert np.isnan(s[3]) and np.isnan(s[4])
+    with pytest.raises(TypeError):
+        orc.unary("sqrt", np.arange(4, dtype=np.int32))
+
+
+def test_sqrt_matches_library_routine():
+    for dtype in (np.float32, np.float64):
+        a = np.abs(RNG.standard_normal(5000)).astype(dtype)
+        assert np.array_equal(orc.unary("sqrt", a), np.sqrt(a))
+    assert orc.unary("sqrt", np.array([2.0]))[0] == math.sqrt(2.0)
+
+
+def test_avg_closed_forms():
+    for n in (1, 2, 1000, 4097):
+        assert orc.avg(np.arange(n, dtype=np.float64)) == (n - 1) / 2                        # n(n-1)/2 / n, exact
+        assert orc.avg(np.arange(n, dtype=np.int32)) == (n - 1) / 2
+    assert orc.avg(np.full(777, 0.375, dtype=np.float32)) == 0.375
+    a = RNG.uniform(-1, 1, 3001)
+    exact_avg = sum(Fraction(float(v)) for v in a) / len(a)
+    assert abs(Fraction(orc.avg(a)) - exact_avg) <= abs(exact_avg) * Fraction(1, 2 ** 50)
+    with pytest.raises(ValueError):
+        orc.avg(np.zeros(0))
+
+
+def test_compwise_divide_contract_listing2():
+    """Listing 2: require not other.exists(is_zero); ensure Result * other = Current (read as the
+    approximate equality of PAPER.md:339, since a/b*b rounds twice)."""
+    a = RNG.uniform(-4, 4, 2000)
+    b = RNG.uniform(0.5, 2, 2000)
+    pre_violated = orc.any(orc.cmp_scalar("eq", b, 0.0))
+    assert pre_violated is False
+    q = orc.zip("div", a, b)
+    for x, y, z in zip(a[:200], b[:200], q[:200]):
+        assert z == round_f64(Fraction(float(x)) / Fraction(float(y)))
+    back = orc.zip("mul", q, b)
+    approx = orc.cmp_scalar("le", orc.unary("abs", orc.zip("sub", back, a)), 1e-12)
+    assert orc.all(approx) is True
+    assert orc.all(orc.cmp("eq", back, a)) == bool(np.all(q * b == a))                       # exact EQ is a different predicate
+    b2 = b.copy(); b2[1234] = 0.0
+    assert orc.any(orc.cmp_scalar("eq", b2, 0.0)) is True
+    b3 = b.copy(); b3[7] = -0.0
+    assert orc.any(orc.cmp_scalar("eq", b3, 0.0)) is True                                    # -0 == +0
+
+
+def test_vector_norm_pythagorean():
+    """sqrt(sum(x*x)) on integer vectors whose norm is an integer: (3,4)->5, (1,2,2)->3, (2,3,6)->7, k copies of (3,4)*..."""
+    for v, nrm in (([3, 4], 5), ([1, 2, 2], 3), ([2, 3, 6], 7), ([1, 4, 8], 9), ([3, 4] * 4, 10)):
+        x = np.array(v, dtype=np.float64)
+        s = np.array([orc.sum(orc.zip("mul", x, x))])
+        assert orc.unary("sqrt", s)[0] == nrm
