@@ -178,6 +178,8 @@ def per_config(torch, sg, W, inputs, peak, which):
         cfg4_section(torch, sg, W, inputs, measure)
     if "ge" in which:
         ge_section(torch, sg, W, inputs, out, peak)
+    if "vecapi" in which:
+        vecapi_section(torch, sg, W, inputs, measure)
     return out
 
 
@@ -256,6 +258,24 @@ def ge_section(torch, sg, W, inputs, out, peak):
             "passes": 3 * n - 2, "template_passes": 3 * n - 2, "det": det, "launches_per_step": 3}
 
 
+def vecapi_section(torch, sg, W, inputs, measure):
+    """the rest of the vector API at 2^26 fp32 / 2^25 fp64 elements (inputs larger than L2)."""
+    for tag, dt, n, gen in (("fp32_2^26", sg.SG_F32, 1 << 26, lambda s, m: inputs.normal_f32(2, s, m)),
+                            ("fp64_2^25", sg.SG_F64, 1 << 25, lambda s, m: inputs.uniform_pm1_f64(1, s, m))):
+        es = 4 if dt == sg.SG_F32 else 8
+        pos = lambda x: (np.abs(x) + x.dtype.type(0.5)).astype(x.dtype)      # positive operands: sqrt domain, non-zero divisors
+        a = torch.from_numpy(pos(gen(0, n))).cuda()
+        b = torch.from_numpy(pos(gen(1, n))).cuda()
+        o = torch.empty_like(a)
+        measure(f"vecapi_project_sqrt_{tag}", lambda ctx: W.project_sqrt(ctx, dt, n, a.data_ptr(), o.data_ptr()), 2 * es * n)
+        measure(f"vecapi_avg_{tag} (sum pass + 1-element divide pass)", lambda ctx: W.avg(ctx, dt, n, a.data_ptr()), es * n)
+        measure(f"vecapi_norm2_{tag} (sum-of-squares pass + 1-element sqrt pass)", lambda ctx: W.norm2(ctx, dt, n, a.data_ptr()), es * n)
+        measure(f"vecapi_compwise_divide_with_pre_and_post_contracts_{tag} (2 passes: 2R+1W, 3R)",
+                lambda ctx: W.compwise_divide(ctx, dt, n, a.data_ptr(), b.data_ptr(), o.data_ptr(), eps=1e-3), 6 * es * n)
+        measure(f"vecapi_approx_equal_{tag}", lambda ctx: W.approx_equal(ctx, dt, n, a.data_ptr(), b.data_ptr(), 1e-3), 2 * es * n)
+        del a, b, o
+
+
 def cfg4_section(torch, sg, W, inputs, measure):
     n4 = 16384
     Mh = inputs.boosted_matrix_f64(5, 0, n4)
@@ -276,7 +296,7 @@ def main():
     ap.add_argument("--log2n", type=int, default=28)
     ap.add_argument("--impl", default="ours")
     ap.add_argument("--headline-only", action="store_true", help="same as --configs none")
-    ap.add_argument("--configs", default="cfg0,cfg1,cfg2,cfg3,cfg4,ge", help="per_config sections to time after the headline (or: none)")
+    ap.add_argument("--configs", default="cfg0,cfg1,cfg2,cfg3,cfg4,ge,vecapi", help="per_config sections to time after the headline (or: none)")
     ap.add_argument("--skip-headline", action="store_true", help="profiling aid: run only the --configs sections and print their JSON")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3)

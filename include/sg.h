@@ -58,12 +58,16 @@ typedef enum { SG_F32 = 0, SG_F64 = 1, SG_I32 = 2, SG_I64 = 3, SG_BOOL = 4 /* 1 
 
 /* Elementwise operations (PAPER.md:205 plus/minus/multiplied_by/divided_by + component-wise variants;
  * predicates of filter/for_all/exists agents PAPER.md:177-191).  Binary ops take two operands, each a
- * collection handle, an immediate or a device scalar; at least one must be a collection. */
+ * collection handle, an immediate or a device scalar; at least one must be a handle.  When no operand is a vector or
+ * matrix (device scalars and immediates only) the result is a ONE-element vector: this is how avg = sum / count
+ * stays on the device. */
 typedef enum {
     SG_ADD = 0, SG_SUB = 1, SG_MUL = 2, SG_DIV = 3, SG_MIN = 4, SG_MAX = 5, SG_MOD = 6,   /* T,T -> T   */
     SG_NEG = 7, SG_ABS = 8,                                                              /* T   -> T   */
     SG_EQ = 9, SG_NE = 10, SG_LT = 11, SG_LE = 12, SG_GT = 13, SG_GE = 14,               /* T,T -> BOOL */
-    SG_AND = 15, SG_OR = 16, SG_NOT = 17                                                 /* BOOL -> BOOL */
+    SG_AND = 15, SG_OR = 16, SG_NOT = 17,                                                /* BOOL -> BOOL */
+    SG_SQRT = 19    /* F32/F64 -> same dtype: correctly rounded IEEE square root, the `project (agent sqrt)` of PAPER.md:171-175
+                       (sqrt(-0) = -0, sqrt(x < 0) = NaN); SG_ERR_DTYPE on integer or BOOL collections.  18 is reserved. */
 } sg_op;
 
 typedef enum { SG_SUM = 0, SG_RMAX = 1, SG_RMIN = 2, SG_COUNT = 3 /* number of true in a BOOL collection */ } sg_red;

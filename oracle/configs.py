@@ -93,3 +93,46 @@ def cfg4(M, k: int) -> dict:
     """Same step through the single plain-definition loop (orc_mat_step)."""
     Mo, rowmax, colsum = orc.mat_step(M, k)
     return {"M": Mo, "rowmax": rowmax, "colsum": colsum}
+
+
+def concatenate(a, b) -> np.ndarray:
+    """concatenate: a new container of the elements of a followed by those of b."""
+    a, b = np.ascontiguousarray(a), np.ascontiguousarray(b)
+    assert a.dtype == b.dtype
+    out = np.empty(a.size + b.size, dtype=a.dtype)
+    out[: a.size] = a
+    out[a.size:] = b
+    return out
+
+
+def quicksort(a) -> np.ndarray:
+    """Listing 3 (PAPER.md:245-268), step by step: pivot := a[a.count // 2] (0-based, DESIGN.md R10); left/right/mid := the three
+    stable filters with item < / > / = pivot; Result := quicksort(left).concatenate(mid).concatenate(quicksort(right)).
+    Precondition a.count > 0.  The recursion of the listing is written with an explicit stack (same calls, same order of
+    results); an empty left or right part is skipped, as its quicksort would violate the precondition."""
+    a = np.ascontiguousarray(a)
+    if a.size == 0:
+        raise ValueError("quicksort: require a.count > 0")
+    pieces = []                     # sorted runs in final order
+    stack = [a]                     # sub-collections still to sort, leftmost on top
+    while stack:
+        v = stack.pop()
+        if isinstance(v, tuple):    # an already final run (a `mid`)
+            pieces.append(v[0])
+            continue
+        if v.size == 1:
+            pieces.append(v)
+            continue
+        pivot = v[v.size // 2]
+        left = orc.filter(v, orc.cmp_scalar("lt", v, pivot))
+        right = orc.filter(v, orc.cmp_scalar("gt", v, pivot))
+        mid = orc.filter(v, orc.cmp_scalar("eq", v, pivot))
+        if right.size:
+            stack.append(right)
+        stack.append((mid,))
+        if left.size:
+            stack.append(left)
+    out = pieces[0]
+    for p in pieces[1:]:
+        out = concatenate(out, p)
+    return out

@@ -288,10 +288,10 @@ static sg_status append_map(sg_ctx* c, uint8_t op, int n_opd, const Operand* opd
 
 sg_status sg_enqueue(sg_ctx* c, sg_op op, const sg_operand* ops, int32_t n, sg_handle dst, sg_handle* out) {
     CK(c && ops && out);
-    if (op < SG_ADD || op > SG_NOT) return sg_fail(c, SG_ERR_ARG, "unknown op");
-    const bool unary = (op == SG_NEG || op == SG_ABS || op == SG_NOT);
+    if (op < SG_ADD || (op > SG_NOT && op != SG_SQRT)) return sg_fail(c, SG_ERR_ARG, "unknown op");
+    const bool unary = (op == SG_NEG || op == SG_ABS || op == SG_NOT || op == SG_SQRT);
     if (n != (unary ? 1 : 2)) return sg_fail(c, SG_ERR_ARG, "wrong operand count");
-    const bool logic = (op >= SG_AND);
+    const bool logic = (op >= SG_AND && op <= SG_NOT);
     Value* vv[2] = {nullptr, nullptr};
     int dtype = -1;
     for (int i = 0; i < n; ++i) {
@@ -305,6 +305,7 @@ sg_status sg_enqueue(sg_ctx* c, sg_op op, const sg_operand* ops, int32_t n, sg_h
     if (dtype < 0) return sg_fail(c, SG_ERR_ARG, "at least one operand must be a collection");
     if (logic != (dtype == SG_BOOL)) return sg_fail(c, SG_ERR_DTYPE, logic ? "logical ops need BOOL operands" : "arithmetic on BOOL");
     if (op == SG_MOD && (dtype == SG_F32 || dtype == SG_F64)) return sg_fail(c, SG_ERR_DTYPE, "MOD needs an integer dtype");
+    if (op == SG_SQRT && dtype != SG_F32 && dtype != SG_F64) return sg_fail(c, SG_ERR_DTYPE, "SQRT needs a float dtype");
     // iteration domain: a matrix operand fixes a 2-D domain; vectors may broadcast along it
     bool is2d = false; int64_t rows = 1, cols = -1; bool have_coll = false;
     for (int i = 0; i < n; ++i)
@@ -339,7 +340,14 @@ sg_status sg_enqueue(sg_ctx* c, sg_op op, const sg_operand* ops, int32_t n, sg_h
             else if (cols != vv[i]->cols) return sg_fail(c, SG_ERR_SHAPE, "vector counts differ");
         }
     }
-    if (!have_coll) return sg_fail(c, SG_ERR_ARG, "at least one operand must be a vector or matrix");
+    if (!have_coll) {
+        // only device scalars (and immediates): a one-element domain, e.g. avg = sum / count computed on the
+        // device from the deferred sum without a host round trip
+        bool have_scalar = false;
+        for (int i = 0; i < n; ++i) have_scalar |= (vv[i] && vv[i]->kind == VK_SCALAR);
+        if (!have_scalar || is2d) return sg_fail(c, SG_ERR_ARG, "at least one operand must be a vector, matrix or device scalar");
+        cols = 1;
+    }
     if (unary) { opd[1] = opd[0]; }
     return append_map(c, (uint8_t)op, unary ? 1 : 2, opd, dtype, is2d, rows, cols, dst, out);
 }

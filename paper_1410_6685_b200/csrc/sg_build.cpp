@@ -51,7 +51,7 @@ struct Builder {
 
 const char* op_name(uint8_t op) {
     static const char* n[] = {"OP_ADD", "OP_SUB", "OP_MUL", "OP_DIV", "OP_MIN", "OP_MAX", "OP_MOD", "OP_NEG", "OP_ABS", "OP_EQ", "OP_NE",
-                              "OP_LT", "OP_LE", "OP_GT", "OP_GE", "OP_AND", "OP_OR", "OP_NOT", "OP_MOV"};
+                              "OP_LT", "OP_LE", "OP_GT", "OP_GE", "OP_AND", "OP_OR", "OP_NOT", "OP_MOV", "OP_SQRT"};
     return op < OP_COUNT_ ? n[op] : "?";
 }
 const char* in_name(uint8_t k) {

@@ -76,6 +76,13 @@ __device__ __forceinline__ int32_t p_abs(int32_t a) { return a < 0 ? (int32_t)(0
 __device__ __forceinline__ long long p_neg(long long a) { return (long long)(0ull - (unsigned long long)a); }
 __device__ __forceinline__ long long p_abs(long long a) { return a < 0 ? (long long)(0ull - (unsigned long long)a) : a; }
 
+// correctly rounded IEEE square root in the pass dtype (sqrt.rn.f32 / sqrt.rn.f64: never the approximate MUFU path);
+// the integer overloads only keep value_op<T> instantiable — sg_enqueue rejects SQRT on integer collections
+__device__ __forceinline__ float p_sqrt(float a) { return __fsqrt_rn(a); }
+__device__ __forceinline__ double p_sqrt(double a) { return __dsqrt_rn(a); }
+__device__ __forceinline__ int32_t p_sqrt(int32_t a) { return a; }
+__device__ __forceinline__ long long p_sqrt(long long a) { return a; }
+
 // int32 division / modulo by a pass-constant divisor d (|d| >= 2) with a host-computed signed magic number
 // (the classic multiply-high scheme for truncating signed division): q = mulhi(x, M) (+x or -x when the sign of
 // M differs from that of d), arithmetic shift by s, plus one if negative.  Exact for every int32 x; the
@@ -103,6 +110,7 @@ template <class T> __device__ __forceinline__ T value_op(uint8_t op, T a, T b) {
         case OP_MOD: return p_mod(a, b);
         case OP_NEG: return p_neg(a);
         case OP_ABS: return p_abs(a);
+        case OP_SQRT: return p_sqrt(a);
         default: return a;      // OP_MOV
     }
 }
@@ -123,7 +131,8 @@ __device__ __forceinline__ bool logic_op(uint8_t op, bool a, bool b) {
         default: return !a;
     }
 }
-__host__ __device__ constexpr bool op_is_value(uint8_t op) { return op <= OP_ABS || op == OP_MOV; }
+__host__ __device__ constexpr bool op_is_value(uint8_t op) { return op <= OP_ABS || op == OP_MOV || op == OP_SQRT; }
+__host__ __device__ constexpr bool op_is_unary_value(uint8_t op) { return op == OP_NEG || op == OP_ABS || op == OP_MOV || op == OP_SQRT; }
 __host__ __device__ constexpr bool op_is_compare(uint8_t op) { return op >= OP_EQ && op <= OP_GE; }
 
 // ---------------------------------------------------------------------------------------------------------

@@ -74,7 +74,7 @@ __device__ __forceinline__ void vm_exec(const SgProg& g, VmRegs<T, E> (&rf)[C], 
             if (op_is_value(ins.op)) {
                 switch (ins.op) {
 #define VOP(OPC) case OPC: _Pragma("unroll") for (int c = 0; c < C; ++c) _Pragma("unroll") for (int e = 0; e < E; ++e) last[c][e] = value_op<T>(OPC, x[c][e], y[c][e]); break;
-                    VOP(OP_ADD) VOP(OP_SUB) VOP(OP_MUL) VOP(OP_DIV) VOP(OP_MIN) VOP(OP_MAX) VOP(OP_MOD) VOP(OP_NEG) VOP(OP_ABS)
+                    VOP(OP_ADD) VOP(OP_SUB) VOP(OP_MUL) VOP(OP_DIV) VOP(OP_MIN) VOP(OP_MAX) VOP(OP_MOD) VOP(OP_NEG) VOP(OP_ABS) VOP(OP_SQRT)
 #undef VOP
                     default: _Pragma("unroll") for (int c = 0; c < C; ++c) _Pragma("unroll") for (int e = 0; e < E; ++e) last[c][e] = x[c][e]; break;
                 }
@@ -216,7 +216,7 @@ template <int E, int C> __device__ __forceinline__ void vm_decode(const SgProg& 
     for (int i = 0; i < n; ++i) {
         const SgInstr ins = g.code[i];
         const bool reads_v = op_is_value(ins.op) || op_is_compare(ins.op);
-        const bool unary = ins.op == OP_NEG || ins.op == OP_ABS || ins.op == OP_MOV;
+        const bool unary = op_is_unary_value(ins.op);
         fwd[i] = 0;
         if (reads_v && last_dst >= 0) {
             if (ins.a == last_dst) fwd[i] = VM_FA;
@@ -238,7 +238,7 @@ template <int E, int C> __device__ __forceinline__ void vm_decode(const SgProg& 
             for (int j = i + 1; j < n && !store; ++j) {
                 const SgInstr nx = g.code[j];
                 if (op_is_value(nx.op) || op_is_compare(nx.op)) {
-                    const bool unary = nx.op == OP_NEG || nx.op == OP_ABS || nx.op == OP_MOV;
+                    const bool unary = op_is_unary_value(nx.op);
                     if (nx.a == ins.dst && fwd[j] != VM_FA) store = true;
                     if (!unary && nx.b == ins.dst && fwd[j] != VM_FB) store = true;
                 }
@@ -342,7 +342,7 @@ __device__ __forceinline__ void vm_exec_uops(uint32_t uops, int n_instr, uint32_
         SG_VM_CMP_BODY(OPC, x, last)                                                                             \
     } break;
             SG_VM_BIN(OP_ADD) SG_VM_BIN(OP_SUB) SG_VM_BIN(OP_MUL) SG_VM_BIN(OP_DIV) SG_VM_BIN(OP_MIN) SG_VM_BIN(OP_MAX) SG_VM_BIN(OP_MOD)
-            SG_VM_UN(OP_NEG) SG_VM_UN(OP_ABS) SG_VM_UN(OP_MOV)
+            SG_VM_UN(OP_NEG) SG_VM_UN(OP_ABS) SG_VM_UN(OP_MOV) SG_VM_UN(OP_SQRT)
             SG_VM_CMP(OP_EQ) SG_VM_CMP(OP_NE) SG_VM_CMP(OP_LT) SG_VM_CMP(OP_LE) SG_VM_CMP(OP_GT) SG_VM_CMP(OP_GE)
 #undef SG_VM_BIN
 #undef SG_VM_UN

@@ -22,6 +22,8 @@ enum : uint8_t {
     OP_AND = 15, OP_OR = 16, OP_NOT = 17,
     // V -> V copy (materialising an input into another buffer)
     OP_MOV = 18,
+    // V -> V, float dtypes only: correctly rounded square root (`project(agent sqrt)`)
+    OP_SQRT = 19,
     OP_COUNT_
 };
 

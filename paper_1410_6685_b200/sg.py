@@ -14,6 +14,7 @@ from ctypes import POINTER, Structure, byref, c_char_p, c_double, c_float, c_int
 SG_F32, SG_F64, SG_I32, SG_I64, SG_BOOL = 0, 1, 2, 3, 4
 (SG_ADD, SG_SUB, SG_MUL, SG_DIV, SG_MIN, SG_MAX, SG_MOD, SG_NEG, SG_ABS, SG_EQ, SG_NE, SG_LT, SG_LE, SG_GT, SG_GE, SG_AND, SG_OR,
  SG_NOT) = range(18)
+SG_SQRT = 19    # 18 is reserved (include/sg.h)
 SG_SUM, SG_RMAX, SG_RMIN, SG_COUNT = 0, 1, 2, 3
 SG_AXIS_ALL, SG_AXIS_ROWS, SG_AXIS_COLS = 0, 1, 2
 SG_OPERAND_HANDLE, SG_OPERAND_IMM_F64, SG_OPERAND_IMM_I64 = 0, 1, 2

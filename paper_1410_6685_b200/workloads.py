@@ -216,3 +216,81 @@ def ge_determinant(ctx, n, pM, pdet, pminpiv, ld=None, eps=0.0, native=True):
     for h in (gt, ok, value, det, minpiv, M):
         sg.sg_release(ctx, h)
     return (detv if okv else 0.0), okv
+
+
+# ------------------------------------------------------------------------------------------------------------------
+# the rest of the vector API
+# ------------------------------------------------------------------------------------------------------------------
+def project_sqrt(ctx, dtype, n, pa, pout=None):
+    """`a.project (agent sqrt)`: a new collection of the correctly rounded square roots."""
+    a = sg.sg_vec_create(ctx, dtype, n, pa)
+    dst = sg.sg_vec_create(ctx, dtype, n, pout) if pout is not None else 0
+    r = sg.sg_enqueue(ctx, sg.SG_SQRT, [a], dst_or_0=dst)
+    return {"a": a, "out": r}
+
+
+def norm2(ctx, dtype, n, pa):
+    """Euclidean norm sqrt(sum(a*a)): Listing 4's dot product followed by the sqrt agent applied to the
+    device-resident sum (a one-element result; fp64 like every float sum).  Two passes: the vector pass and a 1-element pass."""
+    a = sg.sg_vec_create(ctx, dtype, n, pa)
+    sq = sg.sg_enqueue(ctx, sg.SG_MUL, [a, a])
+    s = sg.sg_reduce(ctx, sq, sg.SG_SUM)
+    sg.sg_release(ctx, sq)
+    r = sg.sg_enqueue(ctx, sg.SG_SQRT, [s])
+    return {"a": a, "sum": s, "norm": r}
+
+
+def avg(ctx, dtype, n, pa):
+    """`avg` of a float collection = sum / count, divided on the device: the deferred fp64 sum is a device scalar
+    operand of a one-element pass, nothing is read back in between."""
+    a = sg.sg_vec_create(ctx, dtype, n, pa)
+    s = sg.sg_reduce(ctx, a, sg.SG_SUM)
+    r = sg.sg_enqueue(ctx, sg.SG_DIV, [s, F(float(n))])
+    return {"a": a, "sum": s, "avg": r}
+
+
+def compwise_divide(ctx, dtype, n, pa, pb, pout=None, eps=None):
+    """Listing 2: `require not other.exists (is_zero)`, `Result := a / b`, `ensure Result * other = Current`.
+
+    The precondition is a registered device-evaluated contract fused into the pass that divides (the body writes only a fresh
+    output, R17).  eps given: the postcondition is |Result*other - Current| <= eps (the approximate equality of
+    PAPER.md:339), registered as a POST contract, so it re-reads the STORED quotient in a second pass (R17).  eps=None: exact
+    equality as printed in the listing (false in general: a/b*b rounds twice) — evaluated as a plain quantifier, not
+    registered, in the same pass.  A violated registered contract makes the flush fail with SG_ERR_CONTRACT and its tag."""
+    a = sg.sg_vec_create(ctx, dtype, n, pa)
+    b = sg.sg_vec_create(ctx, dtype, n, pb)
+    z = sg.sg_enqueue(ctx, sg.SG_EQ, [b, F(0.0) if dtype in (sg.SG_F32, sg.SG_F64) else I(0)])
+    has_zero = sg.sg_exists(ctx, z)
+    nz = sg.sg_enqueue(ctx, sg.SG_NOT, [z])
+    pre = sg.sg_forall(ctx, nz)
+    sg.sg_contract(ctx, pre, sg.SG_CONTRACT_PRE, "not other.exists (is_zero)")
+    dst = sg.sg_vec_create(ctx, dtype, n, pout) if pout is not None else 0
+    q = sg.sg_enqueue(ctx, sg.SG_DIV, [a, b], dst_or_0=dst)
+    back = sg.sg_enqueue(ctx, sg.SG_MUL, [q, b])
+    if eps is None:
+        ok = sg.sg_enqueue(ctx, sg.SG_EQ, [back, a])
+        tmp = [back]
+    else:
+        d = sg.sg_enqueue(ctx, sg.SG_SUB, [back, a])
+        ad = sg.sg_enqueue(ctx, sg.SG_ABS, [d])
+        ok = sg.sg_enqueue(ctx, sg.SG_LE, [ad, F(eps)])
+        tmp = [back, d, ad]
+    post = sg.sg_forall(ctx, ok)
+    if eps is not None:
+        sg.sg_contract(ctx, post, sg.SG_CONTRACT_POST, "Result * other = Current (approx)")
+    for h in tmp + [z, nz, ok]:
+        sg.sg_release(ctx, h)
+    return {"a": a, "b": b, "out": q, "pre": pre, "has_zero": has_zero, "post": post}
+
+
+def approx_equal(ctx, dtype, n, pa, pb, eps):
+    """`double_approx_equals` lifted to collections: for_all(|a_i - b_i| <= eps), plus the largest deviation."""
+    a = sg.sg_vec_create(ctx, dtype, n, pa)
+    b = sg.sg_vec_create(ctx, dtype, n, pb)
+    d = sg.sg_enqueue(ctx, sg.SG_SUB, [a, b])
+    ad = sg.sg_enqueue(ctx, sg.SG_ABS, [d])
+    le = sg.sg_enqueue(ctx, sg.SG_LE, [ad, F(eps)])
+    res = {"a": a, "b": b, "all": sg.sg_forall(ctx, le), "maxdev": sg.sg_reduce(ctx, ad, sg.SG_RMAX)}
+    for h in (d, ad, le):
+        sg.sg_release(ctx, h)
+    return res

@@ -247,3 +247,50 @@ def test_released_intermediates_are_never_materialised():
     st_rel, d_rel = plan(lambda c: chain(c, True))
     assert d_kept[0].count("OUT_STORE") == 2 and d_rel[0].count("OUT_STORE") == 1
     assert st_kept.bytes_min - st_rel.bytes_min == 4 * 4096
+
+
+# ----------------------------------------------------------------------------------------------------------
+# plans of the rest of the vector API
+# ----------------------------------------------------------------------------------------------------------
+def test_vector_api_plans():
+    n = 1 << 16
+    st, dumps = plan(lambda c: W.project_sqrt(c, sg.SG_F32, n, None))
+    assert st.n_passes == 1 and "OP_SQRT" in dumps[0]
+    # avg: the vector pass produces the sum, a one-element pass divides it on the device (scalar consumed elementwise)
+    st, dumps = plan(lambda c: W.avg(c, sg.SG_F64, n, None))
+    assert st.n_passes == 2 and "OUT_SUM" in dumps[0] and "OP_DIV" in dumps[1] and "IN_SCALAR" in dumps[1]
+    st, dumps = plan(lambda c: W.norm2(c, sg.SG_F32, n, None))
+    assert st.n_passes == 2 and "OP_MUL" in dumps[0] and "OP_SQRT" in dumps[1]
+    # Listing 2: the precondition is fused into the dividing pass (fresh output); the registered postcondition re-reads the
+    # stored quotient in a second pass (R17); unregistered (exact EQ) it shares the pass
+    st, dumps = plan(lambda c: W.compwise_divide(c, sg.SG_F64, n, None, None, eps=1e-12))
+    assert st.n_passes == 2 and st.pass_n_in[0] == 2 and st.pass_n_in[1] == 3 and st.bytes_min == 6 * 8 * n
+    assert all(k in dumps[0] for k in ("OP_DIV", "OUT_ANY", "OUT_ALL", "OUT_STORE")) and "OP_ABS" not in dumps[0]
+    assert all(k in dumps[1] for k in ("OP_MUL", "OP_ABS", "OP_LE", "OUT_ALL")) and "OP_DIV" not in dumps[1]
+    st, dumps = plan(lambda c: W.compwise_divide(c, sg.SG_F64, n, None, None))
+    assert st.n_passes == 1 and st.bytes_min == 3 * 8 * n and dumps[0].count("OUT_ALL") == 2
+    st, dumps = plan(lambda c: W.approx_equal(c, sg.SG_F32, n, None, None, 1e-5))
+    assert st.n_passes == 1 and st.pass_n_in[0] == 2 and "OUT_MAX" in dumps[0] and "OUT_ALL" in dumps[0]
+
+
+def test_sqrt_and_scalar_only_operands_are_checked_at_enqueue():
+    ctx = sg.sg_ctx_create(-1)
+    try:
+        vi = sg.sg_vec_create(ctx, sg.SG_I32, 8, None)
+        vb = sg.sg_enqueue(ctx, sg.SG_GT, [vi, sg.I(0)])
+        for h in (vi, vb):
+            with pytest.raises(sg.SgError) as e:
+                sg.sg_enqueue(ctx, sg.SG_SQRT, [h])
+            assert e.value.status == sg.SG_ERR_DTYPE
+        with pytest.raises(sg.SgError) as e:
+            sg.sg_enqueue(ctx, 18, [vi])                       # reserved op code
+        assert e.value.status == sg.SG_ERR_ARG
+        with pytest.raises(sg.SgError) as e:
+            sg.sg_enqueue(ctx, sg.SG_ADD, [sg.F(1.0), sg.F(2.0)])   # no handle at all
+        assert e.value.status == sg.SG_ERR_ARG
+        vf = sg.sg_vec_create(ctx, sg.SG_F64, 8, None)
+        s = sg.sg_reduce(ctx, vf, sg.SG_SUM)
+        r = sg.sg_enqueue(ctx, sg.SG_DIV, [s, sg.F(8.0)])
+        assert sg.sg_vec_count(ctx, r) == 1                    # device scalars only -> a one-element vector
+    finally:
+        sg.sg_ctx_destroy(ctx)

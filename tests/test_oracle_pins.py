@@ -655,3 +655,33 @@ def test_vector_norm_pythagorean():
         x = np.array(v, dtype=np.float64)
         s = np.array([orc.sum(orc.zip("mul", x, x))])
         assert orc.unary("sqrt", s)[0] == nrm
+
+
+# ----------------------------------------------------------------------------------------------------------
+# quicksort (Listing 3) and concatenate
+# ----------------------------------------------------------------------------------------------------------
+def test_concatenate_vs_list_semantics():
+    a, b = np.arange(5, dtype=np.float32), np.arange(7, 10, dtype=np.float32)
+    assert ocfg.concatenate(a, b).tolist() == a.tolist() + b.tolist()
+    assert ocfg.concatenate(a[:0], b).tolist() == b.tolist() and ocfg.concatenate(a, b[:0]).tolist() == a.tolist()
+
+
+@pytest.mark.parametrize("n", [1, 2, 3, 10, 257, 3000])
+def test_quicksort_matches_library_sort_and_listing3_postconditions(n):
+    for a in (RNG.standard_normal(n).astype(np.float32),
+              RNG.integers(-5, 6, n).astype(np.float32),                    # many duplicates
+              np.arange(n, dtype=np.float32), np.arange(n, dtype=np.float32)[::-1].copy(), np.zeros(n, dtype=np.float32)):
+        r = ocfg.quicksort(a)
+        assert r.dtype == a.dtype and r.size == a.size                       # ensure Result.count = a.count
+        assert orc.all(orc.adj("le", r))                                     # ensure Result.is_sorted
+        assert np.array_equal(r, np.sort(a, kind="stable"))
+        assert sorted(r.tolist()) == r.tolist() and sorted(a.tolist()) == r.tolist()
+
+
+def test_quicksort_equal_keys_keep_their_order_and_empty_is_rejected():
+    a = np.array([0.0, 3.0, -0.0, 1.0, 0.0, -0.0, 3.0], dtype=np.float32)     # -0 == +0: one `mid`, stable filter keeps the order
+    r = ocfg.quicksort(a)
+    assert r.tolist() == [0.0, 0.0, 0.0, 0.0, 1.0, 3.0, 3.0]
+    assert np.signbit(r[:4]).tolist() == [False, True, False, True]
+    with pytest.raises(ValueError):
+        ocfg.quicksort(np.zeros(0, dtype=np.float32))
