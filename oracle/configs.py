@@ -136,3 +136,22 @@ def quicksort(a) -> np.ndarray:
     for p in pieces[1:]:
         out = concatenate(out, p)
     return out
+
+
+def right_multiply(M, v) -> np.ndarray:
+    """`right_multiply` (matrix x column vector; Listing 1's `multiply` contract shape): result_i =
+    (row(i) compwise_multiply v).sum — Listing 4's dot product per row, with the built-in dimension contract columns = v.count."""
+    M, v = np.ascontiguousarray(M), np.ascontiguousarray(v)
+    assert M.ndim == 2 and M.shape[1] == v.size and M.dtype == v.dtype
+    return np.array([orc.sum(orc.zip("mul", M[i], v)) for i in range(M.shape[0])], dtype=np.float64)
+
+
+def left_multiply(v, M) -> np.ndarray:
+    """`left_multiply` (row vector x matrix): result_c = sum_i v_i * M[i,c] — every row scaled by its v_i (one
+    rounding per product), then the column sums; dimension contract rows = v.count."""
+    M, v = np.ascontiguousarray(M), np.ascontiguousarray(v)
+    assert M.ndim == 2 and M.shape[0] == v.size and M.dtype == v.dtype == np.float64
+    T = np.empty_like(M)
+    for i in range(M.shape[0]):
+        T[i] = orc.scalar("mul", M[i], v[i])
+    return orc.col_sum(T) if M.shape[0] else np.zeros(M.shape[1])

@@ -294,3 +294,66 @@ def approx_equal(ctx, dtype, n, pa, pb, eps):
     for h in (d, ad, le):
         sg.sg_release(ctx, h)
     return res
+
+
+# ------------------------------------------------------------------------------------------------------------------
+# quicksort (Listing 3)
+# ------------------------------------------------------------------------------------------------------------------
+_ES = {sg.SG_F32: 4, sg.SG_F64: 8, sg.SG_I32: 4, sg.SG_I64: 8}
+
+
+def quicksort(ctx, dtype, n, pa, pout, pscratch0, pscratch1, contracts=True):
+    """Listing 3 written over the C ABI.  pa: the input (left untouched); pout: the result; pscratch0/1: two device buffers of n
+    elements each (caller-owned, like every buffer here).
+
+    Each call of the listing's body becomes: the pivot a[a.count // 2] as a DEVICE scalar (it never visits the host: a
+    one-element max), the three predicate agents `item < / = / > pivot` closed over it, their counts in one fused
+    pass (the only values read back: they are the `count`s of left, mid and right, scalar contracts in the paper's sense,
+    PAPER.md:270), then the three stable filters.  `concatenate` costs nothing: since the counts are known,
+    each filter writes straight to its final place — left to [o, o+nl) and right to [o+nl+nm, o+n) of the scratch buffer of
+    the next depth, mid to [o+nl, o+nl+nm) of the result — so quicksort(left) ++ mid ++ quicksort(right) is already contiguous.
+    The recursion runs on an explicit stack (sub-ranges are disjoint, buffers alternate with the depth).
+    Postconditions (contracts=True): Result.is_sorted as a registered device contract, Result.count = a.count on the host.
+    Returns {"out": handle, "partitions": number of listing-body executions}."""
+    if n <= 0:
+        raise ValueError("quicksort: require a.count > 0")
+    es = _ES[dtype]
+    scratch = (pscratch0, pscratch1)
+    stack = [(pa, 0, 0, n, 0)]              # (buffer base, element offset in that buffer, offset o in the result, count, depth)
+    partitions = 0
+    placed = 0
+    while stack:
+        base, off, o, m, depth = stack.pop()
+        partitions += 1
+        a = sg.sg_vec_create(ctx, dtype, m, base + off * es)
+        mid1 = sg.sg_vec_subset(ctx, a, m // 2, m // 2 + 1)
+        pivot = sg.sg_reduce(ctx, mid1, sg.SG_RMAX)                   # the element itself, device-resident
+        lt = sg.sg_enqueue(ctx, sg.SG_LT, [a, H(pivot)])
+        eq = sg.sg_enqueue(ctx, sg.SG_EQ, [a, H(pivot)])
+        gt = sg.sg_enqueue(ctx, sg.SG_GT, [a, H(pivot)])
+        hl, hm = sg.sg_reduce(ctx, lt, sg.SG_COUNT), sg.sg_reduce(ctx, eq, sg.SG_COUNT)
+        nl, nm = sg.sg_scalar_get(ctx, hl), sg.sg_scalar_get(ctx, hm)  # trigger: one flush, two small passes
+        nr = m - nl - nm
+        nxt = scratch[depth % 2]
+        outs = []
+        if nl:
+            outs.append(sg.sg_filter(ctx, a, lt, nxt + o * es, nl))
+        outs.append(sg.sg_filter(ctx, a, eq, pout + (o + nl) * es, nm))
+        if nr:
+            outs.append(sg.sg_filter(ctx, a, gt, nxt + (o + nl + nm) * es, nr))
+        sg.sg_flush(ctx)                                               # asynchronous: nothing is read back
+        placed += nm
+        for h in [hl, hm, lt, eq, gt, pivot, mid1, a] + [x for pair in outs for x in pair]:
+            sg.sg_release(ctx, h)
+        if nr > 0:
+            stack.append((nxt, o + nl + nm, o + nl + nm, nr, depth + 1))
+        if nl > 0:
+            stack.append((nxt, o, o, nl, depth + 1))
+    out = sg.sg_vec_create(ctx, dtype, n, pout)
+    res = {"out": out, "partitions": partitions}
+    if contracts:
+        if placed != n:
+            raise AssertionError(f"quicksort postcondition Result.count = a.count violated: {placed} != {n}")
+        res["sorted"] = sg.sg_forall_adjacent(ctx, out, sg.SG_LE)
+        sg.sg_contract(ctx, res["sorted"], sg.SG_CONTRACT_POST, "Result.is_sorted")
+    return res

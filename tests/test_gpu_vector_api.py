@@ -147,3 +147,41 @@ def test_approx_equal(mode, dtype):
             got_all, got_max = bool(c.get(r["all"])), c.get(r["maxdev"])
         assert got_all == orc.all(orc.cmp_scalar("le", ad, eps))
         assert dtype(got_max) == orc.max(ad)
+
+
+# ----------------------------------------------------------------------------------------------------------
+# quicksort (Listing 3)
+# ----------------------------------------------------------------------------------------------------------
+from oracle import configs as ocfg  # noqa: E402
+
+
+def _quicksort_on_device(a, flags=0):
+    n = a.size
+    with Ctx(flags) as c:
+        ta = dev(a)
+        tout, s0, s1 = (empty_dev(n, a.dtype) for _ in range(3))
+        c.keep += [ta, tout, s0, s1]
+        before = ta.clone()
+        r = W.quicksort(c.ctx, sg.SG_F32 if a.dtype == np.float32 else sg.SG_F64, n, ta.data_ptr(), tout.data_ptr(), s0.data_ptr(), s1.data_ptr())
+        ok = c.get(r["sorted"])
+        got = c.read_vec(r["out"], a.dtype, n)
+        assert bits_equal(before.cpu().numpy(), ta.cpu().numpy())          # the argument is not modified
+    return got, ok, r["partitions"]
+
+
+@pytest.mark.parametrize("n", [1, 2, 3, 17, 1000, 4099, 20011])
+def test_quicksort_listing3(n):
+    for a in (RNG.standard_normal(n).astype(np.float32), RNG.integers(-50, 51, n).astype(np.float32)):
+        got, ok, parts = _quicksort_on_device(a)
+        want = ocfg.quicksort(a)
+        assert ok is True and bits_equal(got, want)                         # stable filters => the result is unique, bit for bit
+        assert parts <= n
+
+
+def test_quicksort_signed_zeros_sorted_input_fp64_and_bytecode():
+    a = np.array([0.0, 3.0, -0.0, 1.0, 0.0, -0.0, 3.0, -2.5], dtype=np.float32)
+    got, ok, _ = _quicksort_on_device(a)
+    assert ok and bits_equal(got, ocfg.quicksort(a))
+    for a in (np.arange(3000, dtype=np.float64), np.arange(3000, dtype=np.float64)[::-1].copy(), RNG.standard_normal(2500)):
+        got, ok, _ = _quicksort_on_device(a, sg.SG_FLAG_FORCE_BYTECODE)
+        assert ok and bits_equal(got, ocfg.quicksort(a))

@@ -685,3 +685,29 @@ def test_quicksort_equal_keys_keep_their_order_and_empty_is_rejected():
     assert np.signbit(r[:4]).tolist() == [False, True, False, True]
     with pytest.raises(ValueError):
         ocfg.quicksort(np.zeros(0, dtype=np.float32))
+
+
+# ----------------------------------------------------------------------------------------------------------
+# matrix-vector products
+# ----------------------------------------------------------------------------------------------------------
+def test_matvec_exact_integer_regime_identity_and_hand_values():
+    M = RNG.integers(-8, 9, (37, 53)).astype(np.float64)
+    v, w = RNG.integers(-8, 9, 53).astype(np.float64), RNG.integers(-8, 9, 37).astype(np.float64)
+    assert np.array_equal(ocfg.right_multiply(M, v), (M.astype(np.int64) @ v.astype(np.int64)).astype(np.float64))   # exact: any order agrees
+    assert np.array_equal(ocfg.left_multiply(w, M), (w.astype(np.int64) @ M.astype(np.int64)).astype(np.float64))
+    x = RNG.standard_normal(9)
+    assert np.array_equal(ocfg.right_multiply(np.eye(9), x), x) and np.array_equal(ocfg.left_multiply(x, np.eye(9)), x)
+    A = np.array([[1.0, 2.0, 3.0], [4.0, 5.0, 6.0]])
+    assert ocfg.right_multiply(A, np.array([1.0, 0.5, -1.0])).tolist() == [-1.0, 0.5]      # not symmetric: a transposed operand fails
+    assert ocfg.left_multiply(np.array([2.0, -1.0]), A).tolist() == [-2.0, -1.0, 0.0]
+
+
+def test_matvec_general_values_against_exact_rationals():
+    M, v, w = RNG.standard_normal((5, 7)), RNG.standard_normal(7), RNG.standard_normal(5)
+    r, l = ocfg.right_multiply(M, v), ocfg.left_multiply(w, M)
+    for i in range(5):      # each product rounds once, the sum of the ROUNDED products is then (nearly) exact
+        ex = sum(Fraction(float(M[i, c] * v[c])) for c in range(7))
+        assert abs(Fraction(float(r[i])) - ex) <= abs(ex) * Fraction(1, 2 ** 51)
+    for c in range(7):
+        ex = sum(Fraction(float(w[i] * M[i, c])) for i in range(5))
+        assert abs(Fraction(float(l[c])) - ex) <= abs(ex) * Fraction(1, 2 ** 51)
