@@ -180,6 +180,10 @@ def per_config(torch, sg, W, inputs, peak, which):
         ge_section(torch, sg, W, inputs, out, peak)
     if "vecapi" in which:
         vecapi_section(torch, sg, W, inputs, measure)
+    if "matvec" in which:
+        matvec_section(torch, sg, W, inputs, measure)
+    if "quicksort" in which:
+        quicksort_section(torch, sg, W, inputs, out)
     return out
 
 
@@ -276,6 +280,38 @@ def vecapi_section(torch, sg, W, inputs, measure):
         del a, b, o
 
 
+def matvec_section(torch, sg, W, inputs, measure):
+    """matrix x vector and vector x matrix at 16384^2 fp64 (2 GiB read once)."""
+    n = 16384
+    M = torch.from_numpy(inputs.boosted_matrix_f64(5, 0, n)).cuda()
+    v = torch.from_numpy(inputs.uniform_pm1_f64(5, 1, n)).cuda()
+    alg = 8 * n * n + 16 * n
+    measure("matvec_right_multiply_fp64_16384^2", lambda ctx: W.right_multiply(ctx, n, n, M.data_ptr(), v.data_ptr()), alg)
+    measure("matvec_left_multiply_fp64_16384^2", lambda ctx: W.left_multiply(ctx, n, n, v.data_ptr(), M.data_ptr()), alg)
+
+
+def quicksort_section(torch, sg, W, inputs, out):
+    """Listing 3 on fp32 normal(0,1) keys; wall time of the whole sort (one count read-back per partition).
+    Launch- and latency-bound by construction (the listing recurses down to single elements): reported, not a roofline line."""
+    stream = torch.cuda.current_stream().cuda_stream
+    for log2n in (12, 16):
+        n = 1 << log2n
+        a = torch.from_numpy(inputs.normal_f32(2, 0, n)).cuda()
+        o, s0, s1 = (torch.empty_like(a) for _ in range(3))
+        best, parts = None, 0
+        for rep in range(2):
+            ctx = sg.sg_ctx_create(0, stream)
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            r = W.quicksort(ctx, sg.SG_F32, n, a.data_ptr(), o.data_ptr(), s0.data_ptr(), s1.data_ptr())
+            ok = sg.sg_scalar_get(ctx, r["sorted"])
+            torch.cuda.synchronize()
+            ms = 1e3 * (time.perf_counter() - t0)
+            sg.sg_ctx_destroy(ctx)
+            best, parts = (ms if best is None else min(best, ms)), r["partitions"]
+        out[f"quicksort_listing3_fp32_2^{log2n} (wall, whole sort)"] = {"ms": best, "partitions": parts, "sorted": bool(ok), "elements/s": n / best * 1e3}
+
+
 def cfg4_section(torch, sg, W, inputs, measure):
     n4 = 16384
     Mh = inputs.boosted_matrix_f64(5, 0, n4)
@@ -296,7 +332,7 @@ def main():
     ap.add_argument("--log2n", type=int, default=28)
     ap.add_argument("--impl", default="ours")
     ap.add_argument("--headline-only", action="store_true", help="same as --configs none")
-    ap.add_argument("--configs", default="cfg0,cfg1,cfg2,cfg3,cfg4,ge,vecapi", help="per_config sections to time after the headline (or: none)")
+    ap.add_argument("--configs", default="cfg0,cfg1,cfg2,cfg3,cfg4,ge,vecapi,matvec,quicksort", help="per_config sections to time after the headline (or: none)")
     ap.add_argument("--skip-headline", action="store_true", help="profiling aid: run only the --configs sections and print their JSON")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3)

@@ -74,6 +74,47 @@ template <class P> struct Meta2D : Meta1D<P> {
     static constexpr bool HAS_ROWS = has_axis(AXIS_ROWS), HAS_COLS = has_axis(AXIS_COLS);
 };
 
+// Warp reduction of R per-row partials at once (R a power of two <= 32).  A butterfly per row costs 5 combines per lane and
+// row; here the first log2(R) exchange steps HALVE the number of rows a lane still holds (a lane sends the half it gives up
+// and combines the half it keeps), so R rows cost R-1 + (5 - log2 R) combines per lane instead of 5R — the double-double
+// combine (11 fp64 operations) is what bounds a row-sum pass otherwise.  Afterwards c[0] of the lanes whose low
+// (5 - log2 R) bits are zero holds the total of row `warp_row_of_lane<R>(lane)`.  Fixed combine order: deterministic.
+template <class T, int R>
+__device__ __forceinline__ void warp_reduce_rows(uint8_t kind, Cell (&c)[R], int lane) {
+    static_assert(R >= 1 && R <= 32 && (R & (R - 1)) == 0, "rows in flight must be a power of two <= 32");
+    int d = 16;
+#pragma unroll
+    for (int h = R / 2; h >= 1; h >>= 1) {
+        const bool upper = (lane & d) != 0;
+#pragma unroll
+        for (int i = 0; i < h; ++i) {
+            const Cell send = upper ? c[i] : c[i + h];
+            Cell keep = upper ? c[i + h] : c[i];
+            const Cell recv = cell_shfl_xor_kind<T>(kind, send, d);
+            cell_combine<T>(kind, keep, recv);
+            c[i] = keep;
+        }
+        d >>= 1;
+    }
+#pragma unroll
+    for (; d >= 1; d >>= 1) {
+        const Cell other = cell_shfl_xor_kind<T>(kind, c[0], d);
+        cell_combine<T>(kind, c[0], other);
+    }
+}
+template <int R> __device__ __forceinline__ int warp_row_of_lane(int lane) {
+    int row = 0, d = 16;
+#pragma unroll
+    for (int h = R / 2; h >= 1; h >>= 1) { if (lane & d) row += h; d >>= 1; }
+    return row;
+}
+template <int R> __device__ __forceinline__ bool warp_row_owner(int lane) {
+    int low = 31;
+#pragma unroll
+    for (int h = R / 2; h >= 1; h >>= 1) low >>= 1;
+    return (lane & low) == 0;
+}
+
 template <class P>
 __global__ void __launch_bounds__(BLOCK, P::min_blocks) pass2d_template(const __grid_constant__ SgArgs a) {
     typedef Meta2D<P> M;
@@ -168,6 +209,13 @@ __global__ void __launch_bounds__(BLOCK, P::min_blocks) pass2d_template(const __
         const int64_t r0 = r_begin + b * RS;
         const int64_t rb = r_begin + (b * RS) / RB * RB;                // start of the current RB-row batch of the per-row combine
         mbar_wait(&full[s], (uint32_t)((b / NS) & 1));
+        Cell rowc[M::NROWS][RS];                 // per-thread partials of the AXIS_ROWS outputs, one per row of the stage
+#pragma unroll
+        for (int o = 0; o < M::S.n_out; ++o)
+            if (out_is_reduction(g.out[o].kind) && g.out[o].axis == AXIS_ROWS) {
+#pragma unroll
+                for (int j = 0; j < RS; ++j) rowc[slots.row[o]][j] = cell_identity<T>(g.out[o].kind);
+            }
 #pragma unroll
         for (int j = 0; j < RS; ++j) {
             const int64_t r = r0 + j;
@@ -206,28 +254,28 @@ __global__ void __launch_bounds__(BLOCK, P::min_blocks) pass2d_template(const __
                         st_stream(reinterpret_cast<VEC*>(rowp + col[u]), x);
                     }
                 } else if (out_is_reduction(out.kind)) {
-                    Cell rowc = cell_identity<T>(out.kind);
 #pragma unroll
                     for (int u = 0; u < U; ++u) {
                         if (!cvalid[u]) continue;
 #pragma unroll
                         for (int e = 0; e < V; ++e) {
                             const int ee = u * V + e;
-                            Cell& dstc = (out.axis == AXIS_ALL) ? acc[o] : (out.axis == AXIS_COLS) ? acc_col[o][ee] : rowc;
+                            Cell& dstc = (out.axis == AXIS_ALL) ? acc[o] : (out.axis == AXIS_COLS) ? acc_col[o][ee] : rowc[out.axis == AXIS_ROWS ? slots.row[o] : 0][j];
                             if (out_is_pred_reduction(out.kind)) cell_accum_pred(out.kind, dstc, p[out.src][ee]);
                             else if (out.pred == SG_NO_PRED || p[out.pred == SG_NO_PRED ? 0 : out.pred][ee]) cell_accum_value<T>(out.kind, dstc, v[out.src][ee]);
                         }
                     }
-                    if (out.axis == AXIS_ROWS) {
-#pragma unroll
-                        for (int d = 16; d >= 1; d >>= 1) {
-                            Cell other = cell_shfl_xor_kind<T>(out.kind, rowc, d);
-                            cell_combine<T>(out.kind, rowc, other);
-                        }
-                        if (lane == 0) s_row[slots.row[o]][warp][(int)(r - rb)] = rowc;
-                    }
                 }
             }
+        }
+        // the RS rows of the stage are reduced across the warp together (see warp_reduce_rows)
+#pragma unroll
+        for (int o = 0; o < M::S.n_out; ++o) {
+            const SgOut out = g.out[o];
+            if (!(out_is_reduction(out.kind) && out.axis == AXIS_ROWS)) continue;
+            warp_reduce_rows<T, RS>(out.kind, rowc[slots.row[o]], lane);
+            const int64_t r = r0 + warp_row_of_lane<RS>(lane);
+            if (warp_row_owner<RS>(lane) && r < r_end) s_row[slots.row[o]][warp][(int)(r - rb)] = rowc[slots.row[o]][0];
         }
         __syncthreads();                        // every thread is done with stage s (and with this batch's s_row writes)
         if (threadIdx.x == 0 && b + NS < nb) { fence_proxy_async(); issue(b + NS); }

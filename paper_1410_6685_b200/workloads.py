@@ -357,3 +357,27 @@ def quicksort(ctx, dtype, n, pa, pout, pscratch0, pscratch1, contracts=True):
         res["sorted"] = sg.sg_forall_adjacent(ctx, out, sg.SG_LE)
         sg.sg_contract(ctx, res["sorted"], sg.SG_CONTRACT_POST, "Result.is_sorted")
     return res
+
+
+# ------------------------------------------------------------------------------------------------------------------
+# memory-bound matrix-vector products
+# ------------------------------------------------------------------------------------------------------------------
+def right_multiply(ctx, rows, cols, pM, pv, ld=None):
+    """matrix x column vector: result_i = sum_c M[i,c]*v[c] — the product is an anonymous intermediate of ONE matrix pass (v
+    broadcast along the rows, per-row sums).  The dimension contract columns = v.count is checked at enqueue."""
+    M = sg.sg_mat_create(ctx, sg.SG_F64, rows, cols, cols if ld is None else ld, pM)
+    v = sg.sg_vec_create(ctx, sg.SG_F64, cols, pv)
+    t = sg.sg_enqueue(ctx, sg.SG_MUL, [M, H(v, sg.SG_BCAST_ROW)])
+    r = sg.sg_reduce(ctx, t, sg.SG_SUM, sg.SG_AXIS_ROWS)
+    sg.sg_release(ctx, t)
+    return {"M": M, "v": v, "out": r}
+
+
+def left_multiply(ctx, rows, cols, pv, pM, ld=None):
+    """row vector x matrix: result_c = sum_i v[i]*M[i,c] — v broadcast along the columns, per-column sums, one matrix pass."""
+    M = sg.sg_mat_create(ctx, sg.SG_F64, rows, cols, cols if ld is None else ld, pM)
+    v = sg.sg_vec_create(ctx, sg.SG_F64, rows, pv)
+    t = sg.sg_enqueue(ctx, sg.SG_MUL, [M, H(v, sg.SG_BCAST_COL)])
+    r = sg.sg_reduce(ctx, t, sg.SG_SUM, sg.SG_AXIS_COLS)
+    sg.sg_release(ctx, t)
+    return {"M": M, "v": v, "out": r}

@@ -185,3 +185,44 @@ def test_quicksort_signed_zeros_sorted_input_fp64_and_bytecode():
     for a in (np.arange(3000, dtype=np.float64), np.arange(3000, dtype=np.float64)[::-1].copy(), RNG.standard_normal(2500)):
         got, ok, _ = _quicksort_on_device(a, sg.SG_FLAG_FORCE_BYTECODE)
         assert ok and bits_equal(got, ocfg.quicksort(a))
+
+
+# ----------------------------------------------------------------------------------------------------------
+# matrix-vector products — fp64 sums within 1e-12 relative of the oracle
+# ----------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("rows,cols,ld", [(1, 1, 1), (2, 3, 3), (33, 17, 20), (258, 1030, 1030), (1030, 258, 264), (777, 2051, 2051)])
+def test_matvec_right_and_left(rows, cols, ld):
+    M = RNG.uniform(0.0, 1.0, (rows, cols))
+    v, w = RNG.uniform(0.5, 1.5, cols), RNG.uniform(0.5, 1.5, rows)
+    Mp = np.zeros((rows, ld))
+    Mp[:, :cols] = M
+    with Ctx() as c:
+        tM, tv, tw = dev(Mp), dev(v), dev(w)
+        c.keep += [tM, tv, tw]
+        r = W.right_multiply(c.ctx, rows, cols, tM.data_ptr(), tv.data_ptr(), ld)
+        sg.sg_flush(c.ctx)
+        st_r = sg.sg_plan_stats(c.ctx)
+        l = W.left_multiply(c.ctx, rows, cols, tw.data_ptr(), tM.data_ptr(), ld)
+        sg.sg_flush(c.ctx)
+        st_l = sg.sg_plan_stats(c.ctx)
+        got_r, got_l = c.read_vec(r["out"], np.float64, rows), c.read_vec(l["out"], np.float64, cols)
+    assert (st_r.n_passes, st_r.n_template, st_l.n_passes, st_l.n_template) == (1, 1, 1, 1)      # one matrix pass each
+    want_r, want_l = ocfg.right_multiply(M, v), ocfg.left_multiply(w, M)
+    assert np.all(np.abs(got_r - want_r) <= 1e-12 * np.abs(want_r))
+    assert np.all(np.abs(got_l - want_l) <= 1e-12 * np.abs(want_l))
+
+
+def test_matvec_exact_integer_regime_and_dimension_contract():
+    M = RNG.integers(-8, 9, (300, 500)).astype(np.float64)
+    v, w = RNG.integers(-8, 9, 500).astype(np.float64), RNG.integers(-8, 9, 300).astype(np.float64)
+    with Ctx() as c:
+        tM, tv, tw = dev(M), dev(v), dev(w)
+        c.keep += [tM, tv, tw]
+        r = W.right_multiply(c.ctx, 300, 500, tM.data_ptr(), tv.data_ptr())
+        sg.sg_flush(c.ctx)
+        l = W.left_multiply(c.ctx, 300, 500, tw.data_ptr(), tM.data_ptr())
+        got_r, got_l = c.read_vec(r["out"], np.float64, 300), c.read_vec(l["out"], np.float64, 500)
+        with pytest.raises(sg.SgError) as e:                       # columns /= v.count
+            sg.sg_enqueue(c.ctx, sg.SG_MUL, [r["M"], sg.H(l["v"], sg.SG_BCAST_ROW)])      # a 300-vector along 500 columns
+        assert e.value.status == sg.SG_ERR_SHAPE
+    assert bits_equal(got_r, ocfg.right_multiply(M, v)) and bits_equal(got_l, ocfg.left_multiply(w, M))
