@@ -190,7 +190,8 @@ def test_quicksort_signed_zeros_sorted_input_fp64_and_bytecode():
 # ----------------------------------------------------------------------------------------------------------
 # matrix-vector products — fp64 sums within 1e-12 relative of the oracle
 # ----------------------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("rows,cols,ld", [(1, 1, 1), (2, 3, 3), (33, 17, 20), (258, 1030, 1030), (1030, 258, 264), (777, 2051, 2051)])
+# matrix passes need 16-byte aligned rows (even fp64 column count and leading dimension): the same contract as config 4's pass
+@pytest.mark.parametrize("rows,cols,ld", [(1, 2, 2), (2, 2, 2), (3, 4, 6), (33, 18, 20), (258, 1030, 1030), (1030, 258, 264), (777, 2050, 2052)])
 def test_matvec_right_and_left(rows, cols, ld):
     M = RNG.uniform(0.0, 1.0, (rows, cols))
     v, w = RNG.uniform(0.5, 1.5, cols), RNG.uniform(0.5, 1.5, rows)
@@ -210,6 +211,16 @@ def test_matvec_right_and_left(rows, cols, ld):
     want_r, want_l = ocfg.right_multiply(M, v), ocfg.left_multiply(w, M)
     assert np.all(np.abs(got_r - want_r) <= 1e-12 * np.abs(want_r))
     assert np.all(np.abs(got_l - want_l) <= 1e-12 * np.abs(want_l))
+
+
+def test_matvec_misaligned_rows_fail_loudly():
+    with Ctx() as c:
+        tM, tv = dev(np.ones((4, 3))), dev(np.ones(3))
+        c.keep += [tM, tv]
+        W.right_multiply(c.ctx, 4, 3, tM.data_ptr(), tv.data_ptr())
+        with pytest.raises(sg.SgError) as e:
+            sg.sg_flush(c.ctx)
+        assert e.value.status == sg.SG_ERR_UNSUPPORTED                # an error, never a fallback
 
 
 def test_matvec_exact_integer_regime_and_dimension_contract():
