@@ -155,3 +155,13 @@ def left_multiply(v, M) -> np.ndarray:
     for i in range(M.shape[0]):
         T[i] = orc.scalar("mul", M[i], v[i])
     return orc.col_sum(T) if M.shape[0] else np.zeros(M.shape[1])
+
+
+def transpose(M) -> np.ndarray:
+    """`transpose`: a new rows x cols -> cols x rows matrix with out[j][i] = M[i][j], written out element by element."""
+    M = np.ascontiguousarray(M)
+    assert M.ndim == 2
+    out = np.empty((M.shape[1], M.shape[0]), dtype=M.dtype)
+    for i in range(M.shape[0]):
+        out[:, i] = M[i, :]
+    return out

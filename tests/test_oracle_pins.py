@@ -711,3 +711,16 @@ def test_matvec_general_values_against_exact_rationals():
     for c in range(7):
         ex = sum(Fraction(float(w[i] * M[i, c])) for i in range(5))
         assert abs(Fraction(float(l[c])) - ex) <= abs(ex) * Fraction(1, 2 ** 51)
+
+
+def test_transpose_hand_values_involution_and_library():
+    A = np.array([[1.0, 2.0, 3.0], [4.0, 5.0, 6.0]])
+    assert ocfg.transpose(A).tolist() == [[1.0, 4.0], [2.0, 5.0], [3.0, 6.0]]
+    for shape in ((1, 1), (1, 7), (7, 1), (33, 65), (130, 64)):
+        for dt in (np.float32, np.float64, np.int32):
+            M = RNG.integers(-1000, 1000, shape).astype(dt)
+            T = ocfg.transpose(M)
+            assert T.shape == shape[::-1] and T.dtype == M.dtype and T.flags["C_CONTIGUOUS"]
+            assert np.array_equal(ocfg.transpose(T), M)                     # involution
+            assert np.array_equal(T, M.T)                                   # library view
+            assert all(T[j, i] == M[i, j] for i in range(0, shape[0], 5) for j in range(0, shape[1], 3))
