@@ -166,6 +166,7 @@ def per_config(torch, sg, W, inputs, peak, which):
         finally:
             sg.sg_ctx_destroy(ctx)
 
+    measure.out, measure.peak = out, peak
     if "cfg0" in which:
         cfg0_section(torch, sg, W, inputs, measure)
     if "cfg1" in which:
@@ -288,13 +289,29 @@ def matvec_section(torch, sg, W, inputs, measure):
     alg = 8 * n * n + 16 * n
     measure("matvec_right_multiply_fp64_16384^2", lambda ctx: W.right_multiply(ctx, n, n, M.data_ptr(), v.data_ptr()), alg)
     measure("matvec_left_multiply_fp64_16384^2", lambda ctx: W.left_multiply(ctx, n, n, v.data_ptr(), M.data_ptr()), alg)
+    # transpose: not a deferred pass (sg_mat_transpose launches at the call), timed with events around 10 calls
+    T = torch.empty_like(M)
+    stream = torch.cuda.current_stream().cuda_stream
+    ctx = sg.sg_ctx_create(0, stream)
+    hM = sg.sg_mat_create(ctx, sg.SG_F64, n, n, n, M.data_ptr())
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    for reps in (3, 10):
+        e0.record()
+        for _ in range(reps):
+            sg.sg_release(ctx, sg.sg_mat_transpose(ctx, hM, T.data_ptr(), n))
+        e1.record()
+        torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / 10
+    sg.sg_ctx_destroy(ctx)
+    measure.out["transpose_fp64_16384^2"] = {"ms": ms, "algorithmic_bytes": 16 * n * n, "GB/s": 16 * n * n / ms / 1e6,
+                                             "frac_of_peak": 16 * n * n / ms / 1e6 / measure.peak, "passes": 1, "template_passes": 0}
 
 
 def quicksort_section(torch, sg, W, inputs, out):
     """Listing 3 on fp32 normal(0,1) keys; wall time of the whole sort (one count read-back per partition).
     Launch- and latency-bound by construction (the listing recurses down to single elements): reported, not a roofline line."""
     stream = torch.cuda.current_stream().cuda_stream
-    for log2n in (12, 16):
+    for log2n in (12, 14):
         n = 1 << log2n
         a = torch.from_numpy(inputs.normal_f32(2, 0, n)).cuda()
         o, s0, s1 = (torch.empty_like(a) for _ in range(3))

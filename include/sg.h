@@ -186,6 +186,13 @@ sg_status sg_vec_read(sg_ctx* ctx, sg_handle v, void* host_out, size_t bytes);
 /* Drop the caller's reference.  An unreferenced pending intermediate is never materialised. */
 sg_status sg_release(sg_ctx* ctx, sg_handle h);
 
+/* transpose: a NEW cols x rows matrix with out[j][i] = m[i][j] (F32/F64/I32/I64), written to dev_out_or_null
+ * (borrowed, leading dimension ld_out elements; NULL => allocated by the context; ld_out 0 => rows of m).  A pure data mover with
+ * no elementwise body to fuse into, so it is not deferred: operations pending on m are flushed first (trigger (2)),
+ * then one tiled kernel is enqueued on the context stream (asynchronous; nothing is read back).  Errors: SG_ERR_ARG,
+ * SG_ERR_DTYPE (BOOL), SG_ERR_ALIAS (dev_out overlaps m), SG_ERR_OOM, SG_ERR_CUDA. */
+sg_status sg_mat_transpose(sg_ctx* ctx, sg_handle m, void* dev_out_or_null, int64_t ld_out, sg_handle* out_mat);
+
 /* Listing 5's loop body for steps k in [k0, k1) of the square F64 matrix m, as a library composite over the
  * primitives above.  Step k: det <- det * M[k,k] and minpiv <- MIN(minpiv, ABS(M[k,k]))
  * on the one-element F64 vectors det / minpiv, then for ALL rows j > k in one matrix pass M[j,:] <- M[j,:] - (M[j,k]/M[k,k]) * M[k,:]

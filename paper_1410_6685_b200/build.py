@@ -15,7 +15,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libsafegpu.so")
-SOURCES = ["sg_kernels.cu", "sg_api.cpp", "sg_plan.cpp", "sg_build.cpp"]
+SOURCES = ["sg_kernels.cu", "sg_api.cpp", "sg_plan.cpp", "sg_build.cpp", "sg_transpose.cu"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-fmad=false", "-std=c++17",
@@ -35,14 +35,39 @@ def _stamp() -> str:
     return h.hexdigest()
 
 
+def _dep_hash(src: str) -> str:
+    """Hash of what an object depends on: its source, the flags, include/sg.h and every header in csrc/ it may include
+    (host .cpp files never include the kernel headers .cuh / .inc; sg_transpose.cu includes only sg_kernels.h / sg_prog.h)."""
+    light = src.endswith(".cpp") or src == "sg_transpose.cu"
+    h = hashlib.sha256()
+    for name in sorted(os.listdir(CSRC)):
+        if name == src or name.endswith(".h") or (not light and name.endswith((".cuh", ".inc"))):
+            with open(os.path.join(CSRC, name), "rb") as f:
+                h.update(name.encode())
+                h.update(f.read())
+    with open(os.path.join(os.path.dirname(HERE), "include", "sg.h"), "rb") as f:
+        h.update(f.read())
+    h.update(" ".join(FLAGS).encode())
+    return h.hexdigest()
+
+
 def _compile(src: str) -> str:
     obj = os.path.join(OBJ, src + ".o")
+    dep_file, dep = obj + ".dep", _dep_hash(src)
+    if os.path.exists(obj) and os.path.exists(dep_file) and open(dep_file).read() == dep:
+        return obj              # unchanged since it was compiled
     subprocess.run([NVCC, *FLAGS, "-c", os.path.join(CSRC, src), "-o", obj], check=True)
+    with open(dep_file, "w") as f:
+        f.write(dep)
     return obj
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
     os.makedirs(OBJ, exist_ok=True)
+    if force:
+        for name in os.listdir(OBJ):
+            if name.endswith(".dep"):
+                os.remove(os.path.join(OBJ, name))
     stamp_file = os.path.join(OBJ, "stamp")
     stamp = _stamp()
     if not force and os.path.exists(LIB) and os.path.exists(stamp_file) and open(stamp_file).read() == stamp:

@@ -352,6 +352,41 @@ sg_status sg_enqueue(sg_ctx* c, sg_op op, const sg_operand* ops, int32_t n, sg_h
     return append_map(c, (uint8_t)op, unary ? 1 : 2, opd, dtype, is2d, rows, cols, dst, out);
 }
 
+sg_status sg_mat_transpose(sg_ctx* c, sg_handle m, void* dev_out, int64_t ld_out, sg_handle* out) {
+    CK(c && out);
+    Value* v;
+    sg_status s;
+    // trigger (2): the kernel below is not part of the pending list, so EVERYTHING pending runs first — a pending operation may
+    // write m's memory (or read the output buffer) through another handle or view of the same storage
+    if (!c->nodes.empty() && (s = sg_flush_impl(c)) != SG_OK) return s;
+    if ((s = need_storage(c, m, &v)) != SG_OK) return s;
+    if (v->kind != VK_MAT) return sg_fail(c, SG_ERR_ARG, "transpose needs a matrix");
+    const int es = dtype_size(v->dtype);
+    if (es != 4 && es != 8) return sg_fail(c, SG_ERR_DTYPE, "transpose of a BOOL matrix");
+    const int64_t rows = v->rows, cols = v->cols, ld_in = v->ld;
+    const char* src = v->ptr;
+    if (ld_out == 0) ld_out = rows;
+    if (ld_out < rows) return sg_fail(c, SG_ERR_ARG, "leading dimension of the transpose is smaller than its column count");
+    if (dev_out) {
+        const char* a0 = src; const char* a1 = src + (size_t)rows * ld_in * es;
+        const char* b0 = (const char*)dev_out; const char* b1 = b0 + (size_t)cols * ld_out * es;
+        if (a0 < b1 && b0 < a1) return sg_fail(c, SG_ERR_ALIAS, "transpose output overlaps its input");
+    }
+    sg_handle h;
+    s = sg_mat_create(c, (sg_dtype)v->dtype, cols, rows, ld_out, dev_out, &h);      // may reallocate the handle table: v is stale now
+    if (s != SG_OK) return s;
+    if (!c->plan_only) {
+        if (sgk_transpose(src, ld_in, rows, cols, val(c, h)->ptr, ld_out, es, c->stream) != cudaSuccess) {
+            cudaGetLastError();
+            sg_release(c, h);
+            return sg_fail(c, SG_ERR_CUDA, "transpose launch failed");
+        }
+    }
+    c->stats.launches_total++;
+    *out = h;
+    return SG_OK;
+}
+
 sg_status sg_mat_col(sg_ctx* c, sg_handle m, int64_t j, int64_t r0, int64_t r1, sg_handle* out) {
     CK(c && out);
     Value* v;

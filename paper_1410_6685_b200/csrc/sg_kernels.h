@@ -4,6 +4,7 @@
 
 #include <cuda_runtime.h>
 #include <stddef.h>
+#include <stdint.h>
 
 #include "sg_prog.h"
 
@@ -29,5 +30,8 @@ int sgk_find_template(const SgProg& prog);          // 0 if none
 int sgk_plan(const SgProg& prog, SgArgs& args, int force_bytecode, int sm_count, int has_device, SgGeom* geom, char* err, size_t errcap);
 
 cudaError_t sgk_launch(const SgProg& prog, const SgArgs& args, const SgGeom& geom, cudaStream_t stream);
+
+// sg_transpose.cu: out[c][r] = in[r][c] for a rows x cols row-major matrix of 4- or 8-byte elements (device pointers).
+cudaError_t sgk_transpose(const void* in, int64_t ld_in, int64_t rows, int64_t cols, void* out, int64_t ld_out, int elem_size, cudaStream_t stream);
 
 #endif  // SG_KERNELS_H_

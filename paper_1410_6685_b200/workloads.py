@@ -381,3 +381,10 @@ def left_multiply(ctx, rows, cols, pv, pM, ld=None):
     r = sg.sg_reduce(ctx, t, sg.SG_SUM, sg.SG_AXIS_COLS)
     sg.sg_release(ctx, t)
     return {"M": M, "v": v, "out": r}
+
+
+def transpose(ctx, dtype, rows, cols, pM, pout=None, ld=None, ld_out=0):
+    """`transpose`: a new cols x rows matrix; one tiled data-mover kernel (sg_mat_transpose), asynchronous."""
+    M = sg.sg_mat_create(ctx, dtype, rows, cols, cols if ld is None else ld, pM)
+    T = sg.sg_mat_transpose(ctx, M, pout, ld_out)
+    return {"M": M, "out": T}

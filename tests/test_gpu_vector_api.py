@@ -237,3 +237,54 @@ def test_matvec_exact_integer_regime_and_dimension_contract():
             sg.sg_enqueue(c.ctx, sg.SG_MUL, [r["M"], sg.H(l["v"], sg.SG_BCAST_ROW)])      # a 300-vector along 500 columns
         assert e.value.status == sg.SG_ERR_SHAPE
     assert bits_equal(got_r, ocfg.right_multiply(M, v)) and bits_equal(got_l, ocfg.left_multiply(w, M))
+
+
+# ----------------------------------------------------------------------------------------------------------
+# transpose — a data mover, bit-exact
+# ----------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("dtype", [np.float64, np.float32, np.int32, np.int64])
+@pytest.mark.parametrize("rows,cols,ld,ld_out", [(1, 1, 1, 0), (1, 7, 7, 0), (7, 1, 3, 9), (64, 64, 64, 0), (65, 63, 70, 66), (130, 1000, 1000, 0),
+                                                 (1000, 130, 136, 1001), (257, 513, 513, 0)])
+def test_transpose(dtype, rows, cols, ld, ld_out):
+    M = RNG.integers(-10**6, 10**6, (rows, cols)).astype(dtype)
+    Mp = np.full((rows, ld), -7, dtype=dtype)
+    Mp[:, :cols] = M
+    ldo = ld_out or rows
+    with Ctx() as c:
+        tM = dev(Mp)
+        tout = dev(np.full((cols, ldo), -9, dtype=dtype))
+        c.keep += [tM, tout]
+        r = W.transpose(c.ctx, gpu_util_dtype(dtype), rows, cols, tM.data_ptr(), tout.data_ptr(), ld, ld_out)
+        c.torch.cuda.synchronize()
+        got = tout.cpu().numpy()
+        # library-allocated output, then transposed back: the involution
+        r2 = W.transpose(c.ctx, gpu_util_dtype(dtype), rows, cols, tM.data_ptr(), None, ld)
+        back = sg.sg_mat_transpose(c.ctx, r2["out"])
+        flat = np.empty(rows * cols, dtype=dtype)
+        sg.sg_vec_read(c.ctx, back, flat.ctypes.data, flat.nbytes)
+    want = ocfg.transpose(M)
+    assert bits_equal(np.ascontiguousarray(got[:, :rows]), want)
+    assert np.all(got[:, rows:] == -9)                                  # padding of the destination is not touched
+    assert bits_equal(flat.reshape(rows, cols), M)
+
+
+def gpu_util_dtype(dtype):
+    from gpu_util import NP2SG
+    return NP2SG[np.dtype(dtype)]
+
+
+def test_transpose_runs_after_pending_writers_and_rejects_overlap():
+    n = 130
+    M = RNG.standard_normal((n, n))
+    with Ctx() as c:
+        tM = dev(M); c.keep.append(tM)
+        hM = sg.sg_mat_create(c.ctx, sg.SG_F64, n, n, n, tM.data_ptr())
+        v = sg.sg_vec_create(c.ctx, sg.SG_F64, n * n, tM.data_ptr())
+        sg.sg_enqueue(c.ctx, sg.SG_MUL, [v, sg.F(2.0)], dst_or_0=v)    # pending in-place writer of the same memory
+        hT = sg.sg_mat_transpose(c.ctx, hM)                            # flushes it first (trigger (2))
+        flat = np.empty(n * n)
+        sg.sg_vec_read(c.ctx, hT, flat.ctypes.data, flat.nbytes)
+        with pytest.raises(sg.SgError) as e:
+            sg.sg_mat_transpose(c.ctx, hM, tM.data_ptr() + 64, 0)
+        assert e.value.status == sg.SG_ERR_ALIAS
+    assert bits_equal(flat.reshape(n, n), ocfg.transpose(orc.scalar("mul", M.reshape(-1), 2.0).reshape(n, n)))
