@@ -331,8 +331,12 @@ def quicksort(ctx, dtype, n, pa, pout, pscratch0, pscratch1, contracts=True):
         lt = sg.sg_enqueue(ctx, sg.SG_LT, [a, H(pivot)])
         eq = sg.sg_enqueue(ctx, sg.SG_EQ, [a, H(pivot)])
         gt = sg.sg_enqueue(ctx, sg.SG_GT, [a, H(pivot)])
-        hl, hm = sg.sg_reduce(ctx, lt, sg.SG_COUNT), sg.sg_reduce(ctx, eq, sg.SG_COUNT)
-        nl, nm = sg.sg_scalar_get(ctx, hl), sg.sg_scalar_get(ctx, hm)  # trigger: one flush, two small passes
+        if m == 1:                                                     # `if a.count = 1 then Result := a`: nothing to count
+            hl = hm = None
+            nl, nm = 0, 1
+        else:
+            hl, hm = sg.sg_reduce(ctx, lt, sg.SG_COUNT), sg.sg_reduce(ctx, eq, sg.SG_COUNT)
+            nl, nm = sg.sg_scalar_get(ctx, hl), sg.sg_scalar_get(ctx, hm)  # trigger: one flush, two small passes
         nr = m - nl - nm
         nxt = scratch[depth % 2]
         outs = []
@@ -344,7 +348,8 @@ def quicksort(ctx, dtype, n, pa, pout, pscratch0, pscratch1, contracts=True):
         sg.sg_flush(ctx)                                               # asynchronous: nothing is read back
         placed += nm
         for h in [hl, hm, lt, eq, gt, pivot, mid1, a] + [x for pair in outs for x in pair]:
-            sg.sg_release(ctx, h)
+            if h is not None:
+                sg.sg_release(ctx, h)
         if nr > 0:
             stack.append((nxt, o + nl + nm, o + nl + nm, nr, depth + 1))
         if nl > 0:
