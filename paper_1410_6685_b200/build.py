@@ -15,7 +15,8 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libsafegpu.so")
-SOURCES = ["sg_kernels.cu", "sg_api.cpp", "sg_plan.cpp", "sg_build.cpp", "sg_transpose.cu"]
+NSHARDS = 8        # == SG_NSHARDS in csrc/sg_tmpl_launch.cuh: the template instances compile as eight translation units in parallel
+SOURCES = [f"sg_vm_shard.cu@{k}" for k in range(4)] + [f"sg_tmpl_shard.cu@{k}" for k in range(NSHARDS)] + ["sg_kernels.cu", "sg_api.cpp", "sg_plan.cpp", "sg_build.cpp", "sg_transpose.cu"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-fmad=false", "-std=c++17",
@@ -51,12 +52,14 @@ def _dep_hash(src: str) -> str:
     return h.hexdigest()
 
 
-def _compile(src: str) -> str:
-    obj = os.path.join(OBJ, src + ".o")
+def _compile(item: str) -> str:
+    src, _, shard = item.partition("@")             # "file@k": shard k of the template instances (-DSG_SHARD=k)
+    obj = os.path.join(OBJ, src + (f".{shard}" if shard else "") + ".o")
     dep_file, dep = obj + ".dep", _dep_hash(src)
     if os.path.exists(obj) and os.path.exists(dep_file) and open(dep_file).read() == dep:
         return obj              # unchanged since it was compiled
-    subprocess.run([NVCC, *FLAGS, "-c", os.path.join(CSRC, src), "-o", obj], check=True)
+    extra = [f"-D{'SG_VM_DTYPE' if src == 'sg_vm_shard.cu' else 'SG_SHARD'}={shard}"] if shard else []
+    subprocess.run([NVCC, *FLAGS, *extra, "-c", os.path.join(CSRC, src), "-o", obj], check=True)
     with open(dep_file, "w") as f:
         f.write(dep)
     return obj
@@ -72,7 +75,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
     stamp = _stamp()
     if not force and os.path.exists(LIB) and os.path.exists(stamp_file) and open(stamp_file).read() == stamp:
         return LIB
-    with concurrent.futures.ThreadPoolExecutor(max_workers=len(SOURCES)) as ex:
+    with concurrent.futures.ThreadPoolExecutor(max_workers=min(len(SOURCES), os.cpu_count() or 4)) as ex:
         objs = list(ex.map(_compile, SOURCES))
     tmp = LIB + f".tmp{os.getpid()}"
     subprocess.run([NVCC, "-shared", "-o", tmp, *objs, "-gencode", "arch=compute_100a,code=sm_100a"], check=True)

@@ -8,177 +8,49 @@
 
 #include <algorithm>
 
-#include "sg_filter.cuh"
-#include "sg_pass1d_tmpl.cuh"
 #include "sg_pass1d_vm.cuh"
-#include "sg_pass2d.cuh"
+#include "sg_tmpl_launch.cuh"
+
+static_assert(SG_NSHARDS == 8, "the shard list below names eight tables");
+const sgk::Entry* sgk_shard_entries_0(int*); const sgk::Entry* sgk_shard_entries_1(int*); const sgk::Entry* sgk_shard_entries_2(int*);
+const sgk::Entry* sgk_shard_entries_3(int*); const sgk::Entry* sgk_shard_entries_4(int*); const sgk::Entry* sgk_shard_entries_5(int*);
+const sgk::Entry* sgk_shard_entries_6(int*); const sgk::Entry* sgk_shard_entries_7(int*);
+
+// sg_vm_shard.cu, one per element type (index = DT_*)
+cudaError_t sgk_launch_bytecode_0(const SgProg&, const SgArgs&, const SgGeom&, cudaStream_t); int sgk_occupancy_bytecode_0(bool, int, int);
+cudaError_t sgk_launch_bytecode_1(const SgProg&, const SgArgs&, const SgGeom&, cudaStream_t); int sgk_occupancy_bytecode_1(bool, int, int);
+cudaError_t sgk_launch_bytecode_2(const SgProg&, const SgArgs&, const SgGeom&, cudaStream_t); int sgk_occupancy_bytecode_2(bool, int, int);
+cudaError_t sgk_launch_bytecode_3(const SgProg&, const SgArgs&, const SgGeom&, cudaStream_t); int sgk_occupancy_bytecode_3(bool, int, int);
 
 namespace {
 
 using namespace sgk;
 
-typedef cudaError_t (*LaunchFn)(const SgArgs&, int grid, cudaStream_t);
-template <class P> constexpr size_t smem_of() {
-    if constexpr ((P::prog.shape.flags & PF_2D) != 0) return sgk::Meta2D<P>::SMEM;
-    else if constexpr ((P::prog.shape.flags & PF_FILTER) != 0) return sgk::FilterTemplateEval<P>::SMEM;
-    else return 0;
-}
-typedef int (*OccFn)();
-
-struct Entry {
-    const char* name;
-    const SgProg* prog;
-    LaunchFn launch;
-    OccFn occupancy;
-    int tile;       // elements per tile (1-D, filter) or strip width (2-D)
+// registry: the shards' tables merged (entry i is owned by shard i % SG_NSHARDS); entry 0 is the bytecode kernel
+struct Registry {
+    Entry e[512];
+    int n = 1;
+    Registry() {
+        e[0] = {"bytecode", nullptr, nullptr, nullptr, 0};
+        typedef const Entry* (*ShardFn)(int*);
+        const ShardFn shards[SG_NSHARDS] = {sgk_shard_entries_0, sgk_shard_entries_1, sgk_shard_entries_2, sgk_shard_entries_3,
+                                            sgk_shard_entries_4, sgk_shard_entries_5, sgk_shard_entries_6, sgk_shard_entries_7};
+        int cnt = 0;
+        const Entry* tabs[SG_NSHARDS];
+        for (int s = 0; s < SG_NSHARDS; ++s) tabs[s] = shards[s](&cnt);
+        for (int i = 0; i < cnt && n < 512; ++i) e[n++] = tabs[i % SG_NSHARDS][i];
+    }
 };
+const Registry& registry() { static const Registry r; return r; }
+#define g_entries (registry().e)
+#define g_n_entries (registry().n)
 
-template <class P> constexpr int tile_of() {
-    if (P::prog.shape.flags & PF_FILTER) return FilterTemplateEval<P>::TILE;
-    return BLOCK * Meta1D<P>::E;
-}
-
-// TMA tensor map of one filter input: the vector seen as `rows` rows of 128 bytes, box = 256 rows (one tile), 128-byte
-// swizzle (sg_filter.cuh).  The driver entry point is fetched once through the runtime (no link against libcuda).
-typedef CUresult (*EncodeTiledFn)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*, const cuuint32_t*,
-                                  const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle, CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-bool encode_filter_tmap(void* out128, const void* base, long rows) {
-    static EncodeTiledFn fn = nullptr;
-    static bool tried = false;
-    if (!tried) {
-        tried = true;
-        void* p = nullptr;
-        cudaDriverEntryPointQueryResult q;
-        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &q) == cudaSuccess && q == cudaDriverEntryPointSuccess) fn = (EncodeTiledFn)p;
-        else cudaGetLastError();
-    }
-    if (!fn || rows <= 0 || rows > 0x7fffffffl) return false;
-    static_assert(sizeof(CUtensorMap) == 128, "tensor map size");
-    const cuuint64_t dims[2] = {32, (cuuint64_t)rows};
-    const cuuint64_t strides[1] = {128};
-    const cuuint32_t box[2] = {32, (cuuint32_t)F_ROWS};
-    const cuuint32_t estr[2] = {1, 1};
-    alignas(64) CUtensorMap m;
-    if (fn(&m, CU_TENSOR_MAP_DATA_TYPE_UINT32, 2, const_cast<void*>(base), dims, strides, box, estr, CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
-           CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) != CUDA_SUCCESS)
-        return false;
-    memcpy(out128, &m, 128);
-    return true;
-}
-template <class P> bool encode_filter_tmaps(SgArgs& a) {
-    typedef FilterTemplateEval<P> EV;
-    if (EV::NSTG == 0 || !((a.vec_ok >> 31) & 1) || a.n_full_tiles <= 0) return false;
-    int slot = 0;       // index among the IN_VEC inputs
-    for (int k = 0; k < P::prog.shape.n_in; ++k) {
-        if (P::prog.in[k].kind != IN_VEC) continue;
-        if (slot < EV::NSTG && !encode_filter_tmap(a.tmap[slot], a.in_ptr[k], (long)a.n_full_tiles * F_ROWS)) return false;
-        ++slot;
-    }
-    return true;
-}
-
-template <class P> cudaError_t launch_template(const SgArgs& a, int grid, cudaStream_t s) {
-    if constexpr ((P::prog.shape.flags & PF_2D) != 0) {
-        static bool attr_set = false;
-        if (!attr_set) { cudaFuncSetAttribute(pass2d_template<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_of<P>()); attr_set = true; }
-        pass2d_template<P><<<grid, BLOCK, smem_of<P>(), s>>>(a);
-    }
-    else if constexpr ((P::prog.shape.flags & PF_FILTER) != 0) {
-        static bool attr_set = false;
-        if (!attr_set) { cudaFuncSetAttribute(filter1d_template<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_of<P>()); attr_set = true; }
-        SgArgs a2 = a;
-        a2.vec_ok &= ~(1 << 30);
-        if (encode_filter_tmaps<P>(a2)) a2.vec_ok |= (1 << 30);
-        filter1d_template<P><<<grid, FilterTemplateEval<P>::CT + 32, smem_of<P>(), s>>>(a2);
-    }
-    else pass1d_template<P><<<grid, BLOCK, 0, s>>>(a);
-    return cudaGetLastError();
-}
-template <class P> int occupancy_template() {
-    static int cached = 0;      // one query per instance per process (the query costs tens of microseconds)
-    if (cached > 0) return cached;
-    int occ = 0;
-    cudaError_t e;
-    if constexpr ((P::prog.shape.flags & PF_2D) != 0) {
-        cudaFuncSetAttribute(pass2d_template<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_of<P>());
-        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, pass2d_template<P>, BLOCK, smem_of<P>());
-    }
-    else if constexpr ((P::prog.shape.flags & PF_FILTER) != 0) {
-        cudaFuncSetAttribute(filter1d_template<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_of<P>());
-        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, filter1d_template<P>, FilterTemplateEval<P>::CT + 32, smem_of<P>());
-    }
-    else e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, pass1d_template<P>, BLOCK, 0);
-    if (e != cudaSuccess || occ <= 0) return 1;
-    cached = occ;
-    return occ;
-}
-
-// Each SG_TEMPLATE(name, unroll, min_blocks, row_unroll, {program}) in the generated file defines a policy type
-// and registers it.  The program initialisers are written by paper_1410_6685_b200/gen_templates.py from the plan
-// builder's own canonical output, so a registered chain always matches its signature.
-#define SG_TEMPLATE(NAME, UNROLL, MINB, ROWU, ...)                                   \
-    struct T_##NAME {                                                                \
-        static constexpr SgProg prog = __VA_ARGS__;                                  \
-        static constexpr int unroll = UNROLL, min_blocks = MINB, row_unroll = ROWU, stages = 3;  \
-    };
-#include "sg_templates_gen.inc"
-#undef SG_TEMPLATE
-
-#define SG_TEMPLATE(NAME, UNROLL, MINB, ROWU, ...) \
-    {#NAME, &T_##NAME::prog, &launch_template<T_##NAME>, &occupancy_template<T_##NAME>, tile_of<T_##NAME>()},
-const Entry g_entries[] = {
-    {"bytecode", nullptr, nullptr, nullptr, 0},
-#include "sg_templates_gen.inc"
-};
-#undef SG_TEMPLATE
-const int g_n_entries = (int)(sizeof(g_entries) / sizeof(g_entries[0]));
-
-template <class T, int C> cudaError_t launch_pass1d_bytecode(const SgProg& g, const SgArgs& a, int grid, cudaStream_t s) {
-    static bool attr_set = false;
-    if (!attr_set) { cudaFuncSetAttribute(pass1d_bytecode<T, C>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)vm_file_bytes(VM_VREG, 1)); attr_set = true; }
-    pass1d_bytecode<T, C><<<grid, BLOCK, vm_file_bytes(g.shape.n_vreg, C), s>>>(g, a);
-    return cudaGetLastError();
-}
-template <class T> cudaError_t launch_bytecode_t(const SgProg& g, const SgArgs& a, const SgGeom& geom, cudaStream_t s) {
-    if (g.shape.flags & PF_FILTER) {
-        static bool attr_set = false;
-        if (!attr_set) { cudaFuncSetAttribute(filter1d_bytecode<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FilterBytecodeEval<T>::SMEM); attr_set = true; }
-        filter1d_bytecode<T><<<geom.grid, BLOCK + 32, FilterBytecodeEval<T>::SMEM, s>>>(g, a);
-        return cudaGetLastError();
-    }
-    return geom.vm_cells == 2 ? launch_pass1d_bytecode<T, 2>(g, a, geom.grid, s) : launch_pass1d_bytecode<T, 1>(g, a, geom.grid, s);
-}
-// blocks per SM of the bytecode kernels (the 1-D pass depends on the size of its register file: queried once per size)
-template <class T> int occupancy_bytecode_t(bool filter, int n_vreg, int cells) {
-    static int cached_filter = 0, cached[VM_VREG + 1][VM_MAX_CELLS + 1] = {};
-    int occ = 0;
-    cudaError_t e;
-    if (filter) {
-        if (cached_filter > 0) return cached_filter;
-        cudaFuncSetAttribute(filter1d_bytecode<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FilterBytecodeEval<T>::SMEM);
-        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, filter1d_bytecode<T>, BLOCK + 32, FilterBytecodeEval<T>::SMEM);
-        if (e != cudaSuccess || occ <= 0) return 1;
-        return cached_filter = occ;
-    }
-    n_vreg = std::min(std::max(n_vreg, 1), VM_VREG);
-    if (cached[n_vreg][cells] > 0) return cached[n_vreg][cells];
-    const size_t smem = vm_file_bytes(n_vreg, cells);
-    if (cells == 2) {
-        cudaFuncSetAttribute(pass1d_bytecode<T, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)vm_file_bytes(VM_VREG, 1));
-        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, pass1d_bytecode<T, 2>, BLOCK, smem);
-    } else {
-        cudaFuncSetAttribute(pass1d_bytecode<T, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)vm_file_bytes(VM_VREG, 1));
-        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, pass1d_bytecode<T, 1>, BLOCK, smem);
-    }
-    if (e != cudaSuccess || occ <= 0) return 1;
-    return cached[n_vreg][cells] = occ;
-}
 int occupancy_bytecode(int dtype, bool filter, int n_vreg = VM_VREG, int cells = 1) {
     switch (dtype) {
-        case DT_F32: return occupancy_bytecode_t<float>(filter, n_vreg, cells);
-        case DT_F64: return occupancy_bytecode_t<double>(filter, n_vreg, cells);
-        case DT_I32: return occupancy_bytecode_t<int32_t>(filter, n_vreg, cells);
-        default: return occupancy_bytecode_t<long long>(filter, n_vreg, cells);
+        case DT_F32: return sgk_occupancy_bytecode_0(filter, n_vreg, cells);
+        case DT_F64: return sgk_occupancy_bytecode_1(filter, n_vreg, cells);
+        case DT_I32: return sgk_occupancy_bytecode_2(filter, n_vreg, cells);
+        default: return sgk_occupancy_bytecode_3(filter, n_vreg, cells);
     }
 }
 
@@ -308,10 +180,10 @@ int sgk_plan(const SgProg& prog, SgArgs& a, int force_bytecode, int sm_count, in
 cudaError_t sgk_launch(const SgProg& prog, const SgArgs& args, const SgGeom& geom, cudaStream_t stream) {
     if (geom.template_id > 0) return g_entries[geom.template_id].launch(args, geom.grid, stream);
     switch (prog.shape.dtype) {
-        case DT_F32: return launch_bytecode_t<float>(prog, args, geom, stream);
-        case DT_F64: return launch_bytecode_t<double>(prog, args, geom, stream);
-        case DT_I32: return launch_bytecode_t<int32_t>(prog, args, geom, stream);
-        case DT_I64: return launch_bytecode_t<long long>(prog, args, geom, stream);
+        case DT_F32: return sgk_launch_bytecode_0(prog, args, geom, stream);
+        case DT_F64: return sgk_launch_bytecode_1(prog, args, geom, stream);
+        case DT_I32: return sgk_launch_bytecode_2(prog, args, geom, stream);
+        case DT_I64: return sgk_launch_bytecode_3(prog, args, geom, stream);
         default: return cudaErrorInvalidValue;
     }
 }

@@ -176,7 +176,7 @@ __global__ void __launch_bounds__(BLOCK, P::min_blocks) pass2d_template(const __
 
     // ---- staged row loop: RS rows per stage, NS stages in flight (bulk copies issued by thread 0) -----------------
     constexpr int RS = RU, NS = M::NS;
-    extern __shared__ __align__(128) unsigned char dyn_smem[];
+    extern __shared__ __align__(1024) unsigned char dyn_smem[];     // same declaration as sg_filter.cuh (one symbol per translation unit)
     T* const stage_base = reinterpret_cast<T*>(dyn_smem);
     uint64_t* const full = reinterpret_cast<uint64_t*>(dyn_smem + (size_t)NS * M::NVECIN * RS * M::SW * sizeof(T));
     const int64_t c0 = (int64_t)strip * M::SW;
