@@ -84,6 +84,25 @@ def unary(op: str, a) -> np.ndarray:
     return out
 
 
+def cast(a, to) -> np.ndarray:
+    """project with the value-preserving conversion as the transform (R23): int -> float rounds to
+    nearest even, float -> int truncates toward zero with saturation and NaN -> 0, int64 -> int32 keeps the low 32 bits."""
+    a = _c(a)
+    to = np.dtype(to)
+    if a.dtype not in _DT or to not in _DT:
+        raise TypeError("cast converts between float32, float64, int32 and int64")
+    out = np.empty(a.shape, dtype=to)
+    _chk(lib().orc_cast(_DT[a.dtype], _DT[to], _n(a), _p(a), _p(out)), "cast")
+    return out
+
+
+def project_sqrt(a) -> np.ndarray:
+    """`c.project (agent (a: INT): DOUBLE do Result := sqrt (a) end)`: an integer collection gives a collection
+    of doubles — the conversion, then the correctly rounded square root, two primitives; a float collection keeps its dtype."""
+    a = _c(a)
+    return unary("sqrt", cast(a, np.float64) if a.dtype.kind == "i" else a)
+
+
 def cmp(op: str, a, b) -> np.ndarray:
     """BOOL[i] = a[i] cmp b[i]  (predicate agents)."""
     a, b = _c(a), _c(b)
@@ -231,7 +250,8 @@ def mat_step(M, kr: int, kc: int | None = None):
 def ge_determinant(M, eps: float = 0.0):
     """Listing 5: determinant by Gaussian elimination without pivoting, on a copy.
 
-    Returns (det, eliminated matrix, zero_step) — zero_step is the step whose |pivot| <= eps (det = 0), else -1."""
+    Returns (det, eliminated matrix, zero_step) — zero_step is the step whose |pivot| <= eps, where the loop ended (det is then
+    Result * pivot: the multiplication precedes the test), else -1."""
     M = np.array(M, dtype=np.float64, order="C", copy=True)
     if M.ndim != 2 or M.shape[0] != M.shape[1]:
         raise ValueError("square matrix expected")

@@ -217,6 +217,52 @@ template <class T> int64_t filter_t(int64_t n, const T* a, const uint8_t* mask, 
     return m;
 }
 
+// ---------------------------------------------------------------------------
+// project (transform: FUNCTION[T, U]): COLLECTION[U] with the value-preserving conversion as the
+// transform — the INT -> DOUBLE half of the paper's example `agent (a: INT): DOUBLE do Result := sqrt (a) end`
+// (PAPER.md:171-175).  The paper does not define conversions; the reading (R23):
+//   integer -> float : the nearest representable value, ties to even (an int32 is always exact in a double);
+//   float -> integer : truncation toward zero; values beyond the target's range saturate at its ends; NaN -> 0;
+//   double -> float  : round to nearest even;  float -> double, int32 -> int64 : exact;
+//   int64 -> int32   : the low 32 bits (two's-complement wrap, like every integer operation here, R14).
+// Written out case by case; the range tests are done in the floating type, where 2^31 and 2^63 are exact.
+// ---------------------------------------------------------------------------
+// float -> integer, F in {float, double}, I in {int32_t, int64_t}; two_p = 2^31 or 2^63 is exact in both floating types
+template <class I, class F> I float_to_int(F x, F two_p) {
+    if (x != x) return 0;                                                  // NaN
+    if (x >= two_p) return std::numeric_limits<I>::max();                  // saturate
+    if (x <= -two_p) return std::numeric_limits<I>::min();                 // -2^31 / -2^63 themselves are the minimum
+    return (I)std::trunc(x);                                               // |x| < 2^(bits-1): the truncated value is representable
+}
+inline void cv(float x, float* r) { *r = x; }
+inline void cv(float x, double* r) { *r = (double)x; }                                     // exact
+inline void cv(float x, int32_t* r) { *r = float_to_int<int32_t, float>(x, 2147483648.0f); }
+inline void cv(float x, int64_t* r) { *r = float_to_int<int64_t, float>(x, 9223372036854775808.0f); }
+inline void cv(double x, float* r) { *r = (float)x; }                                      // IEEE round to nearest even
+inline void cv(double x, double* r) { *r = x; }
+inline void cv(double x, int32_t* r) { *r = float_to_int<int32_t, double>(x, 2147483648.0); }
+inline void cv(double x, int64_t* r) { *r = float_to_int<int64_t, double>(x, 9223372036854775808.0); }
+inline void cv(int32_t x, float* r) { *r = (float)x; }                                     // IEEE round to nearest even
+inline void cv(int32_t x, double* r) { *r = (double)x; }                                   // exact
+inline void cv(int32_t x, int32_t* r) { *r = x; }
+inline void cv(int32_t x, int64_t* r) { *r = (int64_t)x; }                                 // sign extension
+inline void cv(int64_t x, float* r) { *r = (float)x; }                                     // IEEE round to nearest even
+inline void cv(int64_t x, double* r) { *r = (double)x; }                                   // IEEE round to nearest even
+inline void cv(int64_t x, int32_t* r) { *r = (int32_t)(uint32_t)(uint64_t)x; }             // low 32 bits
+inline void cv(int64_t x, int64_t* r) { *r = x; }
+template <class T, class S> void cast_loop(int64_t n, const S* a, T* out) {
+    for (int64_t i = 0; i < n; ++i) cv(a[i], &out[i]);
+}
+template <class S> int cast_from(int to, int64_t n, const S* a, void* out) {
+    switch (to) {
+        case F32: cast_loop(n, a, (float*)out); return 0;
+        case F64: cast_loop(n, a, (double*)out); return 0;
+        case I32: cast_loop(n, a, (int32_t*)out); return 0;
+        case I64: cast_loop(n, a, (int64_t*)out); return 0;
+        default: return -1;
+    }
+}
+
 }  // namespace
 
 #define DISPATCH(dtype, CALL)                                  \
@@ -391,16 +437,22 @@ int orc_mat_step(int64_t rows, int64_t cols, int64_t ld, double* M, int64_t kr, 
 }
 
 // Determinant by Gaussian elimination, Listing 5, step by step in the paper's order:
-//     Result := 1
+//     Result := 1                                                   (PAPER.md:331)
 //     for step = 0 .. n-1:
-//         pivot := M[step][step]                                   (PAPER.md:337)
-//         if pivot is approximately 0 -> Result := 0, stop         (PAPER.md:339 double_approx_equals(pivot, 0.0);
-//                                                                   the paper leaves eps open: |pivot| <= eps, R5)
-//         Result := Result * pivot
-//         for every row j > step: the row operation
-// The listing's row operation is garbled and rescales row j; the reading taken is
-// BASELINE.json:configs[4]'s textbook update, the same orc_mat_step defines: f_j = M[j][step] / pivot (read before
-// the row changes), t = f_j * M[step][c], M[j][c] = M[j][c] - t, one rounding per primitive.  M is overwritten by
+//         pivot := M[step][step]                                    (PAPER.md:337)
+//         Result := Result * pivot                                  (PAPER.md:338 — BEFORE the test below)
+//         if pivot is approximately 0 -> the loop ends              (PAPER.md:339 double_approx_equals(pivot, 0.0) and the
+//                                                                    else-branch PAPER.md:341-343 `step := matrix.rows`; the
+//                                                                    paper leaves eps open: |pivot| <= eps, R5)
+//         for every row j > step:
+//             p_j := M[j][step]
+//             if p_j is approximately 0 -> row j is left as it is   (PAPER.md:351 `if not double_approx_equals (pivot, 0.0)`)
+//             else the row operation
+// So a matrix with an approximately-zero pivot returns Result * pivot: a signed zero when eps = 0, a small non-zero
+// number when eps > 0 — never a hard-wired 0.0 (R11a).
+// The listing's row operation itself is garbled and rescales row j; the reading taken is
+// BASELINE.json:configs[4]'s textbook update, the same orc_mat_step defines: f_j = p_j / pivot (read before the row
+// changes), t = f_j * M[step][c], M[j][c] = M[j][c] - t, one rounding per primitive (R11).  M is overwritten by
 // the eliminated matrix; *zero_step = the step whose pivot was ~0, or -1.
 int orc_ge_determinant(int64_t n, int64_t ld, double* M, double eps, double* det, int64_t* zero_step) {
     if (n < 0 || ld < n) return -3;
@@ -408,10 +460,12 @@ int orc_ge_determinant(int64_t n, int64_t ld, double* M, double eps, double* det
     *zero_step = -1;
     for (int64_t step = 0; step < n; ++step) {
         const double pivot = M[step * ld + step];
-        if (un(ABS, pivot) <= eps) { result = 0.0; *zero_step = step; break; }
         result = result * pivot;
+        if (un(ABS, pivot) <= eps) { *zero_step = step; break; }
         for (int64_t j = step + 1; j < n; ++j) {
-            const double f = M[j * ld + step] / pivot;
+            const double pj = M[j * ld + step];
+            if (un(ABS, pj) <= eps) continue;
+            const double f = pj / pivot;
             for (int64_t c = 0; c < n; ++c) {
                 double t = f * M[step * ld + c];
                 M[j * ld + c] = M[j * ld + c] - t;
@@ -420,6 +474,17 @@ int orc_ge_determinant(int64_t n, int64_t ld, double* M, double eps, double* det
     }
     *det = result;
     return 0;
+}
+
+// dtype-changing projection: see cv() above (R23)
+int orc_cast(int from, int to, int64_t n, const void* a, void* out) {
+    switch (from) {
+        case F32: return cast_from(to, n, (const float*)a, out);
+        case F64: return cast_from(to, n, (const double*)a, out);
+        case I32: return cast_from(to, n, (const int32_t*)a, out);
+        case I64: return cast_from(to, n, (const int64_t*)a, out);
+        default: return -1;
+    }
 }
 
 }  // extern "C"

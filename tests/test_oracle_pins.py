@@ -44,7 +44,18 @@ def test_float_arith_is_correctly_rounded(dtype, op):
     for i in range(a.size):
         q = exact(op, a[i], b[i])
         want = dtype(rnd(q))
-        assert got[i] == want and np.signbit(got[i]) == np.signbit(want) or (q == 0), (op, a[i], b[i], got[i], want)
+        if q != 0:
+            assert got[i] == want and np.signbit(got[i]) == np.signbit(want), (op, a[i], b[i], got[i], want)
+        else:
+            # an exactly-zero result: the rational has no sign, IEEE 754 fixes it — products and quotients take the XOR of the
+            # operand signs; a sum x + y that cancels is +0 under round-to-nearest unless both addends are -0
+            sa, sb = bool(np.signbit(a[i])), bool(np.signbit(b[i]))
+            if op in ("mul", "div"):
+                neg = sa != sb
+            else:
+                sb_eff = sb if op == "add" else not sb
+                neg = sa and sb_eff and a[i] == 0 and b[i] == 0
+            assert got[i] == 0 and bool(np.signbit(got[i])) == neg, (op, a[i], b[i], got[i])
     # scalar forms, both operand orders
     s = dtype(2.5)
     got = orc.scalar(op, a, s)
@@ -57,12 +68,13 @@ def test_float_arith_is_correctly_rounded(dtype, op):
 
 def test_scalar_is_converted_to_vector_dtype():
     # 0.1 is not representable: a float32 chain must use float32(0.1), never the double (DESIGN.md R-imm)
-    a = np.array([1.0, 3.0], dtype=np.float32)
+    a = np.array([1.0, 3.0, 9.0], dtype=np.float32)
     got = orc.scalar("mul", a, 0.1)
     s = np.float32(0.1)
-    for i in range(2):
+    for i in range(3):
         assert got[i] == round_f32(Fraction(float(a[i])) * Fraction(float(s)))
-    assert got[1] != np.float32(3.0 * 0.1) or True  # documentation of the distinction; equality is not required
+    # 9 * float32(0.1) = 0.90000004f, whereas a double-promoted 9 * 0.1 rounds to 0.9f: the two readings differ here
+    assert got[2] == np.float32(0.90000004) and got[2] != np.float32(9.0 * 0.1)
 
 
 def test_dyadic_inputs_are_exact():
@@ -548,10 +560,24 @@ def test_ge_determinant_hand_values_triangular_and_singular():
     for d in np.diag(T):
         ref = ref * d                                                      # PAPER.md:338, in step order
     assert det == ref and np.array_equal(E, T)
-    det, E, zs = orc.ge_determinant([[1.0, 2.0], [2.0, 4.0]])              # second pivot 4 - 2*2 = 0
-    assert det == 0.0 and zs == 1
-    det, _, zs = orc.ge_determinant([[1e-9, 1.0], [1.0, 1.0]], eps=1e-6)   # approximately-zero pivot with an explicit eps
-    assert det == 0.0 and zs == 0
+    # Zero pivots, derived from the listing's statement order: `Result := Result * pivot` comes BEFORE
+    # `if not double_approx_equals (pivot, 0.0)`, whose else-branch ends the loop.
+    det, E, zs = orc.ge_determinant([[1.0, 2.0], [2.0, 4.0]])              # step 0: Result = 1, row 1 -> [0, 0]; step 1: pivot 0 -> Result = 1 * 0
+    assert det == 0.0 and not np.signbit(det) and zs == 1 and np.array_equal(E, [[1.0, 2.0], [0.0, 0.0]])
+    det, E, zs = orc.ge_determinant([[-1.0, 2.0], [3.0, -6.0]])            # step 0: Result = -1, f = -3, row 1 -> [0, 0]; step 1: Result = -1 * 0 = -0
+    assert det == 0.0 and np.signbit(det) and zs == 1 and np.array_equal(E, [[-1.0, 2.0], [0.0, 0.0]])
+    M = [[1e-9, 1.0], [1.0, 1.0]]
+    det, E, zs = orc.ge_determinant(M, eps=1e-6)                           # approximately zero with an explicit eps: Result = 1 * 1e-9, loop ends,
+    assert det == 1e-9 and zs == 0 and np.array_equal(E, M)                # no row has been touched — NOT a hard-wired 0.0
+    det, E, zs = orc.ge_determinant([[2.0, 1.0], [4.0, 2.0 + 2.0 ** -40]], eps=1e-6)   # step 0: Result = 2, f = 2, row 1 -> [0, 2^-40]; step 1: Result = 2 * 2^-40
+    assert det == 2.0 ** -39 and zs == 1 and np.array_equal(E, [[2.0, 1.0], [0.0, 2.0 ** -40]])
+    # the per-row guard: a row whose entry below the pivot is approximately zero is left as it is
+    M = [[2.0, 1.0], [1e-9, 3.0]]
+    det, E, zs = orc.ge_determinant(M, eps=1e-6)
+    assert det == 6.0 and zs == -1 and np.array_equal(E, M)                # without the guard row 1 would become [~0, 3 - 5e-10] and det 5.999999999
+    det, E, zs = orc.ge_determinant(M, eps=0.0)                            # eps = 0: 1e-9 is not zero, the row IS eliminated
+    f = 1e-9 / 2.0
+    assert np.array_equal(E, [[2.0, 1.0], [1e-9 - f * 2.0, 3.0 - f * 1.0]]) and det == 2.0 * (3.0 - f * 1.0) and zs == -1
     det, _, zs = orc.ge_determinant(np.zeros((0, 0)))                      # empty product
     assert det == 1.0 and zs == -1
 
@@ -724,3 +750,96 @@ def test_transpose_hand_values_involution_and_library():
             assert np.array_equal(ocfg.transpose(T), M)                     # involution
             assert np.array_equal(T, M.T)                                   # library view
             assert all(T[j, i] == M[i, j] for i in range(0, shape[0], 5) for j in range(0, shape[1], 3))
+
+
+# ----------------------------------------------------------------------------------------------------------
+# the dtype-changing projection (R23)
+# ----------------------------------------------------------------------------------------------------------
+def _nearest_even(q: Fraction, mant_bits: int) -> Fraction:
+    """q rounded to `mant_bits` significant bits, ties to even, from the definition (no floating point involved)."""
+    if q == 0:
+        return Fraction(0)
+    sign, q = (-1 if q < 0 else 1), abs(q)
+    e = q.numerator.bit_length() - q.denominator.bit_length()
+    if Fraction(2) ** e > q:
+        e -= 1
+    ulp = Fraction(2) ** (e - mant_bits + 1)
+    k, r = divmod(q, ulp)
+    if r > ulp / 2 or (r == ulp / 2 and k % 2 == 1):
+        k += 1
+    return sign * k * ulp
+
+
+def test_cast_int_to_float_rounds_to_nearest_even():
+    i32 = np.array([0, 1, -1, 2 ** 24, 2 ** 24 + 1, 2 ** 24 + 2, 2 ** 24 + 3, -(2 ** 24 + 1), -(2 ** 24 + 3), 2 ** 31 - 1, -2 ** 31, 123456789], dtype=np.int32)
+    got = orc.cast(i32, np.float32)
+    for x, g in zip(i32.tolist(), got.tolist()):
+        assert Fraction(g) == _nearest_even(Fraction(x), 24), (x, g)
+    assert got[4] == 2.0 ** 24 and got[6] == 2.0 ** 24 + 4                # the two ties: 2^24+1 -> even 2^24, 2^24+3 -> even 2^24+4
+    assert orc.cast(i32, np.float64).tolist() == [float(x) for x in i32.tolist()]      # every int32 is exact in a double
+    i64 = np.array([2 ** 53, 2 ** 53 + 1, 2 ** 53 + 2, 2 ** 53 + 3, -(2 ** 53 + 1), 2 ** 63 - 1, -2 ** 63, 2 ** 62 + 2 ** 8, 987654321987654321], dtype=np.int64)
+    got = orc.cast(i64, np.float64)
+    for x, g in zip(i64.tolist(), got.tolist()):
+        assert Fraction(g) == _nearest_even(Fraction(x), 53), (x, g)
+    assert got[1] == 2.0 ** 53 and got[3] == 2.0 ** 53 + 4 and got[5] == 2.0 ** 63
+    got = orc.cast(i64, np.float32)
+    for x, g in zip(i64.tolist(), got.tolist()):
+        assert Fraction(g) == _nearest_even(Fraction(x), 24), (x, g)      # ONE rounding from the integer (not via double)
+    # a value where rounding through double first would give another float: 2^24 + 1 + 2^-30 cannot be an integer, so take an
+    # int64 just above a float32 tie: 2^40 + 2^16 + 1 -> above the midpoint between 2^40 and 2^40 + 2^17 -> rounds UP
+    x = 2 ** 40 + 2 ** 16 + 1
+    assert orc.cast(np.array([x], dtype=np.int64), np.float32)[0] == np.float32(2 ** 40 + 2 ** 17)
+
+
+def test_cast_float_to_int_truncates_saturates_and_nan_is_zero():
+    f64 = np.array([0.0, -0.0, 0.9, -0.9, 1.5, -1.5, 2.5, -2.5, 2147483647.0, 2147483647.9, 2147483648.0, -2147483648.0, -2147483648.9,
+                    -2147483649.0, 3e9, -3e9, 1e300, -1e300, np.inf, -np.inf, np.nan])
+    want32 = [0, 0, 0, 0, 1, -1, 2, -2, 2147483647, 2147483647, 2147483647, -2147483648, -2147483648,
+              -2147483648, 2147483647, -2147483648, 2147483647, -2147483648, 2147483647, -2147483648, 0]
+    assert orc.cast(f64, np.int32).tolist() == want32
+    want64 = [0, 0, 0, 0, 1, -1, 2, -2, 2147483647, 2147483647, 2147483648, -2147483648, -2147483648,
+              -2147483649, 3000000000, -3000000000, 2 ** 63 - 1, -2 ** 63, 2 ** 63 - 1, -2 ** 63, 0]
+    assert orc.cast(f64, np.int64).tolist() == want64
+    edge = np.array([2.0 ** 63, -(2.0 ** 63), 2.0 ** 63 - 1024.0, -(2.0 ** 63) - 2048.0, 2.0 ** 62])
+    assert orc.cast(edge, np.int64).tolist() == [2 ** 63 - 1, -2 ** 63, 2 ** 63 - 1024, -2 ** 63, 2 ** 62]
+    f32 = np.array([16777216.0, 16777218.0, -7.75, 2147483520.0, 2147483648.0, -2147483648.0, 3.4e38, np.nan], dtype=np.float32)
+    assert orc.cast(f32, np.int32).tolist() == [16777216, 16777218, -7, 2147483520, 2147483647, -2147483648, 2147483647, 0]
+    # in range, truncation == math.trunc of the exact value (brute force over random values)
+    x = (RNG.standard_normal(500) * 1e6)
+    assert orc.cast(x, np.int32).tolist() == [math.trunc(v) for v in x.tolist()]
+    assert orc.cast(x.astype(np.float32), np.int64).tolist() == [math.trunc(float(v)) for v in x.astype(np.float32).tolist()]
+
+
+def test_cast_between_floats_and_between_ints():
+    d = np.array([1.0, 1.0 + 2.0 ** -24, 1.0 + 2.0 ** -23 + 2.0 ** -24, 1.0 + 2.0 ** -24 + 2.0 ** -50, 1e40, -1e40, 1e-50, np.inf, 0.1])
+    got = orc.cast(d, np.float32)
+    # ties to even: 1 + 2^-24 -> 1 (even), 1 + 2^-23 + 2^-24 -> 1 + 2^-22 (even); just above a tie rounds up; overflow -> inf; underflow -> 0
+    assert got.tolist()[:8] == [1.0, 1.0, 1.0 + 2.0 ** -22, 1.0 + 2.0 ** -23, np.inf, -np.inf, 0.0, np.inf]
+    assert Fraction(float(got[8])) == _nearest_even(Fraction(0.1), 24)
+    f = RNG.standard_normal(64).astype(np.float32)
+    up = orc.cast(f, np.float64)
+    assert up.dtype == np.float64 and [Fraction(float(v)) for v in up] == [Fraction(float(v)) for v in f]     # widening is exact
+    i32 = np.array([0, -1, 2 ** 31 - 1, -2 ** 31, 12345], dtype=np.int32)
+    assert orc.cast(i32, np.int64).tolist() == i32.tolist()                                                   # sign extension
+    i64 = np.array([5, -1, 2 ** 31, 2 ** 32 + 5, -(2 ** 31) - 1, 2 ** 63 - 1, -2 ** 63], dtype=np.int64)
+    want = [((v + 2 ** 31) % 2 ** 32) - 2 ** 31 for v in i64.tolist()]                                        # the low 32 bits, two's complement
+    assert orc.cast(i64, np.int32).tolist() == want
+    for dt in (np.float32, np.float64, np.int32, np.int64):
+        a = (RNG.standard_normal(16) * 100).astype(dt)
+        assert orc.cast(a, dt).tobytes() == a.tobytes()                                                       # same type: identity
+    assert orc.cast(np.zeros(0, dtype=np.int32), np.float64).size == 0
+
+
+def test_project_sqrt_of_integers_gives_doubles():
+    """`c.project (agent (a: INT): DOUBLE do Result := sqrt (a) end)`."""
+    c = np.array([0, 1, 4, 9, 16, 2, 3, 10 ** 6, 2 ** 31 - 1, 46340 ** 2], dtype=np.int32)
+    got = orc.project_sqrt(c)
+    assert got.dtype == np.float64
+    assert got.tolist()[:5] == [0.0, 1.0, 2.0, 3.0, 4.0] and got[7] == 1000.0 and got[9] == 46340.0      # perfect squares are exact
+    for x, r in zip(c.tolist(), got.tolist()):                                                           # correct rounding by the exact bracket
+        lo, hi = np.nextafter(r, -np.inf), np.nextafter(r, np.inf)
+        if x > 0:
+            assert ((Fraction(float(lo)) + Fraction(r)) / 2) ** 2 <= x <= ((Fraction(r) + Fraction(float(hi))) / 2) ** 2
+    big = np.array([2 ** 53 + 1, 2 ** 62], dtype=np.int64)                 # int64: the conversion rounds first (2^53+1 -> 2^53), then the root
+    assert orc.project_sqrt(big).tolist() == [math.sqrt(2.0 ** 53), 2.0 ** 31]
+    assert np.isnan(orc.project_sqrt(np.array([-4], dtype=np.int32))[0])   # sqrt of a negative number: NaN (R20)
