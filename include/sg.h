@@ -18,7 +18,8 @@
  *    Shape / dtype / alias errors are raised at enqueue (they are the paper's scalar contracts);
  *    device-evaluated contracts and CUDA errors surface at sg_flush / sg_scalar_get.  A failed enqueue leaves
  *    the pending list unchanged.
- *  - One context per host thread; all GPU work is issued on the context's stream.
+ *  - One context per host thread; all GPU work is issued on the context's stream, on the context's device: every entry point
+ *    makes that device current for its own duration and restores the caller's current device before it returns.
  *  - Indices are 0-based; ranges are half-open [start, finish).
  *  - Arithmetic semantics (identical in the CPU oracle): one IEEE-754 rounding per primitive
  *    (no FMA contraction); immediates are converted to the collection's dtype at enqueue; integers wrap;
@@ -66,8 +67,10 @@ typedef enum {
     SG_NEG = 7, SG_ABS = 8,                                                              /* T   -> T   */
     SG_EQ = 9, SG_NE = 10, SG_LT = 11, SG_LE = 12, SG_GT = 13, SG_GE = 14,               /* T,T -> BOOL */
     SG_AND = 15, SG_OR = 16, SG_NOT = 17,                                                /* BOOL -> BOOL */
-    SG_SQRT = 19    /* F32/F64 -> same dtype: correctly rounded IEEE square root, the `project (agent sqrt)` of PAPER.md:171-175
-                       (sqrt(-0) = -0, sqrt(x < 0) = NaN); SG_ERR_DTYPE on integer or BOOL collections.  18 is reserved. */
+    SG_SQRT = 19    /* correctly rounded IEEE square root, the `project (agent sqrt)` of PAPER.md:171-175 (sqrt(-0) = -0,
+                       sqrt(x < 0) = NaN).  F32/F64 -> same dtype.  I32/I64 VECTOR -> F64, the paper's own example
+                       `agent (a: INT): DOUBLE do Result := sqrt (a) end`: the integers are converted (sg_cast) as they are loaded,
+                       in the same pass.  SG_ERR_DTYPE on BOOL.  18 is reserved. */
 } sg_op;
 
 typedef enum { SG_SUM = 0, SG_RMAX = 1, SG_RMIN = 2, SG_COUNT = 3 /* number of true in a BOOL collection */ } sg_red;
@@ -149,11 +152,23 @@ sg_status sg_mat_elem(sg_ctx* ctx, sg_handle m, int64_t i, int64_t j, sg_handle*
  * intermediate result"). */
 sg_status sg_enqueue(sg_ctx* ctx, sg_op op, const sg_operand* operands, int32_t n, sg_handle dst_or_0, sg_handle* out);
 
+/* project (transform: FUNCTION[T, U]): COLLECTION[U] with the value-preserving conversion as the transform:
+ * a deferred vector of dtype `to` whose element i is element i of v converted.  Integer -> float: round to nearest even.
+ * Float -> integer: truncation toward zero, saturating at the target's range, NaN -> 0 (R23).  F64 -> F32: round to
+ * nearest even; F32 -> F64 and I32 -> I64: exact; I64 -> I32: the low 32 bits (wrap).  The conversion costs no pass of its own:
+ * the operand is converted while it is loaded by the pass that consumes the result (a pending operand is stored first — a pass
+ * has one value type).  dst_or_0 as in sg_enqueue (dtype `to`).  Errors: SG_ERR_DTYPE (BOOL), SG_ERR_UNSUPPORTED (matrix,
+ * scalar or strided view). */
+sg_status sg_cast(sg_ctx* ctx, sg_handle v, sg_dtype to, sg_handle dst_or_0, sg_handle* out);
+
 /* Terminal reductions sum/max/min and COUNT, deferred: *out is a scalar handle; reading it is
  * the trigger, so several reductions and contracts of one chain share one pass (R7).
  * SG_AXIS_ROWS / SG_AXIS_COLS on a matrix give a vector handle of per-row / per-column results.
- * Result dtype: SUM -> F64 for float inputs, I64 for int inputs; RMAX/RMIN -> input dtype; COUNT -> I64. */
-sg_status sg_reduce(sg_ctx* ctx, sg_handle h, sg_red kind, sg_axis axis, sg_handle* out);
+ * acc: the accumulator = result dtype.  SG_ACC_DEFAULT, or exactly the dtype the semantics fix: SUM -> SG_F64 for float inputs
+ * (double-double / f64 accumulation), SG_I64 for int inputs (wrapping); RMAX/RMIN -> the input dtype; COUNT -> SG_I64.  Any other
+ * value is SG_ERR_DTYPE: a narrower accumulator could not meet the stated sum tolerances and is not emulated. */
+#define SG_ACC_DEFAULT (-1)
+sg_status sg_reduce(sg_ctx* ctx, sg_handle h, sg_red kind, int32_t acc, sg_axis axis, sg_handle* out);
 /* for_all / exists over a BOOL collection; *out is a BOOL scalar handle. */
 sg_status sg_forall(sg_ctx* ctx, sg_handle h_bool, sg_handle* out_bool);
 sg_status sg_exists(sg_ctx* ctx, sg_handle h_bool, sg_handle* out_bool);
@@ -172,9 +187,14 @@ sg_status sg_contract(sg_ctx* ctx, sg_handle h_bool_scalar, int32_t kind, const 
 
 /* update: plan + launch everything pending, asynchronously on the stream, then copy the
  * flush's scalar results to a pinned host mirror.  Returns SG_ERR_CONTRACT (after a stream sync) only if
- * contracts are registered. */
+ * contracts are registered.  Transactional: when the plan cannot be built (SG_ERR_UNSUPPORTED, SG_ERR_CAPACITY, SG_ERR_ALIAS,
+ * SG_ERR_OOM, ...) nothing has been launched, the error is returned and the pending list is DISCARDED — result handles of the
+ * discarded operations name no data (release them), in-place destinations keep their previous contents, and the context is
+ * ready for new work.  If a launch fails, the passes already queued count as executed and the rest is discarded. */
 sg_status sg_flush(sg_ctx* ctx);
-/* Trigger (1): flushes if s is pending, waits for the stream, copies the scalar (size of its dtype). */
+/* Trigger (1): flushes if s is pending, waits for the stream, copies the scalar (size of its dtype).
+ * SG_ERR_CONTRACT if s is a quantifier that was NOT EVALUATED: its pass ended early at a violated registered contract before s was
+ * decided (a for_all already false or an exists already true on the prefix read so far IS decided and readable). */
 sg_status sg_scalar_get(sg_ctx* ctx, sg_handle s, void* host_out, size_t bytes);
 sg_status sg_scalar_dtype(sg_ctx* ctx, sg_handle s, int32_t* dtype);
 /* Trigger (2): count / device pointer of a collection; flushes (and syncs, for a filter output) if pending. */
@@ -183,7 +203,8 @@ sg_status sg_vec_data(sg_ctx* ctx, sg_handle v, void** dev_ptr);
 /* to_array (PAPER.md:153-155, 195, 284 trigger (2)): flushes if pending, waits, copies the collection's elements
  * (count * element size bytes, contiguous) to HOST memory in one action.  bytes must be >= that size. */
 sg_status sg_vec_read(sg_ctx* ctx, sg_handle v, void* host_out, size_t bytes);
-/* Drop the caller's reference.  An unreferenced pending intermediate is never materialised. */
+/* Drop the caller's reference.  An unreferenced pending intermediate is never materialised.  A collection or scalar that a
+ * pending operation still reads may be released before the flush: its storage lives until that flush has consumed it. */
 sg_status sg_release(sg_ctx* ctx, sg_handle h);
 
 /* transpose: a NEW cols x rows matrix with out[j][i] = m[i][j] (F32/F64/I32/I64), written to dev_out_or_null
@@ -193,15 +214,23 @@ sg_status sg_release(sg_ctx* ctx, sg_handle h);
  * SG_ERR_DTYPE (BOOL), SG_ERR_ALIAS (dev_out overlaps m), SG_ERR_OOM, SG_ERR_CUDA. */
 sg_status sg_mat_transpose(sg_ctx* ctx, sg_handle m, void* dev_out_or_null, int64_t ld_out, sg_handle* out_mat);
 
-/* Listing 5's loop body for steps k in [k0, k1) of the square F64 matrix m, as a library composite over the
- * primitives above.  Step k: det <- det * M[k,k] and minpiv <- MIN(minpiv, ABS(M[k,k]))
- * on the one-element F64 vectors det / minpiv, then for ALL rows j > k in one matrix pass M[j,:] <- M[j,:] - (M[j,k]/M[k,k]) * M[k,:]
- * (BASELINE.json:configs[4]; the factors are read before the rows change).  The pivot stays on the device; every step is
- * flushed asynchronously and nothing is read back, so n steps run without a host synchronisation.  The caller initialises
- * det to 1 and minpiv to +inf and tests the zero-pivot condition of PAPER.md:339 on minpiv afterwards (sg_forall of minpiv > eps).
- * Errors: SG_ERR_ARG (handles, range), SG_ERR_SHAPE (not square, det/minpiv not one element), SG_ERR_DTYPE, SG_ERR_UNSUPPORTED
- * (rows not 16-byte aligned), SG_ERR_CUDA.  Operations already pending are flushed with step k0. */
-sg_status sg_mat_ge_steps(sg_ctx* ctx, sg_handle m, sg_handle det, sg_handle minpiv, int64_t k0, int64_t k1);
+/* Listing 5's loop for steps k in [k0, k1) of the square F64 matrix m (any size and leading dimension), run by
+ * ONE persistent kernel without the host in the loop (the paper's per-row launches are its slow case,
+ * PAPER.md:389).  det and minpiv are one-element F64 vectors with storage; the caller initialises det to 1 (`Result := 1`) and
+ * minpiv to +inf.  Step k, in the listing's statement order:
+ *     pivot := M[k,k];  det <- det * pivot;  minpiv <- MIN(minpiv, ABS(pivot));
+ *     if |pivot| <= eps (`double_approx_equals (pivot, 0.0)` with the explicit eps the paper leaves open): the loop
+ *         ENDS — no row is touched by this or any later step, det keeps the product including this pivot (a signed zero for
+ *         eps = 0), and a later call on the same det/minpiv does nothing (minpiv <= eps records the exit);
+ *     else for ALL rows j > k whose entry M[j,k] is not approximately zero:
+ *         M[j,:] <- M[j,:] - (M[j,k] / M[k,k]) * M[k,:]   (BASELINE.json:configs[4]'s update over all columns, one rounding per
+ *         primitive; the factor is read before the row changes).
+ * Not deferred: operations pending on the context are flushed first, then the kernel is enqueued on the stream (asynchronous,
+ * nothing is read back: n steps run without a host synchronisation).  The zero-pivot decision is taken on the device; the
+ * caller reads det and, if it wants the listing's `ok`, tests minpiv > eps.
+ * Errors: SG_ERR_ARG (handles, range, eps < 0 or NaN), SG_ERR_SHAPE (not square, det/minpiv not one element), SG_ERR_DTYPE,
+ * SG_ERR_CUDA. */
+sg_status sg_mat_ge_steps(sg_ctx* ctx, sg_handle m, sg_handle det, sg_handle minpiv, double eps, int64_t k0, int64_t k1);
 
 sg_status sg_plan_stats(sg_ctx* ctx, sg_stats* out);
 /* Canonical program of pass `pass` of the last flush as text (template generator, tests). Returns bytes needed. */

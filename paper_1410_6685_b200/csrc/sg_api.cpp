@@ -59,13 +59,16 @@ sg_status sg_ctx_create(sg_ctx** out, int device, void* cuda_stream, const sg_al
     c->slab_slots = 1 << 16;
     if (!c->plan_only) {
         // the product path has no CPU fallback: without a usable device every entry point fails loudly
-        cudaDeviceProp prop;
-        if (cudaSetDevice(device) != cudaSuccess || cudaGetDeviceProperties(&prop, device) != cudaSuccess) {
+        int prev = -1, sms = 0;
+        cudaGetDevice(&prev);
+        if (cudaSetDevice(device) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device) != cudaSuccess) {
             cudaGetLastError();
+            if (prev >= 0) cudaSetDevice(prev);
             delete c;
             return SG_ERR_CUDA;
         }
-        c->sm_count = prop.multiProcessorCount;
+        struct Restore { int d; ~Restore() { if (d >= 0) cudaSetDevice(d); } } restore{prev};   // the caller's current device is left as it was
+        c->sm_count = sms;
         c->ctrl_words = 1 << 14;
         bool ok = cudaMalloc((void**)&c->ctrl, sizeof(unsigned int) * c->ctrl_words) == cudaSuccess &&
                   cudaMemset(c->ctrl, 0, sizeof(unsigned int) * c->ctrl_words) == cudaSuccess &&
@@ -84,6 +87,7 @@ sg_status sg_ctx_create(sg_ctx** out, int device, void* cuda_stream, const sg_al
 }
 
 sg_status sg_ctx_destroy(sg_ctx* c) {
+    SgDeviceScope dev_scope(c);
     CK(c);
     if (!c->plan_only) {
         cudaStreamSynchronize(c->stream);
@@ -109,6 +113,7 @@ sg_status sg_ctx_destroy(sg_ctx* c) {
 sg_status sg_ctx_set_flags(sg_ctx* c, uint32_t flags) { CK(c); c->flags = flags; return SG_OK; }
 
 static sg_status make_collection(sg_ctx* c, int kind, sg_dtype dtype, int64_t rows, int64_t cols, int64_t ld, void* dev_ptr, sg_handle* out) {
+    SgDeviceScope dev_scope(c);
     CK(c && out);
     if (dtype < SG_F32 || dtype > SG_BOOL || rows < 0 || cols < 0 || ld < cols) return sg_fail(c, SG_ERR_ARG, "bad dtype or shape");
     Value v;
@@ -159,6 +164,7 @@ static sg_status resolve_count(sg_ctx* c, Value* v) {
 }
 
 sg_status sg_vec_subset(sg_ctx* c, sg_handle h, int64_t start, int64_t finish, sg_handle* out) {
+    SgDeviceScope dev_scope(c);
     CK(c && out);
     Value* v;
     sg_status s = need_storage(c, h, &v);
@@ -173,6 +179,7 @@ sg_status sg_vec_subset(sg_ctx* c, sg_handle h, int64_t start, int64_t finish, s
     return SG_OK;
 }
 sg_status sg_mat_row(sg_ctx* c, sg_handle m, int64_t i, sg_handle* out) {
+    SgDeviceScope dev_scope(c);
     CK(c && out);
     Value* v;
     sg_status s = need_storage(c, m, &v);
@@ -185,6 +192,7 @@ sg_status sg_mat_row(sg_ctx* c, sg_handle m, int64_t i, sg_handle* out) {
     return SG_OK;
 }
 sg_status sg_mat_rows(sg_ctx* c, sg_handle m, int64_t r0, int64_t r1, sg_handle* out) {
+    SgDeviceScope dev_scope(c);
     CK(c && out);
     Value* v;
     sg_status s = need_storage(c, m, &v);
@@ -197,6 +205,7 @@ sg_status sg_mat_rows(sg_ctx* c, sg_handle m, int64_t r0, int64_t r1, sg_handle*
     return SG_OK;
 }
 sg_status sg_mat_elem(sg_ctx* c, sg_handle m, int64_t i, int64_t j, sg_handle* out) {
+    SgDeviceScope dev_scope(c);
     CK(c && out);
     Value* v;
     sg_status s = need_storage(c, m, &v);
@@ -237,9 +246,9 @@ static sg_status operand_value(sg_ctx* c, sg_handle h, Value** out) {
 }
 
 static sg_status append_map(sg_ctx* c, uint8_t op, int n_opd, const Operand* opd, int opd_dtype, bool is2d, int64_t rows, int64_t cols,
-                            sg_handle dst, sg_handle* out) {
+                            sg_handle dst, sg_handle* out, int src_dtype = -1) {
     Node nd;
-    nd.kind = NK_MAP; nd.op = op; nd.n_opd = n_opd;
+    nd.kind = NK_MAP; nd.op = op; nd.n_opd = n_opd; nd.src_dtype = src_dtype;
     for (int i = 0; i < n_opd; ++i) nd.opd[i] = opd[i];
     nd.dtype = opd_dtype; nd.is2d = is2d; nd.rows = rows; nd.cols = cols;
     const bool to_bool = (op >= OP_EQ && op <= OP_NOT);
@@ -286,8 +295,40 @@ static sg_status append_map(sg_ctx* c, uint8_t op, int n_opd, const Operand* opd
     return SG_OK;
 }
 
+// The dtype-changing projection: element i of the result is element i of v converted to `to`.
+sg_status sg_cast(sg_ctx* c, sg_handle h, sg_dtype to, sg_handle dst, sg_handle* out) {
+    SgDeviceScope dev_scope(c);
+    CK(c && out);
+    Value* v;
+    sg_status s = operand_value(c, h, &v);
+    if (s != SG_OK) return s;
+    if (v->kind != VK_VEC) return sg_fail(c, SG_ERR_UNSUPPORTED, "sg_cast needs a vector");
+    if (v->dtype == SG_BOOL || to < SG_F32 || to > SG_I64) return sg_fail(c, SG_ERR_DTYPE, "sg_cast converts between F32, F64, I32 and I64");
+    Operand opd[2];
+    opd[0].kind = OPD_VALUE; opd[0].value = (int)h - 1; opd[1] = opd[0];
+    if ((int)to == v->dtype) return append_map(c, OP_MOV, 1, opd, v->dtype, false, 1, v->cols, dst, out);     // same type: a copy
+    if (v->stride != 1) return sg_fail(c, SG_ERR_UNSUPPORTED, "sg_cast of a strided view");
+    return append_map(c, NODE_OP_CAST, 1, opd, (int)to, false, 1, v->cols, dst, out, v->dtype);
+}
+
 sg_status sg_enqueue(sg_ctx* c, sg_op op, const sg_operand* ops, int32_t n, sg_handle dst, sg_handle* out) {
+    SgDeviceScope dev_scope(c);
     CK(c && ops && out);
+    // `c.project (agent (a: INT): DOUBLE do Result := sqrt (a) end)`: the square root of an INTEGER vector is
+    // a DOUBLE collection — the conversion happens as the integers are loaded, in the same pass as the square root (R20)
+    if (op == SG_SQRT && n == 1 && ops[0].kind == SG_OPERAND_HANDLE) {
+        Value* iv = val(c, ops[0].h);
+        if (iv && iv->kind == VK_VEC && (iv->dtype == SG_I32 || iv->dtype == SG_I64)) {
+            sg_handle as_f64 = 0;
+            sg_status s = sg_cast(c, ops[0].h, SG_F64, 0, &as_f64);
+            if (s != SG_OK) return s;
+            sg_operand o = ops[0];
+            o.h = as_f64;
+            s = sg_enqueue(c, SG_SQRT, &o, 1, dst, out);
+            sg_release(c, as_f64);              // anonymous intermediate: never stored
+            return s;
+        }
+    }
     if (op < SG_ADD || (op > SG_NOT && op != SG_SQRT)) return sg_fail(c, SG_ERR_ARG, "unknown op");
     const bool unary = (op == SG_NEG || op == SG_ABS || op == SG_NOT || op == SG_SQRT);
     if (n != (unary ? 1 : 2)) return sg_fail(c, SG_ERR_ARG, "wrong operand count");
@@ -305,7 +346,7 @@ sg_status sg_enqueue(sg_ctx* c, sg_op op, const sg_operand* ops, int32_t n, sg_h
     if (dtype < 0) return sg_fail(c, SG_ERR_ARG, "at least one operand must be a collection");
     if (logic != (dtype == SG_BOOL)) return sg_fail(c, SG_ERR_DTYPE, logic ? "logical ops need BOOL operands" : "arithmetic on BOOL");
     if (op == SG_MOD && (dtype == SG_F32 || dtype == SG_F64)) return sg_fail(c, SG_ERR_DTYPE, "MOD needs an integer dtype");
-    if (op == SG_SQRT && dtype != SG_F32 && dtype != SG_F64) return sg_fail(c, SG_ERR_DTYPE, "SQRT needs a float dtype");
+    if (op == SG_SQRT && dtype != SG_F32 && dtype != SG_F64) return sg_fail(c, SG_ERR_DTYPE, "SQRT needs a float collection or an integer vector");
     // iteration domain: a matrix operand fixes a 2-D domain; vectors may broadcast along it
     bool is2d = false; int64_t rows = 1, cols = -1; bool have_coll = false;
     for (int i = 0; i < n; ++i)
@@ -353,6 +394,7 @@ sg_status sg_enqueue(sg_ctx* c, sg_op op, const sg_operand* ops, int32_t n, sg_h
 }
 
 sg_status sg_mat_transpose(sg_ctx* c, sg_handle m, void* dev_out, int64_t ld_out, sg_handle* out) {
+    SgDeviceScope dev_scope(c);
     CK(c && out);
     Value* v;
     sg_status s;
@@ -388,6 +430,7 @@ sg_status sg_mat_transpose(sg_ctx* c, sg_handle m, void* dev_out, int64_t ld_out
 }
 
 sg_status sg_mat_col(sg_ctx* c, sg_handle m, int64_t j, int64_t r0, int64_t r1, sg_handle* out) {
+    SgDeviceScope dev_scope(c);
     CK(c && out);
     Value* v;
     sg_status s = need_storage(c, m, &v);
@@ -435,12 +478,17 @@ static sg_status append_reduce(sg_ctx* c, uint8_t kind, sg_handle h, int axis, i
     return SG_OK;
 }
 
-sg_status sg_reduce(sg_ctx* c, sg_handle h, sg_red kind, sg_axis axis, sg_handle* out) {
+sg_status sg_reduce(sg_ctx* c, sg_handle h, sg_red kind, int32_t acc, sg_axis axis, sg_handle* out) {
+    SgDeviceScope dev_scope(c);
     CK(c && out);
     Value* v = val(c, h);
     if (!v) return sg_fail(c, SG_ERR_ARG, "unknown handle");
     if (axis < SG_AXIS_ALL || axis > SG_AXIS_COLS) return sg_fail(c, SG_ERR_ARG, "bad axis");
     const bool is_f = v->dtype == SG_F32 || v->dtype == SG_F64;
+    // accumulator / result dtype: SG_ACC_DEFAULT or exactly the one the semantics fix (include/sg.h); a narrower accumulator
+    // could not meet the sum tolerances stated against the long-double oracle (R1), so it is rejected, not emulated
+    const int natural = (kind == SG_SUM) ? (is_f ? SG_F64 : SG_I64) : (kind == SG_COUNT) ? SG_I64 : v->dtype;
+    if (acc != SG_ACC_DEFAULT && acc != natural) return sg_fail(c, SG_ERR_DTYPE, "unsupported accumulator dtype for this reduction");
     switch (kind) {
         case SG_SUM:
             if (v->dtype == SG_BOOL) return sg_fail(c, SG_ERR_DTYPE, "SUM of BOOL: use COUNT");
@@ -455,6 +503,7 @@ sg_status sg_reduce(sg_ctx* c, sg_handle h, sg_red kind, sg_axis axis, sg_handle
     }
 }
 static sg_status quantifier(sg_ctx* c, uint8_t kind, sg_handle h, sg_handle* out) {
+    SgDeviceScope dev_scope(c);
     CK(c && out);
     Value* v = val(c, h);
     if (!v) return sg_fail(c, SG_ERR_ARG, "unknown handle");
@@ -465,6 +514,7 @@ sg_status sg_forall(sg_ctx* c, sg_handle h, sg_handle* out) { return quantifier(
 sg_status sg_exists(sg_ctx* c, sg_handle h, sg_handle* out) { return quantifier(c, OUT_ANY, h, out); }
 
 sg_status sg_forall_adjacent(sg_ctx* c, sg_handle h, sg_op cmp, sg_handle* out) {
+    SgDeviceScope dev_scope(c);
     CK(c && out);
     if (cmp < SG_EQ || cmp > SG_GE) return sg_fail(c, SG_ERR_ARG, "adjacent predicate needs a comparison");
     Value* v;
@@ -485,6 +535,7 @@ sg_status sg_forall_adjacent(sg_ctx* c, sg_handle h, sg_op cmp, sg_handle* out) 
 }
 
 sg_status sg_filter(sg_ctx* c, sg_handle values, sg_handle mask, void* dev_out, int64_t capacity, sg_handle* out_vec, sg_handle* out_count) {
+    SgDeviceScope dev_scope(c);
     CK(c && out_vec && out_count);
     Value *v, *m;
     sg_status s = operand_value(c, values, &v);
@@ -525,48 +576,38 @@ sg_status sg_contract(sg_ctx* c, sg_handle h, int32_t kind, const char* tag) {
     return SG_OK;
 }
 
-sg_status sg_flush(sg_ctx* c) { CK(c); return sg_flush_impl(c); }
-
-// Listing 5's loop body as a composite over the public primitives (no kernel of its own): the native twin of
-// workloads.ge_step + flush, so that a step costs microseconds of host time instead of a scripting language's call overhead.
-sg_status sg_mat_ge_steps(sg_ctx* c, sg_handle m, sg_handle det, sg_handle minpiv, int64_t k0, int64_t k1) {
+sg_status sg_flush(sg_ctx* c) {
     CK(c);
+    SgDeviceScope dev_scope(c);
+    return sg_flush_impl(c);
+}
+
+// Listing 5's whole loop for steps [k0, k1): one persistent cooperative kernel (sg_ge.cu), no host in the loop.
+sg_status sg_mat_ge_steps(sg_ctx* c, sg_handle m, sg_handle det, sg_handle minpiv, double eps, int64_t k0, int64_t k1) {
+    CK(c);
+    SgDeviceScope dev_scope(c);
+    sg_status s;
+    // like sg_mat_transpose, the kernel is not part of the pending list: everything pending runs first (trigger (2))
+    if (!c->nodes.empty() && (s = sg_flush_impl(c)) != SG_OK) return s;
     Value* vm = val(c, m);
     Value* vd = val(c, det);
     Value* vp = val(c, minpiv);
     if (!vm || !vd || !vp) return sg_fail(c, SG_ERR_ARG, "unknown handle");
+    if (vm->kind != VK_MAT || !vm->materialised || !vd->materialised || !vp->materialised) return sg_fail(c, SG_ERR_ARG, "sg_mat_ge_steps: a matrix and two vectors with storage");
     if (vm->dtype != SG_F64 || vd->dtype != SG_F64 || vp->dtype != SG_F64) return sg_fail(c, SG_ERR_DTYPE, "sg_mat_ge_steps: F64 only");
     if (vm->rows != vm->cols) return sg_fail(c, SG_ERR_SHAPE, "sg_mat_ge_steps: square matrix expected");
     if (vd->rows * vd->cols != 1 || vp->rows * vp->cols != 1) return sg_fail(c, SG_ERR_SHAPE, "sg_mat_ge_steps: det and minpiv are one-element vectors");
     const int64_t n = vm->rows;
     if (k0 < 0 || k1 > n || k0 > k1) return sg_fail(c, SG_ERR_ARG, "sg_mat_ge_steps: step range");
-    auto H = [](sg_handle h, int32_t bcast) { sg_operand o; memset(&o, 0, sizeof o); o.kind = SG_OPERAND_HANDLE; o.bcast = bcast; o.h = h; return o; };
-    for (int64_t k = k0; k < k1; ++k) {
-        sg_handle tmp[8];
-        int nt = 0;
-        sg_status s = SG_OK;
-        sg_handle rowk = 0, d = 0, ad = 0, out = 0;
-#define SG_TRY(call) do { if (s == SG_OK) s = (call); } while (0)
-        SG_TRY(sg_mat_row(c, m, k, &rowk));                 if (s == SG_OK) tmp[nt++] = rowk;
-        SG_TRY(sg_vec_subset(c, rowk, k, k + 1, &d));       if (s == SG_OK) tmp[nt++] = d;
-        { sg_operand o[2] = {H(det, SG_BCAST_NONE), H(d, SG_BCAST_NONE)}; SG_TRY(sg_enqueue(c, SG_MUL, o, 2, det, &out)); }
-        { sg_operand o[1] = {H(d, SG_BCAST_NONE)}; SG_TRY(sg_enqueue(c, SG_ABS, o, 1, 0, &ad)); if (s == SG_OK) tmp[nt++] = ad; }
-        { sg_operand o[2] = {H(minpiv, SG_BCAST_NONE), H(ad, SG_BCAST_NONE)}; SG_TRY(sg_enqueue(c, SG_MIN, o, 2, minpiv, &out)); }
-        if (k + 1 < n) {
-            sg_handle piv = 0, col = 0, f = 0, sub = 0, t = 0;
-            SG_TRY(sg_mat_elem(c, m, k, k, &piv));              if (s == SG_OK) tmp[nt++] = piv;
-            SG_TRY(sg_mat_col(c, m, k, k + 1, n, &col));        if (s == SG_OK) tmp[nt++] = col;
-            { sg_operand o[2] = {H(col, SG_BCAST_NONE), H(piv, SG_BCAST_NONE)}; SG_TRY(sg_enqueue(c, SG_DIV, o, 2, 0, &f)); if (s == SG_OK) tmp[nt++] = f; }
-            SG_TRY(sg_mat_rows(c, m, k + 1, n, &sub));          if (s == SG_OK) tmp[nt++] = sub;
-            { sg_operand o[2] = {H(f, SG_BCAST_COL), H(rowk, SG_BCAST_ROW)}; SG_TRY(sg_enqueue(c, SG_MUL, o, 2, 0, &t)); if (s == SG_OK) tmp[nt++] = t; }
-            { sg_operand o[2] = {H(sub, SG_BCAST_NONE), H(t, SG_BCAST_NONE)}; SG_TRY(sg_enqueue(c, SG_SUB, o, 2, sub, &out)); }
-        }
-#undef SG_TRY
-        for (int i = nt - 1; i >= 0; --i) sg_release(c, tmp[i]);
-        if (s != SG_OK) return s;
-        s = sg_flush_impl(c);
-        if (s != SG_OK) return s;
-    }
+    if (!(eps >= 0.0)) return sg_fail(c, SG_ERR_ARG, "sg_mat_ge_steps: eps must be >= 0");
+    if (k0 == k1) return SG_OK;
+    if (c->plan_only) { c->stats.launches_total++; return SG_OK; }
+    unsigned int* ready = c->ctrl + 4;          // control words 4..7 are not used by the pass kernels
+    if (cudaMemsetAsync(ready, 0, sizeof(unsigned int), c->stream) != cudaSuccess) return sg_fail(c, SG_ERR_CUDA, cudaGetErrorString(cudaGetLastError()));
+    int grid = 0;
+    const cudaError_t e = sgk_ge_loop((double*)vm->ptr, n, vm->ld, (double*)vd->ptr, (double*)vp->ptr, eps, k0, k1, ready, c->sm_count, c->stream, &grid);
+    if (e != cudaSuccess) { cudaGetLastError(); return sg_fail(c, SG_ERR_CUDA, std::string("determinant loop launch failed: ") + cudaGetErrorString(e)); }
+    c->stats.launches_total++;
     return SG_OK;
 }
 
@@ -579,6 +620,7 @@ sg_status sg_scalar_dtype(sg_ctx* c, sg_handle h, int32_t* dtype) {
 }
 
 sg_status sg_scalar_get(sg_ctx* c, sg_handle h, void* host_out, size_t bytes) {
+    SgDeviceScope dev_scope(c);
     CK(c && host_out);
     Value* v = val(c, h);
     if (!v || v->kind != VK_SCALAR) return sg_fail(c, SG_ERR_ARG, "not a scalar handle");
@@ -587,6 +629,7 @@ sg_status sg_scalar_get(sg_ctx* c, sg_handle h, void* host_out, size_t bytes) {
         if (s != SG_OK && s != SG_ERR_CONTRACT) return s;
         v = val(c, h);
     }
+    if (v->undecided) return sg_fail(c, SG_ERR_CONTRACT, "quantifier not evaluated: its pass ended early at a violated contract");
     const size_t sz = dtype_size(v->dtype);
     if (bytes < sz) return sg_fail(c, SG_ERR_ARG, "host buffer too small");
     if (c->plan_only) { memset(host_out, 0, sz); return SG_OK; }
@@ -602,6 +645,7 @@ sg_status sg_scalar_get(sg_ctx* c, sg_handle h, void* host_out, size_t bytes) {
 }
 
 sg_status sg_vec_count(sg_ctx* c, sg_handle h, int64_t* n) {
+    SgDeviceScope dev_scope(c);
     CK(c && n);
     Value* v = val(c, h);
     if (!v) return sg_fail(c, SG_ERR_ARG, "unknown handle");
@@ -615,6 +659,7 @@ sg_status sg_vec_count(sg_ctx* c, sg_handle h, int64_t* n) {
 }
 
 sg_status sg_vec_data(sg_ctx* c, sg_handle h, void** dev_ptr) {
+    SgDeviceScope dev_scope(c);
     CK(c && dev_ptr);
     Value* v = val(c, h);
     if (!v) return sg_fail(c, SG_ERR_ARG, "unknown handle");
@@ -625,6 +670,7 @@ sg_status sg_vec_data(sg_ctx* c, sg_handle h, void** dev_ptr) {
 }
 
 sg_status sg_vec_read(sg_ctx* c, sg_handle h, void* host_out, size_t bytes) {
+    SgDeviceScope dev_scope(c);
     CK(c && host_out);
     void* p = nullptr;
     sg_status s = sg_vec_data(c, h, &p);
@@ -646,15 +692,18 @@ sg_status sg_release(sg_ctx* c, sg_handle h) {
     Value* v = val(c, h);
     if (!v) return sg_fail(c, SG_ERR_ARG, "unknown handle");
     if (v->user_refs > 0) v->user_refs--;
-    if (v->user_refs == 0 && v->node < 0) {      // nothing pending produces it: storage can go now
-        if (v->owned && v->ptr) { c->deferred_free.push_back(v->ptr); v->ptr = nullptr; v->owned = false; }
-        if (v->slot >= 0 && v->kind == VK_SCALAR) { c->slab_free.push_back(v->slot); v->slot = -1; }
-        bool referenced = false;
+    if (v->user_refs == 0 && v->node < 0) {      // nothing pending produces it
+        // ... but a pending operation may still READ it (y = x + 1; release(x); flush): then only the reference goes now, the
+        // flush that consumes the readers gives the storage and the scalar slot back (retire_nodes frees unreferenced values)
         for (auto& n : c->nodes)
             if (!n.done)
                 for (int i = 0; i < n.n_opd; ++i)
-                    if (n.opd[i].kind != OPD_IMM && n.opd[i].value == (int)h - 1) referenced = true;
-        if (!referenced) v->alive = false;
+                    if (n.opd[i].kind != OPD_IMM && n.opd[i].value == (int)h - 1) return SG_OK;
+        for (auto& k : c->contracts)
+            if (k.value == (int)h - 1) return SG_OK;
+        if (v->owned && v->ptr) { c->deferred_free.push_back(v->ptr); v->ptr = nullptr; v->owned = false; }
+        if (v->slot >= 0 && v->kind == VK_SCALAR) { c->slab_free.push_back(v->slot); v->slot = -1; }
+        v->alive = false;
     }
     return SG_OK;
 }

@@ -55,8 +55,8 @@ const char* op_name(uint8_t op) {
     return op < OP_COUNT_ ? n[op] : "?";
 }
 const char* in_name(uint8_t k) {
-    static const char* n[] = {"IN_VEC", "IN_SHIFT", "IN_STRIDED", "IN_SCALAR", "IN_IMM", "IN_ROWB", "IN_COLB", "IN_BOOLVEC"};
-    return k < 8 ? n[k] : "?";
+    static const char* n[] = {"IN_VEC", "IN_SHIFT", "IN_STRIDED", "IN_SCALAR", "IN_IMM", "IN_ROWB", "IN_COLB", "IN_BOOLVEC", "IN_VEC_CVT"};
+    return k < 9 ? n[k] : "?";
 }
 const char* out_name(uint8_t k) {
     static const char* n[] = {"OUT_STORE", "OUT_STORE_BOOL", "OUT_SUM", "OUT_MAX", "OUT_MIN", "OUT_ALL", "OUT_ANY", "OUT_COUNT", "OUT_FILTER"};
@@ -182,6 +182,8 @@ sg_status sg_build_pass(sg_ctx* c, Pass& P, std::vector<char*>& temps, std::stri
         if (v.kind == VK_SCALAR && v.slot >= 0) ptr = c->slab + 8 * v.slot;
         if (!ptr) return sg_fail(c, SG_ERR_ARG, "operand has no storage");
         auto& m = want_pred ? B.preg_of : B.vreg_of;
+        // register cache key: the value, its shifted form, or its converted form (a conversion never shares a register with the raw value:
+        // they live in passes of different dtypes anyway)
         const int key = o.kind == OPD_SHIFT ? -2 - o.value : o.value;
         auto it = m.find(key);
         if (it != m.end()) { *reg = it->second; return SG_OK; }
@@ -189,6 +191,12 @@ sg_status sg_build_pass(sg_ctx* c, Pass& P, std::vector<char*>& temps, std::stri
         if (v.kind == VK_SCALAR) {
             if (want_pred) return sg_fail(c, SG_ERR_UNSUPPORTED, "BOOL scalar operand");
             k = B.add_input(IN_SCALAR, ptr, 0, 0, -1, false, &fresh);
+        } else if (X.kind == NK_MAP && X.op == NODE_OP_CAST) {
+            // dtype-changing projection: the operand is converted to the pass dtype as it is loaded
+            if (P.is2d || v.kind != VK_VEC || v.stride != 1) return sg_fail(c, SG_ERR_UNSUPPORTED, "dtype conversion of a matrix or strided view");
+            k = B.add_input(IN_VEC_CVT, ptr, 1, 0, -1, false, &fresh);
+            if (fresh) { P.n_mem_in++; P.bytes += v.cols * dtype_size(v.dtype); B.inputs[k].src_dtype = (uint8_t)v.dtype; }
+            fresh = false;
         } else if (o.kind == OPD_SHIFT) {
             int base = B.add_input(IN_VEC, ptr, v.stride, 0, -1, false, &fresh);
             if (fresh) { P.n_mem_in++; P.bytes += v.cols * es; }
@@ -261,7 +269,8 @@ sg_status sg_build_pass(sg_ctx* c, Pass& P, std::vector<char*>& temps, std::stri
             const bool to_pred = X.op >= OP_EQ && X.op <= OP_NOT;
             const int d = to_pred ? B.alloc_p() : B.alloc_v();
             (to_pred ? B.preg_of : B.vreg_of)[X.out] = d;
-            g.code[n_instr++] = {X.op, (uint8_t)d, (uint8_t)r[0], (uint8_t)(X.n_opd > 1 ? r[1] : r[0])};
+            const uint8_t opc = X.op == NODE_OP_CAST ? (uint8_t)OP_MOV : X.op;
+            g.code[n_instr++] = {opc, (uint8_t)d, (uint8_t)r[0], (uint8_t)(X.n_opd > 1 ? r[1] : r[0])};
             if (stored(X)) {
                 if (n_out >= SG_MAX_OUT) return sg_fail(c, SG_ERR_CAPACITY, "too many outputs in one pass");
                 Value& ov = V[X.out];
@@ -269,7 +278,7 @@ sg_status sg_build_pass(sg_ctx* c, Pass& P, std::vector<char*>& temps, std::stri
                 if (!ov.ptr) {
                     ov.ptr = (char*)sg_dev_alloc(c, (size_t)(ov.rows * ov.cols * oes));
                     if (!ov.ptr) return sg_fail(c, SG_ERR_OOM, "device allocation failed");
-                    ov.owned = true; ov.ld = ov.cols; ov.stride = 1;
+                    ov.owned = true; ov.fresh_alloc = true; ov.ld = ov.cols; ov.stride = 1;
                 }
                 ov.materialised = true;
                 g.out[n_out] = {(uint8_t)(to_pred ? OUT_STORE_BOOL : OUT_STORE), (uint8_t)d, SG_NO_PRED, AXIS_ALL};
@@ -289,7 +298,7 @@ sg_status sg_build_pass(sg_ctx* c, Pass& P, std::vector<char*>& temps, std::stri
                 if (!ov.ptr) {
                     ov.ptr = (char*)sg_dev_alloc(c, (size_t)(ov.cols * oes));
                     if (!ov.ptr) return sg_fail(c, SG_ERR_OOM, "device allocation failed");
-                    ov.owned = true;
+                    ov.owned = true; ov.fresh_alloc = true;
                 }
                 ov.materialised = true;
                 a.out_ptr[n_out] = ov.ptr;
@@ -307,7 +316,7 @@ sg_status sg_build_pass(sg_ctx* c, Pass& P, std::vector<char*>& temps, std::stri
             if (!ov.ptr) {
                 ov.ptr = (char*)sg_dev_alloc(c, (size_t)(ov.cols * es));
                 if (!ov.ptr) return sg_fail(c, SG_ERR_OOM, "device allocation failed");
-                ov.owned = true;
+                ov.owned = true; ov.fresh_alloc = true;
             }
             ov.materialised = true;
             filter_regs[X.out] = {r[0], r[1]};
@@ -326,7 +335,7 @@ sg_status sg_build_pass(sg_ctx* c, Pass& P, std::vector<char*>& temps, std::stri
     for (size_t k = 0; k < B.inputs.size(); ++k) {
         const PassInput& in = B.inputs[k];
         g.in[k].kind = in.kind;
-        g.in[k].ref = in.kind == IN_SHIFT ? (uint8_t)in.value : 0;
+        g.in[k].ref = in.kind == IN_SHIFT ? (uint8_t)in.value : in.kind == IN_VEC_CVT ? in.src_dtype : 0;
         g.in[k].reg = (uint8_t)in.reg;
         a.in_ptr[k] = in.ptr;
         a.in_stride[k] = in.stride;

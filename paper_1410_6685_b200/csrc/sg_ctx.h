@@ -18,6 +18,9 @@
 
 enum ValueKind { VK_VEC = 0, VK_MAT = 1, VK_SCALAR = 2 };
 enum NodeKind { NK_MAP = 0, NK_REDUCE = 1, NK_FILTER = 2 };
+// node-level opcode of the dtype conversion (sg_cast): never part of a program — the plan builder lowers it to an IN_VEC_CVT
+// input (conversion at load) followed by OP_MOV
+constexpr uint8_t NODE_OP_CAST = 0x40;
 enum OperandKind { OPD_VALUE = 0, OPD_IMM = 1, OPD_SHIFT = 2 /* value shifted by +1 element */ };
 
 struct Value {
@@ -35,6 +38,8 @@ struct Value {
     bool count_known = true;
     int64_t slot = -1;              // VK_SCALAR produced by a reduction: slot in the scalar slab
     bool alive = true;
+    bool fresh_alloc = false;       // storage allocated by the flush in progress (given back if that flush fails before it runs)
+    bool undecided = false;         // quantifier whose pass ended early at a violated contract before it was decided: reading it is an error
 };
 
 struct Operand {
@@ -53,6 +58,7 @@ struct Node {
     int out2 = -1;                  // NK_FILTER: the count scalar
     int axis = AXIS_ALL;
     int dtype = SG_F32;             // operand dtype (V file) — SG_BOOL for pure logic nodes
+    int src_dtype = -1;             // OP_CAST: element type of the operand in memory (converted to `dtype` as it is loaded)
     bool is2d = false;
     int64_t rows = 1, cols = 0;     // iteration domain
     bool inplace = false;           // out's storage was given by the caller (dst_or_0)
@@ -63,9 +69,11 @@ struct Node {
 
 struct Contract { int value; int kind; std::string tag; };
 
-struct MemRange { const char* lo; const char* hi; const char* ptr; int64_t stride, ld, rows, cols; };
+// `exact`: the pass reads element i of the range for element i of its domain (an index-for-index read).  Shifted (neighbour),
+// broadcast and scalar reads are not: an in-place writer of the same storage can never share their pass.
+struct MemRange { const char* lo; const char* hi; const char* ptr; int64_t stride, ld, rows, cols; bool exact; };
 
-struct PassInput { uint8_t kind; const char* ptr; int64_t stride; uint64_t imm; int reg; int value; bool boolvec; int64_t len; };
+struct PassInput { uint8_t kind; const char* ptr; int64_t stride; uint64_t imm; int reg; int value; bool boolvec; int64_t len; uint8_t src_dtype; };
 
 struct Pass {
     bool is2d = false, has_filter = false, has_store = false;
@@ -120,6 +128,21 @@ struct sg_ctx {
     sg_stats stats{};
     std::vector<SgProg> dumps;      // canonical programs of the last flush; sg_plan_dump renders them as text on demand
     std::vector<char*> deferred_free;
+};
+
+// Makes the context's device current for the duration of one entry point and restores the caller's device afterwards
+// (a process may hold contexts on several GPUs; no entry point changes the caller's current device).
+struct SgDeviceScope {
+    int prev = -1;
+    bool switched = false;
+    explicit SgDeviceScope(const sg_ctx* c) {
+        if (!c || c->plan_only) return;
+        if (cudaGetDevice(&prev) != cudaSuccess) { cudaGetLastError(); prev = -1; return; }
+        if (prev != c->device) switched = cudaSetDevice(c->device) == cudaSuccess;
+    }
+    ~SgDeviceScope() { if (switched && prev >= 0) cudaSetDevice(prev); }
+    SgDeviceScope(const SgDeviceScope&) = delete;
+    SgDeviceScope& operator=(const SgDeviceScope&) = delete;
 };
 
 // sg_plan.cpp

@@ -83,6 +83,37 @@ __device__ __forceinline__ double p_sqrt(double a) { return __dsqrt_rn(a); }
 __device__ __forceinline__ int32_t p_sqrt(int32_t a) { return a; }
 __device__ __forceinline__ long long p_sqrt(long long a) { return a; }
 
+// dtype conversion of the dtype-changing projection (sg_cast; R23): integer -> float rounds to
+// nearest even; float -> integer truncates toward zero, saturates at the target's range and maps NaN to 0 (the NaN case is
+// written out: the 64-bit hardware conversion returns INT64_MIN for it); F64 -> F32 rounds to nearest even; I64 -> I32 keeps
+// the low 32 bits.
+template <class T, class S> __device__ __forceinline__ T cvt_elem(S x);
+template <> __device__ __forceinline__ float cvt_elem<float, float>(float x) { return x; }
+template <> __device__ __forceinline__ double cvt_elem<double, double>(double x) { return x; }
+template <> __device__ __forceinline__ int32_t cvt_elem<int32_t, int32_t>(int32_t x) { return x; }
+template <> __device__ __forceinline__ long long cvt_elem<long long, long long>(long long x) { return x; }
+template <> __device__ __forceinline__ float cvt_elem<float, double>(double x) { return __double2float_rn(x); }
+template <> __device__ __forceinline__ float cvt_elem<float, int32_t>(int32_t x) { return __int2float_rn(x); }
+template <> __device__ __forceinline__ float cvt_elem<float, long long>(long long x) { return __ll2float_rn(x); }
+template <> __device__ __forceinline__ double cvt_elem<double, float>(float x) { return (double)x; }
+template <> __device__ __forceinline__ double cvt_elem<double, int32_t>(int32_t x) { return __int2double_rn(x); }
+template <> __device__ __forceinline__ double cvt_elem<double, long long>(long long x) { return __ll2double_rn(x); }
+template <> __device__ __forceinline__ int32_t cvt_elem<int32_t, float>(float x) { return (x != x) ? 0 : __float2int_rz(x); }
+template <> __device__ __forceinline__ int32_t cvt_elem<int32_t, double>(double x) { return (x != x) ? 0 : __double2int_rz(x); }
+template <> __device__ __forceinline__ int32_t cvt_elem<int32_t, long long>(long long x) { return (int32_t)(uint32_t)(unsigned long long)x; }
+template <> __device__ __forceinline__ long long cvt_elem<long long, float>(float x) { return (x != x) ? 0ll : __float2ll_rz(x); }
+template <> __device__ __forceinline__ long long cvt_elem<long long, double>(double x) { return (x != x) ? 0ll : __double2ll_rz(x); }
+template <> __device__ __forceinline__ long long cvt_elem<long long, int32_t>(int32_t x) { return (long long)x; }
+// one element of type DT_* `src_dt` at p[i], converted to T (run-time source type: ragged paths and the bytecode evaluator)
+template <class T> __device__ __forceinline__ T load_cvt(const void* p, int64_t i, uint8_t src_dt) {
+    switch (src_dt) {
+        case DT_F32: return cvt_elem<T, float>(reinterpret_cast<const volatile float*>(p)[i]);
+        case DT_F64: return cvt_elem<T, double>(reinterpret_cast<const volatile double*>(p)[i]);
+        case DT_I32: return cvt_elem<T, int32_t>(reinterpret_cast<const volatile int32_t*>(p)[i]);
+        default: return cvt_elem<T, long long>(reinterpret_cast<const volatile long long*>(p)[i]);
+    }
+}
+
 // int32 division / modulo by a pass-constant divisor d (|d| >= 2) with a host-computed signed magic number
 // (the classic multiply-high scheme for truncating signed division): q = mulhi(x, M) (+x or -x when the sign of
 // M differs from that of d), arithmetic shift by s, plus one if negative.  Exact for every int32 x; the
@@ -279,6 +310,17 @@ template <class VEC> __device__ __forceinline__ VEC ld_stream_rw(const VEC* p) {
 template <class VEC> __device__ __forceinline__ void st_stream(VEC* p, const VEC& v) {
     const int4& r = *reinterpret_cast<const int4*>(&v);
     asm volatile("st.global.L1::no_allocate.v4.s32 [%0], {%1,%2,%3,%4};" ::"l"(p), "r"(r.x), "r"(r.y), "r"(r.z), "r"(r.w) : "memory");
+}
+// N = 8, 16 or 32 streamed bytes (the converting loads read V source elements per 128-bit vector of the pass dtype)
+template <int N> __device__ __forceinline__ void ld_stream_bytes(const void* p, void* out) {
+    static_assert(N == 8 || N == 16 || N == 32, "8, 16 or 32 bytes");
+    int* o = reinterpret_cast<int*>(out);
+    if constexpr (N == 8) asm volatile("ld.global.nc.L1::no_allocate.v2.s32 {%0,%1}, [%2];" : "=r"(o[0]), "=r"(o[1]) : "l"(p));
+    else {
+        asm volatile("ld.global.nc.L1::no_allocate.v4.s32 {%0,%1,%2,%3}, [%4];" : "=r"(o[0]), "=r"(o[1]), "=r"(o[2]), "=r"(o[3]) : "l"(p));
+        if constexpr (N == 32)
+            asm volatile("ld.global.nc.L1::no_allocate.v4.s32 {%0,%1,%2,%3}, [%4];" : "=r"(o[4]), "=r"(o[5]), "=r"(o[6]), "=r"(o[7]) : "l"(reinterpret_cast<const char*>(p) + 16));
+    }
 }
 __device__ __forceinline__ unsigned int ld_relaxed_u32(const unsigned int* p) {
     unsigned int v;

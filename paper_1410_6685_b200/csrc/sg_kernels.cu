@@ -96,16 +96,29 @@ int sgk_plan(const SgProg& prog, SgArgs& a, int force_bytecode, int sm_count, in
         if (prog.out[o].kind == OUT_STORE) consider(a.out_ptr[o], 16 + o);
     for (int k = 0; k < prog.shape.n_in; ++k)
         if (prog.in[k].kind == IN_VEC || (is2d && prog.in[k].kind == IN_ROWB)) consider(a.in_ptr[k], k);
+    // a converting input is read as vectors of V SOURCE elements: the same element misalignment, measured against V * its element size
+    for (int k = 0; k < prog.shape.n_in; ++k) {
+        if (prog.in[k].kind != IN_VEC_CVT) continue;
+        const int ss = elem_size(prog.in[k].ref);
+        const uintptr_t p = (uintptr_t)a.in_ptr[k];
+        if (p % ss != 0) { congruent = false; continue; }
+        const long m = (long)((p % (uintptr_t)(V * ss)) / ss);
+        if (mis < 0) mis = m;
+        if (m == mis) vec_ok |= 1 << k; else congruent = false;
+    }
     if (mis < 0) mis = 0;
 
     if (is2d) {
+        for (int k = 0; k < prog.shape.n_in; ++k)
+            if (prog.in[k].kind == IN_VEC_CVT) return fail(err, errcap, -10, "dtype conversion inside a matrix pass");
         if (tid == 0 && has_device) return fail(err, errcap, -10, "matrix pass has no precompiled template instance (2-D bytecode evaluator not built)");
         bool ok = congruent && mis == 0 && (a.cols % V) == 0;
         for (int k = 0; k < prog.shape.n_in; ++k)
             if (prog.in[k].kind == IN_VEC && (a.in_stride[k] % V) != 0) ok = false;
         for (int o = 0; o < prog.shape.n_out; ++o)
             if (prog.out[o].kind == OUT_STORE && (a.out_len[o] % V) != 0) ok = false;
-        if (!ok) return fail(err, errcap, -10, "matrix pass needs 16-byte aligned rows (base, leading dimension and column count)");
+        // rows that are not 16-byte aligned (odd column counts / leading dimensions): the same kernel's guarded form (bit 29)
+        const int unaligned_rows = ok ? 0 : (1 << 29);
         const int occ = (has_device && tid) ? g_entries[tid].occupancy() : 2;
         const int SW = tid ? g_entries[tid].tile : BLOCK * 2 * V;
         a.n_strips = (int)((a.cols + SW - 1) / SW);
@@ -129,7 +142,7 @@ int sgk_plan(const SgProg& prog, SgArgs& a, int force_bytecode, int sm_count, in
         }
         geom->ws_bytes = off;
         geom->ctrl_words = a.n_strips + (int)n_chunks;
-        a.vec_ok = vec_ok;
+        a.vec_ok = (vec_ok & ~(1 << 29)) | unaligned_rows;
         a.head = 0; a.n_full_tiles = 0;
         return 0;
     }

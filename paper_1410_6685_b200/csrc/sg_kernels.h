@@ -34,4 +34,9 @@ cudaError_t sgk_launch(const SgProg& prog, const SgArgs& args, const SgGeom& geo
 // sg_transpose.cu: out[c][r] = in[r][c] for a rows x cols row-major matrix of 4- or 8-byte elements (device pointers).
 cudaError_t sgk_transpose(const void* in, int64_t ld_in, int64_t rows, int64_t cols, void* out, int64_t ld_out, int elem_size, cudaStream_t stream);
 
+// sg_ge.cu: steps [k0, k1) of Listing 5's determinant loop on the n x n row-major F64 matrix M as one persistent cooperative
+// kernel (device pointers; det / minpiv: one double each; ready: one zeroed 32-bit word).  *launched_grid: the grid used.
+cudaError_t sgk_ge_loop(double* M, int64_t n, int64_t ld, double* det, double* minpiv, double eps, int64_t k0, int64_t k1, unsigned int* ready, int sm_count,
+                        cudaStream_t stream, int* launched_grid);
+
 #endif  // SG_KERNELS_H_

@@ -104,6 +104,7 @@ __device__ __forceinline__ T load_elem(uint8_t kind, uint8_t ref, int k, const S
         case IN_VEC: return (i < a.in_len[k]) ? reinterpret_cast<const volatile T*>(a.in_ptr[k])[i] : T(0);
         case IN_SHIFT: return (i + 1 < a.in_len[ref]) ? reinterpret_cast<const volatile T*>(a.in_ptr[ref])[i + 1] : T(0);
         case IN_STRIDED: return (i < a.in_len[k]) ? reinterpret_cast<const volatile T*>(a.in_ptr[k])[i * a.in_stride[k]] : T(0);
+        case IN_VEC_CVT: return (i < a.in_len[k]) ? load_cvt<T>(a.in_ptr[k], i, ref) : T(0);
         case IN_SCALAR: return *reinterpret_cast<const volatile T*>(a.in_ptr[k]);
         case IN_IMM: { T v; memcpy(&v, &a.imm[k], sizeof(T)); return v; }
         default: return T(0);

@@ -72,6 +72,17 @@ __device__ __forceinline__ void load_input_full(typename Meta1D<P>::T (&v)[Meta1
 #pragma unroll
             for (int e = 0; e < M::V; ++e) v[in.reg][u * M::V + e] = xe[e];
         }
+    } else if constexpr (in.kind == IN_VEC_CVT) {
+        // a collection of another element type S, converted as it is loaded: V source elements (V * sizeof(S) bytes) per vector
+        typedef typename TypeOf<in.ref>::type S;
+        const S* src = reinterpret_cast<const S*>(a.in_ptr[K]) + base;
+#pragma unroll
+        for (int u = 0; u < M::U; ++u) {
+            S x[M::V];
+            ld_stream_bytes<M::V * (int)sizeof(S)>(src + (size_t)(u * BLOCK + threadIdx.x) * M::V, x);
+#pragma unroll
+            for (int e = 0; e < M::V; ++e) v[in.reg][u * M::V + e] = cvt_elem<T, S>(x[e]);
+        }
     } else if constexpr (in.kind == IN_SHIFT) {
         // x[i+1]: own vector shifted by one, last element from the next lane, lane 31 reads one scalar
         constexpr int rr = P::prog.in[in.ref].reg;

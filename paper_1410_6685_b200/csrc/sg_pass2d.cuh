@@ -115,8 +115,12 @@ template <int R> __device__ __forceinline__ bool warp_row_owner(int lane) {
     return (lane & low) == 0;
 }
 
-template <class P>
-__global__ void __launch_bounds__(BLOCK, P::min_blocks) pass2d_template(const __grid_constant__ SgArgs a) {
+// ALIGNED: every row of every matrix operand starts on a 16-byte boundary and holds a whole number of 128-bit vectors (base,
+// leading dimension and column count): rows are staged by bulk copies and stored with 128-bit accesses.  Otherwise (odd column
+// counts or leading dimensions, PAPER.md:209-219 puts no condition on a matrix's shape) the block fills the stage cooperatively
+// with element loads in the same layout, and ROW-broadcast loads, stores and reductions are guarded per ELEMENT.
+template <class P, bool ALIGNED>
+__device__ __forceinline__ void pass2d_body(const SgArgs& a) {
     typedef Meta2D<P> M;
     typedef typename M::T T;
     typedef typename M::VEC VEC;
@@ -132,12 +136,17 @@ __global__ void __launch_bounds__(BLOCK, P::min_blocks) pass2d_template(const __
     const int64_t r_begin = (int64_t)chunk * a.rows_per_chunk;
     const int64_t r_end = (r_begin + a.rows_per_chunk < a.n) ? (r_begin + a.rows_per_chunk) : a.n;
     int64_t col[U];
+    int nval[U];                // valid columns of the thread's vector u: 0 or V when ALIGNED, 0..V otherwise
     bool cvalid[U];
 #pragma unroll
     for (int u = 0; u < U; ++u) {
         col[u] = (int64_t)strip * M::SW + (int64_t)(u * BLOCK + threadIdx.x) * V;
-        cvalid[u] = col[u] + V <= a.cols;
+        const int64_t left = a.cols - col[u];
+        nval[u] = left >= V ? V : (left > 0 ? (int)left : 0);
+        cvalid[u] = ALIGNED ? (left >= V) : (left > 0);
     }
+    // element e of vector u takes part?  (compile-time true inside valid vectors of the aligned form)
+    auto evalid = [&](int u, int e) { return ALIGNED ? true : e < nval[u]; };
 
     T v[M::NV][E];
     bool p[M::NP][E];
@@ -166,7 +175,13 @@ __global__ void __launch_bounds__(BLOCK, P::min_blocks) pass2d_template(const __
 #pragma unroll
             for (int u = 0; u < U; ++u) {
                 VEC x = VEC();
-                if (cvalid[u]) x = *reinterpret_cast<const VEC*>(reinterpret_cast<const T*>(a.in_ptr[k]) + col[u]);
+                T* xw = reinterpret_cast<T*>(&x);
+                if (ALIGNED) { if (cvalid[u]) x = *reinterpret_cast<const VEC*>(reinterpret_cast<const T*>(a.in_ptr[k]) + col[u]); }
+                else {
+#pragma unroll
+                    for (int e = 0; e < V; ++e)
+                        if (e < nval[u]) xw[e] = reinterpret_cast<const T*>(a.in_ptr[k])[col[u] + e];
+                }
                 const T* xe = reinterpret_cast<const T*>(&x);
 #pragma unroll
                 for (int e = 0; e < V; ++e) v[in.reg][u * V + e] = xe[e];
@@ -196,19 +211,37 @@ __global__ void __launch_bounds__(BLOCK, P::min_blocks) pass2d_template(const __
             for (int j = 0; j < nr; ++j) bulk_g2s(dst + (size_t)j * M::SW, src + (size_t)j * a.in_stride[k], row_bytes, &full[s]);
         }
     };
-    if (threadIdx.x == 0) {
-        for (int s = 0; s < NS; ++s) mbar_init(&full[s], 1);
-        mbar_fence_init();
+    // unaligned rows: the whole block copies the rows of batch b into stage b % NS with element loads (same layout)
+    auto fill = [&](int64_t b) {
+        const int s = (int)(b % NS);
+        const int64_t r0 = r_begin + b * RS;
+        const int nr = (int)((r_end - r0) < RS ? (r_end - r0) : RS);
+        const int row_elems = (int)(row_bytes / sizeof(T));
+#pragma unroll
+        for (int k = 0; k < M::S.n_in; ++k) {
+            if (g.in[k].kind != IN_VEC) continue;
+            T* dst = stage_base + ((size_t)s * M::NVECIN + slots.vec[k]) * RS * M::SW;
+            const volatile T* src = reinterpret_cast<const volatile T*>(a.in_ptr[k]) + r0 * a.in_stride[k] + c0;
+            for (int j = 0; j < nr; ++j)
+                for (int c = threadIdx.x; c < row_elems; c += BLOCK) dst[(size_t)j * M::SW + c] = src[(size_t)j * a.in_stride[k] + c];
+        }
+    };
+    if (ALIGNED) {
+        if (threadIdx.x == 0) {
+            for (int s = 0; s < NS; ++s) mbar_init(&full[s], 1);
+            mbar_fence_init();
+        }
+        __syncthreads();
+        if (threadIdx.x == 0)
+            for (int64_t b = 0; b < NS && b < nb; ++b) issue(b);
     }
-    __syncthreads();
-    if (threadIdx.x == 0)
-        for (int64_t b = 0; b < NS && b < nb; ++b) issue(b);
 
     for (int64_t b = 0; b < nb; ++b) {
         const int s = (int)(b % NS);
         const int64_t r0 = r_begin + b * RS;
         const int64_t rb = r_begin + (b * RS) / RB * RB;                // start of the current RB-row batch of the per-row combine
-        mbar_wait(&full[s], (uint32_t)((b / NS) & 1));
+        if (ALIGNED) mbar_wait(&full[s], (uint32_t)((b / NS) & 1));
+        else { fill(b); __syncthreads(); }
         Cell rowc[M::NROWS][RS];                 // per-thread partials of the AXIS_ROWS outputs, one per row of the stage
 #pragma unroll
         for (int o = 0; o < M::S.n_out; ++o)
@@ -247,11 +280,17 @@ __global__ void __launch_bounds__(BLOCK, P::min_blocks) pass2d_template(const __
 #pragma unroll
                     for (int u = 0; u < U; ++u) {
                         if (!cvalid[u]) continue;
-                        VEC x;
-                        T* xe = reinterpret_cast<T*>(&x);
+                        if (ALIGNED) {
+                            VEC x;
+                            T* xe = reinterpret_cast<T*>(&x);
 #pragma unroll
-                        for (int e = 0; e < V; ++e) xe[e] = v[out.src][u * V + e];
-                        st_stream(reinterpret_cast<VEC*>(rowp + col[u]), x);
+                            for (int e = 0; e < V; ++e) xe[e] = v[out.src][u * V + e];
+                            st_stream(reinterpret_cast<VEC*>(rowp + col[u]), x);
+                        } else {
+#pragma unroll
+                            for (int e = 0; e < V; ++e)
+                                if (e < nval[u]) rowp[col[u] + e] = v[out.src][u * V + e];
+                        }
                     }
                 } else if (out_is_reduction(out.kind)) {
 #pragma unroll
@@ -259,6 +298,7 @@ __global__ void __launch_bounds__(BLOCK, P::min_blocks) pass2d_template(const __
                         if (!cvalid[u]) continue;
 #pragma unroll
                         for (int e = 0; e < V; ++e) {
+                            if (!evalid(u, e)) continue;
                             const int ee = u * V + e;
                             Cell& dstc = (out.axis == AXIS_ALL) ? acc[o] : (out.axis == AXIS_COLS) ? acc_col[o][ee] : rowc[out.axis == AXIS_ROWS ? slots.row[o] : 0][j];
                             if (out_is_pred_reduction(out.kind)) cell_accum_pred(out.kind, dstc, p[out.src][ee]);
@@ -278,7 +318,7 @@ __global__ void __launch_bounds__(BLOCK, P::min_blocks) pass2d_template(const __
             if (warp_row_owner<RS>(lane) && r < r_end) s_row[slots.row[o]][warp][(int)(r - rb)] = rowc[slots.row[o]][0];
         }
         __syncthreads();                        // every thread is done with stage s (and with this batch's s_row writes)
-        if (threadIdx.x == 0 && b + NS < nb) { fence_proxy_async(); issue(b + NS); }
+        if (ALIGNED && threadIdx.x == 0 && b + NS < nb) { fence_proxy_async(); issue(b + NS); }
         const int64_t done_rows = (b + 1) * RS < n_rows ? (b + 1) * RS : n_rows;
         if (M::HAS_ROWS && (done_rows % RB == 0 || done_rows == n_rows)) {
             const int64_t rb_end = r_begin + done_rows;
@@ -309,7 +349,8 @@ __global__ void __launch_bounds__(BLOCK, P::min_blocks) pass2d_template(const __
             for (int u = 0; u < U; ++u) {
                 if (!cvalid[u]) continue;
 #pragma unroll
-                for (int e = 0; e < V; ++e) ws[(size_t)chunk * a.cols + col[u] + e] = acc_col[o][u * V + e];
+                for (int e = 0; e < V; ++e)
+                    if (evalid(u, e)) ws[(size_t)chunk * a.cols + col[u] + e] = acc_col[o][u * V + e];
             }
         }
     }
@@ -340,6 +381,7 @@ __global__ void __launch_bounds__(BLOCK, P::min_blocks) pass2d_template(const __
                     if (!cvalid[u]) continue;
 #pragma unroll
                     for (int e = 0; e < V; ++e) {
+                        if (!evalid(u, e)) continue;
                         Cell c = cell_identity<T>(out.kind);
                         for (int ch = 0; ch < a.n_chunks; ++ch) cell_combine<T>(out.kind, c, ldcg_cell(&ws[(size_t)ch * a.cols + col[u] + e]));
                         store_final<T>(out.kind, a.out_ptr[o], col[u] + e, c);
@@ -364,6 +406,12 @@ __global__ void __launch_bounds__(BLOCK, P::min_blocks) pass2d_template(const __
         }
     }
     epilogue_1d<T, NOUT>(acc, kind, a, has_all);
+}
+
+template <class P>
+__global__ void __launch_bounds__(BLOCK, P::min_blocks) pass2d_template(const __grid_constant__ SgArgs a) {
+    if ((a.vec_ok >> 29) & 1) pass2d_body<P, false>(a);     // bit 29: rows are not 16-byte aligned (uniform)
+    else pass2d_body<P, true>(a);
 }
 
 }  // namespace sgk

@@ -24,8 +24,9 @@ namespace {
 
 int es_of(const Value& v) { return dtype_size(v.dtype); }
 
-MemRange range_of(const Value& v) {
+MemRange range_of(const Value& v, bool exact = true) {
     MemRange r;
+    r.exact = exact && v.kind != VK_SCALAR;
     const int64_t es = es_of(v);
     r.ptr = v.ptr; r.stride = v.stride; r.ld = v.ld; r.rows = v.rows; r.cols = v.cols;
     r.lo = v.ptr;
@@ -38,17 +39,28 @@ bool overlaps(const MemRange& a, const MemRange& b) { return a.lo < b.hi && b.lo
 bool same_view(const MemRange& a, const MemRange& b) {
     return a.ptr == b.ptr && a.stride == b.stride && a.ld == b.ld && a.rows == b.rows && a.cols == b.cols;
 }
+// may a pass that reads `r` also write `w` in place?  Only when the read is index-for-index over the very same view: then every
+// element is read by the thread that writes it, before it writes it.  A shifted read (x[i+1] belongs to another thread, warp or
+// block), a broadcast or a scalar read of storage the pass overwrites would see a mix of old and new values.
+bool read_is_private_to_writer(const MemRange& w, const MemRange& r) { return r.exact && same_view(w, r); }
 
 bool pending(const sg_ctx* c, const Value& v) { return v.node >= 0 && !c->nodes[v.node].done; }
 
 }  // namespace
 
-sg_status sg_flush_impl(sg_ctx* c) {
+namespace {
+
+// quantifier outputs of a pass that may end early at a violated contract (PF_EARLY_EXIT with registered for_all contracts)
+struct ExitMember { int value; uint8_t kind; bool is_contract; };
+typedef std::vector<std::vector<ExitMember>> ExitGroups;
+
+// Plans and launches everything pending.  *executed = number of passes whose kernels were queued on the stream when the
+// function returned (all of them on success).  On failure the caller rolls the context back (retire_nodes).
+sg_status flush_body(sg_ctx* c, int* executed, ExitGroups* exit_groups) {
     const bool unfused = c->flags & SG_FLAG_UNFUSED;
     std::vector<Node>& N = c->nodes;
     std::vector<Value>& V = c->values;
     int64_t launches_total = c->stats.launches_total;
-    if (N.empty()) return SG_OK;
     memset(&c->stats, 0, sizeof(c->stats));
     c->stats.launches_total = launches_total;
     c->dumps.clear();
@@ -109,10 +121,13 @@ sg_status sg_flush_impl(sg_ctx* c) {
             if (pending(c, v) && N[v.node].needed) {
                 const Node& Y = N[v.node];
                 if (Y.kind == NK_MAP) {
-                    const bool via_memory = unfused || (X.post && materialises(Y)) || X.opd[j].kind == OPD_SHIFT;
+                    // a neighbour operand and the operand of a dtype conversion are read back from memory: a pass has ONE value
+                    // file, the conversion happens as the operand is loaded (IN_VEC_CVT)
+                    const bool from_memory = X.opd[j].kind == OPD_SHIFT || (X.kind == NK_MAP && X.op == NODE_OP_CAST);
+                    const bool via_memory = unfused || (X.post && materialises(Y)) || from_memory;
                     lb = std::max(lb, Y.pass + (via_memory ? 1 : 0));
                     if (!via_memory) reg_producers.push_back(v.node);
-                    if (X.opd[j].kind == OPD_SHIFT) spill[X.opd[j].value] = 1;
+                    if (from_memory) spill[X.opd[j].value] = 1;
                 } else if (Y.kind == NK_REDUCE) {
                     lb = std::max(lb, Y.pass + 1);
                 } else {    // NK_FILTER: only a reduction over the kept values may follow, in the same pass
@@ -122,7 +137,7 @@ sg_status sg_flush_impl(sg_ctx* c) {
             } else {
                 if (!v.materialised && v.slot < 0) return sg_fail(c, SG_ERR_ARG, "operand has neither storage nor a pending producer");
                 if (v.slot >= 0) continue;                      // scalar slot written by an earlier flush
-                reads.push_back(range_of(v));
+                reads.push_back(range_of(v, X.opd[j].kind != OPD_SHIFT && X.opd[j].bcast == SG_BCAST_NONE));
             }
         }
         if (X.post && post_group[i] >= 0)       // the whole predicate of a POST contract runs after the results it reads are stored
@@ -138,13 +153,13 @@ sg_status sg_flush_impl(sg_ctx* c) {
                 for (const MemRange& w2 : passes[q].writes)
                     if (overlaps(w, w2)) lb = std::max(lb, (int)q + 1);                         // WAW
                 for (const MemRange& r : passes[q].reads)
-                    if (overlaps(w, r)) lb = std::max(lb, (int)q + (same_view(w, r) ? 0 : 1));  // WAR: same pass only index-for-index
+                    if (overlaps(w, r)) lb = std::max(lb, (int)q + (read_is_private_to_writer(w, r) ? 0 : 1));  // WAR: same pass only index-for-index
             }
         }
         // within this very operation: an in-place result may alias an operand only index-for-index
         for (const MemRange& w : writes)
             for (const MemRange& r : reads)
-                if (overlaps(w, r) && !same_view(w, r)) return sg_fail(c, SG_ERR_ALIAS, "in-place operation reads a shifted or overlapping view of its destination");
+                if (overlaps(w, r) && !read_is_private_to_writer(w, r)) return sg_fail(c, SG_ERR_ALIAS, "in-place operation reads a shifted or overlapping view of its destination");
 
         const bool stores = materialises(X);
         const int xdt = (X.dtype == SG_BOOL) ? -1 : X.dtype;
@@ -265,9 +280,13 @@ sg_status sg_flush_impl(sg_ctx* c) {
                 P.args.epoch = c->epoch;
             }
             cudaError_t e = sgk_launch(P.prog, P.args, P.geom, c->stream);
-            if (e != cudaSuccess) return sg_fail(c, SG_ERR_CUDA, std::string("kernel launch failed: ") + cudaGetErrorString(e));
+            if (e != cudaSuccess) {
+                c->stats.launches_total = launches_total;
+                return sg_fail(c, SG_ERR_CUDA, std::string("kernel launch failed: ") + cudaGetErrorString(e));
+            }
             c->last.push_back({P.prog, P.args, P.geom});
             launches_total++;
+            ++*executed;
         }
         cudaEventRecord(t1, c->stream);
         // a8: hand the flush's scalars back in one copy
@@ -288,18 +307,48 @@ sg_status sg_flush_impl(sg_ctx* c) {
         c->deferred_free = temps;
     } else {
         for (Pass& P : passes) c->last.push_back({P.prog, P.args, P.geom});
+        *executed = (int)passes.size();
     }
     c->stats.launches_total = launches_total;
+    // quantifier passes that may end early at a violated contract: remember their members for the contract check
+    for (const Pass& P : passes) {
+        if (!(P.prog.shape.flags & PF_EARLY_EXIT) || !P.args.exit_any || P.args.no_early_exit) continue;
+        std::vector<ExitMember> grp;
+        for (int k : P.nodes) {
+            const Node& n = N[k];
+            if (n.kind != NK_REDUCE || (n.op != OUT_ALL && n.op != OUT_ANY)) continue;
+            bool is_contract = false;
+            for (const Contract& ct : c->contracts) is_contract |= (ct.value == n.out && n.op == OUT_ALL);
+            grp.push_back({n.out, n.op, is_contract});
+        }
+        exit_groups->push_back(grp);
+    }
 
-    // ---- 6. commit: results now have storage; the pending list is consumed -------------------------------
+    return SG_OK;
+}
+
+// Retires the pending list.  Operations of the first `executed` passes ran (their kernels are queued): their results have
+// storage now.  Everything else — operations no live handle needed, and after a failed flush the operations that were never
+// launched — is DISCARDED: storage this flush allocated for their results is given back, their result handles name no data
+// (a discarded filter output is empty) until they are released.  In-place destinations keep their previous contents.
+void retire_nodes(sg_ctx* c, int executed) {
+    std::vector<Node>& N = c->nodes;
+    std::vector<Value>& V = c->values;
     for (Node& n : N) {
         if (n.done) continue;
         n.done = true;
+        const bool ran = n.needed && n.pass >= 0 && n.pass < executed;
         for (int o : {n.out, n.out2}) {
             if (o < 0) continue;
             Value& v = V[o];
             if (v.user_refs < 0) v.user_refs = 0;
             if (v.node >= 0 && &N[v.node] == &n) v.node = -1;
+            if (!ran) {
+                if (v.fresh_alloc && v.ptr) { sg_dev_free(c, v.ptr); v.ptr = nullptr; v.owned = false; }
+                if (!n.inplace && v.kind != VK_SCALAR) v.materialised = false;
+                if (!v.count_known) { v.count_known = true; v.cols = 0; v.ld = 0; }
+            }
+            v.fresh_alloc = false;
         }
     }
     for (int i : c->live) { Value& v = V[i]; if (v.node >= 0 && N[v.node].done) v.node = -1; }
@@ -318,6 +367,28 @@ sg_status sg_flush_impl(sg_ctx* c) {
         if (v.alive) c->live[keep++] = i;
     }
     c->live.resize(keep);
+}
+
+}  // namespace
+
+// The flush is transactional: if planning fails (unsupported chain, too many passes, aliasing, allocation), nothing was launched,
+// the error is reported and the pending list is discarded, so the context stays usable for later work.  If a launch fails, the
+// passes already queued count as executed and the rest is discarded.
+sg_status sg_flush_impl(sg_ctx* c) {
+    if (c->nodes.empty()) return SG_OK;
+    std::vector<Value>& V = c->values;
+    int executed = 0;
+    ExitGroups exit_groups;
+    const sg_status s = flush_body(c, &executed, &exit_groups);
+    if (s != SG_OK) {
+        const std::string why = c->err;
+        c->contracts.clear();               // before retire_nodes: contract scalars of a discarded list give their slots back
+        retire_nodes(c, executed);
+        c->err = why + (executed ? " (later passes discarded)" : " (pending operations discarded)");
+        return s;
+    }
+    // ---- 6. commit: results now have storage; the pending list is consumed -------------------------------
+    retire_nodes(c, 1 << 30);
 
     // ---- 7. contracts: evaluated on the device with the data; read with the scalars ----
     sg_status result = SG_OK;
@@ -332,6 +403,22 @@ sg_status sg_flush_impl(sg_ctx* c) {
                 c->err = std::string(k.kind == SG_CONTRACT_PRE ? "precondition" : "postcondition") + " violated: " + k.tag;
             }
         }
+        // A pass of quantifiers ends as soon as one of its registered for_all contracts is violated (early exit).  The other
+        // quantifiers of that pass were then evaluated on a PREFIX of the data: one that was decided on the prefix (a for_all
+        // already false, an exists already true) is final, the others are not evaluated and reading them is an error.
+        if (result == SG_ERR_CONTRACT && !c->plan_only)
+            for (const auto& grp : exit_groups) {
+                bool violated = false;
+                for (const ExitMember& m : grp)
+                    if (m.is_contract && V[m.value].slot >= 0 && c->slab_host[8 * V[m.value].slot] == 0) violated = true;
+                if (!violated) continue;
+                for (const ExitMember& m : grp) {
+                    Value& v = V[m.value];
+                    if (v.slot < 0) continue;
+                    const bool t = c->slab_host[8 * v.slot] != 0;
+                    if ((m.kind == OUT_ALL && t) || (m.kind == OUT_ANY && !t)) v.undecided = true;
+                }
+            }
         c->contracts.clear();
     }
     if (!c->plan_only) {

@@ -35,7 +35,9 @@ enum : uint8_t {
     IN_IMM = 4,     // host immediate, passed as a kernel argument (the `a` of aX+Y)
     IN_ROWB = 5,    // 2-D: vector indexed by the column, same for every row
     IN_COLB = 6,    // 2-D: vector indexed by the row, same for every column
-    IN_BOOLVEC = 7  // unit-stride BOOL collection (1 byte per element) loaded into a predicate register
+    IN_BOOLVEC = 7, // unit-stride BOOL collection (1 byte per element) loaded into a predicate register
+    IN_VEC_CVT = 8  // unit-stride collection of ANOTHER element type (`ref` = its DT_*), converted to the pass dtype as it is loaded:
+                    // the dtype-changing `project (transform: FUNCTION[T, U]): COLLECTION[U]` of PAPER.md:137-139, 171-175
 };
 
 enum : uint8_t {
@@ -64,7 +66,7 @@ enum : uint8_t {
 #define SG_MAX_TMAP 2
 
 struct SgInstr { uint8_t op, dst, a, b; };
-struct SgIn { uint8_t kind, ref, reg, pad; };      // reg: V (or P for IN_BOOLVEC) register the input is loaded into
+struct SgIn { uint8_t kind, ref, reg, pad; };      // ref: IN_SHIFT: the shifted input; IN_VEC_CVT: source DT_*.  reg: V (or P for IN_BOOLVEC) register the input is loaded into
 struct SgOut { uint8_t kind, src, pred, axis; };
 
 struct SgShape {

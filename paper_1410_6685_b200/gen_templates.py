@@ -60,6 +60,10 @@ def _chains():
     yield "matvec_right", 0, lambda c: W.right_multiply(c, 4096, 4096, None, None)
     yield "matvec_left", 0, lambda c: W.left_multiply(c, 4096, 4096, None, None)
     # the rest of the vector API
+    yield "isqrt_i32", 0, lambda c: W.project_sqrt(c, i32, N, None, pout=0x7000000)                      # INT -> DOUBLE sqrt
+    yield "isqrt_i64", 0, lambda c: W.project_sqrt(c, sg.SG_I64, N, None, pout=0x7000000)
+    yield "cast_i32_f32", 0, lambda c: sg.sg_cast(c, sg.sg_vec_create(c, i32, N, None), f32, sg.sg_vec_create(c, f32, N, 0x7000000))
+    yield "cast_f64_i32", 0, lambda c: sg.sg_cast(c, sg.sg_vec_create(c, f64, N, None), i32, sg.sg_vec_create(c, i32, N, 0x7000000))
     for tag, dt in (("f32", f32), ("f64", f64)):
         yield f"sqrt_{tag}", 0, lambda c, dt=dt: W.project_sqrt(c, dt, N, None, pout=0x7000000)
         yield f"avg_{tag}", 0, lambda c, dt=dt: W.avg(c, dt, N, None)

@@ -22,6 +22,7 @@ SG_BCAST_NONE, SG_BCAST_ROW, SG_BCAST_COL = 0, 1, 2
 SG_CONTRACT_PRE, SG_CONTRACT_POST = 0, 1
 SG_FLAG_UNFUSED, SG_FLAG_FORCE_BYTECODE, SG_FLAG_NO_EARLY_EXIT = 1, 2, 4
 SG_OK = 0
+SG_ACC_DEFAULT = -1
 SG_ERR = {-1: "SG_ERR_ARG", -2: "SG_ERR_SHAPE", -3: "SG_ERR_DTYPE", -4: "SG_ERR_EMPTY", -5: "SG_ERR_ALIAS", -6: "SG_ERR_OOM",
           -7: "SG_ERR_CUDA", -8: "SG_ERR_CONTRACT", -9: "SG_ERR_CAPACITY", -10: "SG_ERR_UNSUPPORTED"}
 SG_ERR_ARG, SG_ERR_SHAPE, SG_ERR_DTYPE, SG_ERR_EMPTY, SG_ERR_ALIAS, SG_ERR_OOM, SG_ERR_CUDA, SG_ERR_CONTRACT, SG_ERR_CAPACITY, \
@@ -29,7 +30,7 @@ SG_ERR_ARG, SG_ERR_SHAPE, SG_ERR_DTYPE, SG_ERR_EMPTY, SG_ERR_ALIAS, SG_ERR_OOM, 
 
 EXPORTS = [
     "sg_ctx_create", "sg_ctx_destroy", "sg_ctx_set_flags", "sg_last_error", "sg_vec_create", "sg_mat_create", "sg_vec_subset",
-    "sg_mat_row", "sg_mat_rows", "sg_mat_col", "sg_mat_elem", "sg_mat_ge_steps", "sg_mat_transpose", "sg_enqueue", "sg_reduce", "sg_forall", "sg_exists",
+    "sg_mat_row", "sg_mat_rows", "sg_mat_col", "sg_mat_elem", "sg_mat_ge_steps", "sg_mat_transpose", "sg_enqueue", "sg_cast", "sg_reduce", "sg_forall", "sg_exists",
     "sg_forall_adjacent", "sg_filter", "sg_contract", "sg_flush", "sg_scalar_get", "sg_scalar_dtype", "sg_vec_count", "sg_vec_data", "sg_vec_read",
     "sg_release", "sg_plan_stats", "sg_plan_dump", "sg_last_flush_ms", "sg_timing_begin", "sg_timing_end", "sg_replay_last", "sg_template_count", "sg_template_name",
     "sg_version",
@@ -80,7 +81,8 @@ def lib() -> ctypes.CDLL:
         L.sg_mat_col.argtypes = [c_void_p, c_int64, c_int64, c_int64, c_int64, POINTER(c_int64)]
         L.sg_mat_elem.argtypes = [c_void_p, c_int64, c_int64, c_int64, POINTER(c_int64)]
         L.sg_enqueue.argtypes = [c_void_p, c_int32, POINTER(sg_operand), c_int32, c_int64, POINTER(c_int64)]
-        L.sg_reduce.argtypes = [c_void_p, c_int64, c_int32, c_int32, POINTER(c_int64)]
+        L.sg_cast.argtypes = [c_void_p, c_int64, c_int32, c_int64, POINTER(c_int64)]
+        L.sg_reduce.argtypes = [c_void_p, c_int64, c_int32, c_int32, c_int32, POINTER(c_int64)]
         L.sg_forall.argtypes = [c_void_p, c_int64, POINTER(c_int64)]
         L.sg_exists.argtypes = [c_void_p, c_int64, POINTER(c_int64)]
         L.sg_forall_adjacent.argtypes = [c_void_p, c_int64, c_int32, POINTER(c_int64)]
@@ -97,7 +99,7 @@ def lib() -> ctypes.CDLL:
         L.sg_plan_dump.argtypes = [c_void_p, c_int32, c_char_p, c_int64]
         L.sg_last_flush_ms.argtypes = [c_void_p, POINTER(c_float)]
         L.sg_replay_last.argtypes = [c_void_p, c_int32, POINTER(c_float)]
-        L.sg_mat_ge_steps.argtypes = [c_void_p, c_int64, c_int64, c_int64, c_int64, c_int64]
+        L.sg_mat_ge_steps.argtypes = [c_void_p, c_int64, c_int64, c_int64, c_double, c_int64, c_int64]
         L.sg_mat_transpose.argtypes = [c_void_p, c_int64, c_void_p, c_int64, POINTER(c_int64)]
         L.sg_timing_begin.argtypes = [c_void_p]
         L.sg_timing_end.argtypes = [c_void_p, POINTER(c_float), POINTER(c_int32)]
@@ -208,8 +210,8 @@ def sg_mat_transpose(ctx, m: int, dev_out: int | None = None, ld_out: int = 0) -
     return _h(lib().sg_mat_transpose, ctx, m, c_void_p(dev_out or 0), ld_out)
 
 
-def sg_mat_ge_steps(ctx, m: int, det: int, minpiv: int, k0: int, k1: int) -> None:
-    _ck(ctx, lib().sg_mat_ge_steps(ctx, m, det, minpiv, k0, k1))
+def sg_mat_ge_steps(ctx, m: int, det: int, minpiv: int, eps: float, k0: int, k1: int) -> None:
+    _ck(ctx, lib().sg_mat_ge_steps(ctx, m, det, minpiv, float(eps), k0, k1))
 
 
 def sg_enqueue(ctx, op: int, operands, dst_or_0: int = 0) -> int:
@@ -218,8 +220,12 @@ def sg_enqueue(ctx, op: int, operands, dst_or_0: int = 0) -> int:
     return _h(lib().sg_enqueue, ctx, op, arr, len(ops), dst_or_0)
 
 
-def sg_reduce(ctx, h: int, kind: int, axis: int = SG_AXIS_ALL) -> int:
-    return _h(lib().sg_reduce, ctx, h, kind, axis)
+def sg_cast(ctx, v: int, to: int, dst_or_0: int = 0) -> int:
+    return _h(lib().sg_cast, ctx, v, to, dst_or_0)
+
+
+def sg_reduce(ctx, h: int, kind: int, axis: int = SG_AXIS_ALL, acc: int = SG_ACC_DEFAULT) -> int:
+    return _h(lib().sg_reduce, ctx, h, kind, acc, axis)
 
 
 def sg_forall(ctx, h_bool: int) -> int:

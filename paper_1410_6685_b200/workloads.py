@@ -193,16 +193,21 @@ def ge_step(ctx, M, n, k, det, minpiv):
 def ge_determinant(ctx, n, pM, pdet, pminpiv, ld=None, eps=0.0, native=True):
     """Listing 5: the whole determinant loop with no host synchronisation between steps.
 
-    pdet / pminpiv: device float64[1] initialised by the caller to 1.0 / +inf.  Every step is flushed asynchronously (scalar
-    + factor pass, matrix pass) — by the library composite sg_mat_ge_steps, or (native=False) by the same calls made from here.  The zero-pivot test of PAPER.md:339 is a device-evaluated contract on
-    the smallest |pivot| seen, checked once at the end: the result is 0.0 if it fails, as in the listing.
-    Returns (det, ok)."""
+    pdet / pminpiv: device float64[1] initialised by the caller to 1.0 / +inf.
+    native=True: sg_mat_ge_steps — ONE persistent kernel runs all n steps, incl. the listing's control flow: Result := Result *
+    pivot before the approximately-zero test, the loop ends at a pivot with |pivot| <= eps, rows whose entry
+    below the pivot is ~0 are skipped.  Every decision of the method is taken on the device; this function
+    only reads the two results back.
+    native=False: the same steps as host-issued primitives (ge_step + one asynchronous flush per step = 3 launches per step):
+    the measurement baseline for the paper's slow case.  It has no device-side loop exit, so it is the listing only
+    for matrices without an approximately-zero pivot or sub-pivot entry.
+    Returns (det, ok): det = Result as the device computed it; ok = no pivot was approximately zero."""
     ld = n if ld is None else ld
     M = sg.sg_mat_create(ctx, sg.SG_F64, n, n, ld, pM)
     det = sg.sg_vec_create(ctx, sg.SG_F64, 1, pdet)
     minpiv = sg.sg_vec_create(ctx, sg.SG_F64, 1, pminpiv)
     if native:
-        sg.sg_mat_ge_steps(ctx, M, det, minpiv, 0, n)           # the same steps enqueued and flushed by the library itself
+        sg.sg_mat_ge_steps(ctx, M, det, minpiv, eps, 0, n)
     else:
         for k in range(n):
             for h in ge_step(ctx, M, n, k, det, minpiv):
@@ -215,16 +220,19 @@ def ge_determinant(ctx, n, pM, pdet, pminpiv, ld=None, eps=0.0, native=True):
     detv = float(sg.sg_scalar_get(ctx, value))
     for h in (gt, ok, value, det, minpiv, M):
         sg.sg_release(ctx, h)
-    return (detv if okv else 0.0), okv
+    return detv, okv
 
 
 # ------------------------------------------------------------------------------------------------------------------
 # the rest of the vector API
 # ------------------------------------------------------------------------------------------------------------------
 def project_sqrt(ctx, dtype, n, pa, pout=None):
-    """`a.project (agent sqrt)`: a new collection of the correctly rounded square roots."""
+    """`a.project (agent sqrt)`: a new collection of the correctly rounded square roots.  An INTEGER collection
+    gives a collection of DOUBLEs (the paper's own example): the integers are converted as they are loaded, one pass, 4 or 8 bytes
+    read and 8 written per element."""
     a = sg.sg_vec_create(ctx, dtype, n, pa)
-    dst = sg.sg_vec_create(ctx, dtype, n, pout) if pout is not None else 0
+    out_dtype = dtype if dtype in (sg.SG_F32, sg.SG_F64) else sg.SG_F64
+    dst = sg.sg_vec_create(ctx, out_dtype, n, pout) if pout is not None else 0
     r = sg.sg_enqueue(ctx, sg.SG_SQRT, [a], dst_or_0=dst)
     return {"a": a, "out": r}
 

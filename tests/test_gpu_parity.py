@@ -11,7 +11,7 @@ import oracle as orc
 from oracle import configs as ocfg
 from paper_1410_6685_b200 import inputs, sg
 from paper_1410_6685_b200 import workloads as W
-from gpu_util import Ctx, rel_err
+from gpu_util import Ctx, dev, rel_err
 
 pytestmark = pytest.mark.gpu
 
@@ -306,6 +306,25 @@ def test_cfg1_full_size():
     assert sum_ok(gs, want["sum"], want["w"], 1e-5) and np.float32(gmx) == want["max"]
 
 
+def test_cfg1_headline_size():
+    """The configuration bench.py's headline line times (BASELINE.json metric: the fused chain at 2^28 elements): sum and max against
+    the oracle on ALL 2^28 elements, then every element of w (the same chain with w kept)."""
+    n = 1 << 28
+    x, y = inputs.normal_f32(2, 0, n), inputs.normal_f32(2, 1, n)
+    want = ocfg.cfg1(x, y)
+    with Ctx() as c:
+        tx, ty = c.torch.from_numpy(x).cuda(), c.torch.from_numpy(y).cuda()
+        r = W.cfg1(c.ctx, n, tx.data_ptr(), ty.data_ptr())
+        gs, gmx = c.get(r["sum"]), c.get(r["max"])
+        st = sg.sg_plan_stats(c.ctx)
+        assert st.n_passes == 1 and st.n_template == 1 and st.bytes_min == 8 * n
+        assert sum_ok(gs, want["sum"], want["w"], 1e-5) and np.float32(gmx) == want["max"]
+        r2 = W.cfg1(c.ctx, n, tx.data_ptr(), ty.data_ptr(), keep_w=True)
+        gs2 = c.get(r2["sum"])
+        w = c.read_vec(r2["w"], np.float32)
+    assert gs2 == gs and bits_equal(w, want["w"])
+
+
 # ----------------------------------------------------------------------------------------------------------
 # config 2
 # ----------------------------------------------------------------------------------------------------------
@@ -485,17 +504,24 @@ def colsum_ok(got, want, col_abs_sum):
     return all(rel_err(g, w, s) <= 1e-12 for g, w, s in zip(got, want, col_abs_sum))
 
 
-@pytest.mark.parametrize("n,k", [(2, 0), (4, 1), (34, 0), (34, 33), (258, 100), (1030, 7), (2050, 2048), (1538, 0)])
-def test_cfg4(n, k):
+# odd n (and odd leading dimensions): rows that are not 16-byte aligned take the matrix pass's guarded form (PAPER.md:209-219 puts
+# no condition on a matrix's shape)
+@pytest.mark.parametrize("n,k,ld", [(2, 0, 2), (4, 1, 4), (34, 0, 34), (34, 33, 34), (258, 100, 258), (1030, 7, 1030), (2050, 2048, 2050), (1538, 0, 1538),
+                                    (3, 0, 3), (3, 1, 3), (33, 5, 33), (33, 31, 37), (129, 0, 129), (1031, 7, 1031), (1031, 1000, 1040), (515, 3, 521), (64, 3, 67)])
+def test_cfg4(n, k, ld):
     M = inputs.boosted_matrix_f64(5, 0, n)
     want = ocfg.cfg4(M, k)
     with Ctx() as c:
-        t = c.torch.from_numpy(M).cuda()
-        r = W.cfg4(c.ctx, n, t.data_ptr(), k)
+        buf = np.full((n, ld), 7.25)
+        buf[:, :n] = M
+        t = c.torch.from_numpy(buf).cuda()
+        r = W.cfg4(c.ctx, n, t.data_ptr(), k, ld=ld)
         sg.sg_flush(c.ctx)
         c.torch.cuda.synchronize()
-        got = t.cpu().numpy()
+        full = t.cpu().numpy()
+        got = np.ascontiguousarray(full[:, :n])
         assert bits_equal(got, want["M"])
+        assert (full[:, n:] == 7.25).all()                              # the padding between rows is never written
         if k + 1 < n:
             rowmax = c.read_vec(r["rowmax"], np.float64)
             colsum = c.read_vec(r["colsum"], np.float64)
@@ -505,30 +531,24 @@ def test_cfg4(n, k):
 
 
 @pytest.mark.parametrize("k", [0, 8191])
-def test_cfg4_full_size_sampled(k):
+def test_cfg4_full_size(k):
+    """BASELINE.json:configs[4] at its full size, in bench.py's launch configuration: EVERY element of M', all n-k-1 row maxima
+    and all n column sums against the oracle's definition (orc_mat_step on the whole matrix takes seconds)."""
     n = 16384
     M = inputs.boosted_matrix_f64(5, 0, n)
-    S = sorted({0, 1, k, min(k + 1, n - 1), 4097, 8190, 8192, 12345, n - 1})
-    Ms, _, colsum_s = orc.mat_step(M[:, [k] + S], k, 0)              # the definition on sampled columns (all rows)
-    rows = sorted({k + 1, k + 2, (k + n) // 2, n - 1})
+    want_M, want_rowmax, want_colsum = orc.mat_step(M, k)
     with Ctx() as c:
         t = c.torch.from_numpy(M).cuda()
         r = W.cfg4(c.ctx, n, t.data_ptr(), k)
         sg.sg_flush(c.ctx)
+        st = sg.sg_plan_stats(c.ctx)
+        assert st.n_passes == 2 and st.n_template == 2
         rowmax = c.read_vec(r["rowmax"], np.float64)
         colsum = c.read_vec(r["colsum"], np.float64)
-        got_cols = t[:, S].cpu().numpy()
-        got_rows = t[rows, :].cpu().numpy()
-        head = t[: k + 1, :].cpu().numpy()
-    assert bits_equal(np.ascontiguousarray(got_cols), np.ascontiguousarray(Ms[:, 1:]))
-    assert bits_equal(head, M[: k + 1])                              # rows <= k untouched
-    assert colsum_ok(colsum[S], colsum_s[1:], np.abs(Ms[k + 1:, 1:]).sum(axis=0))
-    piv = M[k, k]
-    for j, grow in zip(rows, got_rows):
-        f = np.array([M[j, k]]) / piv                                # one row through the oracle primitives
-        wrow = orc.zip("sub", M[j], orc.scalar("mul", M[k], f[0]))
-        assert bits_equal(grow, wrow)
-        assert rowmax[j - k - 1] == orc.max(orc.unary("abs", wrow))
+        got = t.cpu().numpy()
+    assert bits_equal(got, want_M)                                    # all 2^28 elements (rows <= k untouched included)
+    assert rowmax.size == n - k - 1 and bits_equal(rowmax, want_rowmax)
+    assert colsum.size == n and colsum_ok(colsum, want_colsum, np.abs(want_M[k + 1:]).sum(axis=0))
 
 
 # ----------------------------------------------------------------------------------------------------------
@@ -551,8 +571,9 @@ def run_ge(c, M, ld=None, eps=0.0, native=True):
     return got, ok, t.cpu().numpy()[:, :n], float(minpiv.item())
 
 
-# even n and ld: a matrix pass needs 16-byte aligned rows (SG_ERR_UNSUPPORTED otherwise, include/sg.h)
-@pytest.mark.parametrize("n,ld", [(1, 1), (2, 2), (4, 6), (18, 18), (64, 64), (130, 136), (258, 258), (514, 520)])
+# any n and ld (odd ones included: rows that are not 16-byte aligned); sizes from one block's worth of rows to several rows per block
+@pytest.mark.parametrize("n,ld", [(1, 1), (2, 2), (3, 3), (4, 6), (18, 18), (64, 64), (129, 129), (130, 136), (258, 258), (514, 520), (515, 515), (515, 522),
+                                  (1200, 1200)])
 def test_ge_determinant_loop(n, ld):
     M = ge_matrix(n)
     want_det, want_E, zs = orc.ge_determinant(M)
@@ -563,21 +584,158 @@ def test_ge_determinant_loop(n, ld):
         assert bits_equal(np.array([got]), np.array([want_det]))        # same products in the same order: bit-exact
         assert bits_equal(np.ascontiguousarray(E), want_E)              # the eliminated matrix, every element
         assert minpiv == np.min(np.abs(np.diag(want_E)))
-        if n <= 130:                                                    # the same steps driven call by call from the binding
+        assert sg.sg_plan_stats(c.ctx).n_passes <= 2                    # the loop itself is ONE kernel; the flush afterwards reads det / ok back
+        if n <= 130:                                                    # the same steps as host-issued primitives (3 launches per step)
             got2, ok2, E2, _ = run_ge(c, M, ld, native=False)
             assert ok2 and got2 == got and bits_equal(np.ascontiguousarray(E2), want_E)
 
 
-def test_ge_determinant_zero_pivot_contract():
+def test_ge_determinant_in_two_calls_and_large():
+    """Steps [0, h) and [h, n) in two calls give the same bits as one call; 2200 x 2200: several rows per block and step."""
+    n = 2200
+    M = ge_matrix(n)
+    want_det, want_E, zs = orc.ge_determinant(M)
     with Ctx() as c:
-        M = np.array([[1.0, 2.0, 0.0, 0.0], [2.0, 4.0, 1.0, 0.0], [0.0, 1.0, 1.0, 0.0], [0.0, 0.0, 0.0, 1.0]])   # second pivot 4 - 2*2 = 0
-        want, _, zs = orc.ge_determinant(M)
-        got, ok, _, minpiv = run_ge(c, M)
-        assert zs == 1 and want == 0.0 and got == 0.0 and not ok and minpiv == 0.0
+        t = c.torch.from_numpy(M).cuda()
+        det = c.torch.ones(1, dtype=c.torch.float64, device="cuda")
+        mp = c.torch.full((1,), float("inf"), dtype=c.torch.float64, device="cuda")
+        hM = sg.sg_mat_create(c.ctx, sg.SG_F64, n, n, n, t.data_ptr())
+        hd, hp = sg.sg_vec_create(c.ctx, sg.SG_F64, 1, det.data_ptr()), sg.sg_vec_create(c.ctx, sg.SG_F64, 1, mp.data_ptr())
+        sg.sg_mat_ge_steps(c.ctx, hM, hd, hp, 0.0, 0, 777)
+        sg.sg_mat_ge_steps(c.ctx, hM, hd, hp, 0.0, 777, n)
+        c.torch.cuda.synchronize()
+        assert bits_equal(np.array([det.item()]), np.array([want_det])) and bits_equal(t.cpu().numpy(), want_E)
+        assert mp.item() == np.min(np.abs(np.diag(want_E)))
+
+
+def test_ge_determinant_zero_pivot_is_decided_on_the_device():
+    """Result := Result * pivot, THEN the approximately-zero test, whose else-branch ends the loop.  The library takes
+    that decision (no arithmetic in the binding): det is Result * pivot and the matrix is eliminated exactly up to the zero step."""
+    cases = [
+        (np.array([[1.0, 2.0, 0.0, 0.0], [2.0, 4.0, 1.0, 0.0], [0.0, 1.0, 1.0, 0.0], [0.0, 0.0, 0.0, 1.0]]), 0.0),     # second pivot 4 - 2*2 = 0
+        (np.array([[-1.0, 2.0], [3.0, -6.0]]), 0.0),                                                                    # Result = -1 * 0 = -0.0
+        (np.array([[1e-9, 1.0], [1.0, 1.0]]), 1e-6),                                                                    # ~0 with an explicit eps: Result = 1e-9
+        (np.array([[2.0, 1.0], [4.0, 2.0 + 2.0 ** -40]]), 1e-6),                                                        # Result = 2 * 2^-40
+        (np.array([[2.0, 1.0], [1e-9, 3.0]]), 1e-6),                                                                    # the per-row guard (PAPER.md:350-351): row 1 left as it is
+    ]
+    rng = np.random.default_rng(3)
+    big = ge_matrix(300)
+    big[200] = 0.5 * big[100] + 0.25 * big[150]                           # rank deficient: row 200 eliminates to (almost) nothing
+    cases.append((big, 1e-9))
+    sp = ge_matrix(96)
+    sp[rng.integers(0, 96, 200), rng.integers(0, 96, 200)] = 0.0          # exact zeros below the pivots: skipped rows (eps = 0 guard)
+    sp[np.arange(96), np.arange(96)] = 1.0 + np.arange(96) / 96.0
+    cases.append((sp, 0.0))
+    for M, eps in cases:
+        want_det, want_E, zs = orc.ge_determinant(M, eps=eps)
+        with Ctx() as c:
+            got, ok, E, minpiv = run_ge(c, M, eps=eps)
+            assert ok == (zs < 0), (M.shape, eps)
+            assert bits_equal(np.array([got]), np.array([want_det])), (got, want_det)      # incl. the sign of a zero
+            assert bits_equal(np.ascontiguousarray(E), want_E)                               # eliminated up to the zero step, untouched after it
+            if zs >= 0:
+                assert minpiv <= eps
     with Ctx() as c:
-        M = np.array([[1e-9, 1.0], [1.0, 1.0]])                             # approximately zero with an explicit eps
-        assert orc.ge_determinant(M, eps=1e-6)[0] == 0.0
-        got, ok, _, _ = run_ge(c, M, eps=1e-6)
-        assert got == 0.0 and not ok
+        M = np.array([[1e-9, 1.0], [1.0, 1.0]])
         got, ok, _, _ = run_ge(c, M, eps=0.0)                               # eps = 0: the tiny pivot is accepted
         assert ok and bits_equal(np.array([got]), np.array([orc.ge_determinant(M)[0]]))
+
+
+# ----------------------------------------------------------------------------------------------------------
+# plan hazards and context robustness on the device (round-1 review)
+# ----------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("mode", ["template", "bytecode"])
+@pytest.mark.parametrize("n", [2, 33, 1025, (1 << 20) + 3, 1 << 22])
+def test_neighbour_contract_then_inplace_update_reads_the_old_values(mode, n):
+    """require x.is_sorted; x *= -1 in place.  x[i+1] is read by another thread / warp / block than the one that overwrites it: the
+    update must run in a LATER pass.  With both in one pass the contract sees a mix of old and new values (sorted -> unsorted)."""
+    x = inputs.sorted_cumsum_f32(4, 0, n)
+    with Ctx(MODES[mode]) as c:
+        t = dev(x); c.keep.append(t)
+        hx = sg.sg_vec_create(c.ctx, sg.SG_F32, n, t.data_ptr())
+        srt = sg.sg_forall_adjacent(c.ctx, hx, sg.SG_LE)
+        ge0 = sg.sg_enqueue(c.ctx, sg.SG_GE, [hx, sg.F(0.0)])
+        pre = sg.sg_forall(c.ctx, ge0)
+        sg.sg_release(c.ctx, ge0)
+        sg.sg_enqueue(c.ctx, sg.SG_MUL, [hx, sg.F(-1.0)], dst_or_0=hx)
+        assert c.get(srt) is True and c.get(pre) is True
+        assert sg.sg_plan_stats(c.ctx).n_passes == 2
+        got = c.read_vec(hx, np.float32, n)
+    assert bits_equal(got, orc.scalar("mul", x, -1.0))
+
+
+def test_release_before_flush_on_the_device():
+    n = (1 << 16) + 5
+    a = RNG.standard_normal(n).astype(np.float32)
+    with Ctx() as c:
+        x = sg.sg_vec_create(c.ctx, sg.SG_F32, n, None)                 # context-owned storage, filled by a pass
+        ha = c.vec(a)
+        sg.sg_enqueue(c.ctx, sg.SG_ADD, [ha, sg.F(0.0)], dst_or_0=x)
+        sg.sg_flush(c.ctx)
+        y = sg.sg_enqueue(c.ctx, sg.SG_ADD, [x, sg.F(1.0)])
+        sg.sg_release(c.ctx, x)                                         # released while y = x + 1 is pending
+        s = sg.sg_reduce(c.ctx, y, sg.SG_SUM)
+        got_s = c.get(s)
+        q = sg.sg_enqueue(c.ctx, sg.SG_DIV, [s, sg.F(4.0)])             # a materialised scalar consumed by a new chain ...
+        sg.sg_release(c.ctx, s)                                         # ... and released before the flush
+        got_q = c.read_vec(q, np.float64, 1)[0]
+        got_y = c.read_vec(y, np.float32, n)
+    want_y = orc.scalar("add", orc.scalar("add", a, 0.0), 1.0)
+    assert bits_equal(got_y, want_y)
+    assert abs(got_s - orc.sum(want_y)) <= 1e-5 * np.abs(want_y).sum() and got_q == got_s / 4.0
+
+
+def test_failed_flush_discards_and_the_context_goes_on():
+    n = 4096
+    a = RNG.standard_normal(n)
+    with Ctx() as c:
+        ha = c.vec(a)
+        sg.sg_enqueue(c.ctx, sg.SG_ADD, [ha, sg.F(1.0)], dst_or_0=ha)   # an in-place update queued in the same (failing) flush
+        many = [sg.sg_reduce(c.ctx, sg.sg_enqueue(c.ctx, sg.SG_MUL, [ha, sg.F(float(i))]), sg.SG_SUM) for i in range(200)]     # > 16 passes
+        with pytest.raises(sg.SgError) as e:
+            sg.sg_flush(c.ctx)
+        assert e.value.status == sg.SG_ERR_CAPACITY
+        assert bits_equal(c.read_vec(ha, np.float64, n), a)             # nothing ran: the in-place destination keeps its contents
+        r = sg.sg_enqueue(c.ctx, sg.SG_MUL, [ha, sg.F(3.0)])            # the context is usable
+        assert bits_equal(c.read_vec(r, np.float64, n), orc.scalar("mul", a, 3.0))
+        del many
+
+
+def test_early_exit_leaves_no_half_evaluated_quantifier_readable():
+    """A pass of quantifiers ends at the first violated registered contract.  A quantifier of the same pass that was not decided on
+    the prefix read so far is NOT evaluated: reading it is an error; one that was decided (exists already true) is final."""
+    n = 1 << 24
+    x = inputs.sorted_cumsum_f32(4, 0, n)
+    inputs.inject_unsorted(x, 1000)                                     # the violation sits at the very beginning
+    with Ctx() as c:
+        t = dev(x); c.keep.append(t)
+        hx = sg.sg_vec_create(c.ctx, sg.SG_F32, n, t.data_ptr())
+        srt = sg.sg_forall_adjacent(c.ctx, hx, sg.SG_LE)
+        sg.sg_contract(c.ctx, srt, sg.SG_CONTRACT_PRE, "is_sorted")
+        big = sg.sg_enqueue(c.ctx, sg.SG_GT, [hx, sg.F(float(x[n - 1]) * 0.999)])      # witnesses only at the far end
+        ex_far = sg.sg_exists(c.ctx, big)
+        small = sg.sg_enqueue(c.ctx, sg.SG_LT, [hx, sg.F(float(x[10]))])               # witnesses at the very beginning
+        ex_near = sg.sg_exists(c.ctx, small)
+        with pytest.raises(sg.SgError) as e:
+            sg.sg_flush(c.ctx)
+        assert e.value.status == sg.SG_ERR_CONTRACT and "is_sorted" in str(e.value)
+        assert c.get(srt) is False
+        # ex_far: true on the whole vector; after the early exit it is either decided (the pass got that far) or not evaluated — never a wrong False
+        try:
+            assert c.get(ex_far) is True
+        except sg.SgError as err:
+            assert err.status == sg.SG_ERR_CONTRACT and "not evaluated" in str(err)
+        try:
+            assert c.get(ex_near) is True
+        except sg.SgError as err:
+            assert err.status == sg.SG_ERR_CONTRACT
+    with Ctx(sg.SG_FLAG_NO_EARLY_EXIT) as c:                            # without early exit everything is evaluated
+        t = dev(x); c.keep.append(t)
+        hx = sg.sg_vec_create(c.ctx, sg.SG_F32, n, t.data_ptr())
+        srt = sg.sg_forall_adjacent(c.ctx, hx, sg.SG_LE)
+        sg.sg_contract(c.ctx, srt, sg.SG_CONTRACT_PRE, "is_sorted")
+        big = sg.sg_enqueue(c.ctx, sg.SG_GT, [hx, sg.F(float(x[n - 1]) * 0.999)])
+        ex_far = sg.sg_exists(c.ctx, big)
+        with pytest.raises(sg.SgError):
+            sg.sg_flush(c.ctx)
+        assert c.get(ex_far) is True and c.get(srt) is False

@@ -136,22 +136,49 @@ def test_cfg1_to_cfg4_plans():
     assert st.bytes_min == 8 * rows + 8 * rows + (2 * 8 * rows * 16384 + 8 * 16384 + 8 * rows) + 8 * rows + 8 * 16384
 
 
+def test_ge_loop_entry_point_checks_its_arguments():
+    """sg_mat_ge_steps: the whole loop of Listing 5 as one composite call (a persistent kernel on a device; nothing on a plan-only context)."""
+    ctx = sg.sg_ctx_create(-1)
+    try:
+        n = 64
+        M = sg.sg_mat_create(ctx, sg.SG_F64, n, n, n, None)
+        det = sg.sg_vec_create(ctx, sg.SG_F64, 1, None)
+        mp = sg.sg_vec_create(ctx, sg.SG_F64, 1, None)
+        before = sg.sg_plan_stats(ctx).launches_total
+        sg.sg_mat_ge_steps(ctx, M, det, mp, 0.0, 0, n)
+        assert sg.sg_plan_stats(ctx).launches_total == before + 1          # ONE launch for n steps
+        for bad in (dict(eps=-1.0), dict(eps=float("nan")), dict(k0=-1), dict(k1=n + 1), dict(k0=5, k1=4)):
+            kw = dict(eps=0.0, k0=0, k1=n)
+            kw.update(bad)
+            with pytest.raises(sg.SgError) as e:
+                sg.sg_mat_ge_steps(ctx, M, det, mp, kw["eps"], kw["k0"], kw["k1"])
+            assert e.value.status == sg.SG_ERR_ARG
+        with pytest.raises(sg.SgError) as e:
+            sg.sg_mat_ge_steps(ctx, sg.sg_mat_create(ctx, sg.SG_F64, 4, 6, 6, None), det, mp, 0.0, 0, 4)
+        assert e.value.status == sg.SG_ERR_SHAPE
+        with pytest.raises(sg.SgError) as e:
+            sg.sg_mat_ge_steps(ctx, sg.sg_mat_create(ctx, sg.SG_F32, 4, 4, 4, None), det, mp, 0.0, 0, 4)
+        assert e.value.status == sg.SG_ERR_DTYPE
+        with pytest.raises(sg.SgError) as e:
+            sg.sg_mat_ge_steps(ctx, M, sg.sg_vec_create(ctx, sg.SG_F64, 2, None), mp, 0.0, 0, n)
+        assert e.value.status == sg.SG_ERR_SHAPE
+    finally:
+        sg.sg_ctx_destroy(ctx)
+
+
 def test_ge_step_is_two_passes_with_no_read_back():
     """Listing 5's loop body: the paper launches one kernel per row and reads two scalars back per
     row (its slow case); here a step is a scalar + factor pass and ONE matrix pass over all rows."""
-    def step(k, native=False):
+    def step(k):
         def build(c):
             M = sg.sg_mat_create(c, sg.SG_F64, 1000, 1000, 1000, None)
             det, mp = sg.sg_vec_create(c, sg.SG_F64, 1, None), sg.sg_vec_create(c, sg.SG_F64, 1, None)
-            if native:
-                sg.sg_mat_ge_steps(c, M, det, mp, k, k + 1)          # the library composite plans the same passes
-            else:
-                for h in W.ge_step(c, M, 1000, k, det, mp):
-                    sg.sg_release(c, h)
+            for h in W.ge_step(c, M, 1000, k, det, mp):
+                sg.sg_release(c, h)
         return build
     rows = 989
-    for native in (False, True):
-        st, dumps = plan(step(10, native))
+    for _ in (0,):
+        st, dumps = plan(step(10))
         # det, min |pivot| and the factors share one pass (values of different lengths; it has no precompiled instance and runs
         # on the bytecode kernel); the rows change in place in the second (template instance)
         assert st.n_passes == 2 and st.n_template == 1
@@ -163,7 +190,8 @@ def test_ge_step_is_two_passes_with_no_read_back():
     def far(c):                                                       # factor column much longer than one element: three passes, all instances
         M = sg.sg_mat_create(c, sg.SG_F64, 4096, 4096, 4096, None)
         det, mp = sg.sg_vec_create(c, sg.SG_F64, 1, None), sg.sg_vec_create(c, sg.SG_F64, 1, None)
-        sg.sg_mat_ge_steps(c, M, det, mp, 6, 7)
+        for h in W.ge_step(c, M, 4096, 6, det, mp):
+            sg.sg_release(c, h)
     st, dumps = plan(far)
     assert st.n_passes == 3 and st.n_template == 3
 
@@ -278,10 +306,13 @@ def test_sqrt_and_scalar_only_operands_are_checked_at_enqueue():
     try:
         vi = sg.sg_vec_create(ctx, sg.SG_I32, 8, None)
         vb = sg.sg_enqueue(ctx, sg.SG_GT, [vi, sg.I(0)])
-        for h in (vi, vb):
-            with pytest.raises(sg.SgError) as e:
-                sg.sg_enqueue(ctx, sg.SG_SQRT, [h])
-            assert e.value.status == sg.SG_ERR_DTYPE
+        with pytest.raises(sg.SgError) as e:
+            sg.sg_enqueue(ctx, sg.SG_SQRT, [vb])               # BOOL: undefined
+        assert e.value.status == sg.SG_ERR_DTYPE
+        mi = sg.sg_mat_create(ctx, sg.SG_I32, 4, 4, 4, None)
+        with pytest.raises(sg.SgError) as e:
+            sg.sg_enqueue(ctx, sg.SG_SQRT, [mi])               # integer MATRIX: the promoting form is a vector operation
+        assert e.value.status == sg.SG_ERR_DTYPE
         with pytest.raises(sg.SgError) as e:
             sg.sg_enqueue(ctx, 18, [vi])                       # reserved op code
         assert e.value.status == sg.SG_ERR_ARG
@@ -292,5 +323,112 @@ def test_sqrt_and_scalar_only_operands_are_checked_at_enqueue():
         s = sg.sg_reduce(ctx, vf, sg.SG_SUM)
         r = sg.sg_enqueue(ctx, sg.SG_DIV, [s, sg.F(8.0)])
         assert sg.sg_vec_count(ctx, r) == 1                    # device scalars only -> a one-element vector
+    finally:
+        sg.sg_ctx_destroy(ctx)
+
+
+# ----------------------------------------------------------------------------------------------------------
+# dtype-changing project: the conversion happens at load, inside the consumer's pass
+# ----------------------------------------------------------------------------------------------------------
+def test_integer_sqrt_is_one_pass_with_a_converting_load():
+    n = 1 << 16
+    st, dumps = plan(lambda c: sg.sg_enqueue(c, sg.SG_SQRT, [sg.sg_vec_create(c, sg.SG_I32, n, None)]))
+    assert st.n_passes == 1 and "IN_VEC_CVT,2" in dumps[0] and "OP_SQRT" in dumps[0] and "DT_F64" in dumps[0]
+    assert st.bytes_min == 4 * n + 8 * n                     # int32 read once, double written once: 12 B per element
+
+    def chain(c):                                           # a PENDING integer operand is stored first: a pass has one value type
+        x = sg.sg_vec_create(c, sg.SG_I32, n, None)
+        y = sg.sg_enqueue(c, sg.SG_ADD, [x, sg.I(1)])
+        f = sg.sg_cast(c, y, sg.SG_F32)
+        sg.sg_release(c, y)
+        return sg.sg_reduce(c, f, sg.SG_SUM)
+    st, dumps = plan(chain)
+    assert st.n_passes == 2 and "DT_I32" in dumps[0] and "OUT_STORE" in dumps[0] and "DT_F32" in dumps[1] and "IN_VEC_CVT,2" in dumps[1]
+    ctx = sg.sg_ctx_create(-1)
+    try:
+        x = sg.sg_vec_create(ctx, sg.SG_F64, 8, None)
+        assert sg.sg_vec_count(ctx, sg.sg_cast(ctx, x, sg.SG_I64)) == 8
+        with pytest.raises(sg.SgError) as e:
+            sg.sg_cast(ctx, x, sg.SG_BOOL)
+        assert e.value.status == sg.SG_ERR_DTYPE
+        with pytest.raises(sg.SgError) as e:
+            sg.sg_cast(ctx, sg.sg_mat_create(ctx, sg.SG_F64, 2, 2, 2, None), sg.SG_F32)
+        assert e.value.status == sg.SG_ERR_UNSUPPORTED
+        with pytest.raises(sg.SgError) as e:
+            sg.sg_reduce(ctx, x, sg.SG_SUM, acc=sg.SG_F32)   # a narrower accumulator is rejected, not emulated
+        assert e.value.status == sg.SG_ERR_DTYPE
+        sg.sg_reduce(ctx, x, sg.SG_SUM, acc=sg.SG_F64)
+        sg.sg_reduce(ctx, x, sg.SG_RMAX, acc=sg.SG_F64)
+    finally:
+        sg.sg_ctx_destroy(ctx)
+
+
+# ----------------------------------------------------------------------------------------------------------
+# plan hazards and context robustness (round-1 review)
+# ----------------------------------------------------------------------------------------------------------
+def test_inplace_update_never_shares_a_pass_with_a_neighbour_read_of_the_same_storage():
+    """is_sorted(x) reads x[i+1], which belongs to another thread / warp / block: x *= 2 in place must wait for that pass."""
+    n = 1 << 16
+
+    def prog(c):
+        x = sg.sg_vec_create(c, sg.SG_F32, n, None)
+        srt = sg.sg_forall_adjacent(c, x, sg.SG_LE)
+        sg.sg_enqueue(c, sg.SG_MUL, [x, sg.F(2.0)], dst_or_0=x)
+        return srt
+    st, dumps = plan(prog)
+    assert st.n_passes == 2
+    assert "IN_SHIFT" in dumps[0] and "OUT_STORE" not in dumps[0] and "OUT_STORE" in dumps[1]
+
+    def prog2(c):                                           # an index-for-index reader of the same view still fuses (PAPER.md:315-322)
+        x = sg.sg_vec_create(c, sg.SG_F32, n, None)
+        pos = sg.sg_enqueue(c, sg.SG_GE, [x, sg.F(0.0)])
+        ok = sg.sg_forall(c, pos)
+        sg.sg_release(c, pos)
+        sg.sg_enqueue(c, sg.SG_MUL, [x, sg.F(2.0)], dst_or_0=x)
+        return ok
+    st, dumps = plan(prog2)
+    assert st.n_passes == 1 and "OUT_ALL" in dumps[0] and "OUT_STORE" in dumps[0]
+
+
+def test_release_before_flush_keeps_storage_for_pending_readers():
+    ctx = sg.sg_ctx_create(-1)
+    try:
+        x = sg.sg_vec_create(ctx, sg.SG_F32, 1024, None)     # context-owned storage
+        y = sg.sg_enqueue(ctx, sg.SG_ADD, [x, sg.F(1.0)])
+        sg.sg_release(ctx, x)                               # released while y = x + 1 is pending
+        sg.sg_flush(ctx)
+        assert sg.sg_plan_stats(ctx).n_passes == 1
+        s = sg.sg_reduce(ctx, y, sg.SG_SUM)
+        sg.sg_flush(ctx)
+        a = sg.sg_enqueue(ctx, sg.SG_DIV, [s, sg.F(4.0)])    # a materialised scalar consumed by a new chain ...
+        sg.sg_release(ctx, s)                               # ... and released before the flush
+        sg.sg_flush(ctx)
+        assert sg.sg_plan_stats(ctx).n_passes == 1 and sg.sg_vec_count(ctx, a) == 1
+    finally:
+        sg.sg_ctx_destroy(ctx)
+
+
+def test_a_failed_flush_discards_the_pending_list_and_leaves_the_context_usable():
+    ctx = sg.sg_ctx_create(-1)
+    try:
+        x = sg.sg_vec_create(ctx, sg.SG_F64, 1024, None)
+        bad = x
+        for _ in range(40):                                  # a chain longer than one pass holds (SG_MAX_INSTR) ...
+            nxt = sg.sg_enqueue(ctx, sg.SG_ADD, [bad, x])
+            if bad != x:
+                sg.sg_release(ctx, bad)
+            bad = nxt
+        pend = [sg.sg_reduce(ctx, bad, k) for k in (sg.SG_SUM, sg.SG_RMAX, sg.SG_RMIN)] * 1
+        many = [sg.sg_reduce(ctx, sg.sg_enqueue(ctx, sg.SG_MUL, [x, sg.F(float(i))]), sg.SG_SUM) for i in range(200)]   # ... and > 16 passes
+        with pytest.raises(sg.SgError) as e:
+            sg.sg_flush(ctx)
+        assert e.value.status == sg.SG_ERR_CAPACITY and "discarded" in str(e.value)
+        sg.sg_flush(ctx)                                    # nothing is pending any more: the error does not come back
+        y = sg.sg_enqueue(ctx, sg.SG_MUL, [x, sg.F(3.0)])    # unrelated later work runs
+        sg.sg_flush(ctx)
+        st = sg.sg_plan_stats(ctx)
+        assert st.n_passes == 1 and st.n_nodes == 1 and sg.sg_vec_count(ctx, y) == 1024
+        for h in pend + many:
+            sg.sg_release(ctx, h)
     finally:
         sg.sg_ctx_destroy(ctx)
