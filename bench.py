@@ -232,11 +232,12 @@ def cfg3_section(torch, sg, W, inputs, measure):
 
 
 def ge_section(torch, sg, W, inputs, out, peak):
-    """the whole determinant loop of Listing 5 (n steps, 3 launches each, no host synchronisation between
-    steps), device time between two events around the loop.  Algorithmic bytes: step k reads and writes the (n-k-1) x n rows
-    below the pivot row (16 B per updated element), plus the pivot row and the factor column."""
+    """the whole determinant loop of Listing 5.  native: sg_mat_ge_steps, ONE persistent kernel for all n steps
+    (no host in the loop).  host-issued: the same steps as primitives, 3 launches per step (the paper's slow case).
+    Device time between two events around the loop.  Algorithmic bytes: step k reads and writes the (n-k-1) x n rows below the
+    pivot row (16 B per updated element), plus the pivot row and the factor column."""
     stream = torch.cuda.current_stream().cuda_stream
-    for n in (4096, 8192):
+    for n, native in ((4096, True), (8192, True), (2048, True), (2048, False)):
         M0 = torch.from_numpy(inputs.boosted_matrix_f64(5, 0, n) / float(n)).cuda()
         M = M0.clone()
         alg = sum(16 * (n - k - 1) * n + 8 * n + 24 * (n - k - 1) + 40 for k in range(n))
@@ -251,16 +252,18 @@ def ge_section(torch, sg, W, inputs, out, peak):
             torch.cuda.synchronize()
             t0 = time.perf_counter()
             e0.record()
-            det, ok = W.ge_determinant(ctx, n, M.data_ptr(), d.data_ptr(), mp.data_ptr())
+            det, ok = W.ge_determinant(ctx, n, M.data_ptr(), d.data_ptr(), mp.data_ptr(), native=native)
             e1.record()
             torch.cuda.synchronize()
             wall.append(1e3 * (time.perf_counter() - t0))
             times.append(e0.elapsed_time(e1))
+            launches = sg.sg_plan_stats(ctx).launches_total
             sg.sg_ctx_destroy(ctx)
         ms = float(min(times[1:]))
-        out[f"ge_determinant_fp64_{n}^2_whole_loop ({n} steps, 3 launches each, no host sync)"] = {
+        how = "one persistent kernel, no host in the loop" if native else "host-issued primitives, 3 launches per step"
+        out[f"ge_determinant_fp64_{n}^2_whole_loop ({n} steps, {how})"] = {
             "ms": ms, "wall_ms": float(min(wall[1:])), "algorithmic_bytes": int(alg), "GB/s": alg / ms / 1e6, "frac_of_peak": alg / ms / 1e6 / peak,
-            "passes": 3 * n - 2, "template_passes": 3 * n - 2, "det": det, "launches_per_step": 3}
+            "launches": int(launches), "det": det, "note": "the matrix (8 n^2 bytes) fits the 126 MB L2 for n <= 3968: fractions above 1 are L2 hits, not HBM"}
 
 
 def vecapi_section(torch, sg, W, inputs, measure):
@@ -308,10 +311,34 @@ def matvec_section(torch, sg, W, inputs, measure):
 
 
 def quicksort_section(torch, sg, W, inputs, out):
-    """Listing 3 on fp32 normal(0,1) keys; wall time of the whole sort (one count read-back per partition).
-    Launch- and latency-bound by construction (the listing recurses down to single elements): reported, not a roofline line."""
+    """Listing 3 on fp32 normal(0,1) keys.  levels: sg_vec_quicksort, one segmented three-way partition launch per
+    recursion level (device time between two events around the whole sort, incl. the read-backs of the done flag).  host recursion:
+    the listing written over sg_filter calls, one partition at a time (wall time; the round-1 path, kept as the baseline)."""
     stream = torch.cuda.current_stream().cuda_stream
-    for log2n in (12, 14):
+    for log2n in (20, 24):
+        n = 1 << log2n
+        a = torch.from_numpy(inputs.normal_f32(2, 0, n)).cuda()
+        o = torch.empty_like(a)
+        best, launches = None, 0
+        for rep in range(3):
+            ctx = sg.sg_ctx_create(0, stream)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            torch.cuda.synchronize()
+            e0.record()
+            r = W.quicksort_levels(ctx, sg.SG_F32, n, a.data_ptr(), o.data_ptr())
+            ok = sg.sg_scalar_get(ctx, r["sorted"])
+            e1.record()
+            torch.cuda.synchronize()
+            ms = e0.elapsed_time(e1)
+            launches = sg.sg_plan_stats(ctx).launches_total
+            sg.sg_ctx_destroy(ctx)
+            best = ms if best is None else min(best, ms)
+        levels = max(launches - 2, 1)           # init + levels + the is_sorted pass
+        out[f"quicksort_levels_fp32_2^{log2n} (sg_vec_quicksort: one launch per recursion level, is_sorted contract included)"] = {
+            "ms": best, "launches": int(launches), "sorted": bool(ok), "elements/s": n / best * 1e3,
+            "GB/s_per_level_upper_bound": 8.0 * n / (best / levels) / 1e6,
+            "note": "a level reads and writes at most 4 B per key each; deep levels touch only the keys not yet placed"}
+    for log2n in (12,):
         n = 1 << log2n
         a = torch.from_numpy(inputs.normal_f32(2, 0, n)).cuda()
         o, s0, s1 = (torch.empty_like(a) for _ in range(3))
@@ -326,7 +353,8 @@ def quicksort_section(torch, sg, W, inputs, out):
             ms = 1e3 * (time.perf_counter() - t0)
             sg.sg_ctx_destroy(ctx)
             best, parts = (ms if best is None else min(best, ms)), r["partitions"]
-        out[f"quicksort_listing3_fp32_2^{log2n} (wall, whole sort)"] = {"ms": best, "partitions": parts, "sorted": bool(ok), "elements/s": n / best * 1e3}
+        out[f"quicksort_host_recursion_fp32_2^{log2n} (Listing 3 over sg_filter calls, one partition at a time; wall)"] = {
+            "ms": best, "partitions": parts, "sorted": bool(ok), "elements/s": n / best * 1e3}
 
 
 def cfg4_section(torch, sg, W, inputs, measure):

@@ -232,6 +232,19 @@ sg_status sg_mat_transpose(sg_ctx* ctx, sg_handle m, void* dev_out_or_null, int6
  * SG_ERR_CUDA. */
 sg_status sg_mat_ge_steps(sg_ctx* ctx, sg_handle m, sg_handle det, sg_handle minpiv, double eps, int64_t k0, int64_t k1);
 
+/* Listing 3's quicksort as a library composite: Result = quicksort(left) ++ mid ++
+ * quicksort(right) with pivot a[a.count // 2] and the three STABLE filters item < / = / > pivot, so the result is the stable sort
+ * of v (equal keys, -0 and +0 included, keep their order).  One launch per recursion LEVEL: every partition of a level is a
+ * segment of one buffer, a tile is read once and its three compactions are written in the same pass (multi-output partition,
+ * ranks by one decoupled look-back chain per segment), `concatenate` is free (left and right are written at their final
+ * offsets); segments that fit one block are finished in shared memory.  Counts and segment tables stay on the device; the host
+ * reads 20 bytes per batch of levels to learn whether work is left.  *out is a NEW vector (dev_out_or_null: caller's buffer of
+ * v.count elements, else allocated by the context); v is not modified.  Not deferred: pending operations are flushed first.
+ * Errors: SG_ERR_EMPTY (the listing's precondition a.count > 0), SG_ERR_DTYPE (BOOL), SG_ERR_ARG (not a unit-stride vector),
+ * SG_ERR_ALIAS (dev_out overlaps v), SG_ERR_OOM, SG_ERR_CUDA, and SG_ERR_CONTRACT when a key is neither <, = nor > its pivot (a
+ * NaN): the listing's three filters would drop it and violate its own postcondition Result.count = a.count. */
+sg_status sg_vec_quicksort(sg_ctx* ctx, sg_handle v, void* dev_out_or_null, sg_handle* out);
+
 sg_status sg_plan_stats(sg_ctx* ctx, sg_stats* out);
 /* Canonical program of pass `pass` of the last flush as text (template generator, tests). Returns bytes needed. */
 int64_t sg_plan_dump(sg_ctx* ctx, int32_t pass, char* buf, int64_t cap);

@@ -16,7 +16,7 @@ CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libsafegpu.so")
 NSHARDS = 8        # == SG_NSHARDS in csrc/sg_tmpl_launch.cuh: the template instances compile as eight translation units in parallel
-SOURCES = [f"sg_vm_shard.cu@{k}" for k in range(4)] + [f"sg_tmpl_shard.cu@{k}" for k in range(NSHARDS)] + ["sg_kernels.cu", "sg_api.cpp", "sg_plan.cpp", "sg_build.cpp", "sg_transpose.cu", "sg_ge.cu"]
+SOURCES = [f"sg_vm_shard.cu@{k}" for k in range(4)] + [f"sg_tmpl_shard.cu@{k}" for k in range(NSHARDS)] + ["sg_kernels.cu", "sg_api.cpp", "sg_plan.cpp", "sg_build.cpp", "sg_transpose.cu", "sg_ge.cu", "sg_sort.cu"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-fmad=false", "-std=c++17",
@@ -39,7 +39,7 @@ def _stamp() -> str:
 def _dep_hash(src: str) -> str:
     """Hash of what an object depends on: its source, the flags, include/sg.h and every header in csrc/ it may include
     (host .cpp files never include the kernel headers .cuh / .inc; sg_transpose.cu includes only sg_kernels.h / sg_prog.h)."""
-    light = src.endswith(".cpp") or src in ("sg_transpose.cu", "sg_ge.cu")
+    light = src.endswith(".cpp") or src in ("sg_transpose.cu", "sg_ge.cu", "sg_sort.cu")
     h = hashlib.sha256()
     for name in sorted(os.listdir(CSRC)):
         if name == src or name.endswith(".h") or (not light and name.endswith((".cuh", ".inc"))):

@@ -611,6 +611,55 @@ sg_status sg_mat_ge_steps(sg_ctx* c, sg_handle m, sg_handle det, sg_handle minpi
     return SG_OK;
 }
 
+// Listing 3 as a library composite: one segmented three-way partition launch per recursion level (sg_sort.cu).
+sg_status sg_vec_quicksort(sg_ctx* c, sg_handle v, void* dev_out, sg_handle* out) {
+    CK(c && out);
+    SgDeviceScope dev_scope(c);
+    sg_status s;
+    if (!c->nodes.empty() && (s = sg_flush_impl(c)) != SG_OK) return s;     // not part of the pending list: everything pending runs first
+    Value* a;
+    if ((s = need_storage(c, v, &a)) != SG_OK) return s;
+    if ((s = resolve_count(c, a)) != SG_OK) return s;
+    if (a->kind != VK_VEC || a->stride != 1) return sg_fail(c, SG_ERR_ARG, "quicksort needs a unit-stride vector");
+    if (a->dtype == SG_BOOL) return sg_fail(c, SG_ERR_DTYPE, "quicksort of a BOOL collection");
+    const int64_t n = a->cols;
+    if (n <= 0) return sg_fail(c, SG_ERR_EMPTY, "quicksort: require a.count > 0 (PAPER.md:248)");
+    const int es = dtype_size(a->dtype);
+    const char* src = a->ptr;
+    const int dtype = a->dtype;
+    if (dev_out) {
+        const char* b0 = (const char*)dev_out;
+        if (src < b0 + (size_t)n * es && b0 < src + (size_t)n * es) return sg_fail(c, SG_ERR_ALIAS, "quicksort output overlaps its input");
+    }
+    sg_handle h;
+    if ((s = sg_vec_create(c, (sg_dtype)dtype, n, dev_out, &h)) != SG_OK) return s;     // may reallocate the handle table: `a` is stale now
+    if (c->plan_only) { c->stats.launches_total += 2; *out = h; return SG_OK; }
+    const size_t ws_bytes = sgk_quicksort_workspace_bytes(n, es);
+    void* ws = sg_dev_alloc(c, ws_bytes);
+    if (!ws) { sg_release(c, h); return sg_fail(c, SG_ERR_OOM, "quicksort workspace allocation failed"); }
+    const int64_t slot = sg_slot_alloc(c);          // four pinned 8-byte slots' worth of read-back words
+    int64_t slots[4] = {slot, -1, -1, -1};
+    bool contiguous = slot >= 0;
+    for (int i = 1; i < 4 && contiguous; ++i) { slots[i] = sg_slot_alloc(c); contiguous = slots[i] == slot + i; }
+    unsigned int* host_flag = contiguous ? reinterpret_cast<unsigned int*>(c->slab_host + 8 * slot) : nullptr;
+    unsigned int local_flag[8] = {0};
+    int launches = 0;
+    unsigned int error = 0;
+    const cudaError_t e = sgk_quicksort(dtype, src, val(c, h)->ptr, n, ws, c->sm_count, host_flag ? host_flag : local_flag, c->stream, &launches, &error);
+    for (int i = 0; i < 4; ++i)
+        if (slots[i] >= 0) c->slab_free.push_back(slots[i]);
+    c->deferred_free.push_back((char*)ws);
+    c->stats.launches_total += launches;
+    if (e != cudaSuccess) { cudaGetLastError(); sg_release(c, h); return sg_fail(c, SG_ERR_CUDA, std::string("quicksort failed: ") + cudaGetErrorString(e)); }
+    if (error & 2u) { sg_release(c, h); return sg_fail(c, SG_ERR_CAPACITY, "quicksort: segment table overflow"); }
+    if (error & 1u) {
+        sg_release(c, h);
+        return sg_fail(c, SG_ERR_CONTRACT, "postcondition violated: Result.count = a.count (a key is neither <, = nor > its pivot: NaN)");
+    }
+    *out = h;
+    return SG_OK;
+}
+
 sg_status sg_scalar_dtype(sg_ctx* c, sg_handle h, int32_t* dtype) {
     CK(c && dtype);
     Value* v = val(c, h);

@@ -39,4 +39,10 @@ cudaError_t sgk_transpose(const void* in, int64_t ld_in, int64_t rows, int64_t c
 cudaError_t sgk_ge_loop(double* M, int64_t n, int64_t ld, double* det, double* minpiv, double eps, int64_t k0, int64_t k1, unsigned int* ready, int sm_count,
                         cudaStream_t stream, int* launched_grid);
 
+// sg_sort.cu: Listing 3's quicksort, one recursion level per launch over a device-side segment table (DT_* dtype; device pointers;
+// workspace of sgk_quicksort_workspace_bytes; host_flag: 8 pinned 32-bit words).  *error bit 0: a key matched none of <, =, > (NaN).
+size_t sgk_quicksort_workspace_bytes(int64_t n, int elem_size);
+cudaError_t sgk_quicksort(int dtype, const void* in, void* out, int64_t n, void* workspace, int sm_count, unsigned int* host_flag, cudaStream_t stream,
+                          int* launches, unsigned int* error);
+
 #endif  // SG_KERNELS_H_

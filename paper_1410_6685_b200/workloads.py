@@ -215,7 +215,7 @@ def ge_determinant(ctx, n, pM, pdet, pminpiv, ld=None, eps=0.0, native=True):
             sg.sg_flush(ctx)                                    # asynchronous: plan + launches of step k, no read-back
     gt = sg.sg_enqueue(ctx, sg.SG_GT, [minpiv, F(eps)])
     ok = sg.sg_forall(ctx, gt)
-    value = sg.sg_reduce(ctx, det, sg.SG_SUM)                   # sum of one element: hands the scalar back (trigger (1))
+    value = sg.sg_reduce(ctx, det, sg.SG_RMAX)                  # max of one element = the element, bit for bit (a sum would turn -0 into +0): hands the scalar back (trigger (1))
     okv = bool(sg.sg_scalar_get(ctx, ok))
     detv = float(sg.sg_scalar_get(ctx, value))
     for h in (gt, ok, value, det, minpiv, M):
@@ -367,6 +367,21 @@ def quicksort(ctx, dtype, n, pa, pout, pscratch0, pscratch1, contracts=True):
     if contracts:
         if placed != n:
             raise AssertionError(f"quicksort postcondition Result.count = a.count violated: {placed} != {n}")
+        res["sorted"] = sg.sg_forall_adjacent(ctx, out, sg.SG_LE)
+        sg.sg_contract(ctx, res["sorted"], sg.SG_CONTRACT_POST, "Result.is_sorted")
+    return res
+
+
+def quicksort_levels(ctx, dtype, n, pa, pout=None, contracts=True):
+    """Listing 3 through the library composite sg_vec_quicksort: one segmented three-way partition launch per recursion level (the
+    multi-output partition kernel), counts and segment tables stay on the device.  The listing's postconditions: Result.is_sorted
+    as a registered device contract; Result.count = a.count is a scalar contract (O(1))."""
+    a = sg.sg_vec_create(ctx, dtype, n, pa)
+    out = sg.sg_vec_quicksort(ctx, a, pout)
+    res = {"a": a, "out": out}
+    if contracts:
+        if sg.sg_vec_count(ctx, out) != n:
+            raise AssertionError("quicksort postcondition Result.count = a.count violated")
         res["sorted"] = sg.sg_forall_adjacent(ctx, out, sg.SG_LE)
         sg.sg_contract(ctx, res["sorted"], sg.SG_CONTRACT_POST, "Result.is_sorted")
     return res

@@ -184,6 +184,81 @@ def test_quicksort_signed_zeros_sorted_input_fp64_and_bytecode():
         assert ok and bits_equal(got, ocfg.quicksort(a))
 
 
+def _quicksort_levels(a, pout=False):
+    from gpu_util import NP2SG
+    n = a.size
+    with Ctx() as c:
+        ta = dev(a); c.keep.append(ta)
+        before = ta.clone()
+        tout = empty_dev(max(n, 1), a.dtype) if pout else None
+        if tout is not None:
+            c.keep.append(tout)
+        r = W.quicksort_levels(c.ctx, NP2SG[a.dtype], n, ta.data_ptr(), tout.data_ptr() if pout else None)
+        ok = c.get(r["sorted"])
+        got = c.read_vec(r["out"], a.dtype, n)
+        launches = sg.sg_plan_stats(c.ctx).launches_total
+        assert bits_equal(before.cpu().numpy(), ta.cpu().numpy())          # the argument is not modified
+    return got, ok, launches
+
+
+@pytest.mark.parametrize("dtype", [np.float32, np.float64, np.int32, np.int64])
+@pytest.mark.parametrize("n", [1, 2, 3, 17, 1000, 2047, 2048, 2049, 4099, 20011, 65536 + 3])
+def test_quicksort_levels_against_the_listing(dtype, n):
+    """sg_vec_quicksort (one segmented three-way partition launch per recursion level) against the oracle's Listing-3 recursion: random
+    keys, few distinct keys (long `=` runs: the staged mid copies), bit for bit (stable filters make the result unique)."""
+    for a in ((RNG.standard_normal(n) * 1000).astype(dtype), RNG.integers(-50, 51, n).astype(dtype)):
+        got, ok, _ = _quicksort_levels(a, pout=(n % 2 == 0))
+        assert ok is True and bits_equal(got, ocfg.quicksort(a))
+
+
+def test_quicksort_levels_structured_inputs():
+    n = 50000
+    base = np.arange(n, dtype=np.float64)
+    cases = [base, base[::-1].copy(), np.zeros(n), np.where(np.arange(n) % 2 == 0, 0.0, -0.0), np.concatenate([base[: n // 2], base[: n // 2]]),
+             np.repeat(np.arange(5, dtype=np.float64), n // 5)[::-1].copy()]
+    z = RNG.integers(-3, 4, n).astype(np.float32)
+    z[z == 0] = np.where(RNG.random((z == 0).sum()) < 0.5, np.float32(0.0), np.float32(-0.0))      # +0 and -0 keep their order (equal keys)
+    cases.append(z)
+    for a in cases:
+        got, ok, _ = _quicksort_levels(a)
+        assert ok is True and bits_equal(got, ocfg.quicksort(a)) and bits_equal(got, np.sort(a, kind="stable"))
+
+
+def test_quicksort_levels_large_and_contracts():
+    """2^20 + 7 fp32 keys: the listing's result is the stable sort (pinned for the oracle in test_oracle_pins.py at sizes the recursion
+    finishes; a property that holds at any size), compared element by element; a few dozen launches, not one per partition."""
+    n = (1 << 20) + 7
+    a = inputs_normal(n)
+    got, ok, launches = _quicksort_levels(a)
+    assert ok is True and bits_equal(got, np.sort(a, kind="stable"))
+    assert launches < 120
+    m = 1 << 16                                                             # the same kernels on a prefix the oracle's recursion finishes in seconds
+    got, ok, _ = _quicksort_levels(a[:m].copy())
+    assert ok and bits_equal(got, ocfg.quicksort(a[:m]))
+    with Ctx() as c:
+        with pytest.raises(sg.SgError) as e:                                # require a.count > 0 (PAPER.md:248)
+            sg.sg_vec_quicksort(c.ctx, sg.sg_vec_create(c.ctx, sg.SG_F32, 0, None))
+        assert e.value.status == sg.SG_ERR_EMPTY
+        for k in (5, 5000):                                                 # a NaN key is in none of the three filters: Result.count = a.count fails
+            b = a[: 3 * k].copy()
+            b[k] = np.nan
+            with pytest.raises(sg.SgError) as e:
+                sg.sg_vec_quicksort(c.ctx, c.vec(b))
+            assert e.value.status == sg.SG_ERR_CONTRACT and "Result.count" in str(e.value)
+            assert ocfg.quicksort(b).size < b.size                          # the oracle's listing drops it too
+        one = c.vec(np.array([np.nan], dtype=np.float32))                   # a.count = 1: Result := a, nothing is compared
+        assert np.isnan(c.read_vec(sg.sg_vec_quicksort(c.ctx, one), np.float32, 1)[0])
+        t = dev(a[:1000]); c.keep.append(t)
+        with pytest.raises(sg.SgError) as e:
+            sg.sg_vec_quicksort(c.ctx, sg.sg_vec_create(c.ctx, sg.SG_F32, 1000, t.data_ptr()), t.data_ptr() + 400)
+        assert e.value.status == sg.SG_ERR_ALIAS
+
+
+def inputs_normal(n):
+    from paper_1410_6685_b200 import inputs
+    return inputs.normal_f32(2, 0, n)
+
+
 # ----------------------------------------------------------------------------------------------------------
 # SURVEY.md §8(f)(4): matrix-vector products (PAPER.md:217) — fp64 sums within 1e-12 relative of the oracle
 # ----------------------------------------------------------------------------------------------------------
