@@ -86,10 +86,23 @@ class ClockSampler:
 def ncu_traffic(kernel: str, n: int):
     """DRAM bytes per launch of the dominant kernel from the committed ncu --set full capture (profiles/), or None."""
     try:
-        d = json.load(open(os.path.join(ROOT, "profiles", "r01_traffic.json")))[kernel]
+        d = json.load(open(os.path.join(ROOT, "profiles", "r02_traffic.json")))[kernel]
         return d["traffic_bytes"] if d["n"] == n else None
     except Exception:
         return None
+
+
+def host_cpu():
+    """(model string, nproc) of the box the oracle is timed on."""
+    model = "unknown"
+    try:
+        for line in open("/proc/cpuinfo"):
+            if line.lower().startswith("model name"):
+                model = line.split(":", 1)[1].strip()
+                break
+    except Exception:
+        pass
+    return model, os.cpu_count()
 
 
 def oracle_chain_rate(x, y, seconds_target=8.0):
@@ -126,7 +139,8 @@ def run_reference(args):
     line = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32",
             "data": "synthetic", "config": {"workload": f"cfg1 chain fp32, oracle on a bounded sample of 2^23 elements per step (of n=2^{args.log2n})"},
-            "cpu_baseline": {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": "first 2^23 elements of the seeded x,y per step"},
+            "cpu_baseline": {"value": v, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": "first 2^23 elements of the seeded x,y per step",
+                             "cpu_model": host_cpu()[0], "nproc": host_cpu()[1]},
             "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
     print(json.dumps(line))
 
@@ -140,7 +154,7 @@ def per_config(torch, sg, W, inputs, peak, which):
     out = {}
     stream = torch.cuda.current_stream().cuda_stream
 
-    def measure(name, build, alg_bytes, reps=20, flags=0, restore=None):
+    def measure(name, build, alg_bytes, reps=20, flags=0, restore=None, graph=False):
         ctx = sg.sg_ctx_create(0, stream)
         sg.sg_ctx_set_flags(ctx, flags)
         try:
@@ -163,6 +177,9 @@ def per_config(torch, sg, W, inputs, peak, which):
             b = alg_bytes if alg_bytes else st.bytes_min
             out[name] = {"ms": ms, "algorithmic_bytes": int(b), "GB/s": b / ms / 1e6, "frac_of_peak": b / ms / 1e6 / peak, "passes": st.n_passes,
                          "template_passes": st.n_template}
+            if graph:       # sub-10 us passes: the same launches replayed from a CUDA graph, device time and launch-inclusive wall time
+                gd, gw = sg.sg_replay_last_graph(ctx, reps)
+                out[name].update({"graph_device_ms": gd, "graph_wall_ms": gw})
         finally:
             sg.sg_ctx_destroy(ctx)
 
@@ -171,6 +188,10 @@ def per_config(torch, sg, W, inputs, peak, which):
         cfg0_section(torch, sg, W, inputs, measure)
     if "cfg1" in which:
         cfg1_section(torch, sg, W, inputs, measure)
+    if "sweep" in which:
+        sweep_section(torch, sg, W, inputs, measure)
+    if "overhead" in which:
+        contract_overhead_section(torch, sg, W, inputs, measure)
     if "cfg2" in which:
         cfg2_section(torch, sg, W, inputs, measure)
     if "cfg3" in which:
@@ -192,8 +213,14 @@ def cfg0_section(torch, sg, W, inputs, measure):
     # config 0 (fits in L2: a warm number, labelled)
     n0 = 1 << 20
     a, b, c = (torch.from_numpy(inputs.uniform_pm1_f64(1, s, n0)).cuda() for s in range(3))
-    measure("cfg0_fp64_2^20_chain_sum_max_min_contracts (L2-warm, 2 passes)", lambda ctx: W.cfg0(ctx, n0, a.data_ptr(), b.data_ptr(), c.data_ptr()), 64 << 20, 200)
-    measure("cfg0_onepass (z released, L2-warm)", lambda ctx: W.cfg0(ctx, n0, a.data_ptr(), b.data_ptr(), c.data_ptr(), keep_z=False), 24 << 20, 200)
+    measure("cfg0_fp64_2^20_chain_sum_max_min_contracts (L2-warm, 2 passes)", lambda ctx: W.cfg0(ctx, n0, a.data_ptr(), b.data_ptr(), c.data_ptr()), 64 << 20, 200, graph=True)
+    measure("cfg0_onepass (z released, L2-warm)", lambda ctx: W.cfg0(ctx, n0, a.data_ptr(), b.data_ptr(), c.data_ptr(), keep_z=False), 24 << 20, 200, graph=True)
+    # the floor of ANY pass: a one-element pass (nothing to stream) — launch latency + the kernel's fixed prologue / epilogue
+    one = torch.ones(1, dtype=torch.float64, device="cuda")
+    measure("launch_floor_one_element_pass (x + 1 on a 1-element vector)",
+            lambda ctx: sg.sg_enqueue(ctx, sg.SG_ADD, [sg.sg_vec_create(ctx, sg.SG_F64, 1, one.data_ptr()), sg.F(1.0)]), 16, 200, graph=True)
+    measure("launch_floor_one_element_reduction (sum of a 1-element vector: ticket epilogue)",
+            lambda ctx: sg.sg_reduce(ctx, sg.sg_vec_create(ctx, sg.SG_F64, 1, one.data_ptr()), sg.SG_SUM), 8, 200, graph=True)
     # the same two plans with the L2 flushed before every repetition (a 256 MiB scratch buffer is overwritten outside the timed events)
     scratch = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
     measure("cfg0_fp64_2^20_chain_sum_max_min_contracts (L2-cold, 2 passes)", lambda ctx: W.cfg0(ctx, n0, a.data_ptr(), b.data_ptr(), c.data_ptr()), 64 << 20, 5,
@@ -210,6 +237,54 @@ def cfg1_section(torch, sg, W, inputs, measure):
     measure("cfg1_fp32_2^26_fused", lambda ctx: W.cfg1(ctx, n1, x.data_ptr(), y.data_ptr()), 8 * n1)
     measure("cfg1_fp32_2^26_unfused_one_kernel_per_op", lambda ctx: W.cfg1(ctx, n1, x.data_ptr(), y.data_ptr()), 0, 5, sg.SG_FLAG_UNFUSED)
     measure("cfg1_fp32_2^26_fused_bytecode", lambda ctx: W.cfg1(ctx, n1, x.data_ptr(), y.data_ptr()), 8 * n1, 5, sg.SG_FLAG_FORCE_BYTECODE)
+
+
+def sweep_section(torch, sg, W, inputs, measure):
+    """SURVEY.md §8(d) "sweep" row: config 1's chain at n = 2^16 ... 2^28 (mirrors Fig. 4's size axis).  Inputs up to 2^23
+    elements (2 x 32 MiB) fit the 126 MB L2 and are timed L2-warm (labelled); larger ones stream from HBM."""
+    n_max = 1 << 28
+    x = torch.from_numpy(inputs.normal_f32(2, 0, n_max)).cuda()
+    y = torch.from_numpy(inputs.normal_f32(2, 1, n_max)).cuda()
+    for log2n in range(16, 29, 2):
+        n = 1 << log2n
+        tag = "L2-warm" if 8 * n <= (96 << 20) else "HBM"
+        measure(f"sweep_cfg1_chain_fp32_2^{log2n} ({tag})", lambda ctx: W.cfg1(ctx, n, x.data_ptr(), y.data_ptr()), 8 * n, 50 if log2n < 24 else 20)
+
+
+def contract_overhead_section(torch, sg, W, inputs, measure):
+    """SURVEY.md §8(d) note (iv): contract overhead in the paper's sense (Table 4) = time with contracts / time of the
+    body alone.  Config 0: body = the chain + sum/max/min (z stored); contracts = pre exists(a > 0.99) fused into the body pass and post
+    for_all(z == recomputed) as its own pass over the stored z (R17).  Config 3 has no body of its own, so the body is the cheapest
+    consumer of the same vector, sum(x) (4 B per element); its two contracts (x >= 0, is_sorted) are PRE contracts of a body that writes
+    nothing in place, so they FUSE into the body's pass: one read of x for both."""
+    out = measure.out
+    n0 = 1 << 20
+    a, b, c = (torch.from_numpy(inputs.uniform_pm1_f64(1, s, n0)).cuda() for s in range(3))
+    measure("overhead_cfg0_body_only (chain + sum/max/min, L2-warm)", lambda ctx: W.cfg0(ctx, n0, a.data_ptr(), b.data_ptr(), c.data_ptr(), contracts=False), 32 << 20, 200)
+    measure("overhead_cfg0_body_and_contracts (L2-warm)", lambda ctx: W.cfg0(ctx, n0, a.data_ptr(), b.data_ptr(), c.data_ptr()), 64 << 20, 200)
+    n3 = 1 << 28
+    xs = torch.from_numpy(inputs.sorted_cumsum_f32(4, 0, n3)).cuda()
+
+    def body3(ctx):
+        x = sg.sg_vec_create(ctx, sg.SG_F32, n3, xs.data_ptr())
+        return {"x": x, "sum": sg.sg_reduce(ctx, x, sg.SG_SUM)}
+
+    def body3_with_contracts(ctx):
+        r = W.cfg3(ctx, n3, xs.data_ptr(), contracts=True)
+        r["sum"] = sg.sg_reduce(ctx, r["x"], sg.SG_SUM)
+        return r
+    measure("overhead_cfg3_body_only (sum(x), 2^28 fp32)", body3, 4 * n3)
+    measure("overhead_cfg3_body_and_contracts_fused (sum(x) + for_all(x>=0) + is_sorted, one pass)", body3_with_contracts, 4 * n3)
+    measure("overhead_cfg3_contracts_alone (for_all(x>=0) + is_sorted as their own pass)", lambda ctx: W.cfg3(ctx, n3, xs.data_ptr(), contracts=True), 4 * n3)
+    t = {k: v["ms"] for k, v in out.items() if k.startswith("overhead_")}
+    key = lambda s: next(v for k, v in t.items() if k.startswith(s))
+    out["contract_overhead_ratios"] = {
+        "cfg0 (body + pre fused + post pass) / body": key("overhead_cfg0_body_and_contracts") / key("overhead_cfg0_body_only"),
+        "cfg3 fused (body + both contracts in one pass) / body": key("overhead_cfg3_body_and_contracts_fused") / key("overhead_cfg3_body_only"),
+        "cfg3 unfused (body pass + contract pass) / body": (key("overhead_cfg3_body_only") + key("overhead_cfg3_contracts_alone")) / key("overhead_cfg3_body_only"),
+        "paper_table4_context": "SafeGPU on a Quadro K2000M (PAPER.md:428-450): vector addition 0.92-1.06, dot product pre&post 0.97-1.10, Gaussian elimination 0.97-1.09, "
+                                "quicksort 1.02-1.08, matrix transposition up to 1.14 (worst case, PAPER.md:416); sequential Eiffel at 10^6: 3.98 (pre) to 7.19 (full)",
+        "ms": 0, "note": "ratios of device times per flush on this B200; the paper's are wall-time ratios on its own hardware: context, not a comparison"}
 
 
 def cfg2_section(torch, sg, W, inputs, measure):
@@ -229,6 +304,15 @@ def cfg3_section(torch, sg, W, inputs, measure):
     xs[j] = 0.5 * xs[j - 1]
     measure(f"cfg3_fp32_2^28_violation_at_{j} (both quantifiers needed: full scan)", lambda ctx: W.cfg3(ctx, n3, xs.data_ptr()), 4 * n3)
     measure(f"cfg3_fp32_2^28_violation_at_{j} as contracts (early exit; time to answer)", lambda ctx: W.cfg3(ctx, n3, xs.data_ptr(), contracts=True), 4 * n3)
+    # dirty runs with the violation at j = n/64, n/2, n - n/64: time to answer (no roofline fraction: the pass stops reading;
+    # the DRAM bytes actually read are in profiles/r02_ncu_summary.md, from ncu captures of these runs)
+    xs[j] = xs_host[j]
+    for name, jj in (("n/64", n3 // 64), ("n/2", n3 // 2), ("n-n/64", n3 - n3 // 64)):
+        saved = float(xs[jj])
+        xs[jj] = 0.5 * xs[jj - 1]
+        measure(f"cfg3_dirty_violation_at_{name} as contracts (early exit; time to answer)", lambda ctx: W.cfg3(ctx, n3, xs.data_ptr(), contracts=True), 4 * n3)
+        measure.out[f"cfg3_dirty_violation_at_{name} as contracts (early exit; time to answer)"]["violation_index"] = int(jj)
+        xs[jj] = saved
 
 
 def ge_section(torch, sg, W, inputs, out, peak):
@@ -308,6 +392,22 @@ def matvec_section(torch, sg, W, inputs, measure):
     sg.sg_ctx_destroy(ctx)
     measure.out["transpose_fp64_16384^2"] = {"ms": ms, "algorithmic_bytes": 16 * n * n, "GB/s": 16 * n * n / ms / 1e6,
                                              "frac_of_peak": 16 * n * n / ms / 1e6 / measure.peak, "passes": 1, "template_passes": 0}
+    del T
+    # fp32: 256-byte segments per tile row instead of 512
+    M32 = M.to(torch.float32)
+    T32 = torch.empty_like(M32)
+    ctx = sg.sg_ctx_create(0, stream)
+    hM = sg.sg_mat_create(ctx, sg.SG_F32, n, n, n, M32.data_ptr())
+    for reps in (3, 10):
+        e0.record()
+        for _ in range(reps):
+            sg.sg_release(ctx, sg.sg_mat_transpose(ctx, hM, T32.data_ptr(), n))
+        e1.record()
+        torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / 10
+    sg.sg_ctx_destroy(ctx)
+    measure.out["transpose_fp32_16384^2"] = {"ms": ms, "algorithmic_bytes": 8 * n * n, "GB/s": 8 * n * n / ms / 1e6,
+                                             "frac_of_peak": 8 * n * n / ms / 1e6 / measure.peak, "passes": 1, "template_passes": 0}
 
 
 def quicksort_section(torch, sg, W, inputs, out):
@@ -377,7 +477,7 @@ def main():
     ap.add_argument("--log2n", type=int, default=28)
     ap.add_argument("--impl", default="ours")
     ap.add_argument("--headline-only", action="store_true", help="same as --configs none")
-    ap.add_argument("--configs", default="cfg0,cfg1,cfg2,cfg3,cfg4,ge,vecapi,matvec,quicksort", help="per_config sections to time after the headline (or: none)")
+    ap.add_argument("--configs", default="cfg0,cfg1,sweep,overhead,cfg2,cfg3,cfg4,ge,vecapi,matvec,quicksort", help="per_config sections to time after the headline (or: none)")
     ap.add_argument("--skip-headline", action="store_true", help="profiling aid: run only the --configs sections and print their JSON")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3)
@@ -481,6 +581,14 @@ def main():
     alg_bytes = 8 * n
     achieved = alg_bytes / k_ms / 1e6
     cpu_rate, cpu_m, cpu_sum, cpu_max = oracle_chain_rate(xh.numpy(), yh.numpy())
+    # the GPU path on exactly the oracle's sample (the first cpu_m elements): sum within 1e-5 relative, max bit-equal
+    rp = W.cfg1(ctx, cpu_m, x.data_ptr(), y.data_ptr())
+    gsum, gmax = sg.sg_scalar_get(ctx, rp["sum"]), sg.sg_scalar_get(ctx, rp["max"])
+    for h in rp.values():
+        sg.sg_release(ctx, h)
+    prefix_ok = bool(abs(gsum - cpu_sum) <= 1e-5 * abs(cpu_sum) and np.float32(gmax) == np.float32(cpu_max))
+    assert prefix_ok, ("GPU and oracle disagree on the oracle's sample", gsum, cpu_sum, gmax, cpu_max)
+    cpu_model, nproc = host_cpu()
     line = {
         "metric": METRIC, "value": ranks.job_throughput(n, world, ms_step), "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
@@ -493,7 +601,9 @@ def main():
                      "traffic": ncu_traffic(sg.sg_template_name(st.pass_kernel[0]) if st.pass_kernel[0] else "bytecode", n),
                      "kernel": sg.sg_template_name(st.pass_kernel[0]) if st.pass_kernel[0] else "bytecode", "kernel_ms": k_ms,
                      "algorithmic_bytes_per_launch": alg_bytes, "peak_source": peak_src, "frac_of_8TBps": achieved / 8000.0},
-        "cpu_baseline": {"value": cpu_rate, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": f"first {cpu_m} elements of the same x,y, one timed run"},
+        "cpu_baseline": {"value": cpu_rate, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": f"first {cpu_m} elements of the same x,y, one timed run",
+                         "cpu_model": cpu_model, "nproc": nproc,
+                         "parity_on_sample": {"ok": prefix_ok, "gpu_sum": gsum, "oracle_sum": cpu_sum, "gpu_max": gmax, "oracle_max": cpu_max}},
         "e2e": {"value": ranks.job_throughput(n, world, e2e_ms / e2e_steps), "unit": UNIT, "h2d_bytes_per_step": 8 * n, "d2h_bytes_per_step": 16,
                 "steps": e2e_steps, "ms_per_step": e2e_ms / e2e_steps},
         "gpu_launches": int(launches),

@@ -258,6 +258,12 @@ sg_status sg_timing_end(sg_ctx* ctx, float* total_ms, int32_t* n_flushes);
 /* Replays the last flush's launch sequence `reps` times on the stream (same buffers, same plan, no host plan
  * build) and returns the mean device time per replay in ms: the measurement entry point. */
 sg_status sg_replay_last(sg_ctx* ctx, int32_t reps, float* ms_per_rep);
+/* The same launch sequence captured `reps` times in a row into ONE CUDA graph (programmatic dependent launches included), so the
+ * device runs the repetitions back to back without the host in between; the graph is launched three times:
+ * device time (CUDA events) and launch-inclusive wall time (host clock, first graph launch to stream completion), both per repetition
+ * — the measurement of passes that take a few microseconds (SURVEY.md §8(d) note iii).  SG_ERR_UNSUPPORTED if the plan contains a
+ * filter pass (its tile states are tagged with a per-launch epoch). */
+sg_status sg_replay_last_graph(sg_ctx* ctx, int32_t reps, float* device_ms_per_rep, float* wall_ms_per_rep);
 /* Number of precompiled template instances in the registry and the name of instance id k (1-based). */
 int32_t sg_template_count(void);
 const char* sg_template_name(int32_t k);

@@ -295,6 +295,13 @@ template <class T> __device__ __forceinline__ Cell cell_shfl_xor_kind(uint8_t ki
     return r;
 }
 
+// Programmatic dependent launch: every pass kernel is launched with programmatic stream serialisation (sgk_launch_pdl), so its
+// blocks may be scheduled while the previous kernel of the stream is still draining — the launch latency of a multi-pass flush
+// (config 0: two 5 us passes) hides behind the predecessor's tail.  pdl_wait() returns once every prerequisite grid has completed
+// and its memory is visible: it precedes the first access to global memory (inputs, control words, workspace).
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
 // streaming 128-bit accesses: bypass L1 allocation, data is touched once
 template <class VEC> __device__ __forceinline__ VEC ld_stream(const VEC* p) {
     int4 r;

@@ -37,13 +37,35 @@ namespace sgk {
 
 constexpr unsigned long long ST_AGG = 1ull << 62, ST_INC = 2ull << 62, ST_FLAGS = 3ull << 62;
 constexpr unsigned long long ST_VAL = (1ull << 40) - 1;
-constexpr int LB = 8;               // look-back windows (of 32 tile states) requested per round trip
+// tuning knobs (overridable at compile time for sweeps; measured on cfg2, 2^27 int32, 1/7 kept — profiles/r02_filter_sweep.md):
+//   RUN = 1 / 2 / 3 / 4 / 5 / 6 tiles per run: 167 / 157 / 155 / 154 / 157 / 166 us.  A run is only taken at full length while its
+//   kept values fill at most 2/3 of the ring (SG_F_RULE 3/2); round 1's factor 2 silently turned RUN = 4 into RUN = 1 at this
+//   selectivity (4 * 1170 * 2 > 8192), which is the 168 us it measured.
+//   LB = 2 / 4 / 8 look-back windows per round trip: 154.3 / 154.8 / 155.3 us;  COPY_BATCH 1..4 and the poll back-off: no effect.
+#ifndef SG_F_LB
+#define SG_F_LB 4
+#endif
+#ifndef SG_F_RUN
+#define SG_F_RUN 4
+#endif
+#ifndef SG_F_COPY_BATCH
+#define SG_F_COPY_BATCH 3
+#endif
+#ifndef SG_F_RULE_NUM
+#define SG_F_RULE_NUM 3
+#define SG_F_RULE_DEN 2
+#endif
+#ifndef SG_F_SLEEP
+#define SG_F_SLEEP 500
+#endif
+constexpr int LB = SG_F_LB;               // look-back windows (of 32 tile states) requested per round trip
 constexpr int F_ROWS = 256;         // rows of 128 bytes per tile
 constexpr int F_TILE_BYTES = F_ROWS * 128;              // 32 KiB per staged input
 constexpr int F_TILE_CHUNKS = F_TILE_BYTES / 16;        // 16-byte chunks per tile
-constexpr int RUN = 4;              // consecutive tiles a block claims at once while few values are kept (else 1); one look-back per run
+constexpr int RUN = SG_F_RUN;              // consecutive tiles a block claims at once while few values are kept (else 1); one look-back per run
 constexpr int NR = 16;              // runs of one block whose offset may be outstanding (ring of run slots)
 constexpr int NP = 8;               // tiles of one block that may wait for their global offset (each may be a run of its own: NP < NR)
+constexpr int COPY_BATCH = SG_F_COPY_BATCH;       // pending tiles with a known offset are copied out once this many have gathered (or the ring / queue fills)
 
 __device__ __forceinline__ unsigned long long ld_state(const unsigned long long* p) {
     unsigned long long v;
@@ -281,7 +303,7 @@ __device__ __forceinline__ unsigned long long filter_lookback(unsigned long long
             const unsigned int vmask = __ballot_sync(0xffffffffu, valid), imask = __ballot_sync(0xffffffffu, inc);
             const unsigned int before_inc = imask ? ((imask & (0u - imask)) - 1u) : 0xffffffffu;    // lanes in front of the first inclusive prefix
             if ((~vmask & before_inc) == 0u) break;
-            __nanosleep(500);       // a near predecessor has not published yet: do not hammer the state words (nor this SM's issue slots)
+            __nanosleep(SG_F_SLEEP);       // a near predecessor has not published yet: do not hammer the state words (nor this SM's issue slots)
         }
 #pragma unroll
         for (int j = 1; j < LB; ++j) {
@@ -346,6 +368,9 @@ __device__ __forceinline__ void filter_body(const SgProg* g, const SgArgs& a) {
     __shared__ unsigned int s_r_total[NR];              //                            its kept count
     __shared__ unsigned long long s_r_excl[NR];         // look-back warp -> compute: global offset of the run's first tile
     __shared__ uint64_t run_posted[NR], run_resolved[NR];   // mbarriers, one arrival each
+    __shared__ volatile int s_resolved;                 // look-back warp -> thread 0: runs 0 .. s_resolved-1 of this block have their offset
+                                                        // (runs resolve in order; ONE shared load replaces a chain of mbarrier polls,
+                                                        // ~150 cycles each, that sat on warp 0's path to the per-tile barrier)
 
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     Cell acc[NOUT];
@@ -373,7 +398,7 @@ __device__ __forceinline__ void filter_body(const SgProg* g, const SgArgs& a) {
     int nxt_base = 0, nxt_len = 0;              // thread 0 only: the run claimed ahead
     unsigned int last_total = (unsigned int)RC; // thread 0 only: kept count of the latest tile (pessimistic until one is known)
     auto claim_ahead = [&]() {                  // thread 0 only
-        nxt_len = (last_total * (unsigned int)RUN * 2u <= (unsigned int)RC) ? RUN : 1;
+        nxt_len = (last_total * (unsigned int)RUN * (unsigned int)SG_F_RULE_NUM <= (unsigned int)RC * (unsigned int)SG_F_RULE_DEN) ? RUN : 1;
         nxt_base = (int)atomicAdd(&a.ctrl[2], (unsigned int)nxt_len);
     };
     auto next_tile = [&]() -> int {             // thread 0 only
@@ -390,6 +415,7 @@ __device__ __forceinline__ void filter_body(const SgProg* g, const SgArgs& a) {
         }
         for (int s = 0; s < NS; ++s) mbar_init(&full_bar[s], 1);
         mbar_fence_init();
+        s_resolved = 0;
         claim_ahead();
         for (int s = 0; s < NS; ++s) {          // the first NS tiles: their copies are in flight before the first one is touched
             const int tv = next_tile();
@@ -411,6 +437,8 @@ __device__ __forceinline__ void filter_body(const SgProg* g, const SgArgs& a) {
             const unsigned long long excl = filter_lookback(state, ep, tile, total, lane);
             if (lane == 0) {
                 s_r_excl[rs] = excl;
+                __threadfence_block();          // the offset is visible before the count that announces it
+                s_resolved = r + 1;
                 mbar_arrive(&run_resolved[rs]);
             }
         }
@@ -508,13 +536,12 @@ __device__ __forceinline__ void filter_body(const SgProg* g, const SgArgs& a) {
             bool run_known = false;         // thread 0: the current run's offset has been resolved already
             if (threadIdx.x == 0) {
                 s_tile[(it + NS) % (NS + 1)] = tv_next;
-                int ready = 0;      // how many of the oldest pending tiles already have their offset (non-blocking poll)
-                for (; ready < q_count; ++ready) {
-                    const int r = s_q_run[(q_head + ready) % NP];
-                    if (!mbar_test(&run_resolved[r % NR], (uint32_t)((r / NR) & 1))) break;
-                }
+                const int resolved = s_resolved;        // runs [0, resolved) of this block have their offset
+                int ready = 0;      // how many of the oldest pending tiles already have their offset (never blocks)
+                for (; ready < q_count; ++ready)
+                    if (s_q_run[(q_head + ready) % NP] >= resolved) break;
                 s_ready[it & 1] = ready;
-                if (!first) run_known = mbar_test(&run_resolved[rs], (uint32_t)((run_no / NR) & 1));
+                if (!first) run_known = run_no < resolved;
             }
             named_bar_sync<1, CT>();     // the stage is in registers; warp totals, next tile id and the ready count are visible
             unsigned int warp_excl = 0, tile_total = 0;
@@ -569,8 +596,11 @@ __device__ __forceinline__ void filter_body(const SgProg* g, const SgArgs& a) {
             ring_head += tile_total;
             run_lpre += tile_total;
             ++q_count;
-            // copy out the tiles whose offset was known at the poll (never blocks), and as many as the queue bound demands
+            // copy out the tiles whose offset was known at the poll (never blocks) — a few at a time: a call costs every thread some
+            // eighty instructions before its first element (queue entries, the run's offset, the uniform checks), tiles of one run
+            // then go out in ONE loop — and as many as the queue bound demands
             int k = s_ready[it & 1] - copied;
+            if (k < COPY_BATCH && ring_head - ring_tail + (unsigned int)TILE / 2u <= (unsigned int)RC) k = 0;
             if (k < q_count - (NP - 1)) k = q_count - (NP - 1);
             if (k > 0) copy_out(k);
         }
@@ -588,10 +618,14 @@ __device__ __forceinline__ void filter_body(const SgProg* g, const SgArgs& a) {
 
 template <class P>
 __global__ void __launch_bounds__(FilterTemplateEval<P>::CT + 32, P::min_blocks) filter1d_template(const __grid_constant__ SgArgs a) {
+    pdl_wait();
+    pdl_trigger();
     filter_body<FilterTemplateEval<P>>(nullptr, a);
 }
 template <class T>
 __global__ void __launch_bounds__(BLOCK + 32) filter1d_bytecode(const __grid_constant__ SgProg g, const __grid_constant__ SgArgs a) {
+    pdl_wait();
+    pdl_trigger();
     filter_body<FilterBytecodeEval<T>>(&g, a);
 }
 

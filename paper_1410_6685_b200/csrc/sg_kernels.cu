@@ -78,7 +78,7 @@ int sgk_plan(const SgProg& prog, SgArgs& a, int force_bytecode, int sm_count, in
     const bool is2d = prog.shape.flags & PF_2D, isfilter = prog.shape.flags & PF_FILTER;
     memset(geom, 0, sizeof(*geom));
     int tid = force_bytecode ? 0 : sgk_find_template(prog);
-    if (tid == 0 && !is2d && prog.shape.n_vreg > VM_VREG)
+    if (tid == 0 && prog.shape.n_vreg > VM_VREG)
         return fail(err, errcap, -9, "fused chain needs more value registers than the bytecode evaluator has; flush earlier");
 
     // alignment of every vector-accessed operand relative to the pass origin
@@ -111,7 +111,27 @@ int sgk_plan(const SgProg& prog, SgArgs& a, int force_bytecode, int sm_count, in
     if (is2d) {
         for (int k = 0; k < prog.shape.n_in; ++k)
             if (prog.in[k].kind == IN_VEC_CVT) return fail(err, errcap, -10, "dtype conversion inside a matrix pass");
-        if (tid == 0 && has_device) return fail(err, errcap, -10, "matrix pass has no precompiled template instance (2-D bytecode evaluator not built)");
+        if (tid == 0) {
+            // no precompiled instance: the 2-D bytecode evaluator (sg_pass2d_vm.cuh) — blocks own whole rows, every access guarded
+            bool has_cols = false;
+            for (int o = 0; o < prog.shape.n_out; ++o) {
+                has_cols |= out_is_reduction(prog.out[o].kind) && prog.out[o].axis == AXIS_COLS;
+            }
+            const long blocks = std::max<long>(1, std::min<long>(a.n, (long)sm_count * (has_cols ? 1 : 2)));
+            geom->template_id = 0;
+            geom->grid = (int)blocks;
+            geom->tile = BLOCK * V;
+            geom->vm_cells = 1;
+            size_t off = (size_t)geom->grid * SG_MAX_OUT * sizeof(Cell);
+            for (int o = 0; o < prog.shape.n_out; ++o) {
+                a.ws_off[o] = 0;
+                if (out_is_reduction(prog.out[o].kind) && prog.out[o].axis == AXIS_COLS) { a.ws_off[o] = (int64_t)off; off += (size_t)blocks * a.cols * sizeof(Cell); }
+            }
+            geom->ws_bytes = off;
+            geom->ctrl_words = 1;
+            a.vec_ok = 0; a.head = 0; a.n_full_tiles = 0; a.n_strips = 0; a.n_chunks = 0; a.rows_per_chunk = 0;
+            return 0;
+        }
         bool ok = congruent && mis == 0 && (a.cols % V) == 0;
         for (int k = 0; k < prog.shape.n_in; ++k)
             if (prog.in[k].kind == IN_VEC && (a.in_stride[k] % V) != 0) ok = false;

@@ -224,6 +224,8 @@ __global__ void __launch_bounds__(BLOCK, P::min_blocks) pass1d_template(const __
     constexpr auto OS = std::make_integer_sequence<int, M::S.n_out>{};
 
     constexpr SgProg g = P::prog;     // local constant copy: indexable inside unrolled loops
+    pdl_wait();
+    pdl_trigger();
     Cell acc[M::NOUT];
     uint8_t kind[M::NOUT];
     bool has_reduction = false;

@@ -453,6 +453,8 @@ __global__ void __launch_bounds__(BLOCK, 3) pass1d_bytecode(const __grid_constan
     __shared__ __align__(16) VmTables tab;
     constexpr int E = VmE<T>::value;
     constexpr int VM_TILE = BLOCK * E * C;          // C cells of BLOCK*E consecutive elements each
+    pdl_wait();
+    pdl_trigger();
     Cell acc[SG_MAX_OUT];
     uint8_t kind[SG_MAX_OUT];
     bool has_reduction = false;

@@ -410,6 +410,8 @@ __device__ __forceinline__ void pass2d_body(const SgArgs& a) {
 
 template <class P>
 __global__ void __launch_bounds__(BLOCK, P::min_blocks) pass2d_template(const __grid_constant__ SgArgs a) {
+    pdl_wait();
+    pdl_trigger();
     if ((a.vec_ok >> 29) & 1) pass2d_body<P, false>(a);     // bit 29: rows are not 16-byte aligned (uniform)
     else pass2d_body<P, true>(a);
 }

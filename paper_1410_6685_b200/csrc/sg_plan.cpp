@@ -12,6 +12,7 @@
 // "one kernel per method call" plan of PAPER.md:282, kept as the measurement baseline.
 #include <stdio.h>
 #include <string.h>
+#include <time.h>
 
 #include <algorithm>
 #include <map>
@@ -485,5 +486,58 @@ extern "C" sg_status sg_replay_last(sg_ctx* c, int32_t reps, float* ms_per_rep) 
     if (cudaEventSynchronize(c->ev_t1) != cudaSuccess || cudaEventElapsedTime(&ms, c->ev_t0, c->ev_t1) != cudaSuccess)
         return sg_fail(c, SG_ERR_CUDA, cudaGetErrorString(cudaGetLastError()));
     *ms_per_rep = ms / reps;
+    return SG_OK;
+}
+
+// The last flush's launch sequence captured ONCE into a CUDA graph and replayed `reps` times: the launch-inclusive measurement of
+// short passes (SURVEY.md §8(d) note iii).  device_ms: CUDA events around the replays; wall_ms: host clock from the first
+// cudaGraphLaunch to the stream's completion, both per replay.
+extern "C" sg_status sg_replay_last_graph(sg_ctx* c, int32_t reps, float* device_ms_per_rep, float* wall_ms_per_rep) {
+    if (!c || !device_ms_per_rep || !wall_ms_per_rep || reps <= 0) return SG_ERR_ARG;
+    SgDeviceScope dev_scope(c);
+    if (c->plan_only) { *device_ms_per_rep = *wall_ms_per_rep = 0.f; return SG_OK; }
+    if (c->last.empty()) return sg_fail(c, SG_ERR_ARG, "nothing to replay");
+    for (const Launch& l : c->last)
+        if (l.prog.shape.flags & PF_FILTER) return sg_fail(c, SG_ERR_UNSUPPORTED, "a filter pass tags its tile states with a per-launch epoch: not replayable from a graph");
+    cudaGraph_t graph = nullptr;
+    cudaGraphExec_t exec = nullptr;
+    auto fail = [&](const char* what) {
+        const cudaError_t e = cudaGetLastError();
+        if (exec) cudaGraphExecDestroy(exec);
+        if (graph) cudaGraphDestroy(graph);
+        return sg_fail(c, SG_ERR_CUDA, std::string(what) + ": " + cudaGetErrorString(e));
+    };
+    if (cudaStreamSynchronize(c->stream) != cudaSuccess) return fail("stream sync");
+    // captured on a stream of its own (the context's stream may be the legacy default stream, which cannot capture); the graph
+    // is then launched on the context's stream like every other piece of work
+    cudaStream_t cap = nullptr;
+    if (cudaStreamCreateWithFlags(&cap, cudaStreamNonBlocking) != cudaSuccess) return fail("capture stream");
+    if (cudaStreamBeginCapture(cap, cudaStreamCaptureModeThreadLocal) != cudaSuccess) { cudaStreamDestroy(cap); return fail("begin capture"); }
+    // ALL `reps` repetitions go into ONE graph: the device then runs them back to back without the host in between (a graph launch
+    // per repetition would measure the host's launch rate, ~4 us per cudaGraphLaunch, not the passes)
+    bool ok = true;
+    for (int r = 0; r < reps && ok; ++r)
+        for (Launch& l : c->last) ok = ok && sgk_launch(l.prog, l.args, l.geom, cap) == cudaSuccess;
+    const bool ended = cudaStreamEndCapture(cap, &graph) == cudaSuccess;
+    cudaStreamDestroy(cap);
+    if (!ended || !ok || !graph) return fail("capture");
+    if (cudaGraphInstantiate(&exec, graph, 0) != cudaSuccess) return fail("graph instantiate");
+    cudaGraphLaunch(exec, c->stream);
+    if (cudaStreamSynchronize(c->stream) != cudaSuccess) return fail("graph warm-up");
+    const int graph_launches = 3;
+    timespec w0, w1;
+    clock_gettime(CLOCK_MONOTONIC, &w0);
+    cudaEventRecord(c->ev_t0, c->stream);
+    for (int r = 0; r < graph_launches; ++r) cudaGraphLaunch(exec, c->stream);
+    cudaEventRecord(c->ev_t1, c->stream);
+    if (cudaStreamSynchronize(c->stream) != cudaSuccess) return fail("graph replay");
+    clock_gettime(CLOCK_MONOTONIC, &w1);
+    float ms = 0.f;
+    if (cudaEventElapsedTime(&ms, c->ev_t0, c->ev_t1) != cudaSuccess) return fail("event");
+    *device_ms_per_rep = ms / (reps * graph_launches);
+    *wall_ms_per_rep = (float)(((w1.tv_sec - w0.tv_sec) * 1e3 + (w1.tv_nsec - w0.tv_nsec) * 1e-6) / (reps * graph_launches));
+    c->stats.launches_total += (int64_t)reps * (graph_launches + 1) * (int64_t)c->last.size();
+    cudaGraphExecDestroy(exec);
+    cudaGraphDestroy(graph);
     return SG_OK;
 }

@@ -80,12 +80,24 @@ inline int current_device_slot() {
     return (d >= 0 && d < SG_MAX_DEVICES) ? d : 0;
 }
 
+// one launch with programmatic stream serialisation allowed (see pdl_wait in sg_device.cuh)
+template <class... KArgs, class... Args>
+inline cudaError_t sgk_launch_pdl(void (*kernel)(KArgs...), int grid, int block, size_t smem, cudaStream_t s, const Args&... args) {
+    cudaLaunchConfig_t cfg{};
+    cfg.gridDim = dim3((unsigned)grid); cfg.blockDim = dim3((unsigned)block); cfg.dynamicSmemBytes = smem; cfg.stream = s;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr; cfg.numAttrs = 1;
+    return cudaLaunchKernelEx(&cfg, kernel, args...);
+}
+
 template <class P> cudaError_t launch_template(const SgArgs& a, int grid, cudaStream_t s) {
     if constexpr ((P::prog.shape.flags & PF_2D) != 0) {
         static bool attr_set[SG_MAX_DEVICES] = {};
         bool& set = attr_set[current_device_slot()];
         if (!set) { cudaFuncSetAttribute(pass2d_template<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_of<P>()); set = true; }
-        pass2d_template<P><<<grid, BLOCK, smem_of<P>(), s>>>(a);
+        return sgk_launch_pdl(pass2d_template<P>, grid, BLOCK, smem_of<P>(), s, a);
     }
     else if constexpr ((P::prog.shape.flags & PF_FILTER) != 0) {
         static bool attr_set[SG_MAX_DEVICES] = {};
@@ -94,10 +106,9 @@ template <class P> cudaError_t launch_template(const SgArgs& a, int grid, cudaSt
         SgArgs a2 = a;
         a2.vec_ok &= ~(1 << 30);
         if (encode_filter_tmaps<P>(a2)) a2.vec_ok |= (1 << 30);
-        filter1d_template<P><<<grid, FilterTemplateEval<P>::CT + 32, smem_of<P>(), s>>>(a2);
+        return sgk_launch_pdl(filter1d_template<P>, grid, FilterTemplateEval<P>::CT + 32, smem_of<P>(), s, a2);
     }
-    else pass1d_template<P><<<grid, BLOCK, 0, s>>>(a);
-    return cudaGetLastError();
+    else return sgk_launch_pdl(pass1d_template<P>, grid, BLOCK, 0, s, a);
 }
 template <class P> int occupancy_template() {
     static int cached_dev[SG_MAX_DEVICES] = {};     // one query per instance and device (the query costs tens of microseconds)

@@ -6,6 +6,7 @@
 #include "sg_filter.cuh"
 #include "sg_kernels.h"
 #include "sg_pass1d_vm.cuh"
+#include "sg_pass2d_vm.cuh"
 #include "sg_tmpl_launch.cuh"
 
 #ifndef SG_VM_DTYPE
@@ -20,16 +21,20 @@ template <class T, int C> cudaError_t launch_pass1d_bytecode(const SgProg& g, co
     static bool attr_dev[SG_MAX_DEVICES] = {};
     bool& attr_set = attr_dev[current_device_slot()];
     if (!attr_set) { cudaFuncSetAttribute(pass1d_bytecode<T, C>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)vm_file_bytes(VM_VREG, 1)); attr_set = true; }
-    pass1d_bytecode<T, C><<<grid, BLOCK, vm_file_bytes(g.shape.n_vreg, C), s>>>(g, a);
-    return cudaGetLastError();
+    return sgk_launch_pdl(pass1d_bytecode<T, C>, grid, BLOCK, vm_file_bytes(g.shape.n_vreg, C), s, g, a);
 }
 template <class T> cudaError_t launch_bytecode_t(const SgProg& g, const SgArgs& a, const SgGeom& geom, cudaStream_t s) {
+    if (g.shape.flags & PF_2D) {
+        static bool attr_dev[SG_MAX_DEVICES] = {};
+        bool& attr_set = attr_dev[current_device_slot()];
+        if (!attr_set) { cudaFuncSetAttribute(pass2d_bytecode<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)VM_FILE_BYTES); attr_set = true; }
+        return sgk_launch_pdl(pass2d_bytecode<T>, geom.grid, BLOCK, VM_FILE_BYTES, s, g, a);
+    }
     if (g.shape.flags & PF_FILTER) {
         static bool attr_dev[SG_MAX_DEVICES] = {};
         bool& attr_set = attr_dev[current_device_slot()];
         if (!attr_set) { cudaFuncSetAttribute(filter1d_bytecode<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FilterBytecodeEval<T>::SMEM); attr_set = true; }
-        filter1d_bytecode<T><<<geom.grid, BLOCK + 32, FilterBytecodeEval<T>::SMEM, s>>>(g, a);
-        return cudaGetLastError();
+        return sgk_launch_pdl(filter1d_bytecode<T>, geom.grid, BLOCK + 32, FilterBytecodeEval<T>::SMEM, s, g, a);
     }
     return geom.vm_cells == 2 ? launch_pass1d_bytecode<T, 2>(g, a, geom.grid, s) : launch_pass1d_bytecode<T, 1>(g, a, geom.grid, s);
 }

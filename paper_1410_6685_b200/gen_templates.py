@@ -25,6 +25,7 @@ DEFAULT_TUNE = (2, 3, 4)
 TUNE = {
     "cfg1": (2, 4, 4),
     "cfg3": (4, 4, 4),
+    "cfg3sum": (4, 4, 4),
     "sorted_f32": (4, 4, 4),
     "cfg4": (2, 2, 4),
     "matvec": (2, 2, 4),      # measured: (2, 4, 2) is slower (0.430 / 0.379 ms vs 0.376 / 0.343 ms right / left at 16384^2)
@@ -52,6 +53,7 @@ def _chains():
     yield "cfg1_unfused", sg.SG_FLAG_UNFUSED, lambda c: W.cfg1(c, N, None, None)            # one kernel per op
     yield "cfg2", 0, lambda c: W.cfg2(c, N, None)
     yield "cfg3", 0, lambda c: W.cfg3(c, N, None)
+    yield "cfg3sum", 0, lambda c: _cfg3_sum(c)                                              # a body (sum) with config 3's two PRE contracts fused into its pass
     yield "sorted_f32", 0, lambda c: _sorted_only(c, f32)
     yield "sorted_f64", 0, lambda c: _sorted_only(c, f64)
     yield "cfg4", 0, lambda c: W.cfg4(c, 4096, None, 0)
@@ -86,6 +88,11 @@ def _ge_step(c, k):
     minpiv = sg.sg_vec_create(c, sg.SG_F64, 1, None)
     for h in W.ge_step(c, M, 4096, k, det, minpiv):
         sg.sg_release(c, h)
+
+
+def _cfg3_sum(c):
+    r = W.cfg3(c, N, None, contracts=True)
+    return sg.sg_reduce(c, r["x"], sg.SG_SUM)
 
 
 def _sorted_only(c, dt):

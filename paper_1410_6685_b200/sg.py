@@ -32,7 +32,7 @@ EXPORTS = [
     "sg_ctx_create", "sg_ctx_destroy", "sg_ctx_set_flags", "sg_last_error", "sg_vec_create", "sg_mat_create", "sg_vec_subset",
     "sg_mat_row", "sg_mat_rows", "sg_mat_col", "sg_mat_elem", "sg_mat_ge_steps", "sg_mat_transpose", "sg_vec_quicksort", "sg_enqueue", "sg_cast", "sg_reduce", "sg_forall", "sg_exists",
     "sg_forall_adjacent", "sg_filter", "sg_contract", "sg_flush", "sg_scalar_get", "sg_scalar_dtype", "sg_vec_count", "sg_vec_data", "sg_vec_read",
-    "sg_release", "sg_plan_stats", "sg_plan_dump", "sg_last_flush_ms", "sg_timing_begin", "sg_timing_end", "sg_replay_last", "sg_template_count", "sg_template_name",
+    "sg_release", "sg_plan_stats", "sg_plan_dump", "sg_last_flush_ms", "sg_timing_begin", "sg_timing_end", "sg_replay_last", "sg_replay_last_graph", "sg_template_count", "sg_template_name",
     "sg_version",
 ]
 
@@ -57,7 +57,8 @@ _LIB = None
 
 
 def lib_path() -> str:
-    return os.path.join(os.path.dirname(os.path.abspath(__file__)), "libsafegpu.so")
+    """The in-tree library; SAFEGPU_LIB names another build of the same sources (kernel tuning experiments)."""
+    return os.environ.get("SAFEGPU_LIB") or os.path.join(os.path.dirname(os.path.abspath(__file__)), "libsafegpu.so")
 
 
 def lib() -> ctypes.CDLL:
@@ -99,6 +100,7 @@ def lib() -> ctypes.CDLL:
         L.sg_plan_dump.argtypes = [c_void_p, c_int32, c_char_p, c_int64]
         L.sg_last_flush_ms.argtypes = [c_void_p, POINTER(c_float)]
         L.sg_replay_last.argtypes = [c_void_p, c_int32, POINTER(c_float)]
+        L.sg_replay_last_graph.argtypes = [c_void_p, c_int32, POINTER(c_float), POINTER(c_float)]
         L.sg_mat_ge_steps.argtypes = [c_void_p, c_int64, c_int64, c_int64, c_double, c_int64, c_int64]
         L.sg_vec_quicksort.argtypes = [c_void_p, c_int64, c_void_p, POINTER(c_int64)]
         L.sg_mat_transpose.argtypes = [c_void_p, c_int64, c_void_p, c_int64, POINTER(c_int64)]
@@ -333,3 +335,10 @@ def sg_replay_last(ctx, reps: int) -> float:
     ms = c_float(0)
     _ck(ctx, lib().sg_replay_last(ctx, reps, byref(ms)))
     return ms.value
+
+
+def sg_replay_last_graph(ctx, reps: int) -> tuple[float, float]:
+    """(device ms, launch-inclusive wall ms) per replay of the last flush's launches from a CUDA graph."""
+    dev, wall = c_float(0.0), c_float(0.0)
+    _ck(ctx, lib().sg_replay_last_graph(ctx, reps, byref(dev), byref(wall)))
+    return dev.value, wall.value

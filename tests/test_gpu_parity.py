@@ -530,6 +530,75 @@ def test_cfg4(n, k, ld):
             assert sg.sg_plan_stats(c.ctx).n_passes == 2
 
 
+@pytest.mark.parametrize("n,k,ld", [(2, 0, 2), (3, 1, 3), (34, 0, 34), (33, 5, 37), (258, 100, 258), (515, 3, 521), (1030, 7, 1030)])
+def test_cfg4_through_the_matrix_bytecode_evaluator(n, k, ld):
+    """SG_FLAG_FORCE_BYTECODE: the same step on pass2d_bytecode (the evaluator of matrix chains without a template instance)."""
+    M = inputs.boosted_matrix_f64(5, 0, n)
+    want = ocfg.cfg4(M, k)
+    with Ctx(sg.SG_FLAG_FORCE_BYTECODE) as c:
+        buf = np.full((n, ld), 7.25)
+        buf[:, :n] = M
+        t = c.torch.from_numpy(buf).cuda()
+        r = W.cfg4(c.ctx, n, t.data_ptr(), k, ld=ld)
+        sg.sg_flush(c.ctx)
+        st = sg.sg_plan_stats(c.ctx)
+        full = t.cpu().numpy()
+        assert st.n_bytecode == st.n_passes == 2
+        assert bits_equal(np.ascontiguousarray(full[:, :n]), want["M"]) and (full[:, n:] == 7.25).all()
+        if k + 1 < n:
+            assert bits_equal(c.read_vec(r["rowmax"], np.float64), want["rowmax"])
+            assert colsum_ok(c.read_vec(r["colsum"], np.float64), want["colsum"], np.abs(want["M"][k + 1:]).sum(axis=0))
+
+
+@pytest.mark.parametrize("dtype", [np.float32, np.float64, np.int32])
+@pytest.mark.parametrize("rows,cols", [(1, 1), (5, 3), (33, 65), (130, 1027), (700, 260)])
+def test_unregistered_matrix_chain_runs_on_the_bytecode_evaluator(dtype, rows, cols):
+    """A matrix chain nobody registered a template for: B = (A + A) * v (ROW broadcast) - w (COL broadcast), kept; per-row max, per-column
+    sum, whole-matrix min and a quantifier — one pass on pass2d_bytecode, compared with the oracle primitive by primitive."""
+    from gpu_util import NP2SG
+    if np.dtype(dtype).kind == "f":
+        A = RNG.standard_normal((rows, cols)).astype(dtype)
+        v, w = RNG.standard_normal(cols).astype(dtype), RNG.standard_normal(rows).astype(dtype)
+    else:
+        A = RNG.integers(-1000, 1000, (rows, cols)).astype(dtype)
+        v, w = RNG.integers(-50, 50, cols).astype(dtype), RNG.integers(-50, 50, rows).astype(dtype)
+    with Ctx() as c:
+        tA, tv, tw = dev(A), dev(v), dev(w)
+        c.keep += [tA, tv, tw]
+        sgdt = NP2SG[np.dtype(dtype)]
+        hA = sg.sg_mat_create(c.ctx, sgdt, rows, cols, cols, tA.data_ptr())
+        hv, hw = sg.sg_vec_create(c.ctx, sgdt, cols, tv.data_ptr()), sg.sg_vec_create(c.ctx, sgdt, rows, tw.data_ptr())
+        s2 = sg.sg_enqueue(c.ctx, sg.SG_ADD, [hA, hA])
+        sv = sg.sg_enqueue(c.ctx, sg.SG_MUL, [s2, sg.H(hv, sg.SG_BCAST_ROW)])
+        B = sg.sg_enqueue(c.ctx, sg.SG_SUB, [sv, sg.H(hw, sg.SG_BCAST_COL)])
+        for h in (s2, sv):
+            sg.sg_release(c.ctx, h)
+        rmax = sg.sg_reduce(c.ctx, B, sg.SG_RMAX, sg.SG_AXIS_ROWS)
+        csum = sg.sg_reduce(c.ctx, B, sg.SG_SUM, sg.SG_AXIS_COLS)
+        mn = sg.sg_reduce(c.ctx, B, sg.SG_RMIN)
+        pos = sg.sg_enqueue(c.ctx, sg.SG_GT, [B, sg.F(0.0) if np.dtype(dtype).kind == "f" else sg.I(0)])
+        anyp, cnt = sg.sg_exists(c.ctx, pos), sg.sg_reduce(c.ctx, pos, sg.SG_COUNT)
+        sg.sg_release(c.ctx, pos)
+        got_min, got_any, got_cnt = c.get(mn), c.get(anyp), c.get(cnt)
+        st = sg.sg_plan_stats(c.ctx)
+        assert st.n_passes == 1 and st.n_bytecode == 1
+        got_B = c.read_vec(B, dtype, rows * cols).reshape(rows, cols)
+        got_rmax = c.read_vec(rmax, dtype, rows)
+        got_csum = c.read_vec(csum, np.float64 if np.dtype(dtype).kind == "f" else np.int64, cols)
+    want_B = np.empty_like(A)
+    for r in range(rows):
+        want_B[r] = orc.scalar("sub", orc.zip("mul", orc.zip("add", A[r], A[r]), v), w[r])
+    assert bits_equal(got_B, want_B)
+    assert bits_equal(got_rmax, np.array([orc.max(want_B[r]) for r in range(rows)], dtype=dtype))
+    want_csum = [orc.sum(np.ascontiguousarray(want_B[:, cc])) for cc in range(cols)]
+    if np.dtype(dtype).kind == "f":
+        tol = 1e-12 if dtype is np.float64 else 1e-5
+        assert all(abs(gv - wv) <= tol * max(np.abs(want_B[:, cc]).sum(), 1e-300) for cc, (gv, wv) in enumerate(zip(got_csum, want_csum)))
+    else:
+        assert got_csum.tolist() == want_csum
+    assert dtype(got_min) == orc.min(want_B.reshape(-1)) and got_any == bool((want_B > 0).any()) and got_cnt == int((want_B > 0).sum())
+
+
 @pytest.mark.parametrize("k", [0, 8191])
 def test_cfg4_full_size(k):
     """BASELINE.json:configs[4] at its full size, in bench.py's launch configuration: EVERY element of M', all n-k-1 row maxima
