@@ -306,7 +306,7 @@ def cfg3_section(torch, sg, W, inputs, measure):
     measure(f"cfg3_fp32_2^28_violation_at_{j} as contracts (early exit; time to answer)", lambda ctx: W.cfg3(ctx, n3, xs.data_ptr(), contracts=True), 4 * n3)
     # dirty runs with the violation at j = n/64, n/2, n - n/64: time to answer (no roofline fraction: the pass stops reading;
     # the DRAM bytes actually read are in profiles/r02_ncu_summary.md, from ncu captures of these runs)
-    xs[j] = xs_host[j]
+    xs[j] = float(xs_host[j])
     for name, jj in (("n/64", n3 // 64), ("n/2", n3 // 2), ("n-n/64", n3 - n3 // 64)):
         saved = float(xs[jj])
         xs[jj] = 0.5 * xs[jj - 1]
@@ -478,6 +478,8 @@ def main():
     ap.add_argument("--impl", default="ours")
     ap.add_argument("--headline-only", action="store_true", help="same as --configs none")
     ap.add_argument("--configs", default="cfg0,cfg1,sweep,overhead,cfg2,cfg3,cfg4,ge,vecapi,matvec,quicksort", help="per_config sections to time after the headline (or: none)")
+    ap.add_argument("--shard", action="store_true", help="N > 1: ONE 2^log2n collection sharded over the ranks (strong scaling, SURVEY.md 8(e)) "
+                    "instead of independent replicas; partial results all-gathered (12 bytes per rank) and combined by a library pass")
     ap.add_argument("--skip-headline", action="store_true", help="profiling aid: run only the --configs sections and print their JSON")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3)
@@ -503,16 +505,37 @@ def main():
         print(json.dumps({"per_config": per_config(torch, sg, W, inputs, peak, which)}))
         return
 
-    n = 1 << args.log2n
-    sx, sy = ranks.rank_streams(rank)
-    xh = torch.from_numpy(inputs.normal_f32(2, sx, n)).pin_memory()
-    yh = torch.from_numpy(inputs.normal_f32(2, sy, n)).pin_memory()
+    n_total = 1 << args.log2n
+    shard = bool(args.shard and world > 1)
+    if shard:       # one collection, contiguous ranges (the generator is counter-based: a rank makes only its own range)
+        lo, hi = ranks.shard_range(n_total, rank, world)
+        n = hi - lo
+        xh = torch.from_numpy(inputs.normal_f32(2, 0, n, start=lo)).pin_memory()
+        yh = torch.from_numpy(inputs.normal_f32(2, 1, n, start=lo)).pin_memory()
+    else:
+        n = n_total
+        sx, sy = ranks.rank_streams(rank)
+        xh = torch.from_numpy(inputs.normal_f32(2, sx, n)).pin_memory()
+        yh = torch.from_numpy(inputs.normal_f32(2, sy, n)).pin_memory()
     x, y = xh.cuda(), yh.cuda()
     stream = torch.cuda.current_stream().cuda_stream
     ctx = sg.sg_ctx_create(local, stream)
+    part_sum = torch.zeros(1, dtype=torch.float64, device="cuda")
+    part_max = torch.zeros(1, dtype=torch.float32, device="cuda")
+    gathered = {}
+
+    def gather(kind):
+        t = ranks.all_gather_1d(part_sum if kind == "sum" else part_max, dist)     # NCCL all-gather on the same stream: 8 / 4 bytes per rank
+        gathered[kind] = t                                                          # keep the buffer alive until the combine pass has run
+        return t.data_ptr(), t.numel()
+
+    def enqueue():
+        if shard:
+            return W.cfg1_sharded(ctx, n, x.data_ptr(), y.data_ptr(), part_sum.data_ptr(), part_max.data_ptr(), gather)
+        return W.cfg1(ctx, n, x.data_ptr(), y.data_ptr())
 
     def step():
-        r = W.cfg1(ctx, n, x.data_ptr(), y.data_ptr())
+        r = enqueue()
         s, m = sg.sg_scalar_get(ctx, r["sum"]), sg.sg_scalar_get(ctx, r["max"])
         for h in r.values():
             sg.sg_release(ctx, h)
@@ -539,7 +562,7 @@ def main():
     sg.sg_timing_begin(ctx)
     e0.record()
     for _ in range(args.steps):
-        r = W.cfg1(ctx, n, x.data_ptr(), y.data_ptr())
+        r = enqueue()
         sg.sg_flush(ctx)
         pending.append(r)
     e1.record()
@@ -577,6 +600,8 @@ def main():
         return
 
     ms_step = total_ms / args.steps
+    if shard:       # strong scaling: the job is ONE collection of n_total elements; the flush count doubles (local pass + combine pass)
+        kernel_ms = [kernel_total_ms / max(args.steps, 1)]
     k_ms = float(np.mean(kernel_ms))
     alg_bytes = 8 * n
     achieved = alg_bytes / k_ms / 1e6
@@ -591,9 +616,9 @@ def main():
     cpu_model, nproc = host_cpu()
     line = {
         "metric": METRIC, "value": ranks.job_throughput(n, world, ms_step), "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "ms_per_step": ms_step, "higher_is_better": True, "scaling": "strong" if shard else "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": {"workload": f"cfg1 fused 10-op chain + sum + max on fp32 x,y of 2^{args.log2n} elements (BASELINE.json metric: fused chain at 2^28)",
-                   "n": n, "seed": 2, "l2": "inputs (2 x 4n bytes) larger than L2; no flush needed", "plan_passes": st.n_passes,
+                   "n": n, "sharded_over_ranks": shard, "n_total": n_total if shard else n * world, "seed": 2, "l2": "inputs (2 x 4n bytes) larger than L2; no flush needed", "plan_passes": st.n_passes,
                    "template_passes": st.n_template, "step": "enqueue + plan + fused launch + scalar hand-back (async copy to the pinned mirror) through the C ABI; K steps pipelined, scalars read after the region"},
         "GB/s": world * alg_bytes / ms_step / 1e6,
         "frac_of_8TBps": alg_bytes / ms_step / 1e6 / 8000.0,

@@ -90,10 +90,11 @@ def uniform_pm1_f64(seed: int, stream: int, n: int) -> np.ndarray:
     return _fill(np.empty(n, dtype=np.float64), lambda s, c: 2.0 * u01(seed, stream, s, c) - 1.0)
 
 
-def normal_f32(seed: int, stream: int, n: int) -> np.ndarray:
-    """float32[n] ~ N(0,1): Box-Muller in float64 on counters (2i, 2i+1), one output per pair (config 1)."""
+def normal_f32(seed: int, stream: int, n: int, start: int = 0) -> np.ndarray:
+    """float32[n] ~ N(0,1): Box-Muller in float64 on counters (2i, 2i+1), one output per pair (config 1).  start: elements
+    start .. start+n-1 of the same infinite sequence (a rank generates only its shard of a sharded collection)."""
     def chunk(s, c):
-        u = u01(seed, stream, 2 * s, 2 * c)
+        u = u01(seed, stream, 2 * (start + s), 2 * c)
         u1 = 1.0 - u[0::2]          # (0, 1]
         u2 = u[1::2]
         return (np.sqrt(-2.0 * np.log(u1)) * np.cos(2.0 * np.pi * u2)).astype(np.float32)

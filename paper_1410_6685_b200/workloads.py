@@ -116,6 +116,30 @@ def cfg1(ctx, n, px, py, keep_w=False):
     return res
 
 
+def cfg1_sharded(ctx, n_local, px, py, p_part_sum, p_part_max, gather):
+    """config 1 on ONE collection sharded over the ranks.  Each rank runs the fused chain on its contiguous range (px,
+    py: the shard's n_local elements) and leaves its partial sum (f64) and partial max (f32) in the one-element device buffers
+    p_part_sum / p_part_max — device-resident, nothing visits the host.  `gather(kind)` is the exchange step: it returns (device
+    pointer, count) of ALL ranks' partials of that kind in rank order (ranks.all_gather_1d over NCCL: 8 + 4 bytes per rank).  The
+    combine is a pass of the library over those W-element vectors: a sum of W partial sums (double-double accumulation, fixed rank
+    order: deterministic) and the max of W partial maxima under the total order.  Returns the handles of the two global scalars."""
+    x = sg.sg_vec_create(ctx, sg.SG_F32, n_local, px)
+    y = sg.sg_vec_create(ctx, sg.SG_F32, n_local, py)
+    wv = cfg1_chain(ctx, x, y)
+    s, m = sg.sg_reduce(ctx, wv, sg.SG_SUM), sg.sg_reduce(ctx, wv, sg.SG_RMAX)
+    sg.sg_release(ctx, wv)
+    ps = sg.sg_vec_create(ctx, sg.SG_F64, 1, p_part_sum)
+    pm = sg.sg_vec_create(ctx, sg.SG_F32, 1, p_part_max)
+    sg.sg_enqueue(ctx, sg.SG_ADD, [s, F(0.0)], dst_or_0=ps)            # the deferred scalars land in caller-visible device memory ...
+    sg.sg_enqueue(ctx, sg.SG_MAX, [m, m], dst_or_0=pm)
+    sg.sg_flush(ctx)                                                   # ... asynchronously: the collective is stream-ordered after it
+    all_s, w_s = gather("sum")
+    all_m, w_m = gather("max")
+    gs = sg.sg_reduce(ctx, sg.sg_vec_create(ctx, sg.SG_F64, w_s, all_s), sg.SG_SUM)
+    gm = sg.sg_reduce(ctx, sg.sg_vec_create(ctx, sg.SG_F32, w_m, all_m), sg.SG_RMAX)
+    return {"x": x, "y": y, "sum": gs, "max": gm, "part_sum": s, "part_max": m, "ps": ps, "pm": pm}
+
+
 def cfg2(ctx, n, px, pout=None, capacity=0, modulus=7, residue=3):
     """BASELINE.json:configs[2]: stable filter keeping x where x mod 7 == 3, count, int64 sum of the kept values."""
     x = sg.sg_vec_create(ctx, sg.SG_I32, n, px)

@@ -808,3 +808,33 @@ def test_early_exit_leaves_no_half_evaluated_quantifier_readable():
         with pytest.raises(sg.SgError):
             sg.sg_flush(c.ctx)
         assert c.get(ex_far) is True and c.get(srt) is False
+
+
+def test_cfg1_sharded_over_emulated_ranks():
+    """ONE collection in W contiguous shards.  One GPU here, so the W ranks run one after the other (no kernel waits for
+    another): each leaves its partial sum / max in device memory, the all-gather is emulated by a tensor that collects them in rank
+    order, and the combine is the library's pass over the W partials — the same workload function bench.py --shard runs per rank."""
+    from paper_1410_6685_b200 import ranks
+    n, world = (1 << 22) + 5, 3
+    x, y = inputs.normal_f32(2, 0, n), inputs.normal_f32(2, 1, n)
+    want = ocfg.cfg1(x, y)
+    with Ctx() as c:
+        torch = c.torch
+        all_sum = torch.zeros(world, dtype=torch.float64, device="cuda")
+        all_max = torch.zeros(world, dtype=torch.float32, device="cuda")
+        results = []
+        for rank in range(world):
+            lo, hi = ranks.shard_range(n, rank, world)
+            xs, ys = inputs.normal_f32(2, 0, hi - lo, start=lo), inputs.normal_f32(2, 1, hi - lo, start=lo)   # a rank generates only its range
+            assert bits_equal(xs, x[lo:hi])
+            tx, ty = dev(xs), dev(ys)
+            c.keep += [tx, ty]
+            ps, pm = all_sum[rank:rank + 1], all_max[rank:rank + 1]          # this rank's slot of the gathered buffers
+
+            def gather(kind):
+                t = all_sum if kind == "sum" else all_max
+                return t.data_ptr(), rank + 1                                  # the partials gathered so far, in rank order
+            r = W.cfg1_sharded(c.ctx, hi - lo, tx.data_ptr(), ty.data_ptr(), ps.data_ptr(), pm.data_ptr(), gather)
+            results.append((c.get(r["sum"]), c.get(r["max"])))
+        gsum, gmax = results[-1]                                              # after the last rank every partial is there
+    assert sum_ok(gsum, want["sum"], want["w"], 1e-5) and np.float32(gmax) == want["max"]
