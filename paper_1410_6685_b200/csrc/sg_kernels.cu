@@ -45,7 +45,7 @@ const Registry& registry() { static const Registry r; return r; }
 #define g_entries (registry().e)
 #define g_n_entries (registry().n)
 
-int occupancy_bytecode(int dtype, bool filter, int n_vreg = VM_VREG, int cells = 1) {
+int occupancy_bytecode(int dtype, bool filter, int n_vreg = 64 /* file KiB */, int cells = 0 /* vm config */) {
     switch (dtype) {
         case DT_F32: return sgk_occupancy_bytecode_0(filter, n_vreg, cells);
         case DT_F64: return sgk_occupancy_bytecode_1(filter, n_vreg, cells);
@@ -121,7 +121,7 @@ int sgk_plan(const SgProg& prog, SgArgs& a, int force_bytecode, int sm_count, in
             geom->template_id = 0;
             geom->grid = (int)blocks;
             geom->tile = BLOCK * V;
-            geom->vm_cells = 1;
+            geom->vm_cfg = 0;
             size_t off = (size_t)geom->grid * SG_MAX_OUT * sizeof(Cell);
             for (int o = 0; o < prog.shape.n_out; ++o) {
                 a.ws_off[o] = 0;
@@ -191,9 +191,12 @@ int sgk_plan(const SgProg& prog, SgArgs& a, int force_bytecode, int sm_count, in
     // 1-D pass.  Template instances need every vector operand congruent (common head); otherwise the bytecode
     // kernel runs with per-operand 128-bit eligibility.
     if (tid && !congruent) tid = 0;
-    const int cells = vm_cells(prog.shape.n_vreg);
-    const int tile = tid ? g_entries[tid].tile : vm_tile(es, cells);
-    geom->vm_cells = cells;
+    const int vcfg = vm_pick_config(prog);
+    const int tile = tid ? g_entries[tid].tile : vm_tile_cfg(es, vcfg);
+    geom->vm_cfg = vcfg;
+    int vm_r = 0, vm_i = 0;
+    vm_count_regs(prog, &vm_r, &vm_i);
+    const int file_kib = (int)((vm_file_bytes_cfg(vm_r, vm_i, vcfg) + 1023) / 1024);
     long lmin = a.n;
     for (int o = 0; o < prog.shape.n_out; ++o) lmin = std::min<long>(lmin, a.out_len[o]);
     const long head = std::min<long>((V - mis) % V, a.n);
@@ -201,7 +204,7 @@ int sgk_plan(const SgProg& prog, SgArgs& a, int force_bytecode, int sm_count, in
     a.head = head;
     a.n_full_tiles = body / tile;
     a.vec_ok = vec_ok;
-    const int occ = has_device ? (tid ? g_entries[tid].occupancy() : occupancy_bytecode(prog.shape.dtype, false, prog.shape.n_vreg, cells)) : 4;
+    const int occ = has_device ? (tid ? g_entries[tid].occupancy() : occupancy_bytecode(prog.shape.dtype, false, file_kib, vcfg)) : 4;
     long want = tid ? a.n_full_tiles : ((a.n - head + tile - 1) / tile + (head + tile - 1) / tile);
     geom->template_id = tid;
     geom->tile = tile;

@@ -15,7 +15,7 @@ struct SgGeom {
     size_t ws_bytes;        // workspace bytes this launch needs (partial cells)
     size_t state_words;     // filter: tile-state words needed
     int ctrl_words;         // control words needed beyond the first 8 (2-D tickets)
-    int vm_cells;           // bytecode 1-D pass: cells per VM register (1 or 2)
+    int vm_cfg;             // bytecode 1-D pass: configuration index (threads per block, cells per register: vm_config in sg_pass1d_vm.cuh)
 };
 
 // Registry of precompiled template instances (sg_templates_gen.inc).

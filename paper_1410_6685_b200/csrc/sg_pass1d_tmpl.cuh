@@ -250,7 +250,10 @@ __global__ void __launch_bounds__(BLOCK, P::min_blocks) pass1d_template(const __
             // every POLL-th tile the decided word is requested together with the tile's loads and examined after the tile is
             // processed, so the poll costs no extra round trip on the clean path (a strong load per tile measurably slows the
             // stream: 220 -> 184 us on config 3)
-            constexpr unsigned int POLL = 8;
+#ifndef SG_POLL
+#define SG_POLL 8
+#endif
+            constexpr unsigned int POLL = SG_POLL;
             unsigned int decided_word = 0;
             const bool poll = M::early_exit && !a.no_early_exit && (it % POLL) == 0;
             if constexpr (M::early_exit) {

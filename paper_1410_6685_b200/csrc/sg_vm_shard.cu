@@ -17,11 +17,14 @@ namespace {
 
 using namespace sgk;
 
-template <class T, int C> cudaError_t launch_pass1d_bytecode(const SgProg& g, const SgArgs& a, int grid, cudaStream_t s) {
+template <class T, int CFG> cudaError_t launch_pass1d_bytecode(const SgProg& g, const SgArgs& a, int grid, cudaStream_t s) {
+    constexpr int VB = vm_config(CFG).threads, C = vm_config(CFG).cells;
     static bool attr_dev[SG_MAX_DEVICES] = {};
     bool& attr_set = attr_dev[current_device_slot()];
-    if (!attr_set) { cudaFuncSetAttribute(pass1d_bytecode<T, C>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)vm_file_bytes(VM_VREG, 1)); attr_set = true; }
-    return sgk_launch_pdl(pass1d_bytecode<T, C>, grid, BLOCK, vm_file_bytes(g.shape.n_vreg, C), s, g, a);
+    if (!attr_set) { cudaFuncSetAttribute(pass1d_bytecode<T, VB, C>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)VM_MAX_FILE_BYTES); attr_set = true; }
+    int r, i;
+    vm_count_regs(g, &r, &i);
+    return sgk_launch_pdl(pass1d_bytecode<T, VB, C>, grid, VB, vm_file_bytes_cfg(r, i, CFG), s, g, a);
 }
 template <class T> cudaError_t launch_bytecode_t(const SgProg& g, const SgArgs& a, const SgGeom& geom, cudaStream_t s) {
     if (g.shape.flags & PF_2D) {
@@ -36,35 +39,41 @@ template <class T> cudaError_t launch_bytecode_t(const SgProg& g, const SgArgs& 
         if (!attr_set) { cudaFuncSetAttribute(filter1d_bytecode<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FilterBytecodeEval<T>::SMEM); attr_set = true; }
         return sgk_launch_pdl(filter1d_bytecode<T>, geom.grid, BLOCK + 32, FilterBytecodeEval<T>::SMEM, s, g, a);
     }
-    return geom.vm_cells == 2 ? launch_pass1d_bytecode<T, 2>(g, a, geom.grid, s) : launch_pass1d_bytecode<T, 1>(g, a, geom.grid, s);
+    switch (geom.vm_cfg) {
+        case 2: return launch_pass1d_bytecode<T, 2>(g, a, geom.grid, s);
+        case 1: return launch_pass1d_bytecode<T, 1>(g, a, geom.grid, s);
+        default: return launch_pass1d_bytecode<T, 0>(g, a, geom.grid, s);
+    }
 }
-// blocks per SM of the bytecode kernels (the 1-D pass depends on the size of its register file: queried once per size)
-template <class T> int occupancy_bytecode_t(bool filter, int n_vreg, int cells) {
-    static int cached_filter_dev[SG_MAX_DEVICES] = {}, cached_dev[SG_MAX_DEVICES][VM_VREG + 1][VM_MAX_CELLS + 1] = {};
-    const int slot = current_device_slot();
-    int& cached_filter = cached_filter_dev[slot];
-    int (&cached)[VM_VREG + 1][VM_MAX_CELLS + 1] = cached_dev[slot];
+template <class T, int CFG> int occupancy_pass1d(size_t smem) {
+    constexpr int VB = vm_config(CFG).threads, C = vm_config(CFG).cells;
     int occ = 0;
-    cudaError_t e;
+    cudaFuncSetAttribute(pass1d_bytecode<T, VB, C>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)VM_MAX_FILE_BYTES);
+    if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, pass1d_bytecode<T, VB, C>, VB, smem) != cudaSuccess || occ <= 0) { cudaGetLastError(); return 1; }
+    return occ;
+}
+// blocks per SM of the bytecode kernels (the 1-D pass depends on the size of its register file: one query per size and configuration)
+template <class T> int occupancy_bytecode_t(bool filter, int file_kib, int cfg) {
+    static int cached_filter_dev[SG_MAX_DEVICES] = {}, cached_dev[SG_MAX_DEVICES][VM_NCFG][128] = {};
+    const int slot = current_device_slot();
     if (filter) {
+        int& cached_filter = cached_filter_dev[slot];
         if (cached_filter > 0) return cached_filter;
+        int occ = 0;
         cudaFuncSetAttribute(filter1d_bytecode<T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)FilterBytecodeEval<T>::SMEM);
-        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, filter1d_bytecode<T>, BLOCK + 32, FilterBytecodeEval<T>::SMEM);
-        if (e != cudaSuccess || occ <= 0) return 1;
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, filter1d_bytecode<T>, BLOCK + 32, FilterBytecodeEval<T>::SMEM) != cudaSuccess || occ <= 0) { cudaGetLastError(); return 1; }
         return cached_filter = occ;
     }
-    n_vreg = std::min(std::max(n_vreg, 1), VM_VREG);
-    if (cached[n_vreg][cells] > 0) return cached[n_vreg][cells];
-    const size_t smem = vm_file_bytes(n_vreg, cells);
-    if (cells == 2) {
-        cudaFuncSetAttribute(pass1d_bytecode<T, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)vm_file_bytes(VM_VREG, 1));
-        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, pass1d_bytecode<T, 2>, BLOCK, smem);
-    } else {
-        cudaFuncSetAttribute(pass1d_bytecode<T, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)vm_file_bytes(VM_VREG, 1));
-        e = cudaOccupancyMaxActiveBlocksPerMultiprocessor(&occ, pass1d_bytecode<T, 1>, BLOCK, smem);
+    cfg = std::min(std::max(cfg, 0), VM_NCFG - 1);
+    file_kib = std::min(std::max(file_kib, 1), 127);
+    int& cached = cached_dev[slot][cfg][file_kib];
+    if (cached > 0) return cached;
+    const size_t smem = (size_t)file_kib * 1024;
+    switch (cfg) {
+        case 2: return cached = occupancy_pass1d<T, 2>(smem);
+        case 1: return cached = occupancy_pass1d<T, 1>(smem);
+        default: return cached = occupancy_pass1d<T, 0>(smem);
     }
-    if (e != cudaSuccess || occ <= 0) return 1;
-    return cached[n_vreg][cells] = occ;
 }
 }  // namespace
 
@@ -73,6 +82,6 @@ template <class T> int occupancy_bytecode_t(bool filter, int n_vreg, int cells) 
 cudaError_t SG_CAT(sgk_launch_bytecode_, SG_VM_DTYPE)(const SgProg& g, const SgArgs& a, const SgGeom& geom, cudaStream_t s) {
     return launch_bytecode_t<sgk::TypeOf<SG_VM_DTYPE>::type>(g, a, geom, s);
 }
-int SG_CAT(sgk_occupancy_bytecode_, SG_VM_DTYPE)(bool filter, int n_vreg, int cells) {
-    return occupancy_bytecode_t<sgk::TypeOf<SG_VM_DTYPE>::type>(filter, n_vreg, cells);
+int SG_CAT(sgk_occupancy_bytecode_, SG_VM_DTYPE)(bool filter, int file_kib, int cfg) {
+    return occupancy_bytecode_t<sgk::TypeOf<SG_VM_DTYPE>::type>(filter, file_kib, cfg);
 }
