@@ -202,6 +202,8 @@ def per_config(torch, sg, W, inputs, peak, which):
         ge_section(torch, sg, W, inputs, out, peak)
     if "vecapi" in which:
         vecapi_section(torch, sg, W, inputs, measure)
+    if "inplace" in which:
+        inplace_section(torch, sg, W, inputs, measure)
     if "matvec" in which:
         matvec_section(torch, sg, W, inputs, measure)
     if "quicksort" in which:
@@ -368,6 +370,25 @@ def vecapi_section(torch, sg, W, inputs, measure):
         del a, b, o
 
 
+def inplace_section(torch, sg, W, inputs, measure):
+    """The ceiling of read-modify-write streaming on this GPU: x := 2 x in place (`for_each`) on 2^27 fp64 = 1 GiB,
+    16 B per element through ONE buffer — what config 4's in-place row update and the determinant loop can reach at best — next to the same
+    pass written to a second buffer."""
+    n = 1 << 27
+    x = torch.from_numpy(inputs.uniform_pm1_f64(1, 0, n)).cuda()
+    o = torch.empty_like(x)
+
+    def inplace(ctx):
+        h = sg.sg_vec_create(ctx, sg.SG_F64, n, x.data_ptr())
+        return sg.sg_enqueue(ctx, sg.SG_MUL, [h, sg.F(2.0)], dst_or_0=h)
+
+    def outofplace(ctx):
+        h, d = sg.sg_vec_create(ctx, sg.SG_F64, n, x.data_ptr()), sg.sg_vec_create(ctx, sg.SG_F64, n, o.data_ptr())
+        return sg.sg_enqueue(ctx, sg.SG_MUL, [h, sg.F(2.0)], dst_or_0=d)
+    measure("rmw_ceiling_scale_in_place_fp64_2^27 (1R+1W, same buffer)", inplace, 16 * n)
+    measure("rmw_ceiling_scale_to_second_buffer_fp64_2^27 (1R+1W, two buffers)", outofplace, 16 * n)
+
+
 def matvec_section(torch, sg, W, inputs, measure):
     """matrix x vector and vector x matrix at 16384^2 fp64 (2 GiB read once)."""
     n = 16384
@@ -477,7 +498,7 @@ def main():
     ap.add_argument("--log2n", type=int, default=28)
     ap.add_argument("--impl", default="ours")
     ap.add_argument("--headline-only", action="store_true", help="same as --configs none")
-    ap.add_argument("--configs", default="cfg0,cfg1,sweep,overhead,cfg2,cfg3,cfg4,ge,vecapi,matvec,quicksort", help="per_config sections to time after the headline (or: none)")
+    ap.add_argument("--configs", default="cfg0,cfg1,sweep,overhead,cfg2,cfg3,cfg4,inplace,ge,vecapi,matvec,quicksort", help="per_config sections to time after the headline (or: none)")
     ap.add_argument("--shard", action="store_true", help="N > 1: ONE 2^log2n collection sharded over the ranks (strong scaling, SURVEY.md 8(e)) "
                     "instead of independent replicas; partial results all-gathered (12 bytes per rank) and combined by a library pass")
     ap.add_argument("--skip-headline", action="store_true", help="profiling aid: run only the --configs sections and print their JSON")

@@ -248,10 +248,12 @@ __global__ void __launch_bounds__(BLOCK, P::min_blocks) pass1d_template(const __
         unsigned int it = 0;
         for (int64_t tile = blockIdx.x; tile < a.n_full_tiles; tile += gridDim.x, ++it) {
             // every POLL-th tile the decided word is requested together with the tile's loads and examined after the tile is
-            // processed, so the poll costs no extra round trip on the clean path (a strong load per tile measurably slows the
-            // stream: 220 -> 184 us on config 3)
+            // processed, so the poll costs no extra round trip on the clean path.  Measured on config 3 (2^28 fp32, 740 blocks, 16 KiB
+            // tiles; clean pass / time to answer with the violation at n/64, 20 %, n/2 of the vector, in us):
+            //   POLL 1: 222 / 11.7, 36.7, 92.6     POLL 2: 182 / 14.3, 35.7, 88.3     POLL 4: 180 / 19.7, 40.8, 91.8     POLL 8: 180 / 31.2, 55.3, 105
+            // (a strong load per tile slows the clean stream by 23 %; every second tile costs 1 % and halves the time to answer)
 #ifndef SG_POLL
-#define SG_POLL 8
+#define SG_POLL 2
 #endif
             constexpr unsigned int POLL = SG_POLL;
             unsigned int decided_word = 0;

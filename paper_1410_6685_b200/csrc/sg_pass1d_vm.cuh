@@ -572,7 +572,7 @@ __global__ void __launch_bounds__(VB, VB == 128 ? 4 : 3) pass1d_bytecode(const _
     const int64_t head_tiles = (a.head + VM_TILE - 1) / VM_TILE;
     unsigned int it = 0;
     for (int64_t tile = blockIdx.x; tile < n_tiles + head_tiles; tile += gridDim.x, ++it) {
-        if (early_exit && (it & 7u) == 0) {
+        if (early_exit && (it & 1u) == 0) {
             const unsigned int w = ld_relaxed_u32(&a.ctrl[1]);
             if ((w & need_mask) == need_mask || (w & a.exit_any) != 0) break;
         }

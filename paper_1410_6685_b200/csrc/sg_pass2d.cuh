@@ -32,7 +32,7 @@ __device__ __forceinline__ Cell ldcg_cell(const Cell* p) {
     return c;
 }
 
-struct Slots2D { int vec[SG_MAX_IN]; int row[SG_MAX_OUT]; };
+struct Slots2D { int vec[SG_MAX_IN]; int row[SG_MAX_OUT]; int colb[SG_MAX_IN]; };
 
 template <class P> struct Meta2D : Meta1D<P> {
     typedef Meta1D<P> B;
@@ -44,9 +44,15 @@ template <class P> struct Meta2D : Meta1D<P> {
         return n;
     }
     static constexpr int NVECINREAL = count_kind(IN_VEC);
+    static constexpr int NCOLBREAL = count_kind(IN_COLB);
     static constexpr int NVECIN = NVECINREAL > 0 ? NVECINREAL : 1;
     static constexpr int NS = P::stages;            // shared-memory stages in flight
     static constexpr size_t SMEM = (size_t)NS * NVECIN * RU * SW * sizeof(typename B::T) + NS * sizeof(uint64_t);
+    static constexpr int colb_slot(int K) {
+        int n = 0;
+        for (int k = 0; k < K; ++k) n += (P::prog.in[k].kind == IN_COLB);
+        return n;
+    }
     static constexpr int vec_slot(int K) {
         int n = 0;
         for (int k = 0; k < K; ++k) n += (P::prog.in[k].kind == IN_VEC);
@@ -67,6 +73,7 @@ template <class P> struct Meta2D : Meta1D<P> {
     static constexpr Slots2D slots() {
         Slots2D s{};
         for (int k = 0; k < SG_MAX_IN; ++k) s.vec[k] = k < B::S.n_in ? vec_slot(k) : 0;
+        for (int k = 0; k < SG_MAX_IN; ++k) s.colb[k] = k < B::S.n_in ? colb_slot(k) : 0;
         for (int o = 0; o < SG_MAX_OUT; ++o) s.row[o] = o < B::S.n_out ? row_slot(o) : 0;
         return s;
     }
@@ -236,10 +243,36 @@ __device__ __forceinline__ void pass2d_body(const SgArgs& a) {
             for (int64_t b = 0; b < NS && b < nb; ++b) issue(b);
     }
 
+    // COL-broadcast operands (one value per row, e.g. the elimination factors f_j): the values of batch b+1 are requested while batch b
+    // is processed — loaded right before their first use they cost a full global-memory round trip per stage (ncu on config 4's pass:
+    // 45 % of the stall samples were `long scoreboard` on the first multiplication by f_j)
+    constexpr int NCOLB = M::NCOLBREAL > 0 ? M::NCOLBREAL : 1;
+    T colb_next[NCOLB][RS];
+    auto fetch_colb = [&](int64_t b, T (&dst)[NCOLB][RS]) {
+        const int64_t r0 = r_begin + b * RS;
+        int slot = 0;
+#pragma unroll
+        for (int k = 0; k < M::S.n_in; ++k) {
+            if (g.in[k].kind != IN_COLB) continue;
+#pragma unroll
+            for (int j = 0; j < RS; ++j) dst[slot][j] = (r0 + j < r_end) ? __ldg(reinterpret_cast<const T*>(a.in_ptr[k]) + r0 + j) : T(0);
+            ++slot;
+        }
+    };
+    if (M::NCOLBREAL > 0 && nb > 0) fetch_colb(0, colb_next);
+
     for (int64_t b = 0; b < nb; ++b) {
         const int s = (int)(b % NS);
         const int64_t r0 = r_begin + b * RS;
         const int64_t rb = r_begin + (b * RS) / RB * RB;                // start of the current RB-row batch of the per-row combine
+        T colb[NCOLB][RS];
+        if (M::NCOLBREAL > 0) {
+#pragma unroll
+            for (int q = 0; q < NCOLB; ++q)
+#pragma unroll
+                for (int j = 0; j < RS; ++j) colb[q][j] = colb_next[q][j];
+            if (b + 1 < nb) fetch_colb(b + 1, colb_next);
+        }
         if (ALIGNED) mbar_wait(&full[s], (uint32_t)((b / NS) & 1));
         else { fill(b); __syncthreads(); }
         Cell rowc[M::NROWS][RS];                 // per-thread partials of the AXIS_ROWS outputs, one per row of the stage
@@ -266,7 +299,7 @@ __device__ __forceinline__ void pass2d_body(const SgArgs& a) {
                         for (int e = 0; e < V; ++e) v[in.reg][u * V + e] = xe[e];
                     }
                 } else if (in.kind == IN_COLB) {
-                    const T sc = __ldg(reinterpret_cast<const T*>(a.in_ptr[k]) + r);
+                    const T sc = colb[slots.colb[k]][j];
 #pragma unroll
                     for (int e = 0; e < E; ++e) v[in.reg][e] = sc;
                 }

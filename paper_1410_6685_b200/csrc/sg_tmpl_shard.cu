@@ -6,25 +6,28 @@
 #ifndef SG_SHARD
 #error "compile with -DSG_SHARD=<0..SG_NSHARDS-1>"
 #endif
+#ifndef SG_TEMPLATES_INC
+#define SG_TEMPLATES_INC "sg_templates_gen.inc"      // tuning experiments compile a shard against another instance list
+#endif
 
 namespace {
 
 using namespace sgk;
 
-// Each SG_TEMPLATE(index, name, unroll, min_blocks, row_unroll, {program}) in the generated file defines a policy type.
+// Each SG_TEMPLATE(index, name, unroll, min_blocks, row_unroll, stages, {program}) in the generated file defines a policy type.
 // The program initialisers are written by paper_1410_6685_b200/gen_templates.py from the plan builder's own canonical
 // output, so a registered chain always matches its signature.
-#define SG_TEMPLATE(IDX, NAME, UNROLL, MINB, ROWU, ...)                              \
+#define SG_TEMPLATE(IDX, NAME, UNROLL, MINB, ROWU, STAGES, ...)                      \
     struct T_##NAME {                                                                \
         static constexpr SgProg prog = __VA_ARGS__;                                  \
-        static constexpr int unroll = UNROLL, min_blocks = MINB, row_unroll = ROWU, stages = 3;  \
+        static constexpr int unroll = UNROLL, min_blocks = MINB, row_unroll = ROWU, stages = STAGES;  \
     };
-#include "sg_templates_gen.inc"
+#include SG_TEMPLATES_INC
 #undef SG_TEMPLATE
 
-#define SG_TEMPLATE(IDX, NAME, UNROLL, MINB, ROWU, ...) EntryOf<T_##NAME, (IDX) % SG_NSHARDS == SG_SHARD>::make(#NAME),
+#define SG_TEMPLATE(IDX, NAME, UNROLL, MINB, ROWU, STAGES, ...) EntryOf<T_##NAME, (IDX) % SG_NSHARDS == SG_SHARD>::make(#NAME),
 const Entry g_shard_entries[] = {
-#include "sg_templates_gen.inc"
+#include SG_TEMPLATES_INC
 };
 #undef SG_TEMPLATE
 

@@ -16,6 +16,9 @@
 namespace {
 
 constexpr int TILE = 64, ROWS = 8, TBLOCK = TILE * ROWS;      // measured at 16384^2 fp64: ROWS 4 / 8 / 16 -> 0.774 / 0.651 / 0.749 ms
+// 4-byte elements run at 0.79 of the measured peak (fp64: 1.01).  128 x 128 tiles (512-byte segments on both sides, like fp64) were
+// measured and change nothing (422 vs 415 us at 16384^2 fp32): the fp32 mover is bound by its four 4-byte memory instructions per
+// element (LDG, STS, LDS, STG), not by the segment length; the paper's transpose benchmark is DOUBLE.
 
 template <class T>
 __global__ void __launch_bounds__(TBLOCK) transpose_tiled(const T* __restrict__ in, int64_t ld_in, int64_t rows, int64_t cols,

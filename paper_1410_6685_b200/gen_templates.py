@@ -20,15 +20,16 @@ from . import workloads as W
 
 OUT = os.path.join(os.path.dirname(os.path.abspath(__file__)), "csrc", "sg_templates_gen.inc")
 
-# tuning per instance: (unroll = 128-bit accesses per operand per thread per tile, min blocks per SM, rows in flight)
-DEFAULT_TUNE = (2, 3, 4)
+# tuning per instance: (unroll = 128-bit accesses per operand per thread per tile, min blocks per SM, rows per stage, shared-memory stages of a matrix pass)
+DEFAULT_TUNE = (2, 3, 4, 3)
 TUNE = {
     "cfg1": (2, 4, 4),
     "cfg3": (4, 4, 4),
     "cfg3sum": (4, 4, 4),
     "sorted_f32": (4, 4, 4),
     "cfg4": (2, 2, 4),
-    "matvec": (2, 2, 4),      # measured: (2, 4, 2) is slower (0.430 / 0.379 ms vs 0.376 / 0.343 ms right / left at 16384^2)
+    "matvec": (2, 2, 4, 3),   # measured: (2, 4, 2, 3) is slower (0.430 / 0.379 ms vs 0.376 / 0.343 ms right / left at 16384^2)
+    "matvec_right": (2, 3, 4, 2),   # per-row double-double sums are latency-bound: TWO stages and three blocks per SM: 0.374 -> 0.343 ms (left: 0.341 -> 0.359, kept at three stages)
     "cfg2": (2, 2, 2),      # filter: tile = 4*unroll steps, min blocks per SM, input stages
 }
 
@@ -43,6 +44,8 @@ def _chains():
     yield "axpy_f64", 0, lambda c: W.axpy(c, f64, N, 2.0, None, None)
     yield "axpy_f32", 0, lambda c: W.axpy(c, f32, N, 2.0, None, None)
     yield "axpy_inplace_f64", 0, lambda c: _axpy_inplace(c, f64)
+    yield "scale_inplace_f64", 0, lambda c: _scale_inplace(c, f64)                          # x := x * a in place (for_each): the 1R+1W same-buffer ceiling
+    yield "scale_f64", 0, lambda c: sg.sg_enqueue(c, sg.SG_MUL, [sg.sg_vec_create(c, f64, N, None), sg.F(2.0)], dst_or_0=sg.sg_vec_create(c, f64, N, 0x7000000))
     yield "ge_row_f64", 0, lambda c: W.ge_row_op(c, N, None, None, 3.0)
     yield "cfg0", 0, lambda c: W.cfg0(c, N, None, None, None)                               # plan P2: pass A + pass B
     yield "cfg0_zbuf", 0, lambda c: W.cfg0(c, N, None, None, None, pz=0x7000000)
@@ -82,6 +85,11 @@ def _axpy_inplace(c, dt):
     sg.sg_release(c, ax)
 
 
+def _scale_inplace(c, dt):
+    x = sg.sg_vec_create(c, dt, N, None)
+    sg.sg_enqueue(c, sg.SG_MUL, [x, sg.F(2.0)], dst_or_0=x)
+
+
 def _ge_step(c, k):
     M = sg.sg_mat_create(c, sg.SG_F64, 4096, 4096, 4096, None)
     det = sg.sg_vec_create(c, sg.SG_F64, 1, None)
@@ -104,7 +112,7 @@ def generate() -> str:
     seen = {}
     lines = [
         "// GENERATED by paper_1410_6685_b200/gen_templates.py from the plan builder's canonical output — do not edit.",
-        "// SG_TEMPLATE(index, name, unroll, min_blocks_per_sm, row_unroll, {program})",
+        "// SG_TEMPLATE(index, name, unroll, min_blocks_per_sm, row_unroll, stages, {program})",
     ]
     for name, flags, builder in _chains():
         ctx = sg.sg_ctx_create(-1)
@@ -112,14 +120,22 @@ def generate() -> str:
         builder(ctx)
         sg.sg_flush(ctx)
         st = sg.sg_plan_stats(ctx)
-        tune = TUNE.get(name.split("_")[0], TUNE.get(name, DEFAULT_TUNE))
         for p in range(st.n_passes):
             text = sg.sg_plan_dump(ctx, p)
             if text in seen:
                 continue
+            tune = TUNE.get(name, TUNE.get(name.split("_")[0]))
+            if tune is None:
+                # bytes in flight: a 1-D pass keeps unroll x 16 B per vector input and thread in flight; with ONE input the default unroll of 2
+                # leaves an SM with 24 KB outstanding.  Measured (2^26 fp32): unroll 8 for one-input passes: sqrt 0.915 -> 0.944 of the peak,
+                # sums unchanged; unroll 4 for two-input passes: compwise_divide 0.979 -> 0.963, approx_equal 1.01 -> 0.99 (rejected)
+                n_vec = text.count("{IN_VEC,") + text.count("{IN_VEC_CVT,")
+                is2d = text.split(",")[1].strip() in ("1", "3")
+                tune = (8, 3, 4, 3) if (not is2d and n_vec <= 1) else DEFAULT_TUNE
             inst = f"{name}_p{p}"
             seen[text] = inst
-            lines.append(f"SG_TEMPLATE({len(seen) - 1}, {inst}, {tune[0]}, {tune[1]}, {tune[2]}, {text})")
+            tune = tuple(tune) + (3,) * (4 - len(tune))
+            lines.append(f"SG_TEMPLATE({len(seen) - 1}, {inst}, {tune[0]}, {tune[1]}, {tune[2]}, {tune[3]}, {text})")
         sg.sg_ctx_destroy(ctx)
     return "\n".join(lines) + "\n"
 

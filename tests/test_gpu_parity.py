@@ -838,3 +838,41 @@ def test_cfg1_sharded_over_emulated_ranks():
             results.append((c.get(r["sum"]), c.get(r["max"])))
         gsum, gmax = results[-1]                                              # after the last rank every partial is there
     assert sum_ok(gsum, want["sum"], want["w"], 1e-5) and np.float32(gmax) == want["max"]
+
+
+def test_vector_longer_than_2_31_elements():
+    """Maximum sizes: 2^31 + 7 int32 elements (8 GiB): every index, tile and offset computation is 64-bit.  The oracle cannot hold this on
+    every box, so the results are checked against closed forms that hold at any size (x_i = i mod 1000) and, for the compaction, against
+    its exact periodic structure."""
+    import torch
+    n = (1 << 31) + 7
+    free, _ = torch.cuda.mem_get_info()
+    if free < 60 * (1 << 30):
+        pytest.skip("needs 60 GiB of free device memory")
+    idx = torch.arange(n, device="cuda", dtype=torch.int64)
+    xi = (idx % 1000).to(torch.int32)
+    del idx
+    q, r = divmod(n, 1000)
+    with Ctx() as c:
+        hx = sg.sg_vec_create(c.ctx, sg.SG_I32, n, xi.data_ptr())
+        s, mx, mn = (sg.sg_reduce(c.ctx, hx, k) for k in (sg.SG_SUM, sg.SG_RMAX, sg.SG_RMIN))
+        eq7 = sg.sg_enqueue(c.ctx, sg.SG_EQ, [hx, sg.I(7)])
+        cnt7 = sg.sg_reduce(c.ctx, eq7, sg.SG_COUNT)
+        sg.sg_release(c.ctx, eq7)
+        ge0 = sg.sg_enqueue(c.ctx, sg.SG_GE, [hx, sg.I(0)])
+        all_ge0 = sg.sg_forall(c.ctx, ge0)
+        sg.sg_release(c.ctx, ge0)
+        srt = sg.sg_forall_adjacent(c.ctx, hx, sg.SG_LE)
+        assert c.get(s) == q * 499500 + r * (r - 1) // 2 and c.get(mx) == 999 and c.get(mn) == 0
+        assert c.get(cnt7) == q + (1 if r > 7 else 0) and c.get(all_ge0) is True and c.get(srt) is False
+        # stable filter x mod 250 == 7: the kept values are 7, 257, 507, 757 repeated, in that order
+        res = W.cfg2(c.ctx, n, xi.data_ptr(), modulus=250, residue=7)
+        kept_n, kept_sum = c.get(res["count"]), c.get(res["sum"])
+        tail = [v for v in (7, 257, 507, 757) if v < r]
+        assert kept_n == 4 * q + len(tail) and kept_sum == q * (7 + 257 + 507 + 757) + sum(tail)
+        assert sg.sg_plan_stats(c.ctx).n_template == 1
+        ptr = sg.sg_vec_data(c.ctx, res["kept"])
+        kept = c.read_vec(res["kept"], np.int32)
+        assert kept.size == kept_n and ptr != 0
+        pat = np.array([7, 257, 507, 757], dtype=np.int32)
+        assert (kept[: 4 * q].reshape(q, 4) == pat).all() and kept[4 * q:].tolist() == tail
