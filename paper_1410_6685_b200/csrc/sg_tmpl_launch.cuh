@@ -28,8 +28,8 @@ typedef int (*OccFn)();
 
 
 template <class P> constexpr int tile_of() {
-    if (P::prog.shape.flags & PF_FILTER) return FilterTemplateEval<P>::TILE;
-    return BLOCK * Meta1D<P>::E;
+    if constexpr ((P::prog.shape.flags & PF_FILTER) != 0) return FilterTemplateEval<P>::TILE;
+    else return BLOCK * Meta1D<P>::E;
 }
 
 // TMA tensor map of one filter input: the vector seen as `rows` rows of 128 bytes, box = 256 rows (one tile), 128-byte

@@ -126,12 +126,9 @@ def generate() -> str:
                 continue
             tune = TUNE.get(name, TUNE.get(name.split("_")[0]))
             if tune is None:
-                # bytes in flight: a 1-D pass keeps unroll x 16 B per vector input and thread in flight; with ONE input the default unroll of 2
-                # leaves an SM with 24 KB outstanding.  Measured (2^26 fp32): unroll 8 for one-input passes: sqrt 0.915 -> 0.944 of the peak,
-                # sums unchanged; unroll 4 for two-input passes: compwise_divide 0.979 -> 0.963, approx_equal 1.01 -> 0.99 (rejected)
-                n_vec = text.count("{IN_VEC,") + text.count("{IN_VEC_CVT,")
-                is2d = text.split(",")[1].strip() in ("1", "3")
-                tune = (8, 3, 4, 3) if (not is2d and n_vec <= 1) else DEFAULT_TUNE
+                # measured and rejected (2^26 fp32 / 2^25 fp64, of the measured peak): unroll 8 for passes with ONE vector input — sqrt 0.94 ->
+                # 0.88 / 0.97 -> 0.90, scale 0.92 -> 0.935, sums unchanged: the default stays
+                tune = DEFAULT_TUNE
             inst = f"{name}_p{p}"
             seen[text] = inst
             tune = tuple(tune) + (3,) * (4 - len(tune))
