@@ -219,10 +219,14 @@ def cfg0_section(torch, sg, W, inputs, measure):
     measure("cfg0_onepass (z released, L2-warm)", lambda ctx: W.cfg0(ctx, n0, a.data_ptr(), b.data_ptr(), c.data_ptr(), keep_z=False), 24 << 20, 200, graph=True)
     # the floor of ANY pass: a one-element pass (nothing to stream) — launch latency + the kernel's fixed prologue / epilogue
     one = torch.ones(1, dtype=torch.float64, device="cuda")
-    measure("launch_floor_one_element_pass (x + 1 on a 1-element vector)",
-            lambda ctx: sg.sg_enqueue(ctx, sg.SG_ADD, [sg.sg_vec_create(ctx, sg.SG_F64, 1, one.data_ptr()), sg.F(1.0)]), 16, 200, graph=True)
-    measure("launch_floor_one_element_reduction (sum of a 1-element vector: ticket epilogue)",
+    one32, out32 = torch.ones(1, dtype=torch.float32, device="cuda"), torch.ones(1, dtype=torch.float32, device="cuda")
+    measure("launch_floor_one_element_pass (x + 0.5 on a 1-element fp32 vector, template instance)",
+            lambda ctx: sg.sg_enqueue(ctx, sg.SG_ADD, [sg.sg_vec_create(ctx, sg.SG_F32, 1, one32.data_ptr()), sg.F(0.5)],
+                                      dst_or_0=sg.sg_vec_create(ctx, sg.SG_F32, 1, out32.data_ptr())), 8, 200, graph=True)
+    measure("launch_floor_one_element_reduction (sum of a 1-element fp64 vector, template instance)",
             lambda ctx: sg.sg_reduce(ctx, sg.sg_vec_create(ctx, sg.SG_F64, 1, one.data_ptr()), sg.SG_SUM), 8, 200, graph=True)
+    measure("launch_floor_one_element_pass_bytecode (x + 1 on a 1-element fp64 vector: no instance, the interpreter decodes its program per block)",
+            lambda ctx: sg.sg_enqueue(ctx, sg.SG_ADD, [sg.sg_vec_create(ctx, sg.SG_F64, 1, one.data_ptr()), sg.F(1.0)]), 16, 200, graph=True)
     # the same two plans with the L2 flushed before every repetition (a 256 MiB scratch buffer is overwritten outside the timed events)
     scratch = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
     measure("cfg0_fp64_2^20_chain_sum_max_min_contracts (L2-cold, 2 passes)", lambda ctx: W.cfg0(ctx, n0, a.data_ptr(), b.data_ptr(), c.data_ptr()), 64 << 20, 5,
