@@ -468,6 +468,7 @@ extern "C" sg_status sg_timing_end(sg_ctx* c, float* total_ms, int32_t* n_flushe
 
 extern "C" sg_status sg_replay_last(sg_ctx* c, int32_t reps, float* ms_per_rep) {
     if (!c || !ms_per_rep || reps <= 0) return SG_ERR_ARG;
+    SgDeviceScope dev_scope(c);
     if (c->plan_only) { *ms_per_rep = 0.f; return SG_OK; }
     if (c->last.empty()) return sg_fail(c, SG_ERR_ARG, "nothing to replay");
     cudaEventRecord(c->ev_t0, c->stream);

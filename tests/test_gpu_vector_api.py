@@ -254,6 +254,20 @@ def test_quicksort_levels_large_and_contracts():
         assert e.value.status == sg.SG_ERR_ALIAS
 
 
+def test_quicksort_levels_of_a_view_and_of_a_pending_collection():
+    """The argument may be a subset view (any alignment) or a pending collection (flushed first)."""
+    a = inputs_normal(50021)
+    with Ctx() as c:
+        h = c.vec(a)
+        view = sg.sg_vec_subset(c.ctx, h, 3, 50021 - 2)
+        got = c.read_vec(sg.sg_vec_quicksort(c.ctx, view), np.float32)
+        assert bits_equal(got, ocfg.quicksort(a[3:-2]))
+        neg = sg.sg_enqueue(c.ctx, sg.SG_NEG, [h])                          # pending when the sort is asked for
+        got = c.read_vec(sg.sg_vec_quicksort(c.ctx, neg), np.float32)
+        assert bits_equal(got, ocfg.quicksort(orc.unary("neg", a)))
+        assert bits_equal(c.read_vec(h, np.float32), a)
+
+
 def inputs_normal(n):
     from paper_1410_6685_b200 import inputs
     return inputs.normal_f32(2, 0, n)

@@ -432,3 +432,30 @@ def test_a_failed_flush_discards_the_pending_list_and_leaves_the_context_usable(
             sg.sg_release(ctx, h)
     finally:
         sg.sg_ctx_destroy(ctx)
+
+
+def test_composite_entry_points_on_a_plan_only_context():
+    """sg_vec_quicksort / sg_mat_transpose / sg_replay_last_graph check their arguments and flush pending work without a device."""
+    ctx = sg.sg_ctx_create(-1)
+    try:
+        v = sg.sg_vec_create(ctx, sg.SG_F32, 1000, None)
+        w = sg.sg_enqueue(ctx, sg.SG_MUL, [v, sg.F(2.0)])           # pending: the composite flushes it first (trigger (2), PAPER.md:284)
+        before = sg.sg_plan_stats(ctx).launches_total
+        out = sg.sg_vec_quicksort(ctx, w)
+        assert sg.sg_vec_count(ctx, out) == 1000 and sg.sg_plan_stats(ctx).n_passes == 1
+        assert sg.sg_plan_stats(ctx).launches_total > before
+        with pytest.raises(sg.SgError) as e:
+            sg.sg_vec_quicksort(ctx, sg.sg_vec_create(ctx, sg.SG_F32, 0, None))     # require a.count > 0 (PAPER.md:248)
+        assert e.value.status == sg.SG_ERR_EMPTY
+        b = sg.sg_enqueue(ctx, sg.SG_GT, [v, sg.F(0.0)])
+        with pytest.raises(sg.SgError) as e:
+            sg.sg_vec_quicksort(ctx, b)
+        assert e.value.status == sg.SG_ERR_DTYPE
+        with pytest.raises(sg.SgError) as e:
+            sg.sg_vec_quicksort(ctx, sg.sg_mat_create(ctx, sg.SG_F32, 4, 4, 4, None))
+        assert e.value.status == sg.SG_ERR_ARG
+        sg.sg_enqueue(ctx, sg.SG_ADD, [v, sg.F(1.0)])
+        sg.sg_flush(ctx)
+        assert sg.sg_replay_last_graph(ctx, 5) == (0.0, 0.0)       # nothing is launched on a plan-only context
+    finally:
+        sg.sg_ctx_destroy(ctx)
