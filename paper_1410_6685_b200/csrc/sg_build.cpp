@@ -204,9 +204,10 @@ sg_status sg_build_pass(sg_ctx* c, Pass& P, std::vector<char*>& temps, std::stri
             k = B.add_input(IN_SHIFT, nullptr, 0, 0, base, false, &fresh);
             fresh = false;
         } else if (want_pred) {
-            if (P.is2d || v.stride != 1) return sg_fail(c, SG_ERR_UNSUPPORTED, "BOOL matrix / strided BOOL operand read from memory");
-            k = B.add_input(IN_BOOLVEC, ptr, 1, 0, -1, true, &fresh);
-            if (fresh) { P.n_mem_in++; P.bytes += v.cols; }
+            if (v.stride != 1 || (P.is2d && v.kind != VK_MAT)) return sg_fail(c, SG_ERR_UNSUPPORTED, "strided or broadcast BOOL operand read from memory");
+            // a BOOL matrix (a mask somebody kept) is read back by the 2-D bytecode evaluator: in_stride = its leading dimension
+            k = B.add_input(IN_BOOLVEC, ptr, P.is2d ? v.ld : 1, 0, -1, true, &fresh);
+            if (fresh) { P.n_mem_in++; P.bytes += v.rows * v.cols; }
             fresh = false;
         } else if (P.is2d && v.kind == VK_VEC) {
             if (v.stride != 1) return sg_fail(c, SG_ERR_UNSUPPORTED, "strided broadcast vector");

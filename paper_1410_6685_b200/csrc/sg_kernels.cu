@@ -4,6 +4,7 @@
 #include <cuda.h>
 
 #include <stdio.h>
+#include <stdlib.h>
 #include <string.h>
 
 #include <algorithm>
@@ -55,6 +56,11 @@ int occupancy_bytecode(int dtype, bool filter, int n_vreg = 64 /* file KiB */, i
 }
 
 int elem_size(int dtype) { return (dtype == DT_F32 || dtype == DT_I32) ? 4 : 8; }
+
+long env_long(const char* name, long dflt) {
+    const char* s = getenv(name);
+    return (s && *s) ? atol(s) : dflt;
+}
 
 int fail(char* err, size_t cap, int code, const char* msg) {
     if (err && cap) snprintf(err, cap, "%s", msg);
@@ -142,7 +148,8 @@ int sgk_plan(const SgProg& prog, SgArgs& a, int force_bytecode, int sm_count, in
         const int occ = (has_device && tid) ? g_entries[tid].occupancy() : 2;
         const int SW = tid ? g_entries[tid].tile : BLOCK * 2 * V;
         a.n_strips = (int)((a.cols + SW - 1) / SW);
-        const long target = (long)sm_count * occ;
+        static const long mult2d = env_long("SG_GRID_MULT_2D", 1);
+        const long target = (long)sm_count * occ * mult2d;
         long max_chunks = std::max<long>(1, (a.n + RB - 1) / RB);
         long n_chunks = std::min<long>(max_chunks, std::max<long>(1, target / std::max(1, a.n_strips)));
         long rpc = (a.n + n_chunks - 1) / n_chunks;
@@ -208,7 +215,36 @@ int sgk_plan(const SgProg& prog, SgArgs& a, int force_bytecode, int sm_count, in
     long want = tid ? a.n_full_tiles : ((a.n - head + tile - 1) / tile + (head + tile - 1) / tile);
     geom->template_id = tid;
     geom->tile = tile;
-    geom->grid = (int)std::max<long>(1, std::min<long>(want, (long)sm_count * occ));
+    {
+        // Launch shape (measured on B200, profiles/r02_grid_shape.md).  Equal static shares of a persistent grid finish at very
+        // different times on this part: SM pairs differ up to 2x in WRITE throughput (1R+1W over 592 blocks: the median block is
+        // done 100 us before the last of 372 us), read-only streams by 6 % (10 us of 156 us).  So
+        //   * a pass that only stores (no epilogue) runs as many short-lived blocks of K_STORE strided tiles, the hardware block
+        //     scheduler balances them:      x := x * a, 2^27 fp64: 0.360 -> 0.313 ms (0.92 -> 1.06 of the measured copy peak);
+        //     K = 1 / 2 / 3 / 4 / 8: 0.310 / 0.313 / 0.315 / 0.316 / 0.322 ms in place, 0.354 / 0.312 / 0.313 / 0.315 / 0.320 to a second buffer;
+        //   * a pass with reductions keeps the persistent grid (one epilogue per block: 4096 blocks cost +9 %, 131072 blocks 3x)
+        //     but takes only the first PCT % of its share strided, the rest through tile tickets (sg_pass1d_tmpl.cuh):
+        //     read-only, PCT = 100 / 92 / 85 / 75 / 60: config 1 at 2^28 0.338 / 0.327 / 0.324 / 0.325 / 0.327 ms, sum(x) 0.161 / 0.155 /
+        //     0.160 / 0.169 / 0.174 ms; with stores (divide + contracts, 2^26), PCT = 100 / 50 / 30 / 0: 0.258 / 0.249 / 0.250 / 0.250 ms;
+        //   * early-exit passes stay static (their exit is taken per thread, the ticket loop needs a block-uniform one).
+        // The environment variables override the defaults for such sweeps; they are read once.
+        bool has_red = false, has_store = false;
+        for (int o = 0; o < prog.shape.n_out; ++o) {
+            has_red |= out_is_reduction(prog.out[o].kind);
+            has_store |= prog.out[o].kind == OUT_STORE || prog.out[o].kind == OUT_STORE_BOOL;
+        }
+        const bool ee = (prog.shape.flags & PF_EARLY_EXIT) != 0;
+        static const long k_store = env_long("SG_GRID_K_STORE", 2), k_red = env_long("SG_GRID_K_RED", 0), k_ee = env_long("SG_GRID_K_EE", 0);
+        static const long pct_ro = env_long("SG_STATIC_PCT_RO", 85), pct_rw = env_long("SG_STATIC_PCT_RW", 50), dyn_min = env_long("SG_DYN_MIN_ITERS", 8);
+        const long K = !tid ? 0 : ee ? k_ee : has_red ? k_red : k_store;     // the bytecode kernel decodes its program per block: persistent
+        long blocks = std::min<long>(want, (long)sm_count * occ);
+        if (K > 0) blocks = std::max<long>(blocks, (want + K - 1) / K);
+        geom->grid = (int)std::max<long>(1, blocks);
+        const long pct = has_store ? pct_rw : pct_ro;
+        const long per_block = a.n_full_tiles / geom->grid;
+        a.static_tiles = a.n_full_tiles;
+        if (tid && has_red && !ee && pct >= 0 && pct < 100 && per_block >= dyn_min) a.static_tiles = per_block * pct / 100 * geom->grid;
+    }
     geom->ws_bytes = (size_t)geom->grid * SG_MAX_OUT * sizeof(Cell);
     return 0;
 }

@@ -8,6 +8,12 @@
 
 namespace sgk {
 
+__host__ __device__ constexpr bool prog_has_reduction(const SgProg& g) {
+    for (int o = 0; o < g.shape.n_out; ++o)
+        if (out_is_reduction(g.out[o].kind)) return true;
+    return false;
+}
+
 template <class P> struct Meta1D {
     static constexpr SgShape S = P::prog.shape;
     typedef typename TypeOf<S.dtype>::type T;
@@ -20,6 +26,7 @@ template <class P> struct Meta1D {
     static constexpr int NP = S.n_preg > 0 ? S.n_preg : 1;
     static constexpr int NOUT = S.n_out > 0 ? S.n_out : 1;
     static constexpr bool early_exit = (S.flags & PF_EARLY_EXIT) != 0;
+    static constexpr bool has_reduction = prog_has_reduction(P::prog);
 };
 
 // ---- compile-time body: one fold over the instruction list, every register index is a constant --------
@@ -246,7 +253,7 @@ __global__ void __launch_bounds__(BLOCK, P::min_blocks) pass1d_template(const __
         bool p[M::NP][M::E];
         bcast_inputs<P, M::E>(v, a, KS);
         unsigned int it = 0;
-        for (int64_t tile = blockIdx.x; tile < a.n_full_tiles; tile += gridDim.x, ++it) {
+        for (int64_t tile = blockIdx.x; tile < a.static_tiles; tile += gridDim.x, ++it) {
             // every POLL-th tile the decided word is requested together with the tile's loads and examined after the tile is
             // processed, so the poll costs no extra round trip on the clean path.  Measured on config 3 (2^28 fp32, 740 blocks, 16 KiB
             // tiles; clean pass / time to answer with the violation at n/64, 20 %, n/2 of the vector, in us):
@@ -276,6 +283,30 @@ __global__ void __launch_bounds__(BLOCK, P::min_blocks) pass1d_template(const __
                         }
                     }
                     if ((decided_word & need_mask) == need_mask || (decided_word & a.exit_any) != 0) break;
+                }
+            }
+        }
+        // The tiles after static_tiles are handed out one by one through a ticket on ctrl[2], fetched one tile ahead by thread 0
+        // behind the tile's own loads.  Equal static shares finish at different times on this part (read-only stream over 592
+        // blocks: the median block is done 10 us before the last of 156 us; a 1R+1W stream: 100 us of 372 us, SM pairs differ 2x in
+        // write throughput), tickets over the last part of the body let every block finish together (profiles/r02_grid_shape.md).
+        // Only passes with reductions and no early exit take this path (the epilogue resets the counter).
+        if constexpr (!M::early_exit && M::has_reduction) {
+            if (a.static_tiles < a.n_full_tiles) {
+                __shared__ long long s_tile[2];
+                if (threadIdx.x == 0) s_tile[0] = a.static_tiles + atomicAdd(&a.ctrl[2], 1u);
+                __syncthreads();
+                for (int buf = 0;; buf ^= 1) {
+                    const int64_t tile = s_tile[buf];
+                    if (tile >= a.n_full_tiles) break;
+                    const int64_t base = a.head + tile * M::TILE;
+                    load_inputs_full<P>(v, p, a, base, KS);
+                    unsigned int ticket = 0;
+                    if (threadIdx.x == 0) ticket = atomicAdd(&a.ctrl[2], 1u);
+                    exec_body<P, T, M::NV, M::NP, M::E>(v, p, a, IS);
+                    emit_outputs_full<P>(v, p, acc, a, base, OS);
+                    if (threadIdx.x == 0) s_tile[buf ^ 1] = a.static_tiles + ticket;
+                    __syncthreads();
                 }
             }
         }

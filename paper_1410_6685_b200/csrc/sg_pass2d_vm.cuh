@@ -80,6 +80,14 @@ __global__ void __launch_bounds__(BLOCK, 2) pass2d_bytecode(const __grid_constan
             for (int k = 0; k < g.shape.n_in; ++k) {
                 const SgIn in = g.in[k];
                 if (in.kind == IN_SCALAR || in.kind == IN_IMM) continue;
+                if (in.kind == IN_BOOLVEC) {        // a stored BOOL matrix: one byte per element, into a predicate register
+                    unsigned int bits = 0;
+#pragma unroll
+                    for (int e = 0; e < E; ++e)
+                        if (e < nval) bits |= (unsigned int)(reinterpret_cast<const volatile uint8_t*>(a.in_ptr[k])[r * a.in_stride[k] + c + e] != 0) << e;
+                    pf = pput<E>(pf, in.reg, bits);
+                    continue;
+                }
                 T x[E];
 #pragma unroll
                 for (int e = 0; e < E; ++e) {

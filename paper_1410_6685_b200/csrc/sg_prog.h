@@ -103,6 +103,8 @@ struct SgArgs {
     unsigned int* ctrl;             // zeroed control words: [0] ticket, [1] decided mask, [2] dynamic tile counter, [3] overflow
     int64_t head;                   // leading elements handled by the ragged path so that the body is 16-byte aligned
     int64_t n_full_tiles;           // full tiles of the aligned body
+    int64_t static_tiles;           // 1-D template passes: tiles [0, static_tiles) are taken strided (block + it * grid); the tiles after them are
+                                    // handed out by tickets on ctrl[2] (passes with reductions only; = n_full_tiles: no tickets), see sg_kernels.cu
     int32_t vec_ok;                 // bit i: input i may use 128-bit loads; bit (16+o): output o may use 128-bit stores
     int32_t no_early_exit;
     uint32_t exit_any;              // quantifier outputs that are registered for_all contracts: one violation ends the pass

@@ -61,7 +61,7 @@ def _chains():
     yield "sorted_f64", 0, lambda c: _sorted_only(c, f64)
     yield "cfg4", 0, lambda c: W.cfg4(c, 4096, None, 0)
     yield "cfg4_gestep", 0, lambda c: _ge_step(c, 0)                                        # Listing 5 loop body
-    # matrix-vector products, PAPER.md:217 (matrix passes have no bytecode evaluator: they need an instance)
+    # matrix-vector products, PAPER.md:217 (without an instance they would run on the 2-D bytecode evaluator)
     yield "matvec_right", 0, lambda c: W.right_multiply(c, 4096, 4096, None, None)
     yield "matvec_left", 0, lambda c: W.left_multiply(c, 4096, 4096, None, None)
     # the rest of the vector API

@@ -599,6 +599,33 @@ def test_unregistered_matrix_chain_runs_on_the_bytecode_evaluator(dtype, rows, c
     assert dtype(got_min) == orc.min(want_B.reshape(-1)) and got_any == bool((want_B > 0).any()) and got_cnt == int((want_B > 0).sum())
 
 
+def test_bool_matrix_kept_and_read_back_in_a_later_pass():
+    """A BOOL matrix somebody keeps (a mask) is stored one byte per element and read back by a later matrix pass."""
+    rows, cols = 37, 301
+    A = RNG.standard_normal((rows, cols))
+    B = RNG.standard_normal((rows, cols))
+    with Ctx() as c:
+        tA, tB = dev(A), dev(B)
+        c.keep += [tA, tB]
+        hA = sg.sg_mat_create(c.ctx, sg.SG_F64, rows, cols, cols, tA.data_ptr())
+        hB = sg.sg_mat_create(c.ctx, sg.SG_F64, rows, cols, cols, tB.data_ptr())
+        mask = sg.sg_enqueue(c.ctx, sg.SG_GT, [hA, sg.F(0.0)])          # kept: materialised as bytes
+        sg.sg_flush(c.ctx)
+        got_mask = c.read_vec(mask, np.uint8, rows * cols).reshape(rows, cols)
+        other = sg.sg_enqueue(c.ctx, sg.SG_LT, [hB, sg.F(0.5)])
+        both = sg.sg_enqueue(c.ctx, sg.SG_AND, [mask, other])
+        sg.sg_release(c.ctx, other)
+        per_row = sg.sg_reduce(c.ctx, both, sg.SG_COUNT, sg.SG_AXIS_ROWS)
+        total = sg.sg_reduce(c.ctx, both, sg.SG_COUNT)
+        sg.sg_release(c.ctx, both)
+        got_total = c.get(total)
+        got_rows = c.read_vec(per_row, np.int64, rows)
+    want_mask = np.stack([orc.cmp_scalar("gt", A[r], 0.0) for r in range(rows)])
+    want_both = np.stack([orc.logic("and", want_mask[r], orc.cmp_scalar("lt", B[r], 0.5)) for r in range(rows)])
+    assert bits_equal(got_mask, want_mask)
+    assert got_rows.tolist() == [orc.count(want_both[r]) for r in range(rows)] and got_total == orc.count(want_both.reshape(-1))
+
+
 @pytest.mark.parametrize("k", [0, 8191])
 def test_cfg4_full_size(k):
     """BASELINE.json:configs[4] at its full size, in bench.py's launch configuration: EVERY element of M', all n-k-1 row maxima
