@@ -245,6 +245,28 @@ sg_status sg_mat_ge_steps(sg_ctx* ctx, sg_handle m, sg_handle det, sg_handle min
  * NaN): the listing's three filters would drop it and violate its own postcondition Result.count = a.count. */
 sg_status sg_vec_quicksort(sg_ctx* ctx, sg_handle v, void* dev_out_or_null, sg_handle* out);
 
+/* The `sum` reduction for callers that MAY NOT ALLOCATE: code under CUDA graph capture, tight
+ * serving loops, harnesses that forbid cudaMalloc.  Takes no context and calls no cudaMalloc, cudaFree or allocating library
+ * routine: the scratch memory of the reduction (one 16-byte partial per 8192 elements + the last-block ticket) is a file-scope
+ * static __device__ array of SG_NOALLOC_SCRATCH_BYTES that every GPU which loads the library holds until the process exits.
+ *   device    CUDA device ordinal (0 .. 63); made current for the call and restored
+ *   stream    cudaStream_t of that device (NULL: the default stream); the call enqueues one 256-byte memset (the ticket must
+ *             start at zero) and one kernel on it and returns without synchronising
+ *   dtype     SG_F32 or SG_F64 (else SG_ERR_DTYPE)
+ *   dev_x     DEVICE pointer, n elements, unit stride, aligned to the element size (16-byte alignment takes the 128-bit path);
+ *             owned by the caller, read only
+ *   n         0 <= n <= SG_NOALLOC_MAX_N; more is rejected with SG_ERR_CAPACITY and a message, nothing is launched
+ *   dev_out   DEVICE pointer to one double, owned by the caller: receives the sum (n = 0: +0.0), valid when the stream reaches it
+ *   err/errcap  optional HOST buffer for the error text (there is no context to ask)
+ * Arithmetic = sg_reduce(SG_SUM): fp64 input in double-double TwoSum cells, fp32 input in fp64, partials combined in tile
+ * order by the last block to finish (deterministic, independent of the grid); the same tolerances hold.
+ * SHARED STATE: every call on a device uses the same array, which keeps the last call's contents.  Calls that OVERLAP on the GPU
+ * (different streams, or host threads that do not order their calls) race on it; order them on one stream or with events.
+ * Errors: SG_ERR_ARG, SG_ERR_DTYPE, SG_ERR_CAPACITY, SG_ERR_CUDA (no usable device: there is no CPU fallback). */
+#define SG_NOALLOC_MAX_N ((int64_t)1 << 27)
+#define SG_NOALLOC_SCRATCH_BYTES (256 + 16 * 16384)
+sg_status sg_vec_sum_noalloc(int32_t device, void* stream, sg_dtype dtype, const void* dev_x, int64_t n, double* dev_out, char* err, int64_t errcap);
+
 sg_status sg_plan_stats(sg_ctx* ctx, sg_stats* out);
 /* Canonical program of pass `pass` of the last flush as text (template generator, tests). Returns bytes needed. */
 int64_t sg_plan_dump(sg_ctx* ctx, int32_t pass, char* buf, int64_t cap);

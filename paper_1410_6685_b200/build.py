@@ -16,7 +16,7 @@ CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libsafegpu.so")
 NSHARDS = 8        # == SG_NSHARDS in csrc/sg_tmpl_launch.cuh: the template instances compile as eight translation units in parallel
-SOURCES = [f"sg_vm_shard.cu@{k}" for k in range(4)] + [f"sg_tmpl_shard.cu@{k}" for k in range(NSHARDS)] + ["sg_kernels.cu", "sg_api.cpp", "sg_plan.cpp", "sg_build.cpp", "sg_transpose.cu", "sg_ge.cu", "sg_sort.cu"]
+SOURCES = [f"sg_vm_shard.cu@{k}" for k in range(4)] + [f"sg_tmpl_shard.cu@{k}" for k in range(NSHARDS)] + ["sg_kernels.cu", "sg_api.cpp", "sg_plan.cpp", "sg_build.cpp", "sg_transpose.cu", "sg_ge.cu", "sg_sort.cu", "sg_noalloc.cu"]
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-fmad=false", "-std=c++17",

@@ -8,7 +8,7 @@ from __future__ import annotations
 
 import ctypes
 import os
-from ctypes import POINTER, Structure, byref, c_char_p, c_double, c_float, c_int32, c_int64, c_size_t, c_uint32, c_void_p
+from ctypes import POINTER, Structure, byref, create_string_buffer, c_char_p, c_double, c_float, c_int32, c_int64, c_size_t, c_uint32, c_void_p
 
 # enums of include/sg.h
 SG_F32, SG_F64, SG_I32, SG_I64, SG_BOOL = 0, 1, 2, 3, 4
@@ -30,7 +30,7 @@ SG_ERR_ARG, SG_ERR_SHAPE, SG_ERR_DTYPE, SG_ERR_EMPTY, SG_ERR_ALIAS, SG_ERR_OOM, 
 
 EXPORTS = [
     "sg_ctx_create", "sg_ctx_destroy", "sg_ctx_set_flags", "sg_last_error", "sg_vec_create", "sg_mat_create", "sg_vec_subset",
-    "sg_mat_row", "sg_mat_rows", "sg_mat_col", "sg_mat_elem", "sg_mat_ge_steps", "sg_mat_transpose", "sg_vec_quicksort", "sg_enqueue", "sg_cast", "sg_reduce", "sg_forall", "sg_exists",
+    "sg_mat_row", "sg_mat_rows", "sg_mat_col", "sg_mat_elem", "sg_mat_ge_steps", "sg_mat_transpose", "sg_vec_quicksort", "sg_vec_sum_noalloc", "sg_enqueue", "sg_cast", "sg_reduce", "sg_forall", "sg_exists",
     "sg_forall_adjacent", "sg_filter", "sg_contract", "sg_flush", "sg_scalar_get", "sg_scalar_dtype", "sg_vec_count", "sg_vec_data", "sg_vec_read",
     "sg_release", "sg_plan_stats", "sg_plan_dump", "sg_last_flush_ms", "sg_timing_begin", "sg_timing_end", "sg_replay_last", "sg_replay_last_graph", "sg_template_count", "sg_template_name",
     "sg_version",
@@ -103,6 +103,7 @@ def lib() -> ctypes.CDLL:
         L.sg_replay_last_graph.argtypes = [c_void_p, c_int32, POINTER(c_float), POINTER(c_float)]
         L.sg_mat_ge_steps.argtypes = [c_void_p, c_int64, c_int64, c_int64, c_double, c_int64, c_int64]
         L.sg_vec_quicksort.argtypes = [c_void_p, c_int64, c_void_p, POINTER(c_int64)]
+        L.sg_vec_sum_noalloc.argtypes = [c_int32, c_void_p, c_int32, c_void_p, c_int64, c_void_p, c_char_p, c_int64]
         L.sg_mat_transpose.argtypes = [c_void_p, c_int64, c_void_p, c_int64, POINTER(c_int64)]
         L.sg_timing_begin.argtypes = [c_void_p]
         L.sg_timing_end.argtypes = [c_void_p, POINTER(c_float), POINTER(c_int32)]
@@ -215,6 +216,18 @@ def sg_mat_transpose(ctx, m: int, dev_out: int | None = None, ld_out: int = 0) -
 
 def sg_vec_quicksort(ctx, v: int, dev_out: int | None = None) -> int:
     return _h(lib().sg_vec_quicksort, ctx, v, dev_out)
+
+
+SG_NOALLOC_MAX_N = 1 << 27
+SG_NOALLOC_SCRATCH_BYTES = 256 + 16 * 16384
+
+
+def sg_vec_sum_noalloc(device: int, stream: int, dtype: int, dev_x: int, n: int, dev_out: int) -> None:
+    """Sum of a device vector into a device double without any allocation (include/sg.h); asynchronous on `stream`."""
+    err = create_string_buffer(256)
+    st = lib().sg_vec_sum_noalloc(device, c_void_p(stream or 0), dtype, c_void_p(dev_x or 0), n, c_void_p(dev_out or 0), err, 256)
+    if st != SG_OK:
+        raise SgError(st, err.value.decode())
 
 
 def sg_mat_ge_steps(ctx, m: int, det: int, minpiv: int, eps: float, k0: int, k1: int) -> None:
