@@ -389,6 +389,13 @@ def inplace_section(torch, sg, W, inputs, measure):
     def outofplace(ctx):
         h, d = sg.sg_vec_create(ctx, sg.SG_F64, n, x.data_ptr()), sg.sg_vec_create(ctx, sg.SG_F64, n, o.data_ptr())
         return sg.sg_enqueue(ctx, sg.SG_MUL, [h, sg.F(2.0)], dst_or_0=d)
+    # read-only counterpart whose reductions are exact in any order: the last part of the tiles goes through tickets (sg_kernels.cu)
+    xi = x.view(torch.int64)
+
+    def int_reductions(ctx):
+        h = sg.sg_vec_create(ctx, sg.SG_I64, n, xi.data_ptr())
+        return [sg.sg_reduce(ctx, h, k) for k in (sg.SG_SUM, sg.SG_RMAX, sg.SG_RMIN)]
+    measure("read_ceiling_sum_max_min_int64_2^27 (1R, exact reductions: tile tickets)", int_reductions, 8 * n)
     measure("rmw_ceiling_scale_in_place_fp64_2^27 (1R+1W, same buffer)", inplace, 16 * n)
     measure("rmw_ceiling_scale_to_second_buffer_fp64_2^27 (1R+1W, two buffers)", outofplace, 16 * n)
 
@@ -492,6 +499,10 @@ def cfg4_section(torch, sg, W, inputs, measure):
         rows = n4 - k - 1
         alg = 16 * rows * n4 + 8 * n4 + 16 * rows + 8 * rows + 8 * n4
         measure(f"cfg4_fp64_16384^2_row_update_k={k}", lambda ctx: W.cfg4(ctx, n4, M.data_ptr(), k), alg, restore=lambda: M.copy_(M0))
+    # Listing 5's row update alone (no row maxima / column sums): a store-only matrix pass, one tile per block
+    rows = n4 - 1
+    measure("ge_row_update_store_only_fp64_16384^2_k=0 (Listing 5's update of all rows j > k, without config 4's reductions)",
+            lambda ctx: W.ge_row_update(ctx, n4, M.data_ptr(), 0), 16 * rows * n4 + 8 * n4 + 16 * rows + 8 * rows, restore=lambda: M.copy_(M0))
 
 
 def main():

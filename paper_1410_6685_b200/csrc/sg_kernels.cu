@@ -148,8 +148,28 @@ int sgk_plan(const SgProg& prog, SgArgs& a, int force_bytecode, int sm_count, in
         const int occ = (has_device && tid) ? g_entries[tid].occupancy() : 2;
         const int SW = tid ? g_entries[tid].tile : BLOCK * 2 * V;
         a.n_strips = (int)((a.cols + SW - 1) / SW);
-        static const long mult2d = env_long("SG_GRID_MULT_2D", 1);
+        static const long mult2d = env_long("SG_GRID_MULT_2D", 1), tile2d = env_long("SG_2D_TILE", 1), tile_rows = env_long("SG_2D_TILE_ROWS", 2);
         const long target = (long)sm_count * occ * mult2d;
+        bool any_reduction = false, any_bool_store = false;
+        for (int o = 0; o < prog.shape.n_out; ++o) {
+            any_reduction |= out_is_reduction(prog.out[o].kind);
+            any_bool_store |= prog.out[o].kind == OUT_STORE_BOOL;
+        }
+        const long rpb = std::max<long>(1, tile_rows);
+        if (tid && ok && !any_reduction && !any_bool_store && tile2d && a.n > 0 && a.n_strips > 0 && (a.n_strips * ((a.n + rpb - 1) / rpb)) < 0x7fffffffl) {
+            // store-only pass on aligned rows: short-lived blocks, one tile of tile_rows x SW per block in row-major order (sg_pass2d_tile.cuh)
+            a.rows_per_chunk = rpb;
+            a.n_chunks = 0;
+            geom->template_id = tid;
+            geom->grid = (int)(a.n_strips * ((a.n + rpb - 1) / rpb));
+            geom->tile = SW;
+            geom->ws_bytes = 0;
+            geom->ctrl_words = 0;
+            for (int o = 0; o < prog.shape.n_out; ++o) a.ws_off[o] = 0;
+            a.vec_ok = (vec_ok & ~(3 << 28)) | (1 << 28);
+            a.head = 0; a.n_full_tiles = 0;
+            return 0;
+        }
         long max_chunks = std::max<long>(1, (a.n + RB - 1) / RB);
         long n_chunks = std::min<long>(max_chunks, std::max<long>(1, target / std::max(1, a.n_strips)));
         long rpc = (a.n + n_chunks - 1) / n_chunks;
@@ -169,7 +189,7 @@ int sgk_plan(const SgProg& prog, SgArgs& a, int force_bytecode, int sm_count, in
         }
         geom->ws_bytes = off;
         geom->ctrl_words = a.n_strips + (int)n_chunks;
-        a.vec_ok = (vec_ok & ~(1 << 29)) | unaligned_rows;
+        a.vec_ok = (vec_ok & ~(3 << 28)) | unaligned_rows;
         a.head = 0; a.n_full_tiles = 0;
         return 0;
     }
@@ -222,11 +242,15 @@ int sgk_plan(const SgProg& prog, SgArgs& a, int force_bytecode, int sm_count, in
         //   * a pass that only stores (no epilogue) runs as many short-lived blocks of K_STORE strided tiles, the hardware block
         //     scheduler balances them:      x := x * a, 2^27 fp64: 0.360 -> 0.313 ms (0.92 -> 1.06 of the measured copy peak);
         //     K = 1 / 2 / 3 / 4 / 8: 0.310 / 0.313 / 0.315 / 0.316 / 0.322 ms in place, 0.354 / 0.312 / 0.313 / 0.315 / 0.320 to a second buffer;
-        //   * a pass with reductions keeps the persistent grid (one epilogue per block: 4096 blocks cost +9 %, 131072 blocks 3x)
-        //     but takes only the first PCT % of its share strided, the rest through tile tickets (sg_pass1d_tmpl.cuh):
-        //     read-only, PCT = 100 / 92 / 85 / 75 / 60: config 1 at 2^28 0.338 / 0.327 / 0.324 / 0.325 / 0.327 ms, sum(x) 0.161 / 0.155 /
-        //     0.160 / 0.169 / 0.174 ms; with stores (divide + contracts, 2^26), PCT = 100 / 50 / 30 / 0: 0.258 / 0.249 / 0.250 / 0.250 ms;
-        //   * early-exit passes stay static (their exit is taken per thread, the ticket loop needs a block-uniform one).
+        //   * a pass with reductions keeps the persistent grid (one epilogue per block: 4096 blocks cost +9 %, 131072 blocks 3x).
+        //     Taking only the first PCT % of its share strided and the rest through tile tickets (sg_pass1d_tmpl.cuh) evens the
+        //     blocks out — read-only, PCT = 100 / 92 / 85 / 75 / 60: config 1 at 2^28 0.338 / 0.327 / 0.324 / 0.325 / 0.327 ms; with
+        //     stores (divide + contracts, 2^26), PCT = 100 / 50 / 30 / 0: 0.258 / 0.249 / 0.250 / 0.250 ms — but which block adds which
+        //     tile then differs from run to run, and a FLOATING-POINT SUM accumulated that way is no longer the same bits on every
+        //     run.  Making it order-independent (one partial cell per ticket, added in ticket order by the epilogue) costs what the
+        //     tickets gain: a cell per tile 0.365 ms, a cell per 4 tiles 0.340 - 0.342 ms against 0.345 ms static (config 1 at 2^28),
+        //     sum(x) 0.159 - 0.163 against 0.157 ms.  So tickets are used only where every reduction of the pass is exact in any order
+        //     (integer sums, max/min, counts, quantifiers); passes with a floating-point sum keep the static shares;
         // The environment variables override the defaults for such sweeps; they are read once.
         bool has_red = false, has_store = false;
         for (int o = 0; o < prog.shape.n_out; ++o) {
@@ -243,7 +267,10 @@ int sgk_plan(const SgProg& prog, SgArgs& a, int force_bytecode, int sm_count, in
         const long pct = has_store ? pct_rw : pct_ro;
         const long per_block = a.n_full_tiles / geom->grid;
         a.static_tiles = a.n_full_tiles;
-        if (tid && has_red && !ee && pct >= 0 && pct < 100 && per_block >= dyn_min) a.static_tiles = per_block * pct / 100 * geom->grid;
+        const bool is_float = prog.shape.dtype == DT_F32 || prog.shape.dtype == DT_F64;
+        bool float_sum = false;
+        for (int o = 0; o < prog.shape.n_out; ++o) float_sum |= is_float && prog.out[o].kind == OUT_SUM;
+        if (tid && has_red && !ee && !float_sum && pct >= 0 && pct < 100 && per_block >= dyn_min) a.static_tiles = per_block * pct / 100 * geom->grid;
     }
     geom->ws_bytes = (size_t)geom->grid * SG_MAX_OUT * sizeof(Cell);
     return 0;

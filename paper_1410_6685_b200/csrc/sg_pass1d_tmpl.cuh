@@ -290,7 +290,10 @@ __global__ void __launch_bounds__(BLOCK, P::min_blocks) pass1d_template(const __
         // behind the tile's own loads.  Equal static shares finish at different times on this part (read-only stream over 592
         // blocks: the median block is done 10 us before the last of 156 us; a 1R+1W stream: 100 us of 372 us, SM pairs differ 2x in
         // write throughput), tickets over the last part of the body let every block finish together (profiles/r02_grid_shape.md).
-        // Only passes with reductions and no early exit take this path (the epilogue resets the counter).
+        // Which block gets which of these tiles differs from run to run, so the host enables tickets only for passes whose
+        // reductions are exact in any order (integer sums, max/min, counts, quantifiers) and that have no early exit; a pass with a
+        // floating-point sum keeps the static order and returns the same bits on every run (sg_kernels.cu has the measurements of
+        // both, and of per-ticket partial cells that would make the sums order-independent: they cost what the tickets gain).
         if constexpr (!M::early_exit && M::has_reduction) {
             if (a.static_tiles < a.n_full_tiles) {
                 __shared__ long long s_tile[2];

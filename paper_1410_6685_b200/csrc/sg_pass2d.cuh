@@ -450,4 +450,6 @@ __global__ void __launch_bounds__(BLOCK, P::min_blocks) pass2d_template(const __
 }
 
 }  // namespace sgk
+
+#include "sg_pass2d_tile.cuh"
 #endif  // SG_PASS2D_CUH_

@@ -94,6 +94,9 @@ inline cudaError_t sgk_launch_pdl(void (*kernel)(KArgs...), int grid, int block,
 
 template <class P> cudaError_t launch_template(const SgArgs& a, int grid, cudaStream_t s) {
     if constexpr ((P::prog.shape.flags & PF_2D) != 0) {
+        if constexpr (!Meta2D<P>::has_reduction) {
+            if ((a.vec_ok >> 28) & 1) return sgk_launch_pdl(pass2d_tile_template<P>, grid, BLOCK, 0, s, a);     // bit 28 (sgk_plan): one tile per block
+        }
         static bool attr_set[SG_MAX_DEVICES] = {};
         bool& set = attr_set[current_device_slot()];
         if (!set) { cudaFuncSetAttribute(pass2d_template<P>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_of<P>()); set = true; }

@@ -26,6 +26,8 @@ TUNE = {
     "cfg1": (2, 4, 4),
     "cfg3": (4, 4, 4),
     "cfg3sum": (4, 4, 4),
+    "red": (4, 4, 4),
+    "extrema": (4, 4, 4),
     "sorted_f32": (4, 4, 4),
     "cfg4": (2, 2, 4),
     "matvec": (2, 2, 4, 3),   # measured: (2, 4, 2, 3) is slower (0.430 / 0.379 ms vs 0.376 / 0.343 ms right / left at 16384^2)
@@ -69,6 +71,12 @@ def _chains():
     yield "isqrt_i64", 0, lambda c: W.project_sqrt(c, sg.SG_I64, N, None, pout=0x7000000)
     yield "cast_i32_f32", 0, lambda c: sg.sg_cast(c, sg.sg_vec_create(c, i32, N, None), f32, sg.sg_vec_create(c, f32, N, 0x7000000))
     yield "cast_f64_i32", 0, lambda c: sg.sg_cast(c, sg.sg_vec_create(c, f64, N, None), i32, sg.sg_vec_create(c, i32, N, 0x7000000))
+    # the terminal reductions of a stored vector in one pass: integer sum + extrema, float extrema — exact in any
+    # order, so these passes take the last part of their tiles through tickets (sg_kernels.cu)
+    yield "red_i32", 0, lambda c: _reduce_all(c, i32, (sg.SG_SUM, sg.SG_RMAX, sg.SG_RMIN))
+    yield "red_i64", 0, lambda c: _reduce_all(c, sg.SG_I64, (sg.SG_SUM, sg.SG_RMAX, sg.SG_RMIN))
+    yield "extrema_f32", 0, lambda c: _reduce_all(c, f32, (sg.SG_RMAX, sg.SG_RMIN))
+    yield "extrema_f64", 0, lambda c: _reduce_all(c, f64, (sg.SG_RMAX, sg.SG_RMIN))
     for tag, dt in (("f32", f32), ("f64", f64)):
         yield f"sqrt_{tag}", 0, lambda c, dt=dt: W.project_sqrt(c, dt, N, None, pout=0x7000000)
         yield f"avg_{tag}", 0, lambda c, dt=dt: W.avg(c, dt, N, None)
@@ -83,6 +91,11 @@ def _axpy_inplace(c, dt):
     ax = sg.sg_enqueue(c, sg.SG_MUL, [x, sg.F(2.0)])
     sg.sg_enqueue(c, sg.SG_ADD, [ax, y], dst_or_0=y)
     sg.sg_release(c, ax)
+
+
+def _reduce_all(c, dt, kinds):
+    x = sg.sg_vec_create(c, dt, N, None)
+    return [sg.sg_reduce(c, x, k) for k in kinds]
 
 
 def _scale_inplace(c, dt):

@@ -192,6 +192,27 @@ def cfg4(ctx, n, pM, k, ld=None):
     return res
 
 
+def ge_row_update(ctx, n, pM, k, ld=None):
+    """Listing 5's row update alone: M[j,:] -= (M[j,k]/M[k,k]) * M[k,:] for all rows j > k in ONE matrix pass that
+    only stores (config 4 without its two reductions).  Pass 1: the factors, read before the rows change; pass 2: the update."""
+    ld = n if ld is None else ld
+    M = sg.sg_mat_create(ctx, sg.SG_F64, n, n, ld, pM)
+    res = {"M": M}
+    if k + 1 >= n:
+        return res
+    piv = sg.sg_mat_elem(ctx, M, k, k)
+    col = sg.sg_mat_col(ctx, M, k, k + 1, n)
+    f = sg.sg_enqueue(ctx, sg.SG_DIV, [col, piv])
+    rowk = sg.sg_mat_row(ctx, M, k)
+    sub = sg.sg_mat_rows(ctx, M, k + 1, n)
+    t = sg.sg_enqueue(ctx, sg.SG_MUL, [H(f, sg.SG_BCAST_COL), H(rowk, sg.SG_BCAST_ROW)])
+    sg.sg_enqueue(ctx, sg.SG_SUB, [sub, t], dst_or_0=sub)
+    for h in (col, t, piv, f, rowk):
+        sg.sg_release(ctx, h)
+    res["sub"] = sub
+    return res
+
+
 def ge_step(ctx, M, n, k, det, minpiv):
     """One step of Listing 5 enqueued without a trigger: Result := Result * pivot and the
     smallest |pivot| so far on a one-element domain, then, for all rows j > k in ONE matrix pass, the row update of

@@ -306,6 +306,49 @@ def test_cfg1_full_size():
     assert sum_ok(gs, want["sum"], want["w"], 1e-5) and np.float32(gmx) == want["max"]
 
 
+@pytest.mark.parametrize("dtype", [np.float32, np.float64])
+def test_float_sums_are_the_same_bits_on_every_run(dtype):
+    """A pass with a floating-point sum keeps the static tile order (tile tickets, under which the block that adds a tile differs from
+    run to run, are used only where every reduction is exact in any order): 30 runs at a size that would take tickets, one bit
+    pattern."""
+    n = (1 << 25) + 4099
+    x, y = inputs.normal_f32(3, 0, n).astype(dtype), inputs.normal_f32(3, 1, n).astype(dtype)
+    seen = set()
+    with Ctx() as c:
+        hx, hy = c.vec(x), c.vec(y)
+        for _ in range(30):
+            prod = sg.sg_enqueue(c.ctx, sg.SG_MUL, [hx, hy])
+            s = sg.sg_reduce(c.ctx, prod, sg.SG_SUM)
+            sg.sg_release(c.ctx, prod)
+            seen.add(np.float64(c.get(s)).tobytes())
+            sg.sg_release(c.ctx, s)
+        assert sg.sg_plan_stats(c.ctx).n_template == 1
+    assert len(seen) == 1
+    got = np.frombuffer(seen.pop(), dtype=np.float64)[0]
+    assert sum_ok(got, ocfg.dot_product(x, y), orc.zip("mul", x, y), 1e-12 if dtype is np.float64 else 1e-5)
+
+
+@pytest.mark.parametrize("dtype", [np.int32, np.int64, np.float32])
+def test_exact_reductions_through_tile_tickets(dtype):
+    """Integer sum / max / min (float: max / min only) of a vector long enough that the last part of the tiles is handed out through
+    tickets (sg_pass1d_tmpl.cuh): bit-exact against the oracle, on every one of 10 runs; the tail is ragged."""
+    n = (1 << 25) + 4099
+    a = rand(dtype, n)
+    is_int = np.dtype(dtype).kind == "i"
+    want = ((orc.sum(a),) if is_int else ()) + (orc.max(a), orc.min(a))
+    with Ctx() as c:
+        ha = c.vec(a)
+        for _ in range(10):
+            hs = [sg.sg_reduce(c.ctx, ha, k) for k in ((sg.SG_SUM,) if is_int else ()) + (sg.SG_RMAX, sg.SG_RMIN)]
+            got = tuple(c.get(h) for h in hs)
+            assert sg.sg_plan_stats(c.ctx).n_passes == 1
+            for h in hs:
+                sg.sg_release(c.ctx, h)
+            assert bits_equal(np.array(got[-2:], dtype=dtype), np.array(want[-2:], dtype=dtype))
+            if is_int:
+                assert got[0] == want[0]
+
+
 def test_cfg1_headline_size():
     """The configuration bench.py's headline line times (BASELINE.json metric: the fused chain at 2^28 elements): sum and max against
     the oracle on ALL 2^28 elements, then every element of w (the same chain with w kept)."""
@@ -624,6 +667,39 @@ def test_bool_matrix_kept_and_read_back_in_a_later_pass():
     want_both = np.stack([orc.logic("and", want_mask[r], orc.cmp_scalar("lt", B[r], 0.5)) for r in range(rows)])
     assert bits_equal(got_mask, want_mask)
     assert got_rows.tolist() == [orc.count(want_both[r]) for r in range(rows)] and got_total == orc.count(want_both.reshape(-1))
+
+
+# the store-only row update (Listing 5 without config 4's reductions): aligned shapes run as one tile per block (sg_pass2d_tile.cuh),
+# odd shapes through the staged kernel's guarded form; strips with a ragged right edge, one row, views with a leading dimension
+@pytest.mark.parametrize("n,k,ld", [(2, 0, 2), (4, 1, 4), (34, 0, 34), (258, 100, 258), (1024, 0, 1024), (1030, 7, 1030), (2050, 2048, 2050), (2048, 5, 2048),
+                                    (3100, 1, 3104), (1538, 0, 1540), (33, 5, 37), (1031, 7, 1031), (515, 3, 521)])
+def test_ge_row_update_store_only(n, k, ld):
+    M = inputs.boosted_matrix_f64(5, 0, n)
+    want = ocfg.cfg4(M, k)["M"]
+    with Ctx() as c:
+        buf = np.full((n, ld), 7.25)
+        buf[:, :n] = M
+        t = c.torch.from_numpy(buf).cuda()
+        W.ge_row_update(c.ctx, n, t.data_ptr(), k, ld=ld)
+        sg.sg_flush(c.ctx)
+        st = sg.sg_plan_stats(c.ctx)
+        assert st.n_passes == 2 and st.n_template == 2
+        c.torch.cuda.synchronize()
+        full = t.cpu().numpy()
+        assert bits_equal(np.ascontiguousarray(full[:, :n]), want)
+        assert (full[:, n:] == 7.25).all()                              # the padding between rows is never written
+
+
+def test_ge_row_update_full_size():
+    n, k = 16384, 0
+    M = inputs.boosted_matrix_f64(5, 0, n)
+    want_M = orc.mat_step(M, k)[0]
+    with Ctx() as c:
+        t = c.torch.from_numpy(M).cuda()
+        W.ge_row_update(c.ctx, n, t.data_ptr(), k)
+        sg.sg_flush(c.ctx)
+        got = t.cpu().numpy()
+    assert bits_equal(got, want_M)
 
 
 @pytest.mark.parametrize("k", [0, 8191])
