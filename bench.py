@@ -217,6 +217,27 @@ def cfg0_section(torch, sg, W, inputs, measure):
     a, b, c = (torch.from_numpy(inputs.uniform_pm1_f64(1, s, n0)).cuda() for s in range(3))
     measure("cfg0_fp64_2^20_chain_sum_max_min_contracts (L2-warm, 2 passes)", lambda ctx: W.cfg0(ctx, n0, a.data_ptr(), b.data_ptr(), c.data_ptr()), 64 << 20, 200, graph=True)
     measure("cfg0_onepass (z released, L2-warm)", lambda ctx: W.cfg0(ctx, n0, a.data_ptr(), b.data_ptr(), c.data_ptr(), keep_z=False), 24 << 20, 200, graph=True)
+    # what a caller sees: enqueue + plan + two launches + the scalars in host memory (wall clock per step, median of 300; the reductions'
+    # last blocks write their results to the pinned mirror themselves — SAFEGPU_DIRECT_SCALARS=0 routes them through a copy after the
+    # last pass instead: 1 us less kernel time per pass, 10 us more per step)
+    import time
+    ctx = sg.sg_ctx_create(0, torch.cuda.current_stream().cuda_stream)
+    try:
+        wall = []
+        for i in range(350):
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            r = W.cfg0(ctx, n0, a.data_ptr(), b.data_ptr(), c.data_ptr())
+            sg.sg_scalar_get(ctx, r["sum"])
+            if i >= 50:
+                wall.append((time.perf_counter() - t0) * 1e3)
+            for h in r.values():
+                sg.sg_release(ctx, h)
+        measure.out["cfg0_step_wall (enqueue + plan + 2 launches + scalars read on the host; host clock, median of 300)"] = {
+            "ms": float(np.median(wall)), "p10_ms": float(np.percentile(wall, 10)), "algorithmic_bytes": 64 << 20, "GB/s": (64 << 20) / float(np.median(wall)) / 1e6,
+            "frac_of_peak": (64 << 20) / float(np.median(wall)) / 1e6 / measure.peak, "passes": 2, "template_passes": 2}
+    finally:
+        sg.sg_ctx_destroy(ctx)
     # the floor of ANY pass: a one-element pass (nothing to stream) — launch latency + the kernel's fixed prologue / epilogue
     one = torch.ones(1, dtype=torch.float64, device="cuda")
     one32, out32 = torch.ones(1, dtype=torch.float32, device="cuda"), torch.ones(1, dtype=torch.float32, device="cuda")

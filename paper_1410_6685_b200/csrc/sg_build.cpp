@@ -4,6 +4,7 @@
 // Merged elementwise bodies need no barrier (X[i]+Y[i] becomes a*X[i]+Y[i]; PAPER.md:322:
 // (A[i]/pivot) - A[step]); scalars and immediates simply become extra kernel arguments.
 #include <stdio.h>
+#include <stdlib.h>
 #include <string.h>
 
 #include <algorithm>
@@ -12,6 +13,14 @@
 #include "sg_ctx.h"
 
 namespace {
+
+// where the last block of a reduction pass writes an AXIS_ALL result besides its device slot: the slot's place in the pinned host
+// mirror (SgArgs.out_host).  SAFEGPU_DIRECT_SCALARS=0 turns the write-through off (every scalar then goes back through the copy
+// after the flush's last pass): the A/B switch of the measurement in DESIGN.md.
+void* scalar_host_slot(const sg_ctx* c, int64_t slot) {
+    static const bool direct = [] { const char* e = getenv("SAFEGPU_DIRECT_SCALARS"); return !(e && e[0] == '0'); }();
+    return (!direct || c->plan_only || !c->slab_host || slot < 0) ? nullptr : (void*)(c->slab_host + 8 * slot);
+}
 
 struct Builder {
     sg_ctx* c;
@@ -242,6 +251,7 @@ sg_status sg_build_pass(sg_ctx* c, Pass& P, std::vector<char*>& temps, std::stri
             if (n_out >= SG_MAX_OUT) return sg_fail(c, SG_ERR_CAPACITY, "too many outputs in one pass");
             g.out[n_out] = {X.op, (uint8_t)it->second.first, (uint8_t)it->second.second, AXIS_ALL};
             a.out_ptr[n_out] = c->slab + 8 * V[X.out].slot;
+            a.out_host[n_out] = scalar_host_slot(c, V[X.out].slot);
             a.out_len[n_out] = X.cols;
             only_quant = false;
             ++n_out;
@@ -293,8 +303,10 @@ sg_status sg_build_pass(sg_ctx* c, Pass& P, std::vector<char*>& temps, std::stri
             if (n_out >= SG_MAX_OUT) return sg_fail(c, SG_ERR_CAPACITY, "too many outputs in one pass");
             Value& ov = V[X.out];
             g.out[n_out] = {X.op, (uint8_t)r[0], SG_NO_PRED, (uint8_t)X.axis};
-            if (X.axis == AXIS_ALL) a.out_ptr[n_out] = c->slab + 8 * ov.slot;
-            else {
+            if (X.axis == AXIS_ALL) {
+                a.out_ptr[n_out] = c->slab + 8 * ov.slot;
+                a.out_host[n_out] = scalar_host_slot(c, ov.slot);
+            } else {
                 const int64_t oes = dtype_size(ov.dtype);
                 if (!ov.ptr) {
                     ov.ptr = (char*)sg_dev_alloc(c, (size_t)(ov.cols * oes));

@@ -55,6 +55,13 @@ __device__ __forceinline__ void block_reduce_cells(Cell (&acc)[NOUT], const uint
     __syncthreads();
 }
 
+// the 8-byte result of an AXIS_ALL output: the device slot and, when the context gave one, its place in the pinned host mirror —
+// written from here the hand-back needs no copy-engine transfer between this kernel and the next one of the stream
+__device__ __forceinline__ void store_scalar(const SgArgs& a, int o, unsigned long long r) {
+    *reinterpret_cast<unsigned long long*>(a.out_ptr[o]) = r;
+    if (a.out_host[o] != nullptr) *reinterpret_cast<volatile unsigned long long*>(a.out_host[o]) = r;
+}
+
 template <class T, int NOUT>
 __device__ __forceinline__ void epilogue_1d(Cell (&acc)[NOUT], const uint8_t (&kind)[NOUT], const SgArgs& a, bool need_ticket) {
     __shared__ Cell smem[32 * SG_MAX_OUT];
@@ -67,7 +74,7 @@ __device__ __forceinline__ void epilogue_1d(Cell (&acc)[NOUT], const uint8_t (&k
         if (threadIdx.x == 0) {
 #pragma unroll
             for (int o = 0; o < NOUT; ++o)
-                if (out_is_reduction(kind[o])) *reinterpret_cast<unsigned long long*>(a.out_ptr[o]) = cell_final<T>(kind[o], acc[o]);
+                if (out_is_reduction(kind[o])) store_scalar(a, o, cell_final<T>(kind[o], acc[o]));
             a.ctrl[1] = 0; a.ctrl[2] = 0;
         }
         return;
@@ -101,7 +108,7 @@ __device__ __forceinline__ void epilogue_1d(Cell (&acc)[NOUT], const uint8_t (&k
     if (threadIdx.x == 0) {
 #pragma unroll
         for (int o = 0; o < NOUT; ++o)
-            if (out_is_reduction(kind[o])) *reinterpret_cast<unsigned long long*>(a.out_ptr[o]) = cell_final<T>(kind[o], acc[o]);
+            if (out_is_reduction(kind[o])) store_scalar(a, o, cell_final<T>(kind[o], acc[o]));
         a.ctrl[0] = 0; a.ctrl[1] = 0; a.ctrl[2] = 0;       // the end of the kernel makes these visible to the next launch
     }
 }

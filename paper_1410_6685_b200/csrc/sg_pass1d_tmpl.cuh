@@ -8,6 +8,11 @@
 
 namespace sgk {
 
+__host__ __device__ constexpr bool prog_has_float_sum(const SgProg& g) {
+    for (int o = 0; o < g.shape.n_out; ++o)
+        if (g.out[o].kind == OUT_SUM && (g.shape.dtype == DT_F32 || g.shape.dtype == DT_F64)) return true;
+    return false;
+}
 __host__ __device__ constexpr bool prog_has_reduction(const SgProg& g) {
     for (int o = 0; o < g.shape.n_out; ++o)
         if (out_is_reduction(g.out[o].kind)) return true;
@@ -27,6 +32,7 @@ template <class P> struct Meta1D {
     static constexpr int NOUT = S.n_out > 0 ? S.n_out : 1;
     static constexpr bool early_exit = (S.flags & PF_EARLY_EXIT) != 0;
     static constexpr bool has_reduction = prog_has_reduction(P::prog);
+    static constexpr bool tickets = has_reduction && !early_exit && !prog_has_float_sum(P::prog);      // see the ticket loop of pass1d_template
 };
 
 // ---- compile-time body: one fold over the instruction list, every register index is a constant --------
@@ -294,7 +300,7 @@ __global__ void __launch_bounds__(BLOCK, P::min_blocks) pass1d_template(const __
         // reductions are exact in any order (integer sums, max/min, counts, quantifiers) and that have no early exit; a pass with a
         // floating-point sum keeps the static order and returns the same bits on every run (sg_kernels.cu has the measurements of
         // both, and of per-ticket partial cells that would make the sums order-independent: they cost what the tickets gain).
-        if constexpr (!M::early_exit && M::has_reduction) {
+        if constexpr (M::tickets) {
             if (a.static_tiles < a.n_full_tiles) {
                 __shared__ long long s_tile[2];
                 if (threadIdx.x == 0) s_tile[0] = a.static_tiles + atomicAdd(&a.ctrl[2], 1u);

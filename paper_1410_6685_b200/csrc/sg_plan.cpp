@@ -290,12 +290,19 @@ sg_status flush_body(sg_ctx* c, int* executed, ExitGroups* exit_groups) {
             ++*executed;
         }
         cudaEventRecord(t1, c->stream);
-        // a8: hand the flush's scalars back in one copy
+        // a8: hand the flush's scalars back.  The reductions' last blocks have written their results to the pinned mirror themselves
+        // (SgArgs.out_host); whatever else the flush produced in the slab (filter counts, one-element passes) goes back in one copy
         int64_t lo = c->slab_slots, hi = -1;
+        auto written_by_kernel = [&](int64_t slot) {
+            for (const Pass& P : passes)
+                for (int o = 0; o < P.prog.shape.n_out; ++o)
+                    if (P.args.out_host[o] == (void*)(c->slab_host + 8 * slot)) return true;
+            return false;
+        };
         for (const Node& n : N) {
             if (n.done || !n.needed) continue;
             for (int o : {n.out, n.out2})
-                if (o >= 0 && V[o].kind == VK_SCALAR && V[o].slot >= 0) { lo = std::min(lo, V[o].slot); hi = std::max(hi, V[o].slot); }
+                if (o >= 0 && V[o].kind == VK_SCALAR && V[o].slot >= 0 && !written_by_kernel(V[o].slot)) { lo = std::min(lo, V[o].slot); hi = std::max(hi, V[o].slot); }
         }
         if (hi >= lo) {
             if (cudaMemcpyAsync(c->slab_host + 8 * lo, c->slab + 8 * lo, 8 * (size_t)(hi - lo + 1), cudaMemcpyDeviceToHost, c->stream) != cudaSuccess)

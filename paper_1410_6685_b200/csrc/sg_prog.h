@@ -95,6 +95,8 @@ struct SgArgs {
     uint64_t imm[SG_MAX_IN];        // IN_IMM: raw bits of the immediate in the pass dtype
     SgDiv imm_div[SG_MAX_IN];       // IN_IMM, i32 passes: signed magic number for division/modulo by the immediate (valid == 0 if |d| <= 1), see magic_div_i32
     void* out_ptr[SG_MAX_OUT];      // STORE: buffer; reductions/quantifiers: 8-byte device scalar slot (AXIS_ALL) or vector
+    void* out_host[SG_MAX_OUT];     // AXIS_ALL reductions/quantifiers: the slot's place in the PINNED HOST mirror, written by the last block
+                                    // together with the device slot (no copy engine between two passes of a stream), or null
     int64_t out_len[SG_MAX_OUT];    // valid length of the output's source value (<= n); 2-D STORE: leading dimension
     int64_t out_cap[SG_MAX_OUT];    // FILTER: capacity in elements
     void* out_aux[SG_MAX_OUT];      // FILTER: device int64 slot that receives the kept count
