@@ -13,6 +13,14 @@ __host__ __device__ constexpr bool prog_has_float_sum(const SgProg& g) {
         if (g.out[o].kind == OUT_SUM && (g.shape.dtype == DT_F32 || g.shape.dtype == DT_F64)) return true;
     return false;
 }
+#ifndef SG_WARP_CONTIG
+#define SG_WARP_CONTIG 2      // 0: block-interleaved tile layout, 1: warp-contiguous for passes with a neighbour operand, 2: for every pass
+#endif
+__host__ __device__ constexpr bool prog_has_shift(const SgProg& g) {
+    for (int k = 0; k < g.shape.n_in; ++k)
+        if (g.in[k].kind == IN_SHIFT) return true;
+    return false;
+}
 __host__ __device__ constexpr bool prog_has_reduction(const SgProg& g) {
     for (int o = 0; o < g.shape.n_out; ++o)
         if (out_is_reduction(g.out[o].kind)) return true;
@@ -31,6 +39,17 @@ template <class P> struct Meta1D {
     static constexpr int NP = S.n_preg > 0 ? S.n_preg : 1;
     static constexpr int NOUT = S.n_out > 0 ? S.n_out : 1;
     static constexpr bool early_exit = (S.flags & PF_EARLY_EXIT) != 0;
+    // Tile layout: warp w owns the U consecutive runs of 32 vectors [w*U*32, (w+1)*U*32) of the tile (2 KiB of fp32 at U = 4), access u
+    // of lane l is vector (w*U + u)*32 + l.  Round 1 interleaved the warps (vector k -> thread k % BLOCK, access k / BLOCK).  With a
+    // warp-contiguous layout the element after lane 31's vector is lane 0's vector of the warp's NEXT access — a neighbour operand
+    // (IN_SHIFT) is a shuffle, and one scalar load per warp and tile instead of one per access: config 3's body + contracts in one
+    // pass (sum + for_all + is_sorted, 2^28 fp32) 0.1815 -> 0.1615 ms = the time of the body alone.  It also serves the other passes
+    // better (same-run A/B against the interleaved layout): config 1 at 2^28 0.3434 -> 0.3392 ms, x := 2x to a second buffer
+    // 0.3318 -> 0.3134 ms, sqrt 0.0815 -> 0.0808 ms, int64 sum/max/min 0.1529 -> 0.1543 ms (the one that loses).
+    static constexpr bool warp_contig = SG_WARP_CONTIG == 2 || (SG_WARP_CONTIG == 1 && prog_has_shift(P::prog));
+    __device__ static __forceinline__ int vidx(int u) {
+        return warp_contig ? (((int)(threadIdx.x >> 5) * U + u) * 32 + (int)(threadIdx.x & 31)) : (u * BLOCK + (int)threadIdx.x);
+    }
     static constexpr bool has_reduction = prog_has_reduction(P::prog);
     static constexpr bool tickets = has_reduction && !early_exit && !prog_has_float_sum(P::prog);      // see the ticket loop of pass1d_template
 };
@@ -80,7 +99,7 @@ __device__ __forceinline__ void load_input_full(typename Meta1D<P>::T (&v)[Meta1
         const VEC* src = reinterpret_cast<const VEC*>(reinterpret_cast<const T*>(a.in_ptr[K]) + base);
 #pragma unroll
         for (int u = 0; u < M::U; ++u) {
-            VEC x = in.pad ? ld_stream_rw(src + u * BLOCK + threadIdx.x) : ld_stream(src + u * BLOCK + threadIdx.x);
+            VEC x = in.pad ? ld_stream_rw(src + M::vidx(u)) : ld_stream(src + M::vidx(u));
             const T* xe = reinterpret_cast<const T*>(&x);
 #pragma unroll
             for (int e = 0; e < M::V; ++e) v[in.reg][u * M::V + e] = xe[e];
@@ -92,7 +111,7 @@ __device__ __forceinline__ void load_input_full(typename Meta1D<P>::T (&v)[Meta1
 #pragma unroll
         for (int u = 0; u < M::U; ++u) {
             S x[M::V];
-            ld_stream_bytes<M::V * (int)sizeof(S)>(src + (size_t)(u * BLOCK + threadIdx.x) * M::V, x);
+            ld_stream_bytes<M::V * (int)sizeof(S)>(src + (size_t)M::vidx(u) * M::V, x);
 #pragma unroll
             for (int e = 0; e < M::V; ++e) v[in.reg][u * M::V + e] = cvt_elem<T, S>(x[e]);
         }
@@ -105,7 +124,14 @@ __device__ __forceinline__ void load_input_full(typename Meta1D<P>::T (&v)[Meta1
 #pragma unroll
             for (int e = 0; e + 1 < M::V; ++e) v[in.reg][u * M::V + e] = v[rr][u * M::V + e + 1];
             T nxt = __shfl_down_sync(0xffffffffu, v[rr][u * M::V], 1);
-            if ((threadIdx.x & 31) == 31) nxt = __ldg(src + (size_t)(u * BLOCK + threadIdx.x + 1) * M::V);
+            if constexpr (M::warp_contig) {
+                if (u + 1 < M::U) {
+                    const T first_next = __shfl_sync(0xffffffffu, v[rr][(u + 1 < M::U ? u + 1 : u) * M::V], 0);
+                    if ((threadIdx.x & 31) == 31) nxt = first_next;
+                } else if ((threadIdx.x & 31) == 31) nxt = __ldg(src + (size_t)(M::vidx(u) + 1) * M::V);
+            } else {
+                if ((threadIdx.x & 31) == 31) nxt = __ldg(src + (size_t)(M::vidx(u) + 1) * M::V);
+            }
             v[in.reg][u * M::V + M::V - 1] = nxt;
         }
     } else if constexpr (in.kind == IN_STRIDED) {
@@ -114,13 +140,13 @@ __device__ __forceinline__ void load_input_full(typename Meta1D<P>::T (&v)[Meta1
         for (int u = 0; u < M::U; ++u)
 #pragma unroll
             for (int e = 0; e < M::V; ++e)
-                v[in.reg][u * M::V + e] = __ldg(src + (base + (int64_t)(u * BLOCK + threadIdx.x) * M::V + e) * a.in_stride[K]);
+                v[in.reg][u * M::V + e] = __ldg(src + (base + (int64_t)M::vidx(u) * M::V + e) * a.in_stride[K]);
     } else if constexpr (in.kind == IN_BOOLVEC) {
         const uint8_t* src = reinterpret_cast<const uint8_t*>(a.in_ptr[K]) + base;
 #pragma unroll
         for (int u = 0; u < M::U; ++u)
 #pragma unroll
-            for (int e = 0; e < M::V; ++e) p[in.reg][u * M::V + e] = src[(size_t)(u * BLOCK + threadIdx.x) * M::V + e] != 0;
+            for (int e = 0; e < M::V; ++e) p[in.reg][u * M::V + e] = src[(size_t)M::vidx(u) * M::V + e] != 0;
     }
     // IN_SCALAR / IN_IMM are broadcast once before the tile loop
 }
@@ -163,14 +189,14 @@ __device__ __forceinline__ void emit_output_full(typename Meta1D<P>::T (&v)[Meta
             T* xe = reinterpret_cast<T*>(&x);
 #pragma unroll
             for (int e = 0; e < M::V; ++e) xe[e] = v[out.src][u * M::V + e];
-            st_stream(dst + u * BLOCK + threadIdx.x, x);
+            st_stream(dst + M::vidx(u), x);
         }
     } else if constexpr (out.kind == OUT_STORE_BOOL) {
         uint8_t* dst = reinterpret_cast<uint8_t*>(a.out_ptr[O]) + base;
 #pragma unroll
         for (int u = 0; u < M::U; ++u)
 #pragma unroll
-            for (int e = 0; e < M::V; ++e) dst[(size_t)(u * BLOCK + threadIdx.x) * M::V + e] = p[out.src][u * M::V + e];
+            for (int e = 0; e < M::V; ++e) dst[(size_t)M::vidx(u) * M::V + e] = p[out.src][u * M::V + e];
     } else if constexpr (out_is_pred_reduction(out.kind)) {
 #pragma unroll
         for (int e = 0; e < M::E; ++e) cell_accum_pred(out.kind, acc[O], p[out.src][e]);
@@ -249,9 +275,12 @@ __global__ void __launch_bounds__(BLOCK, P::min_blocks) pass1d_template(const __
         has_reduction |= out_is_reduction(kind[o]);
     }
     unsigned int need_mask = 0, flagged = 0;
+    __shared__ unsigned int s_decided;          // early-exit passes: the decided word as warp 0 last saw it
     if constexpr (M::early_exit) {
 #pragma unroll
         for (int o = 0; o < M::S.n_out; ++o) need_mask |= 1u << o;
+        if (threadIdx.x == 0) s_decided = 0;
+        __syncthreads();
     }
 
     {
@@ -260,22 +289,28 @@ __global__ void __launch_bounds__(BLOCK, P::min_blocks) pass1d_template(const __
         bcast_inputs<P, M::E>(v, a, KS);
         unsigned int it = 0;
         for (int64_t tile = blockIdx.x; tile < a.static_tiles; tile += gridDim.x, ++it) {
-            // every POLL-th tile the decided word is requested together with the tile's loads and examined after the tile is
-            // processed, so the poll costs no extra round trip on the clean path.  Measured on config 3 (2^28 fp32, 740 blocks, 16 KiB
-            // tiles; clean pass / time to answer with the violation at n/64, 20 %, n/2 of the vector, in us):
-            //   POLL 1: 222 / 11.7, 36.7, 92.6     POLL 2: 182 / 14.3, 35.7, 88.3     POLL 4: 180 / 19.7, 40.8, 91.8     POLL 8: 180 / 31.2, 55.3, 105
-            // (a strong load per tile slows the clean stream by 23 %; every second tile costs 1 % and halves the time to answer)
+            // every POLL-th tile the decided word is requested BEHIND the tile's loads and examined after the tile is processed, so the
+            // poll costs no round trip of its own.  ONE warp per block asks and passes what it saw to the block through shared memory;
+            // the other warps read it at their own next poll point (no barrier: a stale value only delays the exit).  Measured on
+            // config 3 (2^28 fp32, 740 blocks, 16 KiB tiles, warp-contiguous layout), clean pass / time to answer for a violation at
+            // n/64, 20 %, n/2 of the vector:
+            //   every warp polls, load in front of the tile's loads, every 2nd / 4th / 8th tile / never:  0.193 / 0.171 / 0.162 / 0.160 ms
+            //   one warp per block, in front of the loads, every 2nd tile:                                0.177 ms / 17, 43, 86 us
+            //   one warp per block, behind the loads, every 2nd / 3rd / 4th / 6th tile:                   0.168 / 0.167 / 0.166 / 0.166 ms,
+            //                                                                  to answer 17, 40, 82 / 21, 41, 86 / 25, 48, 86 / 33, 50, 97 us
+            // (a load in front of the tile's loads holds the warp's tile loads back by one L2 round trip per poll, and that warp then
+            // finishes last; ld.relaxed.gpu and ld.global.cg cost the same)
 #ifndef SG_POLL
 #define SG_POLL 2
 #endif
             constexpr unsigned int POLL = SG_POLL;
             unsigned int decided_word = 0;
             const bool poll = M::early_exit && !a.no_early_exit && (it % POLL) == 0;
-            if constexpr (M::early_exit) {
-                if (poll) decided_word = ld_relaxed_u32(&a.ctrl[1]);
-            }
             const int64_t base = a.head + tile * M::TILE;
             load_inputs_full<P>(v, p, a, base, KS);
+            if constexpr (M::early_exit) {
+                if (poll && threadIdx.x < 32) decided_word = ld_relaxed_u32(&a.ctrl[1]);
+            }
             exec_body<P, T, M::NV, M::NP, M::E>(v, p, a, IS);
             emit_outputs_full<P>(v, p, acc, a, base, OS);
             if constexpr (M::early_exit) {
@@ -288,6 +323,9 @@ __global__ void __launch_bounds__(BLOCK, P::min_blocks) pass1d_template(const __
                             if ((threadIdx.x & 31) == 0) atomicOr(&a.ctrl[1], 1u << o);
                         }
                     }
+                    if (threadIdx.x < 32) {
+                        if (decided_word != 0 && threadIdx.x == 0) *reinterpret_cast<volatile unsigned int*>(&s_decided) = decided_word;
+                    } else decided_word = *reinterpret_cast<volatile unsigned int*>(&s_decided);
                     if ((decided_word & need_mask) == need_mask || (decided_word & a.exit_any) != 0) break;
                 }
             }
