@@ -185,8 +185,9 @@ sg_status sg_filter(sg_ctx* ctx, sg_handle values, sg_handle mask_bool, void* de
  * collections materialised by the same flush (R17). */
 sg_status sg_contract(sg_ctx* ctx, sg_handle h_bool_scalar, int32_t kind, const char* tag);
 
-/* update: plan + launch everything pending, asynchronously on the stream, then copy the
- * flush's scalar results to a pinned host mirror.  Returns SG_ERR_CONTRACT (after a stream sync) only if
+/* update: plan + launch everything pending, asynchronously on the stream.  The flush's scalar results reach a
+ * pinned host mirror without a host synchronisation: a reduction's last block writes its 8-byte results there itself, scalars
+ * produced otherwise (filter counts, one-element passes) follow in one asynchronous copy.  Returns SG_ERR_CONTRACT (after a stream sync) only if
  * contracts are registered.  Transactional: when the plan cannot be built (SG_ERR_UNSUPPORTED, SG_ERR_CAPACITY, SG_ERR_ALIAS,
  * SG_ERR_OOM, ...) nothing has been launched, the error is returned and the pending list is DISCARDED — result handles of the
  * discarded operations name no data (release them), in-place destinations keep their previous contents, and the context is

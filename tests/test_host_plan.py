@@ -64,6 +64,27 @@ def test_no_device_means_failure_not_fallback():
     assert ei.value.status == sg.SG_ERR_CUDA
 
 
+def test_noalloc_sum_checks_its_arguments_before_it_touches_a_device():
+    """sg_vec_sum_noalloc (include/sg.h): size limit, dtype, pointers and the device ordinal are rejected on the host, with a message;
+    without a GPU the call fails with SG_ERR_CUDA — there is no CPU fallback."""
+    import torch
+    for args, status, word in (((0, 0, sg.SG_F32, 16, sg.SG_NOALLOC_MAX_N + 1, 16), sg.SG_ERR_CAPACITY, "SG_NOALLOC_MAX_N"),
+                               ((0, 0, sg.SG_I64, 16, 8, 16), sg.SG_ERR_DTYPE, "SG_F32"),
+                               ((0, 0, sg.SG_F64, 0, 8, 16), sg.SG_ERR_ARG, "null"),
+                               ((0, 0, sg.SG_F64, 16, 8, 0), sg.SG_ERR_ARG, "null"),
+                               ((0, 0, sg.SG_F64, 16, -1, 16), sg.SG_ERR_ARG, "negative"),
+                               ((0, 0, sg.SG_F64, 12, 8, 16), sg.SG_ERR_ARG, "aligned"),
+                               ((99, 0, sg.SG_F64, 16, 8, 16), sg.SG_ERR_ARG, "device")):
+        with pytest.raises(sg.SgError) as ei:
+            sg.sg_vec_sum_noalloc(*args)
+        assert ei.value.status == status and word in str(ei.value), (args, str(ei.value))
+    assert sg.SG_NOALLOC_SCRATCH_BYTES == 256 + 16 * (sg.SG_NOALLOC_MAX_N // 8192)
+    if not torch.cuda.is_available():
+        with pytest.raises(sg.SgError) as ei:
+            sg.sg_vec_sum_noalloc(0, 0, sg.SG_F32, 16, 8, 16)
+        assert ei.value.status == sg.SG_ERR_CUDA
+
+
 def test_template_registry_is_current():
     assert sg.sg_template_count() >= 25
     rc = subprocess.run([sys.executable, "-m", "paper_1410_6685_b200.gen_templates", "--check"], cwd=ROOT).returncode
