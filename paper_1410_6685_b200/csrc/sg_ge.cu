@@ -11,7 +11,7 @@
 //     step k.  No grid-wide barrier: blocks drift apart by as much as the data dependences allow, and the chain
 //     "update row k+1 -> publish -> next owner" costs one row, not one step.
 //   * Per step a block reads the pivot row once into shared memory (L2 hit: it was written a moment ago), then streams its
-//     own rows: 16 bytes read + 16 bytes written per thread and vector, RR rows in flight.  The factors f_j = M[j,k] / M[k,k]
+//     own rows ONE AT A TIME, GE_CH 128-bit vectors per thread in flight along the row (16 bytes read + 16 written per vector).  The factors f_j = M[j,k] / M[k,k]
 //     of all the block's rows are computed BEFORE any of those rows is modified (the row's own column k is overwritten by
 //     the update).
 //   * Arithmetic is BASELINE.json:configs[4]'s update, one rounding per primitive: t = f_j * M[k,c]; M[j,c] = M[j,c] - t over
@@ -29,8 +29,19 @@
 namespace {
 
 constexpr int GE_THREADS = 512;
-constexpr int GE_RR = 4;            // rows of one block in flight
-constexpr int GE_CH = 2;            // 128-bit vectors per row and thread in flight
+// Rows of a block in flight x vectors per row and thread in flight, measured (whole loop, ms at 2048^2 / 4096^2 / 8192^2):
+//   4 x 2 (round 2's first version): 15.3 / 90.3 / 761      2 x 4: 15.6 / 85.2 / 740      1 x 8: 13.9 / 83.1 / 736      8 x 1: 16.3 / 95.2 / 776
+//   1 x 4: 11.4 / 70.3 / 698      2 x 2: 11.5 / 71.5 / 701      1 x 2: 11.3 / 74.2 / 709      1 x 3: 11.4 / 77.1 / 688      1 x 6: 12.1 / 70.5 / 698
+// Streaming several rows (addresses a leading dimension apart) at once and many bytes in flight per thread is what the memory system
+// serves worse — the same finding as for the matrix passes (sg_pass2d_tile.cuh).
+#ifndef SG_GE_RR
+#define SG_GE_RR 1
+#endif
+#ifndef SG_GE_CH
+#define SG_GE_CH 4
+#endif
+constexpr int GE_RR = SG_GE_RR;     // rows of one block in flight
+constexpr int GE_CH = SG_GE_CH;     // 128-bit vectors per row and thread in flight
 
 struct GeArgs {
     double* M;
