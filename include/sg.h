@@ -38,7 +38,10 @@ extern "C" {
 #endif
 
 typedef struct sg_ctx sg_ctx;   /* opaque */
-typedef int64_t sg_handle;      /* > 0 valid; vectors, matrices and scalars share one table */
+typedef int64_t sg_handle;      /* > 0 valid, opaque; vectors, matrices and scalars share one table.  A handle is a table slot tagged
+                                 * with the slot's generation: slots of released values are reused, so a loop that releases what it
+                                 * makes keeps the table at its high-water mark; a handle used after its last release is
+                                 * SG_ERR_ARG (unknown handle), never an alias of the slot's next value */
 typedef int32_t sg_status;
 
 enum {
@@ -205,7 +208,8 @@ sg_status sg_vec_data(sg_ctx* ctx, sg_handle v, void** dev_ptr);
  * (count * element size bytes, contiguous) to HOST memory in one action.  bytes must be >= that size. */
 sg_status sg_vec_read(sg_ctx* ctx, sg_handle v, void* host_out, size_t bytes);
 /* Drop the caller's reference.  An unreferenced pending intermediate is never materialised.  A collection or scalar that a
- * pending operation still reads may be released before the flush: its storage lives until that flush has consumed it. */
+ * pending operation still reads may be released before the flush: its storage lives until that flush has consumed it.
+ * After the last release the handle is invalid (SG_ERR_ARG); its table slot is reused by later handles. */
 sg_status sg_release(sg_ctx* ctx, sg_handle h);
 
 /* transpose: a NEW cols x rows matrix with out[j][i] = m[i][j] (F32/F64/I32/I64), written to dev_out_or_null

@@ -13,14 +13,31 @@ sg_status sg_fail(sg_ctx* c, sg_status code, const std::string& msg) {
     return code;
 }
 
+// A handle is (generation << 32) | (slot + 1).  Slots of dead values are recycled (retire_nodes puts them on free_values once no
+// pending operation can name them), so a long-running loop's table stays as large as its high-water mark of live handles; the
+// generation makes a handle that was released, and whose slot now holds another value, an unknown handle instead of an alias.
+static inline int hidx(sg_handle h) { return (int)(h & 0xffffffffll) - 1; }
+static inline sg_handle hnd(const sg_ctx* c, int idx) { return ((sg_handle)c->values[idx].gen << 32) | (sg_handle)(idx + 1); }
 static Value* val(sg_ctx* c, sg_handle h) {
-    if (h <= 0 || (size_t)h > c->values.size() || !c->values[h - 1].alive) return nullptr;
-    return &c->values[h - 1];
+    const int64_t slot = (h & 0xffffffffll) - 1;
+    if (h <= 0 || slot < 0 || (size_t)slot >= c->values.size()) return nullptr;
+    Value& v = c->values[slot];
+    if (!v.alive || (sg_handle)v.gen != (h >> 32)) return nullptr;
+    return &v;
 }
 static sg_handle new_value(sg_ctx* c, const Value& v) {
-    c->values.push_back(v);
-    c->live.push_back((int)c->values.size() - 1);
-    return (sg_handle)c->values.size();
+    int idx;
+    if (!c->free_values.empty()) {
+        idx = c->free_values.back(); c->free_values.pop_back();
+        const uint32_t gen = (c->values[idx].gen + 1) & 0x7fffffffu;
+        c->values[idx] = v;
+        c->values[idx].gen = gen;
+    } else {
+        c->values.push_back(v);
+        idx = (int)c->values.size() - 1;
+    }
+    c->live.push_back(idx);
+    return hnd(c, idx);
 }
 
 void* sg_dev_alloc(sg_ctx* c, size_t bytes) {
@@ -263,25 +280,25 @@ static sg_status append_map(sg_ctx* c, uint8_t op, int n_opd, const Operand* opd
         Value old = *d;
         old.user_refs = 0;                      // the previous contents stay reachable for already-enqueued readers
         old.owned = false;                      // the handle keeps owning the storage
-        const int old_id = (int)new_value(c, old) - 1;
+        const int old_id = hidx(new_value(c, old));
         d = val(c, dst);
         for (int i = 0; i < n_opd; ++i)         // this operation itself reads the previous contents
-            if (nd.opd[i].kind != OPD_IMM && nd.opd[i].value == (int)dst - 1) nd.opd[i].value = old_id;
+            if (nd.opd[i].kind != OPD_IMM && nd.opd[i].value == hidx(dst)) nd.opd[i].value = old_id;
         for (auto& n : c->nodes)                // earlier pending readers of this handle read the previous contents
             if (!n.done)
                 for (int i = 0; i < n.n_opd; ++i)
-                    if (n.opd[i].kind != OPD_IMM && n.opd[i].value == (int)dst - 1) n.opd[i].value = old_id;
+                    if (n.opd[i].kind != OPD_IMM && n.opd[i].value == hidx(dst)) n.opd[i].value = old_id;
         for (auto& n : c->nodes)
-            if (!n.done && n.out == (int)dst - 1) {
+            if (!n.done && n.out == hidx(dst)) {
                 // an earlier pending in-place result is superseded: it becomes an anonymous intermediate version
                 // (row.divided_by(p) then row.in_place_minus(q) -> one expression)
                 n.out = old_id;
                 n.inplace = false;
             }
         for (auto& k : c->contracts)
-            if (k.value == (int)dst - 1) k.value = old_id;
+            if (k.value == hidx(dst)) k.value = old_id;
         d->node = (int)c->nodes.size();
-        nd.out = (int)dst - 1; nd.inplace = true;
+        nd.out = hidx(dst); nd.inplace = true;
         c->nodes.push_back(nd);
         *out = dst;
         return SG_OK;
@@ -289,9 +306,9 @@ static sg_status append_map(sg_ctx* c, uint8_t op, int n_opd, const Operand* opd
     Value v;
     v.kind = is2d ? VK_MAT : VK_VEC; v.dtype = out_dtype; v.rows = rows; v.cols = cols; v.ld = cols; v.stride = 1;
     v.materialised = false; v.user_refs = 1; v.node = (int)c->nodes.size();
-    nd.out = (int)new_value(c, v) - 1;
+    nd.out = hidx(new_value(c, v));
     c->nodes.push_back(nd);
-    *out = nd.out + 1;
+    *out = hnd(c, nd.out);
     return SG_OK;
 }
 
@@ -305,7 +322,7 @@ sg_status sg_cast(sg_ctx* c, sg_handle h, sg_dtype to, sg_handle dst, sg_handle*
     if (v->kind != VK_VEC) return sg_fail(c, SG_ERR_UNSUPPORTED, "sg_cast needs a vector");
     if (v->dtype == SG_BOOL || to < SG_F32 || to > SG_I64) return sg_fail(c, SG_ERR_DTYPE, "sg_cast converts between F32, F64, I32 and I64");
     Operand opd[2];
-    opd[0].kind = OPD_VALUE; opd[0].value = (int)h - 1; opd[1] = opd[0];
+    opd[0].kind = OPD_VALUE; opd[0].value = hidx(h); opd[1] = opd[0];
     if ((int)to == v->dtype) return append_map(c, OP_MOV, 1, opd, v->dtype, false, 1, v->cols, dst, out);     // same type: a copy
     if (v->stride != 1) return sg_fail(c, SG_ERR_UNSUPPORTED, "sg_cast of a strided view");
     return append_map(c, NODE_OP_CAST, 1, opd, (int)to, false, 1, v->cols, dst, out, v->dtype);
@@ -364,7 +381,7 @@ sg_status sg_enqueue(sg_ctx* c, sg_op op, const sg_operand* ops, int32_t n, sg_h
     Operand opd[2];
     for (int i = 0; i < n; ++i) {
         if (!vv[i]) { opd[i].kind = OPD_IMM; opd[i].imm = imm_bits(dtype, ops[i]); continue; }
-        opd[i].kind = OPD_VALUE; opd[i].value = (int)ops[i].h - 1; opd[i].bcast = SG_BCAST_NONE;
+        opd[i].kind = OPD_VALUE; opd[i].value = hidx(ops[i].h); opd[i].bcast = SG_BCAST_NONE;
         if (vv[i]->kind == VK_SCALAR) continue;
         have_coll = true;
         if (is2d) {
@@ -440,7 +457,7 @@ sg_status sg_mat_col(sg_ctx* c, sg_handle m, int64_t j, int64_t r0, int64_t r1, 
     Value w = *v;
     w.kind = VK_VEC; w.ptr = v->ptr + (r0 * v->ld + j) * dtype_size(v->dtype); w.rows = 1; w.cols = r1 - r0; w.stride = v->ld; w.ld = w.cols;
     w.owned = false; w.user_refs = 0; w.node = -1;
-    const int view = (int)new_value(c, w) - 1;
+    const int view = hidx(new_value(c, w));
     Operand opd[2];
     opd[0].kind = OPD_VALUE; opd[0].value = view; opd[1] = opd[0];
     return append_map(c, OP_MOV, 1, opd, w.dtype, false, 1, w.cols, 0, out);
@@ -461,7 +478,7 @@ static sg_status append_reduce(sg_ctx* c, uint8_t kind, sg_handle h, int axis, i
     if ((kind == OUT_MAX || kind == OUT_MIN) && (v->rows * v->cols == 0)) return sg_fail(c, SG_ERR_EMPTY, "max/min of an empty collection");
     Node nd;
     nd.kind = NK_REDUCE; nd.op = kind; nd.n_opd = 1; nd.axis = axis;
-    nd.opd[0].kind = OPD_VALUE; nd.opd[0].value = (int)h - 1;
+    nd.opd[0].kind = OPD_VALUE; nd.opd[0].value = hidx(h);
     nd.dtype = v->dtype; nd.is2d = is2d; nd.rows = v->rows; nd.cols = v->cols;
     Value r;
     r.dtype = result_dtype; r.materialised = false; r.user_refs = 1; r.node = (int)c->nodes.size();
@@ -472,9 +489,9 @@ static sg_status append_reduce(sg_ctx* c, uint8_t kind, sg_handle h, int axis, i
     } else {
         r.kind = VK_VEC; r.rows = 1; r.cols = (axis == AXIS_ROWS) ? v->rows : v->cols; r.ld = r.cols;
     }
-    nd.out = (int)new_value(c, r) - 1;
+    nd.out = hidx(new_value(c, r));
     c->nodes.push_back(nd);
-    *out = nd.out + 1;
+    *out = hnd(c, nd.out);
     return SG_OK;
 }
 
@@ -523,8 +540,8 @@ sg_status sg_forall_adjacent(sg_ctx* c, sg_handle h, sg_op cmp, sg_handle* out) 
     if (v->kind != VK_VEC || v->dtype == SG_BOOL) return sg_fail(c, SG_ERR_ARG, "adjacent predicate needs a numeric vector");
     // b_i = v_i cmp v_{i+1}, i in [0, n-2]: the zip of subset(0,n-1) with subset(1,n)
     Operand opd[2];
-    opd[0].kind = OPD_VALUE; opd[0].value = (int)h - 1;
-    opd[1].kind = OPD_SHIFT; opd[1].value = (int)h - 1;
+    opd[0].kind = OPD_VALUE; opd[0].value = hidx(h);
+    opd[1].kind = OPD_SHIFT; opd[1].value = hidx(h);
     sg_handle b;
     const int64_t m = v->cols > 0 ? v->cols - 1 : 0;
     s = append_map(c, (uint8_t)cmp, 2, opd, v->dtype, false, 1, m, 0, &b);
@@ -547,8 +564,8 @@ sg_status sg_filter(sg_ctx* c, sg_handle values, sg_handle mask, void* dev_out, 
     if (dev_out && capacity < 0) return sg_fail(c, SG_ERR_ARG, "negative capacity");
     Node nd;
     nd.kind = NK_FILTER; nd.n_opd = 2;
-    nd.opd[0].kind = OPD_VALUE; nd.opd[0].value = (int)values - 1;
-    nd.opd[1].kind = OPD_VALUE; nd.opd[1].value = (int)mask - 1;
+    nd.opd[0].kind = OPD_VALUE; nd.opd[0].value = hidx(values);
+    nd.opd[1].kind = OPD_VALUE; nd.opd[1].value = hidx(mask);
     nd.dtype = v->dtype; nd.rows = 1; nd.cols = v->cols;
     Value cnt;
     cnt.kind = VK_SCALAR; cnt.dtype = SG_I64; cnt.rows = cnt.cols = cnt.ld = 1; cnt.user_refs = 1; cnt.node = (int)c->nodes.size();
@@ -559,11 +576,11 @@ sg_status sg_filter(sg_ctx* c, sg_handle values, sg_handle mask, void* dev_out, 
     r.user_refs = 1; r.node = (int)c->nodes.size(); r.count_known = false; r.count_slot = cnt.slot;
     if (dev_out) r.ptr = (char*)dev_out;
     nd.inplace = dev_out != nullptr;
-    nd.out = (int)new_value(c, r) - 1;
-    nd.out2 = (int)new_value(c, cnt) - 1;
+    nd.out = hidx(new_value(c, r));
+    nd.out2 = hidx(new_value(c, cnt));
     c->nodes.push_back(nd);
-    *out_vec = nd.out + 1;
-    *out_count = nd.out2 + 1;
+    *out_vec = hnd(c, nd.out);
+    *out_count = hnd(c, nd.out2);
     return SG_OK;
 }
 
@@ -572,7 +589,7 @@ sg_status sg_contract(sg_ctx* c, sg_handle h, int32_t kind, const char* tag) {
     Value* v = val(c, h);
     if (!v || v->kind != VK_SCALAR || v->dtype != SG_BOOL) return sg_fail(c, SG_ERR_ARG, "a contract is a BOOL scalar");
     if (kind != SG_CONTRACT_PRE && kind != SG_CONTRACT_POST) return sg_fail(c, SG_ERR_ARG, "bad contract kind");
-    c->contracts.push_back({(int)h - 1, kind, tag ? tag : ""});
+    c->contracts.push_back({hidx(h), kind, tag ? tag : ""});
     return SG_OK;
 }
 
@@ -747,9 +764,9 @@ sg_status sg_release(sg_ctx* c, sg_handle h) {
         for (auto& n : c->nodes)
             if (!n.done)
                 for (int i = 0; i < n.n_opd; ++i)
-                    if (n.opd[i].kind != OPD_IMM && n.opd[i].value == (int)h - 1) return SG_OK;
+                    if (n.opd[i].kind != OPD_IMM && n.opd[i].value == hidx(h)) return SG_OK;
         for (auto& k : c->contracts)
-            if (k.value == (int)h - 1) return SG_OK;
+            if (k.value == hidx(h)) return SG_OK;
         if (v->owned && v->ptr) { c->deferred_free.push_back(v->ptr); v->ptr = nullptr; v->owned = false; }
         if (v->slot >= 0 && v->kind == VK_SCALAR) { c->slab_free.push_back(v->slot); v->slot = -1; }
         v->alive = false;

@@ -39,6 +39,7 @@ struct Value {
     int64_t slot = -1;              // VK_SCALAR produced by a reduction: slot in the scalar slab
     bool alive = true;
     bool fresh_alloc = false;       // storage allocated by the flush in progress (given back if that flush fails before it runs)
+    uint32_t gen = 0;               // generation of the table slot (upper half of the handle): a recycled slot does not answer to its old handle
     bool undecided = false;         // quantifier whose pass ended early at a violated contract before it was decided: reading it is an error
 };
 
@@ -102,6 +103,7 @@ struct sg_ctx {
     std::string err;
 
     std::vector<Value> values;      // handle h <-> values[h-1]
+    std::vector<int> free_values;   // slots of dead values no pending operation names any more: reused by new handles
     std::vector<int> live;          // indices of values that may still be alive (compacted at every flush: a flush costs O(live), not O(history))
     std::vector<Node> nodes;        // pending actions, in call order
     std::vector<Contract> contracts;

@@ -268,6 +268,9 @@ int sgk_plan(const SgProg& prog, SgArgs& a, int force_bytecode, int sm_count, in
         const long K = !tid ? 0 : ee ? k_ee : has_red ? k_red : k_store;     // the bytecode kernel decodes its program per block: persistent
         long blocks = std::min<long>(want, (long)sm_count * occ);
         if (K > 0) blocks = std::max<long>(blocks, (want + K - 1) / K);
+        // short reduction passes: fewer, longer-lived blocks (SG_SMALL_OCC per SM while a full grid would get < SG_SMALL_TILES tiles per block)
+        static const long small_occ = env_long("SG_SMALL_OCC", 0), small_tiles = env_long("SG_SMALL_TILES", 4);
+        if (tid && has_red && K == 0 && small_occ > 0 && want < (long)sm_count * occ * small_tiles) blocks = std::min<long>(want, (long)sm_count * std::min<long>(occ, small_occ));
         geom->grid = (int)std::max<long>(1, blocks);
         const long pct = has_store ? pct_rw : pct_ro;
         const long per_block = a.n_full_tiles / geom->grid;

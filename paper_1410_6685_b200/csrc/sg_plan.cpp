@@ -373,6 +373,7 @@ void retire_nodes(sg_ctx* c, int executed) {
             } else v.alive = false;
         }
         if (v.alive) c->live[keep++] = i;
+        else c->free_values.push_back(i);       // the pending list is empty: nothing names this slot any more
     }
     c->live.resize(keep);
 }

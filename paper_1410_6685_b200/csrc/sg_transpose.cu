@@ -16,9 +16,10 @@
 namespace {
 
 constexpr int TILE = 64, ROWS = 8, TBLOCK = TILE * ROWS;      // measured at 16384^2 fp64: ROWS 4 / 8 / 16 -> 0.774 / 0.651 / 0.749 ms
-// 4-byte elements run at 0.79 of the measured peak (fp64: 1.01).  128 x 128 tiles (512-byte segments on both sides, like fp64) were
-// measured and change nothing (422 vs 415 us at 16384^2 fp32): the fp32 mover is bound by its four 4-byte memory instructions per
-// element (LDG, STS, LDS, STG), not by the segment length; the paper's transpose benchmark is DOUBLE.
+// 4-byte elements through this kernel run at 0.79 of the measured peak (fp64: 1.01), and 128 x 128 tiles (512-byte segments on both
+// sides) change nothing (422 vs 415 us at 16384^2 fp32): that mover is bound by its four 4-byte memory instructions per element (LDG,
+// STS, LDS, STG), not by the segment length.  So 4-byte matrices whose rows are 8-byte aligned on both sides take transpose_pairs
+// below: every memory instruction moves 8 bytes, as for fp64.
 
 template <class T>
 __global__ void __launch_bounds__(TBLOCK) transpose_tiled(const T* __restrict__ in, int64_t ld_in, int64_t rows, int64_t cols,
@@ -52,6 +53,49 @@ __global__ void __launch_bounds__(TBLOCK) transpose_tiled(const T* __restrict__ 
     }
 }
 
+
+// 4-byte elements, 8-byte accesses: a tile is PR x 2 source rows by TILE source columns.  A thread loads the two 8-byte pairs of a
+// 2 x 2 block (rows 2q, 2q+1; columns 2t, 2t+1), transposes it in registers and writes the two row-pairs (a[2q][c], a[2q+1][c]) to
+// shared memory; even source columns fill the upper half of the shared tile and odd ones the lower half, so a half-warp's 8-byte
+// stores are a stride of 65 pairs apart (16 distinct bank pairs).  The destination rows are then read as contiguous pairs and stored
+// as PR * 8 = 512-byte segments.  Eight independent 8-byte loads per thread before the barrier, 32 KB per block, as for fp64.
+constexpr int PR = 64;                                         // row pairs per tile: 128 source rows x 64 source columns
+__global__ void __launch_bounds__(TBLOCK) transpose_pairs(const unsigned int* __restrict__ in, int64_t ld_in, int64_t rows, int64_t cols,
+                                                          unsigned int* __restrict__ out, int64_t ld_out, int64_t tiles_c) {
+    __shared__ uint2 tile[TILE][PR + 1];
+    const int64_t tr = blockIdx.x / tiles_c, tc = blockIdx.x % tiles_c;
+    const int64_t r0 = tr * (2 * PR), c0 = tc * TILE;
+    if ((r0 + 2 * PR <= rows) && (c0 + TILE <= cols)) {
+        const int t = threadIdx.x % (TILE / 2), qy = threadIdx.x / (TILE / 2);        // pair column 0..31, row-pair group 0..15
+        constexpr int QS = TBLOCK / (TILE / 2), NQ = PR / QS;                         // 16 row pairs per sweep, 4 sweeps
+        uint2 a0[NQ], a1[NQ];
+#pragma unroll
+        for (int i = 0; i < NQ; ++i) {
+            const unsigned int* src = in + (r0 + 2 * (qy + QS * i)) * ld_in + c0 + 2 * t;
+            a0[i] = __ldcs(reinterpret_cast<const uint2*>(src));
+            a1[i] = __ldcs(reinterpret_cast<const uint2*>(src + ld_in));
+        }
+#pragma unroll
+        for (int i = 0; i < NQ; ++i) {
+            tile[t][qy + QS * i] = make_uint2(a0[i].x, a1[i].x);                      // source column 2t
+            tile[TILE / 2 + t][qy + QS * i] = make_uint2(a0[i].y, a1[i].y);           // source column 2t + 1
+        }
+        __syncthreads();
+        const int q = threadIdx.x % PR, cy = threadIdx.x / PR;                        // row pair 0..63, destination-row group 0..7
+        constexpr int CS = TBLOCK / PR;
+#pragma unroll
+        for (int j = 0; j < TILE / CS; ++j) {
+            const int c = cy + CS * j;
+            __stcs(reinterpret_cast<uint2*>(out + (c0 + c) * ld_out + r0 + 2 * q), tile[(c & 1) * (TILE / 2) + (c >> 1)][q]);
+        }
+    } else {                                                                          // ragged edge tiles: element by element
+        for (int e = threadIdx.x; e < 2 * PR * TILE; e += TBLOCK) {
+            const int64_t c = c0 + e / (2 * PR), r = r0 + e % (2 * PR);
+            if (r < rows && c < cols) out[c * ld_out + r] = in[r * ld_in + c];
+        }
+    }
+}
+
 }  // namespace
 
 cudaError_t sgk_transpose(const void* in, int64_t ld_in, int64_t rows, int64_t cols, void* out, int64_t ld_out, int elem_size, cudaStream_t stream) {
@@ -61,8 +105,14 @@ cudaError_t sgk_transpose(const void* in, int64_t ld_in, int64_t rows, int64_t c
     if (tiles > 0x7fffffffll) return cudaErrorInvalidValue;
     if (elem_size == 8)
         transpose_tiled<unsigned long long><<<(unsigned)tiles, TBLOCK, 0, stream>>>((const unsigned long long*)in, ld_in, rows, cols, (unsigned long long*)out, ld_out, tiles_c);
-    else if (elem_size == 4)
-        transpose_tiled<unsigned int><<<(unsigned)tiles, TBLOCK, 0, stream>>>((const unsigned int*)in, ld_in, rows, cols, (unsigned int*)out, ld_out, tiles_c);
+    else if (elem_size == 4) {
+        const bool pairs = ((reinterpret_cast<uintptr_t>(in) | reinterpret_cast<uintptr_t>(out)) % 8 == 0) && ld_in % 2 == 0 && ld_out % 2 == 0;
+        const int64_t ptiles = ((rows + 2 * PR - 1) / (2 * PR)) * tiles_c;
+        if (pairs && rows >= 2 * PR)
+            transpose_pairs<<<(unsigned)ptiles, TBLOCK, 0, stream>>>((const unsigned int*)in, ld_in, rows, cols, (unsigned int*)out, ld_out, tiles_c);
+        else
+            transpose_tiled<unsigned int><<<(unsigned)tiles, TBLOCK, 0, stream>>>((const unsigned int*)in, ld_in, rows, cols, (unsigned int*)out, ld_out, tiles_c);
+    }
     else
         return cudaErrorInvalidValue;
     return cudaGetLastError();

@@ -328,6 +328,34 @@ def test_float_sums_are_the_same_bits_on_every_run(dtype):
     assert sum_ok(got, ocfg.dot_product(x, y), orc.zip("mul", x, y), 1e-12 if dtype is np.float64 else 1e-5)
 
 
+@pytest.mark.parametrize("mode", ["template", "bytecode"])
+def test_recycled_handle_slots_keep_results_right(mode):
+    """300 steps in one context, every intermediate released: the handle table stays a few slots long (the slots of dead values are
+    reused under a new generation) and every step's stored vector, sum and maximum still match the oracle."""
+    n = 5000
+    x = RNG.standard_normal(n).astype(np.float32)
+    slots = set()
+    with Ctx(MODES[mode]) as c:
+        hx = c.vec(x)
+        for it in range(300):
+            k = np.float32(0.25 * (it % 7) - 0.5)
+            t = sg.sg_enqueue(c.ctx, sg.SG_MUL, [hx, sg.F(float(k))])
+            u = sg.sg_enqueue(c.ctx, sg.SG_ADD, [t, hx])                   # stored: read back below
+            s, m = sg.sg_reduce(c.ctx, u, sg.SG_SUM), sg.sg_reduce(c.ctx, u, sg.SG_RMAX)
+            sg.sg_release(c.ctx, t)
+            got_s, got_m = c.get(s), c.get(m)
+            slots |= {h & 0xffffffff for h in (t, u, s, m)}
+            if it % 50 == 0 or it == 299:
+                want_u = orc.zip("add", orc.scalar("mul", x, k), x)
+                assert bits_equal(c.read_vec(u, np.float32), want_u)
+                assert sum_ok(got_s, orc.sum(want_u), want_u, 1e-5) and np.float32(got_m) == orc.max(want_u)
+            for h in (u, s, m):
+                sg.sg_release(c.ctx, h)
+        with pytest.raises(sg.SgError):                                     # a released handle is unknown, whatever its slot holds now
+            sg.sg_vec_count(c.ctx, u)
+    assert len(slots) <= 12, sorted(slots)
+
+
 @pytest.mark.parametrize("dtype", [np.int32, np.int64, np.float32])
 def test_exact_reductions_through_tile_tickets(dtype):
     """Integer sum / max / min (float: max / min only) of a vector long enough that the last part of the tiles is handed out through

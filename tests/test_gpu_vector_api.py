@@ -337,7 +337,9 @@ def test_matvec_exact_integer_regime_and_dimension_contract():
 # ----------------------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("dtype", [np.float64, np.float32, np.int32, np.int64])
 @pytest.mark.parametrize("rows,cols,ld,ld_out", [(1, 1, 1, 0), (1, 7, 7, 0), (7, 1, 3, 9), (64, 64, 64, 0), (65, 63, 70, 66), (130, 1000, 1000, 0),
-                                                 (1000, 130, 136, 1001), (257, 513, 513, 0)])
+                                                 (1000, 130, 136, 1001), (257, 513, 513, 0),
+                                                 # 4-byte elements with 8-byte aligned rows take the pair kernel (128 x 64 tiles): full tiles, ragged edges, padding
+                                                 (128, 64, 64, 0), (256, 192, 192, 0), (300, 200, 202, 302), (1000, 130, 136, 1002)])
 def test_transpose(dtype, rows, cols, ld, ld_out):
     M = RNG.integers(-10**6, 10**6, (rows, cols)).astype(dtype)
     Mp = np.full((rows, ld), -7, dtype=dtype)

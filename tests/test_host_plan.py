@@ -429,6 +429,46 @@ def test_release_before_flush_keeps_storage_for_pending_readers():
         sg.sg_ctx_destroy(ctx)
 
 
+def test_handle_slots_are_recycled_and_stale_handles_are_unknown():
+    """A long-running loop must not grow the handle table: the slot of a dead value is reused once no pending operation can name
+    it, under a new generation — the released handle is then an unknown handle, never an alias of the slot's new value."""
+    ctx = sg.sg_ctx_create(-1)
+    try:
+        x = sg.sg_vec_create(ctx, sg.SG_F32, 4096, None)
+        slots, first = set(), None
+        for it in range(200):                                 # x -> (x + 1) * 2 -> sum, everything released every step
+            t = sg.sg_enqueue(ctx, sg.SG_ADD, [x, sg.F(1.0)])
+            u = sg.sg_enqueue(ctx, sg.SG_MUL, [t, sg.F(2.0)])
+            s = sg.sg_reduce(ctx, u, sg.SG_SUM)
+            sg.sg_release(ctx, t)
+            sg.sg_flush(ctx)
+            assert sg.sg_plan_stats(ctx).n_passes == 1
+            assert sg.sg_vec_count(ctx, u) == 4096 and sg.sg_vec_count(ctx, s) == 1
+            for h in (t, u, s):
+                slots.add(h & 0xffffffff)
+            first = first or (t, u, s)
+            sg.sg_release(ctx, u)
+            sg.sg_release(ctx, s)
+        assert len(slots) <= 9, slots                          # 600 handles lived in a handful of slots (at most three steps' worth)
+        assert sg.sg_vec_count(ctx, x) == 4096                 # a handle that was never released still answers
+        for h in first:                                        # the first step's handles: their slots hold other values now
+            with pytest.raises(sg.SgError) as e:
+                sg.sg_vec_count(ctx, h)
+            assert e.value.status == sg.SG_ERR_ARG
+            with pytest.raises(sg.SgError):
+                sg.sg_enqueue(ctx, sg.SG_ADD, [h, sg.F(1.0)])
+        # a slot is not reused while a pending operation still reads its value
+        y = sg.sg_enqueue(ctx, sg.SG_ADD, [x, sg.F(3.0)])
+        z = sg.sg_enqueue(ctx, sg.SG_MUL, [y, y])
+        sg.sg_release(ctx, y)
+        fresh = [sg.sg_enqueue(ctx, sg.SG_SUB, [x, sg.F(float(k))]) for k in range(8)]
+        assert all((f & 0xffffffff) != (y & 0xffffffff) for f in fresh)
+        sg.sg_flush(ctx)
+        assert sg.sg_vec_count(ctx, z) == 4096
+    finally:
+        sg.sg_ctx_destroy(ctx)
+
+
 def test_a_failed_flush_discards_the_pending_list_and_leaves_the_context_usable():
     ctx = sg.sg_ctx_create(-1)
     try:
