@@ -446,7 +446,7 @@ def matvec_section(torch, sg, W, inputs, measure):
     measure.out["transpose_fp64_16384^2"] = {"ms": ms, "algorithmic_bytes": 16 * n * n, "GB/s": 16 * n * n / ms / 1e6,
                                              "frac_of_peak": 16 * n * n / ms / 1e6 / measure.peak, "passes": 1, "template_passes": 0}
     del T
-    # fp32: 256-byte segments per tile row instead of 512
+    # fp32: the pair kernel (8-byte accesses, 128 x 64 tiles: 256-byte source segments, 512-byte destination segments)
     M32 = M.to(torch.float32)
     T32 = torch.empty_like(M32)
     ctx = sg.sg_ctx_create(0, stream)

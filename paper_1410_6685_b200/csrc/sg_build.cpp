@@ -51,7 +51,11 @@ struct Builder {
         }
         PassInput in{};
         in.kind = kind; in.ptr = ptr; in.stride = stride; in.imm = imm; in.value = ref; in.boolvec = boolvec;
-        in.reg = boolvec ? alloc_p() : alloc_v();
+        // An input lives in its register from the START of the program (every input of a tile is loaded before the first instruction
+        // runs), so it must never take a register that an earlier temporary has used and given back: `(a+b)*(c+d) + e` would load e
+        // into the register c+d is then computed in.  Inputs always get a register of their own.
+        if (boolvec) { pfree.push_back(0); in.reg = n_preg++; }
+        else { vfree.push_back(0); in.reg = n_vreg++; }
         inputs.push_back(in);
         *fresh = true;
         return (int)inputs.size() - 1;

@@ -29,7 +29,7 @@ TUNE = {
     "red": (4, 4, 4),
     "extrema": (4, 4, 4),
     "sorted_f32": (4, 4, 4),
-    "cfg4": (2, 2, 4),
+    "cfg4": (2, 2, 4),      # measured at 16384^2 (k = 0 / k = 8191): (2,2,4,3) 0.765 / 0.393 ms; (1,4,4,3) 0.780 / 0.400; (2,3,4,2) 0.772 / 0.406 (80 registers, spills); (1,4,8,2) 0.813 / 0.418
     "matvec": (2, 2, 4, 3),   # measured: (2, 4, 2, 3) is slower (0.430 / 0.379 ms vs 0.376 / 0.343 ms right / left at 16384^2)
     "matvec_right": (2, 3, 4, 2),   # per-row double-double sums are latency-bound: TWO stages and three blocks per SM: 0.374 -> 0.343 ms (left: 0.341 -> 0.359, kept at three stages)
     "cfg2": (2, 2, 2),      # filter: tile = 4*unroll steps, min blocks per SM, input stages

@@ -162,6 +162,31 @@ def test_all_primitives(dtype, n):
         assert c.get(cnt) == orc.count(orc.cmp("lt", a, b))
 
 
+@pytest.mark.parametrize("dtype", [np.float32, np.float64, np.int32, np.int64])
+@pytest.mark.parametrize("n", [3, 1025, 70001])
+def test_input_first_named_after_two_temporaries_died(dtype, n):
+    """`((a+b)*(c+d) + e) * 3`: the multiplication gives two registers back and e is first named afterwards.  Every input of a tile is
+    loaded before the first instruction runs, so e must not live in the register c+d is computed in (the plan builder gave inputs
+    recycled registers until round 2: e was overwritten, silently in a template instance, out of bounds in the bytecode file)."""
+    v = [rand(dtype, n) for _ in range(5)]
+    imm = sg.F(3.0) if np.dtype(dtype).kind == "f" else sg.I(3)
+    with Ctx() as c:
+        h = [c.vec(x) for x in v]
+        t1 = sg.sg_enqueue(c.ctx, sg.SG_ADD, [h[0], h[1]])
+        t2 = sg.sg_enqueue(c.ctx, sg.SG_ADD, [h[2], h[3]])
+        t3 = sg.sg_enqueue(c.ctx, sg.SG_MUL, [t1, t2])
+        t4 = sg.sg_enqueue(c.ctx, sg.SG_ADD, [t3, h[4]])
+        t5 = sg.sg_enqueue(c.ctx, sg.SG_MUL, [t4, imm])
+        for t in (t1, t2, t3, t4):
+            sg.sg_release(c.ctx, t)
+        m = sg.sg_reduce(c.ctx, t5, sg.SG_RMAX)
+        got, got_m = c.read_vec(t5, dtype), c.get(m)
+        assert sg.sg_plan_stats(c.ctx).n_passes == 1
+    want = orc.scalar("mul", orc.zip("add", orc.zip("mul", orc.zip("add", v[0], v[1]), orc.zip("add", v[2], v[3])), v[4]), 3.0 if np.dtype(dtype).kind == "f" else 3)
+    assert bits_equal(got, want)
+    assert bits_equal(np.array([got_m], dtype=dtype), np.array([orc.max(want)], dtype=dtype))
+
+
 @pytest.mark.parametrize("dtype,tol", [(np.float32, 1e-5), (np.float64, 1e-12), (np.int32, 0), (np.int64, 0)])
 @pytest.mark.parametrize("n", [1, 2, 33, 1024, 1025, 70001])
 def test_reductions_all_dtypes(dtype, tol, n):

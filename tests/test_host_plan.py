@@ -469,6 +469,69 @@ def test_handle_slots_are_recycled_and_stale_handles_are_unknown():
         sg.sg_ctx_destroy(ctx)
 
 
+_VALUE_OPS = {"OP_ADD", "OP_SUB", "OP_MUL", "OP_DIV", "OP_MIN", "OP_MAX", "OP_MOD", "OP_NEG", "OP_ABS", "OP_MOV", "OP_SQRT"}
+
+
+def _input_registers_are_never_written(dump: str) -> bool:
+    """Every input of a tile is loaded before the first instruction runs, so no instruction may write a register an input lives in."""
+    groups = re.findall(r"\{(IN_[A-Z_]+),(\d+),(\d+),(\d+)\}", dump)
+    v_in = {int(reg) for kind, _, reg, _ in groups if kind != "IN_BOOLVEC"}
+    p_in = {int(reg) for kind, _, reg, _ in groups if kind == "IN_BOOLVEC"}
+    for op, dst, _, _ in re.findall(r"\{(OP_[A-Z]+),(\d+),(\d+),(\d+)\}", dump):
+        if int(dst) in (v_in if op in _VALUE_OPS else p_in):
+            return False
+    return True
+
+
+def test_an_input_never_shares_a_register_with_an_earlier_temporary():
+    """`(a+b)*(c+d) + e`: the multiplication gives two registers back, and e — first named afterwards — must not move into the one
+    c+d was computed in (it is loaded at the start of the tile and would be overwritten).  Checked on that chain, on 200 random
+    operation DAGs (the generator of tests/test_gpu_random_chains.py, planned on a plan-only context) and on every registered
+    template program."""
+    def chain(ctx):
+        v = [sg.sg_vec_create(ctx, sg.SG_F64, 4096, None) for _ in range(5)]
+        t1 = sg.sg_enqueue(ctx, sg.SG_ADD, [v[0], v[1]])
+        t2 = sg.sg_enqueue(ctx, sg.SG_ADD, [v[2], v[3]])
+        t3 = sg.sg_enqueue(ctx, sg.SG_MUL, [t1, t2])
+        t4 = sg.sg_enqueue(ctx, sg.SG_ADD, [t3, v[4]])
+        t5 = sg.sg_enqueue(ctx, sg.SG_MUL, [t4, sg.F(3.0)])
+        for t in (t1, t2, t3, t4):
+            sg.sg_release(ctx, t)
+        return t5
+    st, dumps = plan(chain)
+    assert st.n_passes == 1 and _input_registers_are_never_written(dumps[0]), dumps[0]
+
+    import numpy as np
+    import test_gpu_random_chains as R
+
+    class PlanOnly:                       # the slice of tests/gpu_util.Ctx that run_gpu uses, on a context without a device
+        def __init__(self):
+            self.ctx = sg.sg_ctx_create(-1)
+
+        def vec(self, a):
+            return sg.sg_vec_create(self.ctx, {"float32": sg.SG_F32, "float64": sg.SG_F64, "int32": sg.SG_I32, "int64": sg.SG_I64}[a.dtype.name], a.size, None)
+
+        def get(self, h):
+            return 0
+    for seed in range(200):
+        rng = np.random.default_rng(5000 + seed)
+        dtype = R.DTYPES[seed % 4]
+        n_inputs = int(rng.integers(1, 4))
+        inputs = [R.make_input(rng, dtype, 64) for _ in range(n_inputs)]
+        steps, keep, reds = R.build_dag(rng, dtype, n_inputs)
+        c = PlanOnly()
+        try:
+            _, _, stats = R.run_gpu(c, steps, keep, reds, inputs, dtype)
+            for p in range(stats.n_passes):
+                d = sg.sg_plan_dump(c.ctx, p)
+                assert _input_registers_are_never_written(d), (seed, d)
+        finally:
+            sg.sg_ctx_destroy(c.ctx)
+    inc = open(os.path.join(ROOT, "paper_1410_6685_b200", "csrc", "sg_templates_gen.inc")).read()
+    progs = inc.split("SG_TEMPLATE(")[1:]
+    assert len(progs) >= 50 and all(_input_registers_are_never_written(pr) for pr in progs)
+
+
 def test_a_failed_flush_discards_the_pending_list_and_leaves_the_context_usable():
     ctx = sg.sg_ctx_create(-1)
     try:
