@@ -58,7 +58,8 @@ typedef std::vector<std::vector<ExitMember>> ExitGroups;
 // Plans and launches everything pending.  *executed = number of passes whose kernels were queued on the stream when the
 // function returned (all of them on success).  On failure the caller rolls the context back (retire_nodes).
 sg_status flush_body(sg_ctx* c, int* executed, ExitGroups* exit_groups) {
-    const bool unfused = c->flags & SG_FLAG_UNFUSED;
+    bool unfused = c->flags & SG_FLAG_UNFUSED;
+    struct FlagGuard { sg_ctx* c; uint32_t flags; ~FlagGuard() { c->flags = flags; } } flag_guard{c, c->flags};   // the last-resort lowering below sets SG_FLAG_UNFUSED for this flush only
     std::vector<Node>& N = c->nodes;
     std::vector<Value>& V = c->values;
     int64_t launches_total = c->stats.launches_total;
@@ -108,8 +109,24 @@ sg_status flush_body(sg_ctx* c, int* executed, ExitGroups* exit_groups) {
     }
 
     // ---- 3. pass assignment ------------------------------------------------------------------------------
+    // A pass holds at most SG_MAX_OUT outputs.  Stores and reductions are counted when an operation joins a pass, but an intermediate
+    // that joined as a register value becomes one more output LATER, when a consumer ends up in a later pass (a spill) — so the first
+    // assignment may overfill a pass.  Then the assignment is repeated with outputs held in reserve for such spills (2, 4, 6, 7 of the
+    // 8), and as the last resort with the unfused lowering, which always fits (one operation, one output per pass).
     std::vector<Pass> passes;
-    std::vector<char> spill(V.size(), 0);       // value must be stored because a later pass consumes it (1 byte per handle ever made)
+    std::vector<char> spill;                    // value must be stored because a later pass consumes it
+    auto pass_outputs = [&](const Pass& P) {
+        int outs = 0;
+        for (int k : P.nodes) outs += (N[k].kind != NK_MAP) || materialises(N[k]) || spill[N[k].out];
+        return outs;
+    };
+    static const int reserves[] = {0, 2, 4, 6, 7};
+    for (int attempt = 0;; ++attempt) {
+    if (attempt == 5) { unfused = true; c->flags |= SG_FLAG_UNFUSED; }
+    const int out_limit = SG_MAX_OUT - reserves[attempt < 5 ? attempt : 0];
+    passes.clear();
+    spill.assign(V.size(), 0);
+    for (Node& n : N) if (!n.done) n.pass = -1;
     for (size_t i = 0; i < N.size(); ++i) {
         Node& X = N[i];
         if (X.done || !X.needed) continue;
@@ -173,9 +190,7 @@ sg_status flush_body(sg_ctx* c, int* executed, ExitGroups* exit_groups) {
             if (X.kind == NK_FILTER && (P.has_filter || P.has_store || X.is2d)) return false;
             if (stores && P.has_filter) return false;
             if ((int)P.nodes.size() + 1 > SG_MAX_INSTR) return false;
-            int outs = 0;
-            for (int k : P.nodes) outs += (N[k].kind != NK_MAP) || materialises(N[k]) || spill[N[k].out];
-            if (outs + 1 > SG_MAX_OUT) return false;
+            if (pass_outputs(P) + 1 > out_limit) return false;
             return true;
         };
         int p = -1;
@@ -206,6 +221,10 @@ sg_status flush_body(sg_ctx* c, int* executed, ExitGroups* exit_groups) {
                 if (passes[N[y].pass].has_filter) return sg_fail(c, SG_ERR_UNSUPPORTED, "a filter pass cannot materialise an intermediate");
                 passes[N[y].pass].has_store = true;
             }
+    }
+    bool fits = true;
+    for (const Pass& P : passes) fits = fits && pass_outputs(P) <= SG_MAX_OUT;
+    if (fits || attempt >= 5) break;
     }
     if (passes.size() > 16) return sg_fail(c, SG_ERR_CAPACITY, "more than 16 passes in one flush");
 

@@ -516,12 +516,14 @@ def test_an_input_never_shares_a_register_with_an_earlier_temporary():
     for seed in range(200):
         rng = np.random.default_rng(5000 + seed)
         dtype = R.DTYPES[seed % 4]
-        n_inputs = int(rng.integers(1, 4))
-        inputs = [R.make_input(rng, dtype, 64) for _ in range(n_inputs)]
-        steps, keep, reds = R.build_dag(rng, dtype, n_inputs)
+        inputs = [R.make_input(rng, dtype, 64) for _ in range(int(rng.integers(1, 4)))]
+        steps, keep, reds, _, _, filt = R.build_dag(rng, dtype, inputs)
         c = PlanOnly()
         try:
-            _, _, stats = R.run_gpu(c, steps, keep, reds, inputs, dtype)
+            # every DAG plans: a pass that a later spill would overfill (more than SG_MAX_OUT outputs) is re-planned with outputs held
+            # in reserve — seeds 16, 42, 53, 77, ... failed with SG_ERR_CAPACITY "too many outputs in one pass" before
+            _, _, stats, _ = R.run_gpu(c, steps, keep, reds, inputs, dtype, filt)
+            assert 1 <= stats.n_passes <= 16
             for p in range(stats.n_passes):
                 d = sg.sg_plan_dump(c.ctx, p)
                 assert _input_registers_are_never_written(d), (seed, d)
