@@ -280,6 +280,13 @@ static sg_status append_map(sg_ctx* c, uint8_t op, int n_opd, const Operand* opd
         Value old = *d;
         old.user_refs = 0;                      // the previous contents stay reachable for already-enqueued readers
         old.owned = false;                      // the handle keeps owning the storage
+        if (d->node >= 0 && !c->nodes[d->node].done) {
+            // the previous contents are themselves a PENDING in-place result that this operation supersedes: that value never reaches
+            // the buffer (a dead store) and lives on as an anonymous intermediate.  It must not keep the buffer's address: if a later
+            // pass reads it, it is spilled to storage of its own — spilled into the buffer it would be overwritten by the new result
+            old.ptr = nullptr;
+            old.materialised = false;
+        }
         const int old_id = hidx(new_value(c, old));
         d = val(c, dst);
         for (int i = 0; i < n_opd; ++i)         // this operation itself reads the previous contents

@@ -187,6 +187,27 @@ def test_input_first_named_after_two_temporaries_died(dtype, n):
     assert bits_equal(np.array([got_m], dtype=dtype), np.array([orc.max(want)], dtype=dtype))
 
 
+@pytest.mark.parametrize("mode", ["template", "unfused"])
+@pytest.mark.parametrize("n", [1, 1025, 70001])
+def test_superseded_inplace_result_read_by_a_later_pass(mode, n):
+    """x := a + b (in place), t = x + max(b) (a scalar edge: t lives in a later pass and reads the FIRST version of x), x := max(a, b)
+    (in place again: supersedes the first version, which never reaches the buffer), u = t * x.  The first version is spilled to
+    storage of its own — round 2 spilled it into x's buffer, where the second version overwrote it before the later pass read it."""
+    a, b, x0 = rand(np.float64, n), rand(np.float64, n), rand(np.float64, n)
+    with Ctx(MODES[mode]) as c:
+        ha, hb, hx = c.vec(a), c.vec(b), c.vec(x0)
+        sg.sg_enqueue(c.ctx, sg.SG_ADD, [ha, hb], dst_or_0=hx)
+        s = sg.sg_reduce(c.ctx, hb, sg.SG_RMAX)
+        t = sg.sg_enqueue(c.ctx, sg.SG_ADD, [hx, s])
+        sg.sg_enqueue(c.ctx, sg.SG_MAX, [ha, hb], dst_or_0=hx)
+        u = sg.sg_enqueue(c.ctx, sg.SG_MUL, [t, hx])
+        sg.sg_release(c.ctx, t)
+        got_u, got_x = c.read_vec(u, np.float64), c.read_vec(hx, np.float64)
+    v1, v2 = orc.zip("add", a, b), orc.zip("max", a, b)
+    want_u = orc.zip("mul", orc.scalar("add", v1, float(orc.max(b))), v2)
+    assert bits_equal(got_x, v2) and bits_equal(got_u, want_u)
+
+
 @pytest.mark.parametrize("dtype,tol", [(np.float32, 1e-5), (np.float64, 1e-12), (np.int32, 0), (np.int64, 0)])
 @pytest.mark.parametrize("n", [1, 2, 33, 1024, 1025, 70001])
 def test_reductions_all_dtypes(dtype, tol, n):
