@@ -201,7 +201,9 @@ sg_status sg_flush(sg_ctx* ctx);
  * decided (a for_all already false or an exists already true on the prefix read so far IS decided and readable). */
 sg_status sg_scalar_get(sg_ctx* ctx, sg_handle s, void* host_out, size_t bytes);
 sg_status sg_scalar_dtype(sg_ctx* ctx, sg_handle s, int32_t* dtype);
-/* Trigger (2): count / device pointer of a collection; flushes (and syncs, for a filter output) if pending. */
+/* Trigger (2): count / device pointer of a collection; flushes (and syncs, for a filter output) if the collection is pending — or if
+ * a pending in-place result lives in the same storage under ANOTHER handle (a subset / row view of it, the collection it is a view of):
+ * handles that share storage behave like eager execution in program order. */
 sg_status sg_vec_count(sg_ctx* ctx, sg_handle v, int64_t* n);
 sg_status sg_vec_data(sg_ctx* ctx, sg_handle v, void** dev_ptr);
 /* to_array (PAPER.md:153-155, 195, 284 trigger (2)): flushes if pending, waits, copies the collection's elements

@@ -276,6 +276,72 @@ static sg_status append_map(sg_ctx* c, uint8_t op, int n_opd, const Operand* opd
         if (d->dtype != out_dtype) return sg_fail(c, SG_ERR_DTYPE, "dst dtype differs from the result dtype");
         if (d->rows != rows || d->cols != cols || (d->kind == VK_MAT) != is2d) return sg_fail(c, SG_ERR_SHAPE, "dst shape differs from the result shape");
         if (d->stride != 1) return sg_fail(c, SG_ERR_UNSUPPORTED, "strided dst");
+        // Aliases.  ANOTHER handle whose pending in-place result lives in storage this operation overwrites (the same view created twice,
+        // an overlapping subset, the whole vector and a slice of it) keeps naming that storage: read after this point it must give
+        // what the memory holds once the writes have landed in program order — not its own pending result, which this operation is
+        // about to overwrite (in part).  Its pending result lives on as an anonymous version (still written to the buffer by its
+        // producer, still read by the operations enqueued so far); the handle itself goes back to being plain memory, so later
+        // readers are ordered behind both writers by the plan builder's RAW edges.
+        {
+            const auto span = [](const Value& v, const char** lo, const char** hi) {
+                const int64_t es = dtype_size(v.dtype);
+                *lo = v.ptr;
+                *hi = v.kind == VK_MAT ? v.ptr + ((v.rows > 0 ? (v.rows - 1) * v.ld : 0) + v.cols) * es
+                                       : v.ptr + ((v.cols > 0 ? (v.cols - 1) * v.stride : 0) + 1) * es;
+            };
+            const char *dlo, *dhi;
+            span(*d, &dlo, &dhi);
+            const size_t n_live = c->live.size();
+            for (size_t li = 0; li < n_live; ++li) {
+                const int ai = c->live[li];
+                if (ai == hidx(dst)) continue;
+                const Value& A = c->values[ai];
+                if (!A.alive || A.kind == VK_SCALAR || !A.ptr || A.node < 0 || c->nodes[A.node].done) continue;
+                if (!c->nodes[A.node].inplace || c->nodes[A.node].out != ai) continue;
+                const char *alo, *ahi;
+                span(A, &alo, &ahi);
+                if (!(alo < dhi && dlo < ahi)) continue;
+                Value prev = A;
+                prev.user_refs = 0;
+                prev.owned = false;
+                const int prev_id = hidx(new_value(c, prev));       // may move the table: no reference into it is held here
+                for (auto& n : c->nodes)
+                    if (!n.done)
+                        for (int i = 0; i < n.n_opd; ++i)
+                            if (n.opd[i].kind != OPD_IMM && n.opd[i].value == ai) n.opd[i].value = prev_id;
+                for (int i = 0; i < n_opd; ++i)                      // this operation reads it as it is now: the pending result
+                    if (nd.opd[i].kind != OPD_IMM && nd.opd[i].value == ai) nd.opd[i].value = prev_id;
+                c->nodes[c->values[ai].node].out = prev_id;
+                c->values[ai].node = -1;
+            }
+            d = val(c, dst);
+            // The handle's own pending in-place result is about to be superseded (its store is dropped, the value lives on in
+            // registers).  That is only sound if nobody reads the buffer in between through ANOTHER handle: such a reader — enqueued
+            // after the pending result, or this very operation — must find the pending result in memory.  Rare enough to take the
+            // simple way: run what is pending first (eager execution is always right), then enqueue this operation.
+            if (d->node >= 0 && !c->nodes[d->node].done && c->nodes[d->node].inplace) {
+                const auto reads_alias = [&](const Node& n) {
+                    for (int i = 0; i < n.n_opd; ++i) {
+                        if (n.opd[i].kind == OPD_IMM) continue;
+                        const Value& w = c->values[n.opd[i].value];
+                        if (w.kind == VK_SCALAR || !w.ptr || (w.node >= 0 && !c->nodes[w.node].done)) continue;
+                        const char *wlo, *whi;
+                        span(w, &wlo, &whi);
+                        if (wlo < dhi && dlo < whi) return true;
+                    }
+                    return false;
+                };
+                bool alias_reader = reads_alias(nd);
+                for (size_t k = (size_t)d->node + 1; k < c->nodes.size() && !alias_reader; ++k)
+                    alias_reader = !c->nodes[k].done && reads_alias(c->nodes[k]);
+                if (alias_reader) {
+                    const sg_status fs = sg_flush_impl(c);
+                    if (fs != SG_OK) return fs;
+                    d = val(c, dst);
+                    if (!d) return sg_fail(c, SG_ERR_ARG, "dst released");
+                }
+            }
+        }
         // the handle keeps naming the same storage; its value is now the pending result (SSA over buffers)
         Value old = *d;
         old.user_refs = 0;                      // the previous contents stay reachable for already-enqueued readers
@@ -731,12 +797,34 @@ sg_status sg_vec_count(sg_ctx* c, sg_handle h, int64_t* n) {
     return SG_OK;
 }
 
+// does a pending in-place operation write storage that `v` names (through another handle: a view of it, the vector it is a view of)?
+static bool pending_writer_overlaps(const sg_ctx* c, const Value& v) {
+    if (!v.ptr || v.kind == VK_SCALAR) return false;
+    const auto span = [](const Value& x, const char** lo, const char** hi) {
+        const int64_t es = dtype_size(x.dtype);
+        *lo = x.ptr;
+        *hi = x.kind == VK_MAT ? x.ptr + ((x.rows > 0 ? (x.rows - 1) * x.ld : 0) + x.cols) * es : x.ptr + ((x.cols > 0 ? (x.cols - 1) * x.stride : 0) + 1) * es;
+    };
+    const char *vlo, *vhi;
+    span(v, &vlo, &vhi);
+    for (const Node& n : c->nodes) {
+        if (n.done || !n.inplace || n.out < 0) continue;
+        const Value& w = c->values[n.out];
+        if (!w.ptr || w.kind == VK_SCALAR) continue;
+        const char *wlo, *whi;
+        span(w, &wlo, &whi);
+        if (wlo < vhi && vlo < whi) return true;
+    }
+    return false;
+}
+
 sg_status sg_vec_data(sg_ctx* c, sg_handle h, void** dev_ptr) {
     SgDeviceScope dev_scope(c);
     CK(c && dev_ptr);
     Value* v = val(c, h);
     if (!v) return sg_fail(c, SG_ERR_ARG, "unknown handle");
-    if (v->node >= 0 || !v->materialised) { sg_status s = sg_flush_impl(c); if (s != SG_OK && s != SG_ERR_CONTRACT) return s; v = val(c, h); }
+    // trigger (2): the collection's own pending result, or a pending in-place result in the same storage under another handle
+    if (v->node >= 0 || !v->materialised || pending_writer_overlaps(c, *v)) { sg_status s = sg_flush_impl(c); if (s != SG_OK && s != SG_ERR_CONTRACT) return s; v = val(c, h); }
     if (!v->materialised) return sg_fail(c, SG_ERR_ARG, "collection has no storage");
     *dev_ptr = v->ptr;
     return SG_OK;

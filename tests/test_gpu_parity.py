@@ -208,6 +208,43 @@ def test_superseded_inplace_result_read_by_a_later_pass(mode, n):
     assert bits_equal(got_x, v2) and bits_equal(got_u, want_u)
 
 
+@pytest.mark.parametrize("mode", ["template", "unfused"])
+@pytest.mark.parametrize("pattern", ["read_through_a_handle_after_an_alias_wrote", "alias_read_between_two_inplace_results", "alias_read_by_the_superseding_operation"])
+def test_aliasing_handles_follow_program_order(mode, pattern):
+    """Two handles of the SAME storage (subset views) with in-place updates through both: the pending list must behave
+    like eager execution in program order.  (The randomised view programs of tests/test_gpu_random_chains.py found all three.)"""
+    n, s, L = 5000, 1000, 3000
+    x = RNG.standard_normal(n)
+    mem = x.copy()
+    with Ctx(MODES[mode]) as c:
+        hx = c.vec(x)
+        v0, v1 = sg.sg_vec_subset(c.ctx, hx, s, s + L), sg.sg_vec_subset(c.ctx, hx, s, s + L)
+        cur = lambda: mem[s:s + L].copy()
+        if pattern == "read_through_a_handle_after_an_alias_wrote":
+            sg.sg_enqueue(c.ctx, sg.SG_ADD, [v0, v1], dst_or_0=v0)                  # v0 := v0 + v1
+            mem[s:s + L] = orc.zip("add", cur(), cur())
+            sg.sg_enqueue(c.ctx, sg.SG_MUL, [sg.F(0.25), v1], dst_or_0=v1)          # v1 := 0.25 * v1   (the same memory)
+            mem[s:s + L] = orc.scalar("mul", cur(), 0.25, reversed=True)
+            t = sg.sg_enqueue(c.ctx, sg.SG_SUB, [sg.F(-1.0), v0])                   # reads v0: what the memory holds NOW
+            want_t = orc.scalar("sub", cur(), -1.0, reversed=True)
+        elif pattern == "alias_read_between_two_inplace_results":
+            sg.sg_enqueue(c.ctx, sg.SG_MUL, [v0, sg.F(3.0)], dst_or_0=v0)           # v0 := 3 v0
+            mem[s:s + L] = orc.scalar("mul", cur(), 3.0)
+            t = sg.sg_enqueue(c.ctx, sg.SG_ADD, [v1, v1])                           # reads the alias: must see 3 v0 in memory
+            want_t = orc.zip("add", cur(), cur())
+            sg.sg_enqueue(c.ctx, sg.SG_SUB, [t, sg.F(1.0)], dst_or_0=v0)            # v0 := t - 1: supersedes the first result
+            mem[s:s + L] = orc.scalar("sub", want_t, 1.0)
+        else:
+            sg.sg_enqueue(c.ctx, sg.SG_MUL, [v1, v0], dst_or_0=v0)                  # v0 := v1 * v0
+            mem[s:s + L] = orc.zip("mul", cur(), cur())
+            sg.sg_enqueue(c.ctx, sg.SG_MIN, [v1, v0], dst_or_0=v0)                  # v0 := min(v1, v0): v1 is the squared memory
+            mem[s:s + L] = orc.zip("min", cur(), cur())
+            t = sg.sg_enqueue(c.ctx, sg.SG_NEG, [v1])
+            want_t = orc.unary("neg", cur())
+        got_t, got_x = c.read_vec(t, np.float64), c.read_vec(hx, np.float64)
+    assert bits_equal(got_x, mem) and bits_equal(got_t, want_t)
+
+
 @pytest.mark.parametrize("dtype,tol", [(np.float32, 1e-5), (np.float64, 1e-12), (np.int32, 0), (np.int64, 0)])
 @pytest.mark.parametrize("n", [1, 2, 33, 1024, 1025, 70001])
 def test_reductions_all_dtypes(dtype, tol, n):

@@ -265,3 +265,303 @@ def test_random_chains_match_the_oracle(seed):
     for (kind, _, _), a, b in zip(reds, results["fused"], results.get("unfused", results["fused"])):
         if kind != "sum" or np.dtype(dtype).kind != "f":
             assert a == b or (a != a and b != b), (seed, kind, a, b)
+
+
+# ----------------------------------------------------------------------------------------------------------------------------------
+# the same on the matrix domain: ROW-/COL-broadcast vector operands, per-row / per-column / whole-matrix
+# reductions, in-place results, padded leading dimensions, odd shapes — the 2-D plan builder and pass2d_bytecode
+# ----------------------------------------------------------------------------------------------------------------------------------
+SHAPES = [(1, 1), (3, 5), (33, 65), (64, 130), (130, 257), (7, 1027), (257, 3)]
+AXES = {"all": sg.SG_AXIS_ALL, "rows": sg.SG_AXIS_ROWS, "cols": sg.SG_AXIS_COLS}
+
+
+def _ew(fn, *arrays):
+    """An elementwise oracle primitive applied to matrices: the oracle sees the flattened elements, numpy only moves data."""
+    shape = arrays[0].shape
+    return fn(*[np.ascontiguousarray(a).reshape(-1) for a in arrays]).reshape(shape)
+
+
+def _axis_reduce(fn, M, axis):
+    if axis == "all":
+        return fn(np.ascontiguousarray(M).reshape(-1))
+    if axis == "rows":
+        return [fn(np.ascontiguousarray(M[r])) for r in range(M.shape[0])]
+    return [fn(np.ascontiguousarray(M[:, cc])) for cc in range(M.shape[1])]
+
+
+def build_matrix_dag(rng, dtype, mats, v, w):
+    """Like build_dag on rows x cols values.  Operands of a binary step: ("m", id) a matrix value, ("row",) the ROW-broadcast vector v,
+    ("col",) the COL-broadcast vector w, ("imm", x), or ("axis", kind, axis, id): an exact per-row / per-column reduction of a matrix
+    value, pending in the same flush, broadcast back along the other axis."""
+    is_f = np.dtype(dtype).kind == "f"
+    shape = mats[0].shape
+    want = dict(enumerate(mats))
+    n_in = len(mats)
+    vals, bools, steps, reds = list(range(n_in)), [], [], []
+    storage = set(range(n_in))
+    nid = n_in
+
+    def operand():
+        q = rng.random()
+        if q < 0.50:
+            k = int(rng.choice(vals))
+            return ("m", k), want[k]
+        if q < 0.65:
+            return ("row",), np.ascontiguousarray(np.broadcast_to(v, shape))
+        if q < 0.80:
+            return ("col",), np.ascontiguousarray(np.broadcast_to(w[:, None], shape))
+        if q < 0.90:
+            k = int(rng.choice(vals))
+            if not (is_f and np.isnan(want[k]).any()):
+                kind = str(rng.choice(["max", "min"] + (["sum"] if np.dtype(dtype) == np.dtype(np.int64) else [])))
+                axis = str(rng.choice(["rows", "cols"]))
+                vec = np.array(_axis_reduce({"max": orc.max, "min": orc.min, "sum": orc.sum}[kind], want[k], axis), dtype=dtype)
+                full = np.broadcast_to(vec[:, None], shape) if axis == "rows" else np.broadcast_to(vec, shape)
+                return ("axis", kind, axis, k), np.ascontiguousarray(full)
+        imm = float(rng.choice([0.5, 2.0, -3.25, 7.0])) if is_f else int(rng.choice([2, 3, 7, -5, 1]))
+        return ("imm", imm), imm
+
+    for _ in range(int(rng.integers(3, 11))):
+        r = rng.random()
+        if r < 0.50 or not (bools or r < 0.85):
+            op = str(rng.choice(list(BIN) if not is_f else [k for k in BIN if k != "mod"]))
+            a = int(rng.choice(vals))
+            (bk, bv), swap = operand(), bool(rng.random() < 0.3)
+            if bk[0] == "imm":
+                res = _ew(lambda x: orc.scalar(op, x, bv, reversed=swap), want[a])
+            else:
+                res = _ew(lambda x, y: orc.zip(op, y, x) if swap else orc.zip(op, x, y), want[a], bv)
+            if rng.random() < 0.12:
+                k = int(rng.choice(sorted(storage)))
+                steps.append(("inplace", op, a, bk, swap, k, nid))
+                vals.remove(k); storage.discard(k); storage.add(nid)
+            else:
+                steps.append(("bin", op, a, bk, swap, nid))
+            want[nid] = res
+            vals.append(nid)
+        elif r < 0.62:
+            op = str(rng.choice(["neg", "abs"] + (["sqrt"] if is_f else [])))
+            a = int(rng.choice(vals))
+            steps.append(("un", op, a, nid))
+            want[nid] = _ew(lambda x: orc.unary(op, x), want[a])
+            vals.append(nid)
+        elif r < 0.85:
+            op = str(rng.choice(list(CMP)))
+            a = int(rng.choice(vals))
+            bk, bv = operand()
+            steps.append(("cmp", op, a, bk, nid))
+            want[nid] = _ew(lambda x: orc.cmp_scalar(op, x, bv), want[a]) if bk[0] == "imm" else _ew(lambda x, y: orc.cmp(op, x, y), want[a], bv)
+            bools.append(nid)
+        else:
+            op = str(rng.choice(list(LOGIC)))
+            a = int(rng.choice(bools))
+            b = int(rng.choice(bools)) if op != "not" else -1
+            steps.append(("logic", op, a, b, nid))
+            want[nid] = _ew(lambda x, y: orc.logic(op, x, y), want[a], want[b]) if b >= 0 else _ew(lambda x: orc.logic(op, x), want[a])
+            bools.append(nid)
+        nid += 1
+    produced_v = [k for k in vals if k >= n_in and k not in storage]
+    keep = set(int(x) for x in rng.choice(produced_v, min(len(produced_v), int(rng.integers(0, 3))), replace=False)) if produced_v else set()
+    if bools and rng.random() < 0.3:
+        keep.add(int(rng.choice(bools)))
+    for _ in range(int(rng.integers(1, 4))):
+        reds.append((str(rng.choice(["sum", "max", "min"])), str(rng.choice(list(AXES))), int(rng.choice(vals))))
+    for _ in range(int(rng.integers(0, 3))):
+        if bools:
+            reds.append(("count", str(rng.choice(list(AXES))), int(rng.choice(bools))))
+    return steps, keep, reds, want, storage
+
+
+@pytest.mark.parametrize("seed", range(160))
+def test_random_matrix_chains_match_the_oracle(seed):
+    from gpu_util import NP2SG, dev
+    rng = np.random.default_rng(9000 + seed)
+    dtype = DTYPES[seed % 4]
+    rows, cols = SHAPES[(seed // 4) % len(SHAPES)]
+    is_f = np.dtype(dtype).kind == "f"
+    sgdt = NP2SG[np.dtype(dtype)]
+    mats = [make_input(rng, dtype, rows * cols).reshape(rows, cols) for _ in range(int(rng.integers(1, 3)))]
+    v, w = make_input(rng, dtype, cols), make_input(rng, dtype, rows)
+    lds = [cols + int(rng.choice([0, 0, 1, 3])) for _ in mats]
+    steps, keep, reds, want, storage = build_matrix_dag(rng, dtype, mats, v, w)
+    tol = {np.float32: 1e-5, np.float64: 1e-12}.get(dtype, 0)
+    pad_value = dtype(7)
+    for mode, flags in (("fused", 0), ("unfused", sg.SG_FLAG_UNFUSED)):
+        with Ctx(flags) as c:
+            bufs = []
+            for M, ld in zip(mats, lds):
+                b = np.full((rows, ld), pad_value, dtype=dtype)
+                b[:, :cols] = M
+                bufs.append(dev(b))
+            tv, tw = dev(v), dev(w)
+            c.keep += bufs + [tv, tw]
+            h = {i: sg.sg_mat_create(c.ctx, sgdt, rows, cols, lds[i], bufs[i].data_ptr()) for i in range(len(mats))}
+            buf_of = {i: i for i in range(len(mats))}              # storage id -> caller buffer
+            hv, hw = sg.sg_vec_create(c.ctx, sgdt, cols, tv.data_ptr()), sg.sg_vec_create(c.ctx, sgdt, rows, tw.data_ptr())
+            imm = (lambda x: sg.F(x)) if is_f else (lambda x: sg.I(x))
+            borrowed, extra = set(h), []
+
+            def opd(bk):
+                if bk[0] == "m":
+                    return h[bk[1]]
+                if bk[0] == "row":
+                    return sg.H(hv, sg.SG_BCAST_ROW)
+                if bk[0] == "col":
+                    return sg.H(hw, sg.SG_BCAST_COL)
+                if bk[0] == "axis":
+                    red = sg.sg_reduce(c.ctx, h[bk[3]], RED[bk[1]], AXES[bk[2]])
+                    extra.append(red)
+                    return sg.H(red, sg.SG_BCAST_COL if bk[2] == "rows" else sg.SG_BCAST_ROW)
+                return imm(bk[1])
+            try:
+                for st in steps:
+                    if st[0] in ("bin", "inplace"):
+                        ops = [h[st[2]], opd(st[3])]
+                        if st[4]:
+                            ops.reverse()
+                        if st[0] == "bin":
+                            h[st[5]] = sg.sg_enqueue(c.ctx, BIN[st[1]], ops)
+                        else:
+                            h[st[6]] = sg.sg_enqueue(c.ctx, BIN[st[1]], ops, dst_or_0=h[st[5]])
+                            borrowed.add(st[6])
+                            buf_of[st[6]] = buf_of[st[5]]
+                    elif st[0] == "un":
+                        h[st[3]] = sg.sg_enqueue(c.ctx, UN[st[1]], [h[st[2]]])
+                    elif st[0] == "cmp":
+                        h[st[4]] = sg.sg_enqueue(c.ctx, CMP[st[1]], [h[st[2]], opd(st[3])])
+                    else:
+                        h[st[4]] = sg.sg_enqueue(c.ctx, LOGIC[st[1]], [h[st[2]]] + ([h[st[3]]] if st[3] >= 0 else []))
+                rh = [sg.sg_reduce(c.ctx, h[src], sg.SG_COUNT if kind == "count" else RED[kind], AXES[axis]) for kind, axis, src in reds]
+                for i, hx in h.items():
+                    if i not in borrowed and i not in keep:
+                        sg.sg_release(c.ctx, hx)
+                sg.sg_flush(c.ctx)
+            except sg.SgError as e:
+                if mode == "unfused" and e.status == sg.SG_ERR_CAPACITY:    # more than 16 passes in one flush
+                    continue
+                raise
+            for i in sorted(keep):
+                got = c.read_vec(h[i], want[i].dtype, rows * cols).reshape(rows, cols)
+                assert bits_equal(got, want[i]), (mode, seed, "kept matrix", i, steps)
+            c.torch.cuda.synchronize()
+            for i in sorted(storage):
+                full = bufs[buf_of[i]].cpu().numpy()
+                assert bits_equal(np.ascontiguousarray(full[:, :cols]), want[i]), (mode, seed, "caller matrix", i, steps)
+                assert (full[:, cols:] == pad_value).all(), (mode, seed, "padding touched", i)
+            for (kind, axis, src), r in zip(reds, rh):
+                M = want[src]
+                ctx = (mode, seed, kind, axis, steps)
+                out_dt = np.int64 if kind == "count" or (kind == "sum" and not is_f) else np.float64 if kind == "sum" else dtype
+                got = np.array([c.get(r)], dtype=out_dt) if axis == "all" else c.read_vec(r, out_dt, rows if axis == "rows" else cols)
+                if kind == "count":
+                    assert got.tolist() == np.atleast_1d(_axis_reduce(orc.count, M, axis)).tolist(), ctx
+                elif kind == "sum":
+                    ws = np.atleast_1d(_axis_reduce(orc.sum, M, axis))
+                    if not is_f:
+                        assert got.tolist() == ws.tolist(), ctx
+                    else:
+                        sabs = np.atleast_1d(_axis_reduce(lambda x: float(np.abs(x.astype(np.float64)).sum()), M, axis))
+                        for gvv, wv, sa in zip(got, ws, sabs):
+                            if np.isfinite(wv):
+                                assert rel_err(float(gvv), float(wv), sa) <= tol, (ctx, gvv, wv)
+                            else:
+                                assert (np.isnan(wv) and np.isnan(gvv)) or wv == gvv, (ctx, gvv, wv)
+                else:
+                    ext = orc.max if kind == "max" else orc.min
+                    ok = bits_equal(got, np.atleast_1d(np.array(_axis_reduce(ext, M, axis), dtype=dtype)))
+                    if not ok and is_f and np.isnan(M).any():          # the sign of a generated NaN is the hardware's (DESIGN.md R15)
+                        for sgn in (1.0, -1.0):
+                            Ms = np.where(np.isnan(M), np.copysign(np.nan, sgn), M).astype(M.dtype)
+                            ok = ok or bits_equal(got, np.atleast_1d(np.array(_axis_reduce(ext, Ms, axis), dtype=dtype)))
+                    assert ok, (ctx, got[:8])
+
+
+# ----------------------------------------------------------------------------------------------------------------------------------
+# memory hazards: random programs over OVERLAPPING views (subset, PAPER.md:129-131) of two buffers with in-place updates.  The
+# deferred list must behave like eager execution in program order (a pending reader sees the contents as of its enqueue; RAW / WAR /
+# WAW through overlapping storage order the passes, sg_plan.cpp) — the oracle IS eager execution on numpy views, one primitive at a time.
+# ----------------------------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("seed", range(200))
+def test_random_view_programs_match_eager_execution(seed):
+    from gpu_util import NP2SG, dev
+    rng = np.random.default_rng(20000 + seed)
+    dtype = [np.float64, np.int32, np.float32, np.int64][seed % 4]
+    is_f = np.dtype(dtype).kind == "f"
+    n = int([40, 3000, 70001][(seed // 4) % 3])
+    L = n // 3
+    host = [make_input(rng, dtype, n) for _ in range(2)]
+    views = []
+    for _ in range(int(rng.integers(3, 7))):
+        if views and rng.random() < 0.25:
+            views.append(views[int(rng.integers(0, len(views)))])             # the very same view again
+        else:
+            s = int(rng.integers(0, n - L + 1))
+            if rng.random() < 0.3:
+                s = s // 4 * 4                                                # some 16-byte aligned starts
+            views.append((int(rng.integers(0, 2)), s))
+    overlap = lambda p, q: p[0] == q[0] and abs(p[1] - q[1]) < L
+    imm = (lambda x: sg.F(x)) if is_f else (lambda x: sg.I(x))
+    for mode, flags in (("fused", 0), ("unfused", sg.SG_FLAG_UNFUSED)):
+        mem = [a.copy() for a in host]
+        prog_rng = np.random.default_rng(30000 + seed)                        # the same program in both modes
+        with Ctx(flags) as c:
+            bufs = [dev(a) for a in host]
+            c.keep += bufs
+            hb = [sg.sg_vec_create(c.ctx, NP2SG[np.dtype(dtype)], n, t.data_ptr()) for t in bufs]
+            hv = [sg.sg_vec_subset(c.ctx, hb[b], s, s + L) for b, s in views]
+            cur = lambda k: mem[views[k][0]][views[k][1]:views[k][1] + L].copy()
+            temps, kept, trace = [], [], []                                   # temps: (handle, eager value)
+            try:
+                for _ in range(int(prog_rng.integers(5, 13))):
+                    op = str(prog_rng.choice(["add", "sub", "mul", "max", "min"]))
+                    dst = int(prog_rng.integers(0, len(views))) if prog_rng.random() < 0.45 else -1
+
+                    def pick():
+                        q = prog_rng.random()
+                        if q < 0.2:
+                            x = float(prog_rng.choice([0.5, 2.0, -1.0])) if is_f else int(prog_rng.choice([2, 3, -1]))
+                            return imm(x), x, None
+                        if q < 0.45 and temps:
+                            t = temps[int(prog_rng.integers(0, len(temps)))]
+                            return t[0], t[1], None
+                        for _ in range(20):
+                            k = int(prog_rng.integers(0, len(views)))
+                            # an in-place result may read its destination only index-for-index: the same view, or one that does not overlap
+                            if dst < 0 or views[k] == views[dst] or not overlap(views[k], views[dst]):
+                                return hv[k], cur(k), k
+                        return hv[dst], cur(dst), dst
+                    (ha, va, _), (hb2, vb, _) = pick(), pick()
+                    if not isinstance(va, np.ndarray) and not isinstance(vb, np.ndarray):
+                        ha, va = hv[dst if dst >= 0 else 0], cur(dst if dst >= 0 else 0)     # at least one collection operand
+                    if isinstance(va, np.ndarray) and isinstance(vb, np.ndarray):
+                        res = orc.zip(op, va, vb)
+                    elif isinstance(va, np.ndarray):
+                        res = orc.scalar(op, va, vb)
+                    else:
+                        res = orc.scalar(op, vb, va, reversed=True)
+                    trace.append((op, dst))
+                    if dst >= 0:
+                        sg.sg_enqueue(c.ctx, BIN[op], [ha, hb2], dst_or_0=hv[dst])
+                        b, s = views[dst]
+                        mem[b][s:s + L] = res
+                    else:
+                        temps.append((sg.sg_enqueue(c.ctx, BIN[op], [ha, hb2]), res))
+                for t in temps:
+                    if prog_rng.random() < 0.5:
+                        kept.append(t)
+                    else:
+                        sg.sg_release(c.ctx, t[0])
+                red = [(sg.sg_reduce(c.ctx, hv[k], sg.SG_RMAX), sg.sg_reduce(c.ctx, hv[k], sg.SG_SUM), cur(k)) for k in range(min(2, len(views)))]
+                sg.sg_flush(c.ctx)
+            except sg.SgError as e:
+                if mode == "unfused" and e.status == sg.SG_ERR_CAPACITY:      # more than 16 passes in one flush
+                    continue
+                raise
+            for th, tv in kept:
+                assert bits_equal(c.read_vec(th, dtype), tv), (mode, seed, "kept temporary", trace, views)
+            for hm, hs, val in red:
+                assert bits_equal(np.array([c.get(hm)], dtype=dtype), np.array([orc.max(val)], dtype=dtype)), (mode, seed, "max of a view", trace, views)
+                check_sum(c.get(hs), val, 1e-12 if dtype is np.float64 else 1e-5, (mode, seed, "sum of a view"))
+            c.torch.cuda.synchronize()
+            for b in range(2):
+                assert bits_equal(bufs[b].cpu().numpy(), mem[b]), (mode, seed, "buffer", b, trace, views)
