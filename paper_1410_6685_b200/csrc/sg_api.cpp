@@ -324,7 +324,7 @@ static sg_status append_map(sg_ctx* c, uint8_t op, int n_opd, const Operand* opd
                     for (int i = 0; i < n.n_opd; ++i) {
                         if (n.opd[i].kind == OPD_IMM) continue;
                         const Value& w = c->values[n.opd[i].value];
-                        if (w.kind == VK_SCALAR || !w.ptr || (w.node >= 0 && !c->nodes[w.node].done)) continue;
+                        if (!w.ptr || (w.node >= 0 && !c->nodes[w.node].done)) continue;      // (an element view is a one-element range)
                         const char *wlo, *whi;
                         span(w, &wlo, &whi);
                         if (wlo < dhi && dlo < whi) return true;
@@ -758,12 +758,34 @@ sg_status sg_scalar_dtype(sg_ctx* c, sg_handle h, int32_t* dtype) {
     return SG_OK;
 }
 
+// does a pending in-place operation write storage that `v` names (through another handle: a view of it, the vector it is a view of)?
+static bool pending_writer_overlaps(const sg_ctx* c, const Value& v) {
+    if (!v.ptr) return false;              // (an element view, sg_mat_elem, is a one-element range)
+    const auto span = [](const Value& x, const char** lo, const char** hi) {
+        const int64_t es = dtype_size(x.dtype);
+        *lo = x.ptr;
+        *hi = x.kind == VK_MAT ? x.ptr + ((x.rows > 0 ? (x.rows - 1) * x.ld : 0) + x.cols) * es : x.ptr + ((x.cols > 0 ? (x.cols - 1) * x.stride : 0) + 1) * es;
+    };
+    const char *vlo, *vhi;
+    span(v, &vlo, &vhi);
+    for (const Node& n : c->nodes) {
+        if (n.done || !n.inplace || n.out < 0) continue;
+        const Value& w = c->values[n.out];
+        if (!w.ptr || w.kind == VK_SCALAR) continue;
+        const char *wlo, *whi;
+        span(w, &wlo, &whi);
+        if (wlo < vhi && vlo < whi) return true;
+    }
+    return false;
+}
+
 sg_status sg_scalar_get(sg_ctx* c, sg_handle h, void* host_out, size_t bytes) {
     SgDeviceScope dev_scope(c);
     CK(c && host_out);
     Value* v = val(c, h);
     if (!v || v->kind != VK_SCALAR) return sg_fail(c, SG_ERR_ARG, "not a scalar handle");
-    if (v->node >= 0) {                          // trigger (1)
+    // trigger (1), PAPER.md:284 — also for an element view (sg_mat_elem) whose matrix has a pending in-place result
+    if (v->node >= 0 || (v->slot < 0 && pending_writer_overlaps(c, *v))) {
         sg_status s = sg_flush_impl(c);
         if (s != SG_OK && s != SG_ERR_CONTRACT) return s;
         v = val(c, h);
@@ -795,27 +817,6 @@ sg_status sg_vec_count(sg_ctx* c, sg_handle h, int64_t* n) {
     }
     *n = v->rows * v->cols;     // count is a scalar contract: O(1)
     return SG_OK;
-}
-
-// does a pending in-place operation write storage that `v` names (through another handle: a view of it, the vector it is a view of)?
-static bool pending_writer_overlaps(const sg_ctx* c, const Value& v) {
-    if (!v.ptr || v.kind == VK_SCALAR) return false;
-    const auto span = [](const Value& x, const char** lo, const char** hi) {
-        const int64_t es = dtype_size(x.dtype);
-        *lo = x.ptr;
-        *hi = x.kind == VK_MAT ? x.ptr + ((x.rows > 0 ? (x.rows - 1) * x.ld : 0) + x.cols) * es : x.ptr + ((x.cols > 0 ? (x.cols - 1) * x.stride : 0) + 1) * es;
-    };
-    const char *vlo, *vhi;
-    span(v, &vlo, &vhi);
-    for (const Node& n : c->nodes) {
-        if (n.done || !n.inplace || n.out < 0) continue;
-        const Value& w = c->values[n.out];
-        if (!w.ptr || w.kind == VK_SCALAR) continue;
-        const char *wlo, *whi;
-        span(w, &wlo, &whi);
-        if (wlo < vhi && vlo < whi) return true;
-    }
-    return false;
 }
 
 sg_status sg_vec_data(sg_ctx* c, sg_handle h, void** dev_ptr) {

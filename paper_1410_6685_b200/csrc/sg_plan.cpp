@@ -120,13 +120,24 @@ sg_status flush_body(sg_ctx* c, int* executed, ExitGroups* exit_groups) {
         for (int k : P.nodes) outs += (N[k].kind != NK_MAP) || materialises(N[k]) || spill[N[k].out];
         return outs;
     };
-    static const int reserves[] = {0, 2, 4, 6, 7};
+    // The other limits of a pass (distinct inputs, registers of the evaluator, instructions) are only known once its program is built:
+    // a build that fails on one of them also repeats the assignment, with fewer operations per pass.
+    static const int reserves[] = {0, 2, 4, 6, 7}, node_limits[] = {SG_MAX_INSTR, SG_MAX_INSTR, 16, 8, 4};
+    std::vector<char*> temps;
+    const sg_stats stats0 = c->stats;
     for (int attempt = 0;; ++attempt) {
     if (attempt == 5) { unfused = true; c->flags |= SG_FLAG_UNFUSED; }
     const int out_limit = SG_MAX_OUT - reserves[attempt < 5 ? attempt : 0];
+    const int node_limit = node_limits[attempt < 5 ? attempt : 0];
     passes.clear();
     spill.assign(V.size(), 0);
-    for (Node& n : N) if (!n.done) n.pass = -1;
+    c->stats = stats0;
+    c->dumps.clear();
+    for (Node& n : N) {
+        if (n.done) continue;
+        n.pass = -1;
+        if (n.out >= 0 && V[n.out].user_refs < 0) V[n.out].user_refs = 0;       // spill marks of an abandoned attempt
+    }
     for (size_t i = 0; i < N.size(); ++i) {
         Node& X = N[i];
         if (X.done || !X.needed) continue;
@@ -189,7 +200,7 @@ sg_status flush_body(sg_ctx* c, int* executed, ExitGroups* exit_groups) {
             if (xdt >= 0 && P.dtype >= 0 && P.dtype != xdt) return false;
             if (X.kind == NK_FILTER && (P.has_filter || P.has_store || X.is2d)) return false;
             if (stores && P.has_filter) return false;
-            if ((int)P.nodes.size() + 1 > SG_MAX_INSTR) return false;
+            if ((int)P.nodes.size() + 1 > node_limit) return false;
             if (pass_outputs(P) + 1 > out_limit) return false;
             return true;
         };
@@ -224,13 +235,12 @@ sg_status flush_body(sg_ctx* c, int* executed, ExitGroups* exit_groups) {
     }
     bool fits = true;
     for (const Pass& P : passes) fits = fits && pass_outputs(P) <= SG_MAX_OUT;
-    if (fits || attempt >= 5) break;
-    }
+    if (!fits && attempt < 5) continue;
     if (passes.size() > 16) return sg_fail(c, SG_ERR_CAPACITY, "more than 16 passes in one flush");
 
     // ---- 4. programs, outputs, geometry ------------------------------------------------------------------
     // spilled intermediates become context-owned temporaries, released after the launches are queued
-    std::vector<char*> temps;
+    const auto build_all = [&]() -> sg_status {
     c->stats.n_passes = (int32_t)passes.size();
     for (const Node& n : N) c->stats.n_nodes += (!n.done && n.needed);
     std::vector<char> spill_copy = spill;
@@ -256,6 +266,13 @@ sg_status flush_body(sg_ctx* c, int* executed, ExitGroups* exit_groups) {
         }
         c->stats.bytes_min += P.bytes;
         if (P.geom.template_id > 0) c->stats.n_template++; else c->stats.n_bytecode++;
+    }
+    return SG_OK;
+    };
+    const sg_status built = build_all();
+    if (built == SG_ERR_CAPACITY && attempt < 5) continue;
+    if (built != SG_OK) return built;
+    break;
     }
 
     // ---- 5. resources and launches -----------------------------------------------------------------------

@@ -245,6 +245,26 @@ def test_aliasing_handles_follow_program_order(mode, pattern):
     assert bits_equal(got_x, mem) and bits_equal(got_t, want_t)
 
 
+def test_fourteen_vectors_in_one_expression():
+    """More distinct inputs than one pass holds (10): the chain is split into passes, the result is the oracle's."""
+    n = 70001
+    v = [rand(np.float64, n) for _ in range(14)]
+    with Ctx() as c:
+        h = [c.vec(x) for x in v]
+        acc = h[0]
+        for x in h[1:]:
+            nxt = sg.sg_enqueue(c.ctx, sg.SG_ADD, [acc, x])
+            if acc != h[0]:
+                sg.sg_release(c.ctx, acc)
+            acc = nxt
+        got = c.read_vec(acc, np.float64)
+        assert sg.sg_plan_stats(c.ctx).n_passes >= 2
+    want = v[0]
+    for x in v[1:]:
+        want = orc.zip("add", want, x)
+    assert bits_equal(got, want)
+
+
 @pytest.mark.parametrize("dtype,tol", [(np.float32, 1e-5), (np.float64, 1e-12), (np.int32, 0), (np.int64, 0)])
 @pytest.mark.parametrize("n", [1, 2, 33, 1024, 1025, 70001])
 def test_reductions_all_dtypes(dtype, tol, n):

@@ -565,3 +565,105 @@ def test_random_view_programs_match_eager_execution(seed):
             c.torch.cuda.synchronize()
             for b in range(2):
                 assert bits_equal(bufs[b].cpu().numpy(), mem[b]), (mode, seed, "buffer", b, trace, views)
+
+
+# ----------------------------------------------------------------------------------------------------------------------------------
+# Listing 5's way of working: ROW views of one matrix updated in place with other rows, immediates, element views
+# (the pivot, sg_mat_elem) and pending scalars, mixed with whole-matrix and row-block updates through other handles of the same
+# storage.  The oracle is eager execution on a numpy matrix, one primitive at a time.
+# ----------------------------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("seed", range(160))
+def test_random_row_programs_match_eager_execution(seed):
+    from gpu_util import NP2SG, dev
+    dtype = [np.float64, np.int64, np.float32, np.int32][seed % 4]
+    is_f = np.dtype(dtype).kind == "f"
+    rows, cols = [(6, 17), (9, 130), (5, 1027), (12, 64)][(seed // 4) % 4]
+    rng = np.random.default_rng(40000 + seed)
+    ld = cols + int(rng.choice([0, 0, 1, 2]))
+    pad = dtype(9)
+    host = np.full((rows, ld), pad, dtype=dtype)
+    host[:, :cols] = make_input(rng, dtype, rows * cols).reshape(rows, cols)
+    imm = (lambda x: sg.F(x)) if is_f else (lambda x: sg.I(x))
+    pick_imm = lambda r: float(r.choice([0.5, 2.0, -1.0])) if is_f else int(r.choice([2, 3, -1]))
+    for mode, flags in (("fused", 0), ("unfused", sg.SG_FLAG_UNFUSED)):
+        mem = host.copy()
+        pr = np.random.default_rng(50000 + seed)
+        trace = []
+        with Ctx(flags) as c:
+            tM = dev(host)
+            c.keep.append(tM)
+            hM = sg.sg_mat_create(c.ctx, NP2SG[np.dtype(dtype)], rows, cols, ld, tM.data_ptr())
+            rowh = {}
+
+            def row(i):
+                if i not in rowh:
+                    rowh[i] = sg.sg_mat_row(c.ctx, hM, i)
+                return rowh[i]
+            cur = lambda i: mem[i, :cols].copy()
+            temps, kept = [], []
+            try:
+                for _ in range(int(pr.integers(6, 15))):
+                    op = str(pr.choice(["add", "sub", "mul", "max", "min"]))
+                    i, j = int(pr.integers(0, rows)), int(pr.integers(0, rows))
+                    q = pr.random()
+                    if q < 0.25:                                                    # r_i := r_i op r_j
+                        sg.sg_enqueue(c.ctx, BIN[op], [row(i), row(j)], dst_or_0=row(i))
+                        mem[i, :cols] = orc.zip(op, cur(i), cur(j))
+                        trace.append(("row", op, i, j))
+                    elif q < 0.35:                                                  # r_i := imm op r_i
+                        x = pick_imm(pr)
+                        sg.sg_enqueue(c.ctx, BIN[op], [imm(x), row(i)], dst_or_0=row(i))
+                        mem[i, :cols] = orc.scalar(op, cur(i), x, reversed=True)
+                        trace.append(("row_imm", op, i, x))
+                    elif q < 0.50 and rows > 1:                                     # r_i := r_i op M[a, b], the element read where it lies NOW
+                        a = int(pr.choice([k for k in range(rows) if k != i]))
+                        b = int(pr.integers(0, cols))
+                        e = sg.sg_mat_elem(c.ctx, hM, a, b)
+                        sg.sg_enqueue(c.ctx, BIN[op], [row(i), e], dst_or_0=row(i))
+                        mem[i, :cols] = orc.scalar(op, cur(i), mem[a, b].item())
+                        sg.sg_release(c.ctx, e)
+                        trace.append(("row_elem", op, i, a, b))
+                    elif q < 0.62:                                                  # r_j := r_j op max(r_i): a pending scalar
+                        s = sg.sg_reduce(c.ctx, row(i), sg.SG_RMAX)
+                        sval = orc.max(cur(i))
+                        sg.sg_enqueue(c.ctx, BIN[op], [row(j), s], dst_or_0=row(j))
+                        mem[j, :cols] = orc.scalar(op, cur(j), float(sval) if is_f else int(sval))
+                        sg.sg_release(c.ctx, s)
+                        trace.append(("row_max", op, j, i))
+                    elif q < 0.74:                                                  # t = r_i op r_j
+                        temps.append((sg.sg_enqueue(c.ctx, BIN[op], [row(i), row(j)]), orc.zip(op, cur(i), cur(j))))
+                        trace.append(("temp", op, i, j))
+                    elif q < 0.84 and temps:                                        # r_i := t op r_i
+                        t = temps[int(pr.integers(0, len(temps)))]
+                        sg.sg_enqueue(c.ctx, BIN[op], [t[0], row(i)], dst_or_0=row(i))
+                        mem[i, :cols] = orc.zip(op, t[1], cur(i))
+                        trace.append(("row_temp", op, i))
+                    elif q < 0.92:                                                  # M := M op imm, through the matrix handle
+                        x = pick_imm(pr)
+                        sg.sg_enqueue(c.ctx, BIN[op], [hM, imm(x)], dst_or_0=hM)
+                        mem[:, :cols] = orc.scalar(op, np.ascontiguousarray(mem[:, :cols]).reshape(-1), x).reshape(rows, cols)
+                        trace.append(("mat_imm", op, x))
+                    elif rows > 2:                                                  # B := B op r_k along the rows of a row block, k outside it
+                        r0 = int(pr.integers(0, rows - 1))
+                        r1 = int(pr.integers(r0 + 1, rows))
+                        k = int(pr.choice([k for k in range(rows) if k < r0 or k >= r1]))
+                        hB = sg.sg_mat_rows(c.ctx, hM, r0, r1)
+                        sg.sg_enqueue(c.ctx, BIN[op], [hB, sg.H(row(k), sg.SG_BCAST_ROW)], dst_or_0=hB)
+                        blk = np.ascontiguousarray(mem[r0:r1, :cols])
+                        mem[r0:r1, :cols] = orc.zip(op, blk.reshape(-1), np.ascontiguousarray(np.broadcast_to(cur(k), blk.shape)).reshape(-1)).reshape(blk.shape)
+                        sg.sg_release(c.ctx, hB)
+                        trace.append(("block", op, r0, r1, k))
+                for t in temps:
+                    if pr.random() < 0.6:
+                        kept.append(t)
+                    else:
+                        sg.sg_release(c.ctx, t[0])
+                sg.sg_flush(c.ctx)
+            except sg.SgError as e:
+                if mode == "unfused" and e.status == sg.SG_ERR_CAPACITY:            # more than 16 passes in one flush
+                    continue
+                raise
+            for th, tv in kept:
+                assert bits_equal(c.read_vec(th, dtype), tv), (mode, seed, "kept temporary", trace)
+            c.torch.cuda.synchronize()
+            assert bits_equal(tM.cpu().numpy(), mem), (mode, seed, "matrix", trace)

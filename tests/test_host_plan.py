@@ -534,6 +534,38 @@ def test_an_input_never_shares_a_register_with_an_earlier_temporary():
     assert len(progs) >= 50 and all(_input_registers_are_never_written(pr) for pr in progs)
 
 
+def test_chains_beyond_the_limits_of_one_pass_are_split_not_rejected():
+    """A pass holds at most 10 distinct inputs, 8 outputs, 32 operations and the evaluator's registers.  A chain that needs more is
+    planned as several passes (the assignment repeats with fewer operations per pass; round 2 failed such a flush with SG_ERR_CAPACITY)."""
+    def many_inputs(ctx):                       # v0 + v1 + ... + v13: fourteen distinct vectors in one expression
+        v = [sg.sg_vec_create(ctx, sg.SG_F64, 4096, None) for _ in range(14)]
+        acc = v[0]
+        for x in v[1:]:
+            nxt = sg.sg_enqueue(ctx, sg.SG_ADD, [acc, x])
+            if acc != v[0]:
+                sg.sg_release(ctx, acc)
+            acc = nxt
+        return acc
+    st, dumps = plan(many_inputs)
+    assert 2 <= st.n_passes <= 4 and st.n_nodes == 13
+    assert all(len(re.findall(r"\{IN_", d)) <= 10 for d in dumps)
+
+    def many_registers(ctx):                    # thirteen temporaries a + i alive at once, each with its own immediate
+        a = sg.sg_vec_create(ctx, sg.SG_F32, 4096, None)
+        t = [sg.sg_enqueue(ctx, sg.SG_ADD, [a, sg.F(float(i))]) for i in range(13)]
+        acc = t[0]
+        for x in t[1:]:
+            nxt = sg.sg_enqueue(ctx, sg.SG_MUL, [acc, x])
+            if acc != t[0]:
+                sg.sg_release(ctx, acc)
+            acc = nxt
+        for x in t:
+            sg.sg_release(ctx, x)
+        return acc
+    st, dumps = plan(many_registers)
+    assert st.n_passes >= 2 and st.n_nodes == 25
+
+
 def test_a_failed_flush_discards_the_pending_list_and_leaves_the_context_usable():
     ctx = sg.sg_ctx_create(-1)
     try:
