@@ -667,3 +667,150 @@ def test_random_row_programs_match_eager_execution(seed):
                 assert bits_equal(c.read_vec(th, dtype), tv), (mode, seed, "kept temporary", trace)
             c.torch.cuda.synchronize()
             assert bits_equal(tM.cpu().numpy(), mem), (mode, seed, "matrix", trace)
+
+
+# ----------------------------------------------------------------------------------------------------------------------------------
+# dtype-changing projections (R23): random programs that convert between the four element
+# types (sg_cast, integer sqrt -> DOUBLE), compute in each type, and convert again — on misaligned subset views, into caller buffers,
+# with reductions.  Every conversion is a pass boundary with a converting load (IN_VEC_CVT) of a stored operand.
+# ----------------------------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("seed", range(160))
+def test_random_cast_programs_match_the_oracle(seed):
+    from gpu_util import NP2SG, dev
+    rng = np.random.default_rng(60000 + seed)
+    n = int([40, 3000, 70001][(seed // 4) % 3])
+    L = n // 2
+    base_dt = DTYPES[seed % 4]
+    host = make_input(rng, base_dt, n)
+    if np.dtype(base_dt).kind == "f":                        # values outside the integer ranges, halves, NaN and infinities: the conversion's edge cases
+        host[rng.integers(0, n, max(1, n // 25))] = rng.choice(np.array([2.5, -2.5, 3e9, -3e9, 1e19, -1e19, 16777217.0, np.nan, np.inf, -np.inf], dtype=base_dt))
+    else:
+        host[rng.integers(0, n, max(1, n // 25))] = rng.choice(np.array([16777217, -16777217, 2147483647, -2147483648, 123456789], dtype=base_dt))
+    starts = [int(rng.integers(0, n - L + 1)) for _ in range(2)]
+    for mode, flags in (("fused", 0), ("unfused", sg.SG_FLAG_UNFUSED)):
+        pr = np.random.default_rng(70000 + seed)
+        with Ctx(flags) as c:
+            tb = dev(host)
+            c.keep.append(tb)
+            hb = sg.sg_vec_create(c.ctx, NP2SG[np.dtype(base_dt)], n, tb.data_ptr())
+            vals = [(sg.sg_vec_subset(c.ctx, hb, s, s + L), host[s:s + L].copy()) for s in starts]      # (handle, oracle value)
+            borrowed = len(vals)
+            outs, trace = [], []                                 # caller buffers written by converting in place: (tensor, want)
+            try:
+                for _ in range(int(pr.integers(4, 11))):
+                    h, v = vals[int(pr.integers(0, len(vals)))]
+                    q = pr.random()
+                    if q < 0.45:                                 # convert to another element type (sometimes straight into a caller buffer)
+                        to = DTYPES[int(pr.integers(0, 4))]
+                        w = orc.cast(v, to)
+                        if pr.random() < 0.25:
+                            off = int(pr.integers(0, 4))
+                            t = dev(np.zeros(L + 8, dtype=to))
+                            c.keep.append(t)
+                            hd = sg.sg_vec_subset(c.ctx, sg.sg_vec_create(c.ctx, NP2SG[np.dtype(to)], L + 8, t.data_ptr()), off, off + L)
+                            vals.append((sg.sg_cast(c.ctx, h, NP2SG[np.dtype(to)], hd), w))
+                            outs.append((t, off, w))
+                        else:
+                            vals.append((sg.sg_cast(c.ctx, h, NP2SG[np.dtype(to)]), w))
+                        trace.append(("cast", v.dtype.name, np.dtype(to).name))
+                    elif q < 0.60:                               # sqrt: an integer vector gives doubles (the paper's example)
+                        vals.append((sg.sg_enqueue(c.ctx, sg.SG_SQRT, [h]), orc.project_sqrt(v)))
+                        trace.append(("sqrt", v.dtype.name))
+                    else:                                        # an operation inside one element type
+                        same = [k for k, (_, x) in enumerate(vals) if x.dtype == v.dtype]
+                        h2, v2 = vals[int(pr.choice(same))]
+                        op = str(pr.choice(["add", "sub", "mul", "max", "min"]))
+                        vals.append((sg.sg_enqueue(c.ctx, BIN[op], [h, h2]), orc.zip(op, v, v2)))
+                        trace.append((op, v.dtype.name))
+                keep = [k for k in range(borrowed, len(vals)) if pr.random() < 0.5]
+                red = [(sg.sg_reduce(c.ctx, vals[k][0], sg.SG_RMAX), sg.sg_reduce(c.ctx, vals[k][0], sg.SG_SUM), vals[k][1])
+                       for k in pr.choice(len(vals), min(2, len(vals)), replace=False)]
+                for k in range(borrowed, len(vals)):
+                    if k not in keep and not any(vals[k][1] is w for _, _, w in outs):
+                        sg.sg_release(c.ctx, vals[k][0])
+                sg.sg_flush(c.ctx)
+            except sg.SgError as e:
+                if mode == "unfused" and e.status == sg.SG_ERR_CAPACITY:        # more than 16 passes in one flush
+                    continue
+                raise
+            for k in keep:
+                assert bits_equal(c.read_vec(vals[k][0], vals[k][1].dtype), vals[k][1]), (mode, seed, "kept value", k, trace)
+            for hm, hs, v in red:
+                cands = [orc.max(v)]
+                if v.dtype.kind == "f" and np.isnan(v).any():
+                    cands = [orc.max(np.where(np.isnan(v), np.copysign(np.nan, sgn), v).astype(v.dtype)) for sgn in (1.0, -1.0)]
+                got = np.array([c.get(hm)], dtype=v.dtype)
+                assert any(bits_equal(got, np.array([w], dtype=v.dtype)) for w in cands), (mode, seed, "max", got, cands, trace)
+                check_sum(c.get(hs), v, 1e-12 if v.dtype == np.float64 else 1e-5, (mode, seed, "sum", trace))
+            c.torch.cuda.synchronize()
+            for t, off, w in outs:
+                full = t.cpu().numpy()
+                assert bits_equal(full[off:off + L], w) and not full[:off].any() and not full[off + L:].any(), (mode, seed, "caller buffer", trace)
+            assert bits_equal(tb.cpu().numpy(), host), (mode, seed, "source modified")
+
+
+# ----------------------------------------------------------------------------------------------------------------------------------
+# contracts and the early exit (R19a): random sets of quantifiers over one vector, some registered as
+# PRE / POST contracts, with and without a violation and with and without SG_FLAG_NO_EARLY_EXIT, next to a reduction body.
+# Rules checked: the flush reports SG_ERR_CONTRACT exactly when a registered contract is false; a value that is handed back is the
+# oracle's; "not evaluated" is only ever the answer for a quantifier that was not yet decided when a violated contract ended its pass.
+# ----------------------------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("seed", range(200))
+def test_random_contract_sets_follow_the_rules(seed):
+    from gpu_util import NP2SG
+    rng = np.random.default_rng(80000 + seed)
+    dtype = [np.float32, np.float64, np.int32][seed % 3]
+    is_f = np.dtype(dtype).kind == "f"
+    n = int([33, 5000, 300007, (1 << 21) + 3][(seed // 3) % 4])
+    x = np.sort(rng.integers(0, 1000, n)).astype(dtype)                      # ascending, many ties, values 0 .. 999
+    if rng.random() < 0.6:                                                   # one or two planted breaks of the order / of the range
+        for _ in range(int(rng.integers(1, 3))):
+            j = int(rng.integers(0, n))
+            x[j] = dtype(rng.choice([-5, 2000, 0, 500]))
+    flags = sg.SG_FLAG_NO_EARLY_EXIT if rng.random() < 0.3 else 0
+    imm = (lambda v: sg.F(float(v))) if is_f else (lambda v: sg.I(int(v)))
+    with Ctx(flags) as c:
+        hx = c.vec(x)
+        quants = []                                                          # (handle, truth, kind, registered)
+        for _ in range(int(rng.integers(2, 6))):
+            q = rng.random()
+            if q < 0.3:
+                op = str(rng.choice(["le", "lt", "ge"]))
+                h = sg.sg_forall_adjacent(c.ctx, hx, CMP[op])
+                truth, kind = (bool(orc.all(orc.adj(op, x))) if n > 1 else True), "all"
+            else:
+                op, v = str(rng.choice(list(CMP))), int(rng.choice([-5, 0, 1, 500, 999, 1000, 2000]))
+                m = sg.sg_enqueue(c.ctx, CMP[op], [hx, imm(v)])
+                mask = orc.cmp_scalar(op, x, float(v) if is_f else v)
+                if rng.random() < 0.5:
+                    h, truth, kind = sg.sg_forall(c.ctx, m), bool(orc.all(mask)), "all"
+                else:
+                    h, truth, kind = sg.sg_exists(c.ctx, m), bool(orc.any(mask)), "any"
+                sg.sg_release(c.ctx, m)
+            reg = rng.random() < 0.5
+            if reg:
+                sg.sg_contract(c.ctx, h, sg.SG_CONTRACT_PRE if rng.random() < 0.5 else sg.SG_CONTRACT_POST, "q%d" % len(quants))
+            quants.append((h, truth, kind, reg))
+        body = sg.sg_reduce(c.ctx, hx, sg.SG_SUM) if rng.random() < 0.5 else None        # a reduction body in the same flush
+        violated = [k for k, (_, truth, _, reg) in enumerate(quants) if reg and not truth]
+        try:
+            sg.sg_flush(c.ctx)
+            raised = False
+        except sg.SgError as e:
+            assert e.status == sg.SG_ERR_CONTRACT, (seed, str(e))
+            raised = True
+        assert raised == bool(violated), (seed, "flush status", raised, violated)
+        violated_all = [k for k in violated if quants[k][2] == "all"]       # only a violated for_all contract ends a pass early
+        for k, (h, truth, kind, reg) in enumerate(quants):
+            try:
+                got = c.get(h)
+            except sg.SgError as e:
+                assert e.status == sg.SG_ERR_CONTRACT and "not evaluated" in str(e), (seed, k, str(e))
+                assert violated_all and not flags, (seed, k, "not evaluated without an early exit")
+                # an undecided quantifier reads for_all = true / exists = false so far: one that is false / true on the whole vector may
+                # still be undecided on the prefix, but a VIOLATED contract itself is decided
+                assert k not in violated_all, (seed, k, "the violated contract itself must be readable")
+                continue
+            assert got is truth, (seed, k, kind, got, truth)
+        if body is not None:
+            check_sum(c.get(body), x, 1e-12 if dtype is np.float64 else 1e-5, (seed, "body sum"))
