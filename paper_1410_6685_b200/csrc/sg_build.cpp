@@ -168,6 +168,7 @@ sg_status sg_build_pass(sg_ctx* c, Pass& P, std::vector<char*>& temps, std::stri
         if (stored(X)) pinned[X.out] = 1;
     }
     std::map<int, std::pair<int, int>> filter_regs;     // filter output value -> (values reg, mask reg)
+    std::map<int, int64_t> filter_len;                  // filter output value -> length of the filter's SOURCE (the domain of reductions over the kept values)
     int n_out = 0, n_instr = 0;
     bool only_quant = true;
 
@@ -256,7 +257,7 @@ sg_status sg_build_pass(sg_ctx* c, Pass& P, std::vector<char*>& temps, std::stri
             g.out[n_out] = {X.op, (uint8_t)it->second.first, (uint8_t)it->second.second, AXIS_ALL};
             a.out_ptr[n_out] = c->slab + 8 * V[X.out].slot;
             a.out_host[n_out] = scalar_host_slot(c, V[X.out].slot);
-            a.out_len[n_out] = X.cols;
+            a.out_len[n_out] = filter_len[X.opd[0].value];      // masked reduction over the SOURCE elements (X.cols is the output's capacity: a tight caller buffer would cut the sum short)
             only_quant = false;
             ++n_out;
             continue;
@@ -337,6 +338,7 @@ sg_status sg_build_pass(sg_ctx* c, Pass& P, std::vector<char*>& temps, std::stri
             }
             ov.materialised = true;
             filter_regs[X.out] = {r[0], r[1]};
+            filter_len[X.out] = X.cols;
             g.out[n_out] = {OUT_FILTER, (uint8_t)r[0], (uint8_t)r[1], AXIS_ALL};
             a.out_ptr[n_out] = ov.ptr;
             a.out_len[n_out] = X.cols;

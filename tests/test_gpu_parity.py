@@ -609,6 +609,28 @@ def test_filter_capacity_error():
         assert out.cpu().numpy().tolist() == list(range(10))
 
 
+@pytest.mark.parametrize("dtype", [np.float64, np.int64, np.float32])
+def test_kept_sum_with_a_tight_caller_buffer(dtype):
+    """Filter into a caller buffer of exactly the kept count, with the sum and the maximum of the kept values in the same pass (a
+    chain without a template instance: the bytecode filter kernel).  The reductions run over the SOURCE elements under the mask —
+    round 2 bounded them by the output's capacity and cut the sum short (found by the bursty-mask filter test)."""
+    n = 70001
+    x = rand(dtype, n)
+    zero = 0.0 if np.dtype(dtype).kind == "f" else 0
+    want = orc.filter(x, orc.cmp_scalar("gt", x, zero))
+    with Ctx() as c:
+        hx = c.vec(x)
+        out = dev(np.zeros(want.size, dtype=dtype))
+        c.keep.append(out)
+        m = sg.sg_enqueue(c.ctx, sg.SG_GT, [hx, sg.F(0.0) if np.dtype(dtype).kind == "f" else sg.I(0)])
+        fv, fc = sg.sg_filter(c.ctx, hx, m, out.data_ptr(), want.size)
+        sg.sg_release(c.ctx, m)
+        s, mx = sg.sg_reduce(c.ctx, fv, sg.SG_SUM), sg.sg_reduce(c.ctx, fv, sg.SG_RMAX)
+        assert c.get(fc) == want.size and bits_equal(c.read_vec(fv, dtype, want.size), want)
+        assert sum_ok(c.get(s), orc.sum(want), want, {np.float64: 1e-12, np.float32: 1e-5}.get(dtype, 0)) and dtype(c.get(mx)) == orc.max(want)
+        assert sg.sg_plan_stats(c.ctx).n_bytecode == 1
+
+
 def test_cfg2_full_size():
     n = 1 << 27
     x = inputs.uniform_i31(3, 0, n)

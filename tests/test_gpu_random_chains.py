@@ -814,3 +814,99 @@ def test_random_contract_sets_follow_the_rules(seed):
             assert got is truth, (seed, k, kind, got, truth)
         if body is not None:
             check_sum(c.get(body), x, 1e-12 if dtype is np.float64 else 1e-5, (seed, "body sum"))
+
+
+# ----------------------------------------------------------------------------------------------------------------------------------
+# the filter's protocols (look-back over tile states, runs of tiles, the compaction ring, epoch-tagged states) under BURSTY masks:
+# kept elements come in random runs (a two-state Markov chain with random switch probabilities: from almost nothing kept to long
+# stretches where everything is kept, which fill the ring and shrink the runs), several launches of different lengths per context,
+# misaligned views, all four element types, output into a caller buffer of exactly the needed capacity.
+# ----------------------------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("seed", range(120))
+def test_random_bursty_filters_match_the_oracle(seed):
+    from gpu_util import NP2SG, dev
+    rng = np.random.default_rng(90000 + seed)
+    dtype = DTYPES[seed % 4]
+    is_f = np.dtype(dtype).kind == "f"
+    with Ctx() as c:
+        for launch in range(int(rng.integers(2, 6))):
+            n = int(rng.choice([1, 100, 8191, 8192, 8193, 70001, int(rng.integers(1, 3_000_000))]))
+            p_on, p_off = 10.0 ** -rng.uniform(0.3, 4.5), 10.0 ** -rng.uniform(0.3, 4.5)
+            # run lengths of the two states are geometric: build the pattern from run lengths (fast), trim to n
+            runs, state, total = [], bool(rng.random() < 0.5), 0
+            while total < n:
+                ln = int(rng.geometric(p_off if state else p_on))
+                runs.append((state, ln)); total += ln; state = not state
+            pattern = np.concatenate([np.full(ln, st) for st, ln in runs])[:n]
+            mag = rng.integers(1, 1000, n)
+            x = np.where(pattern, mag, -mag).astype(dtype)
+            off = int(rng.integers(0, 5))
+            buf = np.zeros(n + 8, dtype=dtype)
+            buf[off:off + n] = x
+            t = dev(buf)
+            c.keep.append(t)
+            hx = sg.sg_vec_subset(c.ctx, sg.sg_vec_create(c.ctx, NP2SG[np.dtype(dtype)], n + 8, t.data_ptr()), off, off + n)
+            m = sg.sg_enqueue(c.ctx, sg.SG_GT, [hx, sg.F(0.0) if is_f else sg.I(0)])
+            want = orc.filter(x, orc.cmp_scalar("gt", x, 0.0 if is_f else 0))
+            assert want.size == int(pattern.sum())
+            if rng.random() < 0.5:                                   # into a caller buffer with exactly the capacity needed
+                to = dev(np.full(want.size + 4, 77, dtype=dtype))
+                c.keep.append(to)
+                fv, fc = sg.sg_filter(c.ctx, hx, m, to.data_ptr(), want.size)
+            else:
+                to = None
+                fv, fc = sg.sg_filter(c.ctx, hx, m)
+            sg.sg_release(c.ctx, m)
+            s, mx = sg.sg_reduce(c.ctx, fv, sg.SG_SUM), (sg.sg_reduce(c.ctx, fv, sg.SG_RMAX) if want.size else None)
+            cnt = c.get(fc)
+            ctx = (seed, launch, n, np.dtype(dtype).name, float(p_on), float(p_off))
+            assert cnt == want.size, (ctx, cnt, want.size)
+            assert bits_equal(c.read_vec(fv, dtype, cnt), want), ctx
+            check_sum(c.get(s), want, 1e-12 if dtype is np.float64 else 1e-5, ctx)
+            if mx is not None:
+                assert dtype(c.get(mx)) == orc.max(want), ctx
+            if to is not None:
+                c.torch.cuda.synchronize()
+                assert (to.cpu().numpy()[want.size:] == 77).all(), (ctx, "wrote past the capacity")
+            for h in (fv, fc, s) + ((mx,) if mx is not None else ()):
+                sg.sg_release(c.ctx, h)
+
+
+@pytest.mark.parametrize("seed", range(60))
+def test_random_bursty_filters_through_the_template_instance(seed):
+    """The same bursty masks through config 2's own chain (x mod 7 == 3, count, kept-sum: the TEMPLATE filter kernel with its TMA
+    stages, look-back warp and compaction ring), several launches of different lengths in one context."""
+    from paper_1410_6685_b200 import workloads as W
+    from gpu_util import dev
+    rng = np.random.default_rng(95000 + seed)
+    with Ctx() as c:
+        for launch in range(int(rng.integers(2, 6))):
+            n = int(rng.choice([8192, 70001, 1 << 20, int(rng.integers(1, 6_000_000))]))
+            p_on, p_off = 10.0 ** -rng.uniform(0.3, 5.0), 10.0 ** -rng.uniform(0.3, 5.0)
+            runs, state, total = [], bool(rng.random() < 0.5), 0
+            while total < n:
+                ln = int(rng.geometric(p_off if state else p_on))
+                runs.append((state, ln)); total += ln; state = not state
+            pattern = np.concatenate([np.full(ln, st) for st, ln in runs])[:n]
+            k = rng.integers(0, 1 << 27, n)
+            x = (7 * k + np.where(pattern, 3, rng.choice([0, 1, 2, 4, 5, 6], n))).astype(np.int32)
+            t = dev(x)
+            c.keep.append(t)
+            want = orc.filter(x, orc.cmp_scalar("eq", orc.scalar("mod", x, 7), 3))
+            assert want.size == int(pattern.sum())
+            to = None
+            if rng.random() < 0.5:
+                to = dev(np.full(want.size + 4, 77, dtype=np.int32))
+                c.keep.append(to)
+            r = W.cfg2(c.ctx, n, t.data_ptr(), to.data_ptr() if to is not None else None, want.size if to is not None else 0)
+            cnt = c.get(r["count"])
+            ctx = (seed, launch, n, float(p_on), float(p_off))
+            assert sg.sg_plan_stats(c.ctx).n_template == 1, ctx
+            assert cnt == want.size, (ctx, cnt, want.size)
+            assert bits_equal(c.read_vec(r["kept"], np.int32, cnt), want), ctx
+            assert c.get(r["sum"]) == orc.sum(want), ctx
+            if to is not None:
+                c.torch.cuda.synchronize()
+                assert (to.cpu().numpy()[want.size:] == 77).all(), (ctx, "wrote past the capacity")
+            for h in r.values():
+                sg.sg_release(c.ctx, h)
