@@ -910,3 +910,64 @@ def test_random_bursty_filters_through_the_template_instance(seed):
                 assert (to.cpu().numpy()[want.size:] == 77).all(), (ctx, "wrote past the capacity")
             for h in r.values():
                 sg.sg_release(c.ctx, h)
+
+
+# ----------------------------------------------------------------------------------------------------------------------------------
+# the TEMPLATE matrix kernels and the movers on random shapes: config 4's step (staged pass with row maxima and column sums), the
+# matrix-vector products, transpose (incl. the pair kernel of 4-byte elements) — any rows / columns / leading dimensions / pivot.
+# ----------------------------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("seed", range(60))
+def test_random_shapes_through_the_matrix_templates(seed):
+    from oracle import configs as ocfg
+    from paper_1410_6685_b200 import inputs, workloads as W
+    from gpu_util import NP2SG, dev
+    rng = np.random.default_rng(97000 + seed)
+    # config 4's step
+    n = int(rng.choice([int(rng.integers(2, 70)), int(rng.integers(70, 600)), int(rng.integers(600, 2300))]))
+    k = int(rng.integers(0, n))
+    ld = n + int(rng.choice([0, 0, 1, 2, 5]))
+    M = inputs.boosted_matrix_f64(int(rng.integers(1, 1000)), 0, n)
+    want = ocfg.cfg4(M, k)
+    with Ctx() as c:
+        buf = np.full((n, ld), 7.25)
+        buf[:, :n] = M
+        t = dev(buf)
+        c.keep.append(t)
+        r = W.cfg4(c.ctx, n, t.data_ptr(), k, ld=ld)
+        sg.sg_flush(c.ctx)
+        c.torch.cuda.synchronize()
+        full = t.cpu().numpy()
+        assert bits_equal(np.ascontiguousarray(full[:, :n]), want["M"]) and (full[:, n:] == 7.25).all(), (seed, "cfg4", n, k, ld)
+        if k + 1 < n:
+            assert bits_equal(c.read_vec(r["rowmax"], np.float64), want["rowmax"]), (seed, "rowmax", n, k, ld)
+            cs, scale = c.read_vec(r["colsum"], np.float64), np.abs(want["M"][k + 1:]).sum(axis=0)
+            assert np.all(np.abs(cs - want["colsum"]) <= 1e-12 * np.maximum(np.abs(want["colsum"]), 1e-300) + 2.0 ** -64 * scale), (seed, "colsum", n, k, ld)
+    # matrix-vector products, exact in the integer regime
+    rows, cols = int(rng.integers(1, 1500)), int(rng.integers(1, 1500))
+    ld = cols + int(rng.choice([0, 0, 1, 3]))
+    A = rng.integers(-8, 9, (rows, cols)).astype(np.float64)
+    v, w = rng.integers(-8, 9, cols).astype(np.float64), rng.integers(-8, 9, rows).astype(np.float64)
+    with Ctx() as c:
+        Ap = np.zeros((rows, ld))
+        Ap[:, :cols] = A
+        tA, tv, tw = dev(Ap), dev(v), dev(w)
+        c.keep += [tA, tv, tw]
+        r = W.right_multiply(c.ctx, rows, cols, tA.data_ptr(), tv.data_ptr(), ld)
+        sg.sg_flush(c.ctx)
+        l = W.left_multiply(c.ctx, rows, cols, tw.data_ptr(), tA.data_ptr(), ld)
+        got_r, got_l = c.read_vec(r["out"], np.float64, rows), c.read_vec(l["out"], np.float64, cols)
+        assert bits_equal(got_r, ocfg.right_multiply(A, v)) and bits_equal(got_l, ocfg.left_multiply(w, A)), (seed, "matvec", rows, cols, ld)
+    # transpose, every element type
+    dtype = DTYPES[seed % 4]
+    rows, cols = int(rng.integers(1, 700)), int(rng.integers(1, 700))
+    ld, ldo = cols + int(rng.choice([0, 0, 1, 2, 6])), rows + int(rng.choice([0, 0, 1, 2, 6]))
+    B = rng.integers(-10**6, 10**6, (rows, cols)).astype(dtype)
+    with Ctx() as c:
+        Bp = np.full((rows, ld), -7, dtype=dtype)
+        Bp[:, :cols] = B
+        tB, tout = dev(Bp), dev(np.full((cols, ldo), -9, dtype=dtype))
+        c.keep += [tB, tout]
+        W.transpose(c.ctx, NP2SG[np.dtype(dtype)], rows, cols, tB.data_ptr(), tout.data_ptr(), ld, ldo)
+        c.torch.cuda.synchronize()
+        got = tout.cpu().numpy()
+        assert bits_equal(np.ascontiguousarray(got[:, :rows]), ocfg.transpose(B)) and np.all(got[:, rows:] == -9), (seed, "transpose", rows, cols, ld, ldo)
