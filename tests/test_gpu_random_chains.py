@@ -971,3 +971,61 @@ def test_random_shapes_through_the_matrix_templates(seed):
         c.torch.cuda.synchronize()
         got = tout.cpu().numpy()
         assert bits_equal(np.ascontiguousarray(got[:, :rows]), ocfg.transpose(B)) and np.all(got[:, rows:] == -9), (seed, "transpose", rows, cols, ld, ldo)
+
+
+# ----------------------------------------------------------------------------------------------------------------------------------
+# Listing 5's determinant loop (one persistent kernel) and Listing 3's quicksort (one launch per recursion level) on random inputs:
+# random orders and leading dimensions, planted rank deficiencies, exact zeros below pivots, eps = 0 and eps > 0, the loop split
+# over two calls; keys with few distinct values, runs, signed zeros, every element type.
+# ----------------------------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("seed", range(40))
+def test_random_determinants_and_sorts_match_the_oracle(seed):
+    from oracle import configs as ocfg
+    from paper_1410_6685_b200 import inputs, workloads as W
+    from gpu_util import NP2SG, dev
+    rng = np.random.default_rng(98000 + seed)
+    n = int(rng.choice([int(rng.integers(1, 40)), int(rng.integers(40, 330)), int(rng.integers(330, 700))]))
+    ld = n + int(rng.choice([0, 0, 1, 3]))
+    M = inputs.boosted_matrix_f64(int(rng.integers(1, 1000)), 0, n) / float(n)
+    eps = float(rng.choice([0.0, 0.0, 1e-12, 1e-6]))
+    q = rng.random()
+    if q < 0.3 and n > 3:                                           # rank deficient: one row a combination of two others
+        i, j, k = (int(x) for x in rng.choice(n, 3, replace=False))
+        M[i] = 0.5 * M[j] + 0.25 * M[k]
+    elif q < 0.6 and n > 2:                                         # exact zeros strewn about (guarded rows), a clean diagonal
+        M[rng.integers(0, n, 2 * n), rng.integers(0, n, 2 * n)] = 0.0
+        M[np.arange(n), np.arange(n)] = 1.0 + np.arange(n) / n
+    want_det, want_E, zs = orc.ge_determinant(M, eps=eps)
+    with Ctx() as c:
+        buf = np.zeros((n, ld))
+        buf[:, :n] = M
+        t = dev(buf)
+        det, minpiv = c.torch.ones(1, dtype=c.torch.float64, device="cuda"), c.torch.full((1,), float("inf"), dtype=c.torch.float64, device="cuda")
+        c.keep += [t, det, minpiv]
+        got, ok = W.ge_determinant(c.ctx, n, t.data_ptr(), det.data_ptr(), minpiv.data_ptr(), ld=ld, eps=eps)
+        E = t.cpu().numpy()
+        ctx = (seed, "determinant", n, ld, eps, zs)
+        assert ok == (zs < 0), ctx
+        assert bits_equal(np.array([got]), np.array([want_det])), (ctx, got, want_det)
+        assert bits_equal(np.ascontiguousarray(E[:, :n]), want_E) and not E[:, n:].any(), ctx
+    # quicksort
+    dtype = DTYPES[seed % 4]
+    m = int(rng.choice([int(rng.integers(1, 3000)), int(rng.integers(3000, 60000))]))
+    style = int(rng.integers(0, 5))
+    if style == 0:
+        keys = rng.integers(-5, 6, m)                               # few distinct keys
+    elif style == 1:
+        keys = np.repeat(rng.integers(-1000, 1000, m // 50 + 1), 50)[:m]      # runs of equal keys
+    elif style == 2:
+        keys = np.sort(rng.integers(-10**6, 10**6, m))[::int(rng.choice([1, -1]))]      # sorted / reversed
+    else:
+        keys = rng.integers(-10**6, 10**6, m)
+    keys = keys.astype(dtype)
+    if np.dtype(dtype).kind == "f" and m > 4:
+        keys[rng.integers(0, m, max(1, m // 10))] = rng.choice(np.array([0.0, -0.0], dtype=dtype))     # signed zeros: equal keys, stable order
+    want = ocfg.quicksort(keys)
+    with Ctx() as c:
+        hk = c.vec(keys)
+        out = sg.sg_vec_quicksort(c.ctx, hk)
+        got = c.read_vec(out, dtype)
+    assert bits_equal(got, want), (seed, "quicksort", np.dtype(dtype).name, m, style)
