@@ -117,7 +117,7 @@ typedef struct {
     int32_t n_bytecode;         /* passes that ran the bytecode kernel */
     int64_t bytes_min;          /* algorithmic bytes of the plan: every distinct input read once + every materialised output written once */
     int64_t launches_total;     /* kernels launched by this context since creation */
-    int32_t pass_n_in[16];      /* per pass: distinct memory inputs */
+    int32_t pass_n_in[16];      /* per pass (the first 16 passes of the flush; a flush may hold up to 256): distinct memory inputs */
     int32_t pass_n_instr[16];   /* per pass: elementwise instructions in the fused body */
     int32_t pass_n_out[16];     /* per pass: outputs (stores + reductions + quantifiers + compaction) */
     int32_t pass_n_args[16];    /* per pass: kernel data arguments = memory inputs + scalar/immediate operands + outputs */

@@ -236,7 +236,7 @@ sg_status flush_body(sg_ctx* c, int* executed, ExitGroups* exit_groups) {
     bool fits = true;
     for (const Pass& P : passes) fits = fits && pass_outputs(P) <= SG_MAX_OUT;
     if (!fits && attempt < 5) continue;
-    if (passes.size() > 16) return sg_fail(c, SG_ERR_CAPACITY, "more than 16 passes in one flush");
+    if (passes.size() > 256) return sg_fail(c, SG_ERR_CAPACITY, "more than 256 passes in one flush");     // (sg_stats describes the first 16)
 
     // ---- 4. programs, outputs, geometry ------------------------------------------------------------------
     // spilled intermediates become context-owned temporaries, released after the launches are queued

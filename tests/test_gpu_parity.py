@@ -1016,7 +1016,7 @@ def test_failed_flush_discards_and_the_context_goes_on():
     with Ctx() as c:
         ha = c.vec(a)
         sg.sg_enqueue(c.ctx, sg.SG_ADD, [ha, sg.F(1.0)], dst_or_0=ha)   # an in-place update queued in the same (failing) flush
-        many = [sg.sg_reduce(c.ctx, sg.sg_enqueue(c.ctx, sg.SG_MUL, [ha, sg.F(float(i))]), sg.SG_SUM) for i in range(200)]     # > 16 passes
+        many = [sg.sg_reduce(c.ctx, sg.sg_enqueue(c.ctx, sg.SG_MUL, [ha, sg.F(float(i))]), sg.SG_SUM) for i in range(2200)]     # > 256 passes
         with pytest.raises(sg.SgError) as e:
             sg.sg_flush(c.ctx)
         assert e.value.status == sg.SG_ERR_CAPACITY

@@ -523,7 +523,7 @@ def test_an_input_never_shares_a_register_with_an_earlier_temporary():
             # every DAG plans: a pass that a later spill would overfill (more than SG_MAX_OUT outputs) is re-planned with outputs held
             # in reserve — seeds 16, 42, 53, 77, ... failed with SG_ERR_CAPACITY "too many outputs in one pass" before
             _, _, stats, _ = R.run_gpu(c, steps, keep, reds, inputs, dtype, filt)
-            assert 1 <= stats.n_passes <= 16
+            assert 1 <= stats.n_passes <= 32
             for p in range(stats.n_passes):
                 d = sg.sg_plan_dump(c.ctx, p)
                 assert _input_registers_are_never_written(d), (seed, d)
@@ -577,7 +577,7 @@ def test_a_failed_flush_discards_the_pending_list_and_leaves_the_context_usable(
                 sg.sg_release(ctx, bad)
             bad = nxt
         pend = [sg.sg_reduce(ctx, bad, k) for k in (sg.SG_SUM, sg.SG_RMAX, sg.SG_RMIN)] * 1
-        many = [sg.sg_reduce(ctx, sg.sg_enqueue(ctx, sg.SG_MUL, [x, sg.F(float(i))]), sg.SG_SUM) for i in range(200)]   # ... and > 16 passes
+        many = [sg.sg_reduce(ctx, sg.sg_enqueue(ctx, sg.SG_MUL, [x, sg.F(float(i))]), sg.SG_SUM) for i in range(2200)]   # ... and > 256 passes
         with pytest.raises(sg.SgError) as e:
             sg.sg_flush(ctx)
         assert e.value.status == sg.SG_ERR_CAPACITY and "discarded" in str(e.value)
