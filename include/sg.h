@@ -106,7 +106,8 @@ enum {
     SG_FLAG_UNFUSED = 1,        /* lower every pending op to its own launch with materialised temporaries:
                                    the "one kernel per method call" plan of PAPER.md:282 (measurement baseline) */
     SG_FLAG_FORCE_BYTECODE = 2, /* never pick a precompiled template instance; always run the bytecode kernel */
-    SG_FLAG_NO_EARLY_EXIT = 4   /* quantifier passes read the whole collection even after a witness is found */
+    SG_FLAG_NO_EARLY_EXIT = 4,  /* quantifier passes read the whole collection even after a witness is found */
+    SG_FLAG_NO_PLAN_CACHE = 8   /* plan every flush from scratch (the plan cache below is on by default) */
 };
 
 /* Plan statistics of the last flush (tests, reports). */
@@ -278,6 +279,11 @@ sg_status sg_plan_stats(sg_ctx* ctx, sg_stats* out);
 /* Canonical program of pass `pass` of the last flush as text (template generator, tests). Returns bytes needed. */
 int64_t sg_plan_dump(sg_ctx* ctx, int32_t pass, char* buf, int64_t cap);
 /* Device time of the last flush's launches in milliseconds (CUDA events on the context's stream). */
+/* Plan cache (the optimizer runs at every trigger; a loop triggers the same pending list again and again): the pass
+ * assignment of a pending list is remembered under the list's signature — operations, the identity pattern, storage and liveness of
+ * the values they name, contracts, flags; immediates excluded — and re-used when the same list over the same buffers is flushed
+ * again.  Programs are built and bound to their pointers by every flush.  Counts since the context was created. */
+sg_status sg_plan_cache_stats(sg_ctx* ctx, int64_t* hits, int64_t* misses);
 sg_status sg_last_flush_ms(sg_ctx* ctx, float* ms);
 /* Device time of every flush between begin and end, without a host synchronisation inside the region: each flush records
  * its own CUDA event pair on the context's stream; sg_timing_end waits for the last one and returns the sum in

@@ -92,6 +92,19 @@ struct Pass {
 
 struct Launch { SgProg prog; SgArgs args; SgGeom geom; };
 
+// Plan cache (SURVEY.md §8 a2 "plan cache keyed by DAG signature"): the pass assignment of a pending list — the part of planning that
+// compares every operation with every pass and may repeat itself under tighter limits — remembered under the SIGNATURE of that list:
+// every operation, the identity pattern and the storage (address, shape, liveness) of every value it names, the contracts and the
+// context flags, as bytes.  A step that enqueues the same program over the same buffers again (any immediates) re-uses the
+// assignment; programs are still built and bound to their pointers by every flush.
+struct PlanMemo {
+    std::string key;
+    int attempt = 0;                // which limits the assignment succeeded under (sg_plan.cpp)
+    std::vector<int> node_pass;     // per pending operation: its pass (-1: not needed)
+    std::vector<char> node_spill;   // per pending operation: its result is stored for a later pass
+    std::vector<Pass> passes;       // skeletons: domain, dtype, flags, operations (no programs, no memory ranges)
+};
+
 struct sg_ctx {
     int device = -1;
     bool plan_only = true;
@@ -130,6 +143,9 @@ struct sg_ctx {
     sg_stats stats{};
     std::vector<SgProg> dumps;      // canonical programs of the last flush; sg_plan_dump renders them as text on demand
     std::vector<char*> deferred_free;
+    std::vector<PlanMemo> plan_cache;   // a few entries, replaced round robin
+    size_t plan_cache_next = 0;
+    int64_t plan_cache_hits = 0, plan_cache_misses = 0;
 };
 
 // Makes the context's device current for the duration of one entry point and restores the caller's device afterwards

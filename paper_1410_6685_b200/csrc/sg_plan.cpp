@@ -51,6 +51,57 @@ bool pending(const sg_ctx* c, const Value& v) { return v.node >= 0 && !c->nodes[
 
 namespace {
 
+// The signature of the pending list (PlanMemo, sg_ctx.h): everything the pass assignment reads, as bytes.  Values are numbered in
+// order of first appearance (table slots differ from step to step), described once: kind, dtype, shape, address, liveness, producer.
+// Immediates are left out: they decide nothing in the assignment (a build that then fails a limit falls back to the full planner).
+std::string plan_signature(const sg_ctx* c, bool unfused) {
+    const std::vector<Node>& N = c->nodes;
+    const std::vector<Value>& V = c->values;
+    // upper bound of the key: per operation a head + two operands + two results, each value described at most once per mention
+    constexpr size_t VAL = 4 + 8 * 4 + 5 * 8, NODE = 12 * 4 + 16 + 2 * 8 + 4 * VAL;
+    std::string key;
+    key.resize(16 + N.size() * NODE + c->contracts.size() * (VAL + 4));
+    char* w = &key[0];
+    const auto put = [&](const void* p, size_t n) { memcpy(w, p, n); w += n; };
+    const auto put32 = [&](int32_t x) { memcpy(w, &x, 4); w += 4; };
+    // value numbering by first appearance: a small open-addressed table keyed by the table slot
+    size_t cap = 64;
+    while (cap < 8 * N.size() + 16) cap <<= 1;
+    std::vector<int32_t> slot_key(cap, -1), slot_id(cap, 0);
+    int32_t next_id = 0;
+    const auto value = [&](int vi) {
+        size_t h = ((size_t)vi * 0x9E3779B1u) & (cap - 1);
+        while (slot_key[h] >= 0 && slot_key[h] != vi) h = (h + 1) & (cap - 1);
+        if (slot_key[h] == vi) { put32(slot_id[h]); return; }
+        slot_key[h] = vi; slot_id[h] = next_id;
+        const Value& v = V[vi];
+        put32(-1 - next_id);                            // first appearance: the description follows
+        ++next_id;
+        const int32_t head[8] = {v.kind, v.dtype, (v.node >= 0 && !N[v.node].done) ? v.node : -1, v.materialised, v.slot >= 0, v.user_refs > 0, v.count_known, 0};
+        put(head, sizeof(head));
+        const int64_t shape[5] = {(int64_t)(uintptr_t)v.ptr, v.stride, v.ld, v.rows, v.cols};
+        put(shape, sizeof(shape));
+    };
+    put32((int32_t)N.size());
+    put32(unfused ? 1 : 0);
+    for (const Node& n : N) {
+        const int32_t head[12] = {n.kind, n.op, n.n_opd, n.axis, n.dtype, n.src_dtype, n.is2d, n.inplace, n.needed, n.post, n.done, 0};
+        put(head, sizeof(head));
+        const int64_t dom[2] = {n.rows, n.cols};
+        put(dom, sizeof(dom));
+        for (int j = 0; j < n.n_opd; ++j) {
+            put32(n.opd[j].kind); put32(n.opd[j].bcast);
+            if (n.opd[j].kind != OPD_IMM) value(n.opd[j].value);
+        }
+        if (n.out >= 0) value(n.out); else put32(0x7fffffff);
+        if (n.out2 >= 0) value(n.out2); else put32(0x7fffffff);
+    }
+    put32((int32_t)c->contracts.size());
+    for (const Contract& k : c->contracts) { value(k.value); put32(k.kind); }
+    key.resize((size_t)(w - key.data()));
+    return key;
+}
+
 // quantifier outputs of a pass that may end early at a violated contract (PF_EARLY_EXIT with registered for_all contracts)
 struct ExitMember { int value; uint8_t kind; bool is_contract; };
 typedef std::vector<std::vector<ExitMember>> ExitGroups;
@@ -125,8 +176,18 @@ sg_status flush_body(sg_ctx* c, int* executed, ExitGroups* exit_groups) {
     static const int reserves[] = {0, 2, 4, 6, 7}, node_limits[] = {SG_MAX_INSTR, SG_MAX_INSTR, 16, 8, 4};
     std::vector<char*> temps;
     const sg_stats stats0 = c->stats;
-    for (int attempt = 0;; ++attempt) {
-    if (attempt == 5) { unfused = true; c->flags |= SG_FLAG_UNFUSED; }
+    // plan cache: the same pending list (signature) was assigned before — take that assignment, under the limits it succeeded with
+    const bool use_cache = !(c->flags & SG_FLAG_NO_PLAN_CACHE);
+    std::string signature;
+    const PlanMemo* memo = nullptr;
+    if (use_cache) {
+        signature = plan_signature(c, unfused);
+        for (const PlanMemo& m : c->plan_cache)
+            if (m.key == signature) { memo = &m; break; }
+        if (memo) c->plan_cache_hits++; else c->plan_cache_misses++;
+    }
+    for (int attempt = memo ? memo->attempt : 0;; ++attempt) {
+    if (attempt >= 5) { unfused = true; c->flags |= SG_FLAG_UNFUSED; }
     const int out_limit = SG_MAX_OUT - reserves[attempt < 5 ? attempt : 0];
     const int node_limit = node_limits[attempt < 5 ? attempt : 0];
     passes.clear();
@@ -138,6 +199,13 @@ sg_status flush_body(sg_ctx* c, int* executed, ExitGroups* exit_groups) {
         n.pass = -1;
         if (n.out >= 0 && V[n.out].user_refs < 0) V[n.out].user_refs = 0;       // spill marks of an abandoned attempt
     }
+    if (memo) {
+        passes = memo->passes;
+        for (size_t i = 0; i < N.size(); ++i) {
+            N[i].pass = memo->node_pass[i];
+            if (memo->node_spill[i]) spill[N[i].out] = 1;
+        }
+    } else
     for (size_t i = 0; i < N.size(); ++i) {
         Node& X = N[i];
         if (X.done || !X.needed) continue;
@@ -235,7 +303,10 @@ sg_status flush_body(sg_ctx* c, int* executed, ExitGroups* exit_groups) {
     }
     bool fits = true;
     for (const Pass& P : passes) fits = fits && pass_outputs(P) <= SG_MAX_OUT;
-    if (!fits && attempt < 5) continue;
+    if (!fits && attempt < 5) {
+        if (memo) { c->plan_cache.erase(c->plan_cache.begin() + (memo - c->plan_cache.data())); memo = nullptr; }
+        continue;
+    }
     if (passes.size() > 256) return sg_fail(c, SG_ERR_CAPACITY, "more than 256 passes in one flush");     // (sg_stats describes the first 16)
 
     // ---- 4. programs, outputs, geometry ------------------------------------------------------------------
@@ -270,8 +341,33 @@ sg_status flush_body(sg_ctx* c, int* executed, ExitGroups* exit_groups) {
     return SG_OK;
     };
     const sg_status built = build_all();
-    if (built == SG_ERR_CAPACITY && attempt < 5) continue;
+    if (built == SG_ERR_CAPACITY && attempt < 5) {
+        if (memo) {         // (immediates are not part of the signature: this list needs tighter limits than the remembered one)
+            c->plan_cache.erase(c->plan_cache.begin() + (memo - c->plan_cache.data()));
+            memo = nullptr;
+        }
+        continue;
+    }
     if (built != SG_OK) return built;
+    if (use_cache && !memo) {
+        PlanMemo m;
+        m.key = std::move(signature);
+        m.attempt = attempt;
+        m.node_pass.resize(N.size());
+        m.node_spill.assign(N.size(), 0);
+        for (size_t i = 0; i < N.size(); ++i) {
+            m.node_pass[i] = N[i].pass;
+            m.node_spill[i] = (N[i].out >= 0 && N[i].kind == NK_MAP && N[i].needed) ? spill[N[i].out] : 0;
+        }
+        m.passes.reserve(passes.size());
+        for (const Pass& P : passes) {
+            Pass q;
+            q.is2d = P.is2d; q.has_filter = P.has_filter; q.has_store = P.has_store; q.dtype = P.dtype; q.rows = P.rows; q.cols = P.cols; q.nodes = P.nodes;
+            m.passes.push_back(std::move(q));
+        }
+        if (c->plan_cache.size() < 8) c->plan_cache.push_back(std::move(m));
+        else { c->plan_cache[c->plan_cache_next % 8] = std::move(m); c->plan_cache_next++; }
+    }
     break;
     }
 
@@ -471,6 +567,13 @@ sg_status sg_flush_impl(sg_ctx* c) {
         if (e != cudaSuccess) return sg_fail(c, SG_ERR_CUDA, cudaGetErrorString(e));
     }
     return result;
+}
+
+extern "C" sg_status sg_plan_cache_stats(sg_ctx* c, int64_t* hits, int64_t* misses) {
+    if (!c || !hits || !misses) return SG_ERR_ARG;
+    *hits = c->plan_cache_hits;
+    *misses = c->plan_cache_misses;
+    return SG_OK;
 }
 
 extern "C" sg_status sg_last_flush_ms(sg_ctx* c, float* ms) {

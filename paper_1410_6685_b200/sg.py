@@ -20,7 +20,7 @@ SG_AXIS_ALL, SG_AXIS_ROWS, SG_AXIS_COLS = 0, 1, 2
 SG_OPERAND_HANDLE, SG_OPERAND_IMM_F64, SG_OPERAND_IMM_I64 = 0, 1, 2
 SG_BCAST_NONE, SG_BCAST_ROW, SG_BCAST_COL = 0, 1, 2
 SG_CONTRACT_PRE, SG_CONTRACT_POST = 0, 1
-SG_FLAG_UNFUSED, SG_FLAG_FORCE_BYTECODE, SG_FLAG_NO_EARLY_EXIT = 1, 2, 4
+SG_FLAG_UNFUSED, SG_FLAG_FORCE_BYTECODE, SG_FLAG_NO_EARLY_EXIT, SG_FLAG_NO_PLAN_CACHE = 1, 2, 4, 8
 SG_OK = 0
 SG_ACC_DEFAULT = -1
 SG_ERR = {-1: "SG_ERR_ARG", -2: "SG_ERR_SHAPE", -3: "SG_ERR_DTYPE", -4: "SG_ERR_EMPTY", -5: "SG_ERR_ALIAS", -6: "SG_ERR_OOM",
@@ -32,7 +32,7 @@ EXPORTS = [
     "sg_ctx_create", "sg_ctx_destroy", "sg_ctx_set_flags", "sg_last_error", "sg_vec_create", "sg_mat_create", "sg_vec_subset",
     "sg_mat_row", "sg_mat_rows", "sg_mat_col", "sg_mat_elem", "sg_mat_ge_steps", "sg_mat_transpose", "sg_vec_quicksort", "sg_vec_sum_noalloc", "sg_enqueue", "sg_cast", "sg_reduce", "sg_forall", "sg_exists",
     "sg_forall_adjacent", "sg_filter", "sg_contract", "sg_flush", "sg_scalar_get", "sg_scalar_dtype", "sg_vec_count", "sg_vec_data", "sg_vec_read",
-    "sg_release", "sg_plan_stats", "sg_plan_dump", "sg_last_flush_ms", "sg_timing_begin", "sg_timing_end", "sg_replay_last", "sg_replay_last_graph", "sg_template_count", "sg_template_name",
+    "sg_release", "sg_plan_stats", "sg_plan_dump", "sg_plan_cache_stats", "sg_last_flush_ms", "sg_timing_begin", "sg_timing_end", "sg_replay_last", "sg_replay_last_graph", "sg_template_count", "sg_template_name",
     "sg_version",
 ]
 
@@ -98,6 +98,7 @@ def lib() -> ctypes.CDLL:
         L.sg_vec_read.argtypes = [c_void_p, c_int64, c_void_p, c_size_t]
         L.sg_plan_stats.argtypes = [c_void_p, POINTER(sg_stats)]
         L.sg_plan_dump.argtypes = [c_void_p, c_int32, c_char_p, c_int64]
+        L.sg_plan_cache_stats.argtypes = [c_void_p, POINTER(c_int64), POINTER(c_int64)]
         L.sg_last_flush_ms.argtypes = [c_void_p, POINTER(c_float)]
         L.sg_replay_last.argtypes = [c_void_p, c_int32, POINTER(c_float)]
         L.sg_replay_last_graph.argtypes = [c_void_p, c_int32, POINTER(c_float), POINTER(c_float)]
@@ -325,6 +326,13 @@ def sg_plan_dump(ctx, pass_index: int) -> str:
     buf = ctypes.create_string_buffer(need)
     lib().sg_plan_dump(ctx, pass_index, buf, need)
     return buf.value.decode()
+
+
+def sg_plan_cache_stats(ctx):
+    """(hits, misses) of the plan cache since the context was created."""
+    h, m = c_int64(0), c_int64(0)
+    _ck(ctx, lib().sg_plan_cache_stats(ctx, byref(h), byref(m)))
+    return h.value, m.value
 
 
 def sg_last_flush_ms(ctx) -> float:

@@ -1029,3 +1029,69 @@ def test_random_determinants_and_sorts_match_the_oracle(seed):
         out = sg.sg_vec_quicksort(c.ctx, hk)
         got = c.read_vec(out, dtype)
     assert bits_equal(got, want), (seed, "quicksort", np.dtype(dtype).name, m, style)
+
+
+# ----------------------------------------------------------------------------------------------------------------------------------
+# the plan cache: the same random program enqueued again over the same buffers takes its pass assignment from the
+# cache (a hit) — every round's results must still be the oracle's, with the cache and with SG_FLAG_NO_PLAN_CACHE.
+# ----------------------------------------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("seed", range(120))
+def test_random_chains_replayed_through_the_plan_cache(seed):
+    from gpu_util import NP2SG, dev
+    rng = np.random.default_rng(1000 + seed)                 # the DAGs of test_random_chains_match_the_oracle
+    dtype = DTYPES[seed % 4]
+    n = int(SIZES[(seed // 4) % len(SIZES)])
+    inputs = [make_input(rng, dtype, n) for _ in range(int(rng.integers(1, 4)))]
+    steps, keep, reds, want, storage, filt = build_dag(rng, dtype, inputs, rich=True)
+    tol = {np.float32: 1e-5, np.float64: 1e-12}.get(dtype, 0)
+    rounds = 3
+    for flags in (0, sg.SG_FLAG_NO_PLAN_CACHE):
+        with Ctx(flags) as c:
+            tens = [dev(a) for a in inputs]
+            c.keep += tens
+
+            class Round:                                     # what run_gpu needs of a context: the SAME device buffers every round
+                ctx = c.ctx
+
+                def __init__(self):
+                    self.k = 0
+
+                def vec(self, a):
+                    t = tens[self.k]
+                    self.k += 1
+                    return sg.sg_vec_create(c.ctx, NP2SG[np.dtype(dtype)], a.size, t.data_ptr())
+
+                def get(self, h):
+                    return c.get(h)
+            for rnd in range(rounds):
+                for t, a in zip(tens, inputs):               # in-place steps overwrote the inputs: restore them
+                    t.copy_(c.torch.from_numpy(a))
+                c.torch.cuda.synchronize()
+                h, scal, st, fres = run_gpu(Round(), steps, keep, reds, inputs, dtype, filt)
+                for i in sorted(keep | storage):
+                    assert bits_equal(c.read_vec(h[i], want[i].dtype), want[i]), (flags, seed, rnd, "stored value", i, steps)
+                for (kind, src, _), got in zip(reds, scal):
+                    w = want[src]
+                    if kind == "sum":
+                        check_sum(got, w, tol, (flags, seed, rnd, kind))
+                    elif kind == "count":
+                        assert got == orc.count(w), (flags, seed, rnd, kind)
+                    elif kind in ("all", "any"):
+                        assert got == (orc.all(w) if kind == "all" else orc.any(w)), (flags, seed, rnd, kind)
+                    elif kind.startswith("adj_"):
+                        assert got == (orc.all(orc.adj(kind[4:], w)) if w.size > 1 else True), (flags, seed, rnd, kind)
+                    elif not (w.dtype.kind == "f" and np.isnan(w).any()):
+                        assert bits_equal(np.array([got], dtype=dtype), np.array([(orc.max if kind == "max" else orc.min)(w)], dtype=dtype)), (flags, seed, rnd, kind)
+                if fres is not None:
+                    kept = orc.filter(want[filt[0]], want[filt[1]])
+                    cnt = c.get(fres[1])
+                    assert cnt == kept.size and bits_equal(c.read_vec(fres[0], kept.dtype, cnt), kept), (flags, seed, rnd, "filter")
+                    for x in fres:
+                        sg.sg_release(c.ctx, x)
+                for x in {h[i] for i in range(len(inputs))} | {h[i] for i in keep}:      # what the caller still holds (run_gpu released the rest)
+                    sg.sg_release(c.ctx, x)
+            hits, misses = sg.sg_plan_cache_stats(c.ctx)
+            if flags:
+                assert hits == 0 and misses == 0
+            else:
+                assert hits >= rounds - 1 and misses >= 1, (seed, hits, misses)

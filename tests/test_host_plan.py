@@ -566,6 +566,43 @@ def test_chains_beyond_the_limits_of_one_pass_are_split_not_rejected():
     assert st.n_passes >= 2 and st.n_nodes == 25
 
 
+def test_plan_cache_hits_on_the_same_list_and_misses_on_a_different_one():
+    """the pass assignment is remembered under the signature of the pending list — operations, identity pattern,
+    storage and liveness of the values, contracts, flags; immediates excluded."""
+    ctx = sg.sg_ctx_create(-1)
+    try:
+        bufs = [0x7000000000, 0x7100000000, 0x7200000000]     # (away from a plan-only context's made-up addresses)
+
+        def step(k=2.5, keep_t=False, ptr0=None):
+            a, b, c3 = (sg.sg_vec_create(ctx, sg.SG_F64, 1 << 20, p) for p in ([ptr0 or bufs[0]] + bufs[1:]))
+            t = sg.sg_enqueue(ctx, sg.SG_ADD, [a, b])
+            u = sg.sg_enqueue(ctx, sg.SG_MUL, [t, sg.F(k)])
+            z = sg.sg_enqueue(ctx, sg.SG_SUB, [u, c3])
+            s = sg.sg_reduce(ctx, z, sg.SG_SUM)
+            if not keep_t:
+                sg.sg_release(ctx, t)
+            sg.sg_release(ctx, u)
+            sg.sg_flush(ctx)
+            st = sg.sg_plan_stats(ctx)
+            dumps = [sg.sg_plan_dump(ctx, p) for p in range(st.n_passes)]
+            for h in (a, b, c3, z, s) + ((t,) if keep_t else ()):
+                sg.sg_release(ctx, h)
+            return dumps
+        first = step()
+        assert sg.sg_plan_cache_stats(ctx) == (0, 1)
+        assert step() == first and sg.sg_plan_cache_stats(ctx) == (1, 1)             # the same list again: a hit, the same programs
+        assert step(k=7.0) == first and sg.sg_plan_cache_stats(ctx) == (2, 1)        # another immediate: still a hit
+        kept = step(keep_t=True)                                                     # t stays alive: one more stored output, another list
+        assert kept != first and sg.sg_plan_cache_stats(ctx) == (2, 2)
+        step(ptr0=0x7300000000)                                                        # another buffer: another signature
+        assert sg.sg_plan_cache_stats(ctx) == (2, 3)
+        assert step() == first and step(keep_t=True) == kept and sg.sg_plan_cache_stats(ctx) == (4, 3)    # both lists are remembered
+        sg.sg_ctx_set_flags(ctx, sg.SG_FLAG_NO_PLAN_CACHE)
+        assert step() == first and sg.sg_plan_cache_stats(ctx) == (4, 3)             # switched off: planned from scratch, not counted
+    finally:
+        sg.sg_ctx_destroy(ctx)
+
+
 def test_a_failed_flush_discards_the_pending_list_and_leaves_the_context_usable():
     ctx = sg.sg_ctx_create(-1)
     try:
