@@ -630,6 +630,7 @@ def main():
     clocks = sampler.stop() if rank == 0 else None
     launches = sg.sg_plan_stats(ctx).launches_total - launches0
     st = sg.sg_plan_stats(ctx)
+    cache_hits, cache_misses = sg.sg_plan_cache_stats(ctx)
     for r in pending:                                   # every step's results are read and must agree with the warm-up's
         s1, m1 = sg.sg_scalar_get(ctx, r["sum"]), sg.sg_scalar_get(ctx, r["max"])
         assert s1 == s0 and m1 == m0, (s1, s0, m1, m0)
@@ -676,7 +677,7 @@ def main():
         "ms_per_step": ms_step, "higher_is_better": True, "scaling": "strong" if shard else "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": {"workload": f"cfg1 fused 10-op chain + sum + max on fp32 x,y of 2^{args.log2n} elements (BASELINE.json metric: fused chain at 2^28)",
                    "n": n, "sharded_over_ranks": shard, "n_total": n_total if shard else n * world, "seed": 2, "l2": "inputs (2 x 4n bytes) larger than L2; no flush needed", "plan_passes": st.n_passes,
-                   "template_passes": st.n_template, "step": "enqueue + plan + fused launch + scalar hand-back (async copy to the pinned mirror) through the C ABI; K steps pipelined, scalars read after the region"},
+                   "template_passes": st.n_template, "plan_cache": {"hits": cache_hits, "misses": cache_misses}, "step": "enqueue + plan + fused launch + scalar hand-back (async copy to the pinned mirror) through the C ABI; K steps pipelined, scalars read after the region"},
         "GB/s": world * alg_bytes / ms_step / 1e6,
         "frac_of_8TBps": alg_bytes / ms_step / 1e6 / 8000.0,
         "roofline": {"bound": "hbm", "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,

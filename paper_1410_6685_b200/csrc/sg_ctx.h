@@ -146,6 +146,7 @@ struct sg_ctx {
     std::vector<PlanMemo> plan_cache;   // a few entries, replaced round robin
     size_t plan_cache_next = 0;
     int64_t plan_cache_hits = 0, plan_cache_misses = 0;
+    int plan_cache_miss_streak = 0, plan_cache_pause = 0;   // a loop whose lists never repeat (other buffers every step) stops paying for signatures
 };
 
 // Makes the context's device current for the duration of one entry point and restores the caller's device afterwards

@@ -177,14 +177,21 @@ sg_status flush_body(sg_ctx* c, int* executed, ExitGroups* exit_groups) {
     std::vector<char*> temps;
     const sg_stats stats0 = c->stats;
     // plan cache: the same pending list (signature) was assigned before — take that assignment, under the limits it succeeded with
-    const bool use_cache = !(c->flags & SG_FLAG_NO_PLAN_CACHE);
+    // (a loop whose pending lists never repeat — other buffers or views every step, like Listing 5 written over host-issued row
+    // operations — would only pay for signatures: after 16 misses in a row the cache sits out the next 64 flushes, then tries again)
+    bool use_cache = !(c->flags & SG_FLAG_NO_PLAN_CACHE);
+    if (use_cache && c->plan_cache_pause > 0) { c->plan_cache_pause--; use_cache = false; }
     std::string signature;
     const PlanMemo* memo = nullptr;
     if (use_cache) {
         signature = plan_signature(c, unfused);
         for (const PlanMemo& m : c->plan_cache)
             if (m.key == signature) { memo = &m; break; }
-        if (memo) c->plan_cache_hits++; else c->plan_cache_misses++;
+        if (memo) { c->plan_cache_hits++; c->plan_cache_miss_streak = 0; }
+        else {
+            c->plan_cache_misses++;
+            if (++c->plan_cache_miss_streak >= 16) { c->plan_cache_pause = 64; c->plan_cache_miss_streak = 8; }
+        }
     }
     for (int attempt = memo ? memo->attempt : 0;; ++attempt) {
     if (attempt >= 5) { unfused = true; c->flags |= SG_FLAG_UNFUSED; }
