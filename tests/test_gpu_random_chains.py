@@ -600,7 +600,7 @@ def test_random_row_programs_match_eager_execution(seed):
                     rowh[i] = sg.sg_mat_row(c.ctx, hM, i)
                 return rowh[i]
             cur = lambda i: mem[i, :cols].copy()
-            temps, kept = [], []
+            temps, kept, ctemps = [], [], []
             try:
                 for _ in range(int(pr.integers(6, 15))):
                     op = str(pr.choice(["add", "sub", "mul", "max", "min"]))
@@ -630,9 +630,21 @@ def test_random_row_programs_match_eager_execution(seed):
                         mem[j, :cols] = orc.scalar(op, cur(j), float(sval) if is_f else int(sval))
                         sg.sg_release(c.ctx, s)
                         trace.append(("row_max", op, j, i))
-                    elif q < 0.74:                                                  # t = r_i op r_j
+                    elif q < 0.68:                                                  # t = r_i op r_j
                         temps.append((sg.sg_enqueue(c.ctx, BIN[op], [row(i), row(j)]), orc.zip(op, cur(i), cur(j))))
                         trace.append(("temp", op, i, j))
+                    elif q < 0.74:                                                  # t = column(a)[r0:r1] op column(b)[r0:r1]: deferred strided copies
+                        r0 = int(pr.integers(0, rows))
+                        r1 = int(pr.integers(r0 + 1, rows + 1))
+                        a, b = int(pr.integers(0, cols)), int(pr.integers(0, cols))
+                        ca, cb = sg.sg_mat_col(c.ctx, hM, a, r0, r1), sg.sg_mat_col(c.ctx, hM, b, r0, r1)
+                        ctemps.append((sg.sg_enqueue(c.ctx, BIN[op], [ca, cb]), orc.zip(op, np.ascontiguousarray(mem[r0:r1, a]), np.ascontiguousarray(mem[r0:r1, b]))))
+                        if pr.random() < 0.5:
+                            ctemps.append((ca, np.ascontiguousarray(mem[r0:r1, a]).copy()))
+                        else:
+                            sg.sg_release(c.ctx, ca)
+                        sg.sg_release(c.ctx, cb)
+                        trace.append(("cols", op, a, b, r0, r1))
                     elif q < 0.84 and temps:                                        # r_i := t op r_i
                         t = temps[int(pr.integers(0, len(temps)))]
                         sg.sg_enqueue(c.ctx, BIN[op], [t[0], row(i)], dst_or_0=row(i))
@@ -663,7 +675,7 @@ def test_random_row_programs_match_eager_execution(seed):
                 if mode == "unfused" and e.status == sg.SG_ERR_CAPACITY:            # more than 256 passes in one flush
                     continue
                 raise
-            for th, tv in kept:
+            for th, tv in kept + ctemps:
                 assert bits_equal(c.read_vec(th, dtype), tv), (mode, seed, "kept temporary", trace)
             c.torch.cuda.synchronize()
             assert bits_equal(tM.cpu().numpy(), mem), (mode, seed, "matrix", trace)
