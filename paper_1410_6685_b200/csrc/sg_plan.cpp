@@ -218,7 +218,7 @@ sg_status flush_body(sg_ctx* c, int* executed, ExitGroups* exit_groups) {
         if (X.done || !X.needed) continue;
         int lb = 0, forced = -1;
         std::vector<MemRange> reads, writes;
-        std::vector<int> reg_producers;
+        std::vector<std::pair<int, bool>> reg_producers;     // (producer, the operand is read index-for-index)
         for (int j = 0; j < X.n_opd; ++j) {
             if (X.opd[j].kind == OPD_IMM) continue;
             const Value& v = V[X.opd[j].value];
@@ -230,8 +230,13 @@ sg_status flush_body(sg_ctx* c, int* executed, ExitGroups* exit_groups) {
                     const bool from_memory = X.opd[j].kind == OPD_SHIFT || (X.kind == NK_MAP && X.op == NODE_OP_CAST);
                     const bool via_memory = unfused || (X.post && materialises(Y)) || from_memory;
                     lb = std::max(lb, Y.pass + (via_memory ? 1 : 0));
-                    if (!via_memory) reg_producers.push_back(v.node);
+                    const bool exact = X.opd[j].kind != OPD_SHIFT && X.opd[j].bcast == SG_BCAST_NONE;
+                    if (!via_memory) reg_producers.push_back({v.node, exact});
                     if (from_memory) spill[X.opd[j].value] = 1;
+                    // A pending IN-PLACE result read from memory by a later pass is a read of the caller's buffer: a later in-place
+                    // writer of overlapping storage (another view of it) must not share that pass (WAR).  Spilled temporaries have
+                    // storage of their own and need no such edge.
+                    if (via_memory && Y.inplace && V[Y.out].ptr) reads.push_back(range_of(V[Y.out], exact));
                 } else if (Y.kind == NK_REDUCE) {
                     lb = std::max(lb, Y.pass + 1);
                 } else {    // NK_FILTER: only a reduction over the kept values may follow, in the same pass
@@ -301,12 +306,15 @@ sg_status flush_body(sg_ctx* c, int* executed, ExitGroups* exit_groups) {
         P.has_store |= stores;
         for (const MemRange& r : reads) P.reads.push_back(r);
         for (const MemRange& w : writes) P.writes.push_back(w);
-        for (int y : reg_producers)
+        for (const auto& yp : reg_producers) {
+            const int y = yp.first;
             if (N[y].pass < p) {                                // register edge became a cross-pass edge: spill the value
                 spill[N[y].out] = 1;
                 if (passes[N[y].pass].has_filter) return sg_fail(c, SG_ERR_UNSUPPORTED, "a filter pass cannot materialise an intermediate");
                 passes[N[y].pass].has_store = true;
+                if (N[y].inplace && V[N[y].out].ptr) P.reads.push_back(range_of(V[N[y].out], yp.second));     // (see above: the caller's buffer is read here)
             }
+        }
     }
     bool fits = true;
     for (const Pass& P : passes) fits = fits && pass_outputs(P) <= SG_MAX_OUT;

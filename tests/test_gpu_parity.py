@@ -265,6 +265,32 @@ def test_fourteen_vectors_in_one_expression():
     assert bits_equal(got, want)
 
 
+@pytest.mark.parametrize("mode", ["template", "unfused"])
+def test_inplace_result_read_by_a_later_pass_orders_overlapping_writers(mode):
+    """a := 2a (in place, pass 0); u = a + max(c) (a scalar edge puts it in pass 1, where a's new contents are read from the caller's
+    buffer); b := b + 1 with b an OVERLAPPING view of the same buffer.  The write to b must not share pass 1 with the read of a
+    (another thread's element): the read of a pending in-place result by a later pass is a memory read like any other (WAR edge;
+    found by the soak run of the randomised view programs, seed 1040)."""
+    n, L, s = 200000, 120000, 50000
+    x, y = RNG.standard_normal(n), RNG.standard_normal(L)
+    mem = x.copy()
+    with Ctx(MODES[mode]) as c:
+        hx, hc = c.vec(x), c.vec(y)
+        a, b = sg.sg_vec_subset(c.ctx, hx, 0, L), sg.sg_vec_subset(c.ctx, hx, s, s + L)
+        sg.sg_enqueue(c.ctx, sg.SG_MUL, [a, sg.F(2.0)], dst_or_0=a)
+        mem[0:L] = orc.scalar("mul", mem[0:L].copy(), 2.0)
+        m = sg.sg_reduce(c.ctx, hc, sg.SG_RMAX)
+        u = sg.sg_enqueue(c.ctx, sg.SG_ADD, [a, m])
+        want_u = orc.scalar("add", mem[0:L].copy(), float(orc.max(y)))
+        sg.sg_enqueue(c.ctx, sg.SG_ADD, [b, sg.F(1.0)], dst_or_0=b)
+        mem[s:s + L] = orc.scalar("add", mem[s:s + L].copy(), 1.0)
+        sg.sg_flush(c.ctx)
+        if mode == "template":
+            assert sg.sg_plan_stats(c.ctx).n_passes == 3
+        got_u, got_x = c.read_vec(u, np.float64), c.read_vec(hx, np.float64)
+    assert bits_equal(got_u, want_u) and bits_equal(got_x, mem)
+
+
 @pytest.mark.parametrize("dtype,tol", [(np.float32, 1e-5), (np.float64, 1e-12), (np.int32, 0), (np.int64, 0)])
 @pytest.mark.parametrize("n", [1, 2, 33, 1024, 1025, 70001])
 def test_reductions_all_dtypes(dtype, tol, n):
