@@ -153,7 +153,12 @@ sg_status sg_mat_elem(sg_ctx* ctx, sg_handle m, int64_t i, int64_t j, sg_handle*
  * dst_or_0 != 0: the result replaces the contents of that vector/matrix (in-place variants) and
  * *out == dst_or_0; otherwise *out is a new pending collection that is materialised at flush only if the
  * caller still holds it (sg_release it first to keep an intermediate in registers, "anonymous
- * intermediate result"). */
+ * intermediate result").
+ * Handles that share storage (a collection and its subset / row / row-block / element views): the pending list behaves like eager
+ * execution in program order — an operation reads what the operations enqueued before it left in memory, whichever handle they went
+ * through (R25).  An in-place operation may read its destination only index-for-index (the same view); an operand that
+ * overlaps the destination any other way is SG_ERR_ALIAS at the flush.  A chain that exceeds what one pass holds (10 distinct
+ * inputs, 8 outputs, 32 operations) is planned as several passes; a flush holds up to 256 passes (SG_ERR_CAPACITY beyond). */
 sg_status sg_enqueue(sg_ctx* ctx, sg_op op, const sg_operand* operands, int32_t n, sg_handle dst_or_0, sg_handle* out);
 
 /* project (transform: FUNCTION[T, U]): COLLECTION[U] with the value-preserving conversion as the transform:
