@@ -214,7 +214,12 @@ def check_sum(got, w, tol, ctx):
         if not np.isfinite(ws):
             assert (np.isnan(ws) and np.isnan(got)) or ws == got, (ctx, got, ws)
         else:
-            assert rel_err(got, ws, float(np.abs(w.astype(np.float64)).sum())) <= tol, (ctx, got, ws)
+            # the bar is relative to the RESULT (north_star).  A sum that cancels almost completely (x - x patterns over planted 1e19s:
+            # condition 1e17) cannot meet it in any fixed precision: there the accumulator's resolution relative to sum|x| binds —
+            # n * 2^-53 for fp32 data (fp64 accumulators), 2^-64 for fp64 data (double-double accumulators), R1
+            sabs = float(np.abs(w.astype(np.float64)).sum())
+            floor = sabs * (w.size * 2.0 ** -53 if w.dtype == np.float32 else 2.0 ** -64)
+            assert rel_err(got, ws, sabs) <= tol or abs(got - ws) <= floor, (ctx, got, ws, sabs)
     else:
         assert got == ws, (ctx, got, ws)
 
